@@ -1,0 +1,173 @@
+"""CPU ORACLE -- test infrastructure, not the product.
+
+ctypes access to oracle/optimus_oracle.cpp (plain C++17, fp64, the unfused graph
+one op at a time).  Only tests/, __graft_entry__.smoke() and bench.py's
+cpu_baseline / --impl reference legs may import this package; the product
+package paper_2607_02945_b200 never does, and this package never imports it.
+
+`build()` compiles liboptimus_oracle.so next to the source with g++ (OpenMP for
+the timed run; OpenMP only splits independent rows, never a floating-point sum).
+"""
+import ctypes
+import os
+import subprocess
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "optimus_oracle.cpp")
+_LIB = os.path.join(_HERE, "liboptimus_oracle.so")
+_lib = None
+
+F32, BF16 = 0, 1
+_NP = {F32: np.float32, BF16: np.uint16}
+_ESZ = {F32: 4, BF16: 2}
+
+
+def build(force=False):
+    if (not force and os.path.exists(_LIB)
+            and os.path.getmtime(_LIB) >= os.path.getmtime(_SRC)):
+        return _LIB
+    cmd = ["g++", "-O2", "-std=c++17", "-fopenmp", "-shared", "-fPIC", "-fno-fast-math",
+           "-o", _LIB, _SRC]
+    subprocess.check_call(cmd)
+    return _LIB
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        build()
+        L = ctypes.CDLL(_LIB)
+        c = ctypes
+        vp, i64, i32, dbl = c.c_void_p, c.c_int64, c.c_int32, c.c_double
+        L.oracle_set_threads.argtypes = [c.c_int]
+        L.oracle_get_max_threads.restype = c.c_int
+        L.oracle_round_to_storage.argtypes = [vp, i64, c.c_int, vp]
+        L.oracle_widen.argtypes = [vp, i64, c.c_int, vp]
+        L.oracle_linear.argtypes = [vp, i64, vp, i64, vp, i32, i32, i32, c.c_int, vp]
+        L.oracle_linear_mulreduce.argtypes = [vp, i64, vp, i64, vp, i32, i32, i32, c.c_int, vp]
+        L.oracle_activation.argtypes = [vp, i64, c.c_int]
+        L.oracle_pointwise.argtypes = [vp, i64, i32, i32, c.c_int, c.c_int, vp]
+        L.oracle_layernorm.argtypes = [vp, i64, vp, vp, i32, i32, dbl, c.c_int, c.c_int, vp, vp]
+        L.oracle_split.argtypes = [vp, i64, i32, i32, i32, vp, i32, vp]
+        L.oracle_split.restype = c.c_int
+        L.oracle_cat.argtypes = [vp, vp, i32, i32, i32, vp, i64]
+        _lib = L
+    return _lib
+
+
+def _ptr(a):
+    return None if a is None else a.ctypes.data_as(ctypes.c_void_p)
+
+
+def _chk(a, dt, ndim=None):
+    assert a.dtype == _NP[dt], (a.dtype, dt)
+    assert a.strides[-1] == a.itemsize, "unit inner stride required"
+    if ndim is not None:
+        assert a.ndim == ndim
+    return a
+
+
+def _ld(a):
+    return a.strides[0] // a.itemsize if a.ndim == 2 else a.shape[-1]
+
+
+def set_threads(n):
+    lib().oracle_set_threads(int(n))
+
+
+def max_threads():
+    return int(lib().oracle_get_max_threads())
+
+
+# ------------------------------------------------------------------- ops ----
+def round_to_storage(z, dt):
+    """fp64 array -> storage dtype (fp32, or bf16 bits as uint16), direct RNE."""
+    z = np.ascontiguousarray(z, dtype=np.float64)
+    out = np.empty(z.shape, dtype=_NP[dt])
+    lib().oracle_round_to_storage(_ptr(z), z.size, dt, _ptr(out))
+    return out
+
+
+def widen(a, dt):
+    a = np.ascontiguousarray(a)
+    assert a.dtype == _NP[dt]
+    out = np.empty(a.shape, dtype=np.float64)
+    lib().oracle_widen(_ptr(a), a.size, dt, _ptr(out))
+    return out
+
+
+def linear(x, w, b, dt, mulreduce=False):
+    """Z = X W^T + b in fp64; x:[M,K], w:[N,K], b:[N] or None, storage dtype dt."""
+    _chk(x, dt, 2), _chk(w, dt, 2)
+    M, K = x.shape
+    N, K2 = w.shape
+    assert K == K2
+    if b is not None:
+        b = np.ascontiguousarray(_chk(b, dt, 1))
+        assert b.shape == (N,)
+    z = np.empty((M, N), dtype=np.float64)
+    fn = lib().oracle_linear_mulreduce if mulreduce else lib().oracle_linear
+    fn(_ptr(x), _ld(x), _ptr(w), _ld(w), _ptr(b), M, N, K, dt, _ptr(z))
+    return z
+
+
+def activation(z, act):
+    """elementwise on fp64, returns a new array; act: 0 none, 1 relu, 2 tanh, 3 sigmoid."""
+    z = np.array(z, dtype=np.float64, order="C", copy=True)
+    lib().oracle_activation(_ptr(z), z.size, int(act))
+    return z
+
+
+def pointwise(src, op, dt):
+    """f(src) in fp64 for a 2-D storage tensor with unit inner stride."""
+    _chk(src, dt, 2)
+    rows, width = src.shape
+    out = np.empty((rows, width), dtype=np.float64)
+    lib().oracle_pointwise(_ptr(src), _ld(src), rows, width, int(op), dt, _ptr(out))
+    return out
+
+
+def layernorm(x, gamma, beta, eps, dt, param_dt=None, return_xhat=False):
+    """torch layer_norm over the last dim, fp64.  eps is the fp32 value the
+    descriptor carries, widened (np.float32(eps))."""
+    param_dt = dt if param_dt is None else param_dt
+    _chk(x, dt, 2)
+    rows, D = x.shape
+    if gamma is not None:
+        gamma = np.ascontiguousarray(_chk(gamma, param_dt, 1))
+    if beta is not None:
+        beta = np.ascontiguousarray(_chk(beta, param_dt, 1))
+    y = np.empty((rows, D), dtype=np.float64)
+    xh = np.empty((rows, D), dtype=np.float64) if return_xhat else None
+    lib().oracle_layernorm(_ptr(x), _ld(x), _ptr(gamma), _ptr(beta), rows, D,
+                           float(np.float32(eps)), dt, param_dt, _ptr(y), _ptr(xh))
+    return (y, xh) if return_xhat else y
+
+
+def split(x, sizes):
+    """torch.split(x, sizes, dim=1) on raw storage elements; returns dense pieces."""
+    assert x.ndim == 2 and x.strides[1] == x.itemsize
+    rows, width = x.shape
+    sizes = [int(s) for s in sizes]
+    pieces = [np.empty((rows, s), dtype=x.dtype) for s in sizes]
+    arr = (ctypes.c_void_p * len(sizes))(*[p.ctypes.data for p in pieces])
+    sz = (ctypes.c_int32 * len(sizes))(*sizes)
+    rc = lib().oracle_split(_ptr(x), _ld(x), rows, width, x.itemsize, sz, len(sizes), arr)
+    if rc != 0:
+        raise ValueError("split sizes do not sum to the width")
+    return pieces
+
+
+def cat(pieces):
+    """torch.cat(pieces, dim=1) on raw storage elements."""
+    pieces = [np.ascontiguousarray(p) for p in pieces]
+    rows = pieces[0].shape[0]
+    assert all(p.ndim == 2 and p.shape[0] == rows and p.dtype == pieces[0].dtype for p in pieces)
+    sizes = [p.shape[1] for p in pieces]
+    out = np.empty((rows, sum(sizes)), dtype=pieces[0].dtype)
+    arr = (ctypes.c_void_p * len(sizes))(*[p.ctypes.data for p in pieces])
+    sz = (ctypes.c_int32 * len(sizes))(*sizes)
+    lib().oracle_cat(arr, sz, len(sizes), rows, out.itemsize, _ptr(out), out.shape[1])
+    return out

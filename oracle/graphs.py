@@ -1,0 +1,67 @@
+"""CPU ORACLE (test infrastructure) -- the UNFUSED graphs of BASELINE.json's
+configs, run one op at a time through oracle/optimus_oracle.cpp.
+
+Each function mirrors the graph a PyTorch user writes before Optimus rewrites
+it (PAPER.md:148 group fusion; :166 chained transformations; :403-416 Listing
+2): N independent ops, then torch.cat.  Rounding to the storage dtype happens
+once per *group* output (linear+bias+activation is one group: reading Q2), and
+between the groups of configs[4] (reading Q3).
+"""
+import numpy as np
+
+from . import (BF16, F32, activation, cat, layernorm, linear, pointwise,  # noqa: F401
+               round_to_storage, split)
+
+
+def linear_member(m, dt):
+    """fp64 result of one member: act(x W^T + b)."""
+    z = linear(m["x"], m["w"], m.get("b"), dt)
+    return activation(z, m["act"])
+
+
+def linear_group(members, dt):
+    """-> (list of fp64 outputs, list of storage-dtype outputs)."""
+    z64 = [linear_member(m, dt) for m in members]
+    return z64, [round_to_storage(z, dt) for z in z64]
+
+
+def linear_group_concat(members, dt):
+    z64, ys = linear_group(members, dt)
+    return z64, cat(ys)
+
+
+def layernorm_group(members, dt):
+    y64 = [layernorm(m["x"], m.get("gamma"), m.get("beta"), m["eps"], dt) for m in members]
+    return y64, [round_to_storage(y, dt) for y in y64]
+
+
+def split_pointwise_cat(x, widths, ops, perm, dt):
+    """split(x, widths, dim=1) -> f_j on chunk j -> cat([f_perm[0], f_perm[1], ...], dim=1).
+    perm[j] = source chunk placed at output position j (reading Q14).
+    Returns (fp64 [rows,width] in output order, storage-dtype output)."""
+    pieces = split(x, widths)
+    f64 = [pointwise(p, op, dt) for p, op in zip(pieces, ops)]
+    fst = [round_to_storage(f, dt) for f in f64]
+    out = cat([fst[p] for p in perm])
+    out64 = np.concatenate([f64[p] for p in perm], axis=1)
+    return out64, out
+
+
+def split_copy_cat(x, widths, perm):
+    """movement only: split -> cat in permuted order, raw bits."""
+    pieces = split(x, widths)
+    return cat([pieces[p] for p in perm])
+
+
+def recsys_tower(t, dt=BF16):
+    """LayerNorm -> Linear+ReLU -> Linear for one tower, intermediates
+    materialised in the storage dtype between groups (Q3).
+    Returns dict of storage-dtype stage outputs and fp64 stage outputs, where
+    stage g's fp64 output is computed from stage g-1's *rounded* output."""
+    ln64 = layernorm(t["x"], t["gamma"], t["beta"], t["eps"], dt)
+    ln = round_to_storage(ln64, dt)
+    h64 = activation(linear(ln, t["w1"], t["b1"], dt), 1)
+    h = round_to_storage(h64, dt)
+    o64 = linear(h, t["w2"], t["b2"], dt)
+    o = round_to_storage(o64, dt)
+    return dict(ln=ln, h=h, out=o, ln64=ln64, h64=h64, out64=o64)

@@ -1,0 +1,393 @@
+"""Pins for the CPU oracle (oracle/), none of which re-use the oracle's own
+formulas: the paper's worked example (tests/golden), closed forms, hand-computed
+brute-force cases, identities, library routines on special cases, exhaustive
+rounding enumeration.  SURVEY.md 8(c) P1-P12, Q5, Q13.  CPU only.
+"""
+import math
+import os
+
+import numpy as np
+import pytest
+
+import oracle
+from oracle import BF16, F32, graphs
+import workloads as wl
+
+GOLD = os.path.join(os.path.dirname(__file__), "golden")
+
+
+def bf16(a):
+    """float array exactly representable in bf16 -> bits (asserts exactness)."""
+    a = np.asarray(a, dtype=np.float32)
+    u = wl.bf16_bits_from_f32(a)
+    assert np.array_equal(wl.f32_from_bf16_bits(u), a), "test value not exact in bf16"
+    return u
+
+
+def st(a, dt):
+    return np.asarray(a, dtype=np.float32) if dt == F32 else bf16(a)
+
+
+# ------------------------------------------------------------------ P12 -----
+def _bf16_value(u):
+    """value of a finite non-negative bf16 pattern from the format definition."""
+    e, f = u >> 7, u & 0x7F
+    return math.ldexp(f, -133) if e == 0 else math.ldexp(128 + f, e - 134)
+
+
+def test_p12_bf16_rounding_exhaustive():
+    us = np.arange(0, 0x7F80, dtype=np.int64)               # all finite non-negative patterns
+    vals = np.array([_bf16_value(int(u)) for u in us], dtype=np.float64)
+    # exact values round to themselves, both signs; widen is the inverse
+    assert np.array_equal(oracle.round_to_storage(vals, BF16), us.astype(np.uint16))
+    neg = oracle.round_to_storage(-vals, BF16)
+    assert np.array_equal(neg, (us | 0x8000).astype(np.uint16))
+    assert np.array_equal(oracle.widen(us.astype(np.uint16), BF16), vals)
+    # midpoints between consecutive patterns: ties to even; one double ulp either side decides
+    lo, hi = vals[:-1], vals[1:]
+    mid = (lo + hi) / 2.0
+    assert np.all((mid > lo) & (mid < hi))
+    even = (us[:-1] % 2 == 0)
+    exp_tie = np.where(even, us[:-1], us[1:]).astype(np.uint16)
+    assert np.array_equal(oracle.round_to_storage(mid, BF16), exp_tie)
+    assert np.array_equal(oracle.round_to_storage(np.nextafter(mid, np.inf), BF16), us[1:].astype(np.uint16))
+    assert np.array_equal(oracle.round_to_storage(np.nextafter(mid, -np.inf), BF16), us[:-1].astype(np.uint16))
+    assert np.array_equal(oracle.round_to_storage(-mid, BF16), exp_tie | np.uint16(0x8000))
+    # overflow: max finite is 0x7F7F; the midpoint to 2^128 ties to even = inf
+    vmax = _bf16_value(0x7F7F)
+    top = (vmax + math.ldexp(1.0, 128)) / 2.0
+    r = oracle.round_to_storage(np.array([top, np.nextafter(top, 0.0), 1e300, -1e300, np.inf]), BF16)
+    assert list(r) == [0x7F80, 0x7F7F, 0x7F80, 0xFF80, 0x7F80]
+    # underflow: half the min subnormal ties to even (0); just above -> min subnormal
+    tiny = math.ldexp(1.0, -134)
+    r = oracle.round_to_storage(np.array([tiny, np.nextafter(tiny, 1.0), tiny / 4, 0.0, -0.0]), BF16)
+    assert list(r) == [0, 1, 0, 0, 0x8000]
+    assert oracle.round_to_storage(np.array([np.nan]), BF16)[0] & 0x7FFF > 0x7F80
+
+
+def test_p12_double_rounding_trap():
+    # 1 + 2^-8 + 2^-40 lies just above the bf16 midpoint between 1 and 1+2^-7; rounding through fp32
+    # first lands exactly on the midpoint and then ties to even (1.0): the oracle must round directly.
+    d = 1.0 + 2.0 ** -8 + 2.0 ** -40
+    assert oracle.round_to_storage(np.array([d]), BF16)[0] == 0x3F81
+    assert wl.bf16_bits_from_f32(np.array([np.float32(d)]))[0] == 0x3F80   # the via-fp32 answer differs
+
+
+def test_f32_rounding_matches_ieee_cast():
+    rng = np.random.default_rng(0)
+    z = rng.standard_normal(10000) * np.exp(rng.uniform(-30, 30, 10000))
+    assert np.array_equal(oracle.round_to_storage(z, F32), z.astype(np.float32))
+
+
+# ------------------------------------------------------------------- P1 -----
+def _read_golden():
+    d = {}
+    for line in open(os.path.join(GOLD, "listing2_split_cat.txt")):
+        line = line.strip()
+        if not line or line.startswith("#"):
+            continue
+        k, rest = line.split(None, 1)
+        if ";" in rest:
+            d[k] = np.array([[int(t) for t in row.split()] for row in rest.split(";")])
+        else:
+            d[k] = [int(t) for t in rest.split()]
+    return d
+
+
+@pytest.mark.parametrize("dt", [F32, BF16])
+def test_p1_paper_listing2_is_identity(dt):
+    g = _read_golden()
+    assert g["input_shape"] == [2, 6] and g["cat_dim"] == [1]
+    # (a) explicit integer instance, pieces written by hand in the fixture
+    x = st(g["x"], dt)
+    fs = oracle.split(x, g["first_split"])
+    assert np.array_equal(fs[0], st(g["item0"], dt)) and np.array_equal(fs[1], st(g["item1"], dt))
+    it = oracle.split(fs[1], g["second_split"])
+    assert np.array_equal(it[0], st(g["item2"], dt)) and np.array_equal(it[1], st(g["item3"], dt))
+    out = oracle.cat([fs[0]] + it)
+    assert np.array_equal(out, st(g["cat"], dt)) and np.array_equal(out, x)
+    # (b) the paper's own instance: random [2,6] input, result == input bit for bit (Listing 1)
+    ex = wl.listing2_example(dtype=dt)
+    fs = oracle.split(ex["x"], ex["first_split"])
+    out = oracle.cat([fs[0]] + oracle.split(fs[1], ex["second_split"]))
+    assert out.tobytes() == ex["x"].tobytes()
+
+
+# ------------------------------------------------------------------- P2 -----
+def test_p2_split_cat_identities_and_permutation():
+    rng = np.random.default_rng(5)
+    for trial in range(20):
+        rows, n = int(rng.integers(1, 9)), int(rng.integers(1, 12))
+        widths = [int(w) for w in rng.integers(1, 7, size=n)]
+        W = sum(widths)
+        x = rng.integers(0, 65536, size=(rows, W)).astype(np.uint16)
+        pieces = oracle.split(x, widths)
+        s = 0
+        for p, w in zip(pieces, widths):                    # split against numpy slicing (library)
+            assert np.array_equal(p, x[:, s:s + w])
+            s += w
+        assert np.array_equal(oracle.cat(pieces), x)        # split then cat = identity
+        back = oracle.split(oracle.cat(pieces), widths)     # cat then split = identity
+        assert all(np.array_equal(a, b) for a, b in zip(back, pieces))
+        perm = rng.permutation(n)
+        y = graphs.split_copy_cat(x, widths, perm)
+        assert np.array_equal(y, np.concatenate([x[:, sum(widths[:p]):sum(widths[:p + 1])] for p in perm], axis=1))
+        inv = np.argsort(perm)
+        z = graphs.split_copy_cat(y, [widths[p] for p in perm], inv)
+        assert np.array_equal(z, x)                         # permutation then inverse = identity
+    with pytest.raises(ValueError):
+        oracle.split(np.zeros((2, 6), np.uint16), [2, 3])
+    # strided (non-dense) source
+    big = rng.integers(0, 65536, size=(4, 20)).astype(np.uint16)
+    v = big[:, 3:15]
+    assert np.array_equal(oracle.cat(oracle.split(v, [5, 7])), v)
+
+
+# ------------------------------------------------------------------- P3 -----
+@pytest.mark.parametrize("dt", [F32, BF16])
+def test_p3_linear_hand_computed(dt):
+    # X:[2,2], W:[3,2] ([N,K], torch layout), b:[3].  By hand:
+    # row0: [1*1+2*0, 1*0+2*1, 1*1+2*1] + b = [1,2,3]+[10,20,30]; row1: [3,4,7]+b
+    X = st([[1, 2], [3, 4]], dt)
+    W = st([[1, 0], [0, 1], [1, 1]], dt)
+    b = st([10, 20, 30], dt)
+    Z = oracle.linear(X, W, b, dt)
+    assert np.array_equal(Z, np.array([[11, 22, 33], [13, 24, 37]], dtype=np.float64))
+    # asymmetric 2x3 . (2x3)^T : catches a transposed operand or swapped index
+    X = st([[1, 2, 3], [4, 5, 6]], dt)
+    W = st([[1, -1, 2], [0, 3, -2]], dt)
+    Z = oracle.linear(X, W, None, dt)
+    assert np.array_equal(Z, np.array([[1 - 2 + 6, 6 - 6], [4 - 5 + 12, 15 - 12]], dtype=np.float64))
+
+
+@pytest.mark.parametrize("dt", [F32, BF16])
+def test_p3_layernorm_hand_computed(dt):
+    x = st([[1, 2, 3, 4]], dt)
+    y, xh = oracle.layernorm(x, None, None, 0.0, dt, return_xhat=True)
+    # mu = 2.5, v = 1.25 : xhat = (x-2.5)/sqrt(1.25)
+    exp = np.array([-1.5, -0.5, 0.5, 1.5]) / math.sqrt(1.25)
+    assert np.allclose(y[0], exp, rtol=0, atol=1e-15) and np.array_equal(y, xh)
+    eps = float(np.float32(1e-5))
+    y = oracle.layernorm(x, st([2, 2, 2, 2], dt), st([1, 0, -1, 0.5], dt), 1e-5, dt)
+    exp = np.array([-1.5, -0.5, 0.5, 1.5]) / math.sqrt(1.25 + eps) * 2 + np.array([1, 0, -1, 0.5])
+    assert np.allclose(y[0], exp, rtol=0, atol=1e-15)
+    # constant row -> beta exactly; D = 1 -> beta
+    beta = st([0.5, -0.25, 2, 1], dt)
+    y = oracle.layernorm(st([[3, 3, 3, 3]], dt), st([1, 2, 3, 4], dt), beta, 1e-5, dt)
+    assert np.array_equal(y[0], np.array([0.5, -0.25, 2, 1]))
+    y = oracle.layernorm(st([[7], [-2]], dt), st([3], dt), st([0.75], dt), 1e-5, dt)
+    assert np.array_equal(y, np.array([[0.75], [0.75]]))
+
+
+# ------------------------------------------------------------ P4, P5, P6 ----
+def _rand_linear(rng, M, N, K, dt):
+    x = wl.tensor_normal(int(rng.integers(1 << 30)), 1, (M, K), 0, 1, dt)
+    w = wl.tensor_normal(int(rng.integers(1 << 30)), 2, (N, K), 0, K ** -0.5, dt)
+    b = wl.tensor_normal(int(rng.integers(1 << 30)), 3, (N,), 0, 0.1, dt)
+    return x, w, b
+
+
+@pytest.mark.parametrize("dt", [F32, BF16])
+def test_p4_zero_padding_invariance(dt):
+    """pad_aten_mm_pass: pad -> mm -> slice leaves the result unchanged."""
+    rng = np.random.default_rng(11)
+    M, N, K = 5, 13, 11
+    x, w, b = _rand_linear(rng, M, N, K, dt)
+    z = oracle.linear(x, w, b, dt)
+    xp = np.zeros((M, 16), x.dtype); xp[:, :K] = x
+    wp = np.zeros((16, 16), w.dtype); wp[:N, :K] = w
+    bp = np.zeros((16,), b.dtype); bp[:N] = b
+    zp = oracle.linear(xp, wp, bp, dt)
+    assert np.array_equal(zp[:, :N], z)
+    assert np.array_equal(zp[:, N:], np.zeros((M, 3)))
+
+
+@pytest.mark.parametrize("dt", [F32, BF16])
+def test_p5_linear_equals_mul_then_reduce_and_library(dt):
+    """decompose_mm_pass: mm == pointwise mul + reduce over K; and == the library matmul."""
+    rng = np.random.default_rng(12)
+    for (M, N, K) in [(7, 9, 33), (3, 64, 128), (16, 5, 1)]:
+        x, w, b = _rand_linear(rng, M, N, K, dt)
+        z = oracle.linear(x, w, b, dt)
+        z2 = oracle.linear(x, w, b, dt, mulreduce=True)
+        xd, wd, bd = (wl.f32_from_bf16_bits(a).astype(np.float64) if dt == BF16 else a.astype(np.float64)
+                      for a in (x, w, b))
+        z3 = xd @ wd.T + bd                                   # library routine
+        scale = np.abs(xd) @ np.abs(wd).T + np.abs(bd)
+        assert np.all(np.abs(z - z2) <= 1e-13 * scale)
+        assert np.all(np.abs(z - z3) <= 1e-13 * scale)
+        # strided x (ldx > K)
+        xb = np.zeros((M, K + 5), x.dtype); xb[:, :K] = x
+        assert np.array_equal(oracle.linear(xb[:, :K], w, b, dt), z)
+
+
+def test_p6_equal_shape_group_equals_batched_matmul():
+    """batch fusion: stack -> one batched multiply -> unbind (Fig. 4)."""
+    rng = np.random.default_rng(13)
+    n, M, N, K = 5, 6, 8, 16
+    members = []
+    for i in range(n):
+        x, w, b = _rand_linear(rng, M, N, K, BF16)
+        members.append(dict(x=x, w=w, b=b, act=0))
+    z64, ys = graphs.linear_group(members, BF16)
+    X = np.stack([wl.f32_from_bf16_bits(m["x"]).astype(np.float64) for m in members])
+    W = np.stack([wl.f32_from_bf16_bits(m["w"]).astype(np.float64) for m in members])
+    B = np.stack([wl.f32_from_bf16_bits(m["b"]).astype(np.float64) for m in members])
+    Z = np.matmul(X, W.transpose(0, 2, 1)) + B[:, None, :]
+    for i in range(n):
+        assert np.allclose(z64[i], Z[i], rtol=1e-13, atol=1e-13)
+    # the concat slotting: member i occupies columns [i*N, (i+1)*N)
+    _, ycat = graphs.linear_group_concat(members, BF16)
+    for i in range(n):
+        assert np.array_equal(ycat[:, i * N:(i + 1) * N], ys[i])
+
+
+# ------------------------------------------------------------------- P7 -----
+def test_p7_layernorm_closed_forms():
+    cfg = wl.config1(seed=1, rows=32, n=8)
+    for m in cfg["members"]:
+        x = m["x"]
+        eps = float(np.float32(m["eps"]))
+        y, xh = oracle.layernorm(x, m["gamma"], m["beta"], m["eps"], BF16, return_xhat=True)
+        xd = wl.f32_from_bf16_bits(x).astype(np.float64)
+        v = xd.var(axis=1)                                     # biased variance (library)
+        assert np.all(np.abs(xh.mean(axis=1)) <= 1e-6)         # north_star invariant: mean 0
+        assert np.all(np.abs(xh.var(axis=1) - v / (v + eps)) <= 1e-6)      # Q5 closed form
+        _, xh0 = oracle.layernorm(x, None, None, 0.0, BF16, return_xhat=True)
+        assert np.all(np.abs(xh0.var(axis=1) - 1.0) <= 1e-6)   # north_star invariant, literally, at eps=0
+        assert np.all(np.abs(xh0.mean(axis=1)) <= 1e-6)
+        # affine: y = xhat*gamma + beta
+        g = wl.f32_from_bf16_bits(m["gamma"]).astype(np.float64)
+        b = wl.f32_from_bf16_bits(m["beta"]).astype(np.float64)
+        assert np.allclose(y, xh * g + b, rtol=0, atol=1e-14)
+        # against the textbook formula through numpy
+        ref = (xd - xd.mean(axis=1, keepdims=True)) / np.sqrt(v + eps)[:, None] * g + b
+        assert np.allclose(y, ref, rtol=1e-12, atol=1e-12)
+
+
+def test_p7_layernorm_shift_and_scale_invariance():
+    rng = np.random.default_rng(3)
+    x = rng.integers(-20, 20, size=(6, 24)).astype(np.float32)     # exact in fp32 after shift/scale
+    y = oracle.layernorm(x, None, None, 1e-5, F32)
+    y_shift = oracle.layernorm(x + np.float32(64.0), None, None, 1e-5, F32)
+    assert np.allclose(y, y_shift, rtol=0, atol=1e-12)             # LN(x+c) = LN(x)
+    eps = float(np.float32(1e-5))
+    a = 4.0
+    y_scale = oracle.layernorm(x * np.float32(a), None, None, np.float32(a * a * eps), F32)
+    assert np.allclose(y, y_scale, rtol=0, atol=1e-9)               # LN_{a^2 eps}(a x) = LN_eps(x)
+    # a wrong sign of the normalisation or un-biased variance would fail:
+    xd = x.astype(np.float64)
+    unbiased = (xd - xd.mean(1, keepdims=True)) / np.sqrt(xd.var(1, ddof=1) + eps)[:, None]
+    assert not np.allclose(y, unbiased, rtol=0, atol=1e-4)
+
+
+# ------------------------------------------------------------- P8, Q13 ------
+def test_p8_pointwise_identities_and_values():
+    xs = np.linspace(-12, 12, 4801)
+    t = oracle.activation(xs, 2)
+    s = oracle.activation(xs, 3)
+    r = oracle.activation(xs, 1)
+    assert np.allclose(oracle.activation(-xs, 2), -t, rtol=0, atol=0)           # odd
+    assert np.allclose(s + oracle.activation(-xs, 3), 1.0, rtol=0, atol=4e-16)
+    assert np.allclose(t, 2 * oracle.activation(2 * xs, 3) - 1, rtol=0, atol=1e-15)
+    assert np.array_equal(oracle.activation(r, 1), r) and np.array_equal(r, np.maximum(xs, 0))
+    assert np.array_equal(oracle.activation(xs, 0), xs)
+    # textbook values
+    v = oracle.activation(np.array([0.0, 1.0, -1.0, 0.5]), 2)
+    assert v[0] == 0.0 and abs(v[1] - 0.7615941559557649) < 1e-15 and abs(v[3] - 0.46211715726000974) < 1e-15
+    v = oracle.activation(np.array([0.0, 1.0, -1.0, 40.0, -40.0]), 3)
+    assert v[0] == 0.5 and abs(v[1] - 0.7310585786300049) < 1e-15 and abs(v[2] - 0.2689414213699951) < 1e-15
+    assert abs(v[4] - math.exp(-40.0)) < 1e-30 and v[3] == 1.0
+    # against the C library through python's math module
+    for x in (-3.3, -0.1, 1e-9, 0.7, 5.0):
+        assert abs(oracle.activation(np.array([x]), 2)[0] - math.tanh(x)) <= 2e-16
+        assert abs(oracle.activation(np.array([x]), 3)[0] - 1 / (1 + math.exp(-x))) <= 2e-16
+
+
+def test_q13_special_values():
+    sp = np.array([np.nan, np.inf, -np.inf, -0.0, 0.0])
+    r = oracle.activation(sp, 1)
+    assert np.isnan(r[0]) and r[1] == np.inf and r[2] == 0 and r[3] == 0 and r[4] == 0
+    t = oracle.activation(sp, 2)
+    assert np.isnan(t[0]) and t[1] == 1 and t[2] == -1 and t[3] == 0 and np.signbit(t[3])
+    s = oracle.activation(sp, 3)
+    assert np.isnan(s[0]) and s[1] == 1 and s[2] == 0 and s[3] == 0.5
+    # pointwise on storage applies the same function to the widened value
+    x = bf16([[-2.0, -0.5, 0.0, 0.5, 3.0]])
+    for op in (0, 1, 2, 3):
+        assert np.array_equal(oracle.pointwise(x, op, BF16)[0],
+                              oracle.activation(np.array([-2.0, -0.5, 0.0, 0.5, 3.0]), op))
+
+
+# ------------------------------------------------------------- P9, P11 ------
+def test_p9_small_integer_case_is_exact():
+    rng = np.random.default_rng(9)
+    for (M, N, K, lim) in [(8, 16, 16, 3), (4, 8, 256, 1)]:
+        X = rng.integers(-lim, lim + 1, size=(M, K))
+        W = rng.integers(-lim, lim + 1, size=(N, K))
+        b = rng.integers(-lim, lim + 1, size=(N,))
+        Z = X @ W.T + b                                       # exact integer arithmetic
+        assert np.abs(Z).max() < 256
+        for dt in (F32, BF16):
+            z = oracle.linear(st(X, dt), st(W, dt), st(b, dt), dt)
+            assert np.array_equal(z, Z.astype(np.float64))
+            y = oracle.round_to_storage(oracle.activation(z, 1), dt)
+            assert np.array_equal(y, st(np.maximum(Z, 0), dt))
+
+
+def test_p11_linearity_in_x_with_power_of_two():
+    rng = np.random.default_rng(10)
+    x, w, b = _rand_linear(rng, 6, 10, 24, F32)
+    z = oracle.linear(x, w, b, F32)
+    bd = b.astype(np.float64)
+    for alpha in (2.0, 0.25, -8.0):
+        za = oracle.linear(x * np.float32(alpha), w, b, F32)
+        assert np.array_equal(za, alpha * (z - bd) + bd) or np.allclose(za, alpha * (z - bd) + bd, rtol=1e-15, atol=1e-15)
+    # dropping the bias term would fail this:
+    z0 = oracle.linear(x, w, None, F32)
+    assert np.allclose(z - z0, np.broadcast_to(bd, z.shape), rtol=0, atol=1e-15)
+
+
+# ------------------------------------------------- config graphs (Q2, Q14) --
+def test_config0_graph_separate_equals_concat_slots():
+    cfg = wl.config0()
+    z64, ys = graphs.linear_group(cfg["members"], F32)
+    _, ycat = graphs.linear_group_concat(cfg["members"], F32)
+    assert ycat.shape == (64, 160)
+    off = 0
+    for m, y in zip(cfg["members"], ys):
+        assert y.shape == (64, m["N"]) and np.array_equal(ycat[:, off:off + m["N"]], y)
+        off += m["N"]
+    assert all(np.all(np.abs(z) < 1) for z in z64)            # tanh range
+
+
+def test_config3_graph_permutation_direction():
+    cfg = wl.config3(seed=3, rows=4, width=256, nchunks=8)
+    out64, out = graphs.split_pointwise_cat(cfg["x"], cfg["widths"], cfg["ops"], cfg["perm"], BF16)
+    xd = wl.f32_from_bf16_bits(cfg["x"]).astype(np.float64)
+    starts = np.concatenate(([0], np.cumsum(cfg["widths"])))
+    d = 0
+    for j, p in enumerate(cfg["perm"]):                       # output position j holds SOURCE chunk perm[j]
+        w = cfg["widths"][p]
+        src = xd[:, starts[p]:starts[p] + w]
+        assert np.array_equal(out64[:, d:d + w], oracle.activation(src, cfg["ops"][p]))
+        d += w
+    assert d == 256 and out.shape == (4, 256)
+    assert sum(cfg["widths"]) == 256 and all(w % 8 == 0 and w > 0 for w in cfg["widths"])
+    assert sorted(cfg["perm"]) == list(range(8))
+
+
+def test_workload_draws_are_reproducible_and_shaped():
+    a, b = wl.config2(seed=2, M=8, n=16), wl.config2(seed=2, M=8, n=16)
+    assert all(np.array_equal(p["x"], q["x"]) and p["K"] == q["K"] for p, q in zip(a["members"], b["members"]))
+    assert {m["K"] for m in a["members"]} <= {128, 256, 512, 1024}
+    c = wl.config2(seed=102, M=8, n=16)
+    assert [m["K"] for m in c["members"]] != [m["K"] for m in a["members"]]
+    c1 = wl.config1(seed=1, rows=4096, n=4)
+    for m in c1["members"]:
+        xd = wl.f32_from_bf16_bits(m["x"]).astype(np.float64)
+        assert abs(xd.mean() - m["mu"]) < 0.1 * m["sigma"] and abs(xd.std() - m["sigma"]) < 0.05 * m["sigma"]
+    c3 = wl.config3()
+    assert len(c3["widths"]) == 256 and sum(c3["widths"]) == 8192 and c3["x"].shape == (8192, 8192)
+    xd = wl.f32_from_bf16_bits(c3["x"][:64]).astype(np.float64)
+    assert abs(xd.var() - 2.0) < 0.05
