@@ -1,0 +1,175 @@
+/* optimus_b200.h -- C ABI of liboptimus_b200 (sm_100a / NVIDIA B200).
+ *
+ * The runtime hot path that Optimus' horizontal ("group fusion") and split/cat
+ * rewrites produce (arxiv/paper_2607_02945): a matched group of N independent
+ * same-type operators is replaced by ONE semantically equivalent operator
+ * (section 3.2 "each color-coded group is fused into a single
+ * composite node"; "group fusion allows multiple no-data
+ * dependency instances to be executed within a single kernel launch without
+ * altering the individual input tensor layouts, though it requires customized
+ * kernels").  This library is those customised kernels: one kernel launch per
+ * group, described by an array of per-member descriptors.
+ *
+ * General conventions
+ *   - Plain C.  No exception crosses the ABI; every call returns opt_status and
+ *     records a message readable through opt_last_error() (thread-local).
+ *   - All tensor pointers in descriptors are DEVICE pointers owned by the caller.
+ *     The descriptor array itself is HOST memory, copied during plan_create and
+ *     free to release afterwards.  A plan owns only its device-side tables; the
+ *     tensor pointers baked into it must stay valid until opt_plan_destroy.
+ *   - Layout: every tensor is 2-D row-major with unit column stride; `ld*` is
+ *     the row stride in ELEMENTS.  A column slice of a wider buffer (a concat
+ *     slot, a split chunk) is expressed as base + column offset with ld = width
+ *     of the wider buffer -- "without altering the individual input tensor
+ *     layouts".
+ *   - Member order is output order ("preserving their original order of
+ *     execution").
+ *   - Independence precondition ("Nodes are considered independent if no data
+ *     dependency exists between them"): no member's output may
+ *     overlap any input or any other output of the group; violations that the
+ *     host can see from the address ranges return OPT_ERR_ALIAS.  Inputs may
+ *     alias each other (batch_linear_lhs).  A pointwise chunk
+ *     with dst == src && ldd == lds (in place) is allowed.
+ *   - Unsupported or misaligned groups launch NOTHING and return an error: the
+ *     "guaranteed no-op fallback" of PAPER.md:183.  There is no CPU fallback.
+ *   - Alignment (8 elements for bf16): bf16 paths need 16-byte
+ *     aligned base pointers, ld* % 8 == 0, K % 8 == 0, N % 8 == 0, D % 8 == 0,
+ *     width % 8 == 0.  fp32 paths need 16-byte aligned bases and multiples of 4.
+ *   - 1 <= n <= 65535 members, every dimension >= 1 (members with rows == 0 are
+ *     rejected as OPT_ERR_INVALID_ARG).
+ *   - opt_plan_launch is asynchronous on the given stream: exactly one kernel
+ *     launch, no allocation, no synchronisation, no memcpy.  Results are
+ *     bitwise reproducible run to run (no atomics on outputs, no split-K).
+ */
+#ifndef OPTIMUS_B200_H_
+#define OPTIMUS_B200_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+  OPT_OK = 0,
+  OPT_ERR_INVALID_ARG = 1, /* NULL pointer, n out of range, non-positive dimension, bad enum   */
+  OPT_ERR_UNSUPPORTED = 2, /* valid but outside what the kernels cover (e.g. D too large)      */
+  OPT_ERR_ALIGNMENT = 3,   /* pointer / stride / extent alignment rule violated                */
+  OPT_ERR_ALIAS = 4,       /* an output overlaps an input or another output of the group       */
+  OPT_ERR_CUDA = 5,        /* a CUDA runtime/driver call failed; message has the CUDA error    */
+  OPT_ERR_NO_DEVICE = 6    /* no CUDA device, or the device is not sm_100                      */
+} opt_status;
+
+typedef enum { OPT_F32 = 0, OPT_BF16 = 1 } opt_dtype;
+typedef enum { OPT_ACT_NONE = 0, OPT_ACT_RELU = 1, OPT_ACT_TANH = 2, OPT_ACT_SIGMOID = 3 } opt_act;
+typedef enum { OPT_PW_COPY = 0, OPT_PW_RELU = 1, OPT_PW_TANH = 2, OPT_PW_SIGMOID = 3 } opt_pw_op;
+
+/* One member of a grouped Linear (+bias +activation) -- batch_linear /
+ * batch_linear_post_grad with its epilogue:
+ *     Y = act(X * W^T + bias)
+ * X:[M,K] (ldx), W:[N,K] (ldw; torch nn.Linear layout, K-major), bias:[N] or
+ * NULL, Y:[M,N] (ldy).  For a concatenated output give y = concat_base +
+ * column_offset and ldy = total concat width.  bf16: inputs and output bf16,
+ * products accumulated in fp32 on the tensor cores, bias and activation in
+ * fp32, one round-to-nearest-even to bf16.  fp32: plain fp32 FMA (no TF32).  */
+typedef struct {
+  const void* x;
+  int64_t ldx;
+  const void* w;
+  int64_t ldw;
+  const void* bias;
+  void* y;
+  int64_t ldy;
+  int32_t M, N, K;
+  int32_t act; /* opt_act */
+} opt_linear_member;
+
+/* One member of a batched LayerNorm -- batch_layernorm:
+ *     mu = mean(x_r), v = mean((x_r - mu)^2)  (biased), over the last dim D
+ *     y_r = (x_r - mu) / sqrt(v + eps) * gamma + beta
+ * x:[rows,D] (ldx), y:[rows,D] (ldy), gamma/beta:[D] or NULL (NULL = 1 / 0).
+ * Statistics and affine in fp32 (two-pass over registers), one rounding.     */
+typedef struct {
+  const void* x;
+  int64_t ldx;
+  void* y;
+  int64_t ldy;
+  const void* gamma;
+  const void* beta;
+  int32_t rows, D;
+  float eps;
+} opt_layernorm_member;
+
+/* One chunk of a multi-tensor pointwise / split-cat pass -- batch_relu,
+ * batch_sigmoid, batch_aten_tanh, batch_detach and the data
+ * movement left over by the split/cat rewrites (Listing 2):
+ *     dst[r, 0:width] = op(src[r, 0:width])   for r < rows
+ * A split->f->cat chain is a list of chunks whose src/dst are column slices of
+ * shared bases.  OPT_PW_COPY moves raw bits.                                 */
+typedef struct {
+  const void* src;
+  int64_t lds;
+  void* dst;
+  int64_t ldd;
+  int32_t rows, width;
+  int32_t op; /* opt_pw_op */
+} opt_chunk;
+
+/* One staged host<->device copy of opt_plan_launch_host. */
+typedef struct {
+  void* host;   /* host buffer (pinned for true asynchrony)                   */
+  void* device; /* device buffer                                              */
+  size_t bytes;
+  int32_t to_device; /* 1: host->device before the kernel; 0: device->host after it */
+} opt_host_copy;
+
+typedef struct opt_plan opt_plan; /* opaque; owns device-side tables only */
+
+/* Build a plan for a group.  members: host array of n descriptors.  io: dtype
+ * of activations (and of weights/bias for linear).  param: dtype of gamma/beta.
+ * device: CUDA device ordinal.  On success *plan is set; on failure *plan is
+ * NULL and nothing is launched or left allocated.  Host argument validation
+ * happens before the first CUDA call, so INVALID_ARG / ALIGNMENT / ALIAS /
+ * UNSUPPORTED are reported even on a machine without a GPU.                  */
+opt_status opt_linear_plan_create(const opt_linear_member* members, int32_t n, opt_dtype io,
+                                  int device, opt_plan** plan);
+opt_status opt_layernorm_plan_create(const opt_layernorm_member* members, int32_t n, opt_dtype io,
+                                     opt_dtype param, int device, opt_plan** plan);
+opt_status opt_pointwise_plan_create(const opt_chunk* chunks, int32_t n, opt_dtype io, int device,
+                                     opt_plan** plan);
+
+/* Enqueue the group on `cuda_stream` (a cudaStream_t; NULL = default stream):
+ * exactly ONE kernel launch.  Asynchronous CUDA faults surface at the caller's
+ * next synchronisation.                                                      */
+opt_status opt_plan_launch(const opt_plan* plan, void* cuda_stream);
+
+/* Same, for HOST buffers: on `cuda_stream`, first every copy with to_device=1
+ * (cudaMemcpyAsync host->device), then the one kernel launch, then every copy
+ * with to_device=0 (device->host).  No synchronisation; the caller syncs the
+ * stream before reading the host outputs.                                    */
+opt_status opt_plan_launch_host(const opt_plan* plan, const opt_host_copy* copies, int32_t ncopies,
+                                void* cuda_stream);
+
+/* Algorithmic work of one launch: flops (2*M*N*K summed; 0 for non-GEMM),
+ * bytes (every input read once + every output written once, tables ignored),
+ * launches (always 1) and the number of work tiles/blocks the kernel walks.
+ * Any out pointer may be NULL.                                               */
+opt_status opt_plan_info(const opt_plan* plan, int64_t* flops, int64_t* bytes, int32_t* launches,
+                         int32_t* tiles);
+
+opt_status opt_plan_destroy(opt_plan* plan);
+
+/* Last error message of the calling thread; never NULL ("" if none). */
+const char* opt_last_error(void);
+
+/* Process-wide count of kernel launches issued by this library. */
+uint64_t opt_launch_count(void);
+
+/* Library version string, e.g. "liboptimus_b200 0.1 (sm_100a)". */
+const char* opt_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* OPTIMUS_B200_H_ */

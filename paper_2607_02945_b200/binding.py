@@ -1,0 +1,216 @@
+"""ctypes binding: same names as the C ABI, argument marshalling only."""
+import ctypes as C
+import os
+
+from . import build as _build
+
+OPT_F32, OPT_BF16 = 0, 1
+OPT_ACT_NONE, OPT_ACT_RELU, OPT_ACT_TANH, OPT_ACT_SIGMOID = 0, 1, 2, 3
+OPT_PW_COPY, OPT_PW_RELU, OPT_PW_TANH, OPT_PW_SIGMOID = 0, 1, 2, 3
+(OPT_OK, OPT_ERR_INVALID_ARG, OPT_ERR_UNSUPPORTED, OPT_ERR_ALIGNMENT, OPT_ERR_ALIAS, OPT_ERR_CUDA,
+ OPT_ERR_NO_DEVICE) = range(7)
+_STATUS_NAMES = ["OPT_OK", "OPT_ERR_INVALID_ARG", "OPT_ERR_UNSUPPORTED", "OPT_ERR_ALIGNMENT", "OPT_ERR_ALIAS",
+                 "OPT_ERR_CUDA", "OPT_ERR_NO_DEVICE"]
+
+
+class opt_linear_member(C.Structure):
+    _fields_ = [("x", C.c_void_p), ("ldx", C.c_int64), ("w", C.c_void_p), ("ldw", C.c_int64),
+                ("bias", C.c_void_p), ("y", C.c_void_p), ("ldy", C.c_int64),
+                ("M", C.c_int32), ("N", C.c_int32), ("K", C.c_int32), ("act", C.c_int32)]
+
+
+class opt_layernorm_member(C.Structure):
+    _fields_ = [("x", C.c_void_p), ("ldx", C.c_int64), ("y", C.c_void_p), ("ldy", C.c_int64),
+                ("gamma", C.c_void_p), ("beta", C.c_void_p),
+                ("rows", C.c_int32), ("D", C.c_int32), ("eps", C.c_float)]
+
+
+class opt_chunk(C.Structure):
+    _fields_ = [("src", C.c_void_p), ("lds", C.c_int64), ("dst", C.c_void_p), ("ldd", C.c_int64),
+                ("rows", C.c_int32), ("width", C.c_int32), ("op", C.c_int32)]
+
+
+class opt_host_copy(C.Structure):
+    _fields_ = [("host", C.c_void_p), ("device", C.c_void_p), ("bytes", C.c_size_t), ("to_device", C.c_int32)]
+
+
+class OptError(RuntimeError):
+    def __init__(self, status, message):
+        super().__init__("%s: %s" % (_STATUS_NAMES[status] if 0 <= status < 7 else status, message))
+        self.status = status
+        self.message = message
+
+
+_lib = None
+
+
+def lib_path():
+    return _build.LIB
+
+
+def lib():
+    """Load (building if needed) liboptimus_b200.so.  Raises if it cannot be had: no fallback."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(_build.LIB) or not _build.up_to_date():
+            try:
+                _build.build()
+            except Exception as e:  # noqa: BLE001
+                if not os.path.exists(_build.LIB):
+                    raise ImportError("liboptimus_b200.so is missing and could not be built with nvcc: %r" % (e,))
+        L = C.CDLL(_build.LIB)
+        pp = C.POINTER(C.c_void_p)
+        L.opt_linear_plan_create.argtypes = [C.POINTER(opt_linear_member), C.c_int32, C.c_int, C.c_int, pp]
+        L.opt_layernorm_plan_create.argtypes = [C.POINTER(opt_layernorm_member), C.c_int32, C.c_int, C.c_int,
+                                                C.c_int, pp]
+        L.opt_pointwise_plan_create.argtypes = [C.POINTER(opt_chunk), C.c_int32, C.c_int, C.c_int, pp]
+        L.opt_plan_launch.argtypes = [C.c_void_p, C.c_void_p]
+        L.opt_plan_launch_host.argtypes = [C.c_void_p, C.POINTER(opt_host_copy), C.c_int32, C.c_void_p]
+        L.opt_plan_info.argtypes = [C.c_void_p, C.POINTER(C.c_int64), C.POINTER(C.c_int64), C.POINTER(C.c_int32),
+                                    C.POINTER(C.c_int32)]
+        L.opt_plan_destroy.argtypes = [C.c_void_p]
+        L.opt_last_error.restype = C.c_char_p
+        L.opt_launch_count.restype = C.c_uint64
+        L.opt_version.restype = C.c_char_p
+        for f in (L.opt_linear_plan_create, L.opt_layernorm_plan_create, L.opt_pointwise_plan_create,
+                  L.opt_plan_launch, L.opt_plan_launch_host, L.opt_plan_info, L.opt_plan_destroy):
+            f.restype = C.c_int
+        _lib = L
+    return _lib
+
+
+def opt_last_error():
+    return lib().opt_last_error().decode()
+
+
+def opt_launch_count():
+    return int(lib().opt_launch_count())
+
+
+def opt_version():
+    return lib().opt_version().decode()
+
+
+def _check(st):
+    if st != OPT_OK:
+        raise OptError(st, opt_last_error())
+
+
+def _array(ctype, items):
+    items = list(items)
+    return (ctype * max(len(items), 1))(*items), len(items)
+
+
+class Plan:
+    """Opaque opt_plan handle.  launch() = opt_plan_launch: exactly one kernel launch."""
+
+    def __init__(self, handle):
+        self._h = handle
+
+    def launch(self, stream=None):
+        opt_plan_launch(self, stream)
+
+    def launch_host(self, copies, stream=None):
+        opt_plan_launch_host(self, copies, stream)
+
+    def info(self):
+        return opt_plan_info(self)
+
+    def destroy(self):
+        opt_plan_destroy(self)
+
+    def __del__(self):
+        try:
+            self.destroy()
+        except Exception:  # noqa: BLE001
+            pass
+
+
+def _create(fn, ctype, members, *dtype_and_device):
+    arr, n = _array(ctype, members)
+    h = C.c_void_p()
+    _check(fn(arr, n, *dtype_and_device, C.byref(h)))
+    return Plan(h)
+
+
+def opt_linear_plan_create(members, io, device=0):
+    return _create(lib().opt_linear_plan_create, opt_linear_member, members, io, device)
+
+
+def opt_layernorm_plan_create(members, io, param=None, device=0):
+    return _create(lib().opt_layernorm_plan_create, opt_layernorm_member, members, io,
+                   io if param is None else param, device)
+
+
+def opt_pointwise_plan_create(chunks, io, device=0):
+    return _create(lib().opt_pointwise_plan_create, opt_chunk, chunks, io, device)
+
+
+def _stream_ptr(stream):
+    if stream is None:
+        import torch
+        stream = torch.cuda.current_stream().cuda_stream
+    return C.c_void_p(int(stream))
+
+
+def opt_plan_launch(plan, stream=None):
+    _check(lib().opt_plan_launch(plan._h, _stream_ptr(stream)))
+
+
+def opt_plan_launch_host(plan, copies, stream=None):
+    arr, n = _array(opt_host_copy, copies)
+    _check(lib().opt_plan_launch_host(plan._h, arr, n, _stream_ptr(stream)))
+
+
+def opt_plan_info(plan):
+    fl, by, la, ti = C.c_int64(), C.c_int64(), C.c_int32(), C.c_int32()
+    _check(lib().opt_plan_info(plan._h, C.byref(fl), C.byref(by), C.byref(la), C.byref(ti)))
+    return dict(flops=fl.value, bytes=by.value, launches=la.value, tiles=ti.value)
+
+
+def opt_plan_destroy(plan):
+    if plan._h is not None and plan._h.value:
+        lib().opt_plan_destroy(plan._h)
+    plan._h = None
+
+
+# ---- descriptor helpers: read data_ptr / strides off torch tensors (marshalling only) ----
+def _ld(t):
+    assert t.dim() == 2 and t.stride(1) == 1, "2-D tensor with unit column stride required"
+    return t.stride(0)
+
+
+def linear_member(x, w, bias, y, act=OPT_ACT_NONE):
+    M, K = x.shape
+    N = w.shape[0]
+    assert w.shape[1] == K and tuple(y.shape) == (M, N)
+    return opt_linear_member(x.data_ptr(), _ld(x), w.data_ptr(), _ld(w),
+                             None if bias is None else bias.data_ptr(), y.data_ptr(), _ld(y), M, N, K, int(act))
+
+
+def layernorm_member(x, y, gamma, beta, eps):
+    rows, D = x.shape
+    assert tuple(y.shape) == (rows, D)
+    return opt_layernorm_member(x.data_ptr(), _ld(x), y.data_ptr(), _ld(y),
+                                None if gamma is None else gamma.data_ptr(),
+                                None if beta is None else beta.data_ptr(), rows, D, float(eps))
+
+
+def chunk(src, dst, op=OPT_PW_COPY):
+    rows, width = src.shape
+    assert tuple(dst.shape) == (rows, width)
+    return opt_chunk(src.data_ptr(), _ld(src), dst.data_ptr(), _ld(dst), rows, width, int(op))
+
+
+def split_cat_chunks(x, out, widths, ops, perm):
+    """Chunk list of split(x, widths, dim=1) -> ops[j] on chunk j -> cat in order perm
+    (perm[j] = source chunk at output position j)."""
+    starts = [0]
+    for w in widths:
+        starts.append(starts[-1] + w)
+    chunks, d = [], 0
+    for p in perm:
+        w = widths[p]
+        chunks.append(chunk(x[:, starts[p]:starts[p] + w], out[:, d:d + w], ops[p]))
+        d += w
+    return chunks

@@ -1,0 +1,531 @@
+// Grouped Linear (+bias +activation): N independent  Y_i = act_i(X_i W_i^T + b_i)
+// in ONE launch -- batch_linear / batch_linear_post_grad with the epilogue
+// fused (PAPER.md:292, :148 group fusion; include/optimus_b200.h).
+//
+// Two kernels:
+//   grouped_gemm_sm100_kernel  bf16 in/out, fp32 accumulate.  Persistent, one CTA
+//       per SM, warp-specialised:
+//         warp 0      TMA producer: cp.async.bulk.tensor 2-D loads of a 128x64 X
+//                     tile and a BNx64 W tile (128-byte swizzle) into a 4-stage
+//                     shared-memory ring guarded by full/empty mbarriers;
+//         warp 1      TMEM allocator + MMA issuer: one elected lane issues
+//                     tcgen05.mma.cta_group::1.kind::f16 (M=128, N=BN, K=16) four
+//                     times per stage into a TMEM accumulator, tcgen05.commit
+//                     releases the stage / publishes the accumulator;
+//         warps 2..5  epilogue: tcgen05.ld (32 lanes x 32 columns), + bias,
+//                     activation, RNE to bf16, swizzled st.shared, TMA store
+//                     (cp.async.bulk.tensor, 64x32 boxes) into the member's output
+//                     or its slot of the concatenated output.
+//       TMEM holds two accumulator stages (2 x 256 columns) so the epilogue of
+//       tile t overlaps the MMAs of tile t+1.  The device-side tile scheduler
+//       decodes a linear tile id into (member, m-block, n-block) from the
+//       per-member tile-count prefix sums; tiles of one X row-panel are adjacent
+//       so its re-reads hit L2.
+//   grouped_gemm_f32_kernel    plain fp32 FFMA (no TF32) 64x64 tiles for fp32
+//       groups (configs[0]); same tile scheduler, accurate tanhf/expf epilogue.
+#include <cuda.h>   // CUtensorMap types only; the encoder is fetched through the runtime
+
+#include <algorithm>
+
+#include "common.h"
+
+namespace optb {
+
+// =========================================================== fp32 SIMT path ==
+struct F32Member {
+  const float* x; const float* w; const float* bias; float* y;
+  int64_t ldx, ldw, ldy;
+  int32_t M, N, K, act;
+  int32_t nbn;        // n-blocks per m-block
+  int32_t pad;
+};
+
+constexpr int kF32Tile = 64, kF32BK = 16, kF32Threads = 256;
+
+__device__ __forceinline__ int find_member(const int32_t* __restrict__ starts, int n, int tile) {
+  int lo = 0, hi = n;   // starts[lo] <= tile < starts[hi]
+  while (hi - lo > 1) {
+    const int mid = (lo + hi) >> 1;
+    if (__ldg(starts + mid) <= tile) lo = mid; else hi = mid;
+  }
+  return lo;
+}
+
+__global__ void __launch_bounds__(kF32Threads)
+grouped_gemm_f32_kernel(const F32Member* __restrict__ members, const int32_t* __restrict__ starts, int n_members) {
+  __shared__ float As[kF32BK][kF32Tile + 4];
+  __shared__ float Bs[kF32BK][kF32Tile + 4];
+  const int tile = blockIdx.x;
+  const int mi = find_member(starts, n_members, tile);
+  const F32Member m = members[mi];
+  const int local = tile - __ldg(starts + mi);
+  const int m0 = (local / m.nbn) * kF32Tile, n0 = (local % m.nbn) * kF32Tile;
+  const int tx = threadIdx.x & 15, ty = threadIdx.x >> 4;
+  float acc[4][4] = {};
+  for (int k0 = 0; k0 < m.K; k0 += kF32BK) {
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+      const int idx = threadIdx.x + i * kF32Threads;
+      const int r = idx >> 4, k = idx & 15;
+      As[k][r] = (m0 + r < m.M && k0 + k < m.K) ? __ldg(m.x + (int64_t)(m0 + r) * m.ldx + k0 + k) : 0.f;
+      Bs[k][r] = (n0 + r < m.N && k0 + k < m.K) ? __ldg(m.w + (int64_t)(n0 + r) * m.ldw + k0 + k) : 0.f;
+    }
+    __syncthreads();
+#pragma unroll
+    for (int k = 0; k < kF32BK; ++k) {
+      float a[4], b[4];
+#pragma unroll
+      for (int i = 0; i < 4; ++i) { a[i] = As[k][ty * 4 + i]; b[i] = Bs[k][tx * 4 + i]; }
+#pragma unroll
+      for (int i = 0; i < 4; ++i)
+#pragma unroll
+        for (int j = 0; j < 4; ++j) acc[i][j] = fmaf(a[i], b[j], acc[i][j]);
+    }
+    __syncthreads();
+  }
+#pragma unroll
+  for (int i = 0; i < 4; ++i) {
+    const int r = m0 + ty * 4 + i;
+    if (r >= m.M) continue;
+#pragma unroll
+    for (int j = 0; j < 4; ++j) {
+      const int c = n0 + tx * 4 + j;
+      if (c >= m.N) continue;
+      float v = acc[i][j] + (m.bias ? __ldg(m.bias + c) : 0.f);
+      m.y[(int64_t)r * m.ldy + c] = act_f32<false>(v, m.act);
+    }
+  }
+}
+
+cudaError_t launch_linear_f32(const opt_plan* p, cudaStream_t s) {
+  const char* base = static_cast<const char*>(p->dev_tables);
+  grouped_gemm_f32_kernel<<<p->grid, p->block, 0, s>>>(reinterpret_cast<const F32Member*>(base + p->off0),
+                                                      reinterpret_cast<const int32_t*>(base + p->off1), p->n_members);
+  return cudaGetLastError();
+}
+
+// ===================================================== bf16 tcgen05 path =====
+constexpr int kBM = 128;           // tile rows (UMMA M, cta_group::1)
+constexpr int kBK = 64;            // K per stage = one 128-byte swizzle row of bf16
+constexpr int kMaxBN = 256;        // widest tile (UMMA N)
+constexpr int kStages = 4;
+constexpr int kAccStages = 2;
+constexpr int kTmemCols = 512;     // 2 accumulator stages x 256 fp32 columns
+constexpr int kGemmThreads = 192;  // warp 0 TMA, warp 1 MMA, warps 2..5 epilogue
+constexpr int kABytes = kBM * kBK * 2;          // 16 KB
+constexpr int kBBytesMax = kMaxBN * kBK * 2;    // 32 KB
+constexpr int kStageBytes = kABytes + kBBytesMax;
+constexpr int kEpiBufBytes = 32 * 128;          // one warp's 32 rows x 64 bf16 staging tile
+constexpr int kEpiBufs = 2;                     // per warp
+constexpr int kSmemBar = kStages * kStageBytes + 4 * kEpiBufs * kEpiBufBytes;
+constexpr int kSmemBytes = kSmemBar + 256 + 1024;   // barriers + slack for 1024-byte alignment
+
+struct alignas(128) GemmMember {
+  CUtensorMap tmA;       // X [M,K]   box {64, 128}   load
+  CUtensorMap tmB;       // W [N,K]   box {64, BN}    load
+  CUtensorMap tmY;       // Y [M,N]   box {64, 32}    store
+  const void* bias;      // [N] bf16 or NULL
+  int32_t M, N, K;
+  int32_t bn;            // tile width of this member
+  int32_t nbn;           // n-blocks per m-block
+  int32_t nkb;           // K blocks
+  int32_t act;
+  uint32_t idesc;        // tcgen05 instruction descriptor (M=128, N=bn, bf16 x bf16 -> fp32)
+  uint32_t b_bytes;      // bytes of one W stage = bn * 128
+  int32_t pad[5];
+};
+static_assert(sizeof(GemmMember) % 128 == 0, "GemmMember must keep tensor maps 128-byte aligned");
+
+// ---- PTX wrappers ------------------------------------------------------------
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count));
+}
+__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint32_t bar) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
+// Bounded spin: a protocol bug traps (CUDA error) instead of hanging the GPU.
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
+  uint32_t done = 0;
+  for (uint32_t spin = 0; !done; ++spin) {
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+        "selp.u32 %0, 1, 0, p;\n\t}"
+        : "=r"(done) : "r"(bar), "r"(parity) : "memory");
+    if (spin > (1u << 26)) __trap();
+  }
+}
+__device__ __forceinline__ void tma_load_2d(uint32_t dst, const void* tmap, uint32_t bar, int c0, int c1) {
+  asm volatile(
+      "cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4}], [%2];"
+      ::"r"(dst), "l"(tmap), "r"(bar), "r"(c0), "r"(c1) : "memory");
+}
+__device__ __forceinline__ void tma_store_2d(const void* tmap, uint32_t src, int c0, int c1) {
+  asm volatile("cp.async.bulk.tensor.2d.global.shared::cta.bulk_group [%0, {%2, %3}], [%1];"
+               ::"l"(tmap), "r"(src), "r"(c0), "r"(c1) : "memory");
+}
+__device__ __forceinline__ void tma_store_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
+template <int N>
+__device__ __forceinline__ void tma_store_wait_read() {
+  asm volatile("cp.async.bulk.wait_group.read %0;" ::"n"(N) : "memory");
+}
+__device__ __forceinline__ void tma_store_wait_all() { asm volatile("cp.async.bulk.wait_group 0;" ::: "memory"); }
+__device__ __forceinline__ void fence_proxy_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+__device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
+__device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
+__device__ __forceinline__ void tc_commit(uint32_t bar) {
+  asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void tc_mma_bf16(uint32_t d_tmem, uint64_t a_desc, uint64_t b_desc, uint32_t idesc,
+                                            uint32_t accumulate) {
+  asm volatile(
+      "{\n\t.reg .pred p;\n\t"
+      "setp.ne.b32 p, %4, 0;\n\t"
+      "tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n\t}"
+      ::"r"(d_tmem), "l"(a_desc), "l"(b_desc), "r"(idesc), "r"(accumulate) : "memory");
+}
+// 32 lanes x 32 consecutive fp32 columns: thread t of the warp gets lane (base lane + t)
+__device__ __forceinline__ void tc_ld_32x32(uint32_t taddr, uint32_t (&r)[32]) {
+  asm volatile(
+      "tcgen05.ld.sync.aligned.32x32b.x32.b32 "
+      "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, "
+      "%16, %17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31}, [%32];"
+      : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]),
+        "=r"(r[8]), "=r"(r[9]), "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15]),
+        "=r"(r[16]), "=r"(r[17]), "=r"(r[18]), "=r"(r[19]), "=r"(r[20]), "=r"(r[21]), "=r"(r[22]), "=r"(r[23]),
+        "=r"(r[24]), "=r"(r[25]), "=r"(r[26]), "=r"(r[27]), "=r"(r[28]), "=r"(r[29]), "=r"(r[30]), "=r"(r[31])
+      : "r"(taddr));
+}
+__device__ __forceinline__ void tc_wait_ld() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
+
+// Shared-memory matrix descriptor, K-major operand, 128-byte swizzle: rows of
+// 128 bytes, 8-row groups 1024 bytes apart (SBO), LBO unused, version 1 (sm_100).
+__device__ __forceinline__ uint64_t umma_desc_sw128(uint32_t saddr) {
+  return (uint64_t)((saddr & 0x3FFFFu) >> 4) | ((uint64_t)(1024 >> 4) << 32) | (1ull << 46) | (2ull << 61);
+}
+
+__device__ __forceinline__ float bias_at(const uint4* bv, int i) {   // i-th bf16 of an 8-vector array
+  const uint32_t u = reinterpret_cast<const uint32_t*>(bv)[i >> 1];
+  return (i & 1) ? bf16_hi(u) : bf16_lo(u);
+}
+
+__global__ void __launch_bounds__(kGemmThreads, 1)
+grouped_gemm_sm100_kernel(const GemmMember* __restrict__ members, const int32_t* __restrict__ starts,
+                          int n_members, int total_tiles) {
+  extern __shared__ uint8_t smem_raw[];
+  uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
+  const uint32_t sbase = smem_u32(smem);
+  const uint32_t epi_base = sbase + kStages * kStageBytes;
+  const uint32_t bar_base = sbase + kSmemBar;
+  // barrier layout (8 bytes each): full[kStages], empty[kStages], tmem_full[2], tmem_empty[2], then tmem ptr
+  auto full_bar = [&](int s) { return bar_base + 8u * s; };
+  auto empty_bar = [&](int s) { return bar_base + 8u * (kStages + s); };
+  auto tfull_bar = [&](int s) { return bar_base + 8u * (2 * kStages + s); };
+  auto tempty_bar = [&](int s) { return bar_base + 8u * (2 * kStages + kAccStages + s); };
+  volatile uint32_t* tmem_ptr_smem = reinterpret_cast<volatile uint32_t*>(smem + kSmemBar + 8 * (2 * kStages + 2 * kAccStages));
+
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+
+  if (warp == 0 && lane == 0) {
+    for (int s = 0; s < kStages; ++s) { mbar_init(full_bar(s), 1); mbar_init(empty_bar(s), 1); }
+    for (int s = 0; s < kAccStages; ++s) { mbar_init(tfull_bar(s), 1); mbar_init(tempty_bar(s), 4); }
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    fence_proxy_async_smem();
+  }
+  if (warp == 1) {
+    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;"
+                 ::"r"(smem_u32((const void*)tmem_ptr_smem)), "n"(kTmemCols) : "memory");
+    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+  }
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+  const uint32_t tmem_base = *tmem_ptr_smem;
+
+  if (warp == 0) {
+    // ------------------------------------------------------- TMA producer ----
+    if (lane == 0) {
+      int stage = 0; uint32_t phase = 0;
+      for (int tile = blockIdx.x; tile < total_tiles; tile += gridDim.x) {
+        const int mi = find_member(starts, n_members, tile);
+        const GemmMember* m = members + mi;
+        const int local = tile - __ldg(starts + mi);
+        const int nbn = m->nbn, nkb = m->nkb, bn = m->bn;
+        const int m0 = (local / nbn) * kBM, n0 = (local % nbn) * bn;
+        const uint32_t tx_bytes = kABytes + m->b_bytes;
+        for (int kb = 0; kb < nkb; ++kb) {
+          mbar_wait(empty_bar(stage), phase ^ 1);
+          mbar_expect_tx(full_bar(stage), tx_bytes);
+          const uint32_t sa = sbase + stage * kStageBytes;
+          tma_load_2d(sa, &m->tmA, full_bar(stage), kb * kBK, m0);
+          tma_load_2d(sa + kABytes, &m->tmB, full_bar(stage), kb * kBK, n0);
+          if (++stage == kStages) { stage = 0; phase ^= 1; }
+        }
+      }
+    }
+  } else if (warp == 1) {
+    // --------------------------------------------------------- MMA issuer ----
+    if (lane == 0) {
+      int stage = 0; uint32_t phase = 0;
+      int as = 0; uint32_t aphase = 0;
+      for (int tile = blockIdx.x; tile < total_tiles; tile += gridDim.x) {
+        const int mi = find_member(starts, n_members, tile);
+        const GemmMember* m = members + mi;
+        const int nkb = m->nkb, K = m->K;
+        const uint32_t idesc = m->idesc;
+        mbar_wait(tempty_bar(as), aphase ^ 1);      // epilogue has drained this accumulator stage
+        tc_fence_after();
+        const uint32_t d_tmem = tmem_base + as * kMaxBN;
+        for (int kb = 0; kb < nkb; ++kb) {
+          mbar_wait(full_bar(stage), phase);
+          tc_fence_after();
+          const uint32_t sa = sbase + stage * kStageBytes;
+          const uint64_t adesc = umma_desc_sw128(sa), bdesc = umma_desc_sw128(sa + kABytes);
+          const int ksteps = min(kBK / 16, (K - kb * kBK + 15) / 16);
+          for (int k = 0; k < ksteps; ++k)   // +32 bytes (= +2 encoded) per K=16 step inside the swizzle row
+            tc_mma_bf16(d_tmem, adesc + 2 * k, bdesc + 2 * k, idesc, (kb | k) != 0);
+          tc_commit(empty_bar(stage));       // frees the smem stage when these MMAs retire
+          if (++stage == kStages) { stage = 0; phase ^= 1; }
+        }
+        tc_commit(tfull_bar(as));            // accumulator complete
+        if (++as == kAccStages) { as = 0; aphase ^= 1; }
+      }
+    }
+  } else {
+    // ----------------------------------------------------------- epilogue ----
+    const int quad = warp & 3;               // TMEM lane quadrant this warp may read
+    const uint32_t my_epi = epi_base + (uint32_t)(warp - 2) * kEpiBufs * kEpiBufBytes;
+    int as = 0; uint32_t aphase = 0;
+    int buf = 0;
+    for (int tile = blockIdx.x; tile < total_tiles; tile += gridDim.x) {
+      const int mi = find_member(starts, n_members, tile);
+      const GemmMember* m = members + mi;
+      const int local = tile - __ldg(starts + mi);
+      const int nbn = m->nbn, bn = m->bn, N = m->N, act = m->act;
+      const int m0 = (local / nbn) * kBM, n0 = (local % nbn) * bn;
+      const uint4* bias = reinterpret_cast<const uint4*>(m->bias);
+      mbar_wait(tfull_bar(as), aphase);
+      tc_fence_after();
+      const uint32_t t_row = tmem_base + ((uint32_t)(quad * 32) << 16) + as * kMaxBN;
+      const int nchunks = (bn + 63) >> 6;
+      for (int c = 0; c < nchunks; ++c) {
+        uint32_t v[64];
+        tc_ld_32x32(t_row + c * 64, *reinterpret_cast<uint32_t(*)[32]>(&v[0]));
+        tc_ld_32x32(t_row + c * 64 + 32, *reinterpret_cast<uint32_t(*)[32]>(&v[32]));
+        // bias for the 64 columns of this chunk (warp-uniform addresses -> broadcast loads)
+        const int col0 = n0 + c * 64;
+        uint4 bv[8];
+#pragma unroll
+        for (int j = 0; j < 8; ++j)
+          bv[j] = (bias != nullptr && col0 + j * 8 < N) ? __ldg(bias + ((col0 + j * 8) >> 3)) : make_uint4(0, 0, 0, 0);
+        tc_wait_ld();
+        if (c == nchunks - 1) {              // accumulator fully in registers: hand the TMEM stage back
+          tc_fence_before();
+          __syncwarp();
+          if (lane == 0) mbar_arrive(tempty_bar(as));
+        }
+        // staging buffer free? (the TMA store issued two chunks ago has read it)
+        if (lane == 0) tma_store_wait_read<kEpiBufs - 1>();
+        __syncwarp();
+        const uint32_t sbuf = my_epi + buf * kEpiBufBytes;
+        const uint32_t srow = sbuf + lane * 128;
+#pragma unroll
+        for (int j = 0; j < 8; ++j) {        // 8 columns -> one 16-byte chunk, 128B-swizzled position
+          uint32_t pk[4];
+#pragma unroll
+          for (int e = 0; e < 4; ++e) {
+            float lo = __uint_as_float(v[j * 8 + 2 * e]) + bias_at(&bv[j], 2 * e);
+            float hi = __uint_as_float(v[j * 8 + 2 * e + 1]) + bias_at(&bv[j], 2 * e + 1);
+            pk[e] = pack_bf16x2(act_f32<true>(lo, act), act_f32<true>(hi, act));
+          }
+          asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};"
+                       ::"r"(srow + ((j ^ (lane & 7)) << 4)), "r"(pk[0]), "r"(pk[1]), "r"(pk[2]), "r"(pk[3]) : "memory");
+        }
+        fence_proxy_async_smem();
+        __syncwarp();
+        if (lane == 0) {
+          tma_store_2d(&m->tmY, sbuf, col0, m0 + quad * 32);
+          tma_store_commit();
+        }
+        buf ^= 1;
+      }
+      if (++as == kAccStages) { as = 0; aphase ^= 1; }
+    }
+    if (lane == 0) tma_store_wait_all();
+  }
+
+  tc_fence_before();
+  __syncthreads();
+  if (warp == 1) {
+    tc_fence_after();
+    asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "n"(kTmemCols) : "memory");
+  }
+}
+
+cudaError_t launch_linear_bf16(const opt_plan* p, cudaStream_t s) {
+  const char* base = static_cast<const char*>(p->dev_tables);
+  grouped_gemm_sm100_kernel<<<p->grid, p->block, p->smem, s>>>(reinterpret_cast<const GemmMember*>(base + p->off0),
+                                                              reinterpret_cast<const int32_t*>(base + p->off1),
+                                                              p->n_members, p->total_tiles);
+  return cudaGetLastError();
+}
+
+// ------------------------------------------------------------- host side -----
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                  const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+static opt_status get_encoder(EncodeTiledFn* fn) {
+  static EncodeTiledFn cached = nullptr;
+  if (!cached) {
+    void* f = nullptr;
+    cudaDriverEntryPointQueryResult q;
+    OPT_CUDA_TRY(cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &f, cudaEnableDefault, &q));
+    if (q != cudaDriverEntryPointSuccess || !f) return fail(OPT_ERR_CUDA, "cuTensorMapEncodeTiled not available from the driver");
+    cached = reinterpret_cast<EncodeTiledFn>(f);
+  }
+  *fn = cached;
+  return OPT_OK;
+}
+
+// 2-D bf16 tensor [rows, cols], row stride ld elements, box {box_cols, box_rows}, 128-byte swizzle
+static opt_status encode_2d(EncodeTiledFn enc, CUtensorMap* tm, const void* base, int64_t rows, int64_t cols, int64_t ld,
+                            int box_cols, int box_rows, CUtensorMapL2promotion promo, const char* what, int member) {
+  cuuint64_t dims[2] = {(cuuint64_t)cols, (cuuint64_t)rows};
+  cuuint64_t strides[1] = {(cuuint64_t)ld * 2};
+  cuuint32_t box[2] = {(cuuint32_t)box_cols, (cuuint32_t)box_rows};
+  cuuint32_t estr[2] = {1, 1};
+  CUresult r = enc(tm, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, const_cast<void*>(base), dims, strides, box, estr,
+                   CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, promo, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  if (r != CUDA_SUCCESS)
+    return fail(OPT_ERR_CUDA, "cuTensorMapEncodeTiled(%s of member %d: rows=%lld cols=%lld ld=%lld box=%dx%d) -> CUresult %d",
+                what, member, (long long)rows, (long long)cols, (long long)ld, box_cols, box_rows, (int)r);
+  return OPT_OK;
+}
+
+static int choose_bn(int N) {
+  if (N <= kMaxBN) return (N + 15) / 16 * 16;          // one n-block, UMMA N multiple of 16
+  // several n-blocks: multiples of 64 only (epilogue chunks must not spill into the next block)
+  int best = 256, best_pad = INT32_MAX;
+  for (int bn : {256, 192, 128}) {
+    const int pad = (N + bn - 1) / bn * bn - N;
+    if (pad < best_pad) { best_pad = pad; best = bn; }
+  }
+  return best;
+}
+
+}  // namespace optb
+
+using namespace optb;
+
+extern "C" opt_status opt_linear_plan_create(const opt_linear_member* members, int32_t n, opt_dtype io, int device,
+                                             opt_plan** plan) {
+  if (plan) *plan = nullptr;
+  if (!plan || !members) return fail(OPT_ERR_INVALID_ARG, "opt_linear_plan_create: NULL argument");
+  if (n < 1 || n > 65535) return fail(OPT_ERR_INVALID_ARG, "n = %d outside [1, 65535]", n);
+  if (io != OPT_F32 && io != OPT_BF16) return fail(OPT_ERR_INVALID_ARG, "bad io dtype %d", (int)io);
+  const int esz = elem_size(io), V = vec_elems(io);
+  std::vector<Region> regions;
+  int64_t flops = 0, bytes = 0;
+  for (int32_t i = 0; i < n; ++i) {
+    const opt_linear_member& m = members[i];
+    if (!m.x || !m.w || !m.y) return fail(OPT_ERR_INVALID_ARG, "member %d: NULL pointer", i);
+    if (m.M < 1 || m.N < 1 || m.K < 1) return fail(OPT_ERR_INVALID_ARG, "member %d: M=%d N=%d K=%d must be >= 1", i, m.M, m.N, m.K);
+    if (m.act < OPT_ACT_NONE || m.act > OPT_ACT_SIGMOID) return fail(OPT_ERR_INVALID_ARG, "member %d: bad activation %d", i, m.act);
+    if ((m.M > 1 && (m.ldx < m.K || m.ldy < m.N)) || (m.N > 1 && m.ldw < m.K))
+      return fail(OPT_ERR_INVALID_ARG, "member %d: row stride smaller than the row", i);
+    if (!aligned16(m.x) || !aligned16(m.w) || !aligned16(m.y) || !aligned16(m.bias))
+      return fail(OPT_ERR_ALIGNMENT, "member %d: pointers must be 16-byte aligned", i);
+    if (m.K % V || m.N % V) return fail(OPT_ERR_ALIGNMENT, "member %d: K=%d and N=%d must be multiples of %d (PAPER.md:445)", i, m.K, m.N, V);
+    if (m.ldx % V || m.ldw % V || m.ldy % V) return fail(OPT_ERR_ALIGNMENT, "member %d: row strides must be multiples of %d elements", i, V);
+    regions.push_back({(uintptr_t)m.x, m.ldx * esz, (int64_t)m.K * esz, m.M, false, i});
+    regions.push_back({(uintptr_t)m.w, m.ldw * esz, (int64_t)m.K * esz, m.N, false, i});
+    if (m.bias) regions.push_back({(uintptr_t)m.bias, 0, (int64_t)m.N * esz, 1, false, i});
+    regions.push_back({(uintptr_t)m.y, m.ldy * esz, (int64_t)m.N * esz, m.M, true, i});
+    flops += 2ll * m.M * m.N * m.K;
+    bytes += ((int64_t)m.M * m.K + (int64_t)m.N * m.K + (m.bias ? m.N : 0) + (int64_t)m.M * m.N) * esz;
+  }
+  if (opt_status st = check_independent(regions, /*allow_inplace_self=*/false)) return st;
+
+  int num_sms = 0;
+  if (opt_status st = open_device(device, &num_sms)) return st;
+  auto align_up = [](size_t x) { return (x + 255) & ~size_t(255); };
+  opt_plan* p = new opt_plan();
+  p->device = device; p->io = io; p->n_members = n; p->flops = flops; p->bytes = bytes;
+  std::vector<int32_t> starts(n + 1);
+  int64_t tiles = 0;
+
+  if (io == OPT_F32) {
+    std::vector<F32Member> tab(n);
+    for (int32_t i = 0; i < n; ++i) {
+      const opt_linear_member& m = members[i];
+      F32Member& t = tab[i];
+      t.x = (const float*)m.x; t.w = (const float*)m.w; t.bias = (const float*)m.bias; t.y = (float*)m.y;
+      t.ldx = m.ldx; t.ldw = m.ldw; t.ldy = m.ldy; t.M = m.M; t.N = m.N; t.K = m.K; t.act = m.act;
+      t.nbn = (m.N + kF32Tile - 1) / kF32Tile; t.pad = 0;
+      starts[i] = (int32_t)tiles;
+      tiles += (int64_t)((m.M + kF32Tile - 1) / kF32Tile) * t.nbn;
+      if (tiles > INT32_MAX) { delete p; return fail(OPT_ERR_UNSUPPORTED, "too many tiles"); }
+    }
+    starts[n] = (int32_t)tiles;
+    p->kind = kPlanLinearF32;
+    p->off0 = 0; p->off1 = align_up(tab.size() * sizeof(F32Member));
+    const size_t total = p->off1 + align_up(starts.size() * sizeof(int32_t));
+    std::vector<char> blob(total, 0);
+    memcpy(blob.data(), tab.data(), tab.size() * sizeof(F32Member));
+    memcpy(blob.data() + p->off1, starts.data(), starts.size() * sizeof(int32_t));
+    if (opt_status st = upload_tables(p, blob.data(), total)) { delete p; return st; }
+    p->grid = dim3((unsigned)tiles); p->block = dim3(kF32Threads); p->smem = 0;
+    p->total_tiles = (int32_t)tiles;
+    *plan = p;
+    return OPT_OK;
+  }
+
+  EncodeTiledFn enc = nullptr;
+  if (opt_status st = get_encoder(&enc)) { delete p; return st; }
+  std::vector<GemmMember> tab(n);
+  memset(tab.data(), 0, tab.size() * sizeof(GemmMember));
+  for (int32_t i = 0; i < n; ++i) {
+    const opt_linear_member& m = members[i];
+    GemmMember& t = tab[i];
+    const int bn = choose_bn(m.N);
+    opt_status st;
+    if ((st = encode_2d(enc, &t.tmA, m.x, m.M, m.K, m.ldx, kBK, kBM, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, "X", i)) ||
+        (st = encode_2d(enc, &t.tmB, m.w, m.N, m.K, m.ldw, kBK, bn, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, "W", i)) ||
+        (st = encode_2d(enc, &t.tmY, m.y, m.M, m.N, m.ldy, 64, 32, CU_TENSOR_MAP_L2_PROMOTION_NONE, "Y", i))) {
+      delete p;
+      return st;
+    }
+    t.bias = m.bias; t.M = m.M; t.N = m.N; t.K = m.K; t.bn = bn;
+    t.nbn = (m.N + bn - 1) / bn; t.nkb = (m.K + kBK - 1) / kBK; t.act = m.act;
+    // tcgen05 instruction descriptor, kind::f16: D fp32 (bits 4-5 = 1), A bf16 (bits 7-9 = 1), B bf16
+    // (bits 10-12 = 1), A and B K-major (bits 15, 16 = 0), N>>3 at bits 17-22, M>>4 at bits 24-28.
+    t.idesc = (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(bn >> 3) << 17) | ((uint32_t)(kBM >> 4) << 24);
+    t.b_bytes = (uint32_t)bn * kBK * 2;
+    starts[i] = (int32_t)tiles;
+    tiles += (int64_t)((m.M + kBM - 1) / kBM) * t.nbn;
+    if (tiles > INT32_MAX) { delete p; return fail(OPT_ERR_UNSUPPORTED, "too many tiles"); }
+  }
+  starts[n] = (int32_t)tiles;
+  p->kind = kPlanLinearBf16;
+  p->off0 = 0; p->off1 = align_up(tab.size() * sizeof(GemmMember));
+  const size_t total = p->off1 + align_up(starts.size() * sizeof(int32_t));
+  std::vector<char> blob(total, 0);
+  memcpy(blob.data(), tab.data(), tab.size() * sizeof(GemmMember));
+  memcpy(blob.data() + p->off1, starts.data(), starts.size() * sizeof(int32_t));
+  if (opt_status st = upload_tables(p, blob.data(), total)) { delete p; return st; }
+  cudaError_t e = cudaFuncSetAttribute(grouped_gemm_sm100_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBytes);
+  if (e != cudaSuccess) {
+    cudaFree(p->dev_tables); delete p;
+    return fail(OPT_ERR_CUDA, "cudaFuncSetAttribute(max dynamic smem %d) failed: %s", kSmemBytes, cudaGetErrorString(e));
+  }
+  p->grid = dim3((unsigned)std::min<int64_t>(tiles, num_sms)); p->block = dim3(kGemmThreads); p->smem = kSmemBytes;
+  p->total_tiles = (int32_t)tiles;
+  *plan = p;
+  return OPT_OK;
+}

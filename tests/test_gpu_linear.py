@@ -1,0 +1,165 @@
+"""GPU parity: grouped Linear+bias+activation vs the CPU oracle (through the C ABI)."""
+import numpy as np
+import pytest
+import torch
+
+import oracle
+from oracle import graphs
+import workloads as wl
+from util import BF16, F32, bf16_ulp_distance, empty_dev, row_l2_rel_err, to_dev, to_host
+
+pytestmark = pytest.mark.gpu
+
+TOL_BF16 = 1e-2     # north_star: max relative error, normalised by the row's L2 norm
+TOL_F32 = 1e-5      # DESIGN.md reading Q10 (true fp32 FFMA, K <= 64)
+
+
+@pytest.fixture(scope="module")
+def ob():
+    import paper_2607_02945_b200 as ob
+    return ob
+
+
+def run_linear(ob, members, dt, concat=False):
+    """-> list of host outputs (storage dtype) per member; one launch."""
+    M = members[0]["M"]
+    dx = [to_dev(m["x"], dt) for m in members]
+    dw = [to_dev(m["w"], dt) for m in members]
+    db = [to_dev(m["b"], dt) if m.get("b") is not None else None for m in members]
+    if concat:
+        assert all(m["M"] == M for m in members)
+        width = sum(m["N"] for m in members)
+        ycat = empty_dev((M, width), dt, fill=float("nan"))
+        ys, off = [], 0
+        for m in members:
+            ys.append(ycat[:, off:off + m["N"]])
+            off += m["N"]
+    else:
+        ys = [empty_dev((m["M"], m["N"]), dt, fill=float("nan")) for m in members]
+    descs = [ob.linear_member(x, w, b, y, m["act"]) for x, w, b, y, m in zip(dx, dw, db, ys, members)]
+    plan = ob.opt_linear_plan_create(descs, dt)
+    n0 = ob.opt_launch_count()
+    plan.launch()
+    torch.cuda.synchronize()
+    assert ob.opt_launch_count() - n0 == 1 and plan.info()["launches"] == 1
+    return [to_host(y) for y in ys], plan
+
+
+def mk(seed, i, M, N, K, act, dt=BF16, bias=True):
+    return dict(M=M, N=N, K=K, act=act,
+                x=wl.tensor_normal(seed, 3 * i + 1, (M, K), 0, 1, dt),
+                w=wl.tensor_normal(seed, 3 * i + 2, (N, K), 0, K ** -0.5, dt),
+                b=wl.tensor_normal(seed, 3 * i + 3, (N,), 0, 0.1, dt) if bias else None)
+
+
+def int_member(rng, M, N, K, lim, act, dt=BF16):
+    conv = (lambda a: wl.bf16_bits_from_f32(a.astype(np.float32))) if dt == BF16 else (lambda a: a.astype(np.float32))
+    return dict(M=M, N=N, K=K, act=act, x=conv(rng.integers(-lim, lim + 1, (M, K))),
+                w=conv(rng.integers(-lim, lim + 1, (N, K))), b=conv(rng.integers(-lim, lim + 1, (N,))))
+
+
+# --------------------------------------------------------------------- fp32 --
+def test_config0_fp32_separate_and_concat(ob):
+    cfg = wl.config0()
+    z64, ref = graphs.linear_group(cfg["members"], F32)
+    sep, _ = run_linear(ob, cfg["members"], F32, concat=False)
+    cat, _ = run_linear(ob, cfg["members"], F32, concat=True)
+    for got, gotc, z in zip(sep, cat, z64):
+        assert row_l2_rel_err(got, z, F32) <= TOL_F32
+        assert got.tobytes() == gotc.tobytes()          # P10: concat slot == separate output, bit for bit
+
+
+def test_fp32_exact_integers_and_ragged(ob):
+    rng = np.random.default_rng(1)
+    members = [int_member(rng, 70, 36, 20, 3, 1, F32), int_member(rng, 5, 4, 4, 3, 0, F32),
+               int_member(rng, 129, 68, 100, 1, 1, F32)]
+    outs, _ = run_linear(ob, members, F32)
+    _, ref = graphs.linear_group(members, F32)
+    for g, r in zip(outs, ref):
+        assert np.array_equal(g, r)
+
+
+# --------------------------------------------------------------------- bf16 --
+def test_bf16_single_tile_exact_integers(ob):
+    """P9: small-integer operands, every partial sum exact -> bit-exact whatever the summation order."""
+    rng = np.random.default_rng(2)
+    for (M, N, K, lim, act) in [(128, 128, 64, 1, 0), (128, 64, 16, 3, 1), (128, 256, 128, 1, 0)]:
+        m = int_member(rng, M, N, K, lim, act)
+        outs, _ = run_linear(ob, [m], BF16)
+        _, ref = graphs.linear_group([m], BF16)
+        assert np.array_equal(outs[0], ref[0]), (M, N, K)
+
+
+def test_bf16_exact_integers_ragged_shapes(ob):
+    rng = np.random.default_rng(3)
+    shapes = [(200, 48, 32), (64, 8, 8), (130, 264, 72), (1, 16, 200), (257, 520, 136), (384, 1024, 256)]
+    members = [int_member(rng, M, N, K, 1, i % 2) for i, (M, N, K) in enumerate(shapes)]
+    outs, plan = run_linear(ob, members, BF16)
+    _, ref = graphs.linear_group(members, BF16)
+    for g, r, s in zip(outs, ref, shapes):
+        assert np.array_equal(g, r), s
+    assert plan.info()["flops"] == sum(2 * M * N * K for M, N, K in shapes)
+
+
+@pytest.mark.parametrize("seed", [2, 102, 202])
+def test_config2_small_concat(ob, seed):
+    cfg = wl.config2(seed=seed, M=300, n=24)            # all (K,N) classes, ragged M, concat output
+    z64, ref = graphs.linear_group(cfg["members"], BF16)
+    outs, _ = run_linear(ob, cfg["members"], BF16, concat=True)
+    sep, _ = run_linear(ob, cfg["members"], BF16, concat=False)
+    worst = 0.0
+    for got, s, z, r in zip(outs, sep, z64, ref):
+        worst = max(worst, row_l2_rel_err(got, z, BF16))
+        assert got.tobytes() == s.tobytes()             # P10
+        assert np.percentile(bf16_ulp_distance(got, r), 99) <= 1
+    assert worst <= TOL_BF16, worst
+
+
+def test_bf16_activations_and_no_bias(ob):
+    members = [mk(31, 0, 150, 96, 160, 2), mk(31, 1, 150, 40, 64, 3), mk(31, 2, 150, 128, 256, 0, bias=False),
+               mk(31, 3, 150, 320, 8, 1)]
+    z64, ref = graphs.linear_group(members, BF16)
+    outs, _ = run_linear(ob, members, BF16)
+    for got, z, r in zip(outs, z64, ref):
+        assert row_l2_rel_err(got, z, BF16) <= TOL_BF16
+        assert bf16_ulp_distance(got, r).max() <= 2 or np.percentile(bf16_ulp_distance(got, r), 99.9) <= 2
+
+
+def test_equal_shape_group_matches_batched(ob):
+    """P6: batch fusion special case (equal shapes) through the same grouped kernel, no stack/unbind."""
+    members = [mk(32, i, 256, 128, 128, 1) for i in range(6)]
+    z64, _ = graphs.linear_group(members, BF16)
+    outs, _ = run_linear(ob, members, BF16)
+    for got, z in zip(outs, z64):
+        assert row_l2_rel_err(got, z, BF16) <= TOL_BF16
+
+
+def test_shared_input_batch_linear_lhs(ob):
+    """batch_linear_lhs: members may alias their input."""
+    x = wl.tensor_normal(33, 1, (192, 128), 0, 1, BF16)
+    members = [dict(mk(33, i, 192, 64 * (i + 1), 128, 1), x=x) for i in range(3)]
+    z64, _ = graphs.linear_group(members, BF16)
+    dx = to_dev(x, BF16)
+    dw = [to_dev(m["w"], BF16) for m in members]
+    db = [to_dev(m["b"], BF16) for m in members]
+    ys = [empty_dev((192, m["N"]), BF16) for m in members]
+    plan = ob.opt_linear_plan_create([ob.linear_member(dx, w, b, y, 1) for w, b, y in zip(dw, db, ys)], BF16)
+    plan.launch()
+    torch.cuda.synchronize()
+    for y, z in zip(ys, z64):
+        assert row_l2_rel_err(to_host(y), z, BF16) <= TOL_BF16
+
+
+def test_errors(ob):
+    x = empty_dev((64, 64), BF16, fill=0.0)
+    w = empty_dev((64, 64), BF16, fill=0.0)
+    y = empty_dev((64, 128), BF16, fill=0.0)
+    with pytest.raises(ob.OptError) as e:   # overlapping concat slots
+        ob.opt_linear_plan_create([ob.linear_member(x, w, None, y[:, 0:64]), ob.linear_member(x, w, None, y[:, 32:96])], BF16)
+    assert e.value.status == ob.OPT_ERR_ALIAS
+    with pytest.raises(ob.OptError) as e:   # K not a multiple of 8
+        ob.opt_linear_plan_create([ob.linear_member(x[:, :60], w[:, :60], None, y[:, :64])], BF16)
+    assert e.value.status == ob.OPT_ERR_ALIGNMENT
+    with pytest.raises(ob.OptError) as e:   # output aliases input
+        ob.opt_linear_plan_create([ob.linear_member(x, w, None, x)], BF16)
+    assert e.value.status == ob.OPT_ERR_ALIAS

@@ -1,0 +1,144 @@
+"""GPU parity: multi_pointwise_splitcat vs the CPU oracle (through the C ABI)."""
+import numpy as np
+import pytest
+import torch
+
+import oracle
+from oracle import graphs
+import workloads as wl
+from util import BF16, F32, bf16_ulp_distance, empty_dev, to_dev, to_host
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def ob():
+    import paper_2607_02945_b200 as ob
+    return ob
+
+
+def run_split_cat(ob, x_host, widths, ops, perm, dt=BF16):
+    x = to_dev(x_host, dt)
+    out = empty_dev(x.shape, dt, fill=float("nan"))
+    plan = ob.opt_pointwise_plan_create(ob.split_cat_chunks(x, out, widths, ops, perm), dt)
+    n0 = ob.opt_launch_count()
+    plan.launch()
+    torch.cuda.synchronize()
+    assert ob.opt_launch_count() - n0 == 1 and plan.info()["launches"] == 1
+    return to_host(out), plan
+
+
+@pytest.mark.parametrize("dt", [BF16, F32])
+def test_paper_listing2_example_bit_exact(ob, dt):
+    """PAPER.md:403-416 Listing 2 == Listing 1 (return x).  Widths are in units the
+    alignment rule allows (x8 for bf16, x4 for fp32): [2,4] -> [2*V, 4*V], second split (2*V, 2*V)."""
+    V = 8 if dt == BF16 else 4
+    x_host = wl.tensor_normal(7, 1, (2, 6 * V), 0, 1, dt)
+    widths = [2 * V, 2 * V, 2 * V]          # item0, item2, item3 of the listing
+    got, _ = run_split_cat(ob, x_host, widths, [0, 0, 0], [0, 1, 2], dt)
+    assert got.tobytes() == x_host.tobytes()
+    fs = oracle.split(x_host, [2 * V, 4 * V])
+    ref = oracle.cat([fs[0]] + oracle.split(fs[1], [2 * V, 2 * V]))
+    assert got.tobytes() == ref.tobytes()
+
+
+@pytest.mark.parametrize("seed", [3, 103, 203])
+def test_config3_small_movement_and_math(ob, seed):
+    cfg = wl.config3(seed=seed, rows=200, width=2048, nchunks=64)      # ragged rows, several column blocks
+    x, widths, ops, perm = cfg["x"], cfg["widths"], cfg["ops"], cfg["perm"]
+    # (i) every op = COPY: bit-exact column permutation
+    got, _ = run_split_cat(ob, x, widths, [0] * len(widths), perm)
+    assert got.tobytes() == graphs.split_copy_cat(x, widths, perm).tobytes()
+    # (ii) identity permutation + COPY: split o cat = identity
+    got, _ = run_split_cat(ob, x, widths, [0] * len(widths), list(range(len(widths))))
+    assert got.tobytes() == x.tobytes()
+    # (iii) real ops: <= 2 bf16 ulp of the oracle; ReLU chunks bit-exact
+    got, plan = run_split_cat(ob, x, widths, ops, perm)
+    ref64, ref = graphs.split_pointwise_cat(x, widths, ops, perm, BF16)
+    d = bf16_ulp_distance(got, ref)
+    assert d.max() <= 2, "max ulp %d" % d.max()
+    pos = 0
+    for p in perm:
+        if ops[p] == wl.gen.PW_RELU:
+            assert np.array_equal(bf16_ulp_distance(got[:, pos:pos + widths[p]], ref[:, pos:pos + widths[p]]),
+                                  np.zeros((200, widths[p]), dtype=np.int64))
+        pos += widths[p]
+    assert plan.info()["bytes"] == 2 * x.size * 2
+
+
+def test_multi_tensor_standalone_all_ops(ob):
+    """batch_relu / batch_sigmoid / batch_aten_tanh / batch_detach: n separate tensors, ragged sizes."""
+    shapes = [(1, 8), (3, 24), (64, 64), (257, 136), (1000, 512), (5, 8 * 1031), (2, 8 * 600)]
+    xs = [wl.tensor_normal(11, i + 1, s, 0, 2.0, BF16) for i, s in enumerate(shapes)]
+    ops = [i % 4 for i in range(len(shapes))]
+    dx = [to_dev(x, BF16) for x in xs]
+    dy = [empty_dev(x.shape, BF16, fill=float("nan")) for x in xs]
+    plan = ob.opt_pointwise_plan_create([ob.chunk(a, b, op) for a, b, op in zip(dx, dy, ops)], BF16)
+    n0 = ob.opt_launch_count()
+    plan.launch()
+    torch.cuda.synchronize()
+    assert ob.opt_launch_count() - n0 == 1
+    for x, y, op in zip(xs, dy, ops):
+        ref = oracle.round_to_storage(oracle.pointwise(x, op, BF16), BF16)
+        d = bf16_ulp_distance(to_host(y), ref)
+        assert d.max() <= (0 if op in (0, 1) else 2), (x.shape, op, d.max())
+
+
+def test_strided_chunks_and_in_place(ob):
+    base = wl.tensor_normal(12, 1, (100, 320), 0, 1.5, BF16)
+    b = to_dev(base, BF16)
+    # in place tanh on a column slice, relu on another, rest untouched
+    chunks = [ob.chunk(b[:, 8:72], b[:, 8:72], ob.OPT_PW_TANH), ob.chunk(b[:, 200:264], b[:, 200:264], ob.OPT_PW_RELU)]
+    ob.opt_pointwise_plan_create(chunks, BF16).launch()
+    torch.cuda.synchronize()
+    got = to_host(b)
+    ref = base.copy()
+    ref[:, 8:72] = oracle.round_to_storage(oracle.pointwise(base[:, 8:72], 2, BF16), BF16)
+    ref[:, 200:264] = oracle.round_to_storage(oracle.pointwise(base[:, 200:264], 1, BF16), BF16)
+    assert bf16_ulp_distance(got, ref).max() <= 2
+    assert np.array_equal(got[:, :8], base[:, :8]) and np.array_equal(got[:, 72:200], base[:, 72:200])
+
+
+def test_special_values_q13(ob):
+    vals = np.array([np.nan, np.inf, -np.inf, -0.0, 0.0, 1e-30, -1e-30, 88.0, -88.0, 100.0, -100.0, 3e38, -3e38,
+                     1e-3, -1e-3, 20.0], dtype=np.float32)
+    x = wl.bf16_bits_from_f32(vals).reshape(1, 16)
+    x[0, 0] = 0x7FC0
+    for op in (1, 2, 3):
+        dx = to_dev(x, BF16)
+        dy = empty_dev(x.shape, BF16)
+        ob.opt_pointwise_plan_create([ob.chunk(dx, dy, op)], BF16).launch()
+        torch.cuda.synchronize()
+        ref = oracle.round_to_storage(oracle.pointwise(x, op, BF16), BF16)
+        d = bf16_ulp_distance(to_host(dy), ref)
+        assert d.max() <= 2, (op, to_host(dy), ref)
+
+
+def test_fp32_io(ob):
+    x = wl.tensor_normal(13, 1, (77, 100), 0, 2.0, F32)
+    for op in (0, 1, 2, 3):
+        dx, dy = to_dev(x, F32), empty_dev(x.shape, F32)
+        ob.opt_pointwise_plan_create([ob.chunk(dx, dy, op)], F32).launch()
+        torch.cuda.synchronize()
+        ref = oracle.pointwise(x, op, F32)
+        got = to_host(dy).astype(np.float64)
+        if op in (0, 1):
+            assert np.array_equal(got, ref)
+        else:   # fp32 libdevice tanhf/expf: a few fp32 ulp
+            assert np.all(np.abs(got - ref) <= 4 * 2.0 ** -23 * np.maximum(np.abs(ref), 2.0 ** -20))
+
+
+def test_errors_launch_nothing(ob):
+    x = empty_dev((16, 64), BF16, fill=0.0)
+    y = empty_dev((16, 64), BF16, fill=0.0)
+    n0 = ob.opt_launch_count()
+    with pytest.raises(ob.OptError) as e:
+        ob.opt_pointwise_plan_create([ob.chunk(x[:, :36], y[:, :36])], BF16)         # width % 8
+    assert e.value.status == ob.OPT_ERR_ALIGNMENT
+    with pytest.raises(ob.OptError) as e:
+        ob.opt_pointwise_plan_create([ob.chunk(x[:, :32], y[:, :32]), ob.chunk(x[:, 32:], y[:, 24:56])], BF16)
+    assert e.value.status == ob.OPT_ERR_ALIAS
+    with pytest.raises(ob.OptError) as e:
+        ob.opt_pointwise_plan_create([], BF16)
+    assert e.value.status == ob.OPT_ERR_INVALID_ARG
+    assert ob.opt_launch_count() == n0
