@@ -1,0 +1,523 @@
+#!/usr/bin/env python
+"""bench.py -- the hot path of liboptimus_b200 timed on B200 (contract: DESIGN.md "Measurement").
+
+A STEP is one pass of the whole hot path over one batch of
+seeded synthetic input, i.e. the fused op groups of BASELINE.json configs[1..4] back to back,
+SIX kernel launches, one per group:
+
+    C1   batched LayerNorm      64 members [2048, D_i]                      1 launch
+    C2   grouped Linear+ReLU    128 members, M=4096, concat output          1 launch
+    C3   split-pointwise-cat    [8192, 8192], 256 chunks, permuted          1 launch
+    C4   recsys block           512 towers: LN -> Linear+ReLU -> Linear     3 launches
+
+(configs[0] is the tiny fp32 parity case; it is launch-latency bound and is timed only as a
+side figure.)  Metric: fused op-group latency, microseconds per step (BASELINE.json:metric);
+per-group latency, TFLOP/s or GB/s and roofline fractions ride in "groups".
+
+  python bench.py [--gpus N] [--steps K] [--warmup W]      product arm (CUDA, through the C ABI)
+  python bench.py --impl reference ...                      CPU oracle arm (bounded row sample)
+
+N > 1: "replicas only" -- every rank runs the same step on its own
+GPU, no collective on the data path; time = max over ranks.
+"""
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import workloads as wl  # noqa: E402
+
+BF16, F32 = wl.BF16, wl.F32
+ACT_NONE, ACT_RELU = 0, 1
+FULL = dict(c1_rows=2048, c1_n=64, c2_M=4096, c2_n=128, c3_rows=8192, c3_width=8192, c3_chunks=256,
+            c4_B=8192, c4_n=512)
+SMALL = dict(c1_rows=256, c1_n=16, c2_M=512, c2_n=16, c3_rows=512, c3_width=2048, c3_chunks=64,
+             c4_B=512, c4_n=24)
+
+
+def load_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        with open(p) as f:
+            d = json.load(f)
+        return dict(hbm_gbs=float(d["hbm_gbs"]), bf16_tflops=float(d["bf16_tflops"]),
+                    bf16_tflops_sustained=float(d.get("bf16_tflops_sustained", d["bf16_tflops"])),
+                    source="measured (MEASURED_PEAKS.json)")
+    return dict(hbm_gbs=6650.0, bf16_tflops=1590.0, bf16_tflops_sustained=1400.0,
+                source="fallback (B200_PROFILING.md)")
+
+
+# ------------------------------------------------------------------ arenas ---
+class Arena:
+    """One contiguous buffer carved into 256-byte aligned tensors: host (pinned) and device
+    mirrors share offsets, so a whole group's inputs move with ONE cudaMemcpyAsync."""
+
+    def __init__(self):
+        self.items = []      # (name, offset, host ndarray or None, shape, numpy dtype)
+        self.size = 0
+
+    def _push(self, name, a, shape, dtype):
+        off = self.size
+        self.items.append((name, off, a, tuple(shape), np.dtype(dtype)))
+        self.size = (off + int(np.prod(shape)) * np.dtype(dtype).itemsize + 255) & ~255
+        return len(self.items) - 1
+
+    def add(self, name, a):
+        a = np.ascontiguousarray(a)
+        return self._push(name, a, a.shape, a.dtype)
+
+    def reserve(self, name, shape, dt):
+        """space only (outputs / intermediates): no host data."""
+        return self._push(name, None, shape, np.uint16 if dt == BF16 else np.float32)
+
+    def materialise(self, device, pinned_host):
+        import torch
+        n = max(self.size, 256)
+        self.dev = torch.empty(n, dtype=torch.uint8, device=device)
+        self.host = torch.empty(n, dtype=torch.uint8)
+        if pinned_host:
+            self.host = self.host.pin_memory()
+        hv = self.host.numpy()
+        for _, off, a, _, _ in self.items:
+            if a is not None:
+                hv[off:off + a.nbytes] = a.reshape(-1).view(np.uint8)
+        if any(a is not None for _, _, a, _, _ in self.items):
+            self.dev.copy_(self.host)
+        if not pinned_host:
+            self.host = None
+        return self
+
+    def _span(self, idx):
+        _, off, _, shape, dtype = self.items[idx]
+        return off, int(np.prod(shape)) * dtype.itemsize, shape, dtype
+
+    def tensor(self, idx):
+        """device tensor view of item idx (bf16 or fp32, original shape)."""
+        import torch
+        off, n, shape, dtype = self._span(idx)
+        t = self.dev[off:off + n].view(torch.bfloat16 if dtype == np.uint16 else torch.float32)
+        return t.view(*shape)
+
+    def host_array(self, idx):
+        off, n, shape, dtype = self._span(idx)
+        return self.host.numpy()[off:off + n].view(dtype).reshape(shape)
+
+
+class Group:
+    """One fused op group: a plan (one launch) + what it reads/writes."""
+
+    def __init__(self, name, kind, plan, arena_in, arena_out, bound):
+        self.name, self.kind, self.plan, self.ain, self.aout, self.bound = name, kind, plan, arena_in, arena_out, bound
+        self.info = plan.info()
+
+
+class Step:
+    """All groups of one step, device-resident, built from the seeded generators."""
+
+    def __init__(self, device="cuda:0", sizes=None, pinned_host=True, configs=("c1", "c2", "c3", "c4")):
+        import torch
+        import paper_2607_02945_b200 as ob
+        self.ob, self.torch, self.device = ob, torch, device
+        self.sizes = dict(FULL if sizes is None else sizes)
+        self.pinned = pinned_host
+        self.groups = []
+        dev_index = torch.device(device).index or 0
+        self.dev_index = dev_index
+        for c in configs:
+            getattr(self, "_build_" + c)()
+
+    # ---- C1: batched LayerNorm
+    def _build_c1(self):
+        ob, s = self.ob, self.sizes
+        cfg = wl.config1(rows=s["c1_rows"], n=s["c1_n"])
+        ain, aout = Arena(), Arena()
+        idx = []
+        for m in cfg["members"]:
+            idx.append((ain.add("x", m["x"]), ain.add("gamma", m["gamma"]), ain.add("beta", m["beta"]),
+                        aout.reserve("y", m["x"].shape, BF16)))
+        ain.materialise(self.device, self.pinned), aout.materialise(self.device, self.pinned)
+        descs = [ob.layernorm_member(ain.tensor(ix), aout.tensor(iy), ain.tensor(ig), ain.tensor(ib), m["eps"])
+                 for (ix, ig, ib, iy), m in zip(idx, cfg["members"])]
+        plan = ob.opt_layernorm_plan_create(descs, BF16, BF16, self.dev_index)
+        g = Group("C1_batched_layernorm", "layernorm", plan, ain, aout, "hbm")
+        g.cfg, g.idx = cfg, idx
+        self.groups.append(g)
+
+    # ---- C2: grouped Linear + bias + ReLU, concat output (a2)
+    def _build_c2(self):
+        ob, s = self.ob, self.sizes
+        cfg = wl.config2(M=s["c2_M"], n=s["c2_n"])
+        ain, aout = Arena(), Arena()
+        idx = [(ain.add("x", m["x"]), ain.add("w", m["w"]), ain.add("b", m["b"])) for m in cfg["members"]]
+        iy = aout.reserve("ycat", (cfg["M"], cfg["concat_width"]), BF16)
+        ain.materialise(self.device, self.pinned), aout.materialise(self.device, self.pinned)
+        ycat = aout.tensor(iy)
+        descs = [ob.linear_member(ain.tensor(ix), ain.tensor(iw), ain.tensor(ib),
+                                  ycat[:, m["col_off"]:m["col_off"] + m["N"]], m["act"])
+                 for (ix, iw, ib), m in zip(idx, cfg["members"])]
+        plan = ob.opt_linear_plan_create(descs, BF16, self.dev_index)
+        g = Group("C2_grouped_linear_tower", "linear", plan, ain, aout, "tensor")
+        g.cfg, g.idx, g.iy = cfg, idx, iy
+        self.groups.append(g)
+
+    # ---- C3: split -> pointwise -> cat as one gather/scatter (a4, a5)
+    def _build_c3(self):
+        ob, s = self.ob, self.sizes
+        cfg = wl.config3(rows=s["c3_rows"], width=s["c3_width"], nchunks=s["c3_chunks"])
+        ain, aout = Arena(), Arena()
+        ix = ain.add("x", cfg["x"])
+        iy = aout.reserve("out", cfg["x"].shape, BF16)
+        ain.materialise(self.device, self.pinned), aout.materialise(self.device, self.pinned)
+        chunks = ob.split_cat_chunks(ain.tensor(ix), aout.tensor(iy), cfg["widths"], cfg["ops"], cfg["perm"])
+        plan = ob.opt_pointwise_plan_create(chunks, BF16, self.dev_index)
+        g = Group("C3_split_pointwise_cat", "pointwise", plan, ain, aout, "hbm")
+        g.cfg, g.ix, g.iy = cfg, ix, iy
+        self.groups.append(g)
+
+    # ---- C4: LN group -> GEMM group (+ReLU) -> GEMM group, concat (a6)
+    def _build_c4(self):
+        ob, s = self.ob, self.sizes
+        cfg = wl.config4(B=s["c4_B"], n=s["c4_n"])
+        tw = cfg["towers"]
+        ain, amid, aout = Arena(), Arena(), Arena()
+        idx = []
+        for t in tw:
+            idx.append(dict(x=ain.add("x", t["x"]), gamma=ain.add("gamma", t["gamma"]), beta=ain.add("beta", t["beta"]),
+                            w1=ain.add("w1", t["w1"]), b1=ain.add("b1", t["b1"]), w2=ain.add("w2", t["w2"]),
+                            b2=ain.add("b2", t["b2"]),
+                            xn=amid.reserve("xn", t["x"].shape, BF16), h=amid.reserve("h", (t["B"], t["H"]), BF16)))
+        iy = aout.reserve("out", (cfg["B"], cfg["concat_width"]), BF16)
+        ain.materialise(self.device, self.pinned)
+        amid.materialise(self.device, False)
+        aout.materialise(self.device, self.pinned)
+        out = aout.tensor(iy)
+        T = ain.tensor
+        ln = [ob.layernorm_member(T(i["x"]), amid.tensor(i["xn"]), T(i["gamma"]), T(i["beta"]), t["eps"])
+              for i, t in zip(idx, tw)]
+        l1 = [ob.linear_member(amid.tensor(i["xn"]), T(i["w1"]), T(i["b1"]), amid.tensor(i["h"]), ACT_RELU)
+              for i in idx]
+        l2 = [ob.linear_member(amid.tensor(i["h"]), T(i["w2"]), T(i["b2"]), out[:, k * t["out"]:(k + 1) * t["out"]],
+                               ACT_NONE) for k, (i, t) in enumerate(zip(idx, tw))]
+        empty = Arena().materialise(self.device, self.pinned)
+        g1 = Group("C4a_batched_layernorm", "layernorm", ob.opt_layernorm_plan_create(ln, BF16, BF16, self.dev_index),
+                   ain, empty, "hbm")
+        g2 = Group("C4b_grouped_linear_relu", "linear", ob.opt_linear_plan_create(l1, BF16, self.dev_index),
+                   empty, empty, "hbm")
+        g3 = Group("C4c_grouped_linear_concat", "linear", ob.opt_linear_plan_create(l2, BF16, self.dev_index),
+                   empty, aout, "hbm")
+        for g in (g1, g2, g3):
+            g.cfg, g.idx, g.amid, g.iy = cfg, idx, amid, iy
+        self.groups += [g1, g2, g3]
+
+    # ---- launching
+    def launch_all(self, stream=None):
+        for g in self.groups:
+            g.plan.launch(stream)
+
+    def launch_all_host(self, stream=None):
+        """e2e: per group, H2D of every input arena, the one kernel, D2H of every output arena --
+        all through opt_plan_launch_host (the C ABI call for HOST buffers)."""
+        ob = self.ob
+        for g in self.groups:
+            copies = []
+            if g.ain.size:
+                copies.append(ob.opt_host_copy(g.ain.host.data_ptr(), g.ain.dev.data_ptr(), g.ain.size, 1))
+            if g.aout.size:
+                copies.append(ob.opt_host_copy(g.aout.host.data_ptr(), g.aout.dev.data_ptr(), g.aout.size, 0))
+            g.plan.launch_host(copies, stream)
+
+    def h2d_bytes(self):
+        return sum(g.ain.size for g in self.groups)
+
+    def d2h_bytes(self):
+        return sum(g.aout.size for g in self.groups)
+
+
+# ------------------------------------------------------------- clock watch ---
+class ClockWatch(threading.Thread):
+    """Samples SM clock, power and throttle reasons through NVML while the timed regions run."""
+
+    def __init__(self, index):
+        super().__init__(daemon=True)
+        self.index, self.stop_flag, self.samples = index, threading.Event(), []
+        self.ok = False
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            # NVML enumerates physical devices; honour CUDA_VISIBLE_DEVICES when it is a plain index list
+            vis = os.environ.get("CUDA_VISIBLE_DEVICES")
+            phys = index
+            if vis:
+                try:
+                    phys = int(vis.split(",")[index])
+                except ValueError:
+                    phys = index
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(phys)
+            self.max_mhz = pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM)
+            self.ok = True
+        except Exception as e:  # noqa: BLE001
+            self.err = repr(e)
+
+    def run(self):
+        if not self.ok:
+            return
+        nv = self.nv
+        while not self.stop_flag.is_set():
+            try:
+                mhz = nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM)
+                reasons = nv.nvmlDeviceGetCurrentClocksEventReasons(self.h)
+                util = nv.nvmlDeviceGetUtilizationRates(self.h).gpu
+                self.samples.append((mhz, reasons, util))
+            except Exception:  # noqa: BLE001
+                pass
+            time.sleep(0.01)
+
+    def summary(self):
+        if not self.ok or not self.samples:
+            return dict(sm_mhz=None, sm_max_mhz=getattr(self, "max_mhz", None), reasons=["unavailable"])
+        nv = self.nv
+        mhz = sorted(s[0] for s in self.samples)
+        bits = 0
+        for s in self.samples:
+            bits |= s[1]
+        names = [("hw_slowdown", nv.nvmlClocksEventReasonHwSlowdown),
+                 ("hw_thermal_slowdown", nv.nvmlClocksEventReasonHwThermalSlowdown),
+                 ("sw_thermal_slowdown", nv.nvmlClocksEventReasonSwThermalSlowdown),
+                 ("sw_power_cap", nv.nvmlClocksEventReasonSwPowerCap),
+                 ("hw_power_brake", nv.nvmlClocksEventReasonHwPowerBrakeSlowdown)]
+        return dict(sm_mhz=mhz[len(mhz) // 2], sm_max_mhz=self.max_mhz, samples=len(mhz),
+                    reasons=[n for n, b in names if bits & b])
+
+
+# ------------------------------------------------------------- CPU oracle ----
+def oracle_sample_step(frac=1.0):
+    """The oracle, as it stands, on a bounded ROW sample of the step's workload; returns
+    (extrapolated microseconds per full step, seconds actually spent, description, cores)."""
+    import oracle
+    from oracle import graphs
+    base = dict(c1_rows=2048, c2_M=256, c3_rows=2048, c4_B=128)
+    rows = {k: max(8, int(v * frac) // 8 * 8) for k, v in base.items()}
+    rows["c1_rows"] = min(rows["c1_rows"], FULL["c1_rows"])
+    cores = oracle.max_threads()
+    c1 = wl.config1(rows=rows["c1_rows"])
+    c2 = wl.config2(M=rows["c2_M"])
+    c3 = wl.config3(rows=rows["c3_rows"])
+    c4 = wl.config4(B=rows["c4_B"])
+    parts = []
+    t = time.perf_counter(); graphs.layernorm_group(c1["members"], BF16); parts.append((time.perf_counter() - t, FULL["c1_rows"] / rows["c1_rows"]))
+    t = time.perf_counter(); graphs.linear_group_concat(c2["members"], BF16); parts.append((time.perf_counter() - t, FULL["c2_M"] / rows["c2_M"]))
+    t = time.perf_counter(); graphs.split_pointwise_cat(c3["x"], c3["widths"], c3["ops"], c3["perm"], BF16); parts.append((time.perf_counter() - t, FULL["c3_rows"] / rows["c3_rows"]))
+    t = time.perf_counter()
+    outs = [graphs.recsys_tower(tw)["out"] for tw in c4["towers"]]
+    oracle.cat(outs)
+    parts.append((time.perf_counter() - t, FULL["c4_B"] / rows["c4_B"]))
+    spent = sum(p[0] for p in parts)
+    full_us = sum(p[0] * p[1] for p in parts) * 1e6
+    desc = ("rows sampled per group: C1 %d/%d, C2 %d/%d, C3 %d/%d, C4 %d/%d (all members, all columns); "
+            "time scaled by rows_full/rows_sampled per group" %
+            (rows["c1_rows"], FULL["c1_rows"], rows["c2_M"], FULL["c2_M"], rows["c3_rows"], FULL["c3_rows"],
+             rows["c4_B"], FULL["c4_B"]))
+    return full_us, spent, desc, cores
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    K, W = args.steps, args.warmup
+    frac = min(1.0, (100.0 / max(1, K + W)) / 8.0)          # whole run ~100 s of CPU work
+    vals, spent_all, desc, cores = [], 0.0, "", 0
+    for i in range(W + K):
+        us, spent, desc, cores = oracle_sample_step(frac)
+        if i >= W:
+            vals.append(us)
+            spent_all += spent
+    v = float(np.mean(vals))
+    line = dict(metric="fused_op_group_step_latency", value=v, unit="us", n_gpus=args.gpus, steps=K, warmup=W,
+                ms_per_step=v / 1e3, higher_is_better=False, scaling="weak", vs_baseline=None, dtype="f64",
+                data="synthetic", impl="reference",
+                config=dict(workload=WORKLOAD_NAME, l2="n/a (CPU)"),
+                cpu_baseline=dict(value=v, unit="us", cores=cores, kind="oracle", sample=desc,
+                                  cpu_seconds_per_sampled_step=spent_all / max(1, K)),
+                e2e=dict(value=v, unit="us", h2d_bytes_per_step=0, d2h_bytes_per_step=0), gpu_launches=0)
+    print(json.dumps(line))
+    return 0
+
+
+WORKLOAD_NAME = ("whole hot path = fused groups of BASELINE.json configs[1..4] back to back: C1 batched LN x64, "
+                 "C2 grouped Linear+ReLU x128 (M=4096, concat), C3 split-pointwise-cat 8192x8192/256 chunks, "
+                 "C4 recsys block x512 (LN -> Linear+ReLU -> Linear, concat [8192,32768]); 6 launches/step")
+
+
+# -------------------------------------------------------------- product arm --
+def run_product(args):
+    import torch
+    import torch.distributed as dist
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device -- the product path has no CPU fallback")
+    torch.cuda.set_device(local)
+    device = "cuda:%d" % local
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device(device))
+    import paper_2607_02945_b200 as ob
+
+    peaks = load_peaks()
+    K, W = args.steps, max(args.warmup, 3)
+    t0 = time.time()
+    step = Step(device, SMALL if args.small else FULL, pinned_host=True)
+    build_s = time.time() - t0
+    stream = torch.cuda.current_stream()
+    ng = len(step.groups)
+
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    watch = ClockWatch(local)
+    watch.start()
+
+    # ---- (1) device-resident: W warm-ups, then EXACTLY K steps between two events
+    for _ in range(W):
+        step.launch_all()
+    barrier()
+    n0 = ob.opt_launch_count()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(stream)
+    for _ in range(K):
+        step.launch_all()
+    e1.record(stream)
+    barrier()
+    launches = ob.opt_launch_count() - n0
+    ms_total = e0.elapsed_time(e1)
+
+    # ---- (2) same K steps again with an event pair around every launch -> per-group durations
+    evs = [[(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(ng)]
+           for _ in range(K)]
+    for k in range(K):
+        for gi, g in enumerate(step.groups):
+            evs[k][gi][0].record(stream)
+            g.plan.launch()
+            evs[k][gi][1].record(stream)
+    barrier()
+    per_group_us = [float(np.mean([evs[k][gi][0].elapsed_time(evs[k][gi][1]) for k in range(K)])) * 1e3
+                    for gi in range(ng)]
+    per_group_min_us = [float(np.min([evs[k][gi][0].elapsed_time(evs[k][gi][1]) for k in range(K)])) * 1e3
+                        for gi in range(ng)]
+
+    # ---- (3) end to end through opt_plan_launch_host: pinned host -> device, kernel, device -> host
+    Ke = max(1, min(K, args.e2e_steps))
+    for _ in range(2):
+        step.launch_all_host()
+    barrier()
+    f0, f1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    f0.record(stream)
+    for _ in range(Ke):
+        step.launch_all_host()
+    f1.record(stream)
+    barrier()
+    ms_e2e = f0.elapsed_time(f1)
+
+    watch.stop_flag.set()
+    watch.join(timeout=2)
+
+    # max over ranks
+    if world > 1:
+        t = torch.tensor([ms_total, ms_e2e], device=device, dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms_total, ms_e2e = float(t[0]), float(t[1])
+
+    us_step = ms_total * 1e3 / K
+    us_e2e = ms_e2e * 1e3 / Ke
+
+    groups = {}
+    for g, us, usmin in zip(step.groups, per_group_us, per_group_min_us):
+        fl, by = g.info["flops"], g.info["bytes"]
+        gbs = by / (us * 1e-6) / 1e9
+        tfs = fl / (us * 1e-6) / 1e12
+        t_hbm = by / (peaks["hbm_gbs"] * 1e9) * 1e6
+        t_tc = fl / (peaks["bf16_tflops"] * 1e12) * 1e6
+        groups[g.name] = dict(latency_us=round(us, 2), latency_min_us=round(usmin, 2), launches=1, tiles=g.info["tiles"],
+                              algorithmic_bytes=by, flops=fl, gbs=round(gbs, 1), tflops=round(tfs, 1),
+                              frac_hbm=round(gbs / peaks["hbm_gbs"], 4),
+                              frac_tensor=round(tfs / peaks["bf16_tflops"], 4) if fl else None,
+                              roofline_us=round(max(t_hbm, t_tc), 2),
+                              frac_roofline=round(max(t_hbm, t_tc) / us, 4))
+
+    # dominant kernel of the step = the grouped GEMM (3 of the 6 launches); over a step it is HBM-bound
+    # (C4b/C4c at 85 and 52 flop/B; C2 sits on the ridge and is reported against tensor peak in "groups")
+    gemm = [(g, us) for g, us in zip(step.groups, per_group_us) if g.kind == "linear"]
+    gemm_bytes = sum(g.info["bytes"] for g, _ in gemm)
+    gemm_us = sum(us for _, us in gemm)
+    achieved = gemm_bytes / (gemm_us * 1e-6) / 1e9
+    roofline = dict(bound="hbm", kernel="grouped_gemm_sm100_kernel", achieved=round(achieved, 1), peak=peaks["hbm_gbs"],
+                    unit="GB/s", frac=round(achieved / peaks["hbm_gbs"], 4), traffic=None,
+                    peak_source=peaks["source"] + ", burst copy figure",
+                    launches_per_step=len(gemm), bytes_per_step=gemm_bytes, us_per_step=round(gemm_us, 2),
+                    share_of_step=round(gemm_us / sum(per_group_us), 4))
+    c2 = groups.get("C2_grouped_linear_tower")
+    roofline_tensor = None
+    if c2:
+        roofline_tensor = dict(bound="tensor", kernel="grouped_gemm_sm100_kernel", workload="C2", achieved=c2["tflops"],
+                               peak=peaks["bf16_tflops"], unit="TFLOP/s", frac=c2["frac_tensor"],
+                               frac_of_sustained=round(c2["tflops"] / peaks["bf16_tflops_sustained"], 4))
+
+    line = dict(metric="fused_op_group_step_latency", value=round(us_step, 2), unit="us", n_gpus=world, steps=K, warmup=W,
+                ms_per_step=round(us_step / 1e3, 5), higher_is_better=False, scaling="weak", vs_baseline=None,
+                dtype="bf16", data="synthetic",
+                config=dict(workload=WORKLOAD_NAME if not args.small else "SMALL (debug sizes) " + json.dumps(SMALL),
+                            parallelism="replicas x%d (no data-path collective)" % world,
+                            l2="inputs larger than L2: a step touches %.2f GB, every group's data was last touched one "
+                               "full step earlier" % (sum(g.info["bytes"] for g in step.groups) / 1e9),
+                            groups_per_step=ng),
+                e2e=dict(value=round(us_e2e, 2), unit="us", h2d_bytes_per_step=step.h2d_bytes(),
+                         d2h_bytes_per_step=step.d2h_bytes(), steps=Ke,
+                         api="opt_plan_launch_host (pinned host arenas; every input tensor H2D and every output D2H "
+                             "each step)"),
+                gpu_launches=int(launches), launches_per_step=ng,
+                clocks=watch.summary(), roofline=roofline, roofline_tensor=roofline_tensor, groups=groups,
+                aggregate=dict(steps_per_s=round(world / (us_step * 1e-6), 2)),
+                build_seconds=round(build_s, 1), lib=ob.opt_version())
+
+    if rank == 0 and not args.no_cpu and world >= 1:
+        us, spent, desc, cores = oracle_sample_step(1.0 if not args.small else 0.25)
+        line["cpu_baseline"] = dict(value=round(us, 1), unit="us", cores=cores, kind="oracle", sample=desc,
+                                    cpu_seconds=round(spent, 2))
+    if rank == 0:
+        print(json.dumps(line))
+    if world > 1:
+        dist.barrier()
+        dist.destroy_process_group()
+    return 0
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=30)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="product", choices=["product", "reference"])
+    ap.add_argument("--e2e-steps", type=int, default=5)
+    ap.add_argument("--small", action="store_true", help="debug sizes (not a bench number)")
+    ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+    return run_product(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

@@ -1,0 +1,116 @@
+"""CPU-only checks of the boundary: the C-ABI library builds for sm_100a, loads without a GPU,
+exports every symbol include/optimus_b200.h declares, and validates descriptors on the host
+before the first CUDA call (no compute here)."""
+import ctypes
+import os
+import re
+
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def ob():
+    import paper_2607_02945_b200 as ob
+    ob.lib()
+    return ob
+
+
+def declared_symbols():
+    src = open(os.path.join(ROOT, "include", "optimus_b200.h")).read()
+    src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
+    return sorted(set(re.findall(r"\b(opt_[a-z_]+)\s*\(", src)))
+
+
+def test_every_declared_symbol_is_exported(ob):
+    names = declared_symbols()
+    assert {"opt_linear_plan_create", "opt_layernorm_plan_create", "opt_pointwise_plan_create", "opt_plan_launch",
+            "opt_plan_launch_host", "opt_plan_info", "opt_plan_destroy", "opt_last_error", "opt_launch_count",
+            "opt_version"} <= set(names)
+    L = ctypes.CDLL(ob.lib_path())
+    for n in names:
+        assert hasattr(L, n), "symbol %s declared in the header but not exported" % n
+    # and the Python binding carries the same names
+    for n in names:
+        assert hasattr(ob, n), "binding lacks %s" % n
+
+
+def test_struct_layouts_match_header(ob):
+    assert ctypes.sizeof(ob.opt_linear_member) == 72
+    assert ctypes.sizeof(ob.opt_layernorm_member) == 64
+    assert ctypes.sizeof(ob.opt_chunk) == 48
+    assert ctypes.sizeof(ob.opt_host_copy) == 32
+
+
+def test_sass_is_blackwell_native():
+    """tcgen05.mma / tcgen05.ld / TMA show up as UTC*MMA / LDTM / UTMALDG+UTMASTG in the SASS."""
+    import shutil
+    import subprocess
+    import paper_2607_02945_b200 as ob
+    cuobjdump = shutil.which("cuobjdump") or "/usr/local/cuda/bin/cuobjdump"
+    if not os.path.exists(cuobjdump):
+        pytest.skip("cuobjdump not installed")
+    sass = subprocess.run([cuobjdump, "-sass", ob.lib_path()], capture_output=True, text=True).stdout
+    for mnemonic in ("UTCHMMA", "LDTM", "UTMALDG", "UTMASTG"):
+        assert mnemonic in sass, mnemonic
+    assert "sm_100a" in sass
+
+
+def dummy(addr):
+    return ctypes.c_void_p(addr)
+
+
+def test_host_validation_runs_before_any_cuda_call(ob):
+    """INVALID_ARG / ALIGNMENT / ALIAS come back on a machine without a GPU; a valid group then
+    fails with NO_DEVICE (never a CPU fallback)."""
+    import torch
+    A, B, Cc = 0x10000000, 0x20000000, 0x30000000
+    mk = lambda **kw: ob.opt_linear_member(**{**dict(x=A, ldx=64, w=B, ldw=64, bias=None, y=Cc, ldy=64, M=128, N=64, K=64, act=0), **kw})
+    for member, status in [(mk(K=60), ob.OPT_ERR_ALIGNMENT), (mk(x=A + 2), ob.OPT_ERR_ALIGNMENT),
+                           (mk(M=0), ob.OPT_ERR_INVALID_ARG), (mk(act=9), ob.OPT_ERR_INVALID_ARG),
+                           (mk(y=A), ob.OPT_ERR_ALIAS), (mk(ldy=32), ob.OPT_ERR_INVALID_ARG)]:
+        with pytest.raises(ob.OptError) as e:
+            ob.opt_linear_plan_create([member], ob.OPT_BF16)
+        assert e.value.status == status, (e.value, status)
+    with pytest.raises(ob.OptError) as e:     # two members writing overlapping concat slots
+        ob.opt_linear_plan_create([mk(y=Cc, ldy=128), mk(y=Cc + 64, ldy=128)], ob.OPT_BF16)
+    assert e.value.status == ob.OPT_ERR_ALIAS
+    # adjacent, non-overlapping slots pass the host checks:
+    if not torch.cuda.is_available():
+        with pytest.raises(ob.OptError) as e:
+            ob.opt_linear_plan_create([mk(y=Cc, ldy=128), mk(y=Cc + 128, ldy=128)], ob.OPT_BF16)
+        assert e.value.status == ob.OPT_ERR_NO_DEVICE
+        ln = ob.opt_layernorm_member(x=A, ldx=64, y=B, ldy=64, gamma=None, beta=None, rows=4, D=64, eps=1e-5)
+        with pytest.raises(ob.OptError) as e:
+            ob.opt_layernorm_plan_create([ln], ob.OPT_BF16)
+        assert e.value.status == ob.OPT_ERR_NO_DEVICE
+        ch = ob.opt_chunk(src=A, lds=64, dst=B, ldd=64, rows=4, width=64, op=0)
+        with pytest.raises(ob.OptError) as e:
+            ob.opt_pointwise_plan_create([ch], ob.OPT_BF16)
+        assert e.value.status == ob.OPT_ERR_NO_DEVICE
+    ln = ob.opt_layernorm_member(x=A, ldx=64, y=B, ldy=64, gamma=None, beta=None, rows=4, D=60, eps=1e-5)
+    with pytest.raises(ob.OptError) as e:
+        ob.opt_layernorm_plan_create([ln], ob.OPT_BF16)
+    assert e.value.status == ob.OPT_ERR_ALIGNMENT
+    ch = ob.opt_chunk(src=A, lds=64, dst=A + 64, ldd=64, rows=4, width=64, op=0)   # dst overlaps src rows
+    with pytest.raises(ob.OptError) as e:
+        ob.opt_pointwise_plan_create([ch], ob.OPT_BF16)
+    assert e.value.status == ob.OPT_ERR_ALIAS
+    assert ob.lib().opt_plan_launch(None, None) == ob.OPT_ERR_INVALID_ARG      # NULL plan: error, no launch
+    assert "NULL" in ob.opt_last_error()
+    assert ob.opt_launch_count() == 0
+
+
+def test_product_never_imports_the_oracle():
+    pkg = os.path.join(ROOT, "paper_2607_02945_b200")
+    for dirpath, _, files in os.walk(pkg):
+        for f in files:
+            if f.endswith((".py", ".cu", ".h", ".cpp")):
+                txt = open(os.path.join(dirpath, f)).read()
+                assert "import oracle" not in txt and "from oracle" not in txt and "optimus_oracle" not in txt, f
+    for f in os.listdir(os.path.join(ROOT, "oracle")):
+        if f.endswith((".py", ".cpp")):
+            txt = open(os.path.join(ROOT, "oracle", f)).read()
+            assert "import paper_2607_02945_b200" not in txt and "from paper_2607_02945_b200" not in txt, f
+            assert "csrc" not in txt and "optimus_b200.h" not in txt, f
