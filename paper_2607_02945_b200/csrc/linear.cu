@@ -12,10 +12,12 @@
 //                     tcgen05.mma.cta_group::1.kind::f16 (M=128, N=BN, K=16) four
 //                     times per stage into a TMEM accumulator, tcgen05.commit
 //                     releases the stage / publishes the accumulator;
-//         warps 2..5  epilogue: tcgen05.ld (32 lanes x 32 columns), + bias,
-//                     activation, RNE to bf16, swizzled st.shared, TMA store
-//                     (cp.async.bulk.tensor, 64x32 boxes) into the member's output
-//                     or its slot of the concatenated output.
+//         warps 2..9  epilogue, two warps per TMEM lane quadrant taking alternate
+//                     64-column chunks: tcgen05.ld (32 lanes x 32 columns), + bias
+//                     (fp32, broadcast from shared memory), activation (ReLU folded
+//                     into cvt.rn.relu.bf16x2), RNE to bf16, swizzled st.shared, TMA
+//                     store (cp.async.bulk.tensor, 64x32 boxes) into the member's
+//                     output or its slot of the concatenated output.
 //       TMEM holds two accumulator stages (2 x 256 columns) so the epilogue of
 //       tile t overlaps the MMAs of tile t+1.  The device-side tile scheduler
 //       decodes a linear tile id into (member, m-block, n-block) from the
@@ -111,14 +113,16 @@ constexpr int kMaxBN = 256;        // widest tile (UMMA N)
 constexpr int kStages = 4;
 constexpr int kAccStages = 2;
 constexpr int kTmemCols = 512;     // 2 accumulator stages x 256 fp32 columns
-constexpr int kGemmThreads = 192;  // warp 0 TMA, warp 1 MMA, warps 2..5 epilogue
+constexpr int kEpiWarps = 8;       // two per TMEM lane quadrant, alternating 64-column chunks
+constexpr int kGemmThreads = 64 + 32 * kEpiWarps;   // warp 0 TMA, warp 1 MMA, warps 2..9 epilogue
 constexpr int kABytes = kBM * kBK * 2;          // 16 KB
 constexpr int kBBytesMax = kMaxBN * kBK * 2;    // 32 KB
 constexpr int kStageBytes = kABytes + kBBytesMax;
 constexpr int kEpiBufBytes = 32 * 128;          // one warp's 32 rows x 64 bf16 staging tile
-constexpr int kEpiBufs = 2;                     // per warp
-constexpr int kSmemBar = kStages * kStageBytes + 4 * kEpiBufs * kEpiBufBytes;
-constexpr int kSmemBytes = kSmemBar + 256 + 1024;   // barriers + slack for 1024-byte alignment
+constexpr int kSmemEpi = kStages * kStageBytes;
+constexpr int kSmemBias = kSmemEpi + kEpiWarps * kEpiBufBytes;    // per warp 64 fp32 bias values
+constexpr int kSmemBar = kSmemBias + kEpiWarps * 64 * 4;
+constexpr int kSmemBytes = kSmemBar + 256;      // barriers; the dynamic smem base is 1024-byte aligned (checked)
 
 struct alignas(128) GemmMember {
   CUtensorMap tmA;       // X [M,K]   box {64, 128}   load
@@ -209,18 +213,64 @@ __device__ __forceinline__ uint64_t umma_desc_sw128(uint32_t saddr) {
   return (uint64_t)((saddr & 0x3FFFFu) >> 4) | ((uint64_t)(1024 >> 4) << 32) | (1ull << 46) | (2ull << 61);
 }
 
-__device__ __forceinline__ float bias_at(const uint4* bv, int i) {   // i-th bf16 of an 8-vector array
-  const uint32_t u = reinterpret_cast<const uint32_t*>(bv)[i >> 1];
-  return (i & 1) ? bf16_hi(u) : bf16_lo(u);
+// round two fp32 to a packed bf16x2 (lo in the low half) with the ReLU folded into the conversion:
+// negative -> +0, NaN -> NaN (torch relu semantics, Q13)
+__device__ __forceinline__ uint32_t pack_relu_bf16x2(float lo, float hi) {
+  uint32_t d;
+  asm("cvt.rn.relu.bf16x2.f32 %0, %1, %2;" : "=r"(d) : "f"(hi), "f"(lo));
+  return d;
+}
+
+// Persistent tile walk of one warp role: tile ids blockIdx.x, +gridDim.x, ...; the member index only
+// moves forward, so it is advanced incrementally over the prefix sums.
+struct TileWalk {
+  const int32_t* __restrict__ starts;
+  int n_members, mi, next_start;
+  __device__ __forceinline__ TileWalk(const int32_t* st, int n) : starts(st), n_members(n), mi(0) {
+    next_start = __ldg(st + 1);
+  }
+  // -> member index of `tile`; local = tile - starts[mi]
+  __device__ __forceinline__ int seek(int tile, int* local) {
+    while (tile >= next_start) { ++mi; next_start = __ldg(starts + mi + 1); }
+    *local = tile - __ldg(starts + mi);
+    return mi;
+  }
+};
+
+// Epilogue of one 32-row x 64-column chunk held in v[64] (this thread: one row): + bias (fp32, broadcast
+// from shared memory), activation, RNE to bf16, 128-byte-swizzled st.shared of the row.
+template <int ACT>
+__device__ __forceinline__ void epi_chunk(const uint32_t (&v)[64], const float* bias_s, uint32_t srow, int lane) {
+#pragma unroll
+  for (int j = 0; j < 8; ++j) {          // 8 columns -> one 16-byte chunk, 128B-swizzled position
+    const float4 b0 = *reinterpret_cast<const float4*>(bias_s + 8 * j);
+    const float4 b1 = *reinterpret_cast<const float4*>(bias_s + 8 * j + 4);
+    const float x0 = __uint_as_float(v[8 * j + 0]) + b0.x, x1 = __uint_as_float(v[8 * j + 1]) + b0.y;
+    const float x2 = __uint_as_float(v[8 * j + 2]) + b0.z, x3 = __uint_as_float(v[8 * j + 3]) + b0.w;
+    const float x4 = __uint_as_float(v[8 * j + 4]) + b1.x, x5 = __uint_as_float(v[8 * j + 5]) + b1.y;
+    const float x6 = __uint_as_float(v[8 * j + 6]) + b1.z, x7 = __uint_as_float(v[8 * j + 7]) + b1.w;
+    uint32_t p0, p1, p2, p3;
+    if (ACT == OPT_ACT_RELU) {
+      p0 = pack_relu_bf16x2(x0, x1); p1 = pack_relu_bf16x2(x2, x3);
+      p2 = pack_relu_bf16x2(x4, x5); p3 = pack_relu_bf16x2(x6, x7);
+    } else {
+      p0 = pack_bf16x2(act_f32<true>(x0, ACT), act_f32<true>(x1, ACT));
+      p1 = pack_bf16x2(act_f32<true>(x2, ACT), act_f32<true>(x3, ACT));
+      p2 = pack_bf16x2(act_f32<true>(x4, ACT), act_f32<true>(x5, ACT));
+      p3 = pack_bf16x2(act_f32<true>(x6, ACT), act_f32<true>(x7, ACT));
+    }
+    asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};"
+                 ::"r"(srow + ((j ^ (lane & 7)) << 4)), "r"(p0), "r"(p1), "r"(p2), "r"(p3) : "memory");
+  }
 }
 
 __global__ void __launch_bounds__(kGemmThreads, 1)
 grouped_gemm_sm100_kernel(const GemmMember* __restrict__ members, const int32_t* __restrict__ starts,
                           int n_members, int total_tiles) {
-  extern __shared__ uint8_t smem_raw[];
-  uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
+  extern __shared__ __align__(1024) uint8_t smem[];
   const uint32_t sbase = smem_u32(smem);
-  const uint32_t epi_base = sbase + kStages * kStageBytes;
+  if ((sbase & 1023u) != 0) __trap();            // 128-byte-swizzle tiles need 1024-byte alignment
+  const uint32_t epi_base = sbase + kSmemEpi;
   const uint32_t bar_base = sbase + kSmemBar;
   // barrier layout (8 bytes each): full[kStages], empty[kStages], tmem_full[2], tmem_empty[2], then tmem ptr
   auto full_bar = [&](int s) { return bar_base + 8u * s; };
@@ -233,7 +283,7 @@ grouped_gemm_sm100_kernel(const GemmMember* __restrict__ members, const int32_t*
 
   if (warp == 0 && lane == 0) {
     for (int s = 0; s < kStages; ++s) { mbar_init(full_bar(s), 1); mbar_init(empty_bar(s), 1); }
-    for (int s = 0; s < kAccStages; ++s) { mbar_init(tfull_bar(s), 1); mbar_init(tempty_bar(s), 4); }
+    for (int s = 0; s < kAccStages; ++s) { mbar_init(tfull_bar(s), 1); mbar_init(tempty_bar(s), kEpiWarps); }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     fence_proxy_async_smem();
   }
@@ -251,10 +301,10 @@ grouped_gemm_sm100_kernel(const GemmMember* __restrict__ members, const int32_t*
     // ------------------------------------------------------- TMA producer ----
     if (lane == 0) {
       int stage = 0; uint32_t phase = 0;
+      TileWalk walk(starts, n_members);
       for (int tile = blockIdx.x; tile < total_tiles; tile += gridDim.x) {
-        const int mi = find_member(starts, n_members, tile);
-        const GemmMember* m = members + mi;
-        const int local = tile - __ldg(starts + mi);
+        int local;
+        const GemmMember* m = members + walk.seek(tile, &local);
         const int nbn = m->nbn, nkb = m->nkb, bn = m->bn;
         const int m0 = (local / nbn) * kBM, n0 = (local % nbn) * bn;
         const uint32_t tx_bytes = kABytes + m->b_bytes;
@@ -273,9 +323,10 @@ grouped_gemm_sm100_kernel(const GemmMember* __restrict__ members, const int32_t*
     if (lane == 0) {
       int stage = 0; uint32_t phase = 0;
       int as = 0; uint32_t aphase = 0;
+      TileWalk walk(starts, n_members);
       for (int tile = blockIdx.x; tile < total_tiles; tile += gridDim.x) {
-        const int mi = find_member(starts, n_members, tile);
-        const GemmMember* m = members + mi;
+        int local;
+        const GemmMember* m = members + walk.seek(tile, &local);
         const int nkb = m->nkb, K = m->K;
         const uint32_t idesc = m->idesc;
         mbar_wait(tempty_bar(as), aphase ^ 1);      // epilogue has drained this accumulator stage
@@ -299,52 +350,47 @@ grouped_gemm_sm100_kernel(const GemmMember* __restrict__ members, const int32_t*
   } else {
     // ----------------------------------------------------------- epilogue ----
     const int quad = warp & 3;               // TMEM lane quadrant this warp may read
-    const uint32_t my_epi = epi_base + (uint32_t)(warp - 2) * kEpiBufs * kEpiBufBytes;
+    const int half = (warp - 2) >> 2;        // 0: even 64-column chunks, 1: odd ones
+    const uint32_t sbuf = epi_base + (uint32_t)(warp - 2) * kEpiBufBytes;
+    const uint32_t srow = sbuf + lane * 128;
+    float* bias_s = reinterpret_cast<float*>(smem + kSmemBias) + (warp - 2) * 64;
     int as = 0; uint32_t aphase = 0;
-    int buf = 0;
+    TileWalk walk(starts, n_members);
     for (int tile = blockIdx.x; tile < total_tiles; tile += gridDim.x) {
-      const int mi = find_member(starts, n_members, tile);
-      const GemmMember* m = members + mi;
-      const int local = tile - __ldg(starts + mi);
+      int local;
+      const GemmMember* m = members + walk.seek(tile, &local);
       const int nbn = m->nbn, bn = m->bn, N = m->N, act = m->act;
       const int m0 = (local / nbn) * kBM, n0 = (local % nbn) * bn;
-      const uint4* bias = reinterpret_cast<const uint4*>(m->bias);
+      const uint32_t* bias = reinterpret_cast<const uint32_t*>(m->bias);   // bf16 pairs
       mbar_wait(tfull_bar(as), aphase);
       tc_fence_after();
       const uint32_t t_row = tmem_base + ((uint32_t)(quad * 32) << 16) + as * kMaxBN;
       const int nchunks = (bn + 63) >> 6;
-      for (int c = 0; c < nchunks; ++c) {
+      bool released = false;
+      for (int c = half; c < nchunks; c += 2) {
         uint32_t v[64];
         tc_ld_32x32(t_row + c * 64, *reinterpret_cast<uint32_t(*)[32]>(&v[0]));
         tc_ld_32x32(t_row + c * 64 + 32, *reinterpret_cast<uint32_t(*)[32]>(&v[32]));
-        // bias for the 64 columns of this chunk (warp-uniform addresses -> broadcast loads)
+        // bias of the chunk's 64 columns -> fp32 in shared memory (lane l owns columns 2l, 2l+1)
         const int col0 = n0 + c * 64;
-        uint4 bv[8];
-#pragma unroll
-        for (int j = 0; j < 8; ++j)
-          bv[j] = (bias != nullptr && col0 + j * 8 < N) ? __ldg(bias + ((col0 + j * 8) >> 3)) : make_uint4(0, 0, 0, 0);
+        const int bc = col0 + 2 * lane;
+        const uint32_t bb = (bias != nullptr && bc < N) ? __ldg(bias + (bc >> 1)) : 0u;
+        *reinterpret_cast<float2*>(bias_s + 2 * lane) = make_float2(bf16_lo(bb), bf16_hi(bb));
         tc_wait_ld();
-        if (c == nchunks - 1) {              // accumulator fully in registers: hand the TMEM stage back
+        if (c + 2 >= nchunks) {              // this warp's part of the accumulator is in registers
           tc_fence_before();
           __syncwarp();
           if (lane == 0) mbar_arrive(tempty_bar(as));
+          released = true;
         }
-        // staging buffer free? (the TMA store issued two chunks ago has read it)
-        if (lane == 0) tma_store_wait_read<kEpiBufs - 1>();
-        __syncwarp();
-        const uint32_t sbuf = my_epi + buf * kEpiBufBytes;
-        const uint32_t srow = sbuf + lane * 128;
-#pragma unroll
-        for (int j = 0; j < 8; ++j) {        // 8 columns -> one 16-byte chunk, 128B-swizzled position
-          uint32_t pk[4];
-#pragma unroll
-          for (int e = 0; e < 4; ++e) {
-            float lo = __uint_as_float(v[j * 8 + 2 * e]) + bias_at(&bv[j], 2 * e);
-            float hi = __uint_as_float(v[j * 8 + 2 * e + 1]) + bias_at(&bv[j], 2 * e + 1);
-            pk[e] = pack_bf16x2(act_f32<true>(lo, act), act_f32<true>(hi, act));
-          }
-          asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};"
-                       ::"r"(srow + ((j ^ (lane & 7)) << 4)), "r"(pk[0]), "r"(pk[1]), "r"(pk[2]), "r"(pk[3]) : "memory");
+        // staging buffer free? (the previous TMA store of this warp has read it)
+        if (lane == 0) tma_store_wait_read<0>();
+        __syncwarp();                        // also publishes bias_s to the warp
+        switch (act) {
+          case OPT_ACT_RELU: epi_chunk<OPT_ACT_RELU>(v, bias_s, srow, lane); break;
+          case OPT_ACT_NONE: epi_chunk<OPT_ACT_NONE>(v, bias_s, srow, lane); break;
+          case OPT_ACT_TANH: epi_chunk<OPT_ACT_TANH>(v, bias_s, srow, lane); break;
+          default:           epi_chunk<OPT_ACT_SIGMOID>(v, bias_s, srow, lane); break;
         }
         fence_proxy_async_smem();
         __syncwarp();
@@ -352,7 +398,11 @@ grouped_gemm_sm100_kernel(const GemmMember* __restrict__ members, const int32_t*
           tma_store_2d(&m->tmY, sbuf, col0, m0 + quad * 32);
           tma_store_commit();
         }
-        buf ^= 1;
+      }
+      if (!released) {                       // no chunk for this warp in a narrow tile: still hand the stage back
+        tc_fence_before();
+        __syncwarp();
+        if (lane == 0) mbar_arrive(tempty_bar(as));
       }
       if (++as == kAccStages) { as = 0; aphase ^= 1; }
     }
