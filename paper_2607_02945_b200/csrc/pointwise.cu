@@ -17,7 +17,16 @@
 //     memory, no intermediate tensor.
 //   * dense tensors are re-tiled to [rows', 256 vectors] so the same path
 //     covers the standalone multi-tensor form with a 2 KB map.
+//   * STAGED mode, for groups made of many narrow column slices of one source
+//     row span (the split->f->cat residue, configs[3]: 64-byte segments): a block
+//     owns a tile of whole rows; one thread pulls the rows' source span into
+//     shared memory with cp.async.bulk (TMA, full-line coalesced reads), threads
+//     gather their vector from shared memory in op-sorted order, apply the op,
+//     scatter it to the destination position in a second shared buffer, and the
+//     rows leave with cp.async.bulk stores (full-line writes).  All the
+//     scatter/gather happens on chip; HBM sees two streaming copies.
 #include <algorithm>
+#include <cstdlib>
 #include <map>
 #include <tuple>
 
@@ -32,6 +41,10 @@ struct PwGroup {
   int32_t rows, W;        // rows; vectors per virtual row
   int32_t map_off;        // first map entry of this group
   int32_t tx_log2;        // log2(threads along the virtual row)
+  int32_t src_span;       // STAGED mode: vectors of one source row staged in smem (0 = direct mode)
+  int32_t dst_span;       // STAGED mode: vectors of one destination row staged for a bulk store (0 = direct stores)
+  int32_t tile_rows;      // STAGED mode: rows per block
+  int32_t pad;
 };
 struct PwBlock { int32_t group, q0, r0, nrows; };
 
@@ -39,6 +52,9 @@ constexpr int kPwThreads = 256;
 constexpr int kPwUnroll = 8;
 constexpr int kFlatW = 256;          // vectors per row when a dense tensor is re-tiled
 constexpr int kVecPerBlock = 4096;   // ~64 KB read + 64 KB written per block
+constexpr int kStageBudget = 32 * 1024;   // STAGED mode: shared memory per block (source + destination rows)
+constexpr int kStageMaxSpan = 2048;       // STAGED mode: at most 32 KB per staged row
+constexpr int kStageMaxAvgChunk = 32;     // STAGED mode only when the average segment is < 512 bytes
 
 template <bool BF16, int OP>
 __device__ __forceinline__ int4 pw_apply(int4 v) {
@@ -76,12 +92,82 @@ __device__ __forceinline__ void pw_rows(const int4* __restrict__ s, int4* __rest
   for (; r < rend; r += ty_step) __stcs(d + (int64_t)r * ldd, pw_apply<BF16, OP>(__ldcs(s + (int64_t)r * lds)));
 }
 
+__device__ __forceinline__ uint32_t pw_smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+// STAGED mode: rows [r0, r0+nrows) of group g.  smem = nrows x src_span (+ nrows x dst_span) vectors.
+template <bool BF16, int OP>
+__device__ __forceinline__ void pw_staged_cols(const int4* sin, int4* sout, int4* gdst, const int2 m, int nrows,
+                                               int src_span, int dst_span, int64_t ldd16) {
+  const int so = m.x, dof = m.y & 0x3FFFFFFF;
+  if (sout != nullptr) {
+    for (int r = 0; r < nrows; ++r) sout[r * dst_span + dof] = pw_apply<BF16, OP>(sin[r * src_span + so]);
+  } else {
+    for (int r = 0; r < nrows; ++r) __stcs(gdst + (int64_t)r * ldd16 + dof, pw_apply<BF16, OP>(sin[r * src_span + so]));
+  }
+}
+
 template <bool BF16>
-__global__ void __launch_bounds__(kPwThreads)
+__device__ __forceinline__ void pw_staged_tile(const PwGroup& g, const int2* __restrict__ vmap, int r0, int nrows) {
+  extern __shared__ __align__(128) uint8_t pw_smem[];
+  __shared__ __align__(8) uint64_t bar_storage;
+  const uint32_t bar = pw_smem_u32(&bar_storage);
+  int4* sin = reinterpret_cast<int4*>(pw_smem);
+  int4* sout = g.dst_span ? sin + (size_t)g.tile_rows * g.src_span : nullptr;
+  const uint32_t row_bytes = (uint32_t)g.src_span * 16u;
+  if (threadIdx.x == 0) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(bar));
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(row_bytes * (uint32_t)nrows) : "memory");
+    for (int r = 0; r < nrows; ++r)
+      asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                   ::"r"(pw_smem_u32(sin + (size_t)r * g.src_span)),
+                     "l"(g.src + ((int64_t)(r0 + r) * g.lds16) * 16), "r"(row_bytes), "r"(bar) : "memory");
+  }
+  __syncthreads();                       // barrier initialised before anyone polls it
+  {
+    uint32_t done = 0;
+    while (!done)
+      asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], 0;\n\tselp.u32 %0, 1, 0, p;\n\t}"
+                   : "=r"(done) : "r"(bar) : "memory");
+  }
+  int4* gdst = reinterpret_cast<int4*>(g.dst) + (int64_t)r0 * g.ldd16;
+  for (int q = threadIdx.x; q < g.W; q += kPwThreads) {
+    const int2 m = __ldg(vmap + g.map_off + q);
+    switch ((int)((uint32_t)m.y >> 30)) {   // warp-uniform except at op boundaries of the virtual row
+      case OPT_PW_COPY: pw_staged_cols<BF16, OPT_PW_COPY>(sin, sout, gdst, m, nrows, g.src_span, g.dst_span, g.ldd16); break;
+      case OPT_PW_RELU: pw_staged_cols<BF16, OPT_PW_RELU>(sin, sout, gdst, m, nrows, g.src_span, g.dst_span, g.ldd16); break;
+      case OPT_PW_TANH: pw_staged_cols<BF16, OPT_PW_TANH>(sin, sout, gdst, m, nrows, g.src_span, g.dst_span, g.ldd16); break;
+      default:          pw_staged_cols<BF16, OPT_PW_SIGMOID>(sin, sout, gdst, m, nrows, g.src_span, g.dst_span, g.ldd16); break;
+    }
+  }
+  if (sout != nullptr) {
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // st.shared results -> visible to the bulk-copy engine
+    __syncthreads();
+    if (threadIdx.x == 0) {
+      const uint32_t out_bytes = (uint32_t)g.dst_span * 16u;
+      for (int r = 0; r < nrows; ++r)
+        asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;"
+                     ::"l"(g.dst + ((int64_t)(r0 + r) * g.ldd16) * 16), "r"(pw_smem_u32(sout + (size_t)r * g.dst_span)),
+                       "r"(out_bytes) : "memory");
+      asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+      asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");   // smem must outlive the reads of the store
+    }
+  }
+}
+
+#ifndef PW_MINBLOCKS
+#define PW_MINBLOCKS 6
+#endif
+template <bool BF16>
+__global__ void __launch_bounds__(kPwThreads, PW_MINBLOCKS)
 multi_pointwise_splitcat_kernel(const PwGroup* __restrict__ groups, const int2* __restrict__ vmap,
                                 const PwBlock* __restrict__ blocks) {
   const PwBlock b = blocks[blockIdx.x];
   const PwGroup g = groups[b.group];
+  if (g.src_span) {                       // block-uniform
+    pw_staged_tile<BF16>(g, vmap, b.r0, b.nrows);
+    return;
+  }
   const int tx = threadIdx.x & ((1 << g.tx_log2) - 1);
   const int ty = threadIdx.x >> g.tx_log2;
   const int ty_step = kPwThreads >> g.tx_log2;
@@ -106,9 +192,9 @@ cudaError_t launch_pointwise(const opt_plan* p, cudaStream_t s) {
   auto* vmap = reinterpret_cast<const int2*>(base + p->off1);
   auto* blocks = reinterpret_cast<const PwBlock*>(base + p->off2);
   if (p->io == OPT_BF16)
-    multi_pointwise_splitcat_kernel<true><<<p->grid, p->block, 0, s>>>(groups, vmap, blocks);
+    multi_pointwise_splitcat_kernel<true><<<p->grid, p->block, p->smem, s>>>(groups, vmap, blocks);
   else
-    multi_pointwise_splitcat_kernel<false><<<p->grid, p->block, 0, s>>>(groups, vmap, blocks);
+    multi_pointwise_splitcat_kernel<false><<<p->grid, p->block, p->smem, s>>>(groups, vmap, blocks);
   return cudaGetLastError();
 }
 
@@ -178,6 +264,9 @@ extern "C" opt_status opt_pointwise_plan_create(const opt_chunk* chunks, int32_t
   std::vector<PwGroup> groups;
   std::vector<int2> vmap;
   std::vector<PwBlock> blocks;
+  size_t smem_needed = 0;
+  int64_t stage_budget = kStageBudget;                       // experiment knob: OPT_PW_STAGE_KB=<KB per block>, 0 = direct mode only
+  if (const char* e = getenv("OPT_PW_STAGE_KB")) stage_budget = std::min<int64_t>(200, std::max<int64_t>(0, atol(e))) * 1024;
   for (auto& kv : buckets) {
     std::vector<int>& ids = kv.second;
     std::sort(ids.begin(), ids.end(), [&](int a, int b) { return cc[a].dst < cc[b].dst; });
@@ -207,18 +296,41 @@ extern "C" opt_status opt_pointwise_plan_create(const opt_chunk* chunks, int32_t
       int txl = 0;
       while ((1 << txl) < W && txl < 8) ++txl;
       g.tx_log2 = txl;
+      g.src_span = g.dst_span = g.tile_rows = g.pad = 0;
       // map entries, sorted by (op, dst)
       std::vector<int> order(ids.begin() + i0, ids.begin() + i1);
       std::stable_sort(order.begin(), order.end(), [&](int a, int b) { return cc[a].op < cc[b].op; });
+      char* dmax = dmin;
+      bool self_inplace = false;
       for (int id : order) {
         const CChunk& c = cc[id];
         const int64_t so = (c.src - smin) / 16, dof = (c.dst - dmin) / 16;
+        dmax = std::max(dmax, c.dst + (int64_t)c.wv * 16);
+        self_inplace |= (c.src == c.dst);
         for (int32_t v = 0; v < c.wv; ++v) {
           int2 e;
           e.x = (int32_t)(so + v);
           e.y = (int32_t)((uint32_t)(dof + v) | ((uint32_t)c.op << 30));
           vmap.push_back(e);
         }
+      }
+      // STAGED mode: many narrow slices of one compact source row span (split -> f -> cat residue)
+      const int64_t sspan = (smax - smin) / 16, dspan = (dmax - dmin) / 16;
+      const int64_t nch = (int64_t)(i1 - i0);
+      const bool rows_disjoint = g.rows == 1 || (sspan <= g.lds16 && dspan <= g.ldd16);
+      if (stage_budget > 0 && nch > 1 && W < nch * kStageMaxAvgChunk && rows_disjoint && sspan <= kStageMaxSpan && sspan <= W + W / 4) {
+        g.src_span = (int32_t)sspan;
+        // rows leave through a bulk store only if the chunks tile the destination span without holes
+        // (otherwise the store would clobber bytes the group does not own) and nothing is in place
+        if (dspan == W && dspan <= kStageMaxSpan && !self_inplace && !getenv("OPT_PW_NO_SOUT")) g.dst_span = (int32_t)dspan;
+        const int64_t per_row = (int64_t)(g.src_span + g.dst_span) * 16;
+        g.tile_rows = (int32_t)std::max<int64_t>(1, std::min<int64_t>(stage_budget / per_row, g.rows));
+        smem_needed = std::max<size_t>(smem_needed, (size_t)g.tile_rows * per_row);
+        for (int64_t r0 = 0; r0 < g.rows; r0 += g.tile_rows)
+          blocks.push_back({(int32_t)groups.size(), 0, (int32_t)r0, (int32_t)std::min<int64_t>(g.tile_rows, g.rows - r0)});
+        groups.push_back(g);
+        i0 = i1;
+        continue;
       }
       // work items
       const int TX = 1 << txl, TY = kPwThreads / TX;
@@ -249,6 +361,16 @@ extern "C" opt_status opt_pointwise_plan_create(const opt_chunk* chunks, int32_t
   memcpy(blob.data() + p->off1, vmap.data(), vmap.size() * sizeof(int2));
   memcpy(blob.data() + p->off2, blocks.data(), blocks.size() * sizeof(PwBlock));
   if (opt_status st = upload_tables(p, blob.data(), total)) { delete p; return st; }
+  if (smem_needed > 48 * 1024) {
+    cudaError_t e = io == OPT_BF16
+        ? cudaFuncSetAttribute(multi_pointwise_splitcat_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_needed)
+        : cudaFuncSetAttribute(multi_pointwise_splitcat_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_needed);
+    if (e != cudaSuccess) {
+      cudaFree(p->dev_tables); delete p;
+      return fail(OPT_ERR_CUDA, "cudaFuncSetAttribute(max dynamic smem %zu) failed: %s", smem_needed, cudaGetErrorString(e));
+    }
+  }
+  p->smem = smem_needed;
   p->grid = dim3((unsigned)blocks.size());
   p->block = dim3(kPwThreads);
   p->total_tiles = (int32_t)blocks.size();
