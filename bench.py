@@ -335,6 +335,8 @@ def run_reference(args):
         return 0
     K, W = args.steps, args.warmup
     frac = min(1.0, (100.0 / max(1, K + W)) / 8.0)          # whole run ~100 s of CPU work
+    if args.ref_frac:
+        frac = args.ref_frac
     vals, spent_all, desc, cores = [], 0.0, "", 0
     for i in range(W + K):
         us, spent, desc, cores = oracle_sample_step(frac)
@@ -356,6 +358,23 @@ def run_reference(args):
 WORKLOAD_NAME = ("whole hot path = fused groups of BASELINE.json configs[1..4] back to back: C1 batched LN x64, "
                  "C2 grouped Linear+ReLU x128 (M=4096, concat), C3 split-pointwise-cat 8192x8192/256 chunks, "
                  "C4 recsys block x512 (LN -> Linear+ReLU -> Linear, concat [8192,32768]); 6 launches/step")
+
+
+def max_over_ranks(values, world, device):
+    """Timing rule: a multi-rank number is the MAX over ranks (replicas only).
+    One all_reduce(MAX) on whatever backend the process group has (nccl on GPUs, gloo in the CPU test)."""
+    if world <= 1:
+        return [float(v) for v in values]
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([float(v) for v in values], device=device, dtype=torch.float64)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return [float(v) for v in t.tolist()]
+
+
+def aggregate_steps_per_s(us_step, world):
+    """whole-job throughput of `world` independent replicas whose slowest rank needs us_step per step."""
+    return world / (us_step * 1e-6)
 
 
 # -------------------------------------------------------------- product arm --
@@ -435,10 +454,7 @@ def run_product(args):
     watch.join(timeout=2)
 
     # max over ranks
-    if world > 1:
-        t = torch.tensor([ms_total, ms_e2e], device=device, dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms_total, ms_e2e = float(t[0]), float(t[1])
+    ms_total, ms_e2e = max_over_ranks([ms_total, ms_e2e], world, device)
 
     us_step = ms_total * 1e3 / K
     us_e2e = ms_e2e * 1e3 / Ke
@@ -489,7 +505,7 @@ def run_product(args):
                              "each step)"),
                 gpu_launches=int(launches), launches_per_step=ng,
                 clocks=watch.summary(), roofline=roofline, roofline_tensor=roofline_tensor, groups=groups,
-                aggregate=dict(steps_per_s=round(world / (us_step * 1e-6), 2)),
+                aggregate=dict(steps_per_s=round(aggregate_steps_per_s(us_step, world), 2)),
                 build_seconds=round(build_s, 1), lib=ob.opt_version())
 
     if rank == 0 and not args.no_cpu and world >= 1:
@@ -513,6 +529,7 @@ def main():
     ap.add_argument("--e2e-steps", type=int, default=5)
     ap.add_argument("--small", action="store_true", help="debug sizes (not a bench number)")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
+    ap.add_argument("--ref-frac", type=float, default=0.0, help="reference arm: override the row-sample fraction")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)

@@ -1,0 +1,135 @@
+"""GPU parity at BASELINE.json's FULL sizes, in the launch configuration bench.py times.
+
+The step is built by bench.Step (same arenas, same plans, same six launches).  The oracle cannot
+finish the full groups in seconds, so it computes SAMPLED rows (all members, all columns of the
+sampled rows -- every op of the path is row-independent): first/last rows, rows around every
+128-row tile boundary class, and seeded random rows.  C3's data movement is checked on the whole
+[8192, 8192] tensor bit for bit (numpy fancy indexing of the oracle's column map).
+
+C4 (reading Q3): every group is gated against the oracle fed with the GPU's actual bf16
+input of that group.
+"""
+import numpy as np
+import pytest
+import torch
+
+import oracle
+from oracle import graphs
+import workloads as wl
+from util import BF16, bf16_ulp_distance, row_l2_rel_err, to_host, values64
+
+pytestmark = pytest.mark.gpu
+
+TOL_BF16 = 1e-2
+
+
+def sample_rows(n_rows, k, seed):
+    fixed = [0, 1, 127, 128, 129, n_rows // 2 - 1, n_rows // 2, n_rows - 129, n_rows - 128, n_rows - 2, n_rows - 1]
+    rng = np.random.default_rng(seed)
+    rows = set(r for r in fixed if 0 <= r < n_rows)
+    rows.update(int(r) for r in rng.integers(0, n_rows, size=k))
+    return np.array(sorted(rows))
+
+
+@pytest.fixture(scope="module")
+def step():
+    import bench
+    s = bench.Step("cuda:0", bench.FULL, pinned_host=False)
+    import paper_2607_02945_b200 as ob
+    n0 = ob.opt_launch_count()
+    s.launch_all()
+    torch.cuda.synchronize()
+    assert ob.opt_launch_count() - n0 == 6, "one launch per group"
+    return {g.name: g for g in s.groups}
+
+
+def ln_check(got, x, gamma, beta, eps):
+    y64, xh = oracle.layernorm(x, gamma, beta, eps, BF16, BF16, return_xhat=True)
+    ref = oracle.round_to_storage(y64, BF16)
+    d = bf16_ulp_distance(got, ref)
+    slack = 2.0 ** -16 * (np.abs(xh * values64(gamma, BF16)) + np.abs(values64(beta, BF16)))
+    bad = (d > 2) & ~(np.abs(values64(got, BF16) - y64) <= slack)
+    assert not bad.any(), "LN mismatch: max ulp %d" % d.max()
+    return int((d > 2).sum()), d.size
+
+
+def test_c1_full_layernorm(step):
+    g = step["C1_batched_layernorm"]
+    esc = tot = 0
+    for i, ((ix, ig, ib, iy), m) in enumerate(zip(g.idx, g.cfg["members"])):
+        rows = sample_rows(m["rows"], 24, 1000 + i)
+        got = to_host(g.aout.tensor(iy)[torch.from_numpy(rows).cuda()])
+        e, t = ln_check(got, np.ascontiguousarray(m["x"][rows]), m["gamma"], m["beta"], m["eps"])
+        esc, tot = esc + e, tot + t
+    assert esc < 1e-3 * tot
+
+
+def test_c2_full_grouped_linear(step):
+    g = step["C2_grouped_linear_tower"]
+    ycat = g.aout.tensor(g.iy)
+    worst = 0.0
+    for i, m in enumerate(g.cfg["members"]):
+        rows = sample_rows(m["M"], 12, 2000 + i)
+        got = to_host(ycat[torch.from_numpy(rows).cuda(), m["col_off"]:m["col_off"] + m["N"]])
+        sub = dict(m, x=np.ascontiguousarray(m["x"][rows]))
+        z64 = graphs.linear_member(sub, BF16)
+        worst = max(worst, row_l2_rel_err(got, z64, BF16))
+        assert np.percentile(bf16_ulp_distance(got, oracle.round_to_storage(z64, BF16)), 99) <= 1
+    assert worst <= TOL_BF16, worst
+
+
+def test_c3_full_split_pointwise_cat(step):
+    g = step["C3_split_pointwise_cat"]
+    cfg = g.cfg
+    out = to_host(g.aout.tensor(g.iy))
+    x, widths, ops, perm = cfg["x"], cfg["widths"], cfg["ops"], cfg["perm"]
+    rows = sample_rows(cfg["rows"], 200, 3000)
+    _, ref = graphs.split_pointwise_cat(np.ascontiguousarray(x[rows]), widths, ops, perm, BF16)
+    d = bf16_ulp_distance(out[rows], ref)
+    assert d.max() <= 2, "max ulp %d" % d.max()
+    # whole tensor: ReLU chunks are pure movement for positive inputs -> bit-exact everywhere;
+    # every other column must at least be finite and in the op's range
+    starts = np.concatenate(([0], np.cumsum(widths)))
+    dpos = 0
+    for p in perm:
+        w = widths[p]
+        src = x[:, starts[p]:starts[p] + w]
+        dst = out[:, dpos:dpos + w]
+        if ops[p] == wl.gen.PW_RELU:
+            pos = (src & 0x8000) == 0
+            assert np.array_equal(dst[pos], src[pos])
+            assert np.all(dst[~pos & ((src & 0x7FFF) <= 0x7F80)] == 0)
+        else:
+            v = values64(dst, BF16)
+            lo = -1.0 if ops[p] == wl.gen.PW_TANH else 0.0
+            assert np.all((v >= lo) & (v <= 1.0))
+        dpos += w
+
+
+def test_c4_full_three_groups(step):
+    ga, gb, gc = step["C4a_batched_layernorm"], step["C4b_grouped_linear_relu"], step["C4c_grouped_linear_concat"]
+    towers = ga.cfg["towers"]
+    out = gc.aout.tensor(gc.iy)
+    amid = ga.amid
+    esc = tot = 0
+    worst_b = worst_c = worst_e2e = 0.0
+    for k in range(0, len(towers), 4):                 # every 4th tower: all (D, H) classes, 128 towers
+        t, i = towers[k], ga.idx[k]
+        rows = sample_rows(t["B"], 6, 4000 + k)
+        rsel = torch.from_numpy(rows).cuda()
+        xn = to_host(amid.tensor(i["xn"])[rsel])
+        h = to_host(amid.tensor(i["h"])[rsel])
+        o = to_host(out[rsel, k * t["out"]:(k + 1) * t["out"]])
+        e, n = ln_check(xn, np.ascontiguousarray(t["x"][rows]), t["gamma"], t["beta"], t["eps"])
+        esc, tot = esc + e, tot + n
+        # group 2 from the GPU's own bf16 LN output, group 3 from the GPU's own bf16 H
+        h64 = oracle.activation(oracle.linear(xn, t["w1"], t["b1"], BF16), 1)
+        worst_b = max(worst_b, row_l2_rel_err(h, h64, BF16))
+        o64 = oracle.linear(h, t["w2"], t["b2"], BF16)
+        worst_c = max(worst_c, row_l2_rel_err(o, o64, BF16))
+        # informational end-to-end chain (oracle rounds at each group boundary), 3x looser
+        chain = graphs.recsys_tower(dict(t, x=np.ascontiguousarray(t["x"][rows])))
+        worst_e2e = max(worst_e2e, row_l2_rel_err(o, chain["out64"], BF16))
+    assert esc < 1e-3 * tot
+    assert worst_b <= TOL_BF16 and worst_c <= TOL_BF16, (worst_b, worst_c)
+    assert worst_e2e <= 3 * TOL_BF16, worst_e2e
