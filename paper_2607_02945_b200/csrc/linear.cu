@@ -6,28 +6,35 @@
 //   grouped_gemm_sm100_kernel  bf16 in/out, fp32 accumulate.  Persistent, one CTA
 //       per SM, warp-specialised:
 //         warp 0      TMA producer: cp.async.bulk.tensor 2-D loads of a 128x64 X
-//                     tile and a BNx64 W tile (128-byte swizzle) into a 4-stage
-//                     shared-memory ring guarded by full/empty mbarriers;
+//                     tile and a BNx64 W tile (128-byte swizzle) into a shared-
+//                     memory ring (4..8 stages, sized per plan) guarded by
+//                     full/empty mbarriers;
 //         warp 1      TMEM allocator + MMA issuer: one elected lane issues
 //                     tcgen05.mma.cta_group::1.kind::f16 (M=128, N=BN, K=16) four
 //                     times per stage into a TMEM accumulator, tcgen05.commit
 //                     releases the stage / publishes the accumulator;
-//         warps 2..9  epilogue, two warps per TMEM lane quadrant taking alternate
+//         warp 2      device-side tile scheduler: one atomicAdd per chunk of up
+//                     to 4 tiles (one 128-byte line of the plan's tile table),
+//                     copies each tile's 32-byte entry and its bias slice into a
+//                     4-deep shared-memory queue, prefetches the member's tensor
+//                     maps; the last CTA to finish re-arms the counter;
+//         warps 3..10 epilogue, two warps per TMEM lane quadrant taking alternate
 //                     64-column chunks: tcgen05.ld (32 lanes x 32 columns), + bias
-//                     (fp32, broadcast from shared memory), activation (ReLU folded
-//                     into cvt.rn.relu.bf16x2), RNE to bf16, swizzled st.shared, TMA
-//                     store (cp.async.bulk.tensor, 64x32 boxes) into the member's
-//                     output or its slot of the concatenated output.
+//                     (from the queue slot: no global load in the epilogue),
+//                     activation (ReLU folded into cvt.rn.relu.bf16x2), RNE to
+//                     bf16, swizzled st.shared, TMA store (cp.async.bulk.tensor,
+//                     64x32 boxes) into the member's output or its slot of the
+//                     concatenated output.
 //       TMEM holds two accumulator stages (2 x 256 columns) so the epilogue of
-//       tile t overlaps the MMAs of tile t+1.  The device-side tile scheduler
-//       decodes a linear tile id into (member, m-block, n-block) from the
-//       per-member tile-count prefix sums; tiles of one X row-panel are adjacent
-//       so its re-reads hit L2.
+//       tile t overlaps the MMAs of tile t+1.  Tiles of one X row-panel are
+//       adjacent in the schedule so its re-reads hit L2.  Deterministic: the
+//       scheduler only decides WHICH CTA computes a tile, never how.
 //   grouped_gemm_f32_kernel    plain fp32 FFMA (no TF32) 64x64 tiles for fp32
 //       groups (configs[0]); same tile scheduler, accurate tanhf/expf epilogue.
 #include <cuda.h>   // CUtensorMap types only; the encoder is fetched through the runtime
 
 #include <algorithm>
+#include <cstdlib>
 
 #include "common.h"
 
@@ -110,35 +117,38 @@ cudaError_t launch_linear_f32(const opt_plan* p, cudaStream_t s) {
 constexpr int kBM = 128;           // tile rows (UMMA M, cta_group::1)
 constexpr int kBK = 64;            // K per stage = one 128-byte swizzle row of bf16
 constexpr int kMaxBN = 256;        // widest tile (UMMA N)
-constexpr int kStages = 4;
+constexpr int kMaxStages = 8;      // smem ring depth is chosen per plan (stage = A tile + widest W tile of the group)
 constexpr int kAccStages = 2;
 constexpr int kTmemCols = 512;     // 2 accumulator stages x 256 fp32 columns
 constexpr int kEpiWarps = 8;       // two per TMEM lane quadrant, alternating 64-column chunks
-constexpr int kGemmThreads = 64 + 32 * kEpiWarps;   // warp 0 TMA, warp 1 MMA, warps 2..9 epilogue
+constexpr int kFirstEpiWarp = 3;   // warp 0 TMA, warp 1 MMA, warp 2 tile scheduler, warps 3..10 epilogue
+constexpr int kGemmThreads = 32 * (kFirstEpiWarp + kEpiWarps);
 constexpr int kABytes = kBM * kBK * 2;          // 16 KB
-constexpr int kBBytesMax = kMaxBN * kBK * 2;    // 32 KB
-constexpr int kStageBytes = kABytes + kBBytesMax;
 constexpr int kEpiBufBytes = 32 * 128;          // one warp's 32 rows x 64 bf16 staging tile
-constexpr int kSmemEpi = kStages * kStageBytes;
-constexpr int kSmemBias = kSmemEpi + kEpiWarps * kEpiBufBytes;    // per warp 64 fp32 bias values
-constexpr int kSmemBar = kSmemBias + kEpiWarps * 64 * 4;
-constexpr int kSmemBytes = kSmemBar + 256;      // barriers; the dynamic smem base is 1024-byte aligned (checked)
+constexpr int kQDepth = 4;                      // tile queue: scheduler warp -> TMA / MMA / epilogue warps
+constexpr int kQBiasBytes = kMaxBN * 2;         // the tile's bias slice, bf16
+constexpr int kQSlotBytes = kQBiasBytes + 32;   // + the tile's 32-byte TileEntry
+constexpr int kTilesPerChunk = 4;               // tiles fetched per atomic (one 128-byte table line)
+constexpr int kSmemMax = 227 * 1024;
+constexpr int kSmemFixed = kEpiWarps * kEpiBufBytes + kQDepth * kQSlotBytes + 256;   // staging + queue + barriers
 
 struct alignas(128) GemmMember {
   CUtensorMap tmA;       // X [M,K]   box {64, 128}   load
   CUtensorMap tmB;       // W [N,K]   box {64, BN}    load
   CUtensorMap tmY;       // Y [M,N]   box {64, 32}    store
-  const void* bias;      // [N] bf16 or NULL
-  int32_t M, N, K;
-  int32_t bn;            // tile width of this member
-  int32_t nbn;           // n-blocks per m-block
-  int32_t nkb;           // K blocks
-  int32_t act;
-  uint32_t idesc;        // tcgen05 instruction descriptor (M=128, N=bn, bf16 x bf16 -> fp32)
-  uint32_t b_bytes;      // bytes of one W stage = bn * 128
-  int32_t pad[5];
 };
-static_assert(sizeof(GemmMember) % 128 == 0, "GemmMember must keep tensor maps 128-byte aligned");
+static_assert(sizeof(GemmMember) == 384, "GemmMember must keep tensor maps 128-byte aligned");
+
+// One output tile, everything the three warp roles need (built by the planner, copied into shared
+// memory by the scheduler warp).  member < 0: padding entry of a chunk (skipped).
+struct alignas(16) TileEntry {
+  int32_t member, m0, n0;
+  uint32_t idesc;        // tcgen05 instruction descriptor (M=128, N=bn, bf16 x bf16 -> fp32)
+  uint32_t bn_nkb;       // tile width | K blocks << 16
+  uint32_t misc;         // K=16 steps in the last K block | act << 8 | valid columns (min(bn, N-n0)) << 16
+  const void* bias;      // bias + n0 (bf16) or NULL
+};
+static_assert(sizeof(TileEntry) == 32, "TileEntry is two 16-byte vectors");
 
 // ---- PTX wrappers ------------------------------------------------------------
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
@@ -220,101 +230,150 @@ __device__ __forceinline__ uint32_t pack_relu_bf16x2(float lo, float hi) {
   asm("cvt.rn.relu.bf16x2.f32 %0, %1, %2;" : "=r"(d) : "f"(hi), "f"(lo));
   return d;
 }
+__device__ __forceinline__ uint4 lds128(uint32_t addr) {
+  uint4 v;
+  asm volatile("ld.shared.v4.b32 {%0, %1, %2, %3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "r"(addr) : "memory");
+  return v;
+}
+__device__ __forceinline__ void sts128(uint32_t addr, uint4 v) {
+  asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(addr), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w) : "memory");
+}
 
-// Persistent tile walk of one warp role: tile ids blockIdx.x, +gridDim.x, ...; the member index only
-// moves forward, so it is advanced incrementally over the prefix sums.
-struct TileWalk {
-  const int32_t* __restrict__ starts;
-  int n_members, mi, next_start;
-  __device__ __forceinline__ TileWalk(const int32_t* st, int n) : starts(st), n_members(n), mi(0) {
-    next_start = __ldg(st + 1);
-  }
-  // -> member index of `tile`; local = tile - starts[mi]
-  __device__ __forceinline__ int seek(int tile, int* local) {
-    while (tile >= next_start) { ++mi; next_start = __ldg(starts + mi + 1); }
-    *local = tile - __ldg(starts + mi);
-    return mi;
-  }
-};
-
-// Epilogue of one 32-row x 64-column chunk held in v[64] (this thread: one row): + bias (fp32, broadcast
-// from shared memory), activation, RNE to bf16, 128-byte-swizzled st.shared of the row.
+// Epilogue math of one 32-row x 64-column chunk held in v[64] (this thread: one row): + bias (bf16 in the
+// tile's queue slot, widened to fp32), activation, RNE to bf16 -> 32 packed pairs.
 template <int ACT>
-__device__ __forceinline__ void epi_chunk(const uint32_t (&v)[64], const float* bias_s, uint32_t srow, int lane) {
+__device__ __forceinline__ void epi_math(const uint32_t (&v)[64], uint32_t bias_addr, uint32_t (&p)[32]) {
 #pragma unroll
-  for (int j = 0; j < 8; ++j) {          // 8 columns -> one 16-byte chunk, 128B-swizzled position
-    const float4 b0 = *reinterpret_cast<const float4*>(bias_s + 8 * j);
-    const float4 b1 = *reinterpret_cast<const float4*>(bias_s + 8 * j + 4);
-    const float x0 = __uint_as_float(v[8 * j + 0]) + b0.x, x1 = __uint_as_float(v[8 * j + 1]) + b0.y;
-    const float x2 = __uint_as_float(v[8 * j + 2]) + b0.z, x3 = __uint_as_float(v[8 * j + 3]) + b0.w;
-    const float x4 = __uint_as_float(v[8 * j + 4]) + b1.x, x5 = __uint_as_float(v[8 * j + 5]) + b1.y;
-    const float x6 = __uint_as_float(v[8 * j + 6]) + b1.z, x7 = __uint_as_float(v[8 * j + 7]) + b1.w;
-    uint32_t p0, p1, p2, p3;
-    if (ACT == OPT_ACT_RELU) {
-      p0 = pack_relu_bf16x2(x0, x1); p1 = pack_relu_bf16x2(x2, x3);
-      p2 = pack_relu_bf16x2(x4, x5); p3 = pack_relu_bf16x2(x6, x7);
-    } else {
-      p0 = pack_bf16x2(act_f32<true>(x0, ACT), act_f32<true>(x1, ACT));
-      p1 = pack_bf16x2(act_f32<true>(x2, ACT), act_f32<true>(x3, ACT));
-      p2 = pack_bf16x2(act_f32<true>(x4, ACT), act_f32<true>(x5, ACT));
-      p3 = pack_bf16x2(act_f32<true>(x6, ACT), act_f32<true>(x7, ACT));
+  for (int j = 0; j < 8; ++j) {          // 8 columns per step
+    const uint4 b = lds128(bias_addr + 16 * j);
+    const uint32_t bw[4] = {b.x, b.y, b.z, b.w};
+#pragma unroll
+    for (int t = 0; t < 4; ++t) {
+      const float lo = __uint_as_float(v[8 * j + 2 * t]) + bf16_lo(bw[t]);
+      const float hi = __uint_as_float(v[8 * j + 2 * t + 1]) + bf16_hi(bw[t]);
+      if (ACT == OPT_ACT_RELU) p[4 * j + t] = pack_relu_bf16x2(lo, hi);
+      else p[4 * j + t] = pack_bf16x2(act_f32<true>(lo, ACT), act_f32<true>(hi, ACT));
     }
-    asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};"
-                 ::"r"(srow + ((j ^ (lane & 7)) << 4)), "r"(p0), "r"(p1), "r"(p2), "r"(p3) : "memory");
   }
 }
 
+// Kernel-wide shared-memory map (dynamic, 1024-byte aligned base):
+//   [0, nstages*stage_bytes)   operand ring: per stage a 128x64 X tile then a BNx64 W tile (128B swizzle)
+//   + 8 x 4 KB                 epilogue staging tiles (one per epilogue warp)
+//   + kQDepth x 544 B          tile queue slots: 512 B bias slice (bf16) + 32 B TileEntry
+//   + 256 B                    mbarriers: full[8] empty[8] tfull[2] tempty[2] qfull[4] qempty[4], TMEM base
 __global__ void __launch_bounds__(kGemmThreads, 1)
-grouped_gemm_sm100_kernel(const GemmMember* __restrict__ members, const int32_t* __restrict__ starts,
-                          int n_members, int total_tiles) {
+grouped_gemm_sm100_kernel(const GemmMember* __restrict__ members, const uint4* __restrict__ chunks, int n_chunks,
+                          int* __restrict__ counters, int nstages, int stage_bytes) {
   extern __shared__ __align__(1024) uint8_t smem[];
   const uint32_t sbase = smem_u32(smem);
   if ((sbase & 1023u) != 0) __trap();            // 128-byte-swizzle tiles need 1024-byte alignment
-  const uint32_t epi_base = sbase + kSmemEpi;
-  const uint32_t bar_base = sbase + kSmemBar;
-  // barrier layout (8 bytes each): full[kStages], empty[kStages], tmem_full[2], tmem_empty[2], then tmem ptr
+  const uint32_t epi_base = sbase + (uint32_t)(nstages * stage_bytes);
+  const uint32_t q_base = epi_base + kEpiWarps * kEpiBufBytes;
+  const uint32_t bar_base = q_base + kQDepth * kQSlotBytes;
   auto full_bar = [&](int s) { return bar_base + 8u * s; };
-  auto empty_bar = [&](int s) { return bar_base + 8u * (kStages + s); };
-  auto tfull_bar = [&](int s) { return bar_base + 8u * (2 * kStages + s); };
-  auto tempty_bar = [&](int s) { return bar_base + 8u * (2 * kStages + kAccStages + s); };
-  volatile uint32_t* tmem_ptr_smem = reinterpret_cast<volatile uint32_t*>(smem + kSmemBar + 8 * (2 * kStages + 2 * kAccStages));
+  auto empty_bar = [&](int s) { return bar_base + 8u * (kMaxStages + s); };
+  auto tfull_bar = [&](int s) { return bar_base + 8u * (2 * kMaxStages + s); };
+  auto tempty_bar = [&](int s) { return bar_base + 8u * (2 * kMaxStages + kAccStages + s); };
+  auto qfull_bar = [&](int s) { return bar_base + 8u * (2 * kMaxStages + 2 * kAccStages + s); };
+  auto qempty_bar = [&](int s) { return bar_base + 8u * (2 * kMaxStages + 2 * kAccStages + kQDepth + s); };
+  auto q_slot = [&](int s) { return q_base + (uint32_t)s * kQSlotBytes; };
+  const uint32_t tmem_ptr_addr = bar_base + 8u * (2 * kMaxStages + 2 * kAccStages + 2 * kQDepth);
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
 
   if (warp == 0 && lane == 0) {
-    for (int s = 0; s < kStages; ++s) { mbar_init(full_bar(s), 1); mbar_init(empty_bar(s), 1); }
+    for (int s = 0; s < nstages; ++s) { mbar_init(full_bar(s), 1); mbar_init(empty_bar(s), 1); }
     for (int s = 0; s < kAccStages; ++s) { mbar_init(tfull_bar(s), 1); mbar_init(tempty_bar(s), kEpiWarps); }
+    for (int s = 0; s < kQDepth; ++s) { mbar_init(qfull_bar(s), 1); mbar_init(qempty_bar(s), 2 + kEpiWarps); }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     fence_proxy_async_smem();
   }
   if (warp == 1) {
     asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;"
-                 ::"r"(smem_u32((const void*)tmem_ptr_smem)), "n"(kTmemCols) : "memory");
+                 ::"r"(tmem_ptr_addr), "n"(kTmemCols) : "memory");
     asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
   }
   tc_fence_before();
   __syncthreads();
   tc_fence_after();
-  const uint32_t tmem_base = *tmem_ptr_smem;
+  uint32_t tmem_base;
+  asm volatile("ld.shared.b32 %0, [%1];" : "=r"(tmem_base) : "r"(tmem_ptr_addr) : "memory");
 
-  if (warp == 0) {
+  if (warp == 2) {
+    // ----------------------------------------------------- tile scheduler ----
+    // Dynamic: one atomic per CHUNK of up to 4 tiles (one 128-byte table line); the next chunk id is
+    // fetched while this chunk is published.  Per tile: entry + bias slice -> queue slot -> qfull.
+    int qs = 0; uint32_t qph = 0;
+    int c = blockIdx.x;
+    while (c < n_chunks) {
+      int nextc = 0;
+      if (lane == 0) nextc = atomicAdd(counters, 1) + (int)gridDim.x;
+      uint4 e = make_uint4(0xFFFFFFFFu, 0, 0, 0);
+      if (lane < 2 * kTilesPerChunk) e = __ldg(chunks + (size_t)c * (2 * kTilesPerChunk) + lane);   // lane 2g, 2g+1: tile g
+      uint4 bias_v[kTilesPerChunk];
+      int member[kTilesPerChunk];
+#pragma unroll
+      for (int g = 0; g < kTilesPerChunk; ++g) {
+        member[g] = (int)__shfl_sync(0xffffffffu, e.x, 2 * g);
+        const uint32_t misc = __shfl_sync(0xffffffffu, e.y, 2 * g + 1);
+        const uint32_t blo = __shfl_sync(0xffffffffu, e.z, 2 * g + 1), bhi = __shfl_sync(0xffffffffu, e.w, 2 * g + 1);
+        const uint4* bp = reinterpret_cast<const uint4*>(((uint64_t)bhi << 32) | blo);
+        bias_v[g] = make_uint4(0, 0, 0, 0);
+        if (member[g] >= 0) {
+          if (bp != nullptr && 8 * lane < (int)(misc >> 16)) bias_v[g] = __ldg(bp + lane);
+          if (lane < 3)   // warm the descriptor cache for the member's three tensor maps
+            asm volatile("prefetch.tensormap [%0];" ::"l"(reinterpret_cast<const char*>(members + member[g]) + 128 * lane) : "memory");
+        }
+      }
+#pragma unroll
+      for (int g = 0; g < kTilesPerChunk; ++g) {
+        if (member[g] < 0) continue;       // warp-uniform
+        mbar_wait(qempty_bar(qs), qph ^ 1);
+        const uint32_t slot = q_slot(qs);
+        sts128(slot + 16 * lane, bias_v[g]);
+        if ((lane >> 1) == g) sts128(slot + kQBiasBytes + 16 * (lane & 1), e);
+        __syncwarp();
+        if (lane == 0) mbar_arrive(qfull_bar(qs));
+        if (++qs == kQDepth) { qs = 0; qph ^= 1; }
+      }
+      c = __shfl_sync(0xffffffffu, nextc, 0);
+    }
+    // end marker, then the last CTA to get here re-arms the counters for the next launch of this plan
+    mbar_wait(qempty_bar(qs), qph ^ 1);
+    if (lane == 0) {
+      sts128(q_slot(qs) + kQBiasBytes, make_uint4(0xFFFFFFFFu, 0, 0, 0));
+      mbar_arrive(qfull_bar(qs));
+      __threadfence();
+      if (atomicAdd(counters + 1, 1) == (int)gridDim.x - 1) {
+        counters[0] = 0;
+        counters[1] = 0;
+        __threadfence();
+      }
+    }
+  } else if (warp == 0) {
     // ------------------------------------------------------- TMA producer ----
     if (lane == 0) {
       int stage = 0; uint32_t phase = 0;
-      TileWalk walk(starts, n_members);
-      for (int tile = blockIdx.x; tile < total_tiles; tile += gridDim.x) {
-        int local;
-        const GemmMember* m = members + walk.seek(tile, &local);
-        const int nbn = m->nbn, nkb = m->nkb, bn = m->bn;
-        const int m0 = (local / nbn) * kBM, n0 = (local % nbn) * bn;
-        const uint32_t tx_bytes = kABytes + m->b_bytes;
+      int qs = 0; uint32_t qph = 0;
+      for (;;) {
+        mbar_wait(qfull_bar(qs), qph);
+        const uint4 e0 = lds128(q_slot(qs) + kQBiasBytes);
+        const uint4 e1 = lds128(q_slot(qs) + kQBiasBytes + 16);
+        mbar_arrive(qempty_bar(qs));
+        if (++qs == kQDepth) { qs = 0; qph ^= 1; }
+        if ((int)e0.x < 0) break;
+        const GemmMember* m = members + (int)e0.x;
+        const int m0 = (int)e0.y, n0 = (int)e0.z;
+        const int bn = (int)(e1.x & 0xFFFFu), nkb = (int)(e1.x >> 16);
+        const uint32_t tx_bytes = kABytes + (uint32_t)bn * (kBK * 2);
         for (int kb = 0; kb < nkb; ++kb) {
           mbar_wait(empty_bar(stage), phase ^ 1);
           mbar_expect_tx(full_bar(stage), tx_bytes);
-          const uint32_t sa = sbase + stage * kStageBytes;
+          const uint32_t sa = sbase + stage * stage_bytes;
           tma_load_2d(sa, &m->tmA, full_bar(stage), kb * kBK, m0);
           tma_load_2d(sa + kABytes, &m->tmB, full_bar(stage), kb * kBK, n0);
-          if (++stage == kStages) { stage = 0; phase ^= 1; }
+          if (++stage == nstages) { stage = 0; phase ^= 1; }
         }
       }
     }
@@ -323,25 +382,29 @@ grouped_gemm_sm100_kernel(const GemmMember* __restrict__ members, const int32_t*
     if (lane == 0) {
       int stage = 0; uint32_t phase = 0;
       int as = 0; uint32_t aphase = 0;
-      TileWalk walk(starts, n_members);
-      for (int tile = blockIdx.x; tile < total_tiles; tile += gridDim.x) {
-        int local;
-        const GemmMember* m = members + walk.seek(tile, &local);
-        const int nkb = m->nkb, K = m->K;
-        const uint32_t idesc = m->idesc;
+      int qs = 0; uint32_t qph = 0;
+      for (;;) {
+        mbar_wait(qfull_bar(qs), qph);
+        const uint4 e0 = lds128(q_slot(qs) + kQBiasBytes);
+        const uint4 e1 = lds128(q_slot(qs) + kQBiasBytes + 16);
+        mbar_arrive(qempty_bar(qs));
+        if (++qs == kQDepth) { qs = 0; qph ^= 1; }
+        if ((int)e0.x < 0) break;
+        const uint32_t idesc = e0.w;
+        const int nkb = (int)(e1.x >> 16), klast = (int)(e1.y & 0xFFu);
         mbar_wait(tempty_bar(as), aphase ^ 1);      // epilogue has drained this accumulator stage
         tc_fence_after();
         const uint32_t d_tmem = tmem_base + as * kMaxBN;
         for (int kb = 0; kb < nkb; ++kb) {
           mbar_wait(full_bar(stage), phase);
           tc_fence_after();
-          const uint32_t sa = sbase + stage * kStageBytes;
+          const uint32_t sa = sbase + stage * stage_bytes;
           const uint64_t adesc = umma_desc_sw128(sa), bdesc = umma_desc_sw128(sa + kABytes);
-          const int ksteps = min(kBK / 16, (K - kb * kBK + 15) / 16);
+          const int ksteps = kb + 1 < nkb ? kBK / 16 : klast;
           for (int k = 0; k < ksteps; ++k)   // +32 bytes (= +2 encoded) per K=16 step inside the swizzle row
             tc_mma_bf16(d_tmem, adesc + 2 * k, bdesc + 2 * k, idesc, (kb | k) != 0);
           tc_commit(empty_bar(stage));       // frees the smem stage when these MMAs retire
-          if (++stage == kStages) { stage = 0; phase ^= 1; }
+          if (++stage == nstages) { stage = 0; phase ^= 1; }
         }
         tc_commit(tfull_bar(as));            // accumulator complete
         if (++as == kAccStages) { as = 0; aphase ^= 1; }
@@ -349,19 +412,22 @@ grouped_gemm_sm100_kernel(const GemmMember* __restrict__ members, const int32_t*
     }
   } else {
     // ----------------------------------------------------------- epilogue ----
+    const int ew = warp - kFirstEpiWarp;
     const int quad = warp & 3;               // TMEM lane quadrant this warp may read
-    const int half = (warp - 2) >> 2;        // 0: even 64-column chunks, 1: odd ones
-    const uint32_t sbuf = epi_base + (uint32_t)(warp - 2) * kEpiBufBytes;
+    const int half = ew >> 2;                // 0: even 64-column chunks, 1: odd ones
+    const uint32_t sbuf = epi_base + (uint32_t)ew * kEpiBufBytes;
     const uint32_t srow = sbuf + lane * 128;
-    float* bias_s = reinterpret_cast<float*>(smem + kSmemBias) + (warp - 2) * 64;
     int as = 0; uint32_t aphase = 0;
-    TileWalk walk(starts, n_members);
-    for (int tile = blockIdx.x; tile < total_tiles; tile += gridDim.x) {
-      int local;
-      const GemmMember* m = members + walk.seek(tile, &local);
-      const int nbn = m->nbn, bn = m->bn, N = m->N, act = m->act;
-      const int m0 = (local / nbn) * kBM, n0 = (local % nbn) * bn;
-      const uint32_t* bias = reinterpret_cast<const uint32_t*>(m->bias);   // bf16 pairs
+    int qs = 0; uint32_t qph = 0;
+    for (;;) {
+      mbar_wait(qfull_bar(qs), qph);
+      const uint32_t slot = q_slot(qs);
+      const uint4 e0 = lds128(slot + kQBiasBytes);
+      const uint4 e1 = lds128(slot + kQBiasBytes + 16);
+      if ((int)e0.x < 0) break;
+      const GemmMember* m = members + (int)e0.x;
+      const int m0 = (int)e0.y, n0 = (int)e0.z;
+      const int bn = (int)(e1.x & 0xFFFFu), act = (int)((e1.y >> 8) & 0xFFu);
       mbar_wait(tfull_bar(as), aphase);
       tc_fence_after();
       const uint32_t t_row = tmem_base + ((uint32_t)(quad * 32) << 16) + as * kMaxBN;
@@ -371,11 +437,6 @@ grouped_gemm_sm100_kernel(const GemmMember* __restrict__ members, const int32_t*
         uint32_t v[64];
         tc_ld_32x32(t_row + c * 64, *reinterpret_cast<uint32_t(*)[32]>(&v[0]));
         tc_ld_32x32(t_row + c * 64 + 32, *reinterpret_cast<uint32_t(*)[32]>(&v[32]));
-        // bias of the chunk's 64 columns -> fp32 in shared memory (lane l owns columns 2l, 2l+1)
-        const int col0 = n0 + c * 64;
-        const int bc = col0 + 2 * lane;
-        const uint32_t bb = (bias != nullptr && bc < N) ? __ldg(bias + (bc >> 1)) : 0u;
-        *reinterpret_cast<float2*>(bias_s + 2 * lane) = make_float2(bf16_lo(bb), bf16_hi(bb));
         tc_wait_ld();
         if (c + 2 >= nchunks) {              // this warp's part of the accumulator is in registers
           tc_fence_before();
@@ -383,19 +444,25 @@ grouped_gemm_sm100_kernel(const GemmMember* __restrict__ members, const int32_t*
           if (lane == 0) mbar_arrive(tempty_bar(as));
           released = true;
         }
-        // staging buffer free? (the previous TMA store of this warp has read it)
-        if (lane == 0) tma_store_wait_read<0>();
-        __syncwarp();                        // also publishes bias_s to the warp
+        uint32_t p[32];
+        const uint32_t bias_addr = slot + (uint32_t)c * 128;
         switch (act) {
-          case OPT_ACT_RELU: epi_chunk<OPT_ACT_RELU>(v, bias_s, srow, lane); break;
-          case OPT_ACT_NONE: epi_chunk<OPT_ACT_NONE>(v, bias_s, srow, lane); break;
-          case OPT_ACT_TANH: epi_chunk<OPT_ACT_TANH>(v, bias_s, srow, lane); break;
-          default:           epi_chunk<OPT_ACT_SIGMOID>(v, bias_s, srow, lane); break;
+          case OPT_ACT_RELU: epi_math<OPT_ACT_RELU>(v, bias_addr, p); break;
+          case OPT_ACT_NONE: epi_math<OPT_ACT_NONE>(v, bias_addr, p); break;
+          case OPT_ACT_TANH: epi_math<OPT_ACT_TANH>(v, bias_addr, p); break;
+          default:           epi_math<OPT_ACT_SIGMOID>(v, bias_addr, p); break;
         }
+        // staging buffer free? (the previous TMA store of this warp has read it) -- checked after the math so
+        // that the store engine's read of the previous chunk overlaps it
+        if (lane == 0) tma_store_wait_read<0>();
+        __syncwarp();
+#pragma unroll
+        for (int j = 0; j < 8; ++j)            // 16-byte pieces at their 128B-swizzled position
+          sts128(srow + ((j ^ (lane & 7)) << 4), make_uint4(p[4 * j], p[4 * j + 1], p[4 * j + 2], p[4 * j + 3]));
         fence_proxy_async_smem();
         __syncwarp();
         if (lane == 0) {
-          tma_store_2d(&m->tmY, sbuf, col0, m0 + quad * 32);
+          tma_store_2d(&m->tmY, sbuf, n0 + c * 64, m0 + quad * 32);
           tma_store_commit();
         }
       }
@@ -404,6 +471,9 @@ grouped_gemm_sm100_kernel(const GemmMember* __restrict__ members, const int32_t*
         __syncwarp();
         if (lane == 0) mbar_arrive(tempty_bar(as));
       }
+      __syncwarp();                          // every lane has read the slot's bias
+      if (lane == 0) mbar_arrive(qempty_bar(qs));
+      if (++qs == kQDepth) { qs = 0; qph ^= 1; }
       if (++as == kAccStages) { as = 0; aphase ^= 1; }
     }
     if (lane == 0) tma_store_wait_all();
@@ -418,10 +488,10 @@ grouped_gemm_sm100_kernel(const GemmMember* __restrict__ members, const int32_t*
 }
 
 cudaError_t launch_linear_bf16(const opt_plan* p, cudaStream_t s) {
-  const char* base = static_cast<const char*>(p->dev_tables);
-  grouped_gemm_sm100_kernel<<<p->grid, p->block, p->smem, s>>>(reinterpret_cast<const GemmMember*>(base + p->off0),
-                                                              reinterpret_cast<const int32_t*>(base + p->off1),
-                                                              p->n_members, p->total_tiles);
+  char* base = static_cast<char*>(p->dev_tables);
+  grouped_gemm_sm100_kernel<<<p->grid, p->block, p->smem, s>>>(
+      reinterpret_cast<const GemmMember*>(base + p->off0), reinterpret_cast<const uint4*>(base + p->off1), p->n_chunks,
+      reinterpret_cast<int*>(base + p->off2), p->nstages, p->stage_bytes);
   return cudaGetLastError();
 }
 
@@ -540,6 +610,9 @@ extern "C" opt_status opt_linear_plan_create(const opt_linear_member* members, i
   if (opt_status st = get_encoder(&enc)) { delete p; return st; }
   std::vector<GemmMember> tab(n);
   memset(tab.data(), 0, tab.size() * sizeof(GemmMember));
+  struct MemberTiling { int bn, nbn, nkb, klast; uint32_t idesc; };
+  std::vector<MemberTiling> tiling(n);
+  int max_bn = 16;
   for (int32_t i = 0; i < n; ++i) {
     const opt_linear_member& m = members[i];
     GemmMember& t = tab[i];
@@ -551,31 +624,83 @@ extern "C" opt_status opt_linear_plan_create(const opt_linear_member* members, i
       delete p;
       return st;
     }
-    t.bias = m.bias; t.M = m.M; t.N = m.N; t.K = m.K; t.bn = bn;
-    t.nbn = (m.N + bn - 1) / bn; t.nkb = (m.K + kBK - 1) / kBK; t.act = m.act;
+    MemberTiling& tl = tiling[i];
+    tl.bn = bn; tl.nbn = (m.N + bn - 1) / bn; tl.nkb = (m.K + kBK - 1) / kBK;
+    tl.klast = (m.K - (tl.nkb - 1) * kBK + 15) / 16;
     // tcgen05 instruction descriptor, kind::f16: D fp32 (bits 4-5 = 1), A bf16 (bits 7-9 = 1), B bf16
     // (bits 10-12 = 1), A and B K-major (bits 15, 16 = 0), N>>3 at bits 17-22, M>>4 at bits 24-28.
-    t.idesc = (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(bn >> 3) << 17) | ((uint32_t)(kBM >> 4) << 24);
-    t.b_bytes = (uint32_t)bn * kBK * 2;
-    starts[i] = (int32_t)tiles;
-    tiles += (int64_t)((m.M + kBM - 1) / kBM) * t.nbn;
-    if (tiles > INT32_MAX) { delete p; return fail(OPT_ERR_UNSUPPORTED, "too many tiles"); }
+    tl.idesc = (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(bn >> 3) << 17) | ((uint32_t)(kBM >> 4) << 24);
+    max_bn = std::max(max_bn, bn);
+    const int nmb = (m.M + kBM - 1) / kBM;
+    tiles += (int64_t)nmb * tl.nbn;
+    if (tiles > INT32_MAX / 2) { delete p; return fail(OPT_ERR_UNSUPPORTED, "too many tiles"); }
   }
-  starts[n] = (int32_t)tiles;
+  // Schedule order: member-major, m-block, n-block -- the n-blocks of one X row panel are adjacent, so the
+  // CTAs that take them side by side fetch the panel from HBM once (re-reads hit L2), and a member's W stays
+  // hot in L2 while its tiles are in flight.  (Interleaving tensor-bound with HBM-bound members was measured:
+  // no gain on configs[2], the kernel is bound by L2->SM operand traffic there.)
+  std::vector<TileEntry> flat;
+  flat.reserve((size_t)tiles);
+  for (int32_t i = 0; i < n; ++i) {
+    const opt_linear_member& m = members[i];
+    const MemberTiling& tl = tiling[i];
+    const int nmb = (m.M + kBM - 1) / kBM;
+    for (int mb = 0; mb < nmb; ++mb)
+      for (int nb = 0; nb < tl.nbn; ++nb) {
+        TileEntry e;
+        e.member = i; e.m0 = mb * kBM; e.n0 = nb * tl.bn; e.idesc = tl.idesc;
+        e.bn_nkb = (uint32_t)tl.bn | ((uint32_t)tl.nkb << 16);
+        e.misc = (uint32_t)tl.klast | ((uint32_t)m.act << 8) | ((uint32_t)std::min(tl.bn, m.N - e.n0) << 16);
+        e.bias = m.bias ? static_cast<const char*>(m.bias) + (size_t)e.n0 * 2 : nullptr;
+        flat.push_back(e);
+      }
+  }
+  // Chunks of 4 tiles (one 128-byte line, one atomic); the last ~3 waves go one tile per chunk so that the
+  // tail of the persistent loop is balanced at tile granularity.
+  TileEntry pad_entry;
+  memset(&pad_entry, 0, sizeof pad_entry);
+  pad_entry.member = -1;
+  size_t tail_waves = 3;
+  if (const char* e = getenv("OPT_GEMM_TAIL_WAVES")) tail_waves = (size_t)atol(e);       // experiment knob
+  const size_t tail = std::min(flat.size(), tail_waves * num_sms);
+  const size_t body = flat.size() - tail;
+  std::vector<TileEntry> chunked;
+  // chunk c = tiles c, c+nC, c+2nC, c+3nC of the schedule order: CTAs that run side by side work on
+  // neighbouring tiles (one X panel, fetched from HBM once), and one CTA's consecutive tiles come from
+  // different members (an HBM-bound tile's epilogue overlaps a tensor-bound tile's MMAs)
+  const size_t nC = (body + kTilesPerChunk - 1) / kTilesPerChunk;
+  const bool strided = getenv("OPT_GEMM_CONTIG_CHUNKS") == nullptr;                        // experiment knob
+  for (size_t c = 0; c < nC; ++c)
+    for (int g = 0; g < kTilesPerChunk; ++g) {
+      const size_t k = strided ? (size_t)g * nC + c : c * kTilesPerChunk + g;
+      chunked.push_back(k < body ? flat[k] : pad_entry);
+    }
+  for (size_t k = body; k < flat.size(); ++k) {
+    chunked.push_back(flat[k]);
+    for (int g = 1; g < kTilesPerChunk; ++g) chunked.push_back(pad_entry);
+  }
+  const int64_t n_chunks = (int64_t)(chunked.size() / kTilesPerChunk);
+
+  const int stage_bytes = kABytes + max_bn * kBK * 2;
+  const int nstages = std::min(kMaxStages, (kSmemMax - kSmemFixed) / stage_bytes);
+  const int smem_bytes = nstages * stage_bytes + kSmemFixed;
   p->kind = kPlanLinearBf16;
-  p->off0 = 0; p->off1 = align_up(tab.size() * sizeof(GemmMember));
-  const size_t total = p->off1 + align_up(starts.size() * sizeof(int32_t));
+  p->off0 = 0;
+  p->off1 = align_up(tab.size() * sizeof(GemmMember));
+  p->off2 = p->off1 + align_up(chunked.size() * sizeof(TileEntry));
+  const size_t total = p->off2 + 256;                         // two int32 scheduler counters, zero-initialised
   std::vector<char> blob(total, 0);
   memcpy(blob.data(), tab.data(), tab.size() * sizeof(GemmMember));
-  memcpy(blob.data() + p->off1, starts.data(), starts.size() * sizeof(int32_t));
+  memcpy(blob.data() + p->off1, chunked.data(), chunked.size() * sizeof(TileEntry));
   if (opt_status st = upload_tables(p, blob.data(), total)) { delete p; return st; }
-  cudaError_t e = cudaFuncSetAttribute(grouped_gemm_sm100_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBytes);
+  cudaError_t e = cudaFuncSetAttribute(grouped_gemm_sm100_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemMax);
   if (e != cudaSuccess) {
     cudaFree(p->dev_tables); delete p;
-    return fail(OPT_ERR_CUDA, "cudaFuncSetAttribute(max dynamic smem %d) failed: %s", kSmemBytes, cudaGetErrorString(e));
+    return fail(OPT_ERR_CUDA, "cudaFuncSetAttribute(max dynamic smem %d) failed: %s", kSmemMax, cudaGetErrorString(e));
   }
-  p->grid = dim3((unsigned)std::min<int64_t>(tiles, num_sms)); p->block = dim3(kGemmThreads); p->smem = kSmemBytes;
+  p->grid = dim3((unsigned)std::min<int64_t>(n_chunks, num_sms)); p->block = dim3(kGemmThreads); p->smem = smem_bytes;
   p->total_tiles = (int32_t)tiles;
+  p->n_chunks = (int32_t)n_chunks; p->nstages = nstages; p->stage_bytes = stage_bytes;
   *plan = p;
   return OPT_OK;
 }
