@@ -4,7 +4,10 @@
 //
 // Two kernels:
 //   grouped_gemm_sm100_kernel  bf16 in/out, fp32 accumulate.  Persistent, one CTA
-//       per SM, warp-specialised:
+//       per SM; by default the CTAs work as PAIRS (cluster of 2, tcgen05
+//       cta_group::2) on 256 x BN tiles -- each CTA stages its 128 rows of X and
+//       half of the W tile, the leader issues the MMAs for both, so W crosses
+//       L2->SM once per pair.  Warp-specialised:
 //         warp 0      TMA producer: cp.async.bulk.tensor 2-D loads of a 128x64 X
 //                     tile and a BNx64 W tile (128-byte swizzle) into a shared-
 //                     memory ring (4..8 stages, sized per plan) guarded by
@@ -136,8 +139,9 @@ struct alignas(128) GemmMember {
   CUtensorMap tmA;       // X [M,K]   box {64, 128}   load
   CUtensorMap tmB;       // W [N,K]   box {64, BN}    load
   CUtensorMap tmY;       // Y [M,N]   box {64, 32}    store
+  CUtensorMap tmB2;      // W [N,K]   box {64, BN/2}  load (CTA-pair kernel: each CTA holds half of the W tile)
 };
-static_assert(sizeof(GemmMember) == 384, "GemmMember must keep tensor maps 128-byte aligned");
+static_assert(sizeof(GemmMember) == 512, "GemmMember must keep tensor maps 128-byte aligned");
 
 // One output tile, everything the three warp roles need (built by the planner, copied into shared
 // memory by the scheduler warp).  member < 0: padding entry of a chunk (skipped).
@@ -217,6 +221,53 @@ __device__ __forceinline__ void tc_ld_32x32(uint32_t taddr, uint32_t (&r)[32]) {
 }
 __device__ __forceinline__ void tc_wait_ld() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
 
+// ---- CTA-pair (cta_group::2) variants ------------------------------------------
+__device__ __forceinline__ uint32_t cluster_ctarank() { uint32_t r; asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(r)); return r; }
+__device__ __forceinline__ uint32_t cluster_id_x() { uint32_t r; asm volatile("mov.u32 %0, %%clusterid.x;" : "=r"(r)); return r; }
+__device__ __forceinline__ uint32_t num_clusters_x() { uint32_t r; asm volatile("mov.u32 %0, %%nclusterid.x;" : "=r"(r)); return r; }
+// shared::cluster address of `addr` (a shared::cta address of this CTA) in CTA `rank` of the cluster
+__device__ __forceinline__ uint32_t mapa(uint32_t addr, uint32_t rank) {
+  uint32_t r;
+  asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(addr), "r"(rank));
+  return r;
+}
+__device__ __forceinline__ void cluster_sync_all() {
+  asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
+}
+// arrive on a barrier given by its shared::cluster address (own or peer CTA).  Only "I am done reading" is
+// signalled this way (queue slot, accumulator stage), so CTA-scope release is enough, as for a local barrier.
+__device__ __forceinline__ void mbar_arrive_cluster(uint32_t cluster_bar) {
+  asm volatile("mbarrier.arrive.shared::cluster.b64 _, [%0];" ::"r"(cluster_bar) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx_cluster(uint32_t cluster_bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cluster.b64 _, [%0], %1;" ::"r"(cluster_bar), "r"(bytes) : "memory");
+}
+// 16 bytes into the peer's shared memory, counted on the peer's barrier: data and signal travel together
+// (complete_tx), so the peer's plain mbarrier wait makes them visible -- no cluster-scope fence anywhere
+__device__ __forceinline__ void st_async128(uint32_t cluster_addr, uint4 v, uint32_t cluster_bar) {
+  asm volatile("st.async.weak.shared::cluster.mbarrier::complete_tx::bytes.v4.b32 [%0], {%1, %2, %3, %4}, [%5];"
+               ::"r"(cluster_addr), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w), "r"(cluster_bar) : "memory");
+}
+// TMA load issued by either CTA of a pair; the bytes are counted on the barrier `cluster_bar` (the leader's)
+__device__ __forceinline__ void tma_load_2d_pair(uint32_t dst, const void* tmap, uint32_t cluster_bar, int c0, int c1) {
+  asm volatile(
+      "cp.async.bulk.tensor.2d.cta_group::2.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4}], [%2];"
+      ::"r"(dst), "l"(tmap), "r"(cluster_bar), "r"(c0), "r"(c1) : "memory");
+}
+// commit of the pair's MMAs: arrives on the barrier at this offset in BOTH CTAs
+__device__ __forceinline__ void tc_commit_pair(uint32_t bar) {
+  asm volatile("tcgen05.commit.cta_group::2.mbarrier::arrive::one.shared::cluster.multicast::cluster.b64 [%0], %1;"
+               ::"r"(bar), "h"((uint16_t)3) : "memory");
+}
+__device__ __forceinline__ void tc_mma_bf16_pair(uint32_t d_tmem, uint64_t a_desc, uint64_t b_desc, uint32_t idesc,
+                                                 uint32_t accumulate) {
+  asm volatile(
+      "{\n\t.reg .pred p;\n\t"
+      "setp.ne.b32 p, %4, 0;\n\t"
+      "tcgen05.mma.cta_group::2.kind::f16 [%0], %1, %2, %3, p;\n\t}"
+      ::"r"(d_tmem), "l"(a_desc), "l"(b_desc), "r"(idesc), "r"(accumulate) : "memory");
+}
+
 // Shared-memory matrix descriptor, K-major operand, 128-byte swizzle: rows of
 // 128 bytes, 8-row groups 1024 bytes apart (SBO), LBO unused, version 1 (sm_100).
 __device__ __forceinline__ uint64_t umma_desc_sw128(uint32_t saddr) {
@@ -258,10 +309,16 @@ __device__ __forceinline__ void epi_math(const uint32_t (&v)[64], uint32_t bias_
 }
 
 // Kernel-wide shared-memory map (dynamic, 1024-byte aligned base):
-//   [0, nstages*stage_bytes)   operand ring: per stage a 128x64 X tile then a BNx64 W tile (128B swizzle)
+//   [0, nstages*stage_bytes)   operand ring: per stage a 128x64 X tile then the CTA's W tile (128B swizzle)
 //   + 8 x 4 KB                 epilogue staging tiles (one per epilogue warp)
 //   + kQDepth x 544 B          tile queue slots: 512 B bias slice (bf16) + 32 B TileEntry
 //   + 256 B                    mbarriers: full[8] empty[8] tfull[2] tempty[2] qfull[4] qempty[4], TMEM base
+//
+// NCTA = 1: one CTA per tile (128 x BN).  NCTA = 2: a CTA PAIR (cluster of 2, cta_group::2) per 256 x BN tile:
+// CTA r holds rows [128r, 128r+128) of X and rows [r*BN/2, (r+1)*BN/2) of the W tile, the leader (rank 0) issues
+// the MMAs for both and runs the one scheduler of the pair, each CTA drains its own 128 accumulator rows.  W
+// crosses L2->SM once per pair instead of once per CTA (configs[2] is bound by that traffic).
+template <int NCTA>
 __global__ void __launch_bounds__(kGemmThreads, 1)
 grouped_gemm_sm100_kernel(const GemmMember* __restrict__ members, const uint4* __restrict__ chunks, int n_chunks,
                           int* __restrict__ counters, int nstages, int stage_bytes) {
@@ -281,21 +338,33 @@ grouped_gemm_sm100_kernel(const GemmMember* __restrict__ members, const uint4* _
   const uint32_t tmem_ptr_addr = bar_base + 8u * (2 * kMaxStages + 2 * kAccStages + 2 * kQDepth);
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const uint32_t rank = NCTA == 2 ? cluster_ctarank() : 0u;     // 0 = leader
+  // barriers that live in the LEADER (the peer arrives on them remotely): tempty, qempty
+  auto leader = [&](uint32_t bar) { return NCTA == 2 ? mapa(bar, 0) : bar; };
+  auto arrive_leader = [&](uint32_t bar) { if (NCTA == 2) mbar_arrive_cluster(mapa(bar, 0)); else mbar_arrive(bar); };
+  auto wait_q = [&](uint32_t bar, uint32_t parity) { mbar_wait(bar, parity); };
 
   if (warp == 0 && lane == 0) {
     for (int s = 0; s < nstages; ++s) { mbar_init(full_bar(s), 1); mbar_init(empty_bar(s), 1); }
-    for (int s = 0; s < kAccStages; ++s) { mbar_init(tfull_bar(s), 1); mbar_init(tempty_bar(s), kEpiWarps); }
-    for (int s = 0; s < kQDepth; ++s) { mbar_init(qfull_bar(s), 1); mbar_init(qempty_bar(s), 2 + kEpiWarps); }
+    for (int s = 0; s < kAccStages; ++s) { mbar_init(tfull_bar(s), 1); mbar_init(tempty_bar(s), NCTA * kEpiWarps); }
+    // queue consumers: TMA + epilogue warps of every CTA of the pair, MMA issuer of the leader
+    for (int s = 0; s < kQDepth; ++s) { mbar_init(qfull_bar(s), 1); mbar_init(qempty_bar(s), NCTA * (1 + kEpiWarps) + 1); }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     fence_proxy_async_smem();
   }
   if (warp == 1) {
-    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;"
-                 ::"r"(tmem_ptr_addr), "n"(kTmemCols) : "memory");
-    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+    if (NCTA == 2) {
+      asm volatile("tcgen05.alloc.cta_group::2.sync.aligned.shared::cta.b32 [%0], %1;"
+                   ::"r"(tmem_ptr_addr), "n"(kTmemCols) : "memory");
+      asm volatile("tcgen05.relinquish_alloc_permit.cta_group::2.sync.aligned;" ::: "memory");
+    } else {
+      asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;"
+                   ::"r"(tmem_ptr_addr), "n"(kTmemCols) : "memory");
+      asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+    }
   }
   tc_fence_before();
-  __syncthreads();
+  if (NCTA == 2) cluster_sync_all(); else __syncthreads();      // the peer's barriers are initialised too
   tc_fence_after();
   uint32_t tmem_base;
   asm volatile("ld.shared.b32 %0, [%1];" : "=r"(tmem_base) : "r"(tmem_ptr_addr) : "memory");
@@ -304,51 +373,63 @@ grouped_gemm_sm100_kernel(const GemmMember* __restrict__ members, const uint4* _
     // ----------------------------------------------------- tile scheduler ----
     // Dynamic: one atomic per CHUNK of up to 4 tiles (one 128-byte table line); the next chunk id is
     // fetched while this chunk is published.  Per tile: entry + bias slice -> queue slot -> qfull.
-    int qs = 0; uint32_t qph = 0;
-    int c = blockIdx.x;
-    while (c < n_chunks) {
-      int nextc = 0;
-      if (lane == 0) nextc = atomicAdd(counters, 1) + (int)gridDim.x;
-      uint4 e = make_uint4(0xFFFFFFFFu, 0, 0, 0);
-      if (lane < 2 * kTilesPerChunk) e = __ldg(chunks + (size_t)c * (2 * kTilesPerChunk) + lane);   // lane 2g, 2g+1: tile g
-      uint4 bias_v[kTilesPerChunk];
-      int member[kTilesPerChunk];
+    // CTA pair: the leader's scheduler serves both CTAs (remote shared-memory stores + remote arrive).
+    if (rank == 0) {
+      const int n_sched = NCTA == 2 ? (int)num_clusters_x() : (int)gridDim.x;
+      int qs = 0; uint32_t qph = 0;
+      int c = NCTA == 2 ? (int)cluster_id_x() : (int)blockIdx.x;
+      // queue slot `qs` of both CTAs: local st.shared + arrive; peer: st.async pieces counted on ITS qfull
+      auto publish = [&](int qs_, uint32_t off, uint4 v) {
+        sts128(q_slot(qs_) + off, v);
+        if (NCTA == 2) st_async128(mapa(q_slot(qs_) + off, 1), v, mapa(qfull_bar(qs_), 1));
+      };
+      auto signal_full = [&](int qs_, uint32_t peer_bytes) {
+        mbar_arrive(qfull_bar(qs_));
+        if (NCTA == 2) mbar_expect_tx_cluster(mapa(qfull_bar(qs_), 1), peer_bytes);
+      };
+      while (c < n_chunks) {
+        int nextc = 0;
+        if (lane == 0) nextc = atomicAdd(counters, 1) + n_sched;
+        uint4 e = make_uint4(0xFFFFFFFFu, 0, 0, 0);
+        if (lane < 2 * kTilesPerChunk) e = __ldg(chunks + (size_t)c * (2 * kTilesPerChunk) + lane);   // lane 2g, 2g+1: tile g
+        uint4 bias_v[kTilesPerChunk];
+        int member[kTilesPerChunk];
 #pragma unroll
-      for (int g = 0; g < kTilesPerChunk; ++g) {
-        member[g] = (int)__shfl_sync(0xffffffffu, e.x, 2 * g);
-        const uint32_t misc = __shfl_sync(0xffffffffu, e.y, 2 * g + 1);
-        const uint32_t blo = __shfl_sync(0xffffffffu, e.z, 2 * g + 1), bhi = __shfl_sync(0xffffffffu, e.w, 2 * g + 1);
-        const uint4* bp = reinterpret_cast<const uint4*>(((uint64_t)bhi << 32) | blo);
-        bias_v[g] = make_uint4(0, 0, 0, 0);
-        if (member[g] >= 0) {
-          if (bp != nullptr && 8 * lane < (int)(misc >> 16)) bias_v[g] = __ldg(bp + lane);
-          if (lane < 3)   // warm the descriptor cache for the member's three tensor maps
-            asm volatile("prefetch.tensormap [%0];" ::"l"(reinterpret_cast<const char*>(members + member[g]) + 128 * lane) : "memory");
+        for (int g = 0; g < kTilesPerChunk; ++g) {
+          member[g] = (int)__shfl_sync(0xffffffffu, e.x, 2 * g);
+          const uint32_t misc = __shfl_sync(0xffffffffu, e.y, 2 * g + 1);
+          const uint32_t blo = __shfl_sync(0xffffffffu, e.z, 2 * g + 1), bhi = __shfl_sync(0xffffffffu, e.w, 2 * g + 1);
+          const uint4* bp = reinterpret_cast<const uint4*>(((uint64_t)bhi << 32) | blo);
+          bias_v[g] = make_uint4(0, 0, 0, 0);
+          if (member[g] >= 0) {
+            if (bp != nullptr && 8 * lane < (int)(misc >> 16)) bias_v[g] = __ldg(bp + lane);
+            if (lane < 4)   // warm the descriptor cache for the member's tensor maps
+              asm volatile("prefetch.tensormap [%0];" ::"l"(reinterpret_cast<const char*>(members + member[g]) + 128 * lane) : "memory");
+          }
         }
-      }
 #pragma unroll
-      for (int g = 0; g < kTilesPerChunk; ++g) {
-        if (member[g] < 0) continue;       // warp-uniform
-        mbar_wait(qempty_bar(qs), qph ^ 1);
-        const uint32_t slot = q_slot(qs);
-        sts128(slot + 16 * lane, bias_v[g]);
-        if ((lane >> 1) == g) sts128(slot + kQBiasBytes + 16 * (lane & 1), e);
-        __syncwarp();
-        if (lane == 0) mbar_arrive(qfull_bar(qs));
-        if (++qs == kQDepth) { qs = 0; qph ^= 1; }
+        for (int g = 0; g < kTilesPerChunk; ++g) {
+          if (member[g] < 0) continue;       // warp-uniform
+          wait_q(qempty_bar(qs), qph ^ 1);
+          publish(qs, 16 * lane, bias_v[g]);
+          if ((lane >> 1) == g) publish(qs, kQBiasBytes + 16 * (lane & 1), e);
+          __syncwarp();
+          if (lane == 0) signal_full(qs, kQSlotBytes);
+          if (++qs == kQDepth) { qs = 0; qph ^= 1; }
+        }
+        c = __shfl_sync(0xffffffffu, nextc, 0);
       }
-      c = __shfl_sync(0xffffffffu, nextc, 0);
-    }
-    // end marker, then the last CTA to get here re-arms the counters for the next launch of this plan
-    mbar_wait(qempty_bar(qs), qph ^ 1);
-    if (lane == 0) {
-      sts128(q_slot(qs) + kQBiasBytes, make_uint4(0xFFFFFFFFu, 0, 0, 0));
-      mbar_arrive(qfull_bar(qs));
-      __threadfence();
-      if (atomicAdd(counters + 1, 1) == (int)gridDim.x - 1) {
-        counters[0] = 0;
-        counters[1] = 0;
+      // end marker, then the last scheduler to get here re-arms the counters for the next launch of this plan
+      wait_q(qempty_bar(qs), qph ^ 1);
+      if (lane == 0) {
+        publish(qs, kQBiasBytes, make_uint4(0xFFFFFFFFu, 0, 0, 0));
+        signal_full(qs, 16);
         __threadfence();
+        if (atomicAdd(counters + 1, 1) == n_sched - 1) {
+          counters[0] = 0;
+          counters[1] = 0;
+          __threadfence();
+        }
       }
     }
   } else if (warp == 0) {
@@ -357,42 +438,52 @@ grouped_gemm_sm100_kernel(const GemmMember* __restrict__ members, const uint4* _
       int stage = 0; uint32_t phase = 0;
       int qs = 0; uint32_t qph = 0;
       for (;;) {
-        mbar_wait(qfull_bar(qs), qph);
+        wait_q(qfull_bar(qs), qph);
         const uint4 e0 = lds128(q_slot(qs) + kQBiasBytes);
         const uint4 e1 = lds128(q_slot(qs) + kQBiasBytes + 16);
-        mbar_arrive(qempty_bar(qs));
+        arrive_leader(qempty_bar(qs));
         if (++qs == kQDepth) { qs = 0; qph ^= 1; }
         if ((int)e0.x < 0) break;
         const GemmMember* m = members + (int)e0.x;
-        const int m0 = (int)e0.y, n0 = (int)e0.z;
         const int bn = (int)(e1.x & 0xFFFFu), nkb = (int)(e1.x >> 16);
-        const uint32_t tx_bytes = kABytes + (uint32_t)bn * (kBK * 2);
+        const int m0 = (int)e0.y + (int)rank * kBM;              // this CTA's 128 rows of the (pair) tile
+        const int n0 = (int)e0.z + (int)rank * (bn / NCTA);      // this CTA's rows of the W tile
+        const uint32_t b_bytes = (uint32_t)(bn / NCTA) * (kBK * 2);
+        const CUtensorMap* tmB = NCTA == 2 ? &m->tmB2 : &m->tmB;
         for (int kb = 0; kb < nkb; ++kb) {
           mbar_wait(empty_bar(stage), phase ^ 1);
-          mbar_expect_tx(full_bar(stage), tx_bytes);
           const uint32_t sa = sbase + stage * stage_bytes;
-          tma_load_2d(sa, &m->tmA, full_bar(stage), kb * kBK, m0);
-          tma_load_2d(sa + kABytes, &m->tmB, full_bar(stage), kb * kBK, n0);
+          if (NCTA == 2) {
+            // the leader's barrier counts the bytes of both CTAs
+            if (rank == 0) mbar_expect_tx(full_bar(stage), 2 * (kABytes + b_bytes));
+            const uint32_t lb = mapa(full_bar(stage), 0);
+            tma_load_2d_pair(sa, &m->tmA, lb, kb * kBK, m0);
+            tma_load_2d_pair(sa + kABytes, tmB, lb, kb * kBK, n0);
+          } else {
+            mbar_expect_tx(full_bar(stage), kABytes + b_bytes);
+            tma_load_2d(sa, &m->tmA, full_bar(stage), kb * kBK, m0);
+            tma_load_2d(sa + kABytes, tmB, full_bar(stage), kb * kBK, n0);
+          }
           if (++stage == nstages) { stage = 0; phase ^= 1; }
         }
       }
     }
   } else if (warp == 1) {
-    // --------------------------------------------------------- MMA issuer ----
-    if (lane == 0) {
+    // ------------------------------------------- MMA issuer (leader only) ----
+    if (lane == 0 && rank == 0) {
       int stage = 0; uint32_t phase = 0;
       int as = 0; uint32_t aphase = 0;
       int qs = 0; uint32_t qph = 0;
       for (;;) {
-        mbar_wait(qfull_bar(qs), qph);
+        wait_q(qfull_bar(qs), qph);
         const uint4 e0 = lds128(q_slot(qs) + kQBiasBytes);
         const uint4 e1 = lds128(q_slot(qs) + kQBiasBytes + 16);
-        mbar_arrive(qempty_bar(qs));
+        arrive_leader(qempty_bar(qs));
         if (++qs == kQDepth) { qs = 0; qph ^= 1; }
         if ((int)e0.x < 0) break;
         const uint32_t idesc = e0.w;
         const int nkb = (int)(e1.x >> 16), klast = (int)(e1.y & 0xFFu);
-        mbar_wait(tempty_bar(as), aphase ^ 1);      // epilogue has drained this accumulator stage
+        wait_q(tempty_bar(as), aphase ^ 1);         // the epilogues (of both CTAs) have drained this accumulator stage
         tc_fence_after();
         const uint32_t d_tmem = tmem_base + as * kMaxBN;
         for (int kb = 0; kb < nkb; ++kb) {
@@ -401,12 +492,15 @@ grouped_gemm_sm100_kernel(const GemmMember* __restrict__ members, const uint4* _
           const uint32_t sa = sbase + stage * stage_bytes;
           const uint64_t adesc = umma_desc_sw128(sa), bdesc = umma_desc_sw128(sa + kABytes);
           const int ksteps = kb + 1 < nkb ? kBK / 16 : klast;
-          for (int k = 0; k < ksteps; ++k)   // +32 bytes (= +2 encoded) per K=16 step inside the swizzle row
-            tc_mma_bf16(d_tmem, adesc + 2 * k, bdesc + 2 * k, idesc, (kb | k) != 0);
-          tc_commit(empty_bar(stage));       // frees the smem stage when these MMAs retire
+          for (int k = 0; k < ksteps; ++k) {  // +32 bytes (= +2 encoded) per K=16 step inside the swizzle row
+            if (NCTA == 2) tc_mma_bf16_pair(d_tmem, adesc + 2 * k, bdesc + 2 * k, idesc, (kb | k) != 0);
+            else tc_mma_bf16(d_tmem, adesc + 2 * k, bdesc + 2 * k, idesc, (kb | k) != 0);
+          }
+          // frees the smem stage (in both CTAs) when these MMAs retire
+          if (NCTA == 2) tc_commit_pair(empty_bar(stage)); else tc_commit(empty_bar(stage));
           if (++stage == nstages) { stage = 0; phase ^= 1; }
         }
-        tc_commit(tfull_bar(as));            // accumulator complete
+        if (NCTA == 2) tc_commit_pair(tfull_bar(as)); else tc_commit(tfull_bar(as));   // accumulator complete
         if (++as == kAccStages) { as = 0; aphase ^= 1; }
       }
     }
@@ -420,13 +514,13 @@ grouped_gemm_sm100_kernel(const GemmMember* __restrict__ members, const uint4* _
     int as = 0; uint32_t aphase = 0;
     int qs = 0; uint32_t qph = 0;
     for (;;) {
-      mbar_wait(qfull_bar(qs), qph);
+      wait_q(qfull_bar(qs), qph);
       const uint32_t slot = q_slot(qs);
       const uint4 e0 = lds128(slot + kQBiasBytes);
       const uint4 e1 = lds128(slot + kQBiasBytes + 16);
       if ((int)e0.x < 0) break;
       const GemmMember* m = members + (int)e0.x;
-      const int m0 = (int)e0.y, n0 = (int)e0.z;
+      const int m0 = (int)e0.y + (int)rank * kBM, n0 = (int)e0.z;
       const int bn = (int)(e1.x & 0xFFFFu), act = (int)((e1.y >> 8) & 0xFFu);
       mbar_wait(tfull_bar(as), aphase);
       tc_fence_after();
@@ -441,7 +535,7 @@ grouped_gemm_sm100_kernel(const GemmMember* __restrict__ members, const uint4* _
         if (c + 2 >= nchunks) {              // this warp's part of the accumulator is in registers
           tc_fence_before();
           __syncwarp();
-          if (lane == 0) mbar_arrive(tempty_bar(as));
+          if (lane == 0) arrive_leader(tempty_bar(as));
           released = true;
         }
         uint32_t p[32];
@@ -469,10 +563,10 @@ grouped_gemm_sm100_kernel(const GemmMember* __restrict__ members, const uint4* _
       if (!released) {                       // no chunk for this warp in a narrow tile: still hand the stage back
         tc_fence_before();
         __syncwarp();
-        if (lane == 0) mbar_arrive(tempty_bar(as));
+        if (lane == 0) arrive_leader(tempty_bar(as));
       }
       __syncwarp();                          // every lane has read the slot's bias
-      if (lane == 0) mbar_arrive(qempty_bar(qs));
+      if (lane == 0) arrive_leader(qempty_bar(qs));
       if (++qs == kQDepth) { qs = 0; qph ^= 1; }
       if (++as == kAccStages) { as = 0; aphase ^= 1; }
     }
@@ -480,18 +574,33 @@ grouped_gemm_sm100_kernel(const GemmMember* __restrict__ members, const uint4* _
   }
 
   tc_fence_before();
-  __syncthreads();
+  if (NCTA == 2) cluster_sync_all(); else __syncthreads();      // the peer may still be reading this CTA's W half
   if (warp == 1) {
     tc_fence_after();
-    asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "n"(kTmemCols) : "memory");
+    if (NCTA == 2)
+      asm volatile("tcgen05.dealloc.cta_group::2.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "n"(kTmemCols) : "memory");
+    else
+      asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "n"(kTmemCols) : "memory");
   }
 }
 
 cudaError_t launch_linear_bf16(const opt_plan* p, cudaStream_t s) {
   char* base = static_cast<char*>(p->dev_tables);
-  grouped_gemm_sm100_kernel<<<p->grid, p->block, p->smem, s>>>(
-      reinterpret_cast<const GemmMember*>(base + p->off0), reinterpret_cast<const uint4*>(base + p->off1), p->n_chunks,
-      reinterpret_cast<int*>(base + p->off2), p->nstages, p->stage_bytes);
+  auto* members = reinterpret_cast<const GemmMember*>(base + p->off0);
+  auto* chunks = reinterpret_cast<const uint4*>(base + p->off1);
+  int* counters = reinterpret_cast<int*>(base + p->off2);
+  if (p->ncta == 2) {
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = p->grid; cfg.blockDim = p->block; cfg.dynamicSmemBytes = p->smem; cfg.stream = s;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeClusterDimension;
+    attr[0].val.clusterDim.x = 2; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
+    cfg.attrs = attr; cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, grouped_gemm_sm100_kernel<2>, members, chunks, (int)p->n_chunks, counters,
+                              (int)p->nstages, (int)p->stage_bytes);
+  }
+  grouped_gemm_sm100_kernel<1><<<p->grid, p->block, p->smem, s>>>(members, chunks, p->n_chunks, counters, p->nstages,
+                                                                 p->stage_bytes);
   return cudaGetLastError();
 }
 
@@ -610,6 +719,10 @@ extern "C" opt_status opt_linear_plan_create(const opt_linear_member* members, i
   if (opt_status st = get_encoder(&enc)) { delete p; return st; }
   std::vector<GemmMember> tab(n);
   memset(tab.data(), 0, tab.size() * sizeof(GemmMember));
+  // CTA pair (256-row tiles, W shared by the pair) or single CTA (128-row tiles)
+  int ncta = 2;
+  if (const char* e = getenv("OPT_GEMM_NCTA")) ncta = atoi(e) == 1 ? 1 : 2;                // experiment knob
+  const int tile_m = kBM * ncta;
   struct MemberTiling { int bn, nbn, nkb, klast; uint32_t idesc; };
   std::vector<MemberTiling> tiling(n);
   int max_bn = 16;
@@ -620,7 +733,8 @@ extern "C" opt_status opt_linear_plan_create(const opt_linear_member* members, i
     opt_status st;
     if ((st = encode_2d(enc, &t.tmA, m.x, m.M, m.K, m.ldx, kBK, kBM, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, "X", i)) ||
         (st = encode_2d(enc, &t.tmB, m.w, m.N, m.K, m.ldw, kBK, bn, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, "W", i)) ||
-        (st = encode_2d(enc, &t.tmY, m.y, m.M, m.N, m.ldy, 64, 32, CU_TENSOR_MAP_L2_PROMOTION_NONE, "Y", i))) {
+        (st = encode_2d(enc, &t.tmY, m.y, m.M, m.N, m.ldy, 64, 32, CU_TENSOR_MAP_L2_PROMOTION_NONE, "Y", i)) ||
+        (st = encode_2d(enc, &t.tmB2, m.w, m.N, m.K, m.ldw, kBK, bn / 2, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, "W/2", i))) {
       delete p;
       return st;
     }
@@ -629,9 +743,9 @@ extern "C" opt_status opt_linear_plan_create(const opt_linear_member* members, i
     tl.klast = (m.K - (tl.nkb - 1) * kBK + 15) / 16;
     // tcgen05 instruction descriptor, kind::f16: D fp32 (bits 4-5 = 1), A bf16 (bits 7-9 = 1), B bf16
     // (bits 10-12 = 1), A and B K-major (bits 15, 16 = 0), N>>3 at bits 17-22, M>>4 at bits 24-28.
-    tl.idesc = (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(bn >> 3) << 17) | ((uint32_t)(kBM >> 4) << 24);
+    tl.idesc = (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(bn >> 3) << 17) | ((uint32_t)(tile_m >> 4) << 24);
     max_bn = std::max(max_bn, bn);
-    const int nmb = (m.M + kBM - 1) / kBM;
+    const int nmb = (m.M + tile_m - 1) / tile_m;
     tiles += (int64_t)nmb * tl.nbn;
     if (tiles > INT32_MAX / 2) { delete p; return fail(OPT_ERR_UNSUPPORTED, "too many tiles"); }
   }
@@ -644,11 +758,11 @@ extern "C" opt_status opt_linear_plan_create(const opt_linear_member* members, i
   for (int32_t i = 0; i < n; ++i) {
     const opt_linear_member& m = members[i];
     const MemberTiling& tl = tiling[i];
-    const int nmb = (m.M + kBM - 1) / kBM;
+    const int nmb = (m.M + tile_m - 1) / tile_m;
     for (int mb = 0; mb < nmb; ++mb)
       for (int nb = 0; nb < tl.nbn; ++nb) {
         TileEntry e;
-        e.member = i; e.m0 = mb * kBM; e.n0 = nb * tl.bn; e.idesc = tl.idesc;
+        e.member = i; e.m0 = mb * tile_m; e.n0 = nb * tl.bn; e.idesc = tl.idesc;
         e.bn_nkb = (uint32_t)tl.bn | ((uint32_t)tl.nkb << 16);
         e.misc = (uint32_t)tl.klast | ((uint32_t)m.act << 8) | ((uint32_t)std::min(tl.bn, m.N - e.n0) << 16);
         e.bias = m.bias ? static_cast<const char*>(m.bias) + (size_t)e.n0 * 2 : nullptr;
@@ -662,7 +776,8 @@ extern "C" opt_status opt_linear_plan_create(const opt_linear_member* members, i
   pad_entry.member = -1;
   size_t tail_waves = 3;
   if (const char* e = getenv("OPT_GEMM_TAIL_WAVES")) tail_waves = (size_t)atol(e);       // experiment knob
-  const size_t tail = std::min(flat.size(), tail_waves * num_sms);
+  const int n_sched = num_sms / ncta;                         // persistent CTAs (or CTA pairs)
+  const size_t tail = std::min(flat.size(), tail_waves * n_sched);
   const size_t body = flat.size() - tail;
   std::vector<TileEntry> chunked;
   // chunk c = tiles c, c+nC, c+2nC, c+3nC of the schedule order: CTAs that run side by side work on
@@ -681,7 +796,7 @@ extern "C" opt_status opt_linear_plan_create(const opt_linear_member* members, i
   }
   const int64_t n_chunks = (int64_t)(chunked.size() / kTilesPerChunk);
 
-  const int stage_bytes = kABytes + max_bn * kBK * 2;
+  const int stage_bytes = kABytes + max_bn / ncta * kBK * 2;
   const int nstages = std::min(kMaxStages, (kSmemMax - kSmemFixed) / stage_bytes);
   const int smem_bytes = nstages * stage_bytes + kSmemFixed;
   p->kind = kPlanLinearBf16;
@@ -693,12 +808,15 @@ extern "C" opt_status opt_linear_plan_create(const opt_linear_member* members, i
   memcpy(blob.data(), tab.data(), tab.size() * sizeof(GemmMember));
   memcpy(blob.data() + p->off1, chunked.data(), chunked.size() * sizeof(TileEntry));
   if (opt_status st = upload_tables(p, blob.data(), total)) { delete p; return st; }
-  cudaError_t e = cudaFuncSetAttribute(grouped_gemm_sm100_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemMax);
+  cudaError_t e = ncta == 2
+      ? cudaFuncSetAttribute(grouped_gemm_sm100_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemMax)
+      : cudaFuncSetAttribute(grouped_gemm_sm100_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemMax);
   if (e != cudaSuccess) {
     cudaFree(p->dev_tables); delete p;
     return fail(OPT_ERR_CUDA, "cudaFuncSetAttribute(max dynamic smem %d) failed: %s", kSmemMax, cudaGetErrorString(e));
   }
-  p->grid = dim3((unsigned)std::min<int64_t>(n_chunks, num_sms)); p->block = dim3(kGemmThreads); p->smem = smem_bytes;
+  p->grid = dim3((unsigned)(std::min<int64_t>(n_chunks, n_sched) * ncta)); p->block = dim3(kGemmThreads); p->smem = smem_bytes;
+  p->ncta = ncta;
   p->total_tiles = (int32_t)tiles;
   p->n_chunks = (int32_t)n_chunks; p->nstages = nstages; p->stage_bytes = stage_bytes;
   *plan = p;
