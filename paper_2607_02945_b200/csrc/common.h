@@ -66,7 +66,8 @@ struct opt_plan {
   size_t smem = 0;
   int32_t n_members = 0;
   int32_t total_tiles = 0;
-  int32_t n_chunks = 0, nstages = 0, stage_bytes = 0, ncta = 1;   // grouped GEMM: schedule chunks, smem ring shape
+  int32_t n_chunks = 0, nstages = 0, stage_bytes = 0, ncta = 1;
+  int32_t ln_tile_max = 0, ln_pmax = 0;                 // staged LayerNorm: bytes of a stage's row tile / of one parameter vector   // grouped GEMM: schedule chunks, smem ring shape
   int32_t io = 0, param = 0;
   int64_t flops = 0, bytes = 0;
 };

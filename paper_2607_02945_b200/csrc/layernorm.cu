@@ -19,6 +19,7 @@
 //     shared memory (a block never leaves its member).
 //   * a per-block table (member, first row, row count) maps blocks to members.
 #include <algorithm>
+#include <cstdlib>
 
 #include "common.h"
 
@@ -187,56 +188,122 @@ __device__ __forceinline__ uint32_t f2_to_bf2(f32x2 v) {
   return pack_bf16x2(lo, hi);
 }
 
-constexpr int kLnMaxD = 2048;        // gamma/beta staging: 2 x 8 KB of shared memory
+// ======================================================= bf16 staged path =====
+// Persistent CTAs (3 per SM), 8 consumer warps + 1 producer warp.  The producer takes work items (a
+// tile of ~16 KB of whole rows of one member) from a dynamic scheduler -- one atomic per chunk of 8
+// items -- and streams each tile plus the member's gamma/beta into a 4-stage shared-memory ring with
+// cp.async.bulk (one copy per tile when the rows are contiguous, one per row otherwise), counted on
+// the stage's mbarrier.  Consumers never issue a global load: they read their 16-byte vectors of the
+// row from shared memory, do the fp32 two-pass statistics with width-L shuffles on packed f32x2
+// arithmetic, and store y with 16-byte coalesced st.global.cs.  Bytes in flight are set by the ring
+// (3 x 4 x 16 KB per SM), not by registers.
+struct LnsMember {           // 64 bytes
+  const char* x; char* y; const char* gamma; const char* beta;
+  int64_t ldx16, ldy16;      // row strides in 16-byte vectors
+  int32_t nvec;              // D / 8
+  float eps, inv_D;
+  uint8_t l_log2, vpl, contiguous, pad;     // one 32-bit word: l_log2 | vpl << 8 | contiguous << 16
+};
+static_assert(sizeof(LnsMember) == 64, "LnsMember is one 64-byte record");
+struct LnsItem { int32_t member, row0, nrows, pad; };   // member < 0: padding entry of a chunk
 
-// bf16 in/out.  sg/sb: the member's gamma/beta as fp32 in shared memory.
-template <int VPL, int RU>
-__device__ __forceinline__ void ln_rows_bf16(const LnMember& m, int row0, int nrows, const float* sg, const float* sb) {
-  const int L = 1 << m.l_log2;
+constexpr int kLnsConsumers = 256;
+constexpr int kLnsThreads = kLnsConsumers + 32;
+constexpr int kLnsItemsPerChunk = 8;
+constexpr int kLnsMaxStages = 4;
+constexpr int kLnsHdrBytes = 64;
+constexpr int kLnsSmemBudget = 72 * 1024;      // per CTA: 3 CTAs per SM
+
+__device__ __forceinline__ uint32_t lns_smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void lns_mbar_wait(uint32_t bar, uint32_t parity) {
+  uint32_t done = 0;
+  for (uint32_t spin = 0; !done; ++spin) {
+    asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
+                 : "=r"(done) : "r"(bar), "r"(parity) : "memory");
+    if (spin > (1u << 26)) __trap();      // a protocol bug becomes a CUDA error, not a hang
+  }
+}
+__device__ __forceinline__ void lns_bulk_load(uint32_t dst, const void* src, uint32_t bytes, uint32_t bar) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+               ::"r"(dst), "l"(src), "r"(bytes), "r"(bar) : "memory");
+}
+__device__ __forceinline__ uint4 lns_lds128(uint32_t addr) {
+  uint4 v;
+  asm volatile("ld.shared.v4.b32 {%0, %1, %2, %3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "r"(addr) : "memory");
+  return v;
+}
+
+// gamma / beta vector `vec` (8 elements) of the staged parameters as four f32x2
+template <bool P_BF16>
+__device__ __forceinline__ void lns_param(uint32_t base, bool present, int vec, float dflt, f32x2 (&out)[4]) {
+  if (!present) {
+#pragma unroll
+    for (int k = 0; k < 4; ++k) out[k] = pk2(dflt, dflt);
+  } else if (P_BF16) {
+    const uint4 v = lns_lds128(base + vec * 16);
+    out[0] = bf2_to_f2(v.x); out[1] = bf2_to_f2(v.y); out[2] = bf2_to_f2(v.z); out[3] = bf2_to_f2(v.w);
+  } else {
+    const uint4 a = lns_lds128(base + vec * 32), b = lns_lds128(base + vec * 32 + 16);
+    out[0] = pk2(__uint_as_float(a.x), __uint_as_float(a.y)); out[1] = pk2(__uint_as_float(a.z), __uint_as_float(a.w));
+    out[2] = pk2(__uint_as_float(b.x), __uint_as_float(b.y)); out[3] = pk2(__uint_as_float(b.z), __uint_as_float(b.w));
+  }
+}
+
+struct LnsHdr {               // what the consumers need of a staged item (written by the producer)
+  int32_t member, row0, nrows, nvec;
+  char* y; int64_t ldy16;
+  float eps, inv_D; uint32_t shape;       // l_log2 | vpl << 8 | has_gamma << 16 | has_beta << 17
+  uint32_t pad[5];
+};
+static_assert(sizeof(LnsHdr) == kLnsHdrBytes, "LnsHdr is the 64-byte stage header");
+
+// FAST: every lane's vectors exist (D = 8 L VPL), the tile is whole passes, gamma and beta are present --
+// the common case, compiled without any predicate or branch in the loop body.
+template <bool P_BF16, int VPL, int RU, bool FAST>
+__device__ __forceinline__ void lns_tile(const LnsHdr& h, uint32_t tile, uint32_t sgamma, uint32_t sbeta) {
+  const int l_log2 = h.shape & 0xFF;
+  const bool has_g = FAST || ((h.shape >> 16) & 1), has_b = FAST || ((h.shape >> 17) & 1);
+  const int L = 1 << l_log2;
   const int lane_in_row = threadIdx.x & (L - 1);
-  const int row_in_pass = threadIdx.x >> m.l_log2;
-  const int rpp = kLnThreads >> m.l_log2;              // rows per pass of the block
-  const int niter = (nrows + rpp * RU - 1) / (rpp * RU);
-  const int4* xb = reinterpret_cast<const int4*>(m.x);
-  int4* yb = reinterpret_cast<int4*>(m.y);
-
+  const int row_in_pass = threadIdx.x >> l_log2;
+  const int rpp = kLnsConsumers >> l_log2;
+  const int niter = (h.nrows + rpp * RU - 1) / (rpp * RU);
+  const uint32_t row_bytes = (uint32_t)h.nvec * 16u;
+  int4* yb = reinterpret_cast<int4*>(h.y);
   bool act[VPL];
 #pragma unroll
-  for (int i = 0; i < VPL; ++i) act[i] = lane_in_row + i * L < m.nvec;
+  for (int i = 0; i < VPL; ++i) act[i] = FAST || lane_in_row + i * L < h.nvec;
 
-  int4 nxt[RU][VPL];
-  auto load = [&](int it, int4 (&dst)[RU][VPL]) {
-#pragma unroll
-    for (int u = 0; u < RU; ++u) {
-      const int r = (it * RU + u) * rpp + row_in_pass;
-      const int4* p = xb + (int64_t)(row0 + r) * m.ldx16 + lane_in_row;
-#pragma unroll
-      for (int i = 0; i < VPL; ++i) dst[u][i] = (r < nrows && act[i]) ? __ldcs(p + i * L) : make_int4(0, 0, 0, 0);
-    }
-  };
-  load(0, nxt);
-  for (int it = 0; it < niter; ++it) {
+  // this thread's first vector of the tile; rows advance by rpp per unrolled row, columns by L per vector
+  uint32_t xaddr = tile + (uint32_t)row_in_pass * row_bytes + (uint32_t)lane_in_row * 16u;
+  const uint32_t row_step = (uint32_t)rpp * row_bytes;
+  int4* yrow = yb + (int64_t)(h.row0 + row_in_pass) * h.ldy16 + lane_in_row;
+  const int64_t y_step = (int64_t)rpp * h.ldy16;
+  int rbase = row_in_pass;
+  for (int it = 0; it < niter; ++it, xaddr += RU * row_step, yrow += RU * y_step, rbase += RU * rpp) {
     f32x2 x[RU][VPL][4];
     float s[RU], q[RU];
 #pragma unroll
     for (int u = 0; u < RU; ++u) {
+      const bool rok = FAST || rbase + u * rpp < h.nrows;
       f32x2 acc = 0ull;
 #pragma unroll
       for (int i = 0; i < VPL; ++i) {
-        const uint32_t* w = reinterpret_cast<const uint32_t*>(&nxt[u][i]);
+        uint4 v = make_uint4(0, 0, 0, 0);
+        if (rok && act[i]) v = lns_lds128(xaddr + u * row_step + (uint32_t)(i * L) * 16u);
+        x[u][i][0] = bf2_to_f2(v.x); x[u][i][1] = bf2_to_f2(v.y); x[u][i][2] = bf2_to_f2(v.z); x[u][i][3] = bf2_to_f2(v.w);
 #pragma unroll
-        for (int k = 0; k < 4; ++k) { x[u][i][k] = bf2_to_f2(w[k]); acc = add2(acc, x[u][i][k]); }   // inactive vectors are zeros
+        for (int k = 0; k < 4; ++k) acc = add2(acc, x[u][i][k]);      // inactive vectors are zeros
       }
       s[u] = sum2(acc);
     }
-    load(it + 1, nxt);                                  // next rows in flight during this iteration's math
     for (int o = L >> 1; o > 0; o >>= 1) {
 #pragma unroll
       for (int u = 0; u < RU; ++u) s[u] += __shfl_xor_sync(0xffffffffu, s[u], o);
     }
 #pragma unroll
     for (int u = 0; u < RU; ++u) {
-      const float nmu = -s[u] * m.inv_D;
+      const float nmu = -s[u] * h.inv_D;
       const f32x2 nmu2 = pk2(nmu, nmu);
       f32x2 acc = 0ull;
 #pragma unroll
@@ -253,58 +320,209 @@ __device__ __forceinline__ void ln_rows_bf16(const LnMember& m, int row0, int nr
       for (int u = 0; u < RU; ++u) q[u] += __shfl_xor_sync(0xffffffffu, q[u], o);
     }
 #pragma unroll
-    for (int u = 0; u < RU; ++u) {
-      const float rstd = rsqrtf(q[u] * m.inv_D + m.eps);
-      const f32x2 rstd2 = pk2(rstd, rstd);
-      const int r = (it * RU + u) * rpp + row_in_pass;
-      if (r < nrows) {
-        int4* yp = yb + (int64_t)(row0 + r) * m.ldy16 + lane_in_row;
+    for (int i = 0; i < VPL; ++i) {
+      if (!act[i]) continue;
+      const int vec = lane_in_row + i * L;
+      f32x2 g[4], b[4];
+      lns_param<P_BF16>(sgamma, has_g, vec, 1.f, g);
+      lns_param<P_BF16>(sbeta, has_b, vec, 0.f, b);
 #pragma unroll
-        for (int i = 0; i < VPL; ++i) {
-          if (act[i]) {
-            const int vec = lane_in_row + i * L;
-            const ulonglong2 g0 = *reinterpret_cast<const ulonglong2*>(sg + vec * 8);
-            const ulonglong2 g1 = *reinterpret_cast<const ulonglong2*>(sg + vec * 8 + 4);
-            const ulonglong2 b0 = *reinterpret_cast<const ulonglong2*>(sb + vec * 8);
-            const ulonglong2 b1 = *reinterpret_cast<const ulonglong2*>(sb + vec * 8 + 4);
-            int4 o;
-            o.x = (int)f2_to_bf2(fma2(mul2(x[u][i][0], rstd2), g0.x, b0.x));
-            o.y = (int)f2_to_bf2(fma2(mul2(x[u][i][1], rstd2), g0.y, b0.y));
-            o.z = (int)f2_to_bf2(fma2(mul2(x[u][i][2], rstd2), g1.x, b1.x));
-            o.w = (int)f2_to_bf2(fma2(mul2(x[u][i][3], rstd2), g1.y, b1.y));
-            __stcs(yp + i * L, o);
-          }
-        }
+      for (int u = 0; u < RU; ++u) {
+        if (!FAST && rbase + u * rpp >= h.nrows) continue;
+        const float rstd = rsqrtf(q[u] * h.inv_D + h.eps);
+        const f32x2 rstd2 = pk2(rstd, rstd);
+        int4 o;
+        o.x = (int)f2_to_bf2(fma2(mul2(x[u][i][0], rstd2), g[0], b[0]));
+        o.y = (int)f2_to_bf2(fma2(mul2(x[u][i][1], rstd2), g[1], b[1]));
+        o.z = (int)f2_to_bf2(fma2(mul2(x[u][i][2], rstd2), g[2], b[2]));
+        o.w = (int)f2_to_bf2(fma2(mul2(x[u][i][3], rstd2), g[3], b[3]));
+        __stcs(yrow + u * y_step + i * L, o);
       }
     }
   }
 }
 
+// rows wider than 4 vectors per lane (D > 1024): the row stays in shared memory and is re-read per pass
 template <bool P_BF16>
-__global__ void __launch_bounds__(kLnThreads, 3)
-batched_layernorm_bf16_kernel(const LnMember* __restrict__ members, const LnBlock* __restrict__ blocks) {
-  __shared__ __align__(16) float sg[kLnMaxD];
-  __shared__ __align__(16) float sb[kLnMaxD];
-  const LnBlock b = blocks[blockIdx.x];
-  const LnMember m = members[b.member];
-  for (int v = threadIdx.x; v < m.nvec; v += kLnThreads) {     // gamma/beta -> fp32, once per block
-    float g[8], bt[8];
-    ln_load_param<true, P_BF16>(m.gamma, v, 1.f, g);
-    ln_load_param<true, P_BF16>(m.beta, v, 0.f, bt);
+__device__ __forceinline__ void lns_tile_wide(const LnsHdr& h, uint32_t tile, uint32_t sgamma, uint32_t sbeta) {
+  const bool has_g = (h.shape >> 16) & 1, has_b = (h.shape >> 17) & 1;
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const uint32_t row_bytes = (uint32_t)h.nvec * 16u;
+  int4* yb = reinterpret_cast<int4*>(h.y);
+  for (int r = warp; r < h.nrows; r += kLnsConsumers / 32) {
+    const uint32_t row = tile + (uint32_t)r * row_bytes;
+    f32x2 acc = 0ull;
+    for (int v = lane; v < h.nvec; v += 32) {
+      const uint4 w = lns_lds128(row + v * 16);
+      acc = add2(add2(acc, bf2_to_f2(w.x)), add2(bf2_to_f2(w.y), add2(bf2_to_f2(w.z), bf2_to_f2(w.w))));
+    }
+    float s = sum2(acc);
+    for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
+    const float nmu = -s * h.inv_D;
+    const f32x2 nmu2 = pk2(nmu, nmu);
+    acc = 0ull;
+    for (int v = lane; v < h.nvec; v += 32) {
+      const uint4 w = lns_lds128(row + v * 16);
+      const uint32_t ww[4] = {w.x, w.y, w.z, w.w};
 #pragma unroll
-    for (int e = 0; e < 8; ++e) { sg[v * 8 + e] = g[e]; sb[v * 8 + e] = bt[e]; }
+      for (int k = 0; k < 4; ++k) { const f32x2 d = add2(bf2_to_f2(ww[k]), nmu2); acc = fma2(d, d, acc); }
+    }
+    float q = sum2(acc);
+    for (int o = 16; o > 0; o >>= 1) q += __shfl_xor_sync(0xffffffffu, q, o);
+    const float rstd = rsqrtf(q * h.inv_D + h.eps);
+    const f32x2 rstd2 = pk2(rstd, rstd);
+    for (int v = lane; v < h.nvec; v += 32) {
+      const uint4 w = lns_lds128(row + v * 16);
+      const uint32_t ww[4] = {w.x, w.y, w.z, w.w};
+      f32x2 g[4], b[4];
+      lns_param<P_BF16>(sgamma, has_g, v, 1.f, g);
+      lns_param<P_BF16>(sbeta, has_b, v, 0.f, b);
+      uint32_t o[4];
+#pragma unroll
+      for (int k = 0; k < 4; ++k) o[k] = f2_to_bf2(fma2(mul2(add2(bf2_to_f2(ww[k]), nmu2), rstd2), g[k], b[k]));
+      __stcs(yb + (int64_t)(h.row0 + r) * h.ldy16 + v, make_int4((int)o[0], (int)o[1], (int)o[2], (int)o[3]));
+    }
+  }
+}
+
+// stage layout: [tile_max bytes of rows][gamma: pmax][beta: pmax][64-byte header]
+template <bool P_BF16>
+__global__ void __launch_bounds__(kLnsThreads, 3)
+batched_layernorm_staged_kernel(const LnsMember* __restrict__ members, const LnsItem* __restrict__ items, int n_chunks,
+                                int* __restrict__ counters, int nstages, int tile_max, int pmax) {
+  extern __shared__ __align__(128) uint8_t lns_smem[];
+  __shared__ __align__(8) uint64_t bars[2 * kLnsMaxStages];
+  const uint32_t sbase = lns_smem_u32(lns_smem);
+  const uint32_t stage_bytes = (uint32_t)(tile_max + 2 * pmax + kLnsHdrBytes);
+  auto full_bar = [&](int s) { return lns_smem_u32(&bars[s]); };
+  auto empty_bar = [&](int s) { return lns_smem_u32(&bars[kLnsMaxStages + s]); };
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  if (threadIdx.x == 0) {
+    for (int s = 0; s < nstages; ++s) {
+      asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(full_bar(s)));
+      asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(empty_bar(s)), "n"(kLnsConsumers / 32));
+    }
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   __syncthreads();
-  switch (m.vpl) {   // block-uniform; RU rows at a time so that RU x VPL ~ 4 vectors are in flight per thread
-    case 1: ln_rows_bf16<1, 4>(m, b.row0, b.nrows, sg, sb); break;
-    case 2: ln_rows_bf16<2, 2>(m, b.row0, b.nrows, sg, sb); break;
-    case 3: ln_rows_bf16<3, 1>(m, b.row0, b.nrows, sg, sb); break;
-    case 4: ln_rows_bf16<4, 1>(m, b.row0, b.nrows, sg, sb); break;
-    // D > 1024: the unpacked row would not fit the register budget; the generic path re-unpacks per pass
-    case 5: ln_block<true, P_BF16, 5>(m, b.row0, b.nrows); break;
-    case 6: ln_block<true, P_BF16, 6>(m, b.row0, b.nrows); break;
-    case 7: ln_block<true, P_BF16, 7>(m, b.row0, b.nrows); break;
-    default: ln_block<true, P_BF16, 8>(m, b.row0, b.nrows); break;
+
+  if (warp == kLnsConsumers / 32) {
+    // --------------------------------------------------------- producer ----
+    // Software pipeline over chunks so that no global latency sits between two items: while chunk n is
+    // issued, the member records of chunk n+1 (lane 4g+k holds 16-byte piece k of item g's member), the
+    // item line of chunk n+2 and the id of chunk n+3 are in flight.
+    int s = 0; uint32_t ph = 0;
+    auto fetch_id = [&]() { int v = 0; if (lane == 0) v = atomicAdd(counters, 1) + (int)gridDim.x; return v; };
+    auto load_line = [&](int cc) {
+      int4 v = make_int4(-1, 0, 0, 0);
+      if (lane < kLnsItemsPerChunk && cc < n_chunks) v = __ldg(reinterpret_cast<const int4*>(items) + (size_t)cc * kLnsItemsPerChunk + lane);
+      return v;
+    };
+    auto load_members = [&](const int4& line) {
+      const int mem = __shfl_sync(0xffffffffu, line.x, lane >> 2);
+      uint4 v = make_uint4(0, 0, 0, 0);
+      if (mem >= 0) v = __ldg(reinterpret_cast<const uint4*>(members + mem) + (lane & 3));
+      return v;
+    };
+    int c0 = blockIdx.x;
+    int4 line0 = load_line(c0);
+    int c1 = __shfl_sync(0xffffffffu, fetch_id(), 0);
+    int4 line1 = load_line(c1);
+    int c2 = fetch_id();
+    uint4 mv0 = load_members(line0);
+    while (c0 < n_chunks) {
+      c2 = __shfl_sync(0xffffffffu, c2, 0);
+      const uint4 mv1 = load_members(line1);
+      const int4 line2 = load_line(c2);
+      const int c3 = fetch_id();
+#pragma unroll 1
+      for (int g = 0; g < kLnsItemsPerChunk; ++g) {
+        const int member = __shfl_sync(0xffffffffu, line0.x, g);
+        if (member < 0) continue;      // warp-uniform
+        const int row0 = __shfl_sync(0xffffffffu, line0.y, g), nrows = __shfl_sync(0xffffffffu, line0.z, g);
+        auto piece = [&](uint32_t w, int k) { return __shfl_sync(0xffffffffu, w, 4 * g + k); };
+        auto ptr64 = [](uint32_t lo, uint32_t hi) { return ((uint64_t)hi << 32) | lo; };
+        LnsMember m;
+        m.x = reinterpret_cast<const char*>(ptr64(piece(mv0.x, 0), piece(mv0.y, 0)));
+        m.y = reinterpret_cast<char*>(ptr64(piece(mv0.z, 0), piece(mv0.w, 0)));
+        m.gamma = reinterpret_cast<const char*>(ptr64(piece(mv0.x, 1), piece(mv0.y, 1)));
+        m.beta = reinterpret_cast<const char*>(ptr64(piece(mv0.z, 1), piece(mv0.w, 1)));
+        m.ldx16 = (int64_t)ptr64(piece(mv0.x, 2), piece(mv0.y, 2));
+        m.ldy16 = (int64_t)ptr64(piece(mv0.z, 2), piece(mv0.w, 2));
+        m.nvec = (int)piece(mv0.x, 3); m.eps = __uint_as_float(piece(mv0.y, 3)); m.inv_D = __uint_as_float(piece(mv0.z, 3));
+        const uint32_t shp = piece(mv0.w, 3);                    // l_log2 | vpl << 8 | contiguous << 16
+        m.l_log2 = (uint8_t)(shp & 0xFF); m.vpl = (uint8_t)((shp >> 8) & 0xFF); m.contiguous = (uint8_t)((shp >> 16) & 0xFF);
+        const uint32_t row_bytes = (uint32_t)m.nvec * 16u;
+        const uint32_t pbytes = (uint32_t)m.nvec * (P_BF16 ? 16u : 32u);
+        lns_mbar_wait(empty_bar(s), ph ^ 1);
+        const uint32_t stage = sbase + (uint32_t)s * stage_bytes;
+        const uint32_t fb = full_bar(s);
+        if (lane == 0) {
+          const uint32_t ha = stage + (uint32_t)(tile_max + 2 * pmax);
+          const uint32_t shape = (uint32_t)m.l_log2 | ((uint32_t)m.vpl << 8) | ((m.gamma != nullptr) << 16) | ((m.beta != nullptr) << 17);
+          const uint64_t yp = reinterpret_cast<uint64_t>(m.y);
+          asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(ha), "r"(member), "r"(row0), "r"(nrows), "r"(m.nvec) : "memory");
+          asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(ha + 16), "r"((uint32_t)yp), "r"((uint32_t)(yp >> 32)),
+                       "r"((uint32_t)m.ldy16), "r"((uint32_t)((uint64_t)m.ldy16 >> 32)) : "memory");
+          asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(ha + 32), "r"(__float_as_uint(m.eps)), "r"(__float_as_uint(m.inv_D)),
+                       "r"(shape), "r"(0) : "memory");
+          const uint32_t tx = (uint32_t)nrows * row_bytes + (m.gamma ? pbytes : 0u) + (m.beta ? pbytes : 0u);
+          asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(fb), "r"(tx) : "memory");
+          if (m.gamma) lns_bulk_load(stage + tile_max, m.gamma, pbytes, fb);
+          if (m.beta) lns_bulk_load(stage + tile_max + pmax, m.beta, pbytes, fb);
+          if (m.contiguous) lns_bulk_load(stage, m.x + (int64_t)row0 * m.ldx16 * 16, (uint32_t)nrows * row_bytes, fb);
+        }
+        if (!m.contiguous)
+          for (int r = lane; r < nrows; r += 32)
+            lns_bulk_load(stage + (uint32_t)r * row_bytes, m.x + (int64_t)(row0 + r) * m.ldx16 * 16, row_bytes, fb);
+        if (++s == nstages) { s = 0; ph ^= 1; }
+      }
+      c0 = c1; line0 = line1; mv0 = mv1;
+      c1 = c2; line1 = line2;
+      c2 = c3;
+    }
+    asm volatile("" ::"r"(c2) : "memory");     // the last id fetch has returned before the counters are re-armed
+    // end marker; the last CTA to finish re-arms the scheduler counters for the next launch of the plan
+    lns_mbar_wait(empty_bar(s), ph ^ 1);
+    if (lane == 0) {
+      asm volatile("st.shared.b32 [%0], %1;" ::"r"(sbase + (uint32_t)s * stage_bytes + (uint32_t)(tile_max + 2 * pmax)), "r"(-1) : "memory");
+      asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(full_bar(s)) : "memory");
+      __threadfence();
+      if (atomicAdd(counters + 1, 1) == (int)gridDim.x - 1) { counters[0] = 0; counters[1] = 0; __threadfence(); }
+    }
+  } else {
+    // -------------------------------------------------------- consumers ----
+    int s = 0; uint32_t ph = 0;
+    for (;;) {
+      lns_mbar_wait(full_bar(s), ph);
+      const uint32_t ha = sbase + (uint32_t)s * stage_bytes + (uint32_t)(tile_max + 2 * pmax);
+      const uint4 h0 = lns_lds128(ha), h1 = lns_lds128(ha + 16), h2 = lns_lds128(ha + 32);
+      LnsHdr h;                                   // field by field: stays in registers
+      h.member = (int)h0.x; h.row0 = (int)h0.y; h.nrows = (int)h0.z; h.nvec = (int)h0.w;
+      h.y = reinterpret_cast<char*>(((uint64_t)h1.y << 32) | h1.x);
+      h.ldy16 = (int64_t)(((uint64_t)h1.w << 32) | h1.z);
+      h.eps = __uint_as_float(h2.x); h.inv_D = __uint_as_float(h2.y); h.shape = h2.z;
+      if (h.member < 0) break;
+      const uint32_t tile = sbase + (uint32_t)s * stage_bytes;
+      const uint32_t sg = tile + tile_max, sb = sg + pmax;
+      const int vpl = (h.shape >> 8) & 0xFF, ll = h.shape & 0xFF;
+      const int ru = vpl == 1 ? 4 : vpl == 2 ? 2 : 1;
+      const bool fast = (h.shape >> 16) == 3u && h.nvec == (vpl << ll) && h.nrows % ((kLnsConsumers >> ll) * ru) == 0;
+      switch (fast ? vpl : vpl + 8) {   // CTA-uniform
+        case 1: lns_tile<P_BF16, 1, 4, true>(h, tile, sg, sb); break;
+        case 2: lns_tile<P_BF16, 2, 2, true>(h, tile, sg, sb); break;
+        case 3: lns_tile<P_BF16, 3, 1, true>(h, tile, sg, sb); break;
+        case 4: lns_tile<P_BF16, 4, 1, true>(h, tile, sg, sb); break;
+        case 9: lns_tile<P_BF16, 1, 4, false>(h, tile, sg, sb); break;
+        case 10: lns_tile<P_BF16, 2, 2, false>(h, tile, sg, sb); break;
+        case 11: lns_tile<P_BF16, 3, 1, false>(h, tile, sg, sb); break;
+        case 12: lns_tile<P_BF16, 4, 1, false>(h, tile, sg, sb); break;
+        default: lns_tile_wide<P_BF16>(h, tile, sg, sb); break;
+      }
+      __syncwarp();
+      if (lane == 0) asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(empty_bar(s)) : "memory");
+      if (++s == nstages) { s = 0; ph ^= 1; }
+    }
   }
 }
 
@@ -326,13 +544,23 @@ batched_layernorm_kernel(const LnMember* __restrict__ members, const LnBlock* __
 }
 
 cudaError_t launch_layernorm(const opt_plan* p, cudaStream_t s) {
-  const char* base = static_cast<const char*>(p->dev_tables);
+  char* base = static_cast<char*>(p->dev_tables);
+  const bool io_bf16 = p->io == OPT_BF16, p_bf16 = p->param == OPT_BF16;
+  if (io_bf16) {
+    auto* members = reinterpret_cast<const LnsMember*>(base + p->off0);
+    auto* items = reinterpret_cast<const LnsItem*>(base + p->off1);
+    int* counters = reinterpret_cast<int*>(base + p->off2);
+    if (p_bf16)
+      batched_layernorm_staged_kernel<true><<<p->grid, p->block, p->smem, s>>>(members, items, p->n_chunks, counters, p->nstages,
+                                                                              p->ln_tile_max, p->ln_pmax);
+    else
+      batched_layernorm_staged_kernel<false><<<p->grid, p->block, p->smem, s>>>(members, items, p->n_chunks, counters, p->nstages,
+                                                                               p->ln_tile_max, p->ln_pmax);
+    return cudaGetLastError();
+  }
   auto* members = reinterpret_cast<const LnMember*>(base + p->off0);
   auto* blocks = reinterpret_cast<const LnBlock*>(base + p->off1);
-  const bool io_bf16 = p->io == OPT_BF16, p_bf16 = p->param == OPT_BF16;
-  if (io_bf16 && p_bf16) batched_layernorm_bf16_kernel<true><<<p->grid, p->block, 0, s>>>(members, blocks);
-  else if (io_bf16) batched_layernorm_bf16_kernel<false><<<p->grid, p->block, 0, s>>>(members, blocks);
-  else if (p_bf16) batched_layernorm_kernel<false, true><<<p->grid, p->block, 0, s>>>(members, blocks);
+  if (p_bf16) batched_layernorm_kernel<false, true><<<p->grid, p->block, 0, s>>>(members, blocks);
   else batched_layernorm_kernel<false, false><<<p->grid, p->block, 0, s>>>(members, blocks);
   return cudaGetLastError();
 }
@@ -352,6 +580,9 @@ extern "C" opt_status opt_layernorm_plan_create(const opt_layernorm_member* memb
   std::vector<Region> regions;
   std::vector<LnMember> tab;
   std::vector<LnBlock> blocks;
+  std::vector<LnsMember> stab;      // bf16 staged path
+  std::vector<LnsItem> sitems;
+  int64_t tile_max = 0, pmax = 0;
   int64_t bytes = 0;
   for (int32_t i = 0; i < n; ++i) {
     const opt_layernorm_member& m = members[i];
@@ -384,6 +615,25 @@ extern "C" opt_status opt_layernorm_plan_create(const opt_layernorm_member* memb
       const long score = waste * 1000 / nvec * 16 + (vpl < 2 ? 8 : vpl > 4 ? 4 : 0) + (5 - ll);
       if (score < best_score) { best_score = score; best_l = ll; best_vpl = vpl; }
     }
+    if (io == OPT_BF16) {
+      LnsMember t;
+      t.x = (const char*)m.x; t.y = (char*)m.y; t.gamma = (const char*)m.gamma; t.beta = (const char*)m.beta;
+      t.ldx16 = m.ldx / V; t.ldy16 = m.ldy / V; t.nvec = nvec; t.eps = m.eps; t.inv_D = 1.0f / (float)m.D;
+      t.l_log2 = (uint8_t)best_l; t.vpl = (uint8_t)best_vpl; t.contiguous = (m.rows == 1 || m.ldx == m.D); t.pad = 0;
+      stab.push_back(t);
+      // work items: whole rows, ~16 KB, a multiple of what one pass of the CTA covers
+      const int64_t row_bytes = (int64_t)nvec * 16;
+      const int rpp = kLnsConsumers >> best_l;
+      const int unit = best_vpl > 4 ? kLnsConsumers / 32 : rpp * (best_vpl == 1 ? 4 : best_vpl == 2 ? 2 : 1);
+      int64_t R = std::max<int64_t>(1, 16384 / row_bytes);
+      if (R >= unit) R = R / unit * unit;
+      R = std::min<int64_t>(R, m.rows);
+      tile_max = std::max<int64_t>(tile_max, R * row_bytes);
+      pmax = std::max<int64_t>(pmax, (int64_t)nvec * (param == OPT_BF16 ? 16 : 32));
+      for (int64_t r0 = 0; r0 < m.rows; r0 += R)
+        sitems.push_back({i, (int32_t)r0, (int32_t)std::min<int64_t>(R, m.rows - r0), 0});
+      continue;
+    }
     LnMember t;
     t.x = (const char*)m.x; t.y = (char*)m.y; t.gamma = (const char*)m.gamma; t.beta = (const char*)m.beta;
     t.ldx16 = m.ldx / V; t.ldy16 = m.ldy / V; t.rows = m.rows; t.nvec = nvec;
@@ -404,6 +654,53 @@ extern "C" opt_status opt_layernorm_plan_create(const opt_layernorm_member* memb
   auto align_up = [](size_t x) { return (x + 255) & ~size_t(255); };
   opt_plan* p = new opt_plan();
   p->kind = kPlanLayerNorm; p->device = device; p->io = io; p->param = param; p->n_members = n;
+  p->bytes = bytes; p->flops = 0;
+  if (io == OPT_BF16) {
+    // ring shape: stage = row tile + gamma + beta + header; as many stages (<= 4) as fit 72 KB (3 CTAs per SM)
+    tile_max = (tile_max + 127) & ~int64_t(127);
+    pmax = (pmax + 127) & ~int64_t(127);
+    const int64_t stage_bytes = tile_max + 2 * pmax + kLnsHdrBytes;
+    const int nstages = (int)std::min<int64_t>(kLnsMaxStages, kLnsSmemBudget / stage_bytes);
+    if (nstages < 2) { delete p; return fail(OPT_ERR_UNSUPPORTED, "LayerNorm rows too wide for the shared-memory ring"); }
+    const int n_cta = num_sms * 3;
+    // chunks of 8 consecutive items (one 128-byte table line, one atomic); the last 4 waves one item per chunk
+    const LnsItem pad_item = {-1, 0, 0, 0};
+    size_t tail_waves = 4;
+    if (const char* e = getenv("OPT_LN_TAIL_WAVES")) tail_waves = (size_t)atol(e);          // experiment knob
+    const size_t tail = std::min(sitems.size(), tail_waves * n_cta);
+    const size_t body = sitems.size() - tail;
+    std::vector<LnsItem> chunked;
+    for (size_t k = 0; k < body; k += kLnsItemsPerChunk)
+      for (int g = 0; g < kLnsItemsPerChunk; ++g) chunked.push_back(k + g < body ? sitems[k + g] : pad_item);
+    for (size_t k = body; k < sitems.size(); ++k) {
+      chunked.push_back(sitems[k]);
+      for (int g = 1; g < kLnsItemsPerChunk; ++g) chunked.push_back(pad_item);
+    }
+    const int64_t n_chunks = (int64_t)(chunked.size() / kLnsItemsPerChunk);
+    p->off0 = 0;
+    p->off1 = align_up(stab.size() * sizeof(LnsMember));
+    p->off2 = p->off1 + align_up(chunked.size() * sizeof(LnsItem));
+    const size_t total = p->off2 + 256;                        // scheduler counters, zero-initialised
+    std::vector<char> blob(total, 0);
+    memcpy(blob.data(), stab.data(), stab.size() * sizeof(LnsMember));
+    memcpy(blob.data() + p->off1, chunked.data(), chunked.size() * sizeof(LnsItem));
+    if (opt_status st = upload_tables(p, blob.data(), total)) { delete p; return st; }
+    const int smem = (int)(nstages * stage_bytes);
+    cudaError_t e = param == OPT_BF16
+        ? cudaFuncSetAttribute(batched_layernorm_staged_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem)
+        : cudaFuncSetAttribute(batched_layernorm_staged_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+    if (e != cudaSuccess) {
+      cudaFree(p->dev_tables); delete p;
+      return fail(OPT_ERR_CUDA, "cudaFuncSetAttribute(max dynamic smem %d) failed: %s", smem, cudaGetErrorString(e));
+    }
+    p->grid = dim3((unsigned)std::min<int64_t>(n_chunks, n_cta));
+    p->block = dim3(kLnsThreads);
+    p->smem = (size_t)smem;
+    p->total_tiles = (int32_t)sitems.size();
+    p->n_chunks = (int32_t)n_chunks; p->nstages = nstages; p->ln_tile_max = (int32_t)tile_max; p->ln_pmax = (int32_t)pmax;
+    *plan = p;
+    return OPT_OK;
+  }
   p->off0 = 0;
   p->off1 = align_up(tab.size() * sizeof(LnMember));
   const size_t total = p->off1 + align_up(blocks.size() * sizeof(LnBlock));
