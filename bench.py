@@ -43,6 +43,11 @@ SMALL = dict(c1_rows=256, c1_n=16, c2_M=512, c2_n=16, c3_rows=512, c3_width=2048
              c4_B=512, c4_n=24)
 
 
+# dram__bytes_read.sum + dram__bytes_write.sum of the three grouped-GEMM launches of one step (C2, C4b, C4c), from
+# the committed `ncu --set full` capture profiles/r01_profiles.md section 2 (algorithmic: 7 912 453 120 bytes)
+GEMM_DRAM_TRAFFIC_PER_STEP = 7_855_398_000
+
+
 def load_peaks():
     p = os.path.join(ROOT, "MEASURED_PEAKS.json")
     if os.path.exists(p):
@@ -239,6 +244,111 @@ class Step:
 
     def d2h_bytes(self):
         return sum(g.aout.size for g in self.groups)
+
+
+# ------------------------------------------- one-launch-per-op baseline ------
+class Unfused:
+    """The same groups executed the way the unfused graph runs them: ONE launch per op, through
+    single-member plans of the same library (SURVEY.md 8(d) "Baseline"): Linear and its activation are two
+    launches, split->f->cat is one launch per chunk plus the cat copy.  Same inputs, same outputs."""
+
+    def __init__(self, step):
+        ob, torch = step.ob, step.torch
+        self.seq = {}
+        self.keep = []
+        dev = step.dev_index
+        PW_RELU, PW_COPY = 1, 0
+        for g in step.groups:
+            plans = []
+            if g.name.startswith("C1"):
+                for (ix, ig, ib, iy), m in zip(g.idx, g.cfg["members"]):
+                    d = ob.layernorm_member(g.ain.tensor(ix), g.aout.tensor(iy), g.ain.tensor(ig), g.ain.tensor(ib), m["eps"])
+                    plans.append(ob.opt_layernorm_plan_create([d], BF16, BF16, dev))
+            elif g.name.startswith("C2"):
+                ycat = g.aout.tensor(g.iy)
+                for (ix, iw, ib), m in zip(g.idx, g.cfg["members"]):
+                    y = ycat[:, m["col_off"]:m["col_off"] + m["N"]]
+                    plans.append(ob.opt_linear_plan_create(
+                        [ob.linear_member(g.ain.tensor(ix), g.ain.tensor(iw), g.ain.tensor(ib), y, ACT_NONE)], BF16, dev))
+                    plans.append(ob.opt_pointwise_plan_create([ob.chunk(y, y, PW_RELU)], BF16, dev))
+            elif g.name.startswith("C3"):
+                x, out = g.ain.tensor(g.ix), g.aout.tensor(g.iy)
+                cfg = g.cfg
+                starts = np.concatenate(([0], np.cumsum(cfg["widths"])))
+                tmp, cat, d = [], [], 0
+                for p in cfg["perm"]:
+                    w = cfg["widths"][p]
+                    t = torch.empty((x.shape[0], w), dtype=x.dtype, device=x.device)
+                    tmp.append(t)
+                    plans.append(ob.opt_pointwise_plan_create([ob.chunk(x[:, starts[p]:starts[p] + w], t, cfg["ops"][p])], BF16, dev))
+                    cat.append(ob.chunk(t, out[:, d:d + w], PW_COPY))
+                    d += w
+                plans.append(ob.opt_pointwise_plan_create(cat, BF16, dev))
+                self.keep.append(tmp)
+            elif g.name.startswith("C4a"):
+                T, A = g.ain.tensor, g.amid.tensor
+                out = g.aout if g.aout.size else None
+                tw = g.cfg["towers"]
+                final = step.groups[-1].aout.tensor(g.iy)
+                outs, cat = [], []
+                for k, (i, t) in enumerate(zip(g.idx, tw)):
+                    plans.append(ob.opt_layernorm_plan_create(
+                        [ob.layernorm_member(T(i["x"]), A(i["xn"]), T(i["gamma"]), T(i["beta"]), t["eps"])], BF16, BF16, dev))
+                for k, (i, t) in enumerate(zip(g.idx, tw)):
+                    plans.append(ob.opt_linear_plan_create([ob.linear_member(A(i["xn"]), T(i["w1"]), T(i["b1"]), A(i["h"]), ACT_NONE)], BF16, dev))
+                    plans.append(ob.opt_pointwise_plan_create([ob.chunk(A(i["h"]), A(i["h"]), PW_RELU)], BF16, dev))
+                for k, (i, t) in enumerate(zip(g.idx, tw)):
+                    o = torch.empty((t["B"], t["out"]), dtype=final.dtype, device=final.device)
+                    outs.append(o)
+                    plans.append(ob.opt_linear_plan_create([ob.linear_member(A(i["h"]), T(i["w2"]), T(i["b2"]), o, ACT_NONE)], BF16, dev))
+                    cat.append(ob.chunk(o, final[:, k * t["out"]:(k + 1) * t["out"]], PW_COPY))
+                plans.append(ob.opt_pointwise_plan_create(cat, BF16, dev))
+                self.keep.append(outs)
+                self.seq["C4_recsys_block"] = plans
+                continue
+            else:
+                continue
+            self.seq[g.name] = plans
+
+    def time(self, torch, reps=3):
+        """-> {group: dict(launches, eager_us, graph_us)}: eager = launches issued one by one from the host
+        (what an unfused graph pays); graph = the same sequence replayed as one CUDA graph (GPU-side cost only)."""
+        res = {}
+        st = torch.cuda.current_stream()
+        for name, plans in self.seq.items():
+            for p in plans:
+                p.launch()
+            torch.cuda.synchronize()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(st)
+            for _ in range(reps):
+                for p in plans:
+                    p.launch()
+            e1.record(st)
+            torch.cuda.synchronize()
+            eager = e0.elapsed_time(e1) * 1e3 / reps
+            graph_us = None
+            try:
+                gr = torch.cuda.CUDAGraph()
+                cs = torch.cuda.Stream()
+                cs.wait_stream(st)
+                with torch.cuda.graph(gr, stream=cs):
+                    for p in plans:
+                        p.launch(cs.cuda_stream)
+                gr.replay()
+                torch.cuda.synchronize()
+                e0.record(st)
+                for _ in range(reps):
+                    gr.replay()
+                e1.record(st)
+                torch.cuda.synchronize()
+                graph_us = e0.elapsed_time(e1) * 1e3 / reps
+            except Exception as e:  # noqa: BLE001
+                graph_us = None
+                self.graph_error = repr(e)
+            res[name] = dict(launches=len(plans), eager_us=round(eager, 1), graph_us=None if graph_us is None else round(graph_us, 1))
+        return res
+
 
 
 # ------------------------------------------------------------- clock watch ---
@@ -450,6 +560,42 @@ def run_product(args):
     barrier()
     ms_e2e = f0.elapsed_time(f1)
 
+    # ---- (4) size-matched plain-copy reference for the HBM-bound groups: a device-to-device copy of the same
+    # number of bytes (half read, half written), cold L2, same event protocol.  Small groups cannot reach the
+    # large-copy peak whatever the kernel: launch ramp and tail are a fixed ~8 us.
+    copy_ref = {}
+    flush = torch.empty(256 * 1024 * 1024, dtype=torch.uint8, device=device)
+    for g in step.groups:
+        if g.kind == "linear" or args.profile:
+            continue
+        n = g.info["bytes"] // 2
+        a = torch.empty(n, dtype=torch.uint8, device=device)
+        b = torch.empty(n, dtype=torch.uint8, device=device)
+        b.copy_(a)
+        ts, tk = [], []
+        for _ in range(10):
+            flush.fill_(1)
+            c0, c1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            c0.record(stream); b.copy_(a); c1.record(stream)
+            torch.cuda.synchronize()
+            ts.append(c0.elapsed_time(c1) * 1e3)
+            flush.fill_(1)
+            c0, c1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            c0.record(stream); g.plan.launch(); c1.record(stream)
+            torch.cuda.synchronize()
+            tk.append(c0.elapsed_time(c1) * 1e3)
+        copy_ref[g.name] = (float(np.mean(ts)), float(np.mean(tk)))
+        del a, b
+    del flush
+
+    # ---- (5) one-launch-per-op baseline (same library, single-member plans), outside the timed step
+    unfused = None
+    if not args.no_unfused and not args.profile:
+        try:
+            unfused = Unfused(step).time(torch)
+        except Exception as e:  # noqa: BLE001
+            unfused = dict(error=repr(e))
+
     watch.stop_flag.set()
     watch.join(timeout=2)
 
@@ -472,6 +618,11 @@ def run_product(args):
                               frac_tensor=round(tfs / peaks["bf16_tflops"], 4) if fl else None,
                               roofline_us=round(max(t_hbm, t_tc), 2),
                               frac_roofline=round(max(t_hbm, t_tc) / us, 4))
+        if g.name in copy_ref:      # isolated, cold L2: this kernel next to torch's copy_ of the same byte count
+            cus, kus = copy_ref[g.name]
+            groups[g.name].update(isolated_cold_l2_us=round(kus, 2), same_size_copy_us=round(cus, 2),
+                                  frac_of_same_size_copy=round(cus / kus, 4),
+                                  isolated_frac_hbm=round(by / (kus * 1e-6) / 1e9 / peaks["hbm_gbs"], 4))
 
     # dominant kernel of the step = the grouped GEMM (3 of the 6 launches); over a step it is HBM-bound
     # (C4b/C4c at 85 and 52 flop/B; C2 sits on the ridge and is reported against tensor peak in "groups")
@@ -480,7 +631,8 @@ def run_product(args):
     gemm_us = sum(us for _, us in gemm)
     achieved = gemm_bytes / (gemm_us * 1e-6) / 1e9
     roofline = dict(bound="hbm", kernel="grouped_gemm_sm100_kernel", achieved=round(achieved, 1), peak=peaks["hbm_gbs"],
-                    unit="GB/s", frac=round(achieved / peaks["hbm_gbs"], 4), traffic=None,
+                    unit="GB/s", frac=round(achieved / peaks["hbm_gbs"], 4),
+                    traffic=GEMM_DRAM_TRAFFIC_PER_STEP if not args.small else None,
                     peak_source=peaks["source"] + ", burst copy figure",
                     launches_per_step=len(gemm), bytes_per_step=gemm_bytes, us_per_step=round(gemm_us, 2),
                     share_of_step=round(gemm_us / sum(per_group_us), 4))
@@ -505,10 +657,11 @@ def run_product(args):
                              "each step)"),
                 gpu_launches=int(launches), launches_per_step=ng,
                 clocks=watch.summary(), roofline=roofline, roofline_tensor=roofline_tensor, groups=groups,
+                unfused_baseline=unfused,
                 aggregate=dict(steps_per_s=round(aggregate_steps_per_s(us_step, world), 2)),
                 build_seconds=round(build_s, 1), lib=ob.opt_version())
 
-    if rank == 0 and not args.no_cpu and world >= 1:
+    if rank == 0 and not args.no_cpu and not args.profile and world >= 1:
         us, spent, desc, cores = oracle_sample_step(1.0 if not args.small else 0.25)
         line["cpu_baseline"] = dict(value=round(us, 1), unit="us", cores=cores, kind="oracle", sample=desc,
                                     cpu_seconds=round(spent, 2))
@@ -523,12 +676,15 @@ def run_product(args):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=30)
+    ap.add_argument("--steps", type=int, default=50)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="product", choices=["product", "reference"])
     ap.add_argument("--e2e-steps", type=int, default=5)
     ap.add_argument("--small", action="store_true", help="debug sizes (not a bench number)")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
+    ap.add_argument("--no-unfused", action="store_true", help="skip the one-launch-per-op baseline")
+    ap.add_argument("--profile", action="store_true",
+                    help="only the step's own launches (no cpu_baseline, no unfused baseline, no copy reference): for ncu")
     ap.add_argument("--ref-frac", type=float, default=0.0, help="reference arm: override the row-sample fraction")
     args = ap.parse_args()
     if args.impl == "reference":

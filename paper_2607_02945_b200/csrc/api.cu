@@ -41,13 +41,14 @@ opt_status open_device(int device, int* num_sms) {
                 e == cudaSuccess ? "device count is 0" : cudaGetErrorString(e));
   }
   if (device < 0 || device >= ndev) return fail(OPT_ERR_INVALID_ARG, "device %d out of range [0,%d)", device, ndev);
-  cudaDeviceProp prop;
-  OPT_CUDA_TRY(cudaGetDeviceProperties(&prop, device));
-  if (prop.major != 10)
-    return fail(OPT_ERR_NO_DEVICE, "device %d is sm_%d%d; liboptimus_b200 is built for sm_100a only", device,
-                prop.major, prop.minor);
+  int major = 0, minor = 0, sms = 0;
+  OPT_CUDA_TRY(cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, device));
+  OPT_CUDA_TRY(cudaDeviceGetAttribute(&minor, cudaDevAttrComputeCapabilityMinor, device));
+  OPT_CUDA_TRY(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, device));
+  if (major != 10)
+    return fail(OPT_ERR_NO_DEVICE, "device %d is sm_%d%d; liboptimus_b200 is built for sm_100a only", device, major, minor);
   OPT_CUDA_TRY(cudaSetDevice(device));
-  *num_sms = prop.multiProcessorCount;
+  *num_sms = sms;
   return OPT_OK;
 }
 

@@ -52,7 +52,7 @@ constexpr int kPwThreads = 256;
 constexpr int kPwUnroll = 8;
 constexpr int kFlatW = 256;          // vectors per row when a dense tensor is re-tiled
 constexpr int kVecPerBlock = 4096;   // ~64 KB read + 64 KB written per block
-constexpr int kStageBudget = 32 * 1024;   // STAGED mode: shared memory per block (source + destination rows)
+constexpr int kStageBudget = 100 * 1024;  // STAGED mode: at most this much shared memory per block (3 source rows + 2 destination rows)
 constexpr int kStageMaxSpan = 2048;       // STAGED mode: at most 32 KB per staged row
 constexpr int kStageMaxAvgChunk = 32;     // STAGED mode only when the average segment is < 512 bytes
 
@@ -94,65 +94,93 @@ __device__ __forceinline__ void pw_rows(const int4* __restrict__ s, int4* __rest
 
 __device__ __forceinline__ uint32_t pw_smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
 
-// STAGED mode: rows [r0, r0+nrows) of group g.  smem = nrows x src_span (+ nrows x dst_span) vectors.
-template <bool BF16, int OP>
-__device__ __forceinline__ void pw_staged_cols(const int4* sin, int4* sout, int4* gdst, const int2 m, int nrows,
-                                               int src_span, int dst_span, int64_t ldd16) {
-  const int so = m.x, dof = m.y & 0x3FFFFFFF;
-  if (sout != nullptr) {
-    for (int r = 0; r < nrows; ++r) sout[r * dst_span + dof] = pw_apply<BF16, OP>(sin[r * src_span + so]);
-  } else {
-    for (int r = 0; r < nrows; ++r) __stcs(gdst + (int64_t)r * ldd16 + dof, pw_apply<BF16, OP>(sin[r * src_span + so]));
+// STAGED mode: rows [r0, r0+nrows) of group g, software-pipelined inside the block.
+//   smem = kPwInStages source rows (ring) + 2 destination rows (double buffer, only when dst_span != 0).
+//   Thread 0 keeps kPwInStages-1 row loads (cp.async.bulk) in flight; every thread owns up to 4 virtual
+//   columns whose map entries live in registers for the whole block; per row: gather from the staged
+//   source row, apply, scatter into the staged destination row, which leaves with one bulk store.
+constexpr int kPwInStages = 3;
+
+template <bool BF16>
+__device__ __forceinline__ int4 pw_apply_rt(int4 v, int op) {
+  switch (op) {   // warp-uniform except at op boundaries of the virtual row
+    case OPT_PW_COPY: return v;
+    case OPT_PW_RELU: return pw_apply<BF16, OPT_PW_RELU>(v);
+    case OPT_PW_TANH: return pw_apply<BF16, OPT_PW_TANH>(v);
+    default:          return pw_apply<BF16, OPT_PW_SIGMOID>(v);
   }
 }
 
 template <bool BF16>
 __device__ __forceinline__ void pw_staged_tile(const PwGroup& g, const int2* __restrict__ vmap, int r0, int nrows) {
   extern __shared__ __align__(128) uint8_t pw_smem[];
-  __shared__ __align__(8) uint64_t bar_storage;
-  const uint32_t bar = pw_smem_u32(&bar_storage);
-  int4* sin = reinterpret_cast<int4*>(pw_smem);
-  int4* sout = g.dst_span ? sin + (size_t)g.tile_rows * g.src_span : nullptr;
-  const uint32_t row_bytes = (uint32_t)g.src_span * 16u;
+  __shared__ __align__(8) uint64_t bar_storage[kPwInStages];
+  const uint32_t in_bytes = (uint32_t)g.src_span * 16u, out_bytes = (uint32_t)g.dst_span * 16u;
+  const uint32_t sin0 = pw_smem_u32(pw_smem);
+  const uint32_t sout0 = sin0 + kPwInStages * in_bytes;
+  const bool staged_out = g.dst_span != 0;
+  auto bar = [&](int s) { return pw_smem_u32(&bar_storage[s]); };
+  auto load_row = [&](int r) {            // thread 0 only
+    const int s = r % kPwInStages;
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar(s)), "r"(in_bytes) : "memory");
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 ::"r"(sin0 + (uint32_t)s * in_bytes), "l"(g.src + ((int64_t)(r0 + r) * g.lds16) * 16), "r"(in_bytes), "r"(bar(s)) : "memory");
+  };
   if (threadIdx.x == 0) {
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(bar));
+    for (int s = 0; s < kPwInStages; ++s) asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(bar(s)));
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(row_bytes * (uint32_t)nrows) : "memory");
-    for (int r = 0; r < nrows; ++r)
-      asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
-                   ::"r"(pw_smem_u32(sin + (size_t)r * g.src_span)),
-                     "l"(g.src + ((int64_t)(r0 + r) * g.lds16) * 16), "r"(row_bytes), "r"(bar) : "memory");
+    for (int r = 0; r < kPwInStages - 1 && r < nrows; ++r) load_row(r);
   }
-  __syncthreads();                       // barrier initialised before anyone polls it
-  {
-    uint32_t done = 0;
-    while (!done)
-      asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], 0;\n\tselp.u32 %0, 1, 0, p;\n\t}"
-                   : "=r"(done) : "r"(bar) : "memory");
+  // this thread's map entries (up to 4 virtual columns), fetched while the first rows are in flight
+  constexpr int kPre = 4;
+  int2 pre[kPre];
+#pragma unroll
+  for (int k = 0; k < kPre; ++k) {
+    const int q = threadIdx.x + k * kPwThreads;
+    pre[k] = q < g.W ? __ldg(vmap + g.map_off + q) : make_int2(0, 0);
   }
-  int4* gdst = reinterpret_cast<int4*>(g.dst) + (int64_t)r0 * g.ldd16;
-  for (int q = threadIdx.x; q < g.W; q += kPwThreads) {
-    const int2 m = __ldg(vmap + g.map_off + q);
-    switch ((int)((uint32_t)m.y >> 30)) {   // warp-uniform except at op boundaries of the virtual row
-      case OPT_PW_COPY: pw_staged_cols<BF16, OPT_PW_COPY>(sin, sout, gdst, m, nrows, g.src_span, g.dst_span, g.ldd16); break;
-      case OPT_PW_RELU: pw_staged_cols<BF16, OPT_PW_RELU>(sin, sout, gdst, m, nrows, g.src_span, g.dst_span, g.ldd16); break;
-      case OPT_PW_TANH: pw_staged_cols<BF16, OPT_PW_TANH>(sin, sout, gdst, m, nrows, g.src_span, g.dst_span, g.ldd16); break;
-      default:          pw_staged_cols<BF16, OPT_PW_SIGMOID>(sin, sout, gdst, m, nrows, g.src_span, g.dst_span, g.ldd16); break;
+  __syncthreads();                       // barriers initialised before anyone polls them
+  for (int r = 0; r < nrows; ++r) {
+    const int s = r % kPwInStages;
+    const uint32_t parity = (uint32_t)(r / kPwInStages) & 1u;
+    {
+      uint32_t done = 0;
+      while (!done)
+        asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
+                     : "=r"(done) : "r"(bar(s)), "r"(parity) : "memory");
     }
-  }
-  if (sout != nullptr) {
-    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // st.shared results -> visible to the bulk-copy engine
-    __syncthreads();
-    if (threadIdx.x == 0) {
-      const uint32_t out_bytes = (uint32_t)g.dst_span * 16u;
-      for (int r = 0; r < nrows; ++r)
+    // the bulk store that last used this row's destination buffer (row r-2) has read it
+    if (staged_out && threadIdx.x == 0) asm volatile("cp.async.bulk.wait_group.read 1;" ::: "memory");
+    __syncthreads();                     // + every thread is done with source row r-1: its stage can be refilled
+    if (threadIdx.x == 0 && r + kPwInStages - 1 < nrows) load_row(r + kPwInStages - 1);
+    const uint32_t sin = sin0 + (uint32_t)s * in_bytes;
+    const uint32_t sout = sout0 + (uint32_t)(r & 1) * out_bytes;
+    int4* grow = reinterpret_cast<int4*>(g.dst) + (int64_t)(r0 + r) * g.ldd16;
+    auto column = [&](const int2 m) {
+      int4 v;
+      asm volatile("ld.shared.v4.b32 {%0, %1, %2, %3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "r"(sin + (uint32_t)m.x * 16u) : "memory");
+      v = pw_apply_rt<BF16>(v, (int)((uint32_t)m.y >> 30));
+      const uint32_t dof = (uint32_t)m.y & 0x3FFFFFFFu;
+      if (staged_out)
+        asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(sout + dof * 16u), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w) : "memory");
+      else
+        __stcs(grow + dof, v);
+    };
+#pragma unroll
+    for (int k = 0; k < kPre; ++k)
+      if (threadIdx.x + k * kPwThreads < g.W) column(pre[k]);
+    for (int q = threadIdx.x + kPre * kPwThreads; q < g.W; q += kPwThreads) column(__ldg(vmap + g.map_off + q));
+    if (staged_out) {
+      asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // st.shared results -> visible to the bulk-copy engine
+      __syncthreads();
+      if (threadIdx.x == 0) {
         asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;"
-                     ::"l"(g.dst + ((int64_t)(r0 + r) * g.ldd16) * 16), "r"(pw_smem_u32(sout + (size_t)r * g.dst_span)),
-                       "r"(out_bytes) : "memory");
-      asm volatile("cp.async.bulk.commit_group;" ::: "memory");
-      asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");   // smem must outlive the reads of the store
+                     ::"l"(g.dst + ((int64_t)(r0 + r) * g.ldd16) * 16), "r"(sout), "r"(out_bytes) : "memory");
+        asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+      }
     }
   }
+  if (staged_out && threadIdx.x == 0) asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");   // smem outlives the stores' reads
 }
 
 #ifndef PW_MINBLOCKS
@@ -255,6 +283,8 @@ extern "C" opt_status opt_pointwise_plan_create(const opt_chunk* chunks, int32_t
     }
   }
   if (opt_status st = check_independent(regions, /*allow_inplace_self=*/true)) return st;
+  int num_sms = 0;
+  if (opt_status st = open_device(device, &num_sms)) return st;
 
   // ---- group canonical chunks by (rows, lds16, ldd16)
   std::map<std::tuple<int32_t, int64_t, int64_t>, std::vector<int>> buckets;
@@ -265,7 +295,7 @@ extern "C" opt_status opt_pointwise_plan_create(const opt_chunk* chunks, int32_t
   std::vector<int2> vmap;
   std::vector<PwBlock> blocks;
   size_t smem_needed = 0;
-  int64_t stage_budget = kStageBudget;                       // experiment knob: OPT_PW_STAGE_KB=<KB per block>, 0 = direct mode only
+  int64_t stage_budget = kStageBudget;                       // experiment knob: OPT_PW_STAGE_KB=0 -> direct mode only
   if (const char* e = getenv("OPT_PW_STAGE_KB")) stage_budget = std::min<int64_t>(200, std::max<int64_t>(0, atol(e))) * 1024;
   for (auto& kv : buckets) {
     std::vector<int>& ids = kv.second;
@@ -323,9 +353,12 @@ extern "C" opt_status opt_pointwise_plan_create(const opt_chunk* chunks, int32_t
         // rows leave through a bulk store only if the chunks tile the destination span without holes
         // (otherwise the store would clobber bytes the group does not own) and nothing is in place
         if (dspan == W && dspan <= kStageMaxSpan && !self_inplace && !getenv("OPT_PW_NO_SOUT")) g.dst_span = (int32_t)dspan;
-        const int64_t per_row = (int64_t)(g.src_span + g.dst_span) * 16;
-        g.tile_rows = (int32_t)std::max<int64_t>(1, std::min<int64_t>(stage_budget / per_row, g.rows));
-        smem_needed = std::max<size_t>(smem_needed, (size_t)g.tile_rows * per_row);
+        // one wave of fat blocks: rows split evenly over the resident block slots (2 per SM), each block
+        // pipelines its rows through a 3-stage source ring and a double-buffered destination row
+        const int64_t need = ((int64_t)kPwInStages * g.src_span + 2 * (int64_t)g.dst_span) * 16;
+        const int64_t slots = 2 * (int64_t)num_sms;
+        g.tile_rows = (int32_t)std::max<int64_t>(std::min<int64_t>(4, g.rows), (g.rows + slots - 1) / slots);
+        smem_needed = std::max<size_t>(smem_needed, (size_t)need);
         for (int64_t r0 = 0; r0 < g.rows; r0 += g.tile_rows)
           blocks.push_back({(int32_t)groups.size(), 0, (int32_t)r0, (int32_t)std::min<int64_t>(g.tile_rows, g.rows - r0)});
         groups.push_back(g);
@@ -345,9 +378,6 @@ extern "C" opt_status opt_pointwise_plan_create(const opt_chunk* chunks, int32_t
     }
   }
   if (blocks.size() > (size_t)INT32_MAX) return fail(OPT_ERR_UNSUPPORTED, "too many work items");
-
-  int num_sms = 0;
-  if (opt_status st = open_device(device, &num_sms)) return st;
 
   auto align_up = [](size_t x) { return (x + 255) & ~size_t(255); };
   opt_plan* p = new opt_plan();
