@@ -40,6 +40,11 @@
  *   - opt_plan_launch is asynchronous on the given stream: exactly one kernel
  *     launch, no allocation, no synchronisation, no memcpy.  Results are
  *     bitwise reproducible run to run (no atomics on outputs, no split-K).
+ *   - A plan is single-flight: its device tables hold the work-scheduler
+ *     counters of the persistent kernels (re-armed by the kernel itself at the
+ *     end of every launch), so the same plan may be launched again and again,
+ *     back to back on one stream or as a CUDA-graph node, but must not run
+ *     concurrently with itself on two streams.  Different plans are independent.
  */
 #ifndef OPTIMUS_B200_H_
 #define OPTIMUS_B200_H_

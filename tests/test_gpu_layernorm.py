@@ -109,3 +109,24 @@ def test_unsupported_and_alias(ob):
     with pytest.raises(ob.OptError) as e:
         ob.opt_layernorm_plan_create([ob.layernorm_member(x[:, :60], y[:, :60], None, None, 1e-5)], BF16)
     assert e.value.status == ob.OPT_ERR_ALIGNMENT
+
+
+def test_relaunch_rearms_the_scheduler_and_is_bitwise_reproducible(ob):
+    cfg = wl.config1(seed=301, rows=777, n=40)
+    dev = []
+    for m in cfg["members"]:
+        dev.append((to_dev(m["x"], BF16), empty_dev(m["x"].shape, BF16, fill=float("nan")), to_dev(m["gamma"], BF16),
+                    to_dev(m["beta"], BF16)))
+    plan = ob.opt_layernorm_plan_create([ob.layernorm_member(x, y, g, b, m["eps"]) for (x, y, g, b), m in zip(dev, cfg["members"])], BF16)
+    ref = None
+    for it in range(4):
+        for d in dev:
+            d[1].fill_(float("nan"))
+        plan.launch()
+        torch.cuda.synchronize()
+        got = b"".join(to_host(d[1]).tobytes() for d in dev)
+        if ref is None:
+            ref = got
+            for d, m in zip(dev, cfg["members"]):
+                check_ln(to_host(d[1]), m)
+        assert got == ref
