@@ -65,3 +65,16 @@ def recsys_tower(t, dt=BF16):
     o64 = linear(h, t["w2"], t["b2"], dt)
     o = round_to_storage(o64, dt)
     return dict(ln=ln, h=h, out=o, ln64=ln64, h64=h64, out64=o64)
+
+
+def linear2(m, dt=BF16):
+    """Two chained Linear layers of one member, the unfused graph op by op ("chained
+    transformations", Fig. 5):
+        h = act1(x W1^T + b1)  -> rounded to the storage dtype (the intermediate tensor the unfused graph
+                                  materialises, reading Q3)
+        y = act2(h W2^T + b2)  -> rounded to the storage dtype
+    Returns dict(h64, h, y64, y); y64 is computed from the ROUNDED h."""
+    h64 = activation(linear(m["x"], m["w1"], m.get("b1"), dt), m["act1"])
+    h = round_to_storage(h64, dt)
+    y64 = activation(linear(h, m["w2"], m.get("b2"), dt), m["act2"])
+    return dict(h64=h64, h=h, y64=y64, y=round_to_storage(y64, dt))

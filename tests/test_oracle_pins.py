@@ -391,3 +391,39 @@ def test_workload_draws_are_reproducible_and_shaped():
     assert len(c3["widths"]) == 256 and sum(c3["widths"]) == 8192 and c3["x"].shape == (8192, 8192)
     xd = wl.f32_from_bf16_bits(c3["x"][:64]).astype(np.float64)
     assert abs(xd.var() - 2.0) < 0.05
+
+
+# ------------------------------------------------- linear2 --
+def test_linear2_small_integers_exact_and_rounding_point():
+    """Two chained Linear layers: with small integers every intermediate is an exactly representable
+    integer, so the chain must equal numpy's integer arithmetic bit for bit -- pins operand order, bias,
+    where the ReLU sits and that W2 multiplies the HIDDEN tensor (not x)."""
+    rng = np.random.default_rng(5)
+    M, K, H, N = 7, 16, 24, 8
+    x = rng.integers(-2, 3, (M, K)); w1 = rng.integers(-2, 3, (H, K)); b1 = rng.integers(-2, 3, (H,))
+    w2 = rng.integers(-1, 2, (N, H)); b2 = rng.integers(-2, 3, (N,))
+    h = np.maximum(x @ w1.T + b1, 0)                       # |h| <= 16*4+2 = 66: exact in bf16
+    y = h @ w2.T + b2                                      # |y| <= 24*66+2 < 2^11 but needs 8 bits: keep small
+    assert np.abs(y).max() < 256 * 8
+    m = dict(x=bf16(x), w1=bf16(w1), b1=bf16(b1), w2=bf16(w2), b2=bf16(b2), act1=1, act2=0)
+    r = graphs.linear2(m, BF16)
+    assert np.array_equal(r["h64"], h.astype(np.float64))
+    assert np.array_equal(wl.f32_from_bf16_bits(r["h"]), h.astype(np.float32))
+    assert np.array_equal(r["y64"], y.astype(np.float64))
+    # the hidden tensor is ROUNDED to bf16 before the second layer (reading Q3): 257 is not a bf16 value
+    m2 = dict(x=bf16([[1.0]]), w1=bf16([[257.0 - 1.0]]), b1=bf16([1.0]), w2=bf16([[1.0]]), b2=None, act1=0, act2=0)
+    r2 = graphs.linear2(m2, BF16)
+    assert r2["h64"][0, 0] == 257.0 and wl.f32_from_bf16_bits(r2["h"])[0, 0] == 256.0 and r2["y64"][0, 0] == 256.0
+
+
+def test_linear2_identity_second_layer_returns_hidden():
+    """W2 = I, b2 = 0, act2 = none: y equals the rounded hidden tensor bit for bit (and tanh hidden values
+    equal the oracle's own single-layer group, which P5/P8 pin separately)."""
+    H = 16
+    m = dict(x=wl.tensor_normal(9, 1, (5, 32), 0, 1, BF16), w1=wl.tensor_normal(9, 2, (H, 32), 0, 32 ** -0.5, BF16),
+             b1=wl.tensor_normal(9, 3, (H,), 0, 0.1, BF16), w2=bf16(np.eye(H)), b2=None, act1=2, act2=0)
+    r = graphs.linear2(m, BF16)
+    assert r["y"].tobytes() == r["h"].tobytes()
+    ref = np.tanh(wl.f32_from_bf16_bits(m["x"]).astype(np.float64) @ wl.f32_from_bf16_bits(m["w1"]).astype(np.float64).T
+                  + wl.f32_from_bf16_bits(m["b1"]).astype(np.float64))
+    assert np.allclose(r["h64"], ref, rtol=1e-13, atol=1e-15)
