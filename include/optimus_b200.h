@@ -90,6 +90,34 @@ typedef struct {
   int32_t act; /* opt_act */
 } opt_linear_member;
 
+/* One member of a grouped CHAINED Linear -- two Linear layers of a tower fused
+ * vertically, the hidden tensor never written to HBM ("chained
+ * transformations", Fig. 5; the paper finds horizontal + vertical fusion
+ * combined far better than either alone, Table 3):
+ *     h = act1(X * W1^T + b1)      rounded once to bf16 (the intermediate the
+ *                                  unfused graph materialises)
+ *     Y = act2(h * W2^T + b2)      rounded once to bf16
+ * X:[M,K] (ldx), W1:[H,K] (ldw1), b1:[H] or NULL, W2:[N,H] (ldw2), b2:[N] or
+ * NULL, Y:[M,N] (ldy; concat slot as for opt_linear_member).  bf16 only.
+ * On-chip limits: K <= 256, H <= 512, N <= 64; K % 8 == 0, H % 16 == 0,
+ * N % 16 == 0 (otherwise OPT_ERR_UNSUPPORTED / OPT_ERR_ALIGNMENT: run the two
+ * layers as two opt_linear groups).  The result equals, bit for bit, what two
+ * opt_linear groups produce with h stored in bf16 between them.              */
+typedef struct {
+  const void* x;
+  int64_t ldx;
+  const void* w1;
+  int64_t ldw1;
+  const void* b1;
+  const void* w2;
+  int64_t ldw2;
+  const void* b2;
+  void* y;
+  int64_t ldy;
+  int32_t M, K, H, N;
+  int32_t act1, act2; /* opt_act */
+} opt_linear2_member;
+
 /* One member of a batched LayerNorm -- batch_layernorm:
  *     mu = mean(x_r), v = mean((x_r - mu)^2)  (biased), over the last dim D
  *     y_r = (x_r - mu) / sqrt(v + eps) * gamma + beta
@@ -139,6 +167,8 @@ typedef struct opt_plan opt_plan; /* opaque; owns device-side tables only */
  * UNSUPPORTED are reported even on a machine without a GPU.                  */
 opt_status opt_linear_plan_create(const opt_linear_member* members, int32_t n, opt_dtype io,
                                   int device, opt_plan** plan);
+opt_status opt_linear2_plan_create(const opt_linear2_member* members, int32_t n, opt_dtype io,
+                                   int device, opt_plan** plan);
 opt_status opt_layernorm_plan_create(const opt_layernorm_member* members, int32_t n, opt_dtype io,
                                      opt_dtype param, int device, opt_plan** plan);
 opt_status opt_pointwise_plan_create(const opt_chunk* chunks, int32_t n, opt_dtype io, int device,

@@ -19,6 +19,13 @@ class opt_linear_member(C.Structure):
                 ("M", C.c_int32), ("N", C.c_int32), ("K", C.c_int32), ("act", C.c_int32)]
 
 
+class opt_linear2_member(C.Structure):
+    _fields_ = [("x", C.c_void_p), ("ldx", C.c_int64), ("w1", C.c_void_p), ("ldw1", C.c_int64), ("b1", C.c_void_p),
+                ("w2", C.c_void_p), ("ldw2", C.c_int64), ("b2", C.c_void_p), ("y", C.c_void_p), ("ldy", C.c_int64),
+                ("M", C.c_int32), ("K", C.c_int32), ("H", C.c_int32), ("N", C.c_int32),
+                ("act1", C.c_int32), ("act2", C.c_int32)]
+
+
 class opt_layernorm_member(C.Structure):
     _fields_ = [("x", C.c_void_p), ("ldx", C.c_int64), ("y", C.c_void_p), ("ldy", C.c_int64),
                 ("gamma", C.c_void_p), ("beta", C.c_void_p),
@@ -61,6 +68,7 @@ def lib():
         L = C.CDLL(_build.LIB)
         pp = C.POINTER(C.c_void_p)
         L.opt_linear_plan_create.argtypes = [C.POINTER(opt_linear_member), C.c_int32, C.c_int, C.c_int, pp]
+        L.opt_linear2_plan_create.argtypes = [C.POINTER(opt_linear2_member), C.c_int32, C.c_int, C.c_int, pp]
         L.opt_layernorm_plan_create.argtypes = [C.POINTER(opt_layernorm_member), C.c_int32, C.c_int, C.c_int,
                                                 C.c_int, pp]
         L.opt_pointwise_plan_create.argtypes = [C.POINTER(opt_chunk), C.c_int32, C.c_int, C.c_int, pp]
@@ -72,7 +80,7 @@ def lib():
         L.opt_last_error.restype = C.c_char_p
         L.opt_launch_count.restype = C.c_uint64
         L.opt_version.restype = C.c_char_p
-        for f in (L.opt_linear_plan_create, L.opt_layernorm_plan_create, L.opt_pointwise_plan_create,
+        for f in (L.opt_linear_plan_create, L.opt_linear2_plan_create, L.opt_layernorm_plan_create, L.opt_pointwise_plan_create,
                   L.opt_plan_launch, L.opt_plan_launch_host, L.opt_plan_info, L.opt_plan_destroy):
             f.restype = C.c_int
         _lib = L
@@ -137,6 +145,10 @@ def opt_linear_plan_create(members, io, device=0):
     return _create(lib().opt_linear_plan_create, opt_linear_member, members, io, device)
 
 
+def opt_linear2_plan_create(members, io, device=0):
+    return _create(lib().opt_linear2_plan_create, opt_linear2_member, members, io, device)
+
+
 def opt_layernorm_plan_create(members, io, param=None, device=0):
     return _create(lib().opt_layernorm_plan_create, opt_layernorm_member, members, io,
                    io if param is None else param, device)
@@ -186,6 +198,15 @@ def linear_member(x, w, bias, y, act=OPT_ACT_NONE):
     assert w.shape[1] == K and tuple(y.shape) == (M, N)
     return opt_linear_member(x.data_ptr(), _ld(x), w.data_ptr(), _ld(w),
                              None if bias is None else bias.data_ptr(), y.data_ptr(), _ld(y), M, N, K, int(act))
+
+
+def linear2_member(x, w1, b1, w2, b2, y, act1=OPT_ACT_RELU, act2=OPT_ACT_NONE):
+    M, K = x.shape
+    H, N = w1.shape[0], w2.shape[0]
+    assert w1.shape[1] == K and w2.shape[1] == H and tuple(y.shape) == (M, N)
+    return opt_linear2_member(x.data_ptr(), _ld(x), w1.data_ptr(), _ld(w1), None if b1 is None else b1.data_ptr(),
+                              w2.data_ptr(), _ld(w2), None if b2 is None else b2.data_ptr(), y.data_ptr(), _ld(y),
+                              M, K, H, N, int(act1), int(act2))
 
 
 def layernorm_member(x, y, gamma, beta, eps):

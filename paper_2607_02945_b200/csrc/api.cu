@@ -110,6 +110,7 @@ static cudaError_t launch_any(const opt_plan* p, cudaStream_t s) {
     case kPlanLayerNorm: return launch_layernorm(p, s);
     case kPlanLinearBf16: return launch_linear_bf16(p, s);
     case kPlanLinearF32: return launch_linear_f32(p, s);
+    case kPlanLinear2: return launch_linear2(p, s);
     default: return cudaErrorInvalidValue;
   }
 }

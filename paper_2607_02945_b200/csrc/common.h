@@ -51,7 +51,7 @@ struct Region {
 opt_status check_independent(std::vector<Region>& regions, bool allow_inplace_self);
 
 // ---------------------------------------------------------------- the plan --
-enum PlanKind { kPlanPointwise = 1, kPlanLayerNorm = 2, kPlanLinearBf16 = 3, kPlanLinearF32 = 4 };
+enum PlanKind { kPlanPointwise = 1, kPlanLayerNorm = 2, kPlanLinearBf16 = 3, kPlanLinearF32 = 4, kPlanLinear2 = 5 };
 
 }  // namespace optb
 
@@ -78,6 +78,7 @@ cudaError_t launch_pointwise(const opt_plan* p, cudaStream_t s);
 cudaError_t launch_layernorm(const opt_plan* p, cudaStream_t s);
 cudaError_t launch_linear_bf16(const opt_plan* p, cudaStream_t s);
 cudaError_t launch_linear_f32(const opt_plan* p, cudaStream_t s);
+cudaError_t launch_linear2(const opt_plan* p, cudaStream_t s);
 
 // host->device upload of a table blob; allocates p->dev_tables
 opt_status upload_tables(opt_plan* p, const void* host_blob, size_t bytes);
