@@ -11,14 +11,14 @@
 //
 // Kernel: persistent, one CTA per SM, 352 threads, per 128-row tile of a member:
 //   warp 0  TMA producer: the X tile (K <= 256: up to four 128x64 k-blocks, resident for the whole tile), a
-//           3-stage ring of W1 k-blocks (128 hidden units x 64), a 2-stage ring of W2 slices (N x 128);
-//   warp 1  MMA issuer: per hidden chunk c of 128 units  MMA1(c): acc1[c&1] = X . W1_c^T  (M=128, N<=128),
-//           then MMA2(c-1): acc2 += h_{c-1} . W2_{c-1}^T (M=128, N<=64, K<=128) -- MMA1 of the next chunk is
-//           issued BEFORE waiting for the previous chunk's hidden tile, so the tensor pipe works while the
-//           epilogue warps turn acc1 into h;
+//           6-stage ring of W1 k-blocks (128 hidden units x 64), a 2-stage ring of W2 slices (N x 128);
+//   warp 1  layer-1 MMA issuer: per hidden chunk c of 128 units  acc1[c&1] = X . W1_c^T  (M=128, N<=128); it
+//           never waits for a hidden tile, so the tensor pipe has work while the epilogue turns acc1 into h;
+//   warp 11 layer-2 MMA issuer: acc2 += h_c . W2_c^T (M=128, N<=64, K<=128) as soon as h_c is published
+//           (two issuing threads: a single one was instruction-bound on these short MMAs);
 //   warp 2  tile scheduler (dynamic, one atomic per 4 tiles; entry + b1 + b2 into a 2-deep queue);
 //   warps 3..10  epilogue: acc1 chunk -> +b1, act1, RNE bf16 -> the hidden tile in shared memory, written
-//           directly in the K-major 128-byte-swizzled layout MMA2 reads (double-buffered); after the last
+//           directly in the K-major 128-byte-swizzled layout MMA2 reads; after the last
 //           chunk acc2 -> +b2, act2, RNE -> staging -> TMA store into the member's output / concat slot.
 //   TMEM: acc1 2 x 128 columns, acc2 2 x 64 columns.
 #include <algorithm>
@@ -34,10 +34,11 @@ constexpr int kT_HC = 128;            // hidden chunk: UMMA N of layer 1, K of l
 constexpr int kT_MaxK = 256;          // layer-1 K (input features): the X tile is at most 4 k-blocks
 constexpr int kT_MaxH = 512;          // hidden width: b1 travels in the queue slot
 constexpr int kT_MaxN = 64;           // layer-2 N
-constexpr int kT_W1Stages = 3;
+constexpr int kT_W1Stages = 6;
 constexpr int kT_EpiWarps = 8;
 constexpr int kT_FirstEpiWarp = 3;
-constexpr int kT_Threads = 32 * (kT_FirstEpiWarp + kT_EpiWarps);
+constexpr int kT_Mma2Warp = kT_FirstEpiWarp + kT_EpiWarps;     // warp 11: layer-2 MMA issuer
+constexpr int kT_Threads = 32 * (kT_Mma2Warp + 1);
 constexpr int kT_KBlockBytes = kT_BM * kT_BK * 2;          // 16 KB: a 128 x 64 bf16 k-block
 constexpr int kT_W2KBlockBytes = kT_MaxN * kT_BK * 2;      // 8 KB: a 64 x 64 k-block of W2
 constexpr int kT_QDepth = 2;
@@ -45,12 +46,12 @@ constexpr int kT_QSlotBytes = kT_MaxH * 2 + kT_MaxN * 2 + 32;     // b1 | b2 | T
 // shared-memory map
 constexpr int kT_OffX = 0;
 constexpr int kT_OffW1 = kT_OffX + (kT_MaxK / kT_BK) * kT_KBlockBytes;            //  64 KB
-constexpr int kT_OffH = kT_OffW1 + kT_W1Stages * kT_KBlockBytes;                  // +48 KB
-constexpr int kT_OffW2 = kT_OffH + 2 * 2 * kT_KBlockBytes;                        // +64 KB (2 buffers x 2 k-blocks)
-constexpr int kT_OffOut = kT_OffW2 + 2 * 2 * kT_W2KBlockBytes;                    // +32 KB
-constexpr int kT_OffQ = kT_OffOut + 4 * 4096;                                     // +16 KB
+constexpr int kT_OffH = kT_OffW1 + kT_W1Stages * kT_KBlockBytes;                  // +96 KB
+constexpr int kT_OffW2 = kT_OffH + 2 * kT_KBlockBytes;                            // +32 KB (one hidden tile: 2 k-blocks)
+constexpr int kT_OffOut = kT_OffH;                                                // output staging aliases the hidden tile
+constexpr int kT_OffQ = kT_OffW2 + 2 * 2 * kT_W2KBlockBytes;                      // +32 KB
 constexpr int kT_OffBar = kT_OffQ + kT_QDepth * kT_QSlotBytes;
-constexpr int kT_SmemBytes = kT_OffBar + 256;
+constexpr int kT_SmemBytes = kT_OffBar + 512;
 static_assert(kT_SmemBytes <= 227 * 1024, "chained-GEMM shared memory map exceeds 227 KB");
 constexpr int kT_TmemCols = 512;      // acc1: columns [0,256), acc2: [256,384)
 
@@ -94,18 +95,20 @@ grouped_linear2_sm100_kernel(const L2Member* __restrict__ members, const uint4* 
   // barriers (8 bytes each)
   const uint32_t xa_full = bar_base, xa_empty = bar_base + 8;
   auto w1_full = [&](int s) { return bar_base + 16u + 8u * s; };
-  auto w1_empty = [&](int s) { return bar_base + 40u + 8u * s; };
-  auto w2_full = [&](int s) { return bar_base + 64u + 8u * s; };
-  auto w2_empty = [&](int s) { return bar_base + 80u + 8u * s; };
-  auto a1_full = [&](int s) { return bar_base + 96u + 8u * s; };
-  auto a1_empty = [&](int s) { return bar_base + 112u + 8u * s; };
-  auto h_full = [&](int s) { return bar_base + 128u + 8u * s; };
-  auto h_empty = [&](int s) { return bar_base + 144u + 8u * s; };
-  auto a2_full = [&](int s) { return bar_base + 160u + 8u * s; };
-  auto a2_empty = [&](int s) { return bar_base + 176u + 8u * s; };
-  auto q_full = [&](int s) { return bar_base + 192u + 8u * s; };
-  auto q_empty = [&](int s) { return bar_base + 208u + 8u * s; };
-  const uint32_t tmem_ptr_addr = bar_base + 224u;
+  auto w1_empty = [&](int s) { return bar_base + 16u + 8u * (kT_W1Stages + s); };
+  constexpr uint32_t kB2 = 16u + 16u * kT_W1Stages;        // the two-entry barrier arrays follow
+  auto w2_full = [&](int s) { return bar_base + kB2 + 8u * s; };
+  auto w2_empty = [&](int s) { return bar_base + kB2 + 16u + 8u * s; };
+  auto a1_full = [&](int s) { return bar_base + kB2 + 32u + 8u * s; };
+  auto a1_empty = [&](int s) { return bar_base + kB2 + 48u + 8u * s; };
+  auto h_full = [&](int s) { return bar_base + kB2 + 64u + 8u * s; };
+  auto h_empty = [&](int s) { return bar_base + kB2 + 80u + 8u * s; };
+  auto a2_full = [&](int s) { return bar_base + kB2 + 96u + 8u * s; };
+  auto a2_empty = [&](int s) { return bar_base + kB2 + 112u + 8u * s; };
+  auto q_full = [&](int s) { return bar_base + kB2 + 128u + 8u * s; };
+  auto q_empty = [&](int s) { return bar_base + kB2 + 144u + 8u * s; };
+  const uint32_t tmem_ptr_addr = bar_base + kB2 + 160u;
+  static_assert(16 + 16 * kT_W1Stages + 164 <= 512, "barrier area");
   auto q_slot = [&](int s) { return sbase + kT_OffQ + (uint32_t)s * kT_QSlotBytes; };
   constexpr uint32_t kQEntryOff = kT_MaxH * 2 + kT_MaxN * 2;
 
@@ -119,7 +122,7 @@ grouped_linear2_sm100_kernel(const L2Member* __restrict__ members, const uint4* 
       mbar_init(a1_full(s), 1); mbar_init(a1_empty(s), kT_EpiWarps);
       mbar_init(h_full(s), kT_EpiWarps); mbar_init(h_empty(s), 1);
       mbar_init(a2_full(s), 1); mbar_init(a2_empty(s), kT_EpiWarps);
-      mbar_init(q_full(s), 1); mbar_init(q_empty(s), 2 + kT_EpiWarps);
+      mbar_init(q_full(s), 1); mbar_init(q_empty(s), 3 + kT_EpiWarps);
     }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     fence_proxy_async_smem();
@@ -161,6 +164,12 @@ grouped_linear2_sm100_kernel(const L2Member* __restrict__ members, const uint4* 
           if (b2 != nullptr && 8 * lane < N) b2v = __ldg(b2 + lane);
           if (lane < 4)
             asm volatile("prefetch.tensormap [%0];" ::"l"(reinterpret_cast<const char*>(members + member) + 128 * lane) : "memory");
+          // the tile's X k-blocks -> L2 now: the X buffer is single (64 KB), its load can only be issued when the
+          // previous tile's last MMA1 has retired, and should then find the data in L2 rather than in HBM
+          const int nkb1 = (int)((shape >> 16) & 0xFFu), m0 = (int)__shfl_sync(0xffffffffu, e.y, 2 * g);
+          if (lane < nkb1)
+            asm volatile("cp.async.bulk.prefetch.tensor.2d.L2.global.tile [%0, {%1, %2}];"
+                         ::"l"(&members[member].tmX), "r"(lane * kT_BK), "r"(m0) : "memory");
         }
       };
       int member;
@@ -237,11 +246,15 @@ grouped_linear2_sm100_kernel(const L2Member* __restrict__ members, const uint4* 
       }
     }
   } else if (warp == 1) {
-    // --------------------------------------------------------- MMA issuer ----
+    // ------------------------------------------ MMA issuer, layer 1 ----
+    // acc1[g & 1] = X . W1_c^T for every hidden chunk; never waits for the hidden tile, so the tensor pipe always
+    // has layer-1 work queued while the epilogue warps convert the previous chunk.
     if (lane == 0) {
       int qs = 0; uint32_t qph = 0;
       int w1s = 0; uint32_t w1ph = 0;
-      uint32_t gt = 0, gh = 0;
+      uint32_t gt = 0, g = 0;
+      const uint64_t xd0 = umma_desc_sw128(sbase + kT_OffX), wd0 = umma_desc_sw128(sbase + kT_OffW1);
+      constexpr uint64_t kKB = kT_KBlockBytes >> 4;            // descriptor address units (16 bytes) per k-block
       for (;;) {
         mbar_wait(q_full(qs), qph);
         const uint4 e0 = lds128(q_slot(qs) + kQEntryOff);
@@ -249,54 +262,69 @@ grouped_linear2_sm100_kernel(const L2Member* __restrict__ members, const uint4* 
         if (++qs == kT_QDepth) { qs = 0; qph ^= 1; }
         if ((int)e0.x < 0) break;
         const int H = (int)(e0.z & 0xFFFFu), nkb1 = (int)((e0.z >> 16) & 0xFFu), klast1 = (int)(e0.z >> 24);
-        const int N = (int)(e0.w >> 16);
         const int nch = (H + kT_HC - 1) / kT_HC;
-        const uint32_t acc2 = tmem_base + 256u + (gt & 1u) * 64u;
-        const uint32_t idesc2 = l2_idesc(N);
-        auto mma2 = [&](int c, uint32_t g) {          // acc2 (+)= h_c . W2_c^T
-          const int s = (int)(g & 1u);
-          const uint32_t ph = (g >> 1) & 1u;
-          const int bn = min(kT_HC, H - c * kT_HC);
-          if (c == 0) { mbar_wait(a2_empty(gt & 1u), ((gt >> 1) & 1u) ^ 1u); }
-          mbar_wait(w2_full(s), ph);
-          mbar_wait(h_full(s), ph);
-          tc_fence_after();
-          const uint32_t ha = sbase + kT_OffH + s * 2 * kT_KBlockBytes, wa = sbase + kT_OffW2 + s * 2 * kT_W2KBlockBytes;
-          const int ksteps = bn / 16;
-          for (int k = 0; k < ksteps; ++k) {
-            const int j = k >> 2, kk = k & 3;         // k-block, K=16 step inside it
-            tc_mma_bf16(acc2, umma_desc_sw128(ha + j * kT_KBlockBytes) + 2 * kk,
-                        umma_desc_sw128(wa + j * kT_W2KBlockBytes) + 2 * kk, idesc2, (c | k) != 0);
-          }
-          tc_commit(h_empty(s));
-          tc_commit(w2_empty(s));
-        };
-        for (int c = 0; c < nch; ++c) {
-          const uint32_t g = gh + (uint32_t)c;
-          const int s = (int)(g & 1u);
-          const int bn = min(kT_HC, H - c * kT_HC);
-          const uint32_t idesc1 = l2_idesc(bn);
+        for (int c = 0; c < nch; ++c, ++g) {
+          const uint32_t s = g & 1u;
+          const uint32_t idesc1 = l2_idesc(min(kT_HC, H - c * kT_HC));
           mbar_wait(a1_empty(s), ((g >> 1) & 1u) ^ 1u);      // epilogue has drained this acc1 stage
           if (c == 0) mbar_wait(xa_full, gt & 1u);
           tc_fence_after();
-          const uint32_t acc1 = tmem_base + (uint32_t)s * 128u;
+          const uint32_t acc1 = tmem_base + s * 128u;
           for (int kb = 0; kb < nkb1; ++kb) {
             mbar_wait(w1_full(w1s), w1ph);
             tc_fence_after();
-            const uint64_t adesc = umma_desc_sw128(sbase + kT_OffX + kb * kT_KBlockBytes);
-            const uint64_t bdesc = umma_desc_sw128(sbase + kT_OffW1 + w1s * kT_KBlockBytes);
-            const int ksteps = kb + 1 < nkb1 ? kT_BK / 16 : klast1;
-            for (int k = 0; k < ksteps; ++k) tc_mma_bf16(acc1, adesc + 2 * k, bdesc + 2 * k, idesc1, (kb | k) != 0);
+            const uint64_t adesc = xd0 + (uint64_t)kb * kKB, bdesc = wd0 + (uint64_t)w1s * kKB;
+            if (kb + 1 < nkb1) {                             // +32 bytes (= +2 encoded) per K=16 step
+              tc_mma_bf16(acc1, adesc, bdesc, idesc1, kb != 0);
+              tc_mma_bf16(acc1, adesc + 2, bdesc + 2, idesc1, 1);
+              tc_mma_bf16(acc1, adesc + 4, bdesc + 4, idesc1, 1);
+              tc_mma_bf16(acc1, adesc + 6, bdesc + 6, idesc1, 1);
+            } else {
+              for (int k = 0; k < klast1; ++k) tc_mma_bf16(acc1, adesc + 2 * k, bdesc + 2 * k, idesc1, (kb | k) != 0);
+            }
             tc_commit(w1_empty(w1s));
             if (++w1s == kT_W1Stages) { w1s = 0; w1ph ^= 1; }
           }
           tc_commit(a1_full(s));
           if (c == nch - 1) tc_commit(xa_empty);             // the X tile may be replaced
-          if (c >= 1) mma2(c - 1, g - 1);
         }
-        mma2(nch - 1, gh + nch - 1);
+        ++gt;
+      }
+    }
+  } else if (warp == kT_Mma2Warp) {
+    // ------------------------------------------ MMA issuer, layer 2 ----
+    // acc2 (+)= h_c . W2_c^T as soon as the epilogue has published the hidden tile of chunk c.
+    if (lane == 0) {
+      int qs = 0; uint32_t qph = 0;
+      uint32_t gt = 0, g = 0;
+      const uint64_t hd0 = umma_desc_sw128(sbase + kT_OffH), w2d0 = umma_desc_sw128(sbase + kT_OffW2);
+      constexpr uint64_t kKB = kT_KBlockBytes >> 4, kW2KB = kT_W2KBlockBytes >> 4;
+      for (;;) {
+        mbar_wait(q_full(qs), qph);
+        const uint4 e0 = lds128(q_slot(qs) + kQEntryOff);
+        mbar_arrive(q_empty(qs));
+        if (++qs == kT_QDepth) { qs = 0; qph ^= 1; }
+        if ((int)e0.x < 0) break;
+        const int H = (int)(e0.z & 0xFFFFu), N = (int)(e0.w >> 16);
+        const int nch = (H + kT_HC - 1) / kT_HC;
+        const uint32_t acc2 = tmem_base + 256u + (gt & 1u) * 64u;
+        const uint32_t idesc2 = l2_idesc(N);
+        mbar_wait(a2_empty(gt & 1u), ((gt >> 1) & 1u) ^ 1u);   // the epilogue has drained this acc2 stage
+        for (int c = 0; c < nch; ++c, ++g) {
+          const uint32_t s = g & 1u;
+          const int ksteps = min(kT_HC, H - c * kT_HC) / 16;
+          mbar_wait(w2_full(s), (g >> 1) & 1u);
+          mbar_wait(h_full(0), g & 1u);
+          tc_fence_after();
+          const uint64_t wd = w2d0 + (uint64_t)s * 2 * kW2KB;
+          for (int k = 0; k < ksteps; ++k) {
+            const uint64_t j = (uint64_t)(k >> 2), kk = (uint64_t)(k & 3);   // k-block, K=16 step inside it
+            tc_mma_bf16(acc2, hd0 + j * kKB + 2 * kk, wd + j * kW2KB + 2 * kk, idesc2, (c | k) != 0);
+          }
+          tc_commit(h_empty(0));
+          tc_commit(w2_empty(s));
+        }
         tc_commit(a2_full(gt & 1u));
-        gh += (uint32_t)nch;
         ++gt;
       }
     }
@@ -339,16 +367,20 @@ grouped_linear2_sm100_kernel(const L2Member* __restrict__ members, const uint4* 
         __syncwarp();
         if (lane == 0) mbar_arrive(a1_empty(s));       // acc1 stage is in registers: MMA1 of chunk c+2 may overwrite it
         epi_act(v, slot + (uint32_t)(c * kT_HC + half * 64) * 2u, act1, p);
-        mbar_wait(h_empty(s), ph ^ 1);                 // MMA2 of chunk c-2 has finished reading this hidden buffer
+        // the hidden tile is single-buffered: MMA2 of chunk c-1 sits right behind MMA1 of chunk c in the tensor
+        // pipe, so it has retired by the time this chunk's accumulator has been read and converted.  (The tile
+        // also serves as the output staging of the previous row tile: that TMA store must have read it.)
+        if (half == 0 && lane == 0) tma_store_wait_read<0>();
+        mbar_wait(h_empty(0), (g & 1u) ^ 1u);
         if (mine) {
-          const uint32_t hrow = sbase + kT_OffH + (uint32_t)s * 2u * kT_KBlockBytes + (uint32_t)half * kT_KBlockBytes + row_off;
+          const uint32_t hrow = sbase + kT_OffH + (uint32_t)half * kT_KBlockBytes + row_off;
 #pragma unroll
           for (int j = 0; j < 8; ++j)                  // K-major, 128-byte swizzle: 16-byte piece j of row r sits at j ^ (r & 7)
             sts128(hrow + ((j ^ (lane & 7)) << 4), make_uint4(p[4 * j], p[4 * j + 1], p[4 * j + 2], p[4 * j + 3]));
         }
         fence_proxy_async_smem();                      // generic-proxy writes -> visible to the tensor core's reads
         __syncwarp();
-        if (lane == 0) mbar_arrive(h_full(s));
+        if (lane == 0) mbar_arrive(h_full(0));
       }
       gh += (uint32_t)nch;
       // ---- layer-2 accumulator of the tile
@@ -368,8 +400,7 @@ grouped_linear2_sm100_kernel(const L2Member* __restrict__ members, const uint4* 
         if (lane == 0) mbar_arrive(a2_empty(s2));
         if (half == 0) {
           epi_act(v, slot + kT_MaxH * 2, act2, p);
-          if (lane == 0) tma_store_wait_read<0>();     // the previous store of this warp has read the staging tile
-          __syncwarp();
+          // staging = this warp's own 32 rows of the hidden tile's first k-block: free, every MMA2 of the tile retired
 #pragma unroll
           for (int j = 0; j < 8; ++j)
             sts128(sbuf + lane * 128 + ((j ^ (lane & 7)) << 4), make_uint4(p[4 * j], p[4 * j + 1], p[4 * j + 2], p[4 * j + 3]));
