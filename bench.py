@@ -596,6 +596,47 @@ def run_product(args):
         except Exception as e:  # noqa: BLE001
             unfused = dict(error=repr(e))
 
+    # ---- (6) SURVEY 8(f) rank 1, side figure (NOT part of the step): C4's two GEMM groups as ONE chained-Linear
+    # launch (opt_linear2, hidden tensor on chip) next to the two-launch path, isolated, cold L2, same tensors
+    vertical = None
+    c4 = [g for g in step.groups if g.name.startswith("C4")]
+    if len(c4) == 3 and not args.profile and not args.small:
+        try:
+            ga, gb, gc = c4
+            T, A = ga.ain.tensor, ga.amid.tensor
+            ref_out = gc.aout.tensor(ga.iy)
+            out2 = torch.empty_like(ref_out)
+            descs = [ob.linear2_member(A(i["xn"]), T(i["w1"]), T(i["b1"]), T(i["w2"]), T(i["b2"]),
+                                       out2[:, k * t["out"]:(k + 1) * t["out"]], ACT_RELU, ACT_NONE)
+                     for k, (i, t) in enumerate(zip(ga.idx, ga.cfg["towers"]))]
+            p2 = ob.opt_linear2_plan_create(descs, BF16, step.dev_index)
+            gb.plan.launch(); gc.plan.launch(); p2.launch()
+            torch.cuda.synchronize()
+            same = bool(torch.equal(ref_out.view(torch.int16), out2.view(torch.int16)))
+            flush = torch.empty(256 * 1024 * 1024, dtype=torch.uint8, device=device)
+
+            def cold(fn, n=10):
+                ts = []
+                for _ in range(n):
+                    flush.fill_(1)
+                    c0, c1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                    c0.record(stream); fn(); c1.record(stream)
+                    torch.cuda.synchronize()
+                    ts.append(c0.elapsed_time(c1) * 1e3)
+                return float(np.mean(ts))
+            t1 = cold(p2.launch)
+            t2 = cold(lambda: (gb.plan.launch(), gc.plan.launch()))
+            i2 = p2.info()
+            vertical = dict(workload="C4 towers: Linear(D->H)+ReLU -> Linear(H->64), 512 members, B=8192", launches=1,
+                            linear2_us=round(t1, 1), two_launch_us=round(t2, 1), speedup=round(t2 / t1, 3),
+                            bitwise_equal_to_two_launch=same, flops=i2["flops"], algorithmic_bytes=i2["bytes"],
+                            tflops=round(i2["flops"] / t1 / 1e6, 1),
+                            frac_tensor=round(i2["flops"] / t1 / 1e6 / peaks["bf16_tflops"], 4),
+                            hbm_bytes_saved=int(gb.info["bytes"] + gc.info["bytes"] - i2["bytes"]))
+            del flush, out2
+        except Exception as e:  # noqa: BLE001
+            vertical = dict(error=repr(e))
+
     watch.stop_flag.set()
     watch.join(timeout=2)
 
@@ -657,7 +698,7 @@ def run_product(args):
                              "each step)"),
                 gpu_launches=int(launches), launches_per_step=ng,
                 clocks=watch.summary(), roofline=roofline, roofline_tensor=roofline_tensor, groups=groups,
-                unfused_baseline=unfused,
+                unfused_baseline=unfused, vertical_fusion=vertical,
                 aggregate=dict(steps_per_s=round(aggregate_steps_per_s(us_step, world), 2)),
                 build_seconds=round(build_s, 1), lib=ob.opt_version())
 

@@ -34,14 +34,14 @@ constexpr int kT_HC = 128;            // hidden chunk: UMMA N of layer 1, K of l
 constexpr int kT_MaxK = 256;          // layer-1 K (input features): the X tile is at most 4 k-blocks
 constexpr int kT_MaxH = 512;          // hidden width: b1 travels in the queue slot
 constexpr int kT_MaxN = 64;           // layer-2 N
-constexpr int kT_W1Stages = 6;
+constexpr int kT_W1Stages = 5;
 constexpr int kT_EpiWarps = 8;
 constexpr int kT_FirstEpiWarp = 3;
 constexpr int kT_Mma2Warp = kT_FirstEpiWarp + kT_EpiWarps;     // warp 11: layer-2 MMA issuer
 constexpr int kT_Threads = 32 * (kT_Mma2Warp + 1);
 constexpr int kT_KBlockBytes = kT_BM * kT_BK * 2;          // 16 KB: a 128 x 64 bf16 k-block
 constexpr int kT_W2KBlockBytes = kT_MaxN * kT_BK * 2;      // 8 KB: a 64 x 64 k-block of W2
-constexpr int kT_QDepth = 2;
+constexpr int kT_QDepth = 4;
 constexpr int kT_QSlotBytes = kT_MaxH * 2 + kT_MaxN * 2 + 32;     // b1 | b2 | TileEntry2
 // shared-memory map
 constexpr int kT_OffX = 0;
@@ -106,9 +106,9 @@ grouped_linear2_sm100_kernel(const L2Member* __restrict__ members, const uint4* 
   auto a2_full = [&](int s) { return bar_base + kB2 + 96u + 8u * s; };
   auto a2_empty = [&](int s) { return bar_base + kB2 + 112u + 8u * s; };
   auto q_full = [&](int s) { return bar_base + kB2 + 128u + 8u * s; };
-  auto q_empty = [&](int s) { return bar_base + kB2 + 144u + 8u * s; };
-  const uint32_t tmem_ptr_addr = bar_base + kB2 + 160u;
-  static_assert(16 + 16 * kT_W1Stages + 164 <= 512, "barrier area");
+  auto q_empty = [&](int s) { return bar_base + kB2 + 128u + 8u * (kT_QDepth + s); };
+  const uint32_t tmem_ptr_addr = bar_base + kB2 + 128u + 16u * kT_QDepth;
+  static_assert(16 + 16 * kT_W1Stages + 128 + 16 * kT_QDepth + 4 <= 512, "barrier area");
   auto q_slot = [&](int s) { return sbase + kT_OffQ + (uint32_t)s * kT_QSlotBytes; };
   constexpr uint32_t kQEntryOff = kT_MaxH * 2 + kT_MaxN * 2;
 
@@ -122,8 +122,8 @@ grouped_linear2_sm100_kernel(const L2Member* __restrict__ members, const uint4* 
       mbar_init(a1_full(s), 1); mbar_init(a1_empty(s), kT_EpiWarps);
       mbar_init(h_full(s), kT_EpiWarps); mbar_init(h_empty(s), 1);
       mbar_init(a2_full(s), 1); mbar_init(a2_empty(s), kT_EpiWarps);
-      mbar_init(q_full(s), 1); mbar_init(q_empty(s), 3 + kT_EpiWarps);
     }
+    for (int s = 0; s < kT_QDepth; ++s) { mbar_init(q_full(s), 1); mbar_init(q_empty(s), 3 + kT_EpiWarps); }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     fence_proxy_async_smem();
   }
