@@ -227,9 +227,11 @@ class Step:
         for g in self.groups:
             g.plan.launch(stream)
 
-    def launch_all_host(self, stream=None):
+    def launch_all_host(self, stream=None, streams=None):
         """e2e: per group, H2D of every input arena, the one kernel, D2H of every output arena --
-        all through opt_plan_launch_host (the C ABI call for HOST buffers)."""
+        all through opt_plan_launch_host (the C ABI call for HOST buffers).  `streams`: one CUDA stream per
+        config (C1, C2, C3, C4) -- the configs are independent, so a caller can let their PCIe copies overlap
+        (H2D and D2H are separate DMA engines); C4's three dependent groups stay on one stream."""
         ob = self.ob
         for g in self.groups:
             copies = []
@@ -237,7 +239,10 @@ class Step:
                 copies.append(ob.opt_host_copy(g.ain.host.data_ptr(), g.ain.dev.data_ptr(), g.ain.size, 1))
             if g.aout.size:
                 copies.append(ob.opt_host_copy(g.aout.host.data_ptr(), g.aout.dev.data_ptr(), g.aout.size, 0))
-            g.plan.launch_host(copies, stream)
+            s = stream
+            if streams is not None:
+                s = streams[g.name[:2]].cuda_stream
+            g.plan.launch_host(copies, s)
 
     def h2d_bytes(self):
         return sum(g.ain.size for g in self.groups)
@@ -559,6 +564,21 @@ def run_product(args):
     f1.record(stream)
     barrier()
     ms_e2e = f0.elapsed_time(f1)
+    # the same, the four independent configs on four streams (copies of one config overlap the others')
+    side = {k: torch.cuda.Stream() for k in ("C1", "C2", "C3", "C4")}
+    step.launch_all_host(streams=side)
+    barrier()
+    f2, f3 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    f2.record(stream)
+    for st_ in side.values():
+        st_.wait_stream(stream)
+    for _ in range(Ke):
+        step.launch_all_host(streams=side)
+    for st_ in side.values():
+        stream.wait_stream(st_)
+    f3.record(stream)
+    barrier()
+    ms_e2e_ms = f2.elapsed_time(f3)
 
     # ---- (4) size-matched plain-copy reference for the HBM-bound groups: a device-to-device copy of the same
     # number of bytes (half read, half written), cold L2, same event protocol.  Small groups cannot reach the
@@ -641,7 +661,7 @@ def run_product(args):
     watch.join(timeout=2)
 
     # max over ranks
-    ms_total, ms_e2e = max_over_ranks([ms_total, ms_e2e], world, device)
+    ms_total, ms_e2e, ms_e2e_ms = max_over_ranks([ms_total, ms_e2e, ms_e2e_ms], world, device)
 
     us_step = ms_total * 1e3 / K
     us_e2e = ms_e2e * 1e3 / Ke
@@ -692,10 +712,11 @@ def run_product(args):
                             l2="inputs larger than L2: a step touches %.2f GB, every group's data was last touched one "
                                "full step earlier" % (sum(g.info["bytes"] for g in step.groups) / 1e9),
                             groups_per_step=ng),
-                e2e=dict(value=round(us_e2e, 2), unit="us", h2d_bytes_per_step=step.h2d_bytes(),
-                         d2h_bytes_per_step=step.d2h_bytes(), steps=Ke,
+                e2e=dict(value=round(ms_e2e_ms * 1e3 / Ke, 2), unit="us", h2d_bytes_per_step=step.h2d_bytes(),
+                         d2h_bytes_per_step=step.d2h_bytes(), steps=Ke, single_stream_us=round(us_e2e, 2),
                          api="opt_plan_launch_host (pinned host arenas; every input tensor H2D and every output D2H "
-                             "each step)"),
+                             "each step); value: the four independent configs on four streams so that their PCIe "
+                             "copies overlap, single_stream_us: everything on one stream"),
                 gpu_launches=int(launches), launches_per_step=ng,
                 clocks=watch.summary(), roofline=roofline, roofline_tensor=roofline_tensor, groups=groups,
                 unfused_baseline=unfused, vertical_fusion=vertical,
