@@ -49,6 +49,7 @@ def lib():
         L.oracle_linear_mulreduce.argtypes = [vp, i64, vp, i64, vp, i32, i32, i32, c.c_int, vp]
         L.oracle_activation.argtypes = [vp, i64, c.c_int]
         L.oracle_pointwise.argtypes = [vp, i64, i32, i32, c.c_int, c.c_int, vp]
+        L.oracle_pointwise_ext.argtypes = [vp, i64, vp, i64, i32, i32, c.c_int, dbl, dbl, dbl, c.c_int, vp]
         L.oracle_layernorm.argtypes = [vp, i64, vp, vp, i32, i32, dbl, c.c_int, c.c_int, vp, vp]
         L.oracle_split.argtypes = [vp, i64, i32, i32, i32, vp, i32, vp]
         L.oracle_split.restype = c.c_int
@@ -126,6 +127,25 @@ def pointwise(src, op, dt):
     rows, width = src.shape
     out = np.empty((rows, width), dtype=np.float64)
     lib().oracle_pointwise(_ptr(src), _ld(src), rows, width, int(op), dt, _ptr(out))
+    return out
+
+
+PW_CLAMP, PW_NAN_TO_NUM, PW_SUB, PW_DIV, PW_MUL = 4, 5, 6, 7, 8
+
+
+def pointwise_ext(a, b, op, params, dt):
+    """Table-1 pointwise patterns beyond relu/tanh/sigmoid, fp64, torch semantics:
+    op 4 clamp(a, lo=params[0], hi=params[1]); op 5 nan_to_num(a, nan=params[0], posinf=params[1],
+    neginf=params[2]); op 6/7/8 a - b, a / b, a * b.  Parameters are the fp32 values the descriptor carries."""
+    _chk(a, dt, 2)
+    rows, width = a.shape
+    if b is not None:
+        _chk(b, dt, 2)
+        assert b.shape == a.shape
+    p = [float(np.float32(v)) for v in (list(params) + [0.0, 0.0, 0.0])[:3]]
+    out = np.empty((rows, width), dtype=np.float64)
+    lib().oracle_pointwise_ext(_ptr(a), _ld(a), _ptr(b), 0 if b is None else _ld(b), rows, width, int(op),
+                               p[0], p[1], p[2], dt, _ptr(out))
     return out
 
 

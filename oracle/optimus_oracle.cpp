@@ -177,6 +177,38 @@ void oracle_pointwise(const void* src, int64_t lds, int32_t rows, int32_t width,
       out[(int64_t)r * width + c] = act_apply(widen(src, (int64_t)r * lds + c, dt), op);
 }
 
+// ---- the remaining horizontal pointwise patterns of Table 1: batch_clamp,
+// batch_nan_to_num (unary, scalar parameters) and batch_aten_sub / _div / _mul (binary), torch
+// semantics, on strided 2-D storage tensors -> dense double [rows,width].
+//   op 4 clamp:      y = min(max(x, lo), hi), NaN propagates            (torch.clamp)
+//   op 5 nan_to_num: NaN -> p0, +inf -> p1, -inf -> p2, else x          (torch.nan_to_num)
+//   op 6 / 7 / 8:    a - b, a / b, a * b                                (aten.sub / div / mul)
+// b may be NULL for the unary ops.
+void oracle_pointwise_ext(const void* a, int64_t lda, const void* b, int64_t ldb, int32_t rows, int32_t width,
+                          int op, double p0, double p1, double p2, int dt, double* out) {
+#pragma omp parallel for schedule(static)
+  for (int32_t r = 0; r < rows; ++r)
+    for (int32_t c = 0; c < width; ++c) {
+      const double x = widen(a, (int64_t)r * lda + c, dt);
+      double y;
+      switch (op) {
+        case 4:
+          if (std::isnan(x)) { y = x; break; }
+          y = x < p0 ? p0 : x;
+          y = y > p1 ? p1 : y;
+          break;
+        case 5:
+          y = std::isnan(x) ? p0 : (std::isinf(x) ? (x > 0 ? p1 : p2) : x);
+          break;
+        case 6: y = x - widen(b, (int64_t)r * ldb + c, dt); break;
+        case 7: y = x / widen(b, (int64_t)r * ldb + c, dt); break;
+        case 8: y = x * widen(b, (int64_t)r * ldb + c, dt); break;
+        default: y = x; break;
+      }
+      out[(int64_t)r * width + c] = y;
+    }
+}
+
 // ---- layer_norm over the last dim (batch_layernorm; torch
 // semantics, reading Q4): mu = sum(x)/D; v = sum((x-mu)^2)/D (biased);
 // y_j = (x_j-mu)/sqrt(v+eps) * gamma_j + beta_j.  gamma/beta may be NULL (1/0).

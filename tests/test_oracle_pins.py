@@ -427,3 +427,38 @@ def test_linear2_identity_second_layer_returns_hidden():
     ref = np.tanh(wl.f32_from_bf16_bits(m["x"]).astype(np.float64) @ wl.f32_from_bf16_bits(m["w1"]).astype(np.float64).T
                   + wl.f32_from_bf16_bits(m["b1"]).astype(np.float64))
     assert np.allclose(r["h64"], ref, rtol=1e-13, atol=1e-15)
+
+
+# --------------------------------- Table-1 pointwise patterns --
+def test_pointwise_ext_hand_values_and_special_values():
+    """batch_clamp / batch_nan_to_num / batch_aten_sub,div,mul against hand-computed values (torch semantics)."""
+    inf, nan = float("inf"), float("nan")
+    x = np.array([[-3.0, -0.5, 0.0, 0.75, 2.0, 100.0, inf, -inf]], dtype=np.float32)
+    y = oracle.pointwise_ext(x, None, oracle.PW_CLAMP, [-1.0, 1.5], F32)
+    assert np.array_equal(y, np.array([[-1.0, -0.5, 0.0, 0.75, 1.5, 1.5, 1.5, -1.0]]))
+    xn = np.array([[nan, 1.0]], dtype=np.float32)
+    yn = oracle.pointwise_ext(xn, None, oracle.PW_CLAMP, [-1.0, 1.5], F32)
+    assert np.isnan(yn[0, 0]) and yn[0, 1] == 1.0                      # NaN propagates through clamp
+    # lo > hi: torch.clamp returns hi everywhere (min(max(x, lo), hi))
+    assert np.array_equal(oracle.pointwise_ext(x[:, :4], None, oracle.PW_CLAMP, [2.0, 1.0], F32), np.full((1, 4), 1.0))
+    z = np.array([[nan, inf, -inf, 3.5, -0.0]], dtype=np.float32)
+    w = oracle.pointwise_ext(z, None, oracle.PW_NAN_TO_NUM, [7.0, 9.0, -9.0], F32)
+    assert np.array_equal(w[0, :4], [7.0, 9.0, -9.0, 3.5]) and w[0, 4] == 0.0 and np.signbit(w[0, 4])
+    a = bf16([[6.0, -1.5, 0.25, 8.0]]); b = bf16([[2.0, 0.5, -4.0, 0.0]])
+    assert np.array_equal(oracle.pointwise_ext(a, b, oracle.PW_SUB, [], BF16), [[4.0, -2.0, 4.25, 8.0]])
+    assert np.array_equal(oracle.pointwise_ext(a, b, oracle.PW_MUL, [], BF16), [[12.0, -0.75, -1.0, 0.0]])
+    d = oracle.pointwise_ext(a, b, oracle.PW_DIV, [], BF16)
+    assert np.array_equal(d[0, :3], [3.0, -3.0, -0.0625]) and d[0, 3] == inf
+
+
+def test_pointwise_ext_identities_on_random_data():
+    a = wl.tensor_normal(13, 1, (6, 40), 0.0, 2.0, BF16)
+    b = wl.tensor_normal(13, 2, (6, 40), 1.0, 3.0, BF16)
+    a64, b64 = oracle.widen(a, BF16), oracle.widen(b, BF16)
+    assert np.array_equal(oracle.pointwise_ext(a, b, oracle.PW_SUB, [], BF16), a64 - b64)          # numpy, not the oracle
+    assert np.array_equal(oracle.pointwise_ext(a, b, oracle.PW_MUL, [], BF16), oracle.pointwise_ext(b, a, oracle.PW_MUL, [], BF16))
+    assert np.array_equal(oracle.pointwise_ext(a, a, oracle.PW_DIV, [], BF16), np.ones((6, 40)))
+    c = oracle.pointwise_ext(a, None, oracle.PW_CLAMP, [-1.0, 1.0], BF16)
+    assert np.array_equal(c, np.clip(a64, -1.0, 1.0)) and np.array_equal(np.clip(c, -1.0, 1.0), c)    # idempotent
+    assert np.array_equal(oracle.pointwise_ext(a, None, oracle.PW_CLAMP, [-np.inf, np.inf], BF16), a64)
+    assert np.array_equal(oracle.pointwise_ext(a, None, oracle.PW_NAN_TO_NUM, [0.0, 1.0, -1.0], BF16), a64)   # finite: untouched
