@@ -68,7 +68,15 @@ typedef enum {
 
 typedef enum { OPT_F32 = 0, OPT_BF16 = 1 } opt_dtype;
 typedef enum { OPT_ACT_NONE = 0, OPT_ACT_RELU = 1, OPT_ACT_TANH = 2, OPT_ACT_SIGMOID = 3 } opt_act;
-typedef enum { OPT_PW_COPY = 0, OPT_PW_RELU = 1, OPT_PW_TANH = 2, OPT_PW_SIGMOID = 3 } opt_pw_op;
+typedef enum {
+  OPT_PW_COPY = 0, OPT_PW_RELU = 1, OPT_PW_TANH = 2, OPT_PW_SIGMOID = 3,
+  /* the remaining horizontal pointwise patterns of the paper's Table 1 */
+  OPT_PW_CLAMP = 4,      /* batch_clamp:      dst = min(max(src, p0), p1), NaN propagates (torch.clamp)          */
+  OPT_PW_NAN_TO_NUM = 5, /* batch_nan_to_num: NaN -> p0, +inf -> p1, -inf -> p2, finite values unchanged          */
+  OPT_PW_SUB = 6,        /* batch_aten_sub:   dst = src - src2                                                     */
+  OPT_PW_DIV = 7,        /* batch_aten_div:   dst = src / src2                                                     */
+  OPT_PW_MUL = 8         /* batch_aten_mul:   dst = src * src2                                                     */
+} opt_pw_op;
 
 /* One member of a grouped Linear (+bias +activation) -- batch_linear /
  * batch_linear_post_grad with its epilogue:
@@ -139,7 +147,10 @@ typedef struct {
  * movement left over by the split/cat rewrites (Listing 2):
  *     dst[r, 0:width] = op(src[r, 0:width])   for r < rows
  * A split->f->cat chain is a list of chunks whose src/dst are column slices of
- * shared bases.  OPT_PW_COPY moves raw bits.                                 */
+ * shared bases.  OPT_PW_COPY moves raw bits.  The binary ops read a second
+ * operand src2 (same rows x width, row stride lds2); CLAMP / NAN_TO_NUM take
+ * their scalars from p0..p2 (fp32; the result is rounded to the storage dtype).
+ * For ops 0..3 the extra fields are ignored (zero-initialise the struct).      */
 typedef struct {
   const void* src;
   int64_t lds;
@@ -147,6 +158,9 @@ typedef struct {
   int64_t ldd;
   int32_t rows, width;
   int32_t op; /* opt_pw_op */
+  const void* src2; /* second operand of OPT_PW_SUB / DIV / MUL, else NULL */
+  int64_t lds2;
+  float p0, p1, p2; /* CLAMP: lo, hi;  NAN_TO_NUM: nan, posinf, neginf */
 } opt_chunk;
 
 /* One staged host<->device copy of opt_plan_launch_host. */

@@ -7,6 +7,7 @@ from . import build as _build
 OPT_F32, OPT_BF16 = 0, 1
 OPT_ACT_NONE, OPT_ACT_RELU, OPT_ACT_TANH, OPT_ACT_SIGMOID = 0, 1, 2, 3
 OPT_PW_COPY, OPT_PW_RELU, OPT_PW_TANH, OPT_PW_SIGMOID = 0, 1, 2, 3
+OPT_PW_CLAMP, OPT_PW_NAN_TO_NUM, OPT_PW_SUB, OPT_PW_DIV, OPT_PW_MUL = 4, 5, 6, 7, 8
 (OPT_OK, OPT_ERR_INVALID_ARG, OPT_ERR_UNSUPPORTED, OPT_ERR_ALIGNMENT, OPT_ERR_ALIAS, OPT_ERR_CUDA,
  OPT_ERR_NO_DEVICE) = range(7)
 _STATUS_NAMES = ["OPT_OK", "OPT_ERR_INVALID_ARG", "OPT_ERR_UNSUPPORTED", "OPT_ERR_ALIGNMENT", "OPT_ERR_ALIAS",
@@ -34,7 +35,8 @@ class opt_layernorm_member(C.Structure):
 
 class opt_chunk(C.Structure):
     _fields_ = [("src", C.c_void_p), ("lds", C.c_int64), ("dst", C.c_void_p), ("ldd", C.c_int64),
-                ("rows", C.c_int32), ("width", C.c_int32), ("op", C.c_int32)]
+                ("rows", C.c_int32), ("width", C.c_int32), ("op", C.c_int32),
+                ("src2", C.c_void_p), ("lds2", C.c_int64), ("p0", C.c_float), ("p1", C.c_float), ("p2", C.c_float)]
 
 
 class opt_host_copy(C.Structure):
@@ -217,10 +219,15 @@ def layernorm_member(x, y, gamma, beta, eps):
                                 None if beta is None else beta.data_ptr(), rows, D, float(eps))
 
 
-def chunk(src, dst, op=OPT_PW_COPY):
+def chunk(src, dst, op=OPT_PW_COPY, src2=None, params=()):
     rows, width = src.shape
     assert tuple(dst.shape) == (rows, width)
-    return opt_chunk(src.data_ptr(), _ld(src), dst.data_ptr(), _ld(dst), rows, width, int(op))
+    p = (list(params) + [0.0, 0.0, 0.0])[:3]
+    if src2 is not None:
+        assert tuple(src2.shape) == (rows, width)
+    return opt_chunk(src.data_ptr(), _ld(src), dst.data_ptr(), _ld(dst), rows, width, int(op),
+                     None if src2 is None else src2.data_ptr(), 0 if src2 is None else _ld(src2),
+                     float(p[0]), float(p[1]), float(p[2]))
 
 
 def split_cat_chunks(x, out, widths, ops, perm):

@@ -9,14 +9,14 @@
 // so the result is the one the two-launch path (two grouped GEMMs) produces, without the 2 x M x H x 2 bytes
 // of HBM traffic for h.
 //
-// Kernel: persistent, one CTA per SM, 352 threads, per 128-row tile of a member:
+// Kernel: persistent, one CTA per SM, 384 threads, per 128-row tile of a member:
 //   warp 0  TMA producer: the X tile (K <= 256: up to four 128x64 k-blocks, resident for the whole tile), a
-//           6-stage ring of W1 k-blocks (128 hidden units x 64), a 2-stage ring of W2 slices (N x 128);
+//           5-stage ring of W1 k-blocks (128 hidden units x 64), a 2-stage ring of W2 slices (N x 128);
 //   warp 1  layer-1 MMA issuer: per hidden chunk c of 128 units  acc1[c&1] = X . W1_c^T  (M=128, N<=128); it
 //           never waits for a hidden tile, so the tensor pipe has work while the epilogue turns acc1 into h;
 //   warp 11 layer-2 MMA issuer: acc2 += h_c . W2_c^T (M=128, N<=64, K<=128) as soon as h_c is published
 //           (two issuing threads: a single one was instruction-bound on these short MMAs);
-//   warp 2  tile scheduler (dynamic, one atomic per 4 tiles; entry + b1 + b2 into a 2-deep queue);
+//   warp 2  tile scheduler (dynamic, one atomic per 4 tiles; entry + b1 + b2 into a 4-deep queue);
 //   warps 3..10  epilogue: acc1 chunk -> +b1, act1, RNE bf16 -> the hidden tile in shared memory, written
 //           directly in the K-major 128-byte-swizzled layout MMA2 reads; after the last
 //           chunk acc2 -> +b2, act2, RNE -> staging -> TMA store into the member's output / concat slot.

@@ -44,6 +44,10 @@ struct PwGroup {
   int32_t src_span;       // STAGED mode: vectors of one source row staged in smem (0 = direct mode)
   int32_t dst_span;       // STAGED mode: vectors of one destination row staged for a bulk store (0 = direct stores)
   int32_t tile_rows;      // STAGED mode: rows per block
+  int32_t ext_op;         // EXT mode (0 = off): OPT_PW_CLAMP .. OPT_PW_MUL, one chunk per group, no map
+  const char* src2;       // EXT mode: second operand of the binary ops
+  int64_t lds2_16;
+  float p0, p1, p2;       // EXT mode: scalar parameters
   int32_t pad;
 };
 struct PwBlock { int32_t group, q0, r0, nrows; };
@@ -90,6 +94,58 @@ __device__ __forceinline__ void pw_rows(const int4* __restrict__ s, int4* __rest
     for (int i = 0; i < kPwUnroll; ++i) __stcs(d + (int64_t)(r + i * ty_step) * ldd, pw_apply<BF16, OP>(v[i]));
   }
   for (; r < rend; r += ty_step) __stcs(d + (int64_t)r * ldd, pw_apply<BF16, OP>(__ldcs(s + (int64_t)r * lds)));
+}
+
+// EXT mode: the remaining pointwise patterns of Table 1 -- batch_clamp, batch_nan_to_num
+// (scalar parameters) and batch_aten_sub / div / mul (second operand).  fp32 arithmetic, one rounding.
+__device__ __forceinline__ float pw_ext_scalar(float x, float y, int op, float p0, float p1, float p2) {
+  switch (op) {
+    case OPT_PW_CLAMP: return x != x ? x : fminf(fmaxf(x, p0), p1);            // torch.clamp: min(max(x, lo), hi), NaN stays
+    case OPT_PW_NAN_TO_NUM: return x != x ? p0 : (fabsf(x) == INFINITY ? (x > 0.f ? p1 : p2) : x);
+    case OPT_PW_SUB: return x - y;
+    case OPT_PW_DIV: return x / y;                                             // IEEE division (no fast-math)
+    default: return x * y;                                                     // OPT_PW_MUL
+  }
+}
+template <bool BF16>
+__device__ __forceinline__ int4 pw_ext_apply(int4 a, int4 b, int op, float p0, float p1, float p2) {
+  if (BF16) {
+    uint32_t* ua = reinterpret_cast<uint32_t*>(&a);
+    const uint32_t* ub = reinterpret_cast<const uint32_t*>(&b);
+#pragma unroll
+    for (int i = 0; i < 4; ++i)
+      ua[i] = pack_bf16x2(pw_ext_scalar(bf16_lo(ua[i]), bf16_lo(ub[i]), op, p0, p1, p2),
+                          pw_ext_scalar(bf16_hi(ua[i]), bf16_hi(ub[i]), op, p0, p1, p2));
+  } else {
+    float* fa = reinterpret_cast<float*>(&a);
+    const float* fb = reinterpret_cast<const float*>(&b);
+#pragma unroll
+    for (int i = 0; i < 4; ++i) fa[i] = pw_ext_scalar(fa[i], fb[i], op, p0, p1, p2);
+  }
+  return a;
+}
+template <bool BF16>
+__device__ __forceinline__ void pw_ext_rows(const PwGroup& g, int q, int r, int rend, int ty_step) {
+  const int4* s = reinterpret_cast<const int4*>(g.src) + q;
+  const int4* s2 = g.src2 ? reinterpret_cast<const int4*>(g.src2) + q : nullptr;
+  int4* d = reinterpret_cast<int4*>(g.dst) + q;
+  constexpr int U = 4;
+  for (; r + (U - 1) * ty_step < rend; r += U * ty_step) {
+    int4 v[U], w[U];
+#pragma unroll
+    for (int i = 0; i < U; ++i) {
+      v[i] = __ldcs(s + (int64_t)(r + i * ty_step) * g.lds16);
+      w[i] = s2 ? __ldcs(s2 + (int64_t)(r + i * ty_step) * g.lds2_16) : make_int4(0, 0, 0, 0);
+    }
+#pragma unroll
+    for (int i = 0; i < U; ++i)
+      __stcs(d + (int64_t)(r + i * ty_step) * g.ldd16, pw_ext_apply<BF16>(v[i], w[i], g.ext_op, g.p0, g.p1, g.p2));
+  }
+  for (; r < rend; r += ty_step) {
+    const int4 v = __ldcs(s + (int64_t)r * g.lds16);
+    const int4 w = s2 ? __ldcs(s2 + (int64_t)r * g.lds2_16) : make_int4(0, 0, 0, 0);
+    __stcs(d + (int64_t)r * g.ldd16, pw_ext_apply<BF16>(v, w, g.ext_op, g.p0, g.p1, g.p2));
+  }
 }
 
 __device__ __forceinline__ uint32_t pw_smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
@@ -201,6 +257,10 @@ multi_pointwise_splitcat_kernel(const PwGroup* __restrict__ groups, const int2* 
   const int ty_step = kPwThreads >> g.tx_log2;
   const int q = b.q0 + tx;
   if (q >= g.W) return;
+  if (g.ext_op) {                         // block-uniform: one chunk, no map
+    pw_ext_rows<BF16>(g, q, b.r0 + ty, b.r0 + b.nrows, ty_step);
+    return;
+  }
   const int2 m = __ldg(vmap + g.map_off + q);
   const int op = (int)((uint32_t)m.y >> 30);
   const int4* s = reinterpret_cast<const int4*>(g.src) + m.x;
@@ -232,6 +292,9 @@ struct CChunk {   // canonical chunk, in 16-byte vectors
   char* dst;
   int64_t lds16, ldd16;
   int32_t rows, wv, op;
+  const char* src2 = nullptr;     // EXT ops only
+  int64_t lds2_16 = 0;
+  float p0 = 0.f, p1 = 0.f, p2 = 0.f;
 };
 }  // namespace
 
@@ -253,7 +316,14 @@ extern "C" opt_status opt_pointwise_plan_create(const opt_chunk* chunks, int32_t
     const opt_chunk& c = chunks[i];
     if (!c.src || !c.dst) return fail(OPT_ERR_INVALID_ARG, "chunk %d: NULL pointer", i);
     if (c.rows < 1 || c.width < 1) return fail(OPT_ERR_INVALID_ARG, "chunk %d: rows=%d width=%d must be >= 1", i, c.rows, c.width);
-    if (c.op < OPT_PW_COPY || c.op > OPT_PW_SIGMOID) return fail(OPT_ERR_INVALID_ARG, "chunk %d: bad op %d", i, c.op);
+    if (c.op < OPT_PW_COPY || c.op > OPT_PW_MUL) return fail(OPT_ERR_INVALID_ARG, "chunk %d: bad op %d", i, c.op);
+    const bool ext = c.op >= OPT_PW_CLAMP, binary = c.op >= OPT_PW_SUB;
+    if (binary) {
+      if (!c.src2) return fail(OPT_ERR_INVALID_ARG, "chunk %d: binary op %d needs src2", i, c.op);
+      if (c.rows > 1 && c.lds2 < c.width) return fail(OPT_ERR_INVALID_ARG, "chunk %d: row stride of src2 smaller than width", i);
+      if (!aligned16(c.src2)) return fail(OPT_ERR_ALIGNMENT, "chunk %d: pointers must be 16-byte aligned", i);
+      if (c.rows > 1 && c.lds2 % V) return fail(OPT_ERR_ALIGNMENT, "chunk %d: row strides must be multiples of %d elements", i, V);
+    }
     if (c.rows > 1 && (c.lds < c.width || c.ldd < c.width))
       return fail(OPT_ERR_INVALID_ARG, "chunk %d: row stride smaller than width", i);
     if (!aligned16(c.src) || !aligned16(c.dst)) return fail(OPT_ERR_ALIGNMENT, "chunk %d: pointers must be 16-byte aligned", i);
@@ -262,10 +332,12 @@ extern "C" opt_status opt_pointwise_plan_create(const opt_chunk* chunks, int32_t
       return fail(OPT_ERR_ALIGNMENT, "chunk %d: row strides must be multiples of %d elements", i, V);
     regions.push_back({(uintptr_t)c.src, c.lds * esz, (int64_t)c.width * esz, c.rows, false, i});
     regions.push_back({(uintptr_t)c.dst, c.ldd * esz, (int64_t)c.width * esz, c.rows, true, i});
-    bytes += 2ll * c.rows * c.width * esz;
+    if (binary) regions.push_back({(uintptr_t)c.src2, c.lds2 * esz, (int64_t)c.width * esz, c.rows, false, i});
+    bytes += (binary ? 3ll : 2ll) * c.rows * c.width * esz;
 
     const int64_t wv = c.width / V;
-    const bool dense = c.rows == 1 || (c.lds == c.width && c.ldd == c.width);
+    const bool dense = c.rows == 1 || (c.lds == c.width && c.ldd == c.width && (!binary || c.lds2 == c.width));
+    const size_t cc0 = cc.size();
     if (dense) {
       const int64_t T = (int64_t)c.rows * wv;
       int64_t done = 0;
@@ -281,6 +353,15 @@ extern "C" opt_status opt_pointwise_plan_create(const opt_chunk* chunks, int32_t
       if (wv > INT32_MAX) return fail(OPT_ERR_UNSUPPORTED, "chunk %d too wide", i);
       cc.push_back({(const char*)c.src, (char*)c.dst, c.lds / V, c.ldd / V, c.rows, (int32_t)wv, c.op});
     }
+    if (ext)                                   // same re-tiling for the second operand; scalars ride along
+      for (size_t k = cc0; k < cc.size(); ++k) {
+        CChunk& e = cc[k];
+        if (binary) {
+          e.src2 = (const char*)c.src2 + (e.src - (const char*)c.src);     // dense pieces: same byte offset
+          e.lds2_16 = dense ? e.lds16 : c.lds2 / V;
+        }
+        e.p0 = c.p0; e.p1 = c.p1; e.p2 = c.p2;
+      }
   }
   if (opt_status st = check_independent(regions, /*allow_inplace_self=*/true)) return st;
   int num_sms = 0;
@@ -288,8 +369,11 @@ extern "C" opt_status opt_pointwise_plan_create(const opt_chunk* chunks, int32_t
 
   // ---- group canonical chunks by (rows, lds16, ldd16)
   std::map<std::tuple<int32_t, int64_t, int64_t>, std::vector<int>> buckets;
-  for (int i = 0; i < (int)cc.size(); ++i)
-    buckets[std::make_tuple(cc[i].rows, cc[i].lds16, cc[i].ldd16)].push_back(i);
+  std::vector<int> ext_ids;
+  for (int i = 0; i < (int)cc.size(); ++i) {
+    if (cc[i].op >= OPT_PW_CLAMP) ext_ids.push_back(i);                 // EXT mode: one group per chunk, no map
+    else buckets[std::make_tuple(cc[i].rows, cc[i].lds16, cc[i].ldd16)].push_back(i);
+  }
 
   std::vector<PwGroup> groups;
   std::vector<int2> vmap;
@@ -327,6 +411,7 @@ extern "C" opt_status opt_pointwise_plan_create(const opt_chunk* chunks, int32_t
       while ((1 << txl) < W && txl < 8) ++txl;
       g.tx_log2 = txl;
       g.src_span = g.dst_span = g.tile_rows = g.pad = 0;
+      g.ext_op = 0; g.src2 = nullptr; g.lds2_16 = 0; g.p0 = g.p1 = g.p2 = 0.f;
       // map entries, sorted by (op, dst)
       std::vector<int> order(ids.begin() + i0, ids.begin() + i1);
       std::stable_sort(order.begin(), order.end(), [&](int a, int b) { return cc[a].op < cc[b].op; });
@@ -376,6 +461,25 @@ extern "C" opt_status opt_pointwise_plan_create(const opt_chunk* chunks, int32_t
       groups.push_back(g);
       i0 = i1;
     }
+  }
+  for (int id : ext_ids) {
+    const CChunk& c = cc[id];
+    PwGroup g;
+    memset(&g, 0, sizeof g);
+    g.src = c.src; g.dst = c.dst; g.lds16 = c.lds16; g.ldd16 = c.ldd16; g.rows = c.rows; g.W = c.wv;
+    g.map_off = 0;
+    int txl = 0;
+    while ((1 << txl) < c.wv && txl < 8) ++txl;
+    g.tx_log2 = txl;
+    g.ext_op = c.op; g.src2 = c.src2; g.lds2_16 = c.lds2_16; g.p0 = c.p0; g.p1 = c.p1; g.p2 = c.p2;
+    const int TX = 1 << txl, TY = kPwThreads / TX;
+    int64_t rb = kVecPerBlock / std::min<int64_t>(c.wv, TX);
+    rb = std::max<int64_t>(TY, std::min<int64_t>(rb, g.rows));
+    rb = (rb + TY - 1) / TY * TY;
+    for (int64_t q0 = 0; q0 < c.wv; q0 += TX)
+      for (int64_t r0 = 0; r0 < g.rows; r0 += rb)
+        blocks.push_back({(int32_t)groups.size(), (int32_t)q0, (int32_t)r0, (int32_t)std::min<int64_t>(rb, g.rows - r0)});
+    groups.push_back(g);
   }
   if (blocks.size() > (size_t)INT32_MAX) return fail(OPT_ERR_UNSUPPORTED, "too many work items");
 

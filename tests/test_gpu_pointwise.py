@@ -142,3 +142,68 @@ def test_errors_launch_nothing(ob):
         ob.opt_pointwise_plan_create([], BF16)
     assert e.value.status == ob.OPT_ERR_INVALID_ARG
     assert ob.opt_launch_count() == n0
+
+
+# ---------------------------------------------- Table-1 patterns beyond relu/tanh/sigmoid --
+def _special(a_bits):
+    """sprinkle NaN / +inf / -inf / -0 into a bf16 bit array."""
+    a = a_bits.copy().reshape(-1)
+    a[3::97] = 0x7FC0; a[5::101] = 0x7F80; a[7::103] = 0xFF80; a[11::107] = 0x8000
+    return a.reshape(a_bits.shape)
+
+
+def test_table1_patterns_one_launch_mixed_group(ob):
+    """batch_clamp, batch_nan_to_num, batch_aten_sub / div / mul and a relu member in ONE launch: dense tensors,
+    strided column slices, special values; <= 2 bf16 ulp of the oracle, special values exactly."""
+    ops = [(oracle.PW_CLAMP, [-0.75, 1.25]), (oracle.PW_NAN_TO_NUM, [0.5, 100.0, -100.0]), (oracle.PW_SUB, []),
+           (oracle.PW_DIV, []), (oracle.PW_MUL, []), (oracle.PW_CLAMP, [2.0, 1.0]), (oracle.PW_MUL, [])]
+    shapes = [(300, 512), (77, 200), (1000, 64), (129, 1032), (64, 8), (5, 4096), (513, 256)]
+    host, chunks, keep = [], [], []
+    for i, ((op, prm), (r, w)) in enumerate(zip(ops, shapes)):
+        a = _special(wl.tensor_normal(41, 2 * i + 1, (r, w), 0.0, 2.0, BF16))
+        b = wl.tensor_normal(41, 2 * i + 2, (r, w), 0.5, 1.5, BF16) if op >= oracle.PW_SUB else None
+        strided = i % 2 == 1                               # odd members: column slices of wider buffers
+        pad = 16 if strided else 0
+        da = to_dev(np.pad(a, ((0, 0), (0, pad))), BF16)[:, :w] if strided else to_dev(a, BF16)
+        db = None if b is None else (to_dev(np.pad(b, ((0, 0), (8, pad))), BF16)[:, 8:8 + w] if strided else to_dev(b, BF16))
+        dd = empty_dev((r, w + pad), BF16, fill=float("nan"))[:, :w]
+        chunks.append(ob.chunk(da, dd, op, db, prm))
+        host.append((a, b, op, prm))
+        keep.append((da, db, dd))
+    x = wl.tensor_normal(41, 99, (256, 256), 0, 1, BF16)   # a plain relu member rides in the same launch
+    dx, dy = to_dev(x, BF16), empty_dev((256, 256), BF16)
+    chunks.append(ob.chunk(dx, dy, ob.OPT_PW_RELU))
+    plan = ob.opt_pointwise_plan_create(chunks, BF16)
+    n0 = ob.opt_launch_count()
+    plan.launch()
+    torch.cuda.synchronize()
+    assert ob.opt_launch_count() - n0 == 1
+    for (a, b, op, prm), (_, _, dd) in zip(host, keep):
+        ref = oracle.round_to_storage(oracle.pointwise_ext(a, b, op, prm, BF16), BF16)
+        got = to_host(dd)
+        d = bf16_ulp_distance(got, ref)
+        assert d.max() <= 2, (op, int(d.max()))
+        if op in (oracle.PW_CLAMP, oracle.PW_NAN_TO_NUM, oracle.PW_MUL):
+            nan = (ref & 0x7FFF) > 0x7F80                  # NaN stays NaN (payload is not part of the contract)
+            assert np.array_equal(got[~nan], ref[~nan]) and np.all((got[nan] & 0x7FFF) > 0x7F80)   # else exact
+    assert bf16_ulp_distance(to_host(dy), oracle.round_to_storage(oracle.pointwise(x, 1, BF16), BF16)).max() == 0
+
+
+def test_table1_patterns_fp32_and_errors(ob):
+    a = wl.tensor_normal(42, 1, (100, 36), 0, 2, F32)
+    b = wl.tensor_normal(42, 2, (100, 36), 1, 1, F32)
+    da, db = to_dev(a, F32), to_dev(b, F32)
+    outs = [empty_dev((100, 36), F32) for _ in range(3)]
+    plan = ob.opt_pointwise_plan_create([ob.chunk(da, outs[0], ob.OPT_PW_DIV, db), ob.chunk(da, outs[1], ob.OPT_PW_SUB, db),
+                                         ob.chunk(da, outs[2], ob.OPT_PW_CLAMP, None, [-1.0, 0.5])], F32)
+    plan.launch()
+    torch.cuda.synchronize()
+    for o, op, prm in zip(outs, (oracle.PW_DIV, oracle.PW_SUB, oracle.PW_CLAMP), ([], [], [-1.0, 0.5])):
+        ref = oracle.round_to_storage(oracle.pointwise_ext(a, b if op != oracle.PW_CLAMP else None, op, prm, F32), F32)
+        assert np.array_equal(to_host(o), ref)             # fp32: IEEE sub / div, correctly rounded
+    with pytest.raises(ob.OptError) as e:                  # binary op without a second operand
+        ob.opt_pointwise_plan_create([ob.chunk(da, outs[0], ob.OPT_PW_MUL)], F32)
+    assert e.value.status == ob.OPT_ERR_INVALID_ARG
+    with pytest.raises(ob.OptError) as e:                  # second operand overlaps another member's output
+        ob.opt_pointwise_plan_create([ob.chunk(da, outs[0], ob.OPT_PW_MUL, db), ob.chunk(da, outs[1], ob.OPT_PW_MUL, outs[0])], F32)
+    assert e.value.status == ob.OPT_ERR_ALIAS
