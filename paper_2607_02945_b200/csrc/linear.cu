@@ -35,6 +35,9 @@
 //   grouped_gemm_f32_kernel    plain fp32 FFMA (no TF32) 64x64 tiles for fp32
 //       groups (configs[0]); same tile scheduler, accurate tanhf/expf epilogue.
 #include <algorithm>
+#include <map>
+#include <set>
+#include <tuple>
 #include <cstdlib>
 
 #include "sm100_ptx.h"
@@ -472,6 +475,7 @@ extern "C" opt_status opt_linear_plan_create(const opt_linear_member* members, i
   const int esz = elem_size(io), V = vec_elems(io);
   std::vector<Region> regions;
   int64_t flops = 0, bytes = 0;
+  std::set<std::tuple<const void*, int64_t, int32_t, int32_t>> seen_x;
   for (int32_t i = 0; i < n; ++i) {
     const opt_linear_member& m = members[i];
     if (!m.x || !m.w || !m.y) return fail(OPT_ERR_INVALID_ARG, "member %d: NULL pointer", i);
@@ -488,7 +492,9 @@ extern "C" opt_status opt_linear_plan_create(const opt_linear_member* members, i
     if (m.bias) regions.push_back({(uintptr_t)m.bias, 0, (int64_t)m.N * esz, 1, false, i});
     regions.push_back({(uintptr_t)m.y, m.ldy * esz, (int64_t)m.N * esz, m.M, true, i});
     flops += 2ll * m.M * m.N * m.K;
-    bytes += ((int64_t)m.M * m.K + (int64_t)m.N * m.K + (m.bias ? m.N : 0) + (int64_t)m.M * m.N) * esz;
+    // an input shared by several members (batch_linear_lhs) is read once
+    const bool first_use_of_x = seen_x.insert(std::make_tuple(m.x, m.ldx, m.M, m.K)).second;
+    bytes += ((first_use_of_x ? (int64_t)m.M * m.K : 0) + (int64_t)m.N * m.K + (m.bias ? m.N : 0) + (int64_t)m.M * m.N) * esz;
   }
   if (opt_status st = check_independent(regions, /*allow_inplace_self=*/false)) return st;
 
@@ -560,25 +566,43 @@ extern "C" opt_status opt_linear_plan_create(const opt_linear_member* members, i
     tiles += (int64_t)nmb * tl.nbn;
     if (tiles > INT32_MAX / 2) { delete p; return fail(OPT_ERR_UNSUPPORTED, "too many tiles"); }
   }
-  // Schedule order: member-major, m-block, n-block -- the n-blocks of one X row panel are adjacent, so the
+  // Schedule order: (LHS group,) member-major, m-block, n-block -- the n-blocks of one X row panel are adjacent, so the
   // CTAs that take them side by side fetch the panel from HBM once (re-reads hit L2), and a member's W stays
   // hot in L2 while its tiles are in flight.  (Interleaving tensor-bound with HBM-bound members was measured:
   // no gain on configs[2], the kernel is bound by L2->SM operand traffic there.)
+  // batch_linear_lhs: members that share ONE input X (same pointer, stride, M, K) form an LHS group
+  // whose schedule is m-block-major ACROSS its members -- all n-blocks of all members that read a given X row
+  // panel are adjacent, so the panel is fetched from HBM once for the whole group (weights logically concatenated).
   std::vector<TileEntry> flat;
   flat.reserve((size_t)tiles);
-  for (int32_t i = 0; i < n; ++i) {
+  auto push_tiles = [&](int32_t i, int mb) {
     const opt_linear_member& m = members[i];
     const MemberTiling& tl = tiling[i];
-    const int nmb = (m.M + tile_m - 1) / tile_m;
-    for (int mb = 0; mb < nmb; ++mb)
-      for (int nb = 0; nb < tl.nbn; ++nb) {
-        TileEntry e;
-        e.member = i; e.m0 = mb * tile_m; e.n0 = nb * tl.bn; e.idesc = tl.idesc;
-        e.bn_nkb = (uint32_t)tl.bn | ((uint32_t)tl.nkb << 16);
-        e.misc = (uint32_t)tl.klast | ((uint32_t)m.act << 8) | ((uint32_t)std::min(tl.bn, m.N - e.n0) << 16);
-        e.bias = m.bias ? static_cast<const char*>(m.bias) + (size_t)e.n0 * 2 : nullptr;
-        flat.push_back(e);
-      }
+    for (int nb = 0; nb < tl.nbn; ++nb) {
+      TileEntry e;
+      e.member = i; e.m0 = mb * tile_m; e.n0 = nb * tl.bn; e.idesc = tl.idesc;
+      e.bn_nkb = (uint32_t)tl.bn | ((uint32_t)tl.nkb << 16);
+      e.misc = (uint32_t)tl.klast | ((uint32_t)m.act << 8) | ((uint32_t)std::min(tl.bn, m.N - e.n0) << 16);
+      e.bias = m.bias ? static_cast<const char*>(m.bias) + (size_t)e.n0 * 2 : nullptr;
+      flat.push_back(e);
+    }
+  };
+  {
+    std::map<std::tuple<const void*, int64_t, int32_t, int32_t>, std::vector<int32_t>> lhs;
+    std::vector<std::tuple<const void*, int64_t, int32_t, int32_t>> first_seen;
+    for (int32_t i = 0; i < n; ++i) {
+      const auto key = std::make_tuple(members[i].x, members[i].ldx, members[i].M, members[i].K);
+      if (lhs.find(key) == lhs.end()) first_seen.push_back(key);
+      lhs[key].push_back(i);
+    }
+    const bool no_lhs = getenv("OPT_GEMM_NO_LHS") != nullptr;                              // experiment knob
+    if (no_lhs) { first_seen.clear(); for (int32_t i = 0; i < n; ++i) { const int nmb = (members[i].M + tile_m - 1) / tile_m; for (int mb = 0; mb < nmb; ++mb) push_tiles(i, mb); } }
+    for (const auto& key : first_seen) {
+      const std::vector<int32_t>& grp = lhs[key];
+      const int nmb = (std::get<2>(key) + tile_m - 1) / tile_m;
+      for (int mb = 0; mb < nmb; ++mb)
+        for (int32_t i : grp) push_tiles(i, mb);
+    }
   }
   // Chunks of 4 tiles (one 128-byte line, one atomic); the last ~3 waves go one tile per chunk so that the
   // tail of the persistent loop is balanced at tile granularity.
