@@ -45,7 +45,7 @@ SMALL = dict(c1_rows=256, c1_n=16, c2_M=512, c2_n=16, c3_rows=512, c3_width=2048
 
 # dram__bytes_read.sum + dram__bytes_write.sum of the three grouped-GEMM launches of one step (C2, C4b, C4c), from
 # the committed `ncu --set full` capture profiles/r01_profiles.md section 2 (algorithmic: 7 912 453 120 bytes)
-GEMM_DRAM_TRAFFIC_PER_STEP = 7_855_398_000
+GEMM_DRAM_TRAFFIC_PER_STEP = 7_843_725_000
 
 
 def load_peaks():
