@@ -492,6 +492,53 @@ def aggregate_steps_per_s(us_step, world):
     return world / (us_step * 1e-6)
 
 
+# ------------------------------------------------------- side workloads ------
+def run_side(args):
+    """Small stand-alone workloads for ncu captures of the section-8(f) items (profiles/r01_profiles.md section 4):
+      --side linear2   C4's two GEMM groups as one chained-Linear launch (opt_linear2), 3 launches
+      --side lhs       batch_linear_lhs: 8 members (N=64) on ONE input X [262144, 512]; OPT_GEMM_NO_LHS=1 = plain order
+    Prints one JSON line; not the bench metric."""
+    import torch
+    import paper_2607_02945_b200 as ob
+    torch.cuda.set_device(0)
+    stream = torch.cuda.current_stream()
+
+    def timed(fn, n=5):
+        flush = torch.empty(256 * 1024 * 1024, dtype=torch.uint8, device="cuda")
+        ts = []
+        for _ in range(n):
+            flush.fill_(1)
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(stream); fn(); e1.record(stream)
+            torch.cuda.synchronize()
+            ts.append(e0.elapsed_time(e1) * 1e3)
+        return float(np.mean(ts))
+
+    if args.side == "linear2":
+        step = Step("cuda:0", FULL, pinned_host=False, configs=("c4",))
+        ga, gb, gc = step.groups
+        T, A = ga.ain.tensor, ga.amid.tensor
+        out2 = torch.empty_like(gc.aout.tensor(ga.iy))
+        descs = [ob.linear2_member(A(i["xn"]), T(i["w1"]), T(i["b1"]), T(i["w2"]), T(i["b2"]),
+                                   out2[:, k * t["out"]:(k + 1) * t["out"]], ACT_RELU, ACT_NONE)
+                 for k, (i, t) in enumerate(zip(ga.idx, ga.cfg["towers"]))]
+        plan = ob.opt_linear2_plan_create(descs, BF16, 0)
+        ga.plan.launch()
+        torch.cuda.synchronize()
+        print(json.dumps(dict(side="linear2", us=round(timed(plan.launch, 3), 1), **plan.info())))
+    else:
+        M, K, N, n = 262144, 512, 64, 8
+        g = torch.Generator(device="cuda").manual_seed(0)
+        x = torch.randn(M, K, device="cuda", generator=g).to(torch.bfloat16)
+        ws = [(torch.randn(N, K, device="cuda", generator=g) * K ** -0.5).to(torch.bfloat16) for _ in range(n)]
+        ycat = torch.empty(M, N * n, device="cuda", dtype=torch.bfloat16)
+        plan = ob.opt_linear_plan_create([ob.linear_member(x, w, None, ycat[:, i * N:(i + 1) * N], ACT_RELU)
+                                          for i, w in enumerate(ws)], BF16, 0)
+        print(json.dumps(dict(side="lhs", lhs_order=os.environ.get("OPT_GEMM_NO_LHS") is None,
+                              us=round(timed(plan.launch, 3), 1), **plan.info())))
+    return 0
+
+
 # -------------------------------------------------------------- product arm --
 def run_product(args):
     import torch
@@ -748,7 +795,10 @@ def main():
     ap.add_argument("--profile", action="store_true",
                     help="only the step's own launches (no cpu_baseline, no unfused baseline, no copy reference): for ncu")
     ap.add_argument("--ref-frac", type=float, default=0.0, help="reference arm: override the row-sample fraction")
+    ap.add_argument("--side", default=None, choices=["linear2", "lhs"], help="stand-alone side workload for ncu (not the metric)")
     args = ap.parse_args()
+    if args.side:
+        return run_side(args)
     if args.impl == "reference":
         return run_reference(args)
     return run_product(args)
