@@ -11,15 +11,15 @@
 //
 // Kernel: persistent, one CTA per SM, 384 threads, per 128-row tile of a member:
 //   warp 0  TMA producer: the X tile (K <= 256: up to four 128x64 k-blocks, resident for the whole tile), a
-//           5-stage ring of W1 k-blocks (128 hidden units x 64), a 2-stage ring of W2 slices (N x 128);
+//           4-stage ring of W1 k-blocks (128 hidden units x 64), a 2-stage ring of W2 slices (N x 128);
 //   warp 1  layer-1 MMA issuer: per hidden chunk c of 128 units  acc1[c&1] = X . W1_c^T  (M=128, N<=128); it
 //           never waits for a hidden tile, so the tensor pipe has work while the epilogue turns acc1 into h;
 //   warp 11 layer-2 MMA issuer: acc2 += h_c . W2_c^T (M=128, N<=64, K<=128) as soon as h_c is published
 //           (two issuing threads: a single one was instruction-bound on these short MMAs);
 //   warp 2  tile scheduler (dynamic, one atomic per 4 tiles; entry + b1 + b2 into a 4-deep queue);
 //   warps 3..10  epilogue: acc1 chunk -> +b1, act1, RNE bf16 -> the hidden tile in shared memory, written
-//           directly in the K-major 128-byte-swizzled layout MMA2 reads; after the last
-//           chunk acc2 -> +b2, act2, RNE -> staging -> TMA store into the member's output / concat slot.
+//           directly in the K-major 128-byte-swizzled layout MMA2 reads; a tile's acc2 is drained late (after the
+//           next tile's first chunk): + b2, act2, RNE -> staging -> TMA store into the output / concat slot.
 //   TMEM: acc1 2 x 128 columns, acc2 2 x 64 columns.
 #include <algorithm>
 #include <cstdlib>
@@ -34,7 +34,7 @@ constexpr int kT_HC = 128;            // hidden chunk: UMMA N of layer 1, K of l
 constexpr int kT_MaxK = 256;          // layer-1 K (input features): the X tile is at most 4 k-blocks
 constexpr int kT_MaxH = 512;          // hidden width: b1 travels in the queue slot
 constexpr int kT_MaxN = 64;           // layer-2 N
-constexpr int kT_W1Stages = 5;
+constexpr int kT_W1Stages = 4;
 constexpr int kT_EpiWarps = 8;
 constexpr int kT_FirstEpiWarp = 3;
 constexpr int kT_Mma2Warp = kT_FirstEpiWarp + kT_EpiWarps;     // warp 11: layer-2 MMA issuer
@@ -48,8 +48,8 @@ constexpr int kT_OffX = 0;
 constexpr int kT_OffW1 = kT_OffX + (kT_MaxK / kT_BK) * kT_KBlockBytes;            //  64 KB
 constexpr int kT_OffH = kT_OffW1 + kT_W1Stages * kT_KBlockBytes;                  // +96 KB
 constexpr int kT_OffW2 = kT_OffH + 2 * kT_KBlockBytes;                            // +32 KB (one hidden tile: 2 k-blocks)
-constexpr int kT_OffOut = kT_OffH;                                                // output staging aliases the hidden tile
-constexpr int kT_OffQ = kT_OffW2 + 2 * 2 * kT_W2KBlockBytes;                      // +32 KB
+constexpr int kT_OffOut = kT_OffW2 + 2 * 2 * kT_W2KBlockBytes;                    // +32 KB
+constexpr int kT_OffQ = kT_OffOut + 4 * 4096;                                     // +16 KB output staging (4 warps x 32 rows x 128 B)
 constexpr int kT_OffBar = kT_OffQ + kT_QDepth * kT_QSlotBytes;
 constexpr int kT_SmemBytes = kT_OffBar + 512;
 static_assert(kT_SmemBytes <= 227 * 1024, "chained-GEMM shared memory map exceeds 227 KB");
@@ -330,14 +330,53 @@ grouped_linear2_sm100_kernel(const L2Member* __restrict__ members, const uint4* 
     }
   } else {
     // ----------------------------------------------------------- epilogue ----
+    // Per hidden chunk: acc1 -> registers -> + b1, act1, RNE -> the hidden tile in shared memory (layer-2 A operand).
+    // The layer-2 accumulator of a row tile is drained LATE, after the first hidden chunk of the NEXT tile has been
+    // published: by then its MMAs have long retired, so the warps never sit waiting for them.
     const int ew = warp - kT_FirstEpiWarp;
     const int quad = warp & 3;               // TMEM lane quadrant this warp may read
     const int half = ew >> 2;                // which 64-column half of a 128-wide hidden chunk
     const uint32_t lane_off = (uint32_t)(quad * 32) << 16;
     const uint32_t row_off = (uint32_t)(quad * 32 + lane) * 128u;      // this thread's row inside a k-block
-    const uint32_t sbuf = sbase + kT_OffOut + (uint32_t)quad * 4096u;  // output staging (warps with half == 0)
     int qs = 0; uint32_t qph = 0;
     uint32_t gt = 0, gh = 0;
+    // the tile whose layer-2 accumulator is still to be drained
+    bool pend = false;
+    uint32_t p_slot = 0, p_gt = 0;
+    int p_qs = 0, p_act2 = 0, p_m0 = 0;
+    const L2Member* p_m = nullptr;
+    const uint32_t sbuf = sbase + kT_OffOut + (uint32_t)quad * 4096u;  // output staging (warps with half == 0)
+    auto drain = [&]() {
+      const uint32_t s2 = p_gt & 1u;
+      mbar_wait(a2_full(s2), (p_gt >> 1) & 1u);
+      tc_fence_after();
+      uint32_t v[64], p[32];
+      {
+        const uint32_t t = tmem_base + lane_off + 256u + s2 * 64u;
+        tc_ld_32x32(t, *reinterpret_cast<uint32_t(*)[32]>(&v[0]));
+        tc_ld_32x32(t + 32, *reinterpret_cast<uint32_t(*)[32]>(&v[32]));
+        tc_wait_ld();
+      }
+      tc_fence_before();
+      __syncwarp();
+      if (lane == 0) mbar_arrive(a2_empty(s2));
+      if (half == 0) {
+        epi_act(v, p_slot + kT_MaxH * 2, p_act2, p);
+        if (lane == 0) tma_store_wait_read<0>();       // this warp's previous store has read the staging tile
+        __syncwarp();
+#pragma unroll
+        for (int j = 0; j < 8; ++j)
+          sts128(sbuf + lane * 128 + ((j ^ (lane & 7)) << 4), make_uint4(p[4 * j], p[4 * j + 1], p[4 * j + 2], p[4 * j + 3]));
+        fence_proxy_async_smem();
+        __syncwarp();
+        if (lane == 0) {
+          tma_store_2d(&p_m->tmY, sbuf, 0, p_m0 + quad * 32);
+          tma_store_commit();
+        }
+      }
+      __syncwarp();                          // every lane has read the slot's b2
+      if (lane == 0) mbar_arrive(q_empty(p_qs));
+    };
     for (;;) {
       mbar_wait(q_full(qs), qph);
       const uint32_t slot = q_slot(qs);
@@ -367,10 +406,8 @@ grouped_linear2_sm100_kernel(const L2Member* __restrict__ members, const uint4* 
         __syncwarp();
         if (lane == 0) mbar_arrive(a1_empty(s));       // acc1 stage is in registers: MMA1 of chunk c+2 may overwrite it
         epi_act(v, slot + (uint32_t)(c * kT_HC + half * 64) * 2u, act1, p);
-        // the hidden tile is single-buffered: MMA2 of chunk c-1 sits right behind MMA1 of chunk c in the tensor
-        // pipe, so it has retired by the time this chunk's accumulator has been read and converted.  (The tile
-        // also serves as the output staging of the previous row tile: that TMA store must have read it.)
-        if (half == 0 && lane == 0) tma_store_wait_read<0>();
+        // the hidden tile is single-buffered: MMA2 of chunk c-1 has normally retired by the time this chunk's
+        // accumulator has been read and converted
         mbar_wait(h_empty(0), (g & 1u) ^ 1u);
         if (mine) {
           const uint32_t hrow = sbase + kT_OffH + (uint32_t)half * kT_KBlockBytes + row_off;
@@ -381,42 +418,15 @@ grouped_linear2_sm100_kernel(const L2Member* __restrict__ members, const uint4* 
         fence_proxy_async_smem();                      // generic-proxy writes -> visible to the tensor core's reads
         __syncwarp();
         if (lane == 0) mbar_arrive(h_full(0));
+        if (c == 0 && pend) { drain(); pend = false; }
       }
       gh += (uint32_t)nch;
-      // ---- layer-2 accumulator of the tile
-      {
-        const int s2 = (int)(gt & 1u);
-        mbar_wait(a2_full(s2), (gt >> 1) & 1u);
-        tc_fence_after();
-        uint32_t v[64], p[32];
-        {
-          const uint32_t t = tmem_base + lane_off + 256u + (uint32_t)s2 * 64u;
-          tc_ld_32x32(t, *reinterpret_cast<uint32_t(*)[32]>(&v[0]));
-          tc_ld_32x32(t + 32, *reinterpret_cast<uint32_t(*)[32]>(&v[32]));
-          tc_wait_ld();
-        }
-        tc_fence_before();
-        __syncwarp();
-        if (lane == 0) mbar_arrive(a2_empty(s2));
-        if (half == 0) {
-          epi_act(v, slot + kT_MaxH * 2, act2, p);
-          // staging = this warp's own 32 rows of the hidden tile's first k-block: free, every MMA2 of the tile retired
-#pragma unroll
-          for (int j = 0; j < 8; ++j)
-            sts128(sbuf + lane * 128 + ((j ^ (lane & 7)) << 4), make_uint4(p[4 * j], p[4 * j + 1], p[4 * j + 2], p[4 * j + 3]));
-          fence_proxy_async_smem();
-          __syncwarp();
-          if (lane == 0) {
-            tma_store_2d(&m->tmY, sbuf, 0, m0 + quad * 32);
-            tma_store_commit();
-          }
-        }
-        ++gt;
-      }
-      __syncwarp();                          // every lane has read the slot's biases
-      if (lane == 0) mbar_arrive(q_empty(qs));
+      pend = true;
+      p_slot = slot; p_gt = gt; p_qs = qs; p_act2 = act2; p_m0 = m0; p_m = m;
+      ++gt;
       if (++qs == kT_QDepth) { qs = 0; qph ^= 1; }
     }
+    if (pend) drain();
     if (lane == 0) tma_store_wait_all();
   }
 
