@@ -33,8 +33,12 @@
  *   - Unsupported or misaligned groups launch NOTHING and return an error: the
  *     "guaranteed no-op fallback" of PAPER.md:183.  There is no CPU fallback.
  *   - Alignment (8 elements for bf16): bf16 paths need 16-byte
- *     aligned base pointers, ld* % 8 == 0, K % 8 == 0, N % 8 == 0, D % 8 == 0,
- *     width % 8 == 0.  fp32 paths need 16-byte aligned bases and multiples of 4.
+ *     aligned base pointers, ld* % 8 == 0, D % 8 == 0, width % 8 == 0.  The
+ *     grouped Linear takes ANY K and N (the tails are zero-filled on chip --
+ *     what pad_aten_mm_pass does by padding); when N % 8 != 0 the padding
+ *     elements of y up to the next 16-byte boundary of each row are overwritten
+ *     (nothing else can live there: every base is 16-byte aligned).  fp32 paths need 16-byte aligned
+ *     bases and multiples of 4.
  *   - 1 <= n <= 65535 members, every dimension >= 1 (members with rows == 0 are
  *     rejected as OPT_ERR_INVALID_ARG).
  *   - opt_plan_launch is asynchronous on the given stream: exactly one kernel

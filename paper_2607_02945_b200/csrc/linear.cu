@@ -249,7 +249,15 @@ grouped_gemm_sm100_kernel(const GemmMember* __restrict__ members, const uint4* _
           const uint4* bp = reinterpret_cast<const uint4*>(((uint64_t)bhi << 32) | blo);
           bias_v[g] = make_uint4(0, 0, 0, 0);
           if (member[g] >= 0) {
-            if (bp != nullptr && 8 * lane < (int)(misc >> 16)) bias_v[g] = __ldg(bp + lane);
+            const int nvalid = (int)(misc >> 16);
+            if (bp != nullptr && 8 * lane + 8 <= nvalid) {
+              bias_v[g] = __ldg(bp + lane);
+            } else if (bp != nullptr && 8 * lane < nvalid) {       // ragged N: the last piece element by element
+              const unsigned short* be = reinterpret_cast<const unsigned short*>(bp + lane);
+              uint32_t w[4] = {0, 0, 0, 0};
+              for (int t = 0; t < nvalid - 8 * lane; ++t) w[t >> 1] |= (uint32_t)__ldg(be + t) << (16 * (t & 1));
+              bias_v[g] = make_uint4(w[0], w[1], w[2], w[3]);
+            }
             if (lane < 4)   // warm the descriptor cache for the member's tensor maps
               asm volatile("prefetch.tensormap [%0];" ::"l"(reinterpret_cast<const char*>(members + member[g]) + 128 * lane) : "memory");
           }
@@ -485,7 +493,11 @@ extern "C" opt_status opt_linear_plan_create(const opt_linear_member* members, i
       return fail(OPT_ERR_INVALID_ARG, "member %d: row stride smaller than the row", i);
     if (!aligned16(m.x) || !aligned16(m.w) || !aligned16(m.y) || !aligned16(m.bias))
       return fail(OPT_ERR_ALIGNMENT, "member %d: pointers must be 16-byte aligned", i);
-    if (m.K % V || m.N % V) return fail(OPT_ERR_ALIGNMENT, "member %d: K=%d and N=%d must be multiples of %d (PAPER.md:445)", i, m.K, m.N, V);
+    // bf16: K and N need NOT be multiples of 8 -- TMA zero-fills the K / N tails of the operand tiles and clips the
+    // store, which is what pad_aten_mm_pass achieves by padding; only bases and row strides must be
+    // 16-byte aligned.  fp32 (SIMT path): multiples of 4.
+    if (io == OPT_F32 && (m.K % V || m.N % V))
+      return fail(OPT_ERR_ALIGNMENT, "member %d: K=%d and N=%d must be multiples of %d", i, m.K, m.N, V);
     if (m.ldx % V || m.ldw % V || m.ldy % V) return fail(OPT_ERR_ALIGNMENT, "member %d: row strides must be multiples of %d elements", i, V);
     regions.push_back({(uintptr_t)m.x, m.ldx * esz, (int64_t)m.K * esz, m.M, false, i});
     regions.push_back({(uintptr_t)m.w, m.ldw * esz, (int64_t)m.K * esz, m.N, false, i});

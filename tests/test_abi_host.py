@@ -67,7 +67,7 @@ def test_host_validation_runs_before_any_cuda_call(ob):
     import torch
     A, B, Cc = 0x10000000, 0x20000000, 0x30000000
     mk = lambda **kw: ob.opt_linear_member(**{**dict(x=A, ldx=64, w=B, ldw=64, bias=None, y=Cc, ldy=64, M=128, N=64, K=64, act=0), **kw})
-    for member, status in [(mk(K=60), ob.OPT_ERR_ALIGNMENT), (mk(x=A + 2), ob.OPT_ERR_ALIGNMENT),
+    for member, status in [(mk(ldx=60), ob.OPT_ERR_INVALID_ARG), (mk(ldx=68), ob.OPT_ERR_ALIGNMENT), (mk(x=A + 2), ob.OPT_ERR_ALIGNMENT),
                            (mk(M=0), ob.OPT_ERR_INVALID_ARG), (mk(act=9), ob.OPT_ERR_INVALID_ARG),
                            (mk(y=A), ob.OPT_ERR_ALIAS), (mk(ldy=32), ob.OPT_ERR_INVALID_ARG)]:
         with pytest.raises(ob.OptError) as e:

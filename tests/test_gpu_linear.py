@@ -157,8 +157,9 @@ def test_errors(ob):
     with pytest.raises(ob.OptError) as e:   # overlapping concat slots
         ob.opt_linear_plan_create([ob.linear_member(x, w, None, y[:, 0:64]), ob.linear_member(x, w, None, y[:, 32:96])], BF16)
     assert e.value.status == ob.OPT_ERR_ALIAS
-    with pytest.raises(ob.OptError) as e:   # K not a multiple of 8
-        ob.opt_linear_plan_create([ob.linear_member(x[:, :60], w[:, :60], None, y[:, :64])], BF16)
+    with pytest.raises(ob.OptError) as e:   # row stride not a multiple of 8 elements (16 bytes)
+        xs = empty_dev((64, 68), BF16, fill=0.0)
+        ob.opt_linear_plan_create([ob.linear_member(xs[:, :64], w, None, y[:, :64])], BF16)
     assert e.value.status == ob.OPT_ERR_ALIGNMENT
     with pytest.raises(ob.OptError) as e:   # output aliases input
         ob.opt_linear_plan_create([ob.linear_member(x, w, None, x)], BF16)
@@ -208,3 +209,34 @@ def test_single_cta_kernel_matches_the_cta_pair_kernel(ob, monkeypatch):
     single, _ = run_linear(ob, members, BF16)
     for a, b in zip(pair, single):
         assert a.tobytes() == b.tobytes()
+
+
+def test_unaligned_K_and_N_zero_filled_on_chip(ob):
+    """pad_aten_mm_pass pads K / N to a multiple of 8 so that the aligned kernel can run; here K and N
+    may be anything (16-byte aligned bases and row strides): the tails are zero-filled by TMA, the store is clipped.
+    Integers -> bit-exact vs the oracle; random values within the GEMM tolerance; columns past the 16-byte granule
+    that holds column N-1 stay untouched."""
+    rng = np.random.default_rng(9)
+    shapes = [(200, 13, 13), (64, 52, 100), (130, 20, 72), (257, 300, 7), (3, 1, 1), (128, 129, 65)]     # (M, N, K)
+    members = [int_member(rng, M, N, K, 1, i % 2) for i, (M, N, K) in enumerate(shapes)]
+    members += [mk(61, i, M, N, K, (i + 2) % 4) for i, (M, N, K) in enumerate(shapes)]
+    dev = []
+    for m in members:
+        ldk, ldn = (m["K"] + 7) // 8 * 8 + 8, (m["N"] + 7) // 8 * 8 + 8          # padded, 16-byte aligned row strides
+        x = empty_dev((m["M"], ldk), BF16, fill=float("nan")); x[:, :m["K"]] = to_dev(m["x"], BF16)
+        w = empty_dev((m["N"], ldk), BF16, fill=float("nan")); w[:, :m["K"]] = to_dev(m["w"], BF16)
+        b = empty_dev((1, ldn), BF16, fill=float("nan")); b[0, :m["N"]] = to_dev(m["b"], BF16)
+        y = empty_dev((m["M"], ldn), BF16, fill=float("nan"))
+        dev.append((x, w, b, y))
+    descs = [ob.linear_member(x[:, :m["K"]], w[:, :m["K"]], b[0, :m["N"]], y[:, :m["N"]], m["act"]) for (x, w, b, y), m in zip(dev, members)]
+    ob.opt_linear_plan_create(descs, BF16).launch()
+    torch.cuda.synchronize()
+    z64, ref = graphs.linear_group(members, BF16)
+    for k, ((x, w, b, y), m, z, r) in enumerate(zip(dev, members, z64, ref)):
+        got = to_host(y)
+        if k < len(shapes):
+            assert got[:, :m["N"]].tobytes() == r.tobytes(), shapes[k]
+        else:
+            assert row_l2_rel_err(got[:, :m["N"]], z, BF16) <= TOL_BF16
+        n8 = (m["N"] + 7) // 8 * 8      # the store is clipped at 16-byte granularity: only the granule holding column N-1
+        assert np.all((got[:, n8:] & 0x7FFF) > 0x7F80)                          # columns past it still NaN
