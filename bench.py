@@ -663,6 +663,57 @@ def run_product(args):
         except Exception as e:  # noqa: BLE001
             unfused = dict(error=repr(e))
 
+    # ---- (5b) configs[0] (tiny fp32 group, launch-latency bound): latency of the one fused launch next to the
+    # eight launches of the unfused graph (4 x Linear + 4 x tanh), 200 back-to-back launches each; no roofline claim
+    c0 = None
+    if not args.profile:
+        try:
+            cfg0 = wl.config0()
+            t32 = lambda a: torch.from_numpy(np.ascontiguousarray(a)).to(device)
+            d0 = [(t32(m["x"]), t32(m["w"]), t32(m["b"]), torch.empty((m["M"], m["N"]), dtype=torch.float32, device=device))
+                  for m in cfg0["members"]]
+            fused = ob.opt_linear_plan_create([ob.linear_member(x, w, b, y, m["act"]) for (x, w, b, y), m in zip(d0, cfg0["members"])], F32, step.dev_index)
+            singles = []
+            for (x, w, b, y), m in zip(d0, cfg0["members"]):
+                singles.append(ob.opt_linear_plan_create([ob.linear_member(x, w, b, y, ACT_NONE)], F32, step.dev_index))
+                singles.append(ob.opt_pointwise_plan_create([ob.chunk(y, y, m["act"])], F32, step.dev_index))
+
+            def lat(fn, n=200):
+                for _ in range(10):
+                    fn()
+                torch.cuda.synchronize()
+                a, b_ = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                a.record(stream)
+                for _ in range(n):
+                    fn()
+                b_.record(stream)
+                torch.cuda.synchronize()
+                return a.elapsed_time(b_) * 1e3 / n
+            def graph_lat(plans, reps=50):      # the same launches replayed from one CUDA graph: GPU-side latency only
+                gr, cs = torch.cuda.CUDAGraph(), torch.cuda.Stream()
+                cs.wait_stream(stream)
+                with torch.cuda.graph(gr, stream=cs):
+                    for _ in range(reps):
+                        for p_ in plans:
+                            p_.launch(cs.cuda_stream)
+                gr.replay()
+                torch.cuda.synchronize()
+                a, b_ = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                a.record(stream)
+                for _ in range(4):
+                    gr.replay()
+                b_.record(stream)
+                torch.cuda.synchronize()
+                return a.elapsed_time(b_) * 1e3 / (4 * reps)
+            c0 = dict(workload="configs[0]: 4 Linear+bias+tanh members, fp32, M=64", fused_launches=1,
+                      fused_us=round(lat(fused.launch), 2), fused_graph_us=round(graph_lat([fused]), 2),
+                      unfused_launches=len(singles), unfused_us=round(lat(lambda: [p.launch() for p in singles]), 2),
+                      unfused_graph_us=round(graph_lat(singles), 2),
+                      note="*_us: launched one by one from the host (Python + ctypes: host-bound); *_graph_us: replayed "
+                           "from a CUDA graph")
+        except Exception as e:  # noqa: BLE001
+            c0 = dict(error=repr(e))
+
     # ---- (6) SURVEY 8(f) rank 1, side figure (NOT part of the step): C4's two GEMM groups as ONE chained-Linear
     # launch (opt_linear2, hidden tensor on chip) next to the two-launch path, isolated, cold L2, same tensors
     vertical = None
@@ -766,7 +817,7 @@ def run_product(args):
                              "copies overlap, single_stream_us: everything on one stream"),
                 gpu_launches=int(launches), launches_per_step=ng,
                 clocks=watch.summary(), roofline=roofline, roofline_tensor=roofline_tensor, groups=groups,
-                unfused_baseline=unfused, vertical_fusion=vertical,
+                unfused_baseline=unfused, vertical_fusion=vertical, config0_latency=c0,
                 aggregate=dict(steps_per_s=round(aggregate_steps_per_s(us_step, world), 2)),
                 build_seconds=round(build_s, 1), lib=ob.opt_version())
 

@@ -32,7 +32,7 @@
 //       tile t overlaps the MMAs of tile t+1.  Tiles of one X row-panel are
 //       adjacent in the schedule so its re-reads hit L2.  Deterministic: the
 //       scheduler only decides WHICH CTA computes a tile, never how.
-//   grouped_gemm_f32_kernel    plain fp32 FFMA (no TF32) 64x64 tiles for fp32
+//   grouped_gemm_f32_kernel    plain fp32 FFMA (no TF32) 32x32 tiles for fp32
 //       groups (configs[0]); same tile scheduler, accurate tanhf/expf epilogue.
 #include <algorithm>
 #include <map>
@@ -53,7 +53,7 @@ struct F32Member {
   int32_t pad;
 };
 
-constexpr int kF32Tile = 64, kF32BK = 16, kF32Threads = 256;
+constexpr int kF32Tile = 32, kF32BK = 32, kF32Threads = 256;
 
 __device__ __forceinline__ int find_member(const int32_t* __restrict__ starts, int n, int tile) {
   int lo = 0, hi = n;   // starts[lo] <= tile < starts[hi]
@@ -64,48 +64,52 @@ __device__ __forceinline__ int find_member(const int32_t* __restrict__ starts, i
   return lo;
 }
 
+// fp32 groups are tiny and latency-bound (configs[0]: 8.5e5 flop): 32x32 output tiles so that the group spreads
+// over more SMs, a 32-deep K slice per step, and the NEXT slice's global loads issued before the current slice is
+// multiplied, so only the first load latency is exposed.  Thread t owns outputs (ty + 8i, tx) for i < 4.
 __global__ void __launch_bounds__(kF32Threads)
 grouped_gemm_f32_kernel(const F32Member* __restrict__ members, const int32_t* __restrict__ starts, int n_members) {
-  __shared__ float As[kF32BK][kF32Tile + 4];
-  __shared__ float Bs[kF32BK][kF32Tile + 4];
+  __shared__ float As[kF32BK][kF32Tile + 1];
+  __shared__ float Bs[kF32BK][kF32Tile + 1];
   const int tile = blockIdx.x;
   const int mi = find_member(starts, n_members, tile);
   const F32Member m = members[mi];
   const int local = tile - __ldg(starts + mi);
   const int m0 = (local / m.nbn) * kF32Tile, n0 = (local % m.nbn) * kF32Tile;
-  const int tx = threadIdx.x & 15, ty = threadIdx.x >> 4;
-  float acc[4][4] = {};
+  const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;
+  // loader mapping: element (row lr + 8j, k lk) of the A and B slices, j < 4
+  const int lk = threadIdx.x & 31, lr = threadIdx.x >> 5;
+  float ra[4], rb[4];
+  auto fetch = [&](int k0) {
+#pragma unroll
+    for (int j = 0; j < 4; ++j) {
+      const int r = lr + 8 * j;
+      ra[j] = (m0 + r < m.M && k0 + lk < m.K) ? __ldg(m.x + (int64_t)(m0 + r) * m.ldx + k0 + lk) : 0.f;
+      rb[j] = (n0 + r < m.N && k0 + lk < m.K) ? __ldg(m.w + (int64_t)(n0 + r) * m.ldw + k0 + lk) : 0.f;
+    }
+  };
+  float acc[4] = {0.f, 0.f, 0.f, 0.f};
+  fetch(0);
   for (int k0 = 0; k0 < m.K; k0 += kF32BK) {
 #pragma unroll
-    for (int i = 0; i < 4; ++i) {
-      const int idx = threadIdx.x + i * kF32Threads;
-      const int r = idx >> 4, k = idx & 15;
-      As[k][r] = (m0 + r < m.M && k0 + k < m.K) ? __ldg(m.x + (int64_t)(m0 + r) * m.ldx + k0 + k) : 0.f;
-      Bs[k][r] = (n0 + r < m.N && k0 + k < m.K) ? __ldg(m.w + (int64_t)(n0 + r) * m.ldw + k0 + k) : 0.f;
-    }
+    for (int j = 0; j < 4; ++j) { As[lk][lr + 8 * j] = ra[j]; Bs[lk][lr + 8 * j] = rb[j]; }
     __syncthreads();
+    if (k0 + kF32BK < m.K) fetch(k0 + kF32BK);        // in flight while this slice is multiplied
 #pragma unroll
     for (int k = 0; k < kF32BK; ++k) {
-      float a[4], b[4];
+      const float b = Bs[k][tx];
 #pragma unroll
-      for (int i = 0; i < 4; ++i) { a[i] = As[k][ty * 4 + i]; b[i] = Bs[k][tx * 4 + i]; }
-#pragma unroll
-      for (int i = 0; i < 4; ++i)
-#pragma unroll
-        for (int j = 0; j < 4; ++j) acc[i][j] = fmaf(a[i], b[j], acc[i][j]);
+      for (int i = 0; i < 4; ++i) acc[i] = fmaf(As[k][ty + 8 * i], b, acc[i]);
     }
     __syncthreads();
   }
+  const int c = n0 + tx;
+  if (c < m.N) {
+    const float bias = m.bias ? __ldg(m.bias + c) : 0.f;
 #pragma unroll
-  for (int i = 0; i < 4; ++i) {
-    const int r = m0 + ty * 4 + i;
-    if (r >= m.M) continue;
-#pragma unroll
-    for (int j = 0; j < 4; ++j) {
-      const int c = n0 + tx * 4 + j;
-      if (c >= m.N) continue;
-      float v = acc[i][j] + (m.bias ? __ldg(m.bias + c) : 0.f);
-      m.y[(int64_t)r * m.ldy + c] = act_f32<false>(v, m.act);
+    for (int i = 0; i < 4; ++i) {
+      const int r = m0 + ty + 8 * i;
+      if (r < m.M) m.y[(int64_t)r * m.ldy + c] = act_f32<false>(acc[i] + bias, m.act);
     }
   }
 }
