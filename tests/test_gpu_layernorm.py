@@ -17,9 +17,9 @@ def ob():
 
 
 def check_ln(got_bits, m, dt=BF16, param_dt=None):
-    """DESIGN.md tolerance (Q11 + Q12): <= 2 bf16 ulp of the oracle rounded to bf16, OR within
-    2^-16 * (|xhat*gamma| + |beta|) where the result is a cancellation of larger terms; the escape
-    must be used by < 1e-3 of the elements."""
+    """DESIGN.md tolerance (Q11 + Q12 + Q12b): <= 2 bf16 ulp of the oracle rounded to bf16, OR within
+    2^-16 * (|xhat*gamma| + |beta|) where the result is a cancellation of larger terms, OR within the fp32
+    accuracy floor of x - mu; the escapes must be used by < 1e-3 of the elements."""
     param_dt = dt if param_dt is None else param_dt
     y64, xh = oracle.layernorm(m["x"], m.get("gamma"), m.get("beta"), m["eps"], dt, param_dt, return_xhat=True)
     ref = oracle.round_to_storage(y64, dt)
@@ -27,6 +27,13 @@ def check_ln(got_bits, m, dt=BF16, param_dt=None):
     g = values64(m["gamma"], param_dt) if m.get("gamma") is not None else 1.0
     b = values64(m["beta"], param_dt) if m.get("beta") is not None else 0.0
     slack = 2.0 ** -16 * (np.abs(xh * g) + np.abs(b))
+    # Q12b: x - mu cancels too.  fp32 statistics carry mu with relative error ~ log2(D) 2^-24, so the normalised value
+    # has an ABSOLUTE error floor of ~ 2^-20 (1 + |mu| / sqrt(v + eps)) whatever the kernel; where |y| is that small,
+    # bf16 ulps of y are meaningless.  Allowed: 2^-19 |gamma| (1 + |mu| rstd), i.e. < 2^-11 of a bf16 ulp of xhat ~ 1.
+    x64 = values64(m["x"], dt)
+    mu = x64.mean(axis=1, keepdims=True)
+    rstd = 1.0 / np.sqrt(x64.var(axis=1, keepdims=True) + float(np.float32(m["eps"])))
+    slack = np.maximum(slack, 2.0 ** -19 * np.abs(g) * (1.0 + np.abs(mu) * rstd))
     bad = (d > 2) & ~(np.abs(values64(got_bits, dt) - y64) <= slack)
     assert not bad.any(), "LN mismatch: max ulp %d at %s" % (d.max(), np.argwhere(bad)[:4])
     return int((d > 2).sum()), d.size
