@@ -78,3 +78,19 @@ def linear2(m, dt=BF16):
     h = round_to_storage(h64, dt)
     y64 = activation(linear(h, m["w2"], m.get("b2"), dt), m["act2"])
     return dict(h64=h64, h=h, y64=y64, y=round_to_storage(y64, dt))
+
+
+def _transposed(a):
+    return np.ascontiguousarray(a.T)
+
+
+def linear_dgrad(dy, w, dt=BF16):
+    """Backward of y = x W^T w.r.t. the input: dX[M,K] = dY[M,N] W[N,K] (sum over n in index order), fp64.
+    It is `linear` applied to the transposed weight: dX = dY (W^T)^T (PAPER.md:292 batch_linear_post_grad,
+    PAPER.md:437 training)."""
+    return linear(dy, _transposed(w), None, dt)
+
+
+def linear_wgrad(dy, x, dt=BF16):
+    """Backward w.r.t. the weight: dW[N,K] = dY[M,N]^T X[M,K] (sum over m in index order), fp64."""
+    return linear(_transposed(dy), _transposed(x), None, dt)

@@ -462,3 +462,20 @@ def test_pointwise_ext_identities_on_random_data():
     assert np.array_equal(c, np.clip(a64, -1.0, 1.0)) and np.array_equal(np.clip(c, -1.0, 1.0), c)    # idempotent
     assert np.array_equal(oracle.pointwise_ext(a, None, oracle.PW_CLAMP, [-np.inf, np.inf], BF16), a64)
     assert np.array_equal(oracle.pointwise_ext(a, None, oracle.PW_NAN_TO_NUM, [0.0, 1.0, -1.0], BF16), a64)   # finite: untouched
+
+
+# ------------------------------------------ backward of the grouped Linear --
+def test_linear_backward_integers_and_adjointness():
+    """dgrad / wgrad against numpy integer arithmetic (exact), and the adjoint identities that DEFINE them:
+    <dY, X W^T> = <dY W, X> = <dY^T X, W> on random bf16 data (fp64 sums agree to rounding)."""
+    rng = np.random.default_rng(21)
+    M, N, K = 9, 6, 11
+    dy = rng.integers(-3, 4, (M, N)); w = rng.integers(-3, 4, (N, K)); x = rng.integers(-3, 4, (M, K))
+    assert np.array_equal(graphs.linear_dgrad(bf16(dy), bf16(w)), (dy @ w).astype(np.float64))
+    assert np.array_equal(graphs.linear_wgrad(bf16(dy), bf16(x)), (dy.T @ x).astype(np.float64))
+    dyr = wl.tensor_normal(31, 1, (M, N), 0, 1, BF16); wr = wl.tensor_normal(31, 2, (N, K), 0, 1, BF16)
+    xr = wl.tensor_normal(31, 3, (M, K), 0, 1, BF16)
+    y64 = oracle.linear(xr, wr, None, BF16)
+    lhs = float((oracle.widen(dyr, BF16) * y64).sum())
+    assert abs(lhs - float((graphs.linear_dgrad(dyr, wr) * oracle.widen(xr, BF16)).sum())) <= 1e-12 * max(1.0, abs(lhs))
+    assert abs(lhs - float((graphs.linear_wgrad(dyr, xr) * oracle.widen(wr, BF16)).sum())) <= 1e-12 * max(1.0, abs(lhs))
