@@ -82,6 +82,16 @@ typedef enum {
   OPT_PW_MUL = 8         /* batch_aten_mul:   dst = src * src2                                                     */
 } opt_pw_op;
 
+/* Storage of the two operands of a grouped Linear member.  Default 0: x is [M,K], w is [N,K] (torch nn.Linear).
+ * OPT_LAYOUT_X_TRANSPOSED: x is stored [K,M] (ldx = its row stride); OPT_LAYOUT_W_TRANSPOSED: w is stored [K,N].
+ * With them the same grouped kernel computes the BACKWARD of a grouped Linear (batch_linear_post_grad operates
+ * on post-grad graphs; training QPS is the paper's headline):
+ *     dgrad  dX[M,K] = dY[M,N] * W[N,K]      ->  x = dY, w = W stored [contraction N, K]: W_TRANSPOSED
+ *     wgrad  dW[N,K] = dY[M,N]^T * X[M,K]    ->  x = dY stored [contraction M, N]: X_TRANSPOSED,
+ *                                                w = X stored [contraction M, K]: W_TRANSPOSED
+ * The tensor cores read such operands in place (MN-major shared-memory descriptors): no transposed copy.     */
+enum { OPT_LAYOUT_X_TRANSPOSED = 1, OPT_LAYOUT_W_TRANSPOSED = 2 };
+
 /* One member of a grouped Linear (+bias +activation) -- batch_linear /
  * batch_linear_post_grad with its epilogue:
  *     Y = act(X * W^T + bias)
@@ -99,7 +109,8 @@ typedef struct {
   void* y;
   int64_t ldy;
   int32_t M, N, K;
-  int32_t act; /* opt_act */
+  int32_t act;    /* opt_act */
+  int32_t layout; /* 0, or OPT_LAYOUT_* flags: an operand stored transposed (bf16 groups only) */
 } opt_linear_member;
 
 /* One member of a grouped CHAINED Linear -- two Linear layers of a tower fused

@@ -8,6 +8,7 @@ OPT_F32, OPT_BF16 = 0, 1
 OPT_ACT_NONE, OPT_ACT_RELU, OPT_ACT_TANH, OPT_ACT_SIGMOID = 0, 1, 2, 3
 OPT_PW_COPY, OPT_PW_RELU, OPT_PW_TANH, OPT_PW_SIGMOID = 0, 1, 2, 3
 OPT_PW_CLAMP, OPT_PW_NAN_TO_NUM, OPT_PW_SUB, OPT_PW_DIV, OPT_PW_MUL = 4, 5, 6, 7, 8
+OPT_LAYOUT_X_TRANSPOSED, OPT_LAYOUT_W_TRANSPOSED = 1, 2
 (OPT_OK, OPT_ERR_INVALID_ARG, OPT_ERR_UNSUPPORTED, OPT_ERR_ALIGNMENT, OPT_ERR_ALIAS, OPT_ERR_CUDA,
  OPT_ERR_NO_DEVICE) = range(7)
 _STATUS_NAMES = ["OPT_OK", "OPT_ERR_INVALID_ARG", "OPT_ERR_UNSUPPORTED", "OPT_ERR_ALIGNMENT", "OPT_ERR_ALIAS",
@@ -17,7 +18,7 @@ _STATUS_NAMES = ["OPT_OK", "OPT_ERR_INVALID_ARG", "OPT_ERR_UNSUPPORTED", "OPT_ER
 class opt_linear_member(C.Structure):
     _fields_ = [("x", C.c_void_p), ("ldx", C.c_int64), ("w", C.c_void_p), ("ldw", C.c_int64),
                 ("bias", C.c_void_p), ("y", C.c_void_p), ("ldy", C.c_int64),
-                ("M", C.c_int32), ("N", C.c_int32), ("K", C.c_int32), ("act", C.c_int32)]
+                ("M", C.c_int32), ("N", C.c_int32), ("K", C.c_int32), ("act", C.c_int32), ("layout", C.c_int32)]
 
 
 class opt_linear2_member(C.Structure):
@@ -194,12 +195,14 @@ def _ld(t):
     return t.stride(0)
 
 
-def linear_member(x, w, bias, y, act=OPT_ACT_NONE):
-    M, K = x.shape
-    N = w.shape[0]
-    assert w.shape[1] == K and tuple(y.shape) == (M, N)
+def linear_member(x, w, bias, y, act=OPT_ACT_NONE, layout=0):
+    """layout: OPT_LAYOUT_* flags; a transposed operand is passed as it is stored ([K,M] / [K,N])."""
+    M, N = y.shape
+    K = x.shape[0] if layout & OPT_LAYOUT_X_TRANSPOSED else x.shape[1]
+    assert tuple(x.shape) == ((K, M) if layout & OPT_LAYOUT_X_TRANSPOSED else (M, K))
+    assert tuple(w.shape) == ((K, N) if layout & OPT_LAYOUT_W_TRANSPOSED else (N, K))
     return opt_linear_member(x.data_ptr(), _ld(x), w.data_ptr(), _ld(w),
-                             None if bias is None else bias.data_ptr(), y.data_ptr(), _ld(y), M, N, K, int(act))
+                             None if bias is None else bias.data_ptr(), y.data_ptr(), _ld(y), M, N, K, int(act), int(layout))
 
 
 def linear2_member(x, w1, b1, w2, b2, y, act1=OPT_ACT_RELU, act2=OPT_ACT_NONE):

@@ -138,6 +138,7 @@ constexpr int kQBiasBytes = kMaxBN * 2;         // the tile's bias slice, bf16
 constexpr int kQSlotBytes = kQBiasBytes + 32;   // + the tile's 32-byte TileEntry
 constexpr int kTilesPerChunk = 4;               // tiles fetched per atomic (one 128-byte table line)
 constexpr int kSmemMax = 227 * 1024;
+constexpr uint32_t kTransX = 1u << 28, kTransW = 1u << 29;   // TileEntry::misc flags: operand stored transposed
 constexpr int kSmemFixed = kEpiWarps * kEpiBufBytes + kQDepth * kQSlotBytes + 256;   // staging + queue + barriers
 
 struct alignas(128) GemmMember {
@@ -253,7 +254,7 @@ grouped_gemm_sm100_kernel(const GemmMember* __restrict__ members, const uint4* _
           const uint4* bp = reinterpret_cast<const uint4*>(((uint64_t)bhi << 32) | blo);
           bias_v[g] = make_uint4(0, 0, 0, 0);
           if (member[g] >= 0) {
-            const int nvalid = (int)(misc >> 16);
+            const int nvalid = (int)((misc >> 16) & 0x1FFu);
             if (bp != nullptr && 8 * lane + 8 <= nvalid) {
               bias_v[g] = __ldg(bp + lane);
             } else if (bp != nullptr && 8 * lane < nvalid) {       // ragged N: the last piece element by element
@@ -320,8 +321,17 @@ grouped_gemm_sm100_kernel(const GemmMember* __restrict__ members, const uint4* _
             tma_load_2d_pair(sa + kABytes, tmB, lb, kb * kBK, n0);
           } else {
             mbar_expect_tx(full_bar(stage), kABytes + b_bytes);
-            tma_load_2d(sa, &m->tmA, full_bar(stage), kb * kBK, m0);
-            tma_load_2d(sa + kABytes, tmB, full_bar(stage), kb * kBK, n0);
+            if (e1.y & kTransX) {                    // stored [K, M]: two 64x64 boxes (contraction rows, M contiguous)
+              tma_load_2d(sa, &m->tmA, full_bar(stage), m0, kb * kBK);
+              tma_load_2d(sa + 8192, &m->tmA, full_bar(stage), m0 + 64, kb * kBK);
+            } else {
+              tma_load_2d(sa, &m->tmA, full_bar(stage), kb * kBK, m0);
+            }
+            if (e1.y & kTransW) {                    // stored [K, N]: BN/64 boxes
+              for (int j = 0; j < bn / 64; ++j) tma_load_2d(sa + kABytes + j * 8192, tmB, full_bar(stage), n0 + 64 * j, kb * kBK);
+            } else {
+              tma_load_2d(sa + kABytes, tmB, full_bar(stage), kb * kBK, n0);
+            }
           }
           if (++stage == nstages) { stage = 0; phase ^= 1; }
         }
@@ -349,11 +359,15 @@ grouped_gemm_sm100_kernel(const GemmMember* __restrict__ members, const uint4* _
           mbar_wait(full_bar(stage), phase);
           tc_fence_after();
           const uint32_t sa = sbase + stage * stage_bytes;
-          const uint64_t adesc = umma_desc_sw128(sa), bdesc = umma_desc_sw128(sa + kABytes);
+          const bool tx = NCTA == 1 && (e1.y & kTransX), tw = NCTA == 1 && (e1.y & kTransW);
+          const uint64_t adesc = tx ? umma_desc_sw128_mn(sa) : umma_desc_sw128(sa);
+          const uint64_t bdesc = tw ? umma_desc_sw128_mn(sa + kABytes) : umma_desc_sw128(sa + kABytes);
+          // per K=16 step: K-major +32 bytes inside the swizzle row (+2 encoded); MN-major +2 groups of 8 rows (+128)
+          const uint64_t astep = tx ? 128 : 2, bstep = tw ? 128 : 2;
           const int ksteps = kb + 1 < nkb ? kBK / 16 : klast;
-          for (int k = 0; k < ksteps; ++k) {  // +32 bytes (= +2 encoded) per K=16 step inside the swizzle row
+          for (int k = 0; k < ksteps; ++k) {
             if (NCTA == 2) tc_mma_bf16_pair(d_tmem, adesc + 2 * k, bdesc + 2 * k, idesc, (kb | k) != 0);
-            else tc_mma_bf16(d_tmem, adesc + 2 * k, bdesc + 2 * k, idesc, (kb | k) != 0);
+            else tc_mma_bf16(d_tmem, adesc + astep * k, bdesc + bstep * k, idesc, (kb | k) != 0);
           }
           // frees the smem stage (in both CTAs) when these MMAs retire
           if (NCTA == 2) tc_commit_pair(empty_bar(stage)); else tc_commit(empty_bar(stage));
@@ -493,7 +507,12 @@ extern "C" opt_status opt_linear_plan_create(const opt_linear_member* members, i
     if (!m.x || !m.w || !m.y) return fail(OPT_ERR_INVALID_ARG, "member %d: NULL pointer", i);
     if (m.M < 1 || m.N < 1 || m.K < 1) return fail(OPT_ERR_INVALID_ARG, "member %d: M=%d N=%d K=%d must be >= 1", i, m.M, m.N, m.K);
     if (m.act < OPT_ACT_NONE || m.act > OPT_ACT_SIGMOID) return fail(OPT_ERR_INVALID_ARG, "member %d: bad activation %d", i, m.act);
-    if ((m.M > 1 && (m.ldx < m.K || m.ldy < m.N)) || (m.N > 1 && m.ldw < m.K))
+    if (m.layout & ~(OPT_LAYOUT_X_TRANSPOSED | OPT_LAYOUT_W_TRANSPOSED)) return fail(OPT_ERR_INVALID_ARG, "member %d: bad layout flags %d", i, m.layout);
+    const bool tx = m.layout & OPT_LAYOUT_X_TRANSPOSED, tw = m.layout & OPT_LAYOUT_W_TRANSPOSED;
+    if ((tx || tw) && io != OPT_BF16) return fail(OPT_ERR_UNSUPPORTED, "member %d: transposed operands are implemented for bf16 groups only", i);
+    // stored shapes: x [M,K] or (transposed) [K,M]; w [N,K] or (transposed) [K,N]
+    const int32_t x_rows = tx ? m.K : m.M, x_cols = tx ? m.M : m.K, w_rows = tw ? m.K : m.N, w_cols = tw ? m.N : m.K;
+    if ((x_rows > 1 && m.ldx < x_cols) || (m.M > 1 && m.ldy < m.N) || (w_rows > 1 && m.ldw < w_cols))
       return fail(OPT_ERR_INVALID_ARG, "member %d: row stride smaller than the row", i);
     if (!aligned16(m.x) || !aligned16(m.w) || !aligned16(m.y) || !aligned16(m.bias))
       return fail(OPT_ERR_ALIGNMENT, "member %d: pointers must be 16-byte aligned", i);
@@ -503,13 +522,13 @@ extern "C" opt_status opt_linear_plan_create(const opt_linear_member* members, i
     if (io == OPT_F32 && (m.K % V || m.N % V))
       return fail(OPT_ERR_ALIGNMENT, "member %d: K=%d and N=%d must be multiples of %d", i, m.K, m.N, V);
     if (m.ldx % V || m.ldw % V || m.ldy % V) return fail(OPT_ERR_ALIGNMENT, "member %d: row strides must be multiples of %d elements", i, V);
-    regions.push_back({(uintptr_t)m.x, m.ldx * esz, (int64_t)m.K * esz, m.M, false, i});
-    regions.push_back({(uintptr_t)m.w, m.ldw * esz, (int64_t)m.K * esz, m.N, false, i});
+    regions.push_back({(uintptr_t)m.x, m.ldx * esz, (int64_t)x_cols * esz, x_rows, false, i});
+    regions.push_back({(uintptr_t)m.w, m.ldw * esz, (int64_t)w_cols * esz, w_rows, false, i});
     if (m.bias) regions.push_back({(uintptr_t)m.bias, 0, (int64_t)m.N * esz, 1, false, i});
     regions.push_back({(uintptr_t)m.y, m.ldy * esz, (int64_t)m.N * esz, m.M, true, i});
     flops += 2ll * m.M * m.N * m.K;
     // an input shared by several members (batch_linear_lhs) is read once
-    const bool first_use_of_x = seen_x.insert(std::make_tuple(m.x, m.ldx, m.M, m.K)).second;
+    const bool first_use_of_x = seen_x.insert(std::make_tuple(m.x, m.ldx, m.M, tx ? -m.K : m.K)).second;
     bytes += ((first_use_of_x ? (int64_t)m.M * m.K : 0) + (int64_t)m.N * m.K + (m.bias ? m.N : 0) + (int64_t)m.M * m.N) * esz;
   }
   if (opt_status st = check_independent(regions, /*allow_inplace_self=*/false)) return st;
@@ -555,19 +574,27 @@ extern "C" opt_status opt_linear_plan_create(const opt_linear_member* members, i
   // CTA pair (256-row tiles, W shared by the pair) or single CTA (128-row tiles)
   int ncta = 2;
   if (const char* e = getenv("OPT_GEMM_NCTA")) ncta = atoi(e) == 1 ? 1 : 2;                // experiment knob
+  for (int32_t i = 0; i < n; ++i)
+    if (members[i].layout) ncta = 1;           // MN-major (transposed) operand tiles are built per CTA: single-CTA kernel
   const int tile_m = kBM * ncta;
-  struct MemberTiling { int bn, nbn, nkb, klast; uint32_t idesc; };
+  struct MemberTiling { int bn, nbn, nkb, klast; uint32_t idesc, flags; };
   std::vector<MemberTiling> tiling(n);
   int max_bn = 16;
   for (int32_t i = 0; i < n; ++i) {
     const opt_linear_member& m = members[i];
     GemmMember& t = tab[i];
-    const int bn = choose_bn(m.N);
+    const bool tx = m.layout & OPT_LAYOUT_X_TRANSPOSED, tw = m.layout & OPT_LAYOUT_W_TRANSPOSED;
+    int bn = choose_bn(m.N);
+    if (tw) bn = (bn + 63) / 64 * 64;          // MN-major W tiles are rows of 64x64 boxes
     opt_status st;
-    if ((st = encode_2d(enc, &t.tmA, m.x, m.M, m.K, m.ldx, kBK, kBM, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, "X", i)) ||
-        (st = encode_2d(enc, &t.tmB, m.w, m.N, m.K, m.ldw, kBK, bn, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, "W", i)) ||
-        (st = encode_2d(enc, &t.tmY, m.y, m.M, m.N, m.ldy, 64, 32, CU_TENSOR_MAP_L2_PROMOTION_NONE, "Y", i)) ||
-        (st = encode_2d(enc, &t.tmB2, m.w, m.N, m.K, m.ldw, kBK, bn / 2, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, "W/2", i))) {
+    // K-major operand: box {64 k, rows};  transposed operand (stored [K, out]): box {64 out, 64 k}
+    st = tx ? encode_2d(enc, &t.tmA, m.x, m.K, m.M, m.ldx, 64, kBK, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, "X^T", i)
+            : encode_2d(enc, &t.tmA, m.x, m.M, m.K, m.ldx, kBK, kBM, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, "X", i);
+    if (!st) st = tw ? encode_2d(enc, &t.tmB, m.w, m.K, m.N, m.ldw, 64, kBK, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, "W^T", i)
+                     : encode_2d(enc, &t.tmB, m.w, m.N, m.K, m.ldw, kBK, bn, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, "W", i);
+    if (!st) st = encode_2d(enc, &t.tmY, m.y, m.M, m.N, m.ldy, 64, 32, CU_TENSOR_MAP_L2_PROMOTION_NONE, "Y", i);
+    if (!st && !tw) st = encode_2d(enc, &t.tmB2, m.w, m.N, m.K, m.ldw, kBK, bn / 2, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, "W/2", i);
+    if (st) {
       delete p;
       return st;
     }
@@ -576,7 +603,9 @@ extern "C" opt_status opt_linear_plan_create(const opt_linear_member* members, i
     tl.klast = (m.K - (tl.nkb - 1) * kBK + 15) / 16;
     // tcgen05 instruction descriptor, kind::f16: D fp32 (bits 4-5 = 1), A bf16 (bits 7-9 = 1), B bf16
     // (bits 10-12 = 1), A and B K-major (bits 15, 16 = 0), N>>3 at bits 17-22, M>>4 at bits 24-28.
-    tl.idesc = (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(bn >> 3) << 17) | ((uint32_t)(tile_m >> 4) << 24);
+    tl.idesc = (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)tx << 15) | ((uint32_t)tw << 16) | ((uint32_t)(bn >> 3) << 17) |
+               ((uint32_t)(tile_m >> 4) << 24);
+    tl.flags = (tx ? kTransX : 0u) | (tw ? kTransW : 0u);
     max_bn = std::max(max_bn, bn);
     const int nmb = (m.M + tile_m - 1) / tile_m;
     tiles += (int64_t)nmb * tl.nbn;
@@ -598,7 +627,7 @@ extern "C" opt_status opt_linear_plan_create(const opt_linear_member* members, i
       TileEntry e;
       e.member = i; e.m0 = mb * tile_m; e.n0 = nb * tl.bn; e.idesc = tl.idesc;
       e.bn_nkb = (uint32_t)tl.bn | ((uint32_t)tl.nkb << 16);
-      e.misc = (uint32_t)tl.klast | ((uint32_t)m.act << 8) | ((uint32_t)std::min(tl.bn, m.N - e.n0) << 16);
+      e.misc = (uint32_t)tl.klast | ((uint32_t)m.act << 8) | ((uint32_t)std::min(tl.bn, m.N - e.n0) << 16) | tl.flags;
       e.bias = m.bias ? static_cast<const char*>(m.bias) + (size_t)e.n0 * 2 : nullptr;
       flat.push_back(e);
     }

@@ -129,6 +129,15 @@ __device__ __forceinline__ uint64_t umma_desc_sw128(uint32_t saddr) {
   return (uint64_t)((saddr & 0x3FFFFu) >> 4) | ((uint64_t)(1024 >> 4) << 32) | (1ull << 46) | (2ull << 61);
 }
 
+// Same for an MN-major operand (the stored matrix is [contraction, out-dim], out-dim contiguous -- a transposed
+// input): the tile is a row of 64x64 boxes, each [64 contraction rows][64 out-dim elements = 128 bytes], 128-byte
+// swizzled.  Canonical form ((8,n),(8,k)):((1,LBO),(8,SBO)) in 16-byte units: LBO = one box (8 KB) between
+// 64-element out-dim blocks, SBO = 1024 bytes between groups of 8 contraction rows.  A K=16 step = 2 groups.
+__device__ __forceinline__ uint64_t umma_desc_sw128_mn(uint32_t saddr) {
+  return (uint64_t)((saddr & 0x3FFFFu) >> 4) | ((uint64_t)(8192 >> 4) << 16) | ((uint64_t)(1024 >> 4) << 32) | (1ull << 46) |
+         (2ull << 61);
+}
+
 // round two fp32 to a packed bf16x2 (lo in the low half) with the ReLU folded into the conversion:
 // negative -> +0, NaN -> NaN (torch relu semantics, Q13)
 __device__ __forceinline__ uint32_t pack_relu_bf16x2(float lo, float hi) {

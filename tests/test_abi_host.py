@@ -37,7 +37,7 @@ def test_every_declared_symbol_is_exported(ob):
 
 
 def test_struct_layouts_match_header(ob):
-    assert ctypes.sizeof(ob.opt_linear_member) == 72
+    assert ctypes.sizeof(ob.opt_linear_member) == 80
     assert ctypes.sizeof(ob.opt_layernorm_member) == 64
     assert ctypes.sizeof(ob.opt_chunk) == 80
     assert ctypes.sizeof(ob.opt_host_copy) == 32
