@@ -755,6 +755,48 @@ def run_product(args):
         except Exception as e:  # noqa: BLE001
             vertical = dict(error=repr(e))
 
+    # ---- (7) SURVEY 8(f) rank 3, side figure: backward of C2's grouped Linear through the same grouped kernel
+    # (operands read in their stored layout, no transposed copies): one launch for all dgrads, one for all wgrads
+    backward = None
+    c2g = [g for g in step.groups if g.name.startswith("C2")]
+    if c2g and not args.profile and not args.small:
+        try:
+            g2 = c2g[0]
+            ycat = g2.aout.tensor(g2.iy)
+            dy_cat = torch.empty_like(ycat).normal_(0.0, 1.0)
+            dg, wg, keep = [], [], []
+            for (ix, iw, ib), m in zip(g2.idx, g2.cfg["members"]):
+                x, w = g2.ain.tensor(ix), g2.ain.tensor(iw)
+                dy = dy_cat[:, m["col_off"]:m["col_off"] + m["N"]]
+                dx, dw = torch.empty_like(x), torch.empty_like(w)
+                keep.append((dx, dw))
+                dg.append(ob.linear_member(dy, w, None, dx, ACT_NONE, ob.OPT_LAYOUT_W_TRANSPOSED))
+                wg.append(ob.linear_member(dy, x, None, dw, ACT_NONE, ob.OPT_LAYOUT_X_TRANSPOSED | ob.OPT_LAYOUT_W_TRANSPOSED))
+            pd, pw = ob.opt_linear_plan_create(dg, BF16, step.dev_index), ob.opt_linear_plan_create(wg, BF16, step.dev_index)
+            flush = torch.empty(256 * 1024 * 1024, dtype=torch.uint8, device=device)
+
+            def cold2(fn, n=10):
+                ts = []
+                for _ in range(n):
+                    flush.fill_(1)
+                    c0_, c1_ = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                    c0_.record(stream); fn(); c1_.record(stream)
+                    torch.cuda.synchronize()
+                    ts.append(c0_.elapsed_time(c1_) * 1e3)
+                return float(np.mean(ts))
+            pd.launch(); pw.launch()
+            torch.cuda.synchronize()
+            td, tw_ = cold2(pd.launch), cold2(pw.launch)
+            idg, iwg = pd.info(), pw.info()
+            backward = dict(workload="configs[2] backward: dX = dY W and dW = dY^T X for the 128 members, one launch each",
+                            dgrad_us=round(td, 1), dgrad_tflops=round(idg["flops"] / td / 1e6, 1),
+                            wgrad_us=round(tw_, 1), wgrad_tflops=round(iwg["flops"] / tw_ / 1e6, 1),
+                            frac_tensor_dgrad=round(idg["flops"] / td / 1e6 / peaks["bf16_tflops"], 4),
+                            frac_tensor_wgrad=round(iwg["flops"] / tw_ / 1e6 / peaks["bf16_tflops"], 4))
+            del flush, keep, dy_cat
+        except Exception as e:  # noqa: BLE001
+            backward = dict(error=repr(e))
+
     watch.stop_flag.set()
     watch.join(timeout=2)
 
@@ -817,7 +859,7 @@ def run_product(args):
                              "copies overlap, single_stream_us: everything on one stream"),
                 gpu_launches=int(launches), launches_per_step=ng,
                 clocks=watch.summary(), roofline=roofline, roofline_tensor=roofline_tensor, groups=groups,
-                unfused_baseline=unfused, vertical_fusion=vertical, config0_latency=c0,
+                unfused_baseline=unfused, vertical_fusion=vertical, backward=backward, config0_latency=c0,
                 aggregate=dict(steps_per_s=round(aggregate_steps_per_s(us_step, world), 2)),
                 build_seconds=round(build_s, 1), lib=ob.opt_version())
 
