@@ -51,6 +51,7 @@ def lib():
         L.oracle_pointwise.argtypes = [vp, i64, i32, i32, c.c_int, c.c_int, vp]
         L.oracle_pointwise_ext.argtypes = [vp, i64, vp, i64, i32, i32, c.c_int, dbl, dbl, dbl, c.c_int, vp]
         L.oracle_layernorm.argtypes = [vp, i64, vp, vp, i32, i32, dbl, c.c_int, c.c_int, vp, vp]
+        L.oracle_layernorm_backward.argtypes = [vp, i64, vp, i64, vp, i32, i32, dbl, c.c_int, c.c_int, vp, vp, vp]
         L.oracle_split.argtypes = [vp, i64, i32, i32, i32, vp, i32, vp]
         L.oracle_split.restype = c.c_int
         L.oracle_cat.argtypes = [vp, vp, i32, i32, i32, vp, i64]
@@ -164,6 +165,23 @@ def layernorm(x, gamma, beta, eps, dt, param_dt=None, return_xhat=False):
     lib().oracle_layernorm(_ptr(x), _ld(x), _ptr(gamma), _ptr(beta), rows, D,
                            float(np.float32(eps)), dt, param_dt, _ptr(y), _ptr(xh))
     return (y, xh) if return_xhat else y
+
+
+def layernorm_backward(x, dy, gamma, eps, dt, param_dt=None):
+    """torch layer_norm backward over the last dim, fp64 -> (dx [rows,D], dgamma [D], dbeta [D])."""
+    param_dt = dt if param_dt is None else param_dt
+    _chk(x, dt, 2)
+    _chk(dy, dt, 2)
+    assert x.shape == dy.shape
+    rows, D = x.shape
+    if gamma is not None:
+        gamma = np.ascontiguousarray(_chk(gamma, param_dt, 1))
+    dx = np.empty((rows, D), dtype=np.float64)
+    dg = np.empty((D,), dtype=np.float64)
+    db = np.empty((D,), dtype=np.float64)
+    lib().oracle_layernorm_backward(_ptr(x), _ld(x), _ptr(dy), _ld(dy), _ptr(gamma), rows, D, float(np.float32(eps)),
+                                    dt, param_dt, _ptr(dx), _ptr(dg), _ptr(db))
+    return dx, dg, db
 
 
 def split(x, sizes):

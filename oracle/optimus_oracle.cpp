@@ -239,6 +239,49 @@ void oracle_layernorm(const void* x, int64_t ldx, const void* gamma, const void*
   }
 }
 
+// ---- layer_norm backward (torch native_layer_norm_backward): with
+//   mu, v as in the forward, rstd = 1/sqrt(v+eps), xhat = (x-mu) rstd, g_j = dy_j gamma_j:
+//   dx_j     = rstd * ( g_j - mean_j(g) - xhat_j * mean_j(g xhat) )        per row
+//   dgamma_j = sum_rows dy_j xhat_j ;  dbeta_j = sum_rows dy_j             (rows summed in index order)
+// dx dense [rows,D]; dgamma / dbeta [D] (may be NULL).  gamma may be NULL (= 1).
+void oracle_layernorm_backward(const void* x, int64_t ldx, const void* dy, int64_t lddy, const void* gamma,
+                               int32_t rows, int32_t D, double eps, int dt, int param_dt,
+                               double* dx, double* dgamma, double* dbeta) {
+  std::vector<double> xh_all(dgamma ? (size_t)rows * D : 0);
+#pragma omp parallel for schedule(static)
+  for (int32_t r = 0; r < rows; ++r) {
+    double s = 0.0;
+    for (int32_t j = 0; j < D; ++j) s += widen(x, (int64_t)r * ldx + j, dt);
+    const double mu = s / (double)D;
+    double q = 0.0;
+    for (int32_t j = 0; j < D; ++j) { const double d = widen(x, (int64_t)r * ldx + j, dt) - mu; q += d * d; }
+    const double rstd = 1.0 / std::sqrt(q / (double)D + eps);
+    double sg = 0.0, sgx = 0.0;
+    for (int32_t j = 0; j < D; ++j) {
+      const double xh = (widen(x, (int64_t)r * ldx + j, dt) - mu) * rstd;
+      const double g = widen(dy, (int64_t)r * lddy + j, dt) * (gamma ? widen(gamma, j, param_dt) : 1.0);
+      sg += g; sgx += g * xh;
+      if (dgamma) xh_all[(size_t)r * D + j] = xh;
+    }
+    const double mg = sg / (double)D, mgx = sgx / (double)D;
+    for (int32_t j = 0; j < D; ++j) {
+      const double xh = (widen(x, (int64_t)r * ldx + j, dt) - mu) * rstd;
+      const double g = widen(dy, (int64_t)r * lddy + j, dt) * (gamma ? widen(gamma, j, param_dt) : 1.0);
+      dx[(int64_t)r * D + j] = rstd * (g - mg - xh * mgx);
+    }
+  }
+  for (int32_t j = 0; j < D && (dgamma || dbeta); ++j) {
+    double a = 0.0, b = 0.0;
+    for (int32_t r = 0; r < rows; ++r) {
+      const double d = widen(dy, (int64_t)r * lddy + j, dt);
+      if (dgamma) a += d * xh_all[(size_t)r * D + j];
+      b += d;
+    }
+    if (dgamma) dgamma[j] = a;
+    if (dbeta) dbeta[j] = b;
+  }
+}
+
 // ---- split along dim 1 (torch.split(x, sizes, dim=1)):
 // piece j = x[:, s_j : s_j + w_j], s_j = sum_{t<j} w_t.  Raw element copy
 // (elem_size bytes per element); piece j is written densely [rows, w_j] at

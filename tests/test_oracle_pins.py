@@ -479,3 +479,42 @@ def test_linear_backward_integers_and_adjointness():
     lhs = float((oracle.widen(dyr, BF16) * y64).sum())
     assert abs(lhs - float((graphs.linear_dgrad(dyr, wr) * oracle.widen(xr, BF16)).sum())) <= 1e-12 * max(1.0, abs(lhs))
     assert abs(lhs - float((graphs.linear_wgrad(dyr, xr) * oracle.widen(wr, BF16)).sum())) <= 1e-12 * max(1.0, abs(lhs))
+
+
+# --------------------------------------------- LayerNorm backward --
+def test_layernorm_backward_finite_differences_and_identities():
+    """dx, dgamma, dbeta against central finite differences of the oracle's OWN forward are not a pin (same code
+    base), so the forward used here is numpy's: L(x, gamma, beta) = sum(dy * LN(x)) in fp64.  Plus the closed forms:
+    every dx row sums to 0; with eps = 0 it is also orthogonal to xhat; dbeta = column sums of dy."""
+    rng = np.random.default_rng(17)
+    rows, D, eps = 5, 12, 1e-5
+    x = rng.normal(0.5, 2.0, (rows, D)).astype(np.float32)
+    dy = rng.normal(0.0, 1.0, (rows, D)).astype(np.float32)
+    gamma = rng.normal(1.0, 0.3, (D,)).astype(np.float32)
+    beta = rng.normal(0.0, 0.3, (D,)).astype(np.float32)
+    e32 = float(np.float32(eps))
+
+    def ln(xx, gg, bb):
+        mu = xx.mean(axis=1, keepdims=True)
+        v = ((xx - mu) ** 2).mean(axis=1, keepdims=True)
+        return (xx - mu) / np.sqrt(v + e32) * gg + bb
+    loss = lambda xx, gg, bb: float((dy.astype(np.float64) * ln(xx, gg, bb)).sum())
+    x64, g64, b64 = x.astype(np.float64), gamma.astype(np.float64), beta.astype(np.float64)
+    dx, dg, db = oracle.layernorm_backward(x, dy, gamma, eps, F32)
+    h = 1e-6
+    for (r, j) in [(0, 0), (2, 5), (4, 11), (1, 7)]:
+        xp, xm = x64.copy(), x64.copy(); xp[r, j] += h; xm[r, j] -= h
+        assert abs((loss(xp, g64, b64) - loss(xm, g64, b64)) / (2 * h) - dx[r, j]) <= 1e-7 * max(1.0, abs(dx[r, j]))
+    for j in (0, 3, 11):
+        gp, gm = g64.copy(), g64.copy(); gp[j] += h; gm[j] -= h
+        assert abs((loss(x64, gp, b64) - loss(x64, gm, b64)) / (2 * h) - dg[j]) <= 1e-7 * max(1.0, abs(dg[j]))
+    assert np.allclose(db, dy.astype(np.float64).sum(axis=0), rtol=1e-14, atol=1e-14)
+    assert np.abs(dx.sum(axis=1)).max() <= 1e-12
+    dx0, _, _ = oracle.layernorm_backward(x, dy, gamma, 0.0, F32)
+    mu = x64.mean(axis=1, keepdims=True)
+    xh = (x64 - mu) / np.sqrt(((x64 - mu) ** 2).mean(axis=1, keepdims=True))
+    assert np.abs((dx0 * xh).sum(axis=1)).max() <= 1e-12
+    # gamma = None means 1
+    dx1, dg1, _ = oracle.layernorm_backward(x, dy, None, eps, F32)
+    dx2, dg2, _ = oracle.layernorm_backward(x, dy, np.ones(D, np.float32), eps, F32)
+    assert np.array_equal(dx1, dx2) and np.array_equal(dg1, dg2)
