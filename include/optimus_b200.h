@@ -157,6 +157,27 @@ typedef struct {
   float eps;
 } opt_layernorm_member;
 
+/* One member of a batched LayerNorm BACKWARD (torch
+ * native_layer_norm_backward): with mu, v, xhat as in the forward and g = dy * gamma,
+ *     dx     = rstd * (g - mean(g) - xhat * mean(g * xhat))      rows x D
+ *     dgamma = sum over rows of dy * xhat ;  dbeta = sum over rows of dy      [D]
+ * x, dy:[rows,D] (ldx, lddy), gamma:[D] or NULL (= 1), dx:[rows,D] (lddx); dgamma / dbeta: [D] in the param
+ * dtype, or NULL when not wanted.  bf16 activations, D % 8 == 0, D <= 512 (else OPT_ERR_UNSUPPORTED).  fp32
+ * arithmetic; the column sums are added in a fixed order (bitwise reproducible, no atomics on data).            */
+typedef struct {
+  const void* x;
+  int64_t ldx;
+  const void* dy;
+  int64_t lddy;
+  const void* gamma;
+  void* dx;
+  int64_t lddx;
+  void* dgamma;
+  void* dbeta;
+  int32_t rows, D;
+  float eps;
+} opt_layernorm_bwd_member;
+
 /* One chunk of a multi-tensor pointwise / split-cat pass -- batch_relu,
  * batch_sigmoid, batch_aten_tanh, batch_detach and the data
  * movement left over by the split/cat rewrites (Listing 2):
@@ -200,6 +221,8 @@ opt_status opt_linear2_plan_create(const opt_linear2_member* members, int32_t n,
                                    int device, opt_plan** plan);
 opt_status opt_layernorm_plan_create(const opt_layernorm_member* members, int32_t n, opt_dtype io,
                                      opt_dtype param, int device, opt_plan** plan);
+opt_status opt_layernorm_bwd_plan_create(const opt_layernorm_bwd_member* members, int32_t n, opt_dtype io,
+                                         opt_dtype param, int device, opt_plan** plan);
 opt_status opt_pointwise_plan_create(const opt_chunk* chunks, int32_t n, opt_dtype io, int device,
                                      opt_plan** plan);
 

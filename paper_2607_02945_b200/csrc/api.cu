@@ -111,6 +111,7 @@ static cudaError_t launch_any(const opt_plan* p, cudaStream_t s) {
     case kPlanLinearBf16: return launch_linear_bf16(p, s);
     case kPlanLinearF32: return launch_linear_f32(p, s);
     case kPlanLinear2: return launch_linear2(p, s);
+    case kPlanLayerNormBwd: return launch_layernorm_bwd(p, s);
     default: return cudaErrorInvalidValue;
   }
 }
@@ -160,6 +161,7 @@ opt_status opt_plan_info(const opt_plan* plan, int64_t* flops, int64_t* bytes, i
 opt_status opt_plan_destroy(opt_plan* plan) {
   if (!plan) return OPT_OK;
   if (plan->dev_tables) cudaFree(plan->dev_tables);
+  if (plan->workspace) cudaFree(plan->workspace);
   delete plan;
   return OPT_OK;
 }

@@ -1,0 +1,297 @@
+// batched_layernorm_bwd: the backward of N independent LayerNorms in ONE launch (the paper's
+// headline metric is TRAINING throughput, and batch_layernorm groups appear in the backward graph too).
+//
+//   mu, v over the last dim; rstd = 1/sqrt(v + eps); xhat = (x - mu) rstd; g = dy * gamma
+//   dx     = rstd * (g - mean(g) - xhat * mean(g xhat))                       per row
+//   dgamma = sum_rows dy * xhat ;  dbeta = sum_rows dy                         per column
+//
+// Design (HBM-bound: x and dy read once, dx written once):
+//   * a row is owned by L = 2^k lanes of a warp, each lane keeps its <= 2 16-byte vectors of x and of dy in
+//     registers; fp32 statistics (two-pass) and the two row means by width-L shuffles, as in the forward kernel;
+//   * every thread accumulates dy*xhat and dy for its own columns over the rows it visits; at the end of the block
+//     the row groups are summed through shared memory in a fixed order and the block's partial goes to a plan-owned
+//     workspace; the LAST block of a member (atomic ticket, re-armed by that block) adds the partials in part order
+//     and writes dgamma / dbeta: one launch, no atomics on data, bitwise reproducible.
+#include <algorithm>
+
+#include "common.h"
+
+namespace optb {
+
+struct LnbMember {
+  const char* x; const char* dy; const char* gamma; char* dx; char* dgamma; char* dbeta;
+  int64_t ldx16, lddy16, lddx16;   // row strides in 16-byte vectors
+  float* ws;                       // [nparts][2][D] fp32 partial sums (plan workspace)
+  int32_t* ticket;                 // blocks of this member that have finished
+  int32_t rows, nvec, nparts;
+  float eps, inv_D;
+  int32_t l_log2, vpl;
+};
+struct LnbBlock { int32_t member, row0, nrows, part; };
+
+constexpr int kLnbThreads = 256;
+constexpr int kLnbMaxVpl = 2;        // D <= 512: x, dy and the two column accumulators stay in registers
+
+__device__ __forceinline__ void lnb_unpack(const int4& v, float (&f)[8]) {
+  const uint32_t* u = reinterpret_cast<const uint32_t*>(&v);
+#pragma unroll
+  for (int i = 0; i < 4; ++i) { f[2 * i] = bf16_lo(u[i]); f[2 * i + 1] = bf16_hi(u[i]); }
+}
+
+template <bool P_BF16>
+__device__ __forceinline__ void lnb_store_param(char* base, int col, float v) {
+  if (P_BF16) reinterpret_cast<__nv_bfloat16*>(base)[col] = __float2bfloat16_rn(v);
+  else reinterpret_cast<float*>(base)[col] = v;
+}
+
+template <bool P_BF16, int VPL>
+__device__ __forceinline__ void lnb_block(const LnbMember& m, const LnbBlock& b, float* red) {
+  const int L = 1 << m.l_log2;
+  const int lane_in_row = threadIdx.x & (L - 1);
+  const int row_in_pass = threadIdx.x >> m.l_log2;
+  const int rpp = kLnbThreads >> m.l_log2;
+  const int D = m.nvec * 8;
+  const int4* xb = reinterpret_cast<const int4*>(m.x);
+  const int4* dyb = reinterpret_cast<const int4*>(m.dy);
+  int4* dxb = reinterpret_cast<int4*>(m.dx);
+  bool act[VPL];
+  float gam[VPL][8], acc_g[VPL][8], acc_b[VPL][8];
+#pragma unroll
+  for (int i = 0; i < VPL; ++i) {
+    const int vec = lane_in_row + i * L;
+    act[i] = vec < m.nvec;
+#pragma unroll
+    for (int e = 0; e < 8; ++e) { gam[i][e] = 1.f; acc_g[i][e] = 0.f; acc_b[i][e] = 0.f; }
+    if (act[i] && m.gamma != nullptr) {
+      if (P_BF16) {
+        lnb_unpack(__ldg(reinterpret_cast<const int4*>(m.gamma) + vec), gam[i]);
+      } else {
+        const float4 a = __ldg(reinterpret_cast<const float4*>(m.gamma) + 2 * vec), c = __ldg(reinterpret_cast<const float4*>(m.gamma) + 2 * vec + 1);
+        gam[i][0] = a.x; gam[i][1] = a.y; gam[i][2] = a.z; gam[i][3] = a.w; gam[i][4] = c.x; gam[i][5] = c.y; gam[i][6] = c.z; gam[i][7] = c.w;
+      }
+    }
+  }
+  const int npass = (b.nrows + rpp - 1) / rpp;
+  for (int pass = 0; pass < npass; ++pass) {
+    const int r = pass * rpp + row_in_pass;
+    const bool ok = r < b.nrows;
+    float x[VPL][8], dy[VPL][8];
+    float s = 0.f;
+#pragma unroll
+    for (int i = 0; i < VPL; ++i) {
+      int4 vx = make_int4(0, 0, 0, 0), vd = make_int4(0, 0, 0, 0);
+      if (ok && act[i]) {
+        vx = __ldcs(xb + (int64_t)(b.row0 + r) * m.ldx16 + lane_in_row + i * L);
+        vd = __ldcs(dyb + (int64_t)(b.row0 + r) * m.lddy16 + lane_in_row + i * L);
+      }
+      lnb_unpack(vx, x[i]);
+      lnb_unpack(vd, dy[i]);
+#pragma unroll
+      for (int e = 0; e < 8; ++e) s += x[i][e];
+    }
+    for (int o = L >> 1; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
+    const float mu = s * m.inv_D;
+    float q = 0.f;
+#pragma unroll
+    for (int i = 0; i < VPL; ++i)
+      if (act[i]) {
+#pragma unroll
+        for (int e = 0; e < 8; ++e) { x[i][e] -= mu; q = fmaf(x[i][e], x[i][e], q); }
+      }
+    for (int o = L >> 1; o > 0; o >>= 1) q += __shfl_xor_sync(0xffffffffu, q, o);
+    const float rstd = rsqrtf(q * m.inv_D + m.eps);
+    float sg = 0.f, sgx = 0.f;
+#pragma unroll
+    for (int i = 0; i < VPL; ++i)
+      if (act[i]) {
+#pragma unroll
+        for (int e = 0; e < 8; ++e) {
+          x[i][e] *= rstd;                                   // xhat
+          const float g = dy[i][e] * gam[i][e];
+          sg += g; sgx = fmaf(g, x[i][e], sgx);
+        }
+      }
+    for (int o = L >> 1; o > 0; o >>= 1) {
+      sg += __shfl_xor_sync(0xffffffffu, sg, o);
+      sgx += __shfl_xor_sync(0xffffffffu, sgx, o);
+    }
+    const float mg = sg * m.inv_D, mgx = sgx * m.inv_D;
+    if (ok) {
+#pragma unroll
+      for (int i = 0; i < VPL; ++i)
+        if (act[i]) {
+          float o8[8];
+#pragma unroll
+          for (int e = 0; e < 8; ++e) {
+            acc_g[i][e] = fmaf(dy[i][e], x[i][e], acc_g[i][e]);
+            acc_b[i][e] += dy[i][e];
+            o8[e] = rstd * (dy[i][e] * gam[i][e] - mg - x[i][e] * mgx);
+          }
+          int4 o;
+          o.x = (int)pack_bf16x2(o8[0], o8[1]); o.y = (int)pack_bf16x2(o8[2], o8[3]);
+          o.z = (int)pack_bf16x2(o8[4], o8[5]); o.w = (int)pack_bf16x2(o8[6], o8[7]);
+          __stcs(dxb + (int64_t)(b.row0 + r) * m.lddx16 + lane_in_row + i * L, o);
+        }
+    }
+  }
+  // ---- column sums of the block: row groups -> shared memory -> fixed-order sum -> workspace part
+  const bool want = m.dgamma != nullptr || m.dbeta != nullptr;
+  if (!want) return;
+  float* red_g = red;                       // [rpp][D]
+  float* red_b = red + rpp * D;
+#pragma unroll
+  for (int i = 0; i < VPL; ++i)
+    if (act[i]) {
+#pragma unroll
+      for (int e = 0; e < 8; ++e) {
+        red_g[row_in_pass * D + (lane_in_row + i * L) * 8 + e] = acc_g[i][e];
+        red_b[row_in_pass * D + (lane_in_row + i * L) * 8 + e] = acc_b[i][e];
+      }
+    }
+  __syncthreads();
+  float* part = m.ws + (size_t)b.part * 2 * D;
+  for (int c = threadIdx.x; c < D; c += kLnbThreads) {
+    float a = 0.f, bb = 0.f;
+    for (int g = 0; g < rpp; ++g) { a += red_g[g * D + c]; bb += red_b[g * D + c]; }
+    part[c] = a;
+    part[D + c] = bb;
+  }
+  // ---- last block of the member: add the parts in part order, write dgamma / dbeta, re-arm the ticket
+  __shared__ int is_last;
+  __threadfence();
+  __syncthreads();
+  if (threadIdx.x == 0) is_last = atomicAdd(m.ticket, 1) == m.nparts - 1;
+  __syncthreads();
+  if (!is_last) return;
+  __threadfence();
+  for (int c = threadIdx.x; c < D; c += kLnbThreads) {
+    float a = 0.f, bb = 0.f;
+    for (int p = 0; p < m.nparts; ++p) {
+      a += __ldcg(m.ws + (size_t)p * 2 * D + c);
+      bb += __ldcg(m.ws + (size_t)p * 2 * D + D + c);
+    }
+    if (m.dgamma) lnb_store_param<P_BF16>(m.dgamma, c, a);
+    if (m.dbeta) lnb_store_param<P_BF16>(m.dbeta, c, bb);
+  }
+  if (threadIdx.x == 0) *m.ticket = 0;
+}
+
+template <bool P_BF16>
+__global__ void __launch_bounds__(kLnbThreads, 2)
+batched_layernorm_bwd_kernel(const LnbMember* __restrict__ members, const LnbBlock* __restrict__ blocks) {
+  extern __shared__ __align__(16) float lnb_red[];      // 2 x rpp x D floats = 32 KB
+  const LnbBlock b = blocks[blockIdx.x];
+  const LnbMember m = members[b.member];
+  if (m.vpl == 1) lnb_block<P_BF16, 1>(m, b, lnb_red);
+  else lnb_block<P_BF16, 2>(m, b, lnb_red);
+}
+
+cudaError_t launch_layernorm_bwd(const opt_plan* p, cudaStream_t s) {
+  const char* base = static_cast<const char*>(p->dev_tables);
+  auto* members = reinterpret_cast<const LnbMember*>(base + p->off0);
+  auto* blocks = reinterpret_cast<const LnbBlock*>(base + p->off1);
+  if (p->param == OPT_BF16) batched_layernorm_bwd_kernel<true><<<p->grid, p->block, p->smem, s>>>(members, blocks);
+  else batched_layernorm_bwd_kernel<false><<<p->grid, p->block, p->smem, s>>>(members, blocks);
+  return cudaGetLastError();
+}
+
+}  // namespace optb
+
+using namespace optb;
+
+extern "C" opt_status opt_layernorm_bwd_plan_create(const opt_layernorm_bwd_member* members, int32_t n, opt_dtype io,
+                                                    opt_dtype param, int device, opt_plan** plan) {
+  if (plan) *plan = nullptr;
+  if (!plan || !members) return fail(OPT_ERR_INVALID_ARG, "opt_layernorm_bwd_plan_create: NULL argument");
+  if (n < 1 || n > 65535) return fail(OPT_ERR_INVALID_ARG, "n = %d outside [1, 65535]", n);
+  if ((io != OPT_F32 && io != OPT_BF16) || (param != OPT_F32 && param != OPT_BF16)) return fail(OPT_ERR_INVALID_ARG, "bad dtype");
+  if (io != OPT_BF16) return fail(OPT_ERR_UNSUPPORTED, "LayerNorm backward is implemented for bf16 activations only");
+  const int pesz = elem_size(param);
+  std::vector<Region> regions;
+  std::vector<LnbMember> tab;
+  std::vector<LnbBlock> blocks;
+  std::vector<int64_t> ws_off;            // float offset of each member's partials in the workspace
+  int64_t bytes = 0, ws_floats = 0;
+  for (int32_t i = 0; i < n; ++i) {
+    const opt_layernorm_bwd_member& m = members[i];
+    if (!m.x || !m.dy || !m.dx) return fail(OPT_ERR_INVALID_ARG, "member %d: NULL pointer", i);
+    if (m.rows < 1 || m.D < 1) return fail(OPT_ERR_INVALID_ARG, "member %d: rows=%d D=%d must be >= 1", i, m.rows, m.D);
+    if (!(m.eps >= 0.f)) return fail(OPT_ERR_INVALID_ARG, "member %d: eps must be >= 0", i);
+    if (m.rows > 1 && (m.ldx < m.D || m.lddy < m.D || m.lddx < m.D)) return fail(OPT_ERR_INVALID_ARG, "member %d: row stride smaller than D", i);
+    if (!aligned16(m.x) || !aligned16(m.dy) || !aligned16(m.dx) || !aligned16(m.gamma) || !aligned16(m.dgamma) || !aligned16(m.dbeta))
+      return fail(OPT_ERR_ALIGNMENT, "member %d: pointers must be 16-byte aligned", i);
+    if (m.D % 8) return fail(OPT_ERR_ALIGNMENT, "member %d: D=%d is not a multiple of 8", i, m.D);
+    if (m.rows > 1 && (m.ldx % 8 || m.lddy % 8 || m.lddx % 8)) return fail(OPT_ERR_ALIGNMENT, "member %d: row strides must be multiples of 8 elements", i);
+    const int nvec = m.D / 8;
+    if (nvec > 32 * kLnbMaxVpl) return fail(OPT_ERR_UNSUPPORTED, "member %d: D=%d exceeds the register-resident limit %d", i, m.D, 32 * kLnbMaxVpl * 8);
+    regions.push_back({(uintptr_t)m.x, m.ldx * 2, (int64_t)m.D * 2, m.rows, false, i});
+    regions.push_back({(uintptr_t)m.dy, m.lddy * 2, (int64_t)m.D * 2, m.rows, false, i});
+    regions.push_back({(uintptr_t)m.dx, m.lddx * 2, (int64_t)m.D * 2, m.rows, true, i});
+    if (m.gamma) regions.push_back({(uintptr_t)m.gamma, 0, (int64_t)m.D * pesz, 1, false, i});
+    if (m.dgamma) regions.push_back({(uintptr_t)m.dgamma, 0, (int64_t)m.D * pesz, 1, true, i});
+    if (m.dbeta) regions.push_back({(uintptr_t)m.dbeta, 0, (int64_t)m.D * pesz, 1, true, i});
+    bytes += 3ll * m.rows * m.D * 2 + ((m.gamma ? 1 : 0) + (m.dgamma ? 1 : 0) + (m.dbeta ? 1 : 0)) * (int64_t)m.D * pesz;
+    // lanes per row: fewest lanes such that at most kLnbMaxVpl vectors per lane
+    int ll = 0;
+    while ((nvec + (1 << ll) - 1) / (1 << ll) > kLnbMaxVpl) ++ll;
+    const int L = 1 << ll, vpl = (nvec + L - 1) / L, rpp = kLnbThreads >> ll;
+    // rows per block: whole passes, ~64 KB of x per block
+    const int64_t passes = std::max<int64_t>(1, 65536 / ((int64_t)rpp * m.D * 2));
+    const int64_t rpb = rpp * passes;
+    const int32_t nparts = (int32_t)((m.rows + rpb - 1) / rpb);
+    LnbMember t;
+    memset(&t, 0, sizeof t);
+    t.x = (const char*)m.x; t.dy = (const char*)m.dy; t.gamma = (const char*)m.gamma; t.dx = (char*)m.dx;
+    t.dgamma = (char*)m.dgamma; t.dbeta = (char*)m.dbeta;
+    t.ldx16 = m.ldx / 8; t.lddy16 = m.lddy / 8; t.lddx16 = m.lddx / 8;
+    t.rows = m.rows; t.nvec = nvec; t.nparts = nparts; t.eps = m.eps; t.inv_D = 1.0f / (float)m.D; t.l_log2 = ll; t.vpl = vpl;
+    tab.push_back(t);
+    ws_off.push_back(ws_floats);
+    ws_floats += (int64_t)nparts * 2 * m.D;
+    for (int32_t part = 0; part < nparts; ++part)
+      blocks.push_back({i, (int32_t)(part * rpb), (int32_t)std::min<int64_t>(rpb, m.rows - part * rpb), part});
+  }
+  if (opt_status st = check_independent(regions, /*allow_inplace_self=*/false)) return st;
+  if (blocks.size() > (size_t)INT32_MAX) return fail(OPT_ERR_UNSUPPORTED, "too many work items");
+
+  int num_sms = 0;
+  if (opt_status st = open_device(device, &num_sms)) return st;
+  auto align_up = [](size_t x) { return (x + 255) & ~size_t(255); };
+  opt_plan* p = new opt_plan();
+  p->kind = kPlanLayerNormBwd; p->device = device; p->io = io; p->param = param; p->n_members = n;
+  p->bytes = bytes; p->flops = 0;
+  // workspace: per-block partial column sums (fully written before they are read: no initialisation needed)
+  if (cudaMalloc(&p->workspace, std::max<int64_t>(ws_floats, 1) * sizeof(float)) != cudaSuccess) {
+    cudaGetLastError(); delete p;
+    return fail(OPT_ERR_CUDA, "cudaMalloc of the %lld-byte partial-sum workspace failed", (long long)ws_floats * 4);
+  }
+  p->off0 = 0;
+  p->off1 = align_up(tab.size() * sizeof(LnbMember));
+  p->off2 = p->off1 + align_up(blocks.size() * sizeof(LnbBlock));
+  const size_t total = p->off2 + align_up((size_t)n * sizeof(int32_t));      // per-member tickets, zero-initialised
+  std::vector<char> blob(total, 0);
+  memcpy(blob.data() + p->off1, blocks.data(), blocks.size() * sizeof(LnbBlock));
+  if (cudaMalloc(&p->dev_tables, total) != cudaSuccess) {
+    cudaGetLastError(); cudaFree(p->workspace); delete p;
+    return fail(OPT_ERR_CUDA, "cudaMalloc of the plan tables failed");
+  }
+  p->table_bytes = total;
+  for (int32_t i = 0; i < n; ++i) {
+    tab[i].ws = static_cast<float*>(p->workspace) + ws_off[i];
+    tab[i].ticket = reinterpret_cast<int32_t*>(static_cast<char*>(p->dev_tables) + p->off2) + i;
+  }
+  memcpy(blob.data(), tab.data(), tab.size() * sizeof(LnbMember));
+  cudaError_t e = cudaMemcpy(p->dev_tables, blob.data(), total, cudaMemcpyHostToDevice);
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(param == OPT_BF16 ? (const void*)batched_layernorm_bwd_kernel<true> : (const void*)batched_layernorm_bwd_kernel<false>,
+                                                 cudaFuncAttributeMaxDynamicSharedMemorySize, 32768);
+  if (e != cudaSuccess) {
+    cudaFree(p->dev_tables); cudaFree(p->workspace); delete p;
+    return fail(OPT_ERR_CUDA, "plan upload failed: %s", cudaGetErrorString(e));
+  }
+  p->grid = dim3((unsigned)blocks.size());
+  p->block = dim3(kLnbThreads);
+  p->smem = 32768;
+  p->total_tiles = (int32_t)blocks.size();
+  *plan = p;
+  return OPT_OK;
+}
