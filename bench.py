@@ -793,6 +793,26 @@ def run_product(args):
                             wgrad_us=round(tw_, 1), wgrad_tflops=round(iwg["flops"] / tw_ / 1e6, 1),
                             frac_tensor_dgrad=round(idg["flops"] / td / 1e6 / peaks["bf16_tflops"], 4),
                             frac_tensor_wgrad=round(iwg["flops"] / tw_ / 1e6 / peaks["bf16_tflops"], 4))
+            # LayerNorm backward of C4a's 512 members (dx, dgamma, dbeta), one launch
+            c4a = [g for g in step.groups if g.name.startswith("C4a")]
+            if c4a:
+                ga = c4a[0]
+                lb, keep2 = [], []
+                for i in ga.idx:
+                    x, gam = ga.ain.tensor(i["x"]), ga.ain.tensor(i["gamma"])
+                    dyl = torch.empty_like(x).normal_(0.0, 1.0)
+                    dxl, dgl, dbl = torch.empty_like(x), torch.empty_like(gam), torch.empty_like(gam)
+                    keep2.append((dyl, dxl, dgl, dbl))
+                    lb.append(ob.layernorm_bwd_member(x, dyl, gam, dxl, dgl, dbl, 1e-5))
+                pl = ob.opt_layernorm_bwd_plan_create(lb, BF16, BF16, step.dev_index)
+                pl.launch()
+                torch.cuda.synchronize()
+                tl = cold2(pl.launch)
+                il = pl.info()
+                backward.update(layernorm_bwd_workload="configs[4] LayerNorm group backward (512 members, dx + dgamma + dbeta), one launch",
+                                layernorm_bwd_us=round(tl, 1), layernorm_bwd_gbs=round(il["bytes"] / tl / 1e3, 1),
+                                layernorm_bwd_frac_hbm=round(il["bytes"] / tl / 1e3 / peaks["hbm_gbs"], 4))
+                del keep2
             del flush, keep, dy_cat
         except Exception as e:  # noqa: BLE001
             backward = dict(error=repr(e))

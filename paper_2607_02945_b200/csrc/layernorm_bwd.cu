@@ -72,6 +72,19 @@ __device__ __forceinline__ void lnb_block(const LnbMember& m, const LnbBlock& b,
     }
   }
   const int npass = (b.nrows + rpp - 1) / rpp;
+  int4 nx[VPL], nd[VPL];                    // the next pass's vectors, in flight during this pass's arithmetic
+  auto fetch = [&](int pass) {
+    const int r = pass * rpp + row_in_pass;
+#pragma unroll
+    for (int i = 0; i < VPL; ++i) {
+      nx[i] = nd[i] = make_int4(0, 0, 0, 0);
+      if (pass < npass && r < b.nrows && act[i]) {
+        nx[i] = __ldcs(xb + (int64_t)(b.row0 + r) * m.ldx16 + lane_in_row + i * L);
+        nd[i] = __ldcs(dyb + (int64_t)(b.row0 + r) * m.lddy16 + lane_in_row + i * L);
+      }
+    }
+  };
+  fetch(0);
   for (int pass = 0; pass < npass; ++pass) {
     const int r = pass * rpp + row_in_pass;
     const bool ok = r < b.nrows;
@@ -79,16 +92,12 @@ __device__ __forceinline__ void lnb_block(const LnbMember& m, const LnbBlock& b,
     float s = 0.f;
 #pragma unroll
     for (int i = 0; i < VPL; ++i) {
-      int4 vx = make_int4(0, 0, 0, 0), vd = make_int4(0, 0, 0, 0);
-      if (ok && act[i]) {
-        vx = __ldcs(xb + (int64_t)(b.row0 + r) * m.ldx16 + lane_in_row + i * L);
-        vd = __ldcs(dyb + (int64_t)(b.row0 + r) * m.lddy16 + lane_in_row + i * L);
-      }
-      lnb_unpack(vx, x[i]);
-      lnb_unpack(vd, dy[i]);
+      lnb_unpack(nx[i], x[i]);
+      lnb_unpack(nd[i], dy[i]);
 #pragma unroll
       for (int e = 0; e < 8; ++e) s += x[i][e];
     }
+    fetch(pass + 1);
     for (int o = L >> 1; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
     const float mu = s * m.inv_D;
     float q = 0.f;
@@ -176,13 +185,15 @@ __device__ __forceinline__ void lnb_block(const LnbMember& m, const LnbBlock& b,
   if (threadIdx.x == 0) *m.ticket = 0;
 }
 
-template <bool P_BF16>
-__global__ void __launch_bounds__(kLnbThreads, 2)
+// Two instantiations: groups whose rows all fit one vector per lane (D <= 256) run 4 blocks per SM in 64
+// registers; groups with wider rows keep two vectors per lane and run 2 blocks per SM without spilling.
+template <bool P_BF16, int MAXVPL>
+__global__ void __launch_bounds__(kLnbThreads, MAXVPL == 1 ? 4 : 2)
 batched_layernorm_bwd_kernel(const LnbMember* __restrict__ members, const LnbBlock* __restrict__ blocks) {
-  extern __shared__ __align__(16) float lnb_red[];      // 2 x rpp x D floats = 32 KB
+  extern __shared__ __align__(16) float lnb_red[];      // 2 x rpp x D floats <= 32 KB
   const LnbBlock b = blocks[blockIdx.x];
   const LnbMember m = members[b.member];
-  if (m.vpl == 1) lnb_block<P_BF16, 1>(m, b, lnb_red);
+  if (MAXVPL == 1 || m.vpl == 1) lnb_block<P_BF16, 1>(m, b, lnb_red);
   else lnb_block<P_BF16, 2>(m, b, lnb_red);
 }
 
@@ -190,8 +201,14 @@ cudaError_t launch_layernorm_bwd(const opt_plan* p, cudaStream_t s) {
   const char* base = static_cast<const char*>(p->dev_tables);
   auto* members = reinterpret_cast<const LnbMember*>(base + p->off0);
   auto* blocks = reinterpret_cast<const LnbBlock*>(base + p->off1);
-  if (p->param == OPT_BF16) batched_layernorm_bwd_kernel<true><<<p->grid, p->block, p->smem, s>>>(members, blocks);
-  else batched_layernorm_bwd_kernel<false><<<p->grid, p->block, p->smem, s>>>(members, blocks);
+  const bool narrow = p->nstages == 1;      // max vectors per lane over the group (stored in nstages)
+  if (p->param == OPT_BF16) {
+    if (narrow) batched_layernorm_bwd_kernel<true, 1><<<p->grid, p->block, p->smem, s>>>(members, blocks);
+    else batched_layernorm_bwd_kernel<true, 2><<<p->grid, p->block, p->smem, s>>>(members, blocks);
+  } else {
+    if (narrow) batched_layernorm_bwd_kernel<false, 1><<<p->grid, p->block, p->smem, s>>>(members, blocks);
+    else batched_layernorm_bwd_kernel<false, 2><<<p->grid, p->block, p->smem, s>>>(members, blocks);
+  }
   return cudaGetLastError();
 }
 
@@ -231,8 +248,9 @@ extern "C" opt_status opt_layernorm_bwd_plan_create(const opt_layernorm_bwd_memb
     if (m.dgamma) regions.push_back({(uintptr_t)m.dgamma, 0, (int64_t)m.D * pesz, 1, true, i});
     if (m.dbeta) regions.push_back({(uintptr_t)m.dbeta, 0, (int64_t)m.D * pesz, 1, true, i});
     bytes += 3ll * m.rows * m.D * 2 + ((m.gamma ? 1 : 0) + (m.dgamma ? 1 : 0) + (m.dbeta ? 1 : 0)) * (int64_t)m.D * pesz;
-    // lanes per row: fewest lanes such that at most kLnbMaxVpl vectors per lane
+    // lanes per row
     int ll = 0;
+    while (ll < 5 && (1 << ll) < nvec) ++ll;                  // one vector per lane when the row fits a warp
     while ((nvec + (1 << ll) - 1) / (1 << ll) > kLnbMaxVpl) ++ll;
     const int L = 1 << ll, vpl = (nvec + L - 1) / L, rpp = kLnbThreads >> ll;
     // rows per block: whole passes, ~64 KB of x per block
@@ -282,8 +300,12 @@ extern "C" opt_status opt_layernorm_bwd_plan_create(const opt_layernorm_bwd_memb
   }
   memcpy(blob.data(), tab.data(), tab.size() * sizeof(LnbMember));
   cudaError_t e = cudaMemcpy(p->dev_tables, blob.data(), total, cudaMemcpyHostToDevice);
-  if (e == cudaSuccess) e = cudaFuncSetAttribute(param == OPT_BF16 ? (const void*)batched_layernorm_bwd_kernel<true> : (const void*)batched_layernorm_bwd_kernel<false>,
-                                                 cudaFuncAttributeMaxDynamicSharedMemorySize, 32768);
+  int max_vpl = 1;
+  for (const LnbMember& t : tab) max_vpl = std::max(max_vpl, t.vpl);
+  p->nstages = max_vpl;
+  const void* fn = param == OPT_BF16 ? (max_vpl == 1 ? (const void*)batched_layernorm_bwd_kernel<true, 1> : (const void*)batched_layernorm_bwd_kernel<true, 2>)
+                                     : (max_vpl == 1 ? (const void*)batched_layernorm_bwd_kernel<false, 1> : (const void*)batched_layernorm_bwd_kernel<false, 2>);
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, 32768);
   if (e != cudaSuccess) {
     cudaFree(p->dev_tables); cudaFree(p->workspace); delete p;
     return fail(OPT_ERR_CUDA, "plan upload failed: %s", cudaGetErrorString(e));
