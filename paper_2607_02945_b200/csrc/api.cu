@@ -104,7 +104,7 @@ opt_status upload_tables(opt_plan* p, const void* host_blob, size_t bytes) {
   return OPT_OK;
 }
 
-static cudaError_t launch_any(const opt_plan* p, cudaStream_t s) {
+static cudaError_t launch_kind(const opt_plan* p, cudaStream_t s) {
   switch (p->kind) {
     case kPlanPointwise: return launch_pointwise(p, s);
     case kPlanLayerNorm: return launch_layernorm(p, s);
@@ -114,6 +114,18 @@ static cudaError_t launch_any(const opt_plan* p, cudaStream_t s) {
     case kPlanLayerNormBwd: return launch_layernorm_bwd(p, s);
     default: return cudaErrorInvalidValue;
   }
+}
+
+// The kernel goes to the PLAN's device whatever the caller's current device is (restored afterwards).
+static cudaError_t launch_any(const opt_plan* p, cudaStream_t s) {
+  int cur = -1;
+  cudaError_t e = cudaGetDevice(&cur);
+  if (e != cudaSuccess) return e;
+  if (cur == p->device) return launch_kind(p, s);
+  if ((e = cudaSetDevice(p->device)) != cudaSuccess) return e;
+  e = launch_kind(p, s);
+  cudaSetDevice(cur);
+  return e;
 }
 
 }  // namespace optb
