@@ -174,20 +174,6 @@ __device__ __forceinline__ void ln_block(const LnMember& m, int row0, int nrows)
   }
 }
 
-// ---- packed fp32 pairs (sm_100 add/mul/fma.rn.f32x2) -------------------------
-typedef unsigned long long f32x2;
-__device__ __forceinline__ f32x2 pk2(float lo, float hi) { f32x2 r; asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi)); return r; }
-__device__ __forceinline__ float sum2(f32x2 v) { float lo, hi; asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v)); return lo + hi; }
-__device__ __forceinline__ f32x2 add2(f32x2 a, f32x2 b) { f32x2 r; asm("add.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b)); return r; }
-__device__ __forceinline__ f32x2 mul2(f32x2 a, f32x2 b) { f32x2 r; asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b)); return r; }
-__device__ __forceinline__ f32x2 fma2(f32x2 a, f32x2 b, f32x2 c) { f32x2 r; asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(a), "l"(b), "l"(c)); return r; }
-__device__ __forceinline__ f32x2 bf2_to_f2(uint32_t u) { return pk2(bf16_lo(u), bf16_hi(u)); }
-__device__ __forceinline__ uint32_t f2_to_bf2(f32x2 v) {
-  float lo, hi;
-  asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v));
-  return pack_bf16x2(lo, hi);
-}
-
 // ======================================================= bf16 staged path =====
 // Persistent CTAs (3 per SM), 8 consumer warps + 1 producer warp.  The producer takes work items (a
 // tile of ~16 KB of whole rows of one member) from a dynamic scheduler -- one atomic per chunk of 8

@@ -44,30 +44,41 @@ __device__ __forceinline__ void lnb_store_param(char* base, int col, float v) {
   else reinterpret_cast<float*>(base)[col] = v;
 }
 
-template <bool P_BF16, int VPL>
+// butterfly sum over the L = 2^LL lanes that own a row (unrolled)
+template <int LL>
+__device__ __forceinline__ float lnb_rowsum(float v) {
+#pragma unroll
+  for (int o = (1 << LL) >> 1; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+  return v;
+}
+
+template <bool P_BF16, int VPL, int LL>
 __device__ __forceinline__ void lnb_block(const LnbMember& m, const LnbBlock& b, float* red) {
-  const int L = 1 << m.l_log2;
+  constexpr int L = 1 << LL;
   const int lane_in_row = threadIdx.x & (L - 1);
-  const int row_in_pass = threadIdx.x >> m.l_log2;
-  const int rpp = kLnbThreads >> m.l_log2;
+  const int row_in_pass = threadIdx.x >> LL;
+  constexpr int rpp = kLnbThreads >> LL;
   const int D = m.nvec * 8;
   const int4* xb = reinterpret_cast<const int4*>(m.x);
   const int4* dyb = reinterpret_cast<const int4*>(m.dy);
   int4* dxb = reinterpret_cast<int4*>(m.dx);
   bool act[VPL];
-  float gam[VPL][8], acc_g[VPL][8], acc_b[VPL][8];
+  f32x2 gam[VPL][4], acc_g[VPL][4], acc_b[VPL][4];       // packed fp32 pairs (add/mul/fma.rn.f32x2)
 #pragma unroll
   for (int i = 0; i < VPL; ++i) {
     const int vec = lane_in_row + i * L;
     act[i] = vec < m.nvec;
 #pragma unroll
-    for (int e = 0; e < 8; ++e) { gam[i][e] = 1.f; acc_g[i][e] = 0.f; acc_b[i][e] = 0.f; }
+    for (int k = 0; k < 4; ++k) { gam[i][k] = pk2(1.f, 1.f); acc_g[i][k] = 0ull; acc_b[i][k] = 0ull; }
     if (act[i] && m.gamma != nullptr) {
       if (P_BF16) {
-        lnb_unpack(__ldg(reinterpret_cast<const int4*>(m.gamma) + vec), gam[i]);
+        const int4 v = __ldg(reinterpret_cast<const int4*>(m.gamma) + vec);
+        const uint32_t* u = reinterpret_cast<const uint32_t*>(&v);
+#pragma unroll
+        for (int k = 0; k < 4; ++k) gam[i][k] = bf2_to_f2(u[k]);
       } else {
         const float4 a = __ldg(reinterpret_cast<const float4*>(m.gamma) + 2 * vec), c = __ldg(reinterpret_cast<const float4*>(m.gamma) + 2 * vec + 1);
-        gam[i][0] = a.x; gam[i][1] = a.y; gam[i][2] = a.z; gam[i][3] = a.w; gam[i][4] = c.x; gam[i][5] = c.y; gam[i][6] = c.z; gam[i][7] = c.w;
+        gam[i][0] = pk2(a.x, a.y); gam[i][1] = pk2(a.z, a.w); gam[i][2] = pk2(c.x, c.y); gam[i][3] = pk2(c.z, c.w);
       }
     }
   }
@@ -88,58 +99,53 @@ __device__ __forceinline__ void lnb_block(const LnbMember& m, const LnbBlock& b,
   for (int pass = 0; pass < npass; ++pass) {
     const int r = pass * rpp + row_in_pass;
     const bool ok = r < b.nrows;
-    float x[VPL][8], dy[VPL][8];
-    float s = 0.f;
+    f32x2 x[VPL][4], dy[VPL][4];
+    // three row sums that do not depend on the mean go through ONE butterfly: sum x, sum g, sum g x  (g = dy gamma);
+    // sum g xhat = rstd (sum g x - mu sum g)
+    f32x2 s2 = 0ull, sg2 = 0ull, sgx2 = 0ull;
 #pragma unroll
     for (int i = 0; i < VPL; ++i) {
-      lnb_unpack(nx[i], x[i]);
-      lnb_unpack(nd[i], dy[i]);
+      const uint32_t* ux = reinterpret_cast<const uint32_t*>(&nx[i]);
+      const uint32_t* ud = reinterpret_cast<const uint32_t*>(&nd[i]);
 #pragma unroll
-      for (int e = 0; e < 8; ++e) s += x[i][e];
+      for (int k = 0; k < 4; ++k) {
+        x[i][k] = bf2_to_f2(ux[k]);                          // inactive vectors are zeros
+        dy[i][k] = bf2_to_f2(ud[k]);
+        const f32x2 g = mul2(dy[i][k], gam[i][k]);
+        s2 = add2(s2, x[i][k]); sg2 = add2(sg2, g); sgx2 = fma2(g, x[i][k], sgx2);
+      }
     }
     fetch(pass + 1);
-    for (int o = L >> 1; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
+    const float s = lnb_rowsum<LL>(sum2(s2)), sg = lnb_rowsum<LL>(sum2(sg2));
+    float sgx = lnb_rowsum<LL>(sum2(sgx2));
     const float mu = s * m.inv_D;
-    float q = 0.f;
+    const f32x2 nmu2 = pk2(-mu, -mu);
+    f32x2 q2 = 0ull;
 #pragma unroll
     for (int i = 0; i < VPL; ++i)
       if (act[i]) {
 #pragma unroll
-        for (int e = 0; e < 8; ++e) { x[i][e] -= mu; q = fmaf(x[i][e], x[i][e], q); }
+        for (int k = 0; k < 4; ++k) { x[i][k] = add2(x[i][k], nmu2); q2 = fma2(x[i][k], x[i][k], q2); }
       }
-    for (int o = L >> 1; o > 0; o >>= 1) q += __shfl_xor_sync(0xffffffffu, q, o);
+    const float q = lnb_rowsum<LL>(sum2(q2));
     const float rstd = rsqrtf(q * m.inv_D + m.eps);
-    float sg = 0.f, sgx = 0.f;
-#pragma unroll
-    for (int i = 0; i < VPL; ++i)
-      if (act[i]) {
-#pragma unroll
-        for (int e = 0; e < 8; ++e) {
-          x[i][e] *= rstd;                                   // xhat
-          const float g = dy[i][e] * gam[i][e];
-          sg += g; sgx = fmaf(g, x[i][e], sgx);
-        }
-      }
-    for (int o = L >> 1; o > 0; o >>= 1) {
-      sg += __shfl_xor_sync(0xffffffffu, sg, o);
-      sgx += __shfl_xor_sync(0xffffffffu, sgx, o);
-    }
+    sgx = rstd * (sgx - mu * sg);
     const float mg = sg * m.inv_D, mgx = sgx * m.inv_D;
+    const f32x2 rstd2 = pk2(rstd, rstd), nmg2 = pk2(-mg, -mg), nmgx2 = pk2(-mgx, -mgx);
     if (ok) {
 #pragma unroll
       for (int i = 0; i < VPL; ++i)
         if (act[i]) {
-          float o8[8];
+          uint32_t o[4];
 #pragma unroll
-          for (int e = 0; e < 8; ++e) {
-            acc_g[i][e] = fmaf(dy[i][e], x[i][e], acc_g[i][e]);
-            acc_b[i][e] += dy[i][e];
-            o8[e] = rstd * (dy[i][e] * gam[i][e] - mg - x[i][e] * mgx);
+          for (int k = 0; k < 4; ++k) {
+            const f32x2 xh = mul2(x[i][k], rstd2);
+            acc_g[i][k] = fma2(dy[i][k], xh, acc_g[i][k]);
+            acc_b[i][k] = add2(acc_b[i][k], dy[i][k]);
+            // rstd * (dy gamma - mean(g) - xhat mean(g xhat))
+            o[k] = f2_to_bf2(mul2(fma2(xh, nmgx2, fma2(dy[i][k], gam[i][k], nmg2)), rstd2));
           }
-          int4 o;
-          o.x = (int)pack_bf16x2(o8[0], o8[1]); o.y = (int)pack_bf16x2(o8[2], o8[3]);
-          o.z = (int)pack_bf16x2(o8[4], o8[5]); o.w = (int)pack_bf16x2(o8[6], o8[7]);
-          __stcs(dxb + (int64_t)(b.row0 + r) * m.lddx16 + lane_in_row + i * L, o);
+          __stcs(dxb + (int64_t)(b.row0 + r) * m.lddx16 + lane_in_row + i * L, make_int4((int)o[0], (int)o[1], (int)o[2], (int)o[3]));
         }
     }
   }
@@ -152,9 +158,9 @@ __device__ __forceinline__ void lnb_block(const LnbMember& m, const LnbBlock& b,
   for (int i = 0; i < VPL; ++i)
     if (act[i]) {
 #pragma unroll
-      for (int e = 0; e < 8; ++e) {
-        red_g[row_in_pass * D + (lane_in_row + i * L) * 8 + e] = acc_g[i][e];
-        red_b[row_in_pass * D + (lane_in_row + i * L) * 8 + e] = acc_b[i][e];
+      for (int k = 0; k < 4; ++k) {                          // 8-byte stores: one packed pair each
+        reinterpret_cast<f32x2*>(red_g + row_in_pass * D + (lane_in_row + i * L) * 8)[k] = acc_g[i][k];
+        reinterpret_cast<f32x2*>(red_b + row_in_pass * D + (lane_in_row + i * L) * 8)[k] = acc_b[i][k];
       }
     }
   __syncthreads();
@@ -193,8 +199,18 @@ batched_layernorm_bwd_kernel(const LnbMember* __restrict__ members, const LnbBlo
   extern __shared__ __align__(16) float lnb_red[];      // 2 x rpp x D floats <= 32 KB
   const LnbBlock b = blocks[blockIdx.x];
   const LnbMember m = members[b.member];
-  if (MAXVPL == 1 || m.vpl == 1) lnb_block<P_BF16, 1>(m, b, lnb_red);
-  else lnb_block<P_BF16, 2>(m, b, lnb_red);
+  if (MAXVPL == 1 || m.vpl == 1) {
+    switch (m.l_log2) {      // block-uniform
+      case 0: lnb_block<P_BF16, 1, 0>(m, b, lnb_red); break;
+      case 1: lnb_block<P_BF16, 1, 1>(m, b, lnb_red); break;
+      case 2: lnb_block<P_BF16, 1, 2>(m, b, lnb_red); break;
+      case 3: lnb_block<P_BF16, 1, 3>(m, b, lnb_red); break;
+      case 4: lnb_block<P_BF16, 1, 4>(m, b, lnb_red); break;
+      default: lnb_block<P_BF16, 1, 5>(m, b, lnb_red); break;
+    }
+  } else {
+    lnb_block<P_BF16, 2, 5>(m, b, lnb_red);      // two vectors per lane only occur with full-warp rows
+  }
 }
 
 cudaError_t launch_layernorm_bwd(const opt_plan* p, cudaStream_t s) {
