@@ -744,9 +744,12 @@ def run_product(args):
                 return float(np.mean(ts))
             t1 = cold(p2.launch)
             t2 = cold(lambda: (gb.plan.launch(), gc.plan.launch()))
+            t3 = cold(lambda: (ga.plan.launch(), p2.launch()))                       # whole C4 block: LN + chained Linear
+            t4 = cold(lambda: (ga.plan.launch(), gb.plan.launch(), gc.plan.launch()))  # whole C4 block: three groups
             i2 = p2.info()
             vertical = dict(workload="C4 towers: Linear(D->H)+ReLU -> Linear(H->64), 512 members, B=8192", launches=1,
                             linear2_us=round(t1, 1), two_launch_us=round(t2, 1), speedup=round(t2 / t1, 3),
+                            c4_block_ln_plus_linear2_us=round(t3, 1), c4_block_three_groups_us=round(t4, 1),
                             bitwise_equal_to_two_launch=same, flops=i2["flops"], algorithmic_bytes=i2["bytes"],
                             tflops=round(i2["flops"] / t1 / 1e6, 1),
                             frac_tensor=round(i2["flops"] / t1 / 1e6 / peaks["bf16_tflops"], 4),

@@ -51,6 +51,8 @@ def lib():
         L.oracle_pointwise.argtypes = [vp, i64, i32, i32, c.c_int, c.c_int, vp]
         L.oracle_pointwise_ext.argtypes = [vp, i64, vp, i64, i32, i32, c.c_int, dbl, dbl, dbl, c.c_int, vp]
         L.oracle_layernorm.argtypes = [vp, i64, vp, vp, i32, i32, dbl, c.c_int, c.c_int, vp, vp]
+        L.oracle_quant_e4m3.argtypes = [vp, i64, i32, i32, dbl, c.c_int, vp]
+        L.oracle_dequant_e4m3.argtypes = [vp, i64, i32, i32, dbl, vp]
         L.oracle_layernorm_backward.argtypes = [vp, i64, vp, i64, vp, i32, i32, dbl, c.c_int, c.c_int, vp, vp, vp]
         L.oracle_split.argtypes = [vp, i64, i32, i32, i32, vp, i32, vp]
         L.oracle_split.restype = c.c_int
@@ -147,6 +149,24 @@ def pointwise_ext(a, b, op, params, dt):
     out = np.empty((rows, width), dtype=np.float64)
     lib().oracle_pointwise_ext(_ptr(a), _ld(a), _ptr(b), 0 if b is None else _ld(b), rows, width, int(op),
                                p[0], p[1], p[2], dt, _ptr(out))
+    return out
+
+
+def quant_e4m3(src, scale, dt):
+    """FP8 E4M3 codes (uint8) of src * scale, round-to-nearest-even, saturating at +-448."""
+    _chk(src, dt, 2)
+    rows, width = src.shape
+    out = np.empty((rows, width), dtype=np.uint8)
+    lib().oracle_quant_e4m3(_ptr(src), _ld(src), rows, width, float(np.float32(scale)), dt, _ptr(out))
+    return out
+
+
+def dequant_e4m3(codes, scale):
+    """fp64 values of FP8 E4M3 codes times scale."""
+    codes = np.ascontiguousarray(codes, dtype=np.uint8)
+    rows, width = codes.shape
+    out = np.empty((rows, width), dtype=np.float64)
+    lib().oracle_dequant_e4m3(_ptr(codes), width, rows, width, float(np.float32(scale)), _ptr(out))
     return out
 
 

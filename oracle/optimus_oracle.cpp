@@ -209,6 +209,44 @@ void oracle_pointwise_ext(const void* a, int64_t lda, const void* b, int64_t ldb
     }
 }
 
+// ---- FP8 (OCP E4M3: 1 sign, 4 exponent bits with bias 7, 3 mantissa bits; no infinity, S.1111.111 = NaN,
+// largest finite 448) quantisation of saved activations -- activation_quantization_aten_pass (PAPER.md:341-345,
+// :487-489: "quantized into a lower-precision format, such as FP8, in the forward pass ... dequantized back to
+// their original precision before use", optional scaling).
+//   quantise:   code = e4m3_rne_satfinite(x * scale)    (|v| > 448 and +-inf saturate to +-448, NaN -> NaN)
+//   dequantise: y    = value(code) * scale
+static double e4m3_value(uint8_t c) {
+  const int e = (c >> 3) & 0xF, m = c & 7;
+  double v;
+  if (e == 0xF && m == 7) return std::nan("");
+  if (e == 0) v = std::ldexp((double)m, -9);                 // subnormal: m * 2^-6 * 2^-3
+  else v = std::ldexp(8.0 + m, e - 10);                      // (1 + m/8) * 2^(e-7)
+  return (c & 0x80) ? -v : v;
+}
+static uint8_t f64_to_e4m3(double x) {
+  if (std::isnan(x)) return 0x7F;
+  const uint8_t sign = std::signbit(x) ? 0x80 : 0;
+  const double a = std::fabs(x);
+  if (a >= 448.0) return sign | 0x7E;                        // satfinite (also inf)
+  // nearest representable code in [0x00, 0x7E], ties to the even code: the codes are monotone in value
+  int lo = 0, hi = 0x7E;
+  while (hi - lo > 1) { const int mid = (lo + hi) >> 1; if (e4m3_value((uint8_t)mid) <= a) lo = mid; else hi = mid; }
+  const double vl = e4m3_value((uint8_t)lo), vh = e4m3_value((uint8_t)hi);
+  const double dl = a - vl, dh = vh - a;
+  int c = dl < dh ? lo : (dh < dl ? hi : ((lo & 1) ? hi : lo));
+  return sign | (uint8_t)c;
+}
+void oracle_quant_e4m3(const void* src, int64_t lds, int32_t rows, int32_t width, double scale, int dt, uint8_t* out) {
+#pragma omp parallel for schedule(static)
+  for (int32_t r = 0; r < rows; ++r)
+    for (int32_t c = 0; c < width; ++c) out[(int64_t)r * width + c] = f64_to_e4m3(widen(src, (int64_t)r * lds + c, dt) * scale);
+}
+void oracle_dequant_e4m3(const uint8_t* src, int64_t lds, int32_t rows, int32_t width, double scale, double* out) {
+#pragma omp parallel for schedule(static)
+  for (int32_t r = 0; r < rows; ++r)
+    for (int32_t c = 0; c < width; ++c) out[(int64_t)r * width + c] = e4m3_value(src[(int64_t)r * lds + c]) * scale;
+}
+
 // ---- layer_norm over the last dim (batch_layernorm; torch
 // semantics, reading Q4): mu = sum(x)/D; v = sum((x-mu)^2)/D (biased);
 // y_j = (x_j-mu)/sqrt(v+eps) * gamma_j + beta_j.  gamma/beta may be NULL (1/0).

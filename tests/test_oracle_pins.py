@@ -518,3 +518,39 @@ def test_layernorm_backward_finite_differences_and_identities():
     dx1, dg1, _ = oracle.layernorm_backward(x, dy, None, eps, F32)
     dx2, dg2, _ = oracle.layernorm_backward(x, dy, np.ones(D, np.float32), eps, F32)
     assert np.array_equal(dx1, dx2) and np.array_equal(dg1, dg2)
+
+
+# -------------------------------- FP8 E4M3 activation quantisation --
+def _e4m3_from_definition(c):
+    """value of a code from the format definition (OCP FP8 E4M3: bias 7, no infinities, S.1111.111 = NaN)."""
+    e, m = (c >> 3) & 0xF, c & 7
+    if e == 0xF and m == 7:
+        return float("nan")
+    v = m * 2.0 ** -9 if e == 0 else (1 + m / 8.0) * 2.0 ** (e - 7)
+    return -v if c & 0x80 else v
+
+
+def test_e4m3_decode_exhaustive_and_encode_ties_saturation():
+    codes = np.arange(256, dtype=np.uint8).reshape(1, 256)
+    vals = oracle.dequant_e4m3(codes, 1.0)[0]
+    ref = np.array([_e4m3_from_definition(int(c)) for c in range(256)])
+    assert np.array_equal(np.isnan(vals), np.isnan(ref)) and np.array_equal(vals[~np.isnan(ref)], ref[~np.isnan(ref)])
+    assert vals[0x7E] == 448.0 and vals[0x01] == 2.0 ** -9 and vals[0x08] == 2.0 ** -6
+    # encode: every finite code maps to itself; midpoints between neighbours go to the EVEN code; just off the
+    # midpoint goes to the nearer one; beyond 448 saturates; NaN stays NaN; inf saturates (satfinite)
+    pos = np.array([_e4m3_from_definition(c) for c in range(0x7F)])
+    enc = lambda a: oracle.quant_e4m3(np.asarray(a, dtype=np.float32).reshape(1, -1), 1.0, F32)[0]
+    assert np.array_equal(enc(pos), np.arange(0x7F)) and np.array_equal(enc(-pos[1:]), np.arange(1, 0x7F) | 0x80)
+    mids = (pos[:-1] + pos[1:]) / 2                       # exactly representable in fp32
+    got = enc(mids)
+    want = np.where(np.arange(0x7E) % 2 == 0, np.arange(0x7E), np.arange(1, 0x7F))
+    assert np.array_equal(got, want)
+    assert np.array_equal(enc(np.nextafter(mids.astype(np.float32), np.float32(np.inf))), np.arange(1, 0x7F))
+    assert np.array_equal(enc(np.nextafter(mids.astype(np.float32), np.float32(0))), np.arange(0x7E))
+    assert list(enc([448.0, 449.0, 1e9, np.inf, -np.inf, -500.0])) == [0x7E, 0x7E, 0x7E, 0x7E, 0xFE, 0xFE]
+    assert enc([np.nan])[0] & 0x7F == 0x7F
+    # scaling: quantise(x, s) == quantise(x * s, 1) for a power-of-two scale; dequantise multiplies back
+    x = wl.tensor_normal(51, 1, (4, 64), 0, 3.0, BF16)
+    q = oracle.quant_e4m3(x, 0.25, BF16)
+    assert np.array_equal(q, enc(wl.f32_from_bf16_bits(x).reshape(-1) * 0.25).reshape(4, 64))
+    assert np.array_equal(oracle.dequant_e4m3(q, 4.0), oracle.dequant_e4m3(q, 1.0) * 4.0)
