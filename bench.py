@@ -816,6 +816,23 @@ def run_product(args):
                                 layernorm_bwd_us=round(tl, 1), layernorm_bwd_gbs=round(il["bytes"] / tl / 1e3, 1),
                                 layernorm_bwd_frac_hbm=round(il["bytes"] / tl / 1e3 / peaks["hbm_gbs"], 4))
                 del keep2
+                # activation_quantization_aten_pass: the 512 saved LayerNorm outputs -> FP8 E4M3 and back, one launch each
+                A = ga.amid.tensor
+                q8 = [torch.empty(A(i["xn"]).shape, dtype=torch.uint8, device=device) for i in ga.idx]
+                r16 = [torch.empty_like(A(i["xn"])) for i in ga.idx]
+                pq = ob.opt_pointwise_plan_create([ob.chunk(A(i["xn"]), q, ob.OPT_PW_QUANT_E4M3, None, [16.0])
+                                                   for i, q in zip(ga.idx, q8)], BF16, step.dev_index)
+                pdq = ob.opt_pointwise_plan_create([ob.chunk(q, r, ob.OPT_PW_DEQUANT_E4M3, None, [1.0 / 16.0])
+                                                    for q, r in zip(q8, r16)], BF16, step.dev_index)
+                pq.launch(); pdq.launch()
+                torch.cuda.synchronize()
+                tq, tdq = cold2(pq.launch), cold2(pdq.launch)
+                backward.update(fp8_workload="configs[4] saved LayerNorm outputs (512 x [B, D] bf16) -> FP8 E4M3 and back, one launch each",
+                                fp8_quant_us=round(tq, 1), fp8_quant_gbs=round(pq.info()["bytes"] / tq / 1e3, 1),
+                                fp8_quant_frac_hbm=round(pq.info()["bytes"] / tq / 1e3 / peaks["hbm_gbs"], 4),
+                                fp8_dequant_us=round(tdq, 1), fp8_dequant_gbs=round(pdq.info()["bytes"] / tdq / 1e3, 1),
+                                fp8_dequant_frac_hbm=round(pdq.info()["bytes"] / tdq / 1e3 / peaks["hbm_gbs"], 4))
+                del q8, r16
             del flush, keep, dy_cat
         except Exception as e:  # noqa: BLE001
             backward = dict(error=repr(e))

@@ -79,7 +79,10 @@ typedef enum {
   OPT_PW_NAN_TO_NUM = 5, /* batch_nan_to_num: NaN -> p0, +inf -> p1, -inf -> p2, finite values unchanged          */
   OPT_PW_SUB = 6,        /* batch_aten_sub:   dst = src - src2                                                     */
   OPT_PW_DIV = 7,        /* batch_aten_div:   dst = src / src2                                                     */
-  OPT_PW_MUL = 8         /* batch_aten_mul:   dst = src * src2                                                     */
+  OPT_PW_MUL = 8,        /* batch_aten_mul:   dst = src * src2                                                     */
+  /* activation_quantization_aten_pass: saved activations kept in FP8 (OCP E4M3) */
+  OPT_PW_QUANT_E4M3 = 9,    /* dst (fp8, 1 byte/element, ldd in fp8 elements) = e4m3_rne_satfinite(src * p0)      */
+  OPT_PW_DEQUANT_E4M3 = 10  /* dst (bf16) = value(src fp8 code, lds in fp8 elements) * p0                          */
 } opt_pw_op;
 
 /* Storage of the two operands of a grouped Linear member.  Default 0: x is [M,K], w is [N,K] (torch nn.Linear).

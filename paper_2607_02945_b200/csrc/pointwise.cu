@@ -30,6 +30,8 @@
 #include <map>
 #include <tuple>
 
+#include <cuda_fp8.h>
+
 #include "common.h"
 
 namespace optb {
@@ -124,6 +126,57 @@ __device__ __forceinline__ int4 pw_ext_apply(int4 a, int4 b, int op, float p0, f
   }
   return a;
 }
+// FP8 E4M3 quantise / dequantise of saved activations (activation_quantization_aten_pass): the
+// bf16 side moves 16-byte vectors, the fp8 side the matching 8-byte vectors; p0 is the scale.  Saturating RNE, NaN -> NaN.
+__device__ __forceinline__ int2 pw_quant_e4m3(int4 v, float scale) {
+  const uint32_t* u = reinterpret_cast<const uint32_t*>(&v);
+  uint32_t o[2];
+#pragma unroll
+  for (int i = 0; i < 2; ++i) {
+    const uint32_t lo = __nv_cvt_float2_to_fp8x2(make_float2(bf16_lo(u[2 * i]) * scale, bf16_hi(u[2 * i]) * scale), __NV_SATFINITE, __NV_E4M3);
+    const uint32_t hi = __nv_cvt_float2_to_fp8x2(make_float2(bf16_lo(u[2 * i + 1]) * scale, bf16_hi(u[2 * i + 1]) * scale), __NV_SATFINITE, __NV_E4M3);
+    o[i] = lo | (hi << 16);
+  }
+  return make_int2((int)o[0], (int)o[1]);
+}
+__device__ __forceinline__ int4 pw_dequant_e4m3(int2 v, float scale) {
+  const uint32_t w[2] = {(uint32_t)v.x, (uint32_t)v.y};
+  uint32_t o[4];
+#pragma unroll
+  for (int i = 0; i < 4; ++i) {
+    const __half2_raw h = __nv_cvt_fp8x2_to_halfraw2((__nv_fp8x2_storage_t)((w[i >> 1] >> (16 * (i & 1))) & 0xFFFFu), __NV_E4M3);
+    const float2 f = __half22float2(*reinterpret_cast<const __half2*>(&h));
+    o[i] = pack_bf16x2(f.x * scale, f.y * scale);
+  }
+  return make_int4((int)o[0], (int)o[1], (int)o[2], (int)o[3]);
+}
+__device__ __forceinline__ void pw_fp8_rows(const PwGroup& g, int q, int r, int rend, int ty_step) {
+  constexpr int U = 4;
+  if (g.ext_op == OPT_PW_QUANT_E4M3) {
+    const int4* s = reinterpret_cast<const int4*>(g.src) + q;
+    int2* d = reinterpret_cast<int2*>(g.dst) + q;
+    for (; r + (U - 1) * ty_step < rend; r += U * ty_step) {
+      int4 v[U];
+#pragma unroll
+      for (int i = 0; i < U; ++i) v[i] = __ldcs(s + (int64_t)(r + i * ty_step) * g.lds16);
+#pragma unroll
+      for (int i = 0; i < U; ++i) __stcs(d + (int64_t)(r + i * ty_step) * g.ldd16, pw_quant_e4m3(v[i], g.p0));
+    }
+    for (; r < rend; r += ty_step) __stcs(d + (int64_t)r * g.ldd16, pw_quant_e4m3(__ldcs(s + (int64_t)r * g.lds16), g.p0));
+  } else {
+    const int2* s = reinterpret_cast<const int2*>(g.src) + q;
+    int4* d = reinterpret_cast<int4*>(g.dst) + q;
+    for (; r + (U - 1) * ty_step < rend; r += U * ty_step) {
+      int2 v[U];
+#pragma unroll
+      for (int i = 0; i < U; ++i) v[i] = __ldcs(s + (int64_t)(r + i * ty_step) * g.lds16);
+#pragma unroll
+      for (int i = 0; i < U; ++i) __stcs(d + (int64_t)(r + i * ty_step) * g.ldd16, pw_dequant_e4m3(v[i], g.p0));
+    }
+    for (; r < rend; r += ty_step) __stcs(d + (int64_t)r * g.ldd16, pw_dequant_e4m3(__ldcs(s + (int64_t)r * g.lds16), g.p0));
+  }
+}
+
 template <bool BF16>
 __device__ __forceinline__ void pw_ext_rows(const PwGroup& g, int q, int r, int rend, int ty_step) {
   const int4* s = reinterpret_cast<const int4*>(g.src) + q;
@@ -258,7 +311,8 @@ multi_pointwise_splitcat_kernel(const PwGroup* __restrict__ groups, const int2* 
   const int q = b.q0 + tx;
   if (q >= g.W) return;
   if (g.ext_op) {                         // block-uniform: one chunk, no map
-    pw_ext_rows<BF16>(g, q, b.r0 + ty, b.r0 + b.nrows, ty_step);
+    if (g.ext_op >= OPT_PW_QUANT_E4M3) pw_fp8_rows(g, q, b.r0 + ty, b.r0 + b.nrows, ty_step);
+    else pw_ext_rows<BF16>(g, q, b.r0 + ty, b.r0 + b.nrows, ty_step);
     return;
   }
   const int2 m = __ldg(vmap + g.map_off + q);
@@ -316,8 +370,12 @@ extern "C" opt_status opt_pointwise_plan_create(const opt_chunk* chunks, int32_t
     const opt_chunk& c = chunks[i];
     if (!c.src || !c.dst) return fail(OPT_ERR_INVALID_ARG, "chunk %d: NULL pointer", i);
     if (c.rows < 1 || c.width < 1) return fail(OPT_ERR_INVALID_ARG, "chunk %d: rows=%d width=%d must be >= 1", i, c.rows, c.width);
-    if (c.op < OPT_PW_COPY || c.op > OPT_PW_MUL) return fail(OPT_ERR_INVALID_ARG, "chunk %d: bad op %d", i, c.op);
-    const bool ext = c.op >= OPT_PW_CLAMP, binary = c.op >= OPT_PW_SUB;
+    if (c.op < OPT_PW_COPY || c.op > OPT_PW_DEQUANT_E4M3) return fail(OPT_ERR_INVALID_ARG, "chunk %d: bad op %d", i, c.op);
+    const bool ext = c.op >= OPT_PW_CLAMP, binary = c.op >= OPT_PW_SUB && c.op <= OPT_PW_MUL;
+    const bool fp8 = c.op >= OPT_PW_QUANT_E4M3;
+    if (fp8 && io != OPT_BF16) return fail(OPT_ERR_UNSUPPORTED, "chunk %d: FP8 quantisation is implemented for bf16 activations only", i);
+    // element sizes of the two sides: quantise writes fp8, dequantise reads fp8
+    const int s_esz = c.op == OPT_PW_DEQUANT_E4M3 ? 1 : esz, d_esz = c.op == OPT_PW_QUANT_E4M3 ? 1 : esz;
     if (binary) {
       if (!c.src2) return fail(OPT_ERR_INVALID_ARG, "chunk %d: binary op %d needs src2", i, c.op);
       if (c.rows > 1 && c.lds2 < c.width) return fail(OPT_ERR_INVALID_ARG, "chunk %d: row stride of src2 smaller than width", i);
@@ -330,10 +388,10 @@ extern "C" opt_status opt_pointwise_plan_create(const opt_chunk* chunks, int32_t
     if (c.width % V) return fail(OPT_ERR_ALIGNMENT, "chunk %d: width %d is not a multiple of %d", i, c.width, V);
     if (c.rows > 1 && (c.lds % V || c.ldd % V))
       return fail(OPT_ERR_ALIGNMENT, "chunk %d: row strides must be multiples of %d elements", i, V);
-    regions.push_back({(uintptr_t)c.src, c.lds * esz, (int64_t)c.width * esz, c.rows, false, i});
-    regions.push_back({(uintptr_t)c.dst, c.ldd * esz, (int64_t)c.width * esz, c.rows, true, i});
+    regions.push_back({(uintptr_t)c.src, c.lds * s_esz, (int64_t)c.width * s_esz, c.rows, false, i});
+    regions.push_back({(uintptr_t)c.dst, c.ldd * d_esz, (int64_t)c.width * d_esz, c.rows, true, i});
     if (binary) regions.push_back({(uintptr_t)c.src2, c.lds2 * esz, (int64_t)c.width * esz, c.rows, false, i});
-    bytes += (binary ? 3ll : 2ll) * c.rows * c.width * esz;
+    bytes += (int64_t)c.rows * c.width * (s_esz + d_esz + (binary ? esz : 0));
 
     const int64_t wv = c.width / V;
     const bool dense = c.rows == 1 || (c.lds == c.width && c.ldd == c.width && (!binary || c.lds2 == c.width));
@@ -347,8 +405,9 @@ extern "C" opt_status opt_pointwise_plan_create(const opt_chunk* chunks, int32_t
         cc.push_back({(const char*)c.src, (char*)c.dst, kFlatW, kFlatW, (int32_t)r2, kFlatW, c.op});
         done = r2 * kFlatW;
       }
-      if (T > done)
-        cc.push_back({(const char*)c.src + done * 16, (char*)c.dst + done * 16, 0, 0, 1, (int32_t)(T - done), c.op});
+      if (T > done)       // (a vector is 8 elements on both sides: 16 bytes of bf16 / fp32x4, 8 bytes of fp8)
+        cc.push_back({(const char*)c.src + done * (c.op == OPT_PW_DEQUANT_E4M3 ? 8 : 16),
+                      (char*)c.dst + done * (c.op == OPT_PW_QUANT_E4M3 ? 8 : 16), 0, 0, 1, (int32_t)(T - done), c.op});
     } else {
       if (wv > INT32_MAX) return fail(OPT_ERR_UNSUPPORTED, "chunk %d too wide", i);
       cc.push_back({(const char*)c.src, (char*)c.dst, c.lds / V, c.ldd / V, c.rows, (int32_t)wv, c.op});

@@ -207,3 +207,107 @@ def test_table1_patterns_fp32_and_errors(ob):
     with pytest.raises(ob.OptError) as e:                  # second operand overlaps another member's output
         ob.opt_pointwise_plan_create([ob.chunk(da, outs[0], ob.OPT_PW_MUL, db), ob.chunk(da, outs[1], ob.OPT_PW_MUL, outs[0])], F32)
     assert e.value.status == ob.OPT_ERR_ALIAS
+
+
+def _quant_case(seed, i, rows, w, std, strided):
+    a = _special(wl.tensor_normal(seed, i, (rows, w), 0.0, std, BF16))
+    pad = 16 if strided else 0
+    da = to_dev(np.pad(a, ((0, 0), (0, pad))), BF16)[:, :w]
+    dq = torch.full((rows, w + pad), 0xAA, dtype=torch.uint8, device="cuda")[:, :w]
+    return a, da, dq
+
+
+def test_fp8_e4m3_quant_dequant_one_launch_each(ob):
+    """activation_quantization_aten_pass: a group of saved activations -> FP8 E4M3 codes in one
+    launch, and back in one launch.  The code is an integer decided by floating point: both sides decide it on the
+    kernel's fp32 product x * scale (bit-exact); with a power-of-two scale that product is exact and the fp64 oracle
+    on (x, scale) agrees too.  Dequantised values: exact (a 4-bit significand times a power of two fits bf16) for
+    power-of-two scales, <= 1 bf16 ulp otherwise."""
+    shapes = [(300, 512), (77, 200), (1000, 64), (129, 1032), (64, 8), (5, 4096), (2048, 256)]
+    scales = [1.0, 0.25, 16.0, 0.7310791015625, 3.3, 1.0 / 448.0, 37.0]
+    stds = [2.0, 100.0, 0.05, 1.0, 300.0, 1000.0, 3.0]
+    host, chunks, keep = [], [], []
+    for i, ((r, w), sc, sd) in enumerate(zip(shapes, scales, stds)):
+        a, da, dq = _quant_case(51, i, r, w, sd, strided=i % 2 == 1)
+        chunks.append(ob.chunk(da, dq, ob.OPT_PW_QUANT_E4M3, None, [sc]))
+        host.append((a, sc))
+        keep.append((da, dq))
+    plan = ob.opt_pointwise_plan_create(chunks, BF16)
+    n0 = ob.opt_launch_count()
+    plan.launch()
+    torch.cuda.synchronize()
+    assert ob.opt_launch_count() - n0 == 1
+    codes = []
+    for (a, sc), (_, dq) in zip(host, keep):
+        got = dq.cpu().numpy()
+        prod32 = (wl.f32_from_bf16_bits(a) * np.float32(sc)).astype(np.float32)       # the kernel's precision
+        ref = oracle.quant_e4m3(prod32, 1.0, F32)
+        assert np.array_equal(got, ref), (sc, int((got != ref).sum()))
+        ref64 = oracle.quant_e4m3(a, sc, BF16)                                        # the plain fp64 definition
+        bad = got != ref64
+        if np.log2(sc) == np.round(np.log2(sc)):
+            assert not bad.any()
+        else:   # rounding the product to fp32 first can only move it onto / off a tie: adjacent code.  (Not always
+            #       rare: with scale = fp32(1/448), x = 7 * odd * 2^n puts the fp32 product exactly on a tie.)
+            assert bad.mean() < 0.05 and np.all(np.abs(got[bad].astype(int) - ref64[bad].astype(int)) <= 1)
+        assert (got == 0x7F).sum() + (got == 0xFF).sum() == ((a & 0x7FFF) > 0x7F80).sum()   # NaN <-> NaN only
+        codes.append(got)
+    # untouched padding of the strided outputs
+    for i, (_, dq) in enumerate(keep):
+        if i % 2 == 1:
+            base = dq.as_strided((dq.shape[0], dq.shape[1] + 16), (dq.stride(0), 1))
+            assert bool((base[:, dq.shape[1]:] == 0xAA).all())
+
+    # dequantise the codes back, one launch
+    chunks, outs = [], []
+    for i, ((a, sc), (_, dq)) in enumerate(zip(host, keep)):
+        pad = 8 if i % 2 == 0 else 0
+        dy = empty_dev((dq.shape[0], dq.shape[1] + pad), BF16, fill=float("nan"))[:, :dq.shape[1]]
+        chunks.append(ob.chunk(dq, dy, ob.OPT_PW_DEQUANT_E4M3, None, [1.0 / sc]))
+        outs.append(dy)
+    plan = ob.opt_pointwise_plan_create(chunks, BF16)
+    n0 = ob.opt_launch_count()
+    plan.launch()
+    torch.cuda.synchronize()
+    assert ob.opt_launch_count() - n0 == 1
+    for (a, sc), c, dy in zip(host, codes, outs):
+        ref = oracle.round_to_storage(oracle.dequant_e4m3(c, 1.0 / sc), BF16)
+        got = to_host(dy)
+        d = bf16_ulp_distance(got, ref)
+        pow2 = np.log2(sc) == np.round(np.log2(sc))
+        assert d.max() <= (0 if pow2 else 1), (sc, int(d.max()))
+
+
+def test_fp8_e4m3_all_codes_and_rounding_boundaries(ob):
+    """every one of the 256 codes through dequantise (exact), and every bf16 value in [-2^10, 2^10] through quantise
+    (all rounding ties, subnormal codes, saturation at 448, signed zero) bit-exact against the fp64 oracle."""
+    c = np.arange(256, dtype=np.uint8).reshape(1, 256).repeat(3, 0)
+    dc = torch.from_numpy(c).cuda()
+    dy = empty_dev((3, 256), BF16)
+    ob.opt_pointwise_plan_create([ob.chunk(dc, dy, ob.OPT_PW_DEQUANT_E4M3, None, [1.0])], BF16).launch()
+    torch.cuda.synchronize()
+    ref = oracle.round_to_storage(oracle.dequant_e4m3(c, 1.0), BF16)
+    assert bf16_ulp_distance(to_host(dy), ref).max() == 0
+    assert np.array_equal(to_host(dy)[:, :0x7F], ref[:, :0x7F]) and np.array_equal(to_host(dy)[:, 0x80:0xFF], ref[:, 0x80:0xFF])
+
+    allb = np.arange(65536, dtype=np.uint32).astype(np.uint16).reshape(64, 1024)
+    da = to_dev(allb, BF16)
+    dq = torch.empty((64, 1024), dtype=torch.uint8, device="cuda")
+    ob.opt_pointwise_plan_create([ob.chunk(da, dq, ob.OPT_PW_QUANT_E4M3, None, [1.0])], BF16).launch()
+    torch.cuda.synchronize()
+    got, ref = dq.cpu().numpy(), oracle.quant_e4m3(allb, 1.0, BF16)
+    nan = (ref & 0x7F) == 0x7F                             # NaN -> NaN (the sign of a NaN code is not part of the contract)
+    assert np.array_equal(got[~nan], ref[~nan]) and np.all((got[nan] & 0x7F) == 0x7F)
+
+
+def test_fp8_errors(ob):
+    a = empty_dev((16, 64), F32, fill=1.0)
+    q = torch.empty((16, 64), dtype=torch.uint8, device="cuda")
+    with pytest.raises(ob.OptError) as e:                  # fp32 activations: not implemented
+        ob.opt_pointwise_plan_create([ob.chunk(a, q, ob.OPT_PW_QUANT_E4M3, None, [1.0])], F32)
+    assert e.value.status == ob.OPT_ERR_UNSUPPORTED
+    b = empty_dev((16, 64), BF16, fill=1.0)
+    with pytest.raises(ob.OptError) as e:                  # fp8 row stride must keep 8-byte vectors aligned
+        ob.opt_pointwise_plan_create([ob.chunk(b, torch.empty((16, 68), dtype=torch.uint8, device="cuda")[:, :64],
+                                               ob.OPT_PW_QUANT_E4M3, None, [1.0])], BF16)
+    assert e.value.status == ob.OPT_ERR_ALIGNMENT
