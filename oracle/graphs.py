@@ -10,7 +10,7 @@ between the groups of configs[4] (reading Q3).
 import numpy as np
 
 from . import (BF16, F32, activation, cat, layernorm, linear, pointwise,  # noqa: F401
-               round_to_storage, split)
+               round_to_storage, split, widen)
 
 
 def linear_member(m, dt):
@@ -78,6 +78,25 @@ def linear2(m, dt=BF16):
     h = round_to_storage(h64, dt)
     y64 = activation(linear(h, m["w2"], m.get("b2"), dt), m["act2"])
     return dict(h64=h64, h=h, y64=y64, y=round_to_storage(y64, dt))
+
+
+def ln_linear2(m, dt=BF16):
+    """LayerNorm -> Linear + act1 -> Linear + act2 of one tower as ONE vertically fused op ("chained
+    transformations", Fig. 5, the LayerNorm folded in).  Reading Q25: the
+    fused op never materialises the normalised tensor, so it is NOT rounded here; the hidden tensor is still
+    rounded to the storage dtype (as in `linear2`, reading Q3):
+        xn = layer_norm(x; gamma, beta, eps)          fp64, unrounded
+        h  = act1(xn W1^T + b1)  -> rounded            (first layer: a plain fp64 matmul on the unrounded xn)
+        y  = act2(h W2^T + b2)   -> rounded
+    Returns dict(xn64, h64, h, y64, y)."""
+    xn64 = layernorm(m["x"], m.get("gamma"), m.get("beta"), m["eps"], dt)
+    z = xn64 @ widen(m["w1"], dt).T
+    if m.get("b1") is not None:
+        z = z + widen(m["b1"], dt)[None, :]
+    h64 = activation(z, m["act1"])
+    h = round_to_storage(h64, dt)
+    y64 = activation(linear(h, m["w2"], m.get("b2"), dt), m["act2"])
+    return dict(xn64=xn64, h64=h64, h=h, y64=y64, y=round_to_storage(y64, dt))
 
 
 def _transposed(a):

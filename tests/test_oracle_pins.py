@@ -429,6 +429,44 @@ def test_linear2_identity_second_layer_returns_hidden():
     assert np.allclose(r["h64"], ref, rtol=1e-13, atol=1e-15)
 
 
+def test_ln_linear2_sign_rows_reduce_to_integer_chain_and_affine_invariance():
+    """LayerNorm folded into the chain (reading Q25).  Rows made of equally many -1 and +1 have mean 0 and variance
+    1, so with eps = 0 the normalised row IS the row, and with small integer gamma / beta the whole chain is integer
+    arithmetic: must equal numpy's integers bit for bit (pins: gamma multiplies before beta is added, LN feeds W1,
+    ReLU sits after the first layer, W2 multiplies the hidden tensor).  Layer norm is invariant under x -> a x + c
+    (a > 0) when eps = 0: the same rows mapped to {2, 8} give the same result to rounding.  A row that is NOT
+    pre-normalised is checked against a literal numpy transcription of torch's layer_norm formula."""
+    rng = np.random.default_rng(11)
+    M, K, H, N = 6, 16, 24, 8
+    x = np.stack([rng.permutation(np.repeat([-1, 1], K // 2)) for _ in range(M)])
+    g = rng.integers(-2, 3, (K,)); be = rng.integers(-2, 3, (K,))
+    w1 = rng.integers(-2, 3, (H, K)); b1 = rng.integers(-2, 3, (H,))
+    w2 = rng.integers(-1, 2, (N, H)); b2 = rng.integers(-2, 3, (N,))
+    xn = x * g + be
+    h = np.maximum(xn @ w1.T + b1, 0)                      # |h| <= 16*4*2+2 = 130: exact in bf16
+    y = h @ w2.T + b2
+    m = dict(x=bf16(x), gamma=bf16(g), beta=bf16(be), eps=0.0, w1=bf16(w1), b1=bf16(b1), w2=bf16(w2), b2=bf16(b2), act1=1, act2=0)
+    r = graphs.ln_linear2(m, BF16)
+    assert np.array_equal(r["xn64"], xn.astype(np.float64))
+    assert np.array_equal(r["h64"], h.astype(np.float64)) and np.array_equal(r["y64"], y.astype(np.float64))
+    m2 = dict(m, x=bf16(3 * x + 5))                        # {-1, 1} -> {2, 8}: same normalised rows
+    r2 = graphs.ln_linear2(m2, BF16)
+    assert np.allclose(r2["y64"], y, rtol=0, atol=1e-9)
+    # general rows, eps > 0: literal formula in numpy
+    xg = wl.tensor_normal(12, 1, (5, K), 1.5, 2.0, BF16)
+    m3 = dict(m, x=xg, eps=1e-5, act1=2)
+    xd = wl.f32_from_bf16_bits(xg).astype(np.float64)
+    mu = xd.mean(1, keepdims=True); v = ((xd - mu) ** 2).mean(1, keepdims=True)
+    xn3 = (xd - mu) / np.sqrt(v + np.float64(np.float32(1e-5))) * g + be
+    h3 = np.tanh(xn3 @ w1.T + b1)
+    r3 = graphs.ln_linear2(m3, BF16)
+    assert np.allclose(r3["h64"], h3, rtol=1e-12, atol=1e-13)
+    # the fused op skips exactly one rounding of the unfused graph (Q3 vs Q25): results agree to bf16 resolution
+    t = graphs.recsys_tower(dict(x=xg, gamma=m["gamma"], beta=m["beta"], eps=1e-5, w1=m["w1"], b1=m["b1"], w2=m["w2"], b2=m["b2"]), BF16)
+    r4 = graphs.ln_linear2(dict(m3, act1=1), BF16)
+    assert np.abs(r4["y64"] - t["out64"]).max() <= 2.0 ** -6 * np.abs(t["out64"]).max()
+
+
 # --------------------------------- Table-1 pointwise patterns (SURVEY 8(f) rank 2) --
 def test_pointwise_ext_hand_values_and_special_values():
     """batch_clamp / batch_nan_to_num / batch_aten_sub,div,mul against hand-computed values (torch semantics)."""
