@@ -742,7 +742,19 @@ def run_product(args):
                     torch.cuda.synchronize()
                     ts.append(c0.elapsed_time(c1) * 1e3)
                 return float(np.mean(ts))
+            # the whole tower in ONE launch: LayerNorm folded into the chain (opt_ln_linear2, reading Q25)
+            out3 = torch.empty_like(ref_out)
+            p3 = ob.opt_ln_linear2_plan_create(
+                [ob.ln_linear2_member(T(i["x"]), T(i["gamma"]), T(i["beta"]), t["eps"], T(i["w1"]), T(i["b1"]), T(i["w2"]), T(i["b2"]),
+                                      out3[:, k * t["out"]:(k + 1) * t["out"]], ACT_RELU, ACT_NONE)
+                 for k, (i, t) in enumerate(zip(ga.idx, ga.cfg["towers"]))], BF16, step.dev_index)
+            ga.plan.launch(); gb.plan.launch(); gc.plan.launch(); p3.launch()
+            torch.cuda.synchronize()
+            d3 = (out3.float() - ref_out.float())
+            rel3 = float((d3.norm(dim=1) / ref_out.float().norm(dim=1).clamp_min(1e-30)).max())
+            del d3
             t1 = cold(p2.launch)
+            t5 = cold(p3.launch)
             t2 = cold(lambda: (gb.plan.launch(), gc.plan.launch()))
             t3 = cold(lambda: (ga.plan.launch(), p2.launch()))                       # whole C4 block: LN + chained Linear
             t4 = cold(lambda: (ga.plan.launch(), gb.plan.launch(), gc.plan.launch()))  # whole C4 block: three groups
@@ -750,11 +762,14 @@ def run_product(args):
             vertical = dict(workload="C4 towers: Linear(D->H)+ReLU -> Linear(H->64), 512 members, B=8192", launches=1,
                             linear2_us=round(t1, 1), two_launch_us=round(t2, 1), speedup=round(t2 / t1, 3),
                             c4_block_ln_plus_linear2_us=round(t3, 1), c4_block_three_groups_us=round(t4, 1),
+                            c4_block_one_launch_us=round(t5, 1), c4_block_one_launch_speedup=round(t4 / t5, 3),
+                            c4_block_one_launch_bytes=p3.info()["bytes"],
+                            c4_block_one_launch_row_l2_vs_three_groups=round(rel3, 5),
                             bitwise_equal_to_two_launch=same, flops=i2["flops"], algorithmic_bytes=i2["bytes"],
                             tflops=round(i2["flops"] / t1 / 1e6, 1),
                             frac_tensor=round(i2["flops"] / t1 / 1e6 / peaks["bf16_tflops"], 4),
                             hbm_bytes_saved=int(gb.info["bytes"] + gc.info["bytes"] - i2["bytes"]))
-            del flush, out2
+            del flush, out2, out3
         except Exception as e:  # noqa: BLE001
             vertical = dict(error=repr(e))
 

@@ -144,6 +144,26 @@ typedef struct {
   int32_t act1, act2; /* opt_act */
 } opt_linear2_member;
 
+/* One member of a grouped LayerNorm + CHAINED Linear (SURVEY 8(f) rank 1 with the
+ * LayerNorm folded in; the tower of BASELINE.json configs[4]: Fig. 5):
+ *     xn = layer_norm(x; gamma, beta, eps) over K   (never materialised, NOT rounded)
+ *     h  = act1(xn * W1^T + b1)                      rounded once to bf16
+ *     Y  = act2(h * W2^T + b2)                       rounded once to bf16
+ * chain.x is the LayerNorm's INPUT [M,K]; every other field of `chain`, the
+ * limits and the alignment rules are those of opt_linear2_member.  gamma / beta:
+ * [K] bf16 or NULL (1 / 0).  Computed as rstd_r * (x * (W1 diag(gamma))^T - mu_r * s) + c
+ * with W1 diag(gamma) rounded to bf16, s_n = sum_k of it, c_n = sum_k beta_k W1[n,k] +
+ * b1_n in fp32, refolded from the CURRENT W1 / gamma / beta / b1 inside every
+ * launch (plan-owned workspace); row statistics in fp32.  Differs from the
+ * three-group path (LayerNorm output stored in bf16) by that one rounding.    */
+typedef struct {
+  opt_linear2_member chain;
+  const void* gamma;
+  const void* beta;
+  float eps;
+  int32_t reserved; /* 0 */
+} opt_ln_linear2_member;
+
 /* One member of a batched LayerNorm -- batch_layernorm:
  *     mu = mean(x_r), v = mean((x_r - mu)^2)  (biased), over the last dim D
  *     y_r = (x_r - mu) / sqrt(v + eps) * gamma + beta
@@ -222,6 +242,8 @@ opt_status opt_linear_plan_create(const opt_linear_member* members, int32_t n, o
                                   int device, opt_plan** plan);
 opt_status opt_linear2_plan_create(const opt_linear2_member* members, int32_t n, opt_dtype io,
                                    int device, opt_plan** plan);
+opt_status opt_ln_linear2_plan_create(const opt_ln_linear2_member* members, int32_t n, opt_dtype io,
+                                      int device, opt_plan** plan);
 opt_status opt_layernorm_plan_create(const opt_layernorm_member* members, int32_t n, opt_dtype io,
                                      opt_dtype param, int device, opt_plan** plan);
 opt_status opt_layernorm_bwd_plan_create(const opt_layernorm_bwd_member* members, int32_t n, opt_dtype io,

@@ -29,6 +29,11 @@ class opt_linear2_member(C.Structure):
                 ("act1", C.c_int32), ("act2", C.c_int32)]
 
 
+class opt_ln_linear2_member(C.Structure):
+    _fields_ = [("chain", opt_linear2_member), ("gamma", C.c_void_p), ("beta", C.c_void_p), ("eps", C.c_float),
+                ("reserved", C.c_int32)]
+
+
 class opt_layernorm_member(C.Structure):
     _fields_ = [("x", C.c_void_p), ("ldx", C.c_int64), ("y", C.c_void_p), ("ldy", C.c_int64),
                 ("gamma", C.c_void_p), ("beta", C.c_void_p),
@@ -79,6 +84,7 @@ def lib():
         pp = C.POINTER(C.c_void_p)
         L.opt_linear_plan_create.argtypes = [C.POINTER(opt_linear_member), C.c_int32, C.c_int, C.c_int, pp]
         L.opt_linear2_plan_create.argtypes = [C.POINTER(opt_linear2_member), C.c_int32, C.c_int, C.c_int, pp]
+        L.opt_ln_linear2_plan_create.argtypes = [C.POINTER(opt_ln_linear2_member), C.c_int32, C.c_int, C.c_int, pp]
         L.opt_layernorm_plan_create.argtypes = [C.POINTER(opt_layernorm_member), C.c_int32, C.c_int, C.c_int,
                                                 C.c_int, pp]
         L.opt_layernorm_bwd_plan_create.argtypes = [C.POINTER(opt_layernorm_bwd_member), C.c_int32, C.c_int, C.c_int,
@@ -92,7 +98,7 @@ def lib():
         L.opt_last_error.restype = C.c_char_p
         L.opt_launch_count.restype = C.c_uint64
         L.opt_version.restype = C.c_char_p
-        for f in (L.opt_linear_plan_create, L.opt_linear2_plan_create, L.opt_layernorm_plan_create, L.opt_layernorm_bwd_plan_create, L.opt_pointwise_plan_create,
+        for f in (L.opt_linear_plan_create, L.opt_linear2_plan_create, L.opt_ln_linear2_plan_create, L.opt_layernorm_plan_create, L.opt_layernorm_bwd_plan_create, L.opt_pointwise_plan_create,
                   L.opt_plan_launch, L.opt_plan_launch_host, L.opt_plan_info, L.opt_plan_destroy):
             f.restype = C.c_int
         _lib = L
@@ -161,6 +167,10 @@ def opt_linear2_plan_create(members, io, device=0):
     return _create(lib().opt_linear2_plan_create, opt_linear2_member, members, io, device)
 
 
+def opt_ln_linear2_plan_create(members, io, device=0):
+    return _create(lib().opt_ln_linear2_plan_create, opt_ln_linear2_member, members, io, device)
+
+
 def opt_layernorm_plan_create(members, io, param=None, device=0):
     return _create(lib().opt_layernorm_plan_create, opt_layernorm_member, members, io,
                    io if param is None else param, device)
@@ -226,6 +236,13 @@ def linear2_member(x, w1, b1, w2, b2, y, act1=OPT_ACT_RELU, act2=OPT_ACT_NONE):
     return opt_linear2_member(x.data_ptr(), _ld(x), w1.data_ptr(), _ld(w1), None if b1 is None else b1.data_ptr(),
                               w2.data_ptr(), _ld(w2), None if b2 is None else b2.data_ptr(), y.data_ptr(), _ld(y),
                               M, K, H, N, int(act1), int(act2))
+
+
+def ln_linear2_member(x, gamma, beta, eps, w1, b1, w2, b2, y, act1=OPT_ACT_RELU, act2=OPT_ACT_NONE):
+    assert gamma is None or tuple(gamma.shape) == (x.shape[1],)
+    assert beta is None or tuple(beta.shape) == (x.shape[1],)
+    return opt_ln_linear2_member(linear2_member(x, w1, b1, w2, b2, y, act1, act2), None if gamma is None else gamma.data_ptr(),
+                                 None if beta is None else beta.data_ptr(), float(eps), 0)
 
 
 def layernorm_member(x, y, gamma, beta, eps):

@@ -51,7 +51,7 @@ struct Region {
 opt_status check_independent(std::vector<Region>& regions, bool allow_inplace_self);
 
 // ---------------------------------------------------------------- the plan --
-enum PlanKind { kPlanPointwise = 1, kPlanLayerNorm = 2, kPlanLinearBf16 = 3, kPlanLinearF32 = 4, kPlanLinear2 = 5, kPlanLayerNormBwd = 6 };
+enum PlanKind { kPlanPointwise = 1, kPlanLayerNorm = 2, kPlanLinearBf16 = 3, kPlanLinearF32 = 4, kPlanLinear2 = 5, kPlanLayerNormBwd = 6, kPlanLnLinear2 = 7 };
 
 }  // namespace optb
 
@@ -62,7 +62,7 @@ struct opt_plan {
   void* workspace = nullptr;    // optional scratch owned by the plan (LayerNorm backward: per-block partial sums)
   size_t table_bytes = 0;
   // offsets of sub-tables inside dev_tables (meaning depends on kind)
-  size_t off0 = 0, off1 = 0, off2 = 0;
+  size_t off0 = 0, off1 = 0, off2 = 0, off3 = 0;
   dim3 grid{1, 1, 1}, block{1, 1, 1};
   size_t smem = 0;
   int32_t n_members = 0;

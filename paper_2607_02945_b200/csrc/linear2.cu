@@ -21,6 +21,21 @@
 //           directly in the K-major 128-byte-swizzled layout MMA2 reads; a tile's acc2 is drained late (after the
 //           next tile's first chunk): + b2, act2, RNE -> staging -> TMA store into the output / concat slot.
 //   TMEM: acc1 2 x 128 columns, acc2 2 x 64 columns.
+//
+// LN = true (opt_ln_linear2_plan_create): a LayerNorm over K in front of the chain, folded in algebraically so that
+// the normalised tensor never exists (reading Q25):
+//     xn W1^T + b1 = rstd_r * (x W1g^T - mu_r * s + sigma_r * c),   W1g = W1 diag(gamma) (bf16), s_n = sum_k W1g[n,k],
+//                                                 c_n = sum_k beta_k W1[n,k] + b1_n,  sigma_r = 1 / rstd_r
+//   and the two rank-1 terms ride on the tensor core as ONE extra K=16 MMA step per hidden chunk: an augmented
+//   A k-slice [-mu_h, -mu_h, -mu_l, sigma_h, sigma_h, sigma_l, 0...] per row against an augmented B k-slice
+//   [s_h, s_l, s_h, c_h, c_l, c_h, 0...] per hidden unit (hi / lo bf16 splits: products exact in fp32, the dropped
+//   lo x lo term is 2^-16 relative).  So:
+//   * prologue: every CTA folds a share of the members (W1g and the augmented slice into the plan's workspace) and
+//     publishes a per-member epoch flag; the scheduler warp waits for a member's flag before it queues one of its
+//     tiles (no grid-wide barrier: a CTA only ever waits for a prologue, and prologues wait for nothing);
+//   * the raw X tile feeds MMA1 with W1g; four extra warps compute mu_r, sigma_r of the 128 rows from the same
+//     shared-memory tile WHILE the MMAs run (shifted single pass, fp32) and write the augmented A slice;
+//   * epilogue 1 is h = act1(rstd_r * acc): no per-column operand at all.
 #include <algorithm>
 #include <cstdlib>
 
@@ -38,11 +53,11 @@ constexpr int kT_W1Stages = 4;
 constexpr int kT_EpiWarps = 8;
 constexpr int kT_FirstEpiWarp = 3;
 constexpr int kT_Mma2Warp = kT_FirstEpiWarp + kT_EpiWarps;     // warp 11: layer-2 MMA issuer
-constexpr int kT_Threads = 32 * (kT_Mma2Warp + 1);
+constexpr int kT_StatWarp0 = kT_Mma2Warp + 1;                  // LN: warps 12..15 row statistics
+constexpr int kT_StatWarps = 4;
 constexpr int kT_KBlockBytes = kT_BM * kT_BK * 2;          // 16 KB: a 128 x 64 bf16 k-block
 constexpr int kT_W2KBlockBytes = kT_MaxN * kT_BK * 2;      // 8 KB: a 64 x 64 k-block of W2
 constexpr int kT_QDepth = 4;
-constexpr int kT_QSlotBytes = kT_MaxH * 2 + kT_MaxN * 2 + 32;     // b1 | b2 | TileEntry2
 // shared-memory map
 constexpr int kT_OffX = 0;
 constexpr int kT_OffW1 = kT_OffX + (kT_MaxK / kT_BK) * kT_KBlockBytes;            //  64 KB
@@ -50,9 +65,21 @@ constexpr int kT_OffH = kT_OffW1 + kT_W1Stages * kT_KBlockBytes;                
 constexpr int kT_OffW2 = kT_OffH + 2 * kT_KBlockBytes;                            // +32 KB (one hidden tile: 2 k-blocks)
 constexpr int kT_OffOut = kT_OffW2 + 2 * 2 * kT_W2KBlockBytes;                    // +32 KB
 constexpr int kT_OffQ = kT_OffOut + 4 * 4096;                                     // +16 KB output staging (4 warps x 32 rows x 128 B)
-constexpr int kT_OffBar = kT_OffQ + kT_QDepth * kT_QSlotBytes;
-constexpr int kT_SmemBytes = kT_OffBar + 512;
-static_assert(kT_SmemBytes <= 227 * 1024, "chained-GEMM shared memory map exceeds 227 KB");
+template <bool LN>
+struct L2Cfg {
+  static constexpr int kThreads = 32 * (LN ? kT_StatWarp0 + kT_StatWarps : kT_Mma2Warp + 1);
+  // LN: the augmented A k-slice (a 128 x 64 k-block in the swizzled layout, 16 columns used) sits before the queue
+  static constexpr int kOffAug = kT_OffQ;
+  static constexpr int kOffQ = kT_OffQ + (LN ? kT_KBlockBytes : 0);
+  // queue slot:  b1 (bf16) | b2 | TileEntry2     or, LN:  b2 | TileEntry2
+  static constexpr int kOffB2 = LN ? 0 : kT_MaxH * 2;
+  static constexpr int kQEntryOff = kOffB2 + kT_MaxN * 2;
+  static constexpr int kQSlotBytes = kQEntryOff + 32;
+  static constexpr int kOffStats = kOffQ + kT_QDepth * kQSlotBytes;               // LN: 2 x 128 rows x rstd
+  static constexpr int kOffBar = kOffStats + (LN ? 2 * kT_BM * 4 : 0);
+  static constexpr int kSmemBytes = kOffBar + 384;
+  static_assert(kSmemBytes <= 227 * 1024, "chained-GEMM shared memory map exceeds 227 KB");
+};
 constexpr int kT_TmemCols = 512;      // acc1: columns [0,256), acc2: [256,384)
 
 struct alignas(128) L2Member {
@@ -60,8 +87,9 @@ struct alignas(128) L2Member {
   CUtensorMap tmW1;      // W1 [H,K]   box {64, 128}  load
   CUtensorMap tmW2;      // W2 [N,H]   box {64, N}    load
   CUtensorMap tmY;       // Y  [M,N]   box {64, 32}   store
+  CUtensorMap tmAug;     // LN: augmented B slice [H,16], box {64, 128} (columns 16.. zero-filled)  load
 };
-static_assert(sizeof(L2Member) == 512, "L2Member keeps tensor maps 128-byte aligned");
+static_assert(sizeof(L2Member) == 640, "L2Member keeps tensor maps 128-byte aligned");
 
 struct alignas(16) TileEntry2 {       // member < 0: padding entry of a chunk
   int32_t member, m0;
@@ -71,6 +99,16 @@ struct alignas(16) TileEntry2 {       // member < 0: padding entry of a chunk
   const void* b2;        // [N] bf16 or NULL
 };
 static_assert(sizeof(TileEntry2) == 32, "TileEntry2 is two 16-byte vectors");
+
+struct alignas(16) L2Fold {            // LN: what the prologue needs to fold one member's LayerNorm affine into W1
+  const uint16_t* w1; int64_t ldw1;
+  const uint16_t* gamma; const uint16_t* beta; const uint16_t* b1;
+  uint16_t* w1g;         // [H,K] dense bf16 (workspace)
+  uint16_t* aug;         // [H,16] bf16: s_h, s_l, s_h, c_h, c_l, c_h, 0 ... (workspace)
+  int32_t H, K;
+  float eps; int32_t pad;
+};
+static_assert(sizeof(L2Fold) == 80, "L2Fold layout");
 
 __device__ __forceinline__ uint32_t l2_idesc(int n) {   // kind::f16, bf16 x bf16 -> fp32, M = 128, K-major A and B
   return (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(n >> 3) << 17) | ((uint32_t)(kT_BM >> 4) << 24);
@@ -85,9 +123,112 @@ __device__ __forceinline__ void epi_act(const uint32_t (&v)[64], uint32_t bias_a
   }
 }
 
-__global__ void __launch_bounds__(kT_Threads, 1)
+// LN kernel: 14 warps put four warps on every SM sub-partition, i.e. at most 128 registers per thread, so its
+// epilogue works on 32 accumulator columns at a time.
+// Layer 1: h = act(rstd_r * acc) (this thread's row; the per-column terms were added by the tensor core).
+template <int ACT>
+__device__ __forceinline__ void epi_math_ln32(const uint32_t (&v)[32], float A, uint32_t (&p)[16]) {
+#pragma unroll
+  for (int j = 0; j < 16; ++j) {
+    const float f0 = A * __uint_as_float(v[2 * j]), f1 = A * __uint_as_float(v[2 * j + 1]);
+    if (ACT == OPT_ACT_RELU) p[j] = pack_relu_bf16x2(f0, f1);
+    else p[j] = pack_bf16x2(act_f32<true>(f0, ACT), act_f32<true>(f1, ACT));
+  }
+}
+__device__ __forceinline__ void epi_act_ln32(const uint32_t (&v)[32], float A, int act, uint32_t (&p)[16]) {
+  switch (act) {
+    case OPT_ACT_RELU: epi_math_ln32<OPT_ACT_RELU>(v, A, p); break;
+    case OPT_ACT_NONE: epi_math_ln32<OPT_ACT_NONE>(v, A, p); break;
+    case OPT_ACT_TANH: epi_math_ln32<OPT_ACT_TANH>(v, A, p); break;
+    default:           epi_math_ln32<OPT_ACT_SIGMOID>(v, A, p); break;
+  }
+}
+// Layer 2, 32 columns: + bias (bf16 in the queue slot), activation, RNE.
+template <int ACT>
+__device__ __forceinline__ void epi_math32(const uint32_t (&v)[32], uint32_t bias_addr, uint32_t (&p)[16]) {
+#pragma unroll
+  for (int j = 0; j < 4; ++j) {          // 8 columns per step
+    const uint4 b = lds128(bias_addr + 16 * j);
+    const uint32_t bw[4] = {b.x, b.y, b.z, b.w};
+#pragma unroll
+    for (int t = 0; t < 4; ++t) {
+      const float lo = __uint_as_float(v[8 * j + 2 * t]) + bf16_lo(bw[t]);
+      const float hi = __uint_as_float(v[8 * j + 2 * t + 1]) + bf16_hi(bw[t]);
+      if (ACT == OPT_ACT_RELU) p[4 * j + t] = pack_relu_bf16x2(lo, hi);
+      else p[4 * j + t] = pack_bf16x2(act_f32<true>(lo, ACT), act_f32<true>(hi, ACT));
+    }
+  }
+}
+__device__ __forceinline__ void epi_act32(const uint32_t (&v)[32], uint32_t bias_addr, int act, uint32_t (&p)[16]) {
+  switch (act) {
+    case OPT_ACT_RELU: epi_math32<OPT_ACT_RELU>(v, bias_addr, p); break;
+    case OPT_ACT_NONE: epi_math32<OPT_ACT_NONE>(v, bias_addr, p); break;
+    case OPT_ACT_TANH: epi_math32<OPT_ACT_TANH>(v, bias_addr, p); break;
+    default:           epi_math32<OPT_ACT_SIGMOID>(v, bias_addr, p); break;
+  }
+}
+
+// LN prologue: fold one member.  A row n of W1 is handled by LP = pow2 >= K/8 lanes (one 16-byte vector each):
+//   W1g[n,k] = bf16(W1[n,k] * gamma_k);  s_n = sum_k W1g[n,k];  c_n = sum_k beta_k W1[n,k] + b1_n   (fp32, fixed order)
+//   aug[n, 0..5] = s_h, s_l, s_h, c_h, c_l, c_h  (v_h = bf16(v), v_l = bf16(v - v_h)), aug[n, 6..15] = 0
+__device__ __forceinline__ void l2_fold_member(const L2Fold& f, int warp, int nwarps, int lane) {
+  const int nv = f.K >> 3;
+  int LP = 1;
+  while (LP < nv) LP <<= 1;
+  const int rows_per_pass = 32 / LP, sub = lane / LP, j = lane % LP;
+  uint4 g = make_uint4(0x3F803F80u, 0x3F803F80u, 0x3F803F80u, 0x3F803F80u), be = make_uint4(0, 0, 0, 0);   // gamma = 1, beta = 0
+  if (j < nv) {
+    if (f.gamma) g = __ldg(reinterpret_cast<const uint4*>(f.gamma) + j);
+    if (f.beta) be = __ldg(reinterpret_cast<const uint4*>(f.beta) + j);
+  }
+  const uint32_t gw[4] = {g.x, g.y, g.z, g.w}, bw[4] = {be.x, be.y, be.z, be.w};
+  constexpr int kBatch = 16;               // rows in flight per lane: the fold is latency-bound (one L2 round trip per batch)
+  const int stride = nwarps * rows_per_pass;
+  for (int nb = warp * rows_per_pass; nb < f.H; nb += kBatch * stride) {
+    uint4 w[kBatch];
+#pragma unroll
+    for (int b = 0; b < kBatch; ++b) {
+      const int n = nb + b * stride + sub;
+      w[b] = make_uint4(0, 0, 0, 0);
+      if (n < f.H && j < nv) w[b] = __ldg(reinterpret_cast<const uint4*>(f.w1 + (int64_t)n * f.ldw1) + j);
+    }
+#pragma unroll
+    for (int b = 0; b < kBatch; ++b) {
+      const int n = nb + b * stride + sub;
+      if (nb + b * stride >= f.H) break;                   // warp-uniform
+      float ssum = 0.f, csum = 0.f;
+      const uint32_t ww[4] = {w[b].x, w[b].y, w[b].z, w[b].w};
+      uint32_t o[4];
+#pragma unroll
+      for (int t = 0; t < 4; ++t) {
+        o[t] = pack_bf16x2(bf16_lo(ww[t]) * bf16_lo(gw[t]), bf16_hi(ww[t]) * bf16_hi(gw[t]));
+        ssum += bf16_lo(o[t]) + bf16_hi(o[t]);
+        csum = fmaf(bf16_lo(ww[t]), bf16_lo(bw[t]), fmaf(bf16_hi(ww[t]), bf16_hi(bw[t]), csum));
+      }
+      if (n < f.H && j < nv) *(reinterpret_cast<uint4*>(f.w1g + (int64_t)n * f.K) + j) = make_uint4(o[0], o[1], o[2], o[3]);
+      for (int d = LP >> 1; d >= 1; d >>= 1) {
+        ssum += __shfl_xor_sync(0xffffffffu, ssum, d);
+        csum += __shfl_xor_sync(0xffffffffu, csum, d);
+      }
+      if (n < f.H && j == 0) {
+        if (f.b1) csum += __uint_as_float((uint32_t)__ldg(f.b1 + n) << 16);
+        const uint32_t s2 = pack_bf16x2(ssum, 0.f), c2 = pack_bf16x2(csum, 0.f);                 // hi parts (low halves)
+        const uint32_t sl = pack_bf16x2(ssum - bf16_lo(s2), 0.f), cl = pack_bf16x2(csum - bf16_lo(c2), 0.f);
+        uint4* a = reinterpret_cast<uint4*>(f.aug + (int64_t)n * 16);
+        a[0] = make_uint4((s2 & 0xFFFFu) | (sl << 16), (s2 & 0xFFFFu) | (c2 << 16), (cl & 0xFFFFu) | (c2 << 16), 0u);
+        a[1] = make_uint4(0u, 0u, 0u, 0u);
+      }
+    }
+  }
+}
+
+template <bool LN>
+__global__ void __launch_bounds__(L2Cfg<LN>::kThreads, 1)
 grouped_linear2_sm100_kernel(const L2Member* __restrict__ members, const uint4* __restrict__ chunks, int n_chunks,
-                             int* __restrict__ counters) {
+                             int* __restrict__ counters, const L2Fold* __restrict__ folds, int* __restrict__ flags,
+                             int n_members) {
+  using Cfg = L2Cfg<LN>;
+  constexpr int kT_QSlotBytes = Cfg::kQSlotBytes, kT_OffBar = Cfg::kOffBar;
   extern __shared__ __align__(1024) uint8_t smem[];
   const uint32_t sbase = smem_u32(smem);
   if ((sbase & 1023u) != 0) __trap();            // 128-byte-swizzle tiles need 1024-byte alignment
@@ -108,14 +249,18 @@ grouped_linear2_sm100_kernel(const L2Member* __restrict__ members, const uint4* 
   auto q_full = [&](int s) { return bar_base + kB2 + 128u + 8u * s; };
   auto q_empty = [&](int s) { return bar_base + kB2 + 128u + 8u * (kT_QDepth + s); };
   const uint32_t tmem_ptr_addr = bar_base + kB2 + 128u + 16u * kT_QDepth;
-  static_assert(16 + 16 * kT_W1Stages + 128 + 16 * kT_QDepth + 4 <= 512, "barrier area");
-  auto q_slot = [&](int s) { return sbase + kT_OffQ + (uint32_t)s * kT_QSlotBytes; };
-  constexpr uint32_t kQEntryOff = kT_MaxH * 2 + kT_MaxN * 2;
+  auto st_full = [&](int s) { return tmem_ptr_addr + 8u + 8u * s; };           // LN: row statistics of a tile
+  auto st_empty = [&](int s) { return tmem_ptr_addr + 24u + 8u * s; };
+  static_assert(16 + 16 * kT_W1Stages + 128 + 16 * kT_QDepth + 8 + 32 <= 384, "barrier area");
+  auto q_slot = [&](int s) { return sbase + Cfg::kOffQ + (uint32_t)s * kT_QSlotBytes; };
+  constexpr uint32_t kQEntryOff = Cfg::kQEntryOff, kOffB2 = Cfg::kOffB2;
+  const uint32_t stats_base = sbase + Cfg::kOffStats, aug_base = sbase + Cfg::kOffAug;
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
 
   if (warp == 0 && lane == 0) {
-    mbar_init(xa_full, 1); mbar_init(xa_empty, 1);
+    mbar_init(xa_full, 1); mbar_init(xa_empty, LN ? 1 + kT_StatWarps : 1);      // LN: the statistics warps read the X tile too
+    if (LN) for (int s = 0; s < 2; ++s) { mbar_init(st_full(s), kT_StatWarps); mbar_init(st_empty(s), kT_EpiWarps); }
     for (int s = 0; s < kT_W1Stages; ++s) { mbar_init(w1_full(s), 1); mbar_init(w1_empty(s), 1); }
     for (int s = 0; s < 2; ++s) {
       mbar_init(w2_full(s), 1); mbar_init(w2_empty(s), 1);
@@ -123,7 +268,7 @@ grouped_linear2_sm100_kernel(const L2Member* __restrict__ members, const uint4* 
       mbar_init(h_full(s), kT_EpiWarps); mbar_init(h_empty(s), 1);
       mbar_init(a2_full(s), 1); mbar_init(a2_empty(s), kT_EpiWarps);
     }
-    for (int s = 0; s < kT_QDepth; ++s) { mbar_init(q_full(s), 1); mbar_init(q_empty(s), 3 + kT_EpiWarps); }
+    for (int s = 0; s < kT_QDepth; ++s) { mbar_init(q_full(s), 1); mbar_init(q_empty(s), 3 + kT_EpiWarps + (LN ? kT_StatWarps : 0)); }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     fence_proxy_async_smem();
   }
@@ -137,6 +282,21 @@ grouped_linear2_sm100_kernel(const L2Member* __restrict__ members, const uint4* 
   tc_fence_after();
   uint32_t tmem_base;
   asm volatile("ld.shared.b32 %0, [%1];" : "=r"(tmem_base) : "r"(tmem_ptr_addr) : "memory");
+
+  int epoch1 = 0;                                  // LN: value a member's flag carries once folded in THIS launch
+  if (LN) {
+    epoch1 = *reinterpret_cast<volatile int*>(counters + 2) + 1;
+    for (int i = blockIdx.x; i < n_members; i += gridDim.x) {
+      const L2Fold f = folds[i];
+      l2_fold_member(f, warp, Cfg::kThreads / 32, lane);
+    }
+    asm volatile("fence.proxy.async;" ::: "memory");       // W1g is read back through TMA (async proxy)
+    __threadfence();
+    __syncthreads();
+    if (threadIdx.x == 0)
+      for (int i = blockIdx.x; i < n_members; i += gridDim.x)
+        asm volatile("st.release.gpu.global.s32 [%0], %1;" ::"l"(flags + i), "r"(epoch1) : "memory");
+  }
 
   if (warp == 2) {
     // ----------------------------------------------------- tile scheduler ----
@@ -159,10 +319,19 @@ grouped_linear2_sm100_kernel(const L2Member* __restrict__ members, const uint4* 
         const int H = (int)(shape & 0xFFFFu), N = (int)(misc >> 16);
         b1a = b1b = b2v = make_uint4(0, 0, 0, 0);
         if (member >= 0) {
-          if (b1 != nullptr && 8 * lane < H) b1a = __ldg(b1 + lane);
-          if (b1 != nullptr && 8 * (lane + 32) < H) b1b = __ldg(b1 + lane + 32);
+          if (LN) {
+            // the member's folded weights / s / c come from some CTA's prologue of THIS launch: wait for its flag
+            if (lane == 0) {
+              int f;
+              do { asm volatile("ld.acquire.gpu.global.s32 %0, [%1];" : "=r"(f) : "l"(flags + member) : "memory"); } while (f != epoch1);
+            }
+            __syncwarp();
+          } else {
+            if (b1 != nullptr && 8 * lane < H) b1a = __ldg(b1 + lane);
+            if (b1 != nullptr && 8 * (lane + 32) < H) b1b = __ldg(b1 + lane + 32);
+          }
           if (b2 != nullptr && 8 * lane < N) b2v = __ldg(b2 + lane);
-          if (lane < 4)
+          if (lane < (LN ? 5 : 4))
             asm volatile("prefetch.tensormap [%0];" ::"l"(reinterpret_cast<const char*>(members + member) + 128 * lane) : "memory");
           // the tile's X k-blocks -> L2 now: the X buffer is single (64 KB), its load can only be issued when the
           // previous tile's last MMA1 has retired, and should then find the data in L2 rather than in HBM
@@ -182,9 +351,11 @@ grouped_linear2_sm100_kernel(const L2Member* __restrict__ members, const uint4* 
         if (cur < 0) continue;             // warp-uniform
         mbar_wait(q_empty(qs), qph ^ 1);
         const uint32_t slot = q_slot(qs);
-        sts128(slot + 16 * lane, c1a);
-        sts128(slot + 512 + 16 * lane, c1b);
-        if (lane < kT_MaxN / 8) sts128(slot + kT_MaxH * 2 + 16 * lane, c2);
+        if (!LN) {
+          sts128(slot + 16 * lane, c1a);
+          sts128(slot + 512 + 16 * lane, c1b);
+        }
+        if (lane < kT_MaxN / 8) sts128(slot + kOffB2 + 16 * lane, c2);
         if ((lane >> 1) == g) sts128(slot + kQEntryOff + 16 * (lane & 1), e);
         __syncwarp();
         if (lane == 0) mbar_arrive(q_full(qs));
@@ -197,7 +368,11 @@ grouped_linear2_sm100_kernel(const L2Member* __restrict__ members, const uint4* 
       sts128(q_slot(qs) + kQEntryOff, make_uint4(0xFFFFFFFFu, 0, 0, 0));
       mbar_arrive(q_full(qs));
       __threadfence();
-      if (atomicAdd(counters + 1, 1) == (int)gridDim.x - 1) { counters[0] = 0; counters[1] = 0; __threadfence(); }
+      if (atomicAdd(counters + 1, 1) == (int)gridDim.x - 1) {
+        counters[0] = 0; counters[1] = 0;
+        if (LN) counters[2] = epoch1;      // the next launch's flags carry the next epoch
+        __threadfence();
+      }
     }
   } else if (warp == 0) {
     // ------------------------------------------------------- TMA producer ----
@@ -218,6 +393,7 @@ grouped_linear2_sm100_kernel(const L2Member* __restrict__ members, const uint4* 
         const int H = (int)(e0.z & 0xFFFFu), nkb1 = (int)((e0.z >> 16) & 0xFFu);
         const int N = (int)(e0.w >> 16);
         const int nch = (H + kT_HC - 1) / kT_HC;
+        if (LN) asm volatile("fence.proxy.async;" ::: "memory");   // W1g: generic-proxy writes of this launch -> TMA reads
         // X tile: resident for the whole tile, reloaded when the last MMA1 of the previous tile has retired
         mbar_wait(xa_empty, (gt & 1u) ^ 1u);
         mbar_expect_tx(xa_full, (uint32_t)nkb1 * kT_KBlockBytes);
@@ -237,6 +413,12 @@ grouped_linear2_sm100_kernel(const L2Member* __restrict__ members, const uint4* 
             mbar_wait(w1_empty(w1s), w1ph ^ 1);
             mbar_expect_tx(w1_full(w1s), kT_KBlockBytes);
             tma_load_2d(sbase + kT_OffW1 + w1s * kT_KBlockBytes, &m->tmW1, w1_full(w1s), kb * kT_BK, c * kT_HC);
+            if (++w1s == kT_W1Stages) { w1s = 0; w1ph ^= 1; }
+          }
+          if (LN) {                                    // the chunk's augmented slice travels through the same ring
+            mbar_wait(w1_empty(w1s), w1ph ^ 1);
+            mbar_expect_tx(w1_full(w1s), kT_KBlockBytes);
+            tma_load_2d(sbase + kT_OffW1 + w1s * kT_KBlockBytes, &m->tmAug, w1_full(w1s), 0, c * kT_HC);
             if (++w1s == kT_W1Stages) { w1s = 0; w1ph ^= 1; }
           }
           if (c >= 1) load_w2(c - 1, gh + c - 1);
@@ -285,6 +467,14 @@ grouped_linear2_sm100_kernel(const L2Member* __restrict__ members, const uint4* 
             tc_commit(w1_empty(w1s));
             if (++w1s == kT_W1Stages) { w1s = 0; w1ph ^= 1; }
           }
+          if (LN) {                                          // + (-mu_r s_n + sigma_r c_n): one K=16 step
+            if (c == 0) mbar_wait(st_full(gt & 1u), (gt >> 1) & 1u);   // the statistics warps have written the A slice
+            mbar_wait(w1_full(w1s), w1ph);
+            tc_fence_after();
+            tc_mma_bf16(acc1, umma_desc_sw128(aug_base), wd0 + (uint64_t)w1s * kKB, idesc1, 1);
+            tc_commit(w1_empty(w1s));
+            if (++w1s == kT_W1Stages) { w1s = 0; w1ph ^= 1; }
+          }
           tc_commit(a1_full(s));
           if (c == nch - 1) tc_commit(xa_empty);             // the X tile may be replaced
         }
@@ -328,6 +518,57 @@ grouped_linear2_sm100_kernel(const L2Member* __restrict__ members, const uint4* 
         ++gt;
       }
     }
+  } else if (LN && warp >= kT_StatWarp0) {
+    // -------------------------------------------- LN: row statistics of the X tile ----
+    // Each lane owns one of the tile's 128 rows and reads it from the swizzled tile while MMA1 runs on it.
+    // Shifted single pass (shift = the row's first element): sum(x - x0), sum((x - x0)^2) in fp32.
+    const int sw = warp - kT_StatWarp0;
+    int qs = 0; uint32_t qph = 0;
+    uint32_t gt = 0;
+    for (;;) {
+      mbar_wait(q_full(qs), qph);
+      const uint4 e0 = lds128(q_slot(qs) + kQEntryOff);
+      __syncwarp();
+      if (lane == 0) mbar_arrive(q_empty(qs));
+      if (++qs == kT_QDepth) { qs = 0; qph ^= 1; }
+      if ((int)e0.x < 0) break;
+      const int K = __ldg(&folds[(int)e0.x].K);
+      const float eps = __ldg(&folds[(int)e0.x].eps);
+      const uint32_t ss = gt & 1u;
+      mbar_wait(st_empty(ss), ((gt >> 1) & 1u) ^ 1u);
+      mbar_wait(xa_full, gt & 1u);
+      const int r0 = sw * 32 + lane;
+      const uint32_t a0 = sbase + kT_OffX + (uint32_t)r0 * 128u;
+      const uint32_t x7 = (uint32_t)(lane & 7);                   // r0 & 7
+      const float s0 = bf16_lo(lds128(a0 + (x7 << 4)).x);         // logical chunk 0, element 0: the shift
+      const f32x2 ns = pk2(-s0, -s0);
+      f32x2 sumA = pk2(0.f, 0.f), sumB = sumA, sqA = sumA, sqB = sumA;
+      const int nv = K >> 3;
+#pragma unroll 4
+      for (int c = 0; c < nv; ++c) {
+        const uint4 u = lds128(a0 + (uint32_t)(c >> 3) * kT_KBlockBytes + ((((uint32_t)c & 7u) ^ x7) << 4));
+        const f32x2 d0 = add2(bf2_to_f2(u.x), ns), d1 = add2(bf2_to_f2(u.y), ns);
+        const f32x2 d2 = add2(bf2_to_f2(u.z), ns), d3 = add2(bf2_to_f2(u.w), ns);
+        sumA = add2(sumA, d0); sqA = fma2(d0, d0, sqA);
+        sumB = add2(sumB, d1); sqB = fma2(d1, d1, sqB);
+        sumA = add2(sumA, d2); sqA = fma2(d2, d2, sqA);
+        sumB = add2(sumB, d3); sqB = fma2(d3, d3, sqB);
+      }
+      const float inv = 1.f / (float)K;
+      const float m0 = sum2(add2(sumA, sumB)) * inv;
+      const float sig = sqrtf(fmaxf(fmaf(-m0, m0, sum2(add2(sqA, sqB)) * inv), 0.f) + eps), nmu = -(s0 + m0);
+      // augmented A slice of this row: -mu_h, -mu_h, -mu_l, sigma_h, sigma_h, sigma_l, 0, 0 | 0 x 8
+      const uint32_t mh = pack_bf16x2(nmu, 0.f) & 0xFFFFu, gh2 = pack_bf16x2(sig, 0.f) & 0xFFFFu;
+      const uint32_t ml = pack_bf16x2(nmu - bf16_lo(mh), 0.f) & 0xFFFFu, gl = pack_bf16x2(sig - bf16_lo(gh2), 0.f) & 0xFFFFu;
+      const uint32_t arow = aug_base + (uint32_t)r0 * 128u;
+      sts128(arow + (x7 << 4), make_uint4(mh | (mh << 16), ml | (gh2 << 16), gh2 | (gl << 16), 0u));
+      sts128(arow + ((1u ^ x7) << 4), make_uint4(0u, 0u, 0u, 0u));
+      asm volatile("st.shared.f32 [%0], %1;" ::"r"(stats_base + ss * (kT_BM * 4) + (uint32_t)r0 * 4u), "f"(1.f / sig) : "memory");
+      fence_proxy_async_smem();                      // the A slice is read by the tensor core
+      __syncwarp();
+      if (lane == 0) { mbar_arrive(st_full(ss)); mbar_arrive(xa_empty); }
+      ++gt;
+    }
   } else {
     // ----------------------------------------------------------- epilogue ----
     // Per hidden chunk: acc1 -> registers -> + b1, act1, RNE -> the hidden tile in shared memory (layer-2 A operand).
@@ -350,18 +591,33 @@ grouped_linear2_sm100_kernel(const L2Member* __restrict__ members, const uint4* 
       const uint32_t s2 = p_gt & 1u;
       mbar_wait(a2_full(s2), (p_gt >> 1) & 1u);
       tc_fence_after();
-      uint32_t v[64], p[32];
-      {
+      uint32_t p[32];
+      if constexpr (LN) {                      // 32 columns at a time; only the storing warps read the accumulator
+        uint32_t(&pa)[16] = *reinterpret_cast<uint32_t(*)[16]>(&p[0]);
+        uint32_t(&pb)[16] = *reinterpret_cast<uint32_t(*)[16]>(&p[16]);
+        if (half == 0) {
+          const uint32_t t = tmem_base + lane_off + 256u + s2 * 64u;
+          uint32_t v[32];
+          tc_ld_32x32(t, v); tc_wait_ld();
+          epi_act32(v, p_slot + kOffB2, p_act2, pa);
+          tc_ld_32x32(t + 32, v); tc_wait_ld();
+          epi_act32(v, p_slot + kOffB2 + 64, p_act2, pb);
+        }
+        tc_fence_before();
+        __syncwarp();
+        if (lane == 0) mbar_arrive(a2_empty(s2));
+      } else {
+        uint32_t v[64];
         const uint32_t t = tmem_base + lane_off + 256u + s2 * 64u;
         tc_ld_32x32(t, *reinterpret_cast<uint32_t(*)[32]>(&v[0]));
         tc_ld_32x32(t + 32, *reinterpret_cast<uint32_t(*)[32]>(&v[32]));
         tc_wait_ld();
+        tc_fence_before();
+        __syncwarp();
+        if (lane == 0) mbar_arrive(a2_empty(s2));
+        if (half == 0) epi_act(v, p_slot + kOffB2, p_act2, p);
       }
-      tc_fence_before();
-      __syncwarp();
-      if (lane == 0) mbar_arrive(a2_empty(s2));
       if (half == 0) {
-        epi_act(v, p_slot + kT_MaxH * 2, p_act2, p);
         if (lane == 0) tma_store_wait_read<0>();       // this warp's previous store has read the staging tile
         __syncwarp();
 #pragma unroll
@@ -387,6 +643,14 @@ grouped_linear2_sm100_kernel(const L2Member* __restrict__ members, const uint4* 
       const int H = (int)(e0.z & 0xFFFFu);
       const int act1 = (int)(e0.w & 0xFFu), act2 = (int)((e0.w >> 8) & 0xFFu);
       const int nch = (H + kT_HC - 1) / kT_HC;
+      float lnA = 0.f;                                // LN: rstd of this thread's row
+      if (LN) {
+        const uint32_t ss = gt & 1u;
+        mbar_wait(st_full(ss), (gt >> 1) & 1u);
+        asm volatile("ld.shared.f32 %0, [%1];" : "=f"(lnA) : "r"(stats_base + ss * (kT_BM * 4) + (uint32_t)(quad * 32 + lane) * 4u) : "memory");
+        __syncwarp();
+        if (lane == 0) mbar_arrive(st_empty(ss));
+      }
       for (int c = 0; c < nch; ++c) {
         const uint32_t g = gh + (uint32_t)c;
         const int s = (int)(g & 1u);
@@ -395,25 +659,47 @@ grouped_linear2_sm100_kernel(const L2Member* __restrict__ members, const uint4* 
         const bool mine = half * 64 < bn;            // this warp's 64 columns exist in the chunk
         mbar_wait(a1_full(s), ph);
         tc_fence_after();
-        uint32_t v[64], p[32];
-        {                                              // (columns past the chunk's width hold stale data: never used)
-          const uint32_t t = tmem_base + lane_off + (uint32_t)s * 128u + (uint32_t)half * 64u;
+        const uint32_t t = tmem_base + lane_off + (uint32_t)s * 128u + (uint32_t)half * 64u;
+        if constexpr (LN) {                            // (columns past the chunk's width hold stale data: never used)
+          uint32_t va[32], vb[32], q[16];
+          tc_ld_32x32(t, va);
+          tc_ld_32x32(t + 32, vb);
+          tc_wait_ld();
+          tc_fence_before();
+          __syncwarp();
+          if (lane == 0) mbar_arrive(a1_empty(s));
+          mbar_wait(h_empty(0), (g & 1u) ^ 1u);
+          const uint32_t hrow = sbase + kT_OffH + (uint32_t)half * kT_KBlockBytes + row_off;
+          epi_act_ln32(va, lnA, act1, q);
+          if (mine) {
+#pragma unroll
+            for (int j = 0; j < 4; ++j)
+              sts128(hrow + ((j ^ (lane & 7)) << 4), make_uint4(q[4 * j], q[4 * j + 1], q[4 * j + 2], q[4 * j + 3]));
+          }
+          epi_act_ln32(vb, lnA, act1, q);
+          if (mine) {
+#pragma unroll
+            for (int j = 0; j < 4; ++j)
+              sts128(hrow + (((j + 4) ^ (lane & 7)) << 4), make_uint4(q[4 * j], q[4 * j + 1], q[4 * j + 2], q[4 * j + 3]));
+          }
+        } else {
+          uint32_t v[64], p[32];
           tc_ld_32x32(t, *reinterpret_cast<uint32_t(*)[32]>(&v[0]));
           tc_ld_32x32(t + 32, *reinterpret_cast<uint32_t(*)[32]>(&v[32]));
           tc_wait_ld();
-        }
-        tc_fence_before();
-        __syncwarp();
-        if (lane == 0) mbar_arrive(a1_empty(s));       // acc1 stage is in registers: MMA1 of chunk c+2 may overwrite it
-        epi_act(v, slot + (uint32_t)(c * kT_HC + half * 64) * 2u, act1, p);
-        // the hidden tile is single-buffered: MMA2 of chunk c-1 has normally retired by the time this chunk's
-        // accumulator has been read and converted
-        mbar_wait(h_empty(0), (g & 1u) ^ 1u);
-        if (mine) {
-          const uint32_t hrow = sbase + kT_OffH + (uint32_t)half * kT_KBlockBytes + row_off;
+          tc_fence_before();
+          __syncwarp();
+          if (lane == 0) mbar_arrive(a1_empty(s));     // acc1 stage is in registers: MMA1 of chunk c+2 may overwrite it
+          epi_act(v, slot + (uint32_t)(c * kT_HC + half * 64) * 2u, act1, p);
+          // the hidden tile is single-buffered: MMA2 of chunk c-1 has normally retired by the time this chunk's
+          // accumulator has been read and converted
+          mbar_wait(h_empty(0), (g & 1u) ^ 1u);
+          if (mine) {
+            const uint32_t hrow = sbase + kT_OffH + (uint32_t)half * kT_KBlockBytes + row_off;
 #pragma unroll
-          for (int j = 0; j < 8; ++j)                  // K-major, 128-byte swizzle: 16-byte piece j of row r sits at j ^ (r & 7)
-            sts128(hrow + ((j ^ (lane & 7)) << 4), make_uint4(p[4 * j], p[4 * j + 1], p[4 * j + 2], p[4 * j + 3]));
+            for (int j = 0; j < 8; ++j)                // K-major, 128-byte swizzle: 16-byte piece j of row r sits at j ^ (r & 7)
+              sts128(hrow + ((j ^ (lane & 7)) << 4), make_uint4(p[4 * j], p[4 * j + 1], p[4 * j + 2], p[4 * j + 3]));
+          }
         }
         fence_proxy_async_smem();                      // generic-proxy writes -> visible to the tensor core's reads
         __syncwarp();
@@ -440,9 +726,14 @@ grouped_linear2_sm100_kernel(const L2Member* __restrict__ members, const uint4* 
 
 cudaError_t launch_linear2(const opt_plan* p, cudaStream_t s) {
   char* base = static_cast<char*>(p->dev_tables);
-  grouped_linear2_sm100_kernel<<<p->grid, p->block, p->smem, s>>>(
-      reinterpret_cast<const L2Member*>(base + p->off0), reinterpret_cast<const uint4*>(base + p->off1), p->n_chunks,
-      reinterpret_cast<int*>(base + p->off2));
+  const L2Member* mem = reinterpret_cast<const L2Member*>(base + p->off0);
+  const uint4* chunks = reinterpret_cast<const uint4*>(base + p->off1);
+  int* counters = reinterpret_cast<int*>(base + p->off2);
+  if (p->kind == kPlanLnLinear2)       // counters (256 B) | per-member flags | fold table
+    grouped_linear2_sm100_kernel<true><<<p->grid, p->block, p->smem, s>>>(
+        mem, chunks, p->n_chunks, counters, reinterpret_cast<const L2Fold*>(base + p->off3), counters + 64, p->n_members);
+  else
+    grouped_linear2_sm100_kernel<false><<<p->grid, p->block, p->smem, s>>>(mem, chunks, p->n_chunks, counters, nullptr, nullptr, 0);
   return cudaGetLastError();
 }
 
@@ -450,17 +741,21 @@ cudaError_t launch_linear2(const opt_plan* p, cudaStream_t s) {
 
 using namespace optb;
 
-extern "C" opt_status opt_linear2_plan_create(const opt_linear2_member* members, int32_t n, opt_dtype io, int device,
-                                              opt_plan** plan) {
+namespace {
+// one planner for both entry points: lnm == nullptr -> plain chain (members), else LayerNorm + chain (lnm[i].chain)
+opt_status create_linear2(const opt_linear2_member* members, const opt_ln_linear2_member* lnm, int32_t n, opt_dtype io,
+                          int device, opt_plan** plan) {
+  const bool LN = lnm != nullptr;
+  auto M_ = [&](int32_t i) -> const opt_linear2_member& { return LN ? lnm[i].chain : members[i]; };
   if (plan) *plan = nullptr;
-  if (!plan || !members) return fail(OPT_ERR_INVALID_ARG, "opt_linear2_plan_create: NULL argument");
+  if (!plan || (!members && !lnm)) return fail(OPT_ERR_INVALID_ARG, "opt_linear2_plan_create: NULL argument");
   if (n < 1 || n > 65535) return fail(OPT_ERR_INVALID_ARG, "n = %d outside [1, 65535]", n);
   if (io != OPT_F32 && io != OPT_BF16) return fail(OPT_ERR_INVALID_ARG, "bad io dtype %d", (int)io);
   if (io != OPT_BF16) return fail(OPT_ERR_UNSUPPORTED, "chained Linear is implemented for bf16 groups only");
   std::vector<Region> regions;
   int64_t flops = 0, bytes = 0, tiles = 0;
   for (int32_t i = 0; i < n; ++i) {
-    const opt_linear2_member& m = members[i];
+    const opt_linear2_member& m = M_(i);
     if (!m.x || !m.w1 || !m.w2 || !m.y) return fail(OPT_ERR_INVALID_ARG, "member %d: NULL pointer", i);
     if (m.M < 1 || m.K < 1 || m.H < 1 || m.N < 1)
       return fail(OPT_ERR_INVALID_ARG, "member %d: M=%d K=%d H=%d N=%d must be >= 1", i, m.M, m.K, m.H, m.N);
@@ -483,6 +778,15 @@ extern "C" opt_status opt_linear2_plan_create(const opt_linear2_member* members,
     if (m.b1) regions.push_back({(uintptr_t)m.b1, 0, (int64_t)m.H * 2, 1, false, i});
     if (m.b2) regions.push_back({(uintptr_t)m.b2, 0, (int64_t)m.N * 2, 1, false, i});
     regions.push_back({(uintptr_t)m.y, m.ldy * 2, (int64_t)m.N * 2, m.M, true, i});
+    if (LN) {
+      const opt_ln_linear2_member& l = lnm[i];
+      if (!aligned16(l.gamma) || !aligned16(l.beta)) return fail(OPT_ERR_ALIGNMENT, "member %d: pointers must be 16-byte aligned", i);
+      if (!(l.eps >= 0.f)) return fail(OPT_ERR_INVALID_ARG, "member %d: eps must be >= 0", i);
+      if (l.gamma) regions.push_back({(uintptr_t)l.gamma, 0, (int64_t)m.K * 2, 1, false, i});
+      if (l.beta) regions.push_back({(uintptr_t)l.beta, 0, (int64_t)m.K * 2, 1, false, i});
+      bytes += ((l.gamma ? m.K : 0) + (l.beta ? m.K : 0)) * 2;
+      flops += 2ll * m.H * m.K;                              // the fold: W1 diag(gamma), s, c
+    }
     flops += 2ll * m.M * m.H * (m.K + m.N);
     bytes += ((int64_t)m.M * m.K + (int64_t)m.H * m.K + (m.b1 ? m.H : 0) + (int64_t)m.N * m.H + (m.b2 ? m.N : 0) +
               (int64_t)m.M * m.N) * 2;
@@ -496,18 +800,45 @@ extern "C" opt_status opt_linear2_plan_create(const opt_linear2_member* members,
   EncodeTiledFn enc = nullptr;
   if (opt_status st = get_encoder(&enc)) return st;
   auto align_up = [](size_t x) { return (x + 255) & ~size_t(255); };
+  // LN: workspace = per member  W1g [H,K] bf16 | augmented slice [H,16] bf16
+  std::vector<L2Fold> folds(LN ? n : 0);
+  char* ws = nullptr;
+  if (LN) {
+    size_t wbytes = 0;
+    std::vector<size_t> offs(n);
+    for (int32_t i = 0; i < n; ++i) {
+      offs[i] = wbytes;
+      wbytes += align_up((size_t)M_(i).H * M_(i).K * 2) + align_up((size_t)M_(i).H * 32);
+    }
+    cudaError_t e = cudaMalloc(reinterpret_cast<void**>(&ws), wbytes);
+    if (e != cudaSuccess) return fail(OPT_ERR_CUDA, "workspace allocation (%zu bytes) failed: %s", wbytes, cudaGetErrorString(e));
+    for (int32_t i = 0; i < n; ++i) {
+      const opt_linear2_member& m = M_(i);
+      L2Fold& f = folds[i];
+      memset(&f, 0, sizeof f);
+      f.w1 = static_cast<const uint16_t*>(m.w1); f.ldw1 = m.ldw1;
+      f.gamma = static_cast<const uint16_t*>(lnm[i].gamma); f.beta = static_cast<const uint16_t*>(lnm[i].beta);
+      f.b1 = static_cast<const uint16_t*>(m.b1);
+      f.w1g = reinterpret_cast<uint16_t*>(ws + offs[i]);
+      f.aug = reinterpret_cast<uint16_t*>(ws + offs[i] + align_up((size_t)m.H * m.K * 2));
+      f.H = m.H; f.K = m.K; f.eps = lnm[i].eps;
+    }
+  }
+  struct WsGuard { char* p; ~WsGuard() { if (p) cudaFree(p); } } ws_guard{ws};     // freed on every error path
   std::vector<L2Member> tab(n);
   memset(tab.data(), 0, tab.size() * sizeof(L2Member));
   std::vector<TileEntry2> flat;
   flat.reserve((size_t)tiles);
   for (int32_t i = 0; i < n; ++i) {
-    const opt_linear2_member& m = members[i];
+    const opt_linear2_member& m = M_(i);
     L2Member& t = tab[i];
     opt_status st;
     if ((st = encode_2d(enc, &t.tmX, m.x, m.M, m.K, m.ldx, kT_BK, kT_BM, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, "X", i)) ||
-        (st = encode_2d(enc, &t.tmW1, m.w1, m.H, m.K, m.ldw1, kT_BK, kT_HC, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, "W1", i)) ||
+        (st = encode_2d(enc, &t.tmW1, LN ? (const void*)folds[i].w1g : m.w1, m.H, m.K, LN ? (int64_t)m.K : m.ldw1, kT_BK, kT_HC,
+                        CU_TENSOR_MAP_L2_PROMOTION_L2_256B, "W1", i)) ||
         (st = encode_2d(enc, &t.tmW2, m.w2, m.N, m.H, m.ldw2, kT_BK, m.N, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, "W2", i)) ||
-        (st = encode_2d(enc, &t.tmY, m.y, m.M, m.N, m.ldy, 64, 32, CU_TENSOR_MAP_L2_PROMOTION_NONE, "Y", i)))
+        (st = encode_2d(enc, &t.tmY, m.y, m.M, m.N, m.ldy, 64, 32, CU_TENSOR_MAP_L2_PROMOTION_NONE, "Y", i)) ||
+        (LN && (st = encode_2d(enc, &t.tmAug, folds[i].aug, m.H, 16, 16, kT_BK, kT_HC, CU_TENSOR_MAP_L2_PROMOTION_NONE, "aug", i))))
       return st;
     const int nkb1 = (m.K + kT_BK - 1) / kT_BK, klast1 = (m.K - (nkb1 - 1) * kT_BK + 15) / 16;
     for (int mb = 0; mb < (m.M + kT_BM - 1) / kT_BM; ++mb) {
@@ -515,7 +846,7 @@ extern "C" opt_status opt_linear2_plan_create(const opt_linear2_member* members,
       e.member = i; e.m0 = mb * kT_BM;
       e.shape = (uint32_t)m.H | ((uint32_t)nkb1 << 16) | ((uint32_t)klast1 << 24);
       e.misc = (uint32_t)m.act1 | ((uint32_t)m.act2 << 8) | ((uint32_t)m.N << 16);
-      e.b1 = m.b1; e.b2 = m.b2;
+      e.b1 = LN ? nullptr : m.b1; e.b2 = m.b2;
       flat.push_back(e);
     }
   }
@@ -540,22 +871,41 @@ extern "C" opt_status opt_linear2_plan_create(const opt_linear2_member* members,
   const int64_t n_chunks = (int64_t)(chunked.size() / 4);
 
   opt_plan* p = new opt_plan();
-  p->kind = kPlanLinear2; p->device = device; p->io = io; p->n_members = n; p->flops = flops; p->bytes = bytes;
+  p->kind = LN ? kPlanLnLinear2 : kPlanLinear2; p->device = device; p->io = io; p->n_members = n; p->flops = flops; p->bytes = bytes;
   p->off0 = 0;
   p->off1 = align_up(tab.size() * sizeof(L2Member));
   p->off2 = p->off1 + align_up(chunked.size() * sizeof(TileEntry2));
-  const size_t total = p->off2 + 256;                         // two int32 scheduler counters, zero-initialised
+  // scheduler counters (256 bytes: chunk, done, LN epoch), then LN: per-member flags, fold table; zero-initialised
+  p->off3 = p->off2 + 256 + align_up((size_t)(LN ? n : 0) * 4);
+  const size_t total = p->off3 + folds.size() * sizeof(L2Fold);
   std::vector<char> blob(total, 0);
+  if (LN) memcpy(blob.data() + p->off3, folds.data(), folds.size() * sizeof(L2Fold));
   memcpy(blob.data(), tab.data(), tab.size() * sizeof(L2Member));
   memcpy(blob.data() + p->off1, chunked.data(), chunked.size() * sizeof(TileEntry2));
   if (opt_status st = upload_tables(p, blob.data(), total)) { delete p; return st; }
-  cudaError_t e = cudaFuncSetAttribute(grouped_linear2_sm100_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kT_SmemBytes);
+  const int smem_bytes = LN ? L2Cfg<true>::kSmemBytes : L2Cfg<false>::kSmemBytes;
+  cudaError_t e = LN ? cudaFuncSetAttribute(grouped_linear2_sm100_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_bytes)
+                     : cudaFuncSetAttribute(grouped_linear2_sm100_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_bytes);
   if (e != cudaSuccess) {
     cudaFree(p->dev_tables); delete p;
-    return fail(OPT_ERR_CUDA, "cudaFuncSetAttribute(max dynamic smem %d) failed: %s", kT_SmemBytes, cudaGetErrorString(e));
+    return fail(OPT_ERR_CUDA, "cudaFuncSetAttribute(max dynamic smem %d) failed: %s", smem_bytes, cudaGetErrorString(e));
   }
-  p->grid = dim3((unsigned)std::min<int64_t>(n_chunks, num_sms)); p->block = dim3(kT_Threads); p->smem = kT_SmemBytes;
+  p->grid = dim3((unsigned)std::min<int64_t>(n_chunks, num_sms));
+  p->block = dim3(LN ? L2Cfg<true>::kThreads : L2Cfg<false>::kThreads); p->smem = smem_bytes;
   p->total_tiles = (int32_t)tiles; p->n_chunks = (int32_t)n_chunks;
+  p->workspace = ws; ws_guard.p = nullptr;
   *plan = p;
   return OPT_OK;
+}
+}  // namespace
+
+extern "C" opt_status opt_linear2_plan_create(const opt_linear2_member* members, int32_t n, opt_dtype io, int device,
+                                              opt_plan** plan) {
+  return create_linear2(members, nullptr, n, io, device, plan);
+}
+
+extern "C" opt_status opt_ln_linear2_plan_create(const opt_ln_linear2_member* members, int32_t n, opt_dtype io, int device,
+                                                 opt_plan** plan) {
+  if (!members) { if (plan) *plan = nullptr; return fail(OPT_ERR_INVALID_ARG, "opt_ln_linear2_plan_create: NULL argument"); }
+  return create_linear2(nullptr, members, n, io, device, plan);
 }

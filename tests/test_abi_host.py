@@ -40,6 +40,7 @@ def test_struct_layouts_match_header(ob):
     assert ctypes.sizeof(ob.opt_linear_member) == 80
     assert ctypes.sizeof(ob.opt_layernorm_member) == 64
     assert ctypes.sizeof(ob.opt_chunk) == 80
+    assert ctypes.sizeof(ob.opt_linear2_member) == 104 and ctypes.sizeof(ob.opt_ln_linear2_member) == 128
     assert ctypes.sizeof(ob.opt_host_copy) == 32
 
 
