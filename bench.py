@@ -496,6 +496,7 @@ def aggregate_steps_per_s(us_step, world):
 def run_side(args):
     """Small stand-alone workloads for ncu captures of the section-8(f) items (profiles/r01_profiles.md section 4):
       --side linear2   C4's two GEMM groups as one chained-Linear launch (opt_linear2), 3 launches
+      --side ln_linear2  the whole C4 block (LayerNorm folded into the chain, opt_ln_linear2) as one launch
       --side lhs       batch_linear_lhs: 8 members (N=64) on ONE input X [262144, 512]; OPT_GEMM_NO_LHS=1 = plain order
     Prints one JSON line; not the bench metric."""
     import torch
@@ -526,6 +527,18 @@ def run_side(args):
         ga.plan.launch()
         torch.cuda.synchronize()
         print(json.dumps(dict(side="linear2", us=round(timed(plan.launch, 3), 1), **plan.info())))
+    elif args.side == "ln_linear2":
+        step = Step("cuda:0", FULL, pinned_host=False, configs=("c4",))
+        ga = step.groups[0]
+        T = ga.ain.tensor
+        out3 = torch.empty_like(step.groups[2].aout.tensor(ga.iy))
+        plan = ob.opt_ln_linear2_plan_create(
+            [ob.ln_linear2_member(T(i["x"]), T(i["gamma"]), T(i["beta"]), t["eps"], T(i["w1"]), T(i["b1"]), T(i["w2"]), T(i["b2"]),
+                                  out3[:, k * t["out"]:(k + 1) * t["out"]], ACT_RELU, ACT_NONE)
+             for k, (i, t) in enumerate(zip(ga.idx, ga.cfg["towers"]))], BF16, 0)
+        plan.launch()
+        torch.cuda.synchronize()
+        print(json.dumps(dict(side="ln_linear2", us=round(timed(plan.launch, 3), 1), **plan.info())))
     else:
         M, K, N, n = 262144, 512, 64, 8
         g = torch.Generator(device="cuda").manual_seed(0)
@@ -943,7 +956,7 @@ def main():
     ap.add_argument("--profile", action="store_true",
                     help="only the step's own launches (no cpu_baseline, no unfused baseline, no copy reference): for ncu")
     ap.add_argument("--ref-frac", type=float, default=0.0, help="reference arm: override the row-sample fraction")
-    ap.add_argument("--side", default=None, choices=["linear2", "lhs"], help="stand-alone side workload for ncu (not the metric)")
+    ap.add_argument("--side", default=None, choices=["linear2", "ln_linear2", "lhs"], help="stand-alone side workload for ncu (not the metric)")
     args = ap.parse_args()
     if args.side:
         return run_side(args)
