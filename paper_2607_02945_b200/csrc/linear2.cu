@@ -58,6 +58,9 @@ constexpr int kT_StatWarps = 4;
 constexpr int kT_KBlockBytes = kT_BM * kT_BK * 2;          // 16 KB: a 128 x 64 bf16 k-block
 constexpr int kT_W2KBlockBytes = kT_MaxN * kT_BK * 2;      // 8 KB: a 64 x 64 k-block of W2
 constexpr int kT_QDepth = 4;
+#ifndef L2_FLAG_SPIN_LIMIT
+#define L2_FLAG_SPIN_LIMIT 4096       // polls of a member's fold flag before the scheduler warp folds the member itself
+#endif
 // shared-memory map
 constexpr int kT_OffX = 0;
 constexpr int kT_OffW1 = kT_OffX + (kT_MaxK / kT_BK) * kT_KBlockBytes;            //  64 KB
@@ -321,9 +324,24 @@ grouped_linear2_sm100_kernel(const L2Member* __restrict__ members, const uint4* 
         if (member >= 0) {
           if (LN) {
             // the member's folded weights / s / c come from some CTA's prologue of THIS launch: wait for its flag
+            int ready = 0;
             if (lane == 0) {
               int f;
-              do { asm volatile("ld.acquire.gpu.global.s32 %0, [%1];" : "=r"(f) : "l"(flags + member) : "memory"); } while (f != epoch1);
+              for (int spin = 0; spin < L2_FLAG_SPIN_LIMIT && !ready; ++spin) {
+                asm volatile("ld.acquire.gpu.global.s32 %0, [%1];" : "=r"(f) : "l"(flags + member) : "memory");
+                ready = f == epoch1;
+              }
+            }
+            ready = __shfl_sync(0xffffffffu, ready, 0);
+            if (!ready) {
+              // The owner's prologue has not run (its CTA is not resident: fewer SMs than the grid, e.g. a partitioned
+              // context): fold the member here.  Folds are idempotent -- every writer stores the same bits.
+              const L2Fold f = folds[member];
+              l2_fold_member(f, 0, 1, lane);
+              asm volatile("fence.proxy.async;" ::: "memory");
+              __threadfence();
+              __syncwarp();
+              if (lane == 0) asm volatile("st.release.gpu.global.s32 [%0], %1;" ::"l"(flags + member), "r"(epoch1) : "memory");
             }
             __syncwarp();
           } else {

@@ -97,3 +97,37 @@ def test_pointwise_300_random_chunks_all_ops(ob):
         assert d.max() <= 2, (op, int(d.max()))
         if op == 0:
             assert to_host(dd).tobytes() == a.tobytes()
+
+
+def test_ln_linear2_300_random_towers(ob):
+    """300 towers with random (M, K, H, N), activations, optional affine / biases, in ONE launch: every fold flag,
+    tile tail and chunk width the LayerNorm-folded chain distinguishes; relaunched three times (epoch flags)."""
+    from test_gpu_ln_linear2 import KEYS, mk as mk_tower
+    rng = np.random.default_rng(2027)
+    members, descs, keep = [], [], []
+    for i in range(300):
+        M, K, H, N = int(rng.integers(1, 400)), 8 * int(rng.integers(1, 33)), 16 * int(rng.integers(1, 33)), 16 * int(rng.integers(1, 5))
+        m = mk_tower(74, i, M, K, H, N, act1=int(rng.integers(0, 4)), act2=int(rng.integers(0, 4)), bias=bool(rng.integers(0, 2)),
+                     affine=bool(rng.integers(0, 4)), mean=float(rng.uniform(-2, 2)), std=float(rng.uniform(0.5, 3)))
+        d = {k: (to_dev(m[k], BF16) if m.get(k) is not None else None) for k in KEYS}
+        y = empty_dev((M, N), BF16, fill=float("nan"))
+        members.append(m)
+        keep.append((d, y))
+        descs.append(ob.ln_linear2_member(d["x"], d["gamma"], d["beta"], m["eps"], d["w1"], d["b1"], d["w2"], d["b2"], y, m["act1"], m["act2"]))
+    plan = ob.opt_ln_linear2_plan_create(descs, BF16)
+    n0 = ob.opt_launch_count()
+    plan.launch()
+    torch.cuda.synchronize()
+    assert ob.opt_launch_count() - n0 == 1
+    first = [to_host(y) for _, y in keep]
+    # Reading Q26 (DESIGN.md section 2): the chain has three bf16 rounding stages (folded weight, hidden tensor, output)
+    # instead of the single GEMM's one, and rows of 16 outputs behind a ReLU can keep only a few small elements, so
+    # the row-L2 metric has a heavier tail than on a GEMM row: gate 2e-2 on the worst of ~60 000 rows, and the
+    # typical row (median over members of the worst row) must sit at the bf16 rounding floor.
+    per_member = [row_l2_rel_err(got, graphs.ln_linear2(m, BF16)["y64"], BF16) for got, m in zip(first, members)]
+    assert max(per_member) <= 2e-2, max(per_member)
+    assert float(np.median(per_member)) <= 5e-3, float(np.median(per_member))
+    for _ in range(3):
+        plan.launch()
+    torch.cuda.synchronize()
+    assert all(to_host(y).tobytes() == f.tobytes() for (_, y), f in zip(keep, first))
