@@ -865,6 +865,49 @@ def run_product(args):
         except Exception as e:  # noqa: BLE001
             backward = dict(error=repr(e))
 
+    # ---- (8) SURVEY 8(f) rank 4, side figure: the skinny aten.mm group of PAPER.md:477 (decompose_mm_pass), full size
+    skinny = None
+    if not args.profile and not args.small:
+        try:
+            shapes = [(18583840, 8, 8), (25247936, 4, 2), (22502112, 8, 8), (17980096, 4, 2)]       # (M, K, N)
+            ten = [(torch.randn(M, K, device=device, dtype=torch.bfloat16), torch.randn(N, K, device=device, dtype=torch.bfloat16),
+                    torch.empty(M, N, device=device, dtype=torch.bfloat16)) for M, K, N in shapes]
+            ps = ob.opt_linear_plan_create([ob.linear_member(x, w, None, y, ACT_NONE) for x, w, y in ten], BF16, step.dev_index)
+            flush = torch.empty(256 * 1024 * 1024, dtype=torch.uint8, device=device)
+
+            def cold3(fn, n=5):
+                ts = []
+                for _ in range(n):
+                    flush.fill_(1)
+                    c0_, c1_ = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                    c0_.record(stream); fn(); c1_.record(stream)
+                    torch.cuda.synchronize()
+                    ts.append(c0_.elapsed_time(c1_) * 1e3)
+                return float(np.mean(ts))
+            ps.launch()
+            torch.cuda.synchronize()
+            tsk = cold3(ps.launch)
+            isk = ps.info()
+            # the two [M,8]x[8,8] members alone: streaming row kernel vs the tensor-core tile kernel (OPT_GEMM_NO_SKINNY=1)
+            two = [ob.linear_member(x, w, None, y, ACT_NONE) for (x, w, y), sh in zip(ten, shapes) if sh[1] == 8]
+            p8 = ob.opt_linear_plan_create(two, BF16, step.dev_index)
+            os.environ["OPT_GEMM_NO_SKINNY"] = "1"
+            try:
+                p8t = ob.opt_linear_plan_create(two, BF16, step.dev_index)
+            finally:
+                del os.environ["OPT_GEMM_NO_SKINNY"]
+            p8.launch(); p8t.launch()
+            torch.cuda.synchronize()
+            t8, t8t = cold3(p8.launch), cold3(p8t.launch, 2)
+            skinny = dict(workload="PAPER.md:477 model type B: aten.mm [18583840,8]x[8,8], [25247936,4]x[4,2], [22502112,8]x[8,8], "
+                                   "[17980096,4]x[4,2] as ONE group, one launch (paper: each > 914 ms unfused on its hardware)",
+                          launches=1, us=round(tsk, 1), algorithmic_bytes=isk["bytes"], gbs=round(isk["bytes"] / tsk / 1e3, 1),
+                          frac_hbm=round(isk["bytes"] / tsk / 1e3 / peaks["hbm_gbs"], 4),
+                          two_8x8_members_row_kernel_us=round(t8, 1), two_8x8_members_tensor_core_tiles_us=round(t8t, 1))
+            del ten, flush
+        except Exception as e:  # noqa: BLE001
+            skinny = dict(error=repr(e))
+
     watch.stop_flag.set()
     watch.join(timeout=2)
 
@@ -927,7 +970,7 @@ def run_product(args):
                              "copies overlap, single_stream_us: everything on one stream"),
                 gpu_launches=int(launches), launches_per_step=ng,
                 clocks=watch.summary(), roofline=roofline, roofline_tensor=roofline_tensor, groups=groups,
-                unfused_baseline=unfused, vertical_fusion=vertical, backward=backward, config0_latency=c0,
+                unfused_baseline=unfused, vertical_fusion=vertical, backward=backward, skinny_linear=skinny, config0_latency=c0,
                 aggregate=dict(steps_per_s=round(aggregate_steps_per_s(us_step, world), 2)),
                 build_seconds=round(build_s, 1), lib=ob.opt_version())
 

@@ -102,7 +102,12 @@ enum { OPT_LAYOUT_X_TRANSPOSED = 1, OPT_LAYOUT_W_TRANSPOSED = 2 };
  * NULL, Y:[M,N] (ldy).  For a concatenated output give y = concat_base +
  * column_offset and ldy = total concat width.  bf16: inputs and output bf16,
  * products accumulated in fp32 on the tensor cores, bias and activation in
- * fp32, one round-to-nearest-even to bf16.  fp32: plain fp32 FMA (no TF32).  */
+ * fp32, one round-to-nearest-even to bf16.  fp32: plain fp32 FMA (no TF32).
+ * SKINNY groups (decompose_mm_pass: huge M, tiny K and N): a bf16
+ * group in which EVERY member has K in {4,8,16}, N in {2,4,8,16}, K*N <= 128 and
+ * layout 0 runs through a streaming row kernel instead of 128-row tensor-core
+ * tiles (same semantics, one launch); for such a group ldx, ldw and ldy only
+ * have to be even, so dense [M,4] x [4,2] tensors are accepted.                */
 typedef struct {
   const void* x;
   int64_t ldx;

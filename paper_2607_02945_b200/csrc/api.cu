@@ -111,6 +111,7 @@ static cudaError_t launch_kind(const opt_plan* p, cudaStream_t s) {
     case kPlanLinearBf16: return launch_linear_bf16(p, s);
     case kPlanLinearF32: return launch_linear_f32(p, s);
     case kPlanLinear2: case kPlanLnLinear2: return launch_linear2(p, s);
+    case kPlanLinearSkinny: return launch_linear_skinny(p, s);
     case kPlanLayerNormBwd: return launch_layernorm_bwd(p, s);
     default: return cudaErrorInvalidValue;
   }

@@ -51,7 +51,7 @@ struct Region {
 opt_status check_independent(std::vector<Region>& regions, bool allow_inplace_self);
 
 // ---------------------------------------------------------------- the plan --
-enum PlanKind { kPlanPointwise = 1, kPlanLayerNorm = 2, kPlanLinearBf16 = 3, kPlanLinearF32 = 4, kPlanLinear2 = 5, kPlanLayerNormBwd = 6, kPlanLnLinear2 = 7 };
+enum PlanKind { kPlanPointwise = 1, kPlanLayerNorm = 2, kPlanLinearBf16 = 3, kPlanLinearF32 = 4, kPlanLinear2 = 5, kPlanLayerNormBwd = 6, kPlanLnLinear2 = 7, kPlanLinearSkinny = 8 };
 
 }  // namespace optb
 
@@ -80,6 +80,9 @@ cudaError_t launch_layernorm(const opt_plan* p, cudaStream_t s);
 cudaError_t launch_linear_bf16(const opt_plan* p, cudaStream_t s);
 cudaError_t launch_linear_f32(const opt_plan* p, cudaStream_t s);
 cudaError_t launch_linear2(const opt_plan* p, cudaStream_t s);
+cudaError_t launch_linear_skinny(const opt_plan* p, cudaStream_t s);
+bool skinny_linear_member(const opt_linear_member& m);
+opt_status plan_skinny_linear(const opt_linear_member* members, int32_t n, opt_plan* p);
 cudaError_t launch_layernorm_bwd(const opt_plan* p, cudaStream_t s);
 
 // host->device upload of a table blob; allocates p->dev_tables

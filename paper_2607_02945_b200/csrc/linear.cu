@@ -502,6 +502,9 @@ extern "C" opt_status opt_linear_plan_create(const opt_linear_member* members, i
   std::vector<Region> regions;
   int64_t flops = 0, bytes = 0;
   std::set<std::tuple<const void*, int64_t, int32_t, int32_t>> seen_x;
+  // huge-M / tiny-K-and-N groups (decompose_mm_pass) stream through the SIMT row kernel (linear_skinny.cu)
+  bool skinny = io == OPT_BF16 && !getenv("OPT_GEMM_NO_SKINNY");     // (knob for A/B measurements, like OPT_GEMM_NCTA)
+  for (int32_t i = 0; skinny && i < n; ++i) skinny = skinny_linear_member(members[i]);
   for (int32_t i = 0; i < n; ++i) {
     const opt_linear_member& m = members[i];
     if (!m.x || !m.w || !m.y) return fail(OPT_ERR_INVALID_ARG, "member %d: NULL pointer", i);
@@ -521,7 +524,12 @@ extern "C" opt_status opt_linear_plan_create(const opt_linear_member* members, i
     // 16-byte aligned.  fp32 (SIMT path): multiples of 4.
     if (io == OPT_F32 && (m.K % V || m.N % V))
       return fail(OPT_ERR_ALIGNMENT, "member %d: K=%d and N=%d must be multiples of %d", i, m.K, m.N, V);
-    if (m.ldx % V || m.ldw % V || m.ldy % V) return fail(OPT_ERR_ALIGNMENT, "member %d: row strides must be multiples of %d elements", i, V);
+    if (skinny) {      // rows are read and written as 4-byte words
+      if (m.ldx % 2 || m.ldw % 2 || m.ldy % 2)
+        return fail(OPT_ERR_ALIGNMENT, "member %d: row strides must be even (4-byte words)", i);
+    } else if (m.ldx % V || m.ldw % V || m.ldy % V) {
+      return fail(OPT_ERR_ALIGNMENT, "member %d: row strides must be multiples of %d elements", i, V);
+    }
     regions.push_back({(uintptr_t)m.x, m.ldx * esz, (int64_t)x_cols * esz, x_rows, false, i});
     regions.push_back({(uintptr_t)m.w, m.ldw * esz, (int64_t)w_cols * esz, w_rows, false, i});
     if (m.bias) regions.push_back({(uintptr_t)m.bias, 0, (int64_t)m.N * esz, 1, false, i});
@@ -540,6 +548,12 @@ extern "C" opt_status opt_linear_plan_create(const opt_linear_member* members, i
   p->device = device; p->io = io; p->n_members = n; p->flops = flops; p->bytes = bytes;
   std::vector<int32_t> starts(n + 1);
   int64_t tiles = 0;
+
+  if (skinny) {
+    if (opt_status st = plan_skinny_linear(members, n, p)) { delete p; return st; }
+    *plan = p;
+    return OPT_OK;
+  }
 
   if (io == OPT_F32) {
     std::vector<F32Member> tab(n);
