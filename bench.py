@@ -497,6 +497,8 @@ def run_side(args):
     """Small stand-alone workloads for ncu captures of the section-8(f) items (profiles/r01_profiles.md section 4):
       --side linear2   C4's two GEMM groups as one chained-Linear launch (opt_linear2), 3 launches
       --side ln_linear2  the whole C4 block (LayerNorm folded into the chain, opt_ln_linear2) as one launch
+      --side skinny    the paper's four skinny aten.mm as one group (streaming row kernel)
+      --side fp8       configs[4]'s saved LayerNorm outputs -> FP8 E4M3 and back (one launch each)
       --side lhs       batch_linear_lhs: 8 members (N=64) on ONE input X [262144, 512]; OPT_GEMM_NO_LHS=1 = plain order
     Prints one JSON line; not the bench metric."""
     import torch
@@ -539,6 +541,27 @@ def run_side(args):
         plan.launch()
         torch.cuda.synchronize()
         print(json.dumps(dict(side="ln_linear2", us=round(timed(plan.launch, 3), 1), **plan.info())))
+    elif args.side == "skinny":
+        shapes = [(18583840, 8, 8), (25247936, 4, 2), (22502112, 8, 8), (17980096, 4, 2)]       # PAPER.md:477, (M, K, N)
+        ten = [(torch.randn(M, K, device="cuda", dtype=torch.bfloat16), torch.randn(N, K, device="cuda", dtype=torch.bfloat16),
+                torch.empty(M, N, device="cuda", dtype=torch.bfloat16)) for M, K, N in shapes]
+        plan = ob.opt_linear_plan_create([ob.linear_member(x, w, None, y, ACT_NONE) for x, w, y in ten], BF16, 0)
+        plan.launch()
+        torch.cuda.synchronize()
+        print(json.dumps(dict(side="skinny", us=round(timed(plan.launch, 3), 1), **plan.info())))
+    elif args.side == "fp8":
+        step = Step("cuda:0", FULL, pinned_host=False, configs=("c4",))
+        ga = step.groups[0]
+        ga.plan.launch()
+        A = ga.amid.tensor
+        q8 = [torch.empty(A(i["xn"]).shape, dtype=torch.uint8, device="cuda") for i in ga.idx]
+        r16 = [torch.empty_like(A(i["xn"])) for i in ga.idx]
+        pq = ob.opt_pointwise_plan_create([ob.chunk(A(i["xn"]), q, ob.OPT_PW_QUANT_E4M3, None, [16.0]) for i, q in zip(ga.idx, q8)], BF16, 0)
+        pdq = ob.opt_pointwise_plan_create([ob.chunk(q, r, ob.OPT_PW_DEQUANT_E4M3, None, [1.0 / 16.0]) for q, r in zip(q8, r16)], BF16, 0)
+        pq.launch(); pdq.launch()
+        torch.cuda.synchronize()
+        print(json.dumps(dict(side="fp8", quant_us=round(timed(pq.launch, 3), 1), dequant_us=round(timed(pdq.launch, 3), 1),
+                              quant_bytes=pq.info()["bytes"], dequant_bytes=pdq.info()["bytes"])))
     else:
         M, K, N, n = 262144, 512, 64, 8
         g = torch.Generator(device="cuda").manual_seed(0)
@@ -999,7 +1022,7 @@ def main():
     ap.add_argument("--profile", action="store_true",
                     help="only the step's own launches (no cpu_baseline, no unfused baseline, no copy reference): for ncu")
     ap.add_argument("--ref-frac", type=float, default=0.0, help="reference arm: override the row-sample fraction")
-    ap.add_argument("--side", default=None, choices=["linear2", "ln_linear2", "lhs"], help="stand-alone side workload for ncu (not the metric)")
+    ap.add_argument("--side", default=None, choices=["linear2", "ln_linear2", "lhs", "skinny", "fp8"], help="stand-alone side workload for ncu (not the metric)")
     args = ap.parse_args()
     if args.side:
         return run_side(args)
