@@ -7,17 +7,18 @@
 // tile would spend its time on zero-filled operands (measured: 3.8x slower).  The right tensor-core shape for it is
 // the warp-level mma.sync m16n8k8 / m16n8k16: a warp multiplies 16 rows at a time, and the fragment layouts make
 // every global access a 4-byte word per lane with the lanes of a row group contiguous (thread (g, t) of the warp
-// owns x[row g][2t..2t+1] and y[row g][2t..2t+1]): no shared memory, ~1 instruction per row per warp, 40 registers.  W ([N,K], a few hundred bytes) and the
+// owns x[row g][2t..2t+1] and y[row g][2t..2t+1]): no shared memory, ~1 instruction per row per warp, 64 registers.  W ([N,K], a few hundred bytes) and the
 // bias live in registers as B / C fragments; tails (K = 4 < 8, N < 8) are zero fragments and masked stores.
 // One launch for the whole group; a block walks 4096 consecutive rows of one member in chunks of 512.  Measured on
 // the paper's group (1.83 GB): occupancy beats per-thread unrolling and register double-buffering (16 loads in flight
-// per lane at 2 blocks / SM: 500 us; 8 loads at 6 blocks / SM: 334 us = 84 % of the HBM copy peak).  fp32 accumulation, one
+// per lane at 2 blocks / SM: 500 us; 8 loads at 4 - 6 blocks / SM: 328 us = 85 % of the HBM copy peak).  fp32 accumulation, one
 // rounding: the semantics of opt_linear_member.
 //
 // Routing (opt_linear_plan_create): a bf16 group takes this path when EVERY member has K in {4, 8, 16},
 // N in {2, 4, 8, 16}, K * N <= 128 and untransposed operands.  Row strides then only need to be even (4-byte words),
 // which admits the paper's dense [M, 4] and [M, 2] tensors.
 #include <algorithm>
+#include <type_traits>
 
 #include "common.h"
 
@@ -28,7 +29,7 @@ constexpr int kSkThreads = 256;
 #define SK_UNROLL 4
 #endif
 #ifndef SK_MINBLOCKS
-#define SK_MINBLOCKS 6             // occupancy is what hides the latency here: 6 x 256 threads per SM at <= 40 registers
+#define SK_MINBLOCKS 4             // occupancy is what hides the latency here: 4 x 256 threads per SM at <= 64 registers
 #endif
 constexpr int kSkUnroll = SK_UNROLL;                   // 16-row MMA groups per warp and chunk: 8 warps x 4 x 16 = 512 rows
 constexpr int kSkChunkRows = (kSkThreads / 32) * kSkUnroll * 16;
@@ -82,25 +83,28 @@ __device__ __forceinline__ void sk_rows(const SkMember& m, int row0) {
     bias[f][0] = (m.bias && c0 < N) ? __uint_as_float((uint32_t)__ldg(m.bias + c0) << 16) : 0.f;
     bias[f][1] = (m.bias && c0 + 1 < N) ? __uint_as_float((uint32_t)__ldg(m.bias + c0 + 1) << 16) : 0.f;
   }
-  constexpr int AR = K == 16 ? 4 : 2;
-  auto load = [&](uint32_t (&a)[kSkUnroll][AR], int base) {      // A fragments of kSkUnroll 16-row groups (independent, streaming)
+  // one chunk = kSkUnroll 16-row groups per warp.  FULL: every row of the chunk exists (no row predicates);
+  // NOACT: no activation (both block-uniform).  Row pointers advance by a constant stride of 8 rows.
+  auto chunk = [&](int base, auto full_tag, auto noact_tag) {
+    constexpr bool FULL = decltype(full_tag)::value, NOACT = decltype(noact_tag)::value;
+    constexpr int AR = K == 16 ? 4 : 2;
+    const int64_t sx8 = 4 * m.ldx, sy8 = 4 * m.ldy;            // 8 rows, in 4-byte words
+    const uint32_t* px = reinterpret_cast<const uint32_t*>(m.x + (int64_t)(base + g) * m.ldx) + t;
+    uint32_t* py = reinterpret_cast<uint32_t*>(m.y + (int64_t)(base + g) * m.ldy) + t;
+    uint32_t a[kSkUnroll][AR];
 #pragma unroll
-    for (int u = 0; u < kSkUnroll; ++u) {
+    for (int u = 0; u < kSkUnroll; ++u) {                      // all loads first: independent, streaming
       const int rlo = base + u * 16 + g, rhi = rlo + 8;
-      const uint32_t* plo = reinterpret_cast<const uint32_t*>(m.x + (int64_t)rlo * m.ldx) + t;
-      const uint32_t* phi = reinterpret_cast<const uint32_t*>(m.x + (int64_t)rhi * m.ldx) + t;
-      a[u][0] = (rlo < m.M && kin) ? __ldcs(plo) : 0u;
-      a[u][1] = (rhi < m.M && kin) ? __ldcs(phi) : 0u;
+      const uint32_t* plo = px + (2 * u) * sx8;
+      const uint32_t* phi = plo + sx8;
+      const bool vlo = FULL || rlo < m.M, vhi = FULL || rhi < m.M;
+      a[u][0] = (vlo && kin) ? __ldcs(plo) : 0u;
+      a[u][1] = (vhi && kin) ? __ldcs(phi) : 0u;
       if (K == 16) {
-        a[u][2] = rlo < m.M ? __ldcs(plo + 4) : 0u;
-        a[u][3] = rhi < m.M ? __ldcs(phi + 4) : 0u;
+        a[u][AR - 2] = vlo ? __ldcs(plo + 4) : 0u;
+        a[u][AR - 1] = vhi ? __ldcs(phi + 4) : 0u;
       }
     }
-  };
-  int base = row0 + warp * (kSkUnroll * 16);
-  for (int ch = 0; ch < kSkChunks && base - warp * (kSkUnroll * 16) < m.M; ++ch, base += kSkChunkRows) {
-    uint32_t a[kSkUnroll][AR];
-    load(a, base);
 #pragma unroll
     for (int u = 0; u < kSkUnroll; ++u) {
       const int rlo = base + u * 16 + g, rhi = rlo + 8;
@@ -114,13 +118,21 @@ __device__ __forceinline__ void sk_rows(const SkMember& m, int row0) {
           mma_1688(c, a[u][0], a[u][1], b[f][0]);
         }
         if (8 * f + 2 * t < N) {                       // N is even: a column pair is valid or not as a whole
-          const uint32_t lo = pack_bf16x2(act_f32<true>(c[0], m.act), act_f32<true>(c[1], m.act));
-          const uint32_t hi = pack_bf16x2(act_f32<true>(c[2], m.act), act_f32<true>(c[3], m.act));
-          if (rlo < m.M) __stcs(reinterpret_cast<uint32_t*>(m.y + (int64_t)rlo * m.ldy) + 4 * f + t, lo);
-          if (rhi < m.M) __stcs(reinterpret_cast<uint32_t*>(m.y + (int64_t)rhi * m.ldy) + 4 * f + t, hi);
+          const uint32_t lo = NOACT ? pack_bf16x2(c[0], c[1]) : pack_bf16x2(act_f32<true>(c[0], m.act), act_f32<true>(c[1], m.act));
+          const uint32_t hi = NOACT ? pack_bf16x2(c[2], c[3]) : pack_bf16x2(act_f32<true>(c[2], m.act), act_f32<true>(c[3], m.act));
+          if (FULL || rlo < m.M) __stcs(py + (2 * u) * sy8 + 4 * f, lo);
+          if (FULL || rhi < m.M) __stcs(py + (2 * u + 1) * sy8 + 4 * f, hi);
         }
       }
     }
+  };
+  using T = std::true_type;
+  using F = std::false_type;
+  const int wofs = warp * (kSkUnroll * 16);
+  for (int ch = 0, start = row0; ch < kSkChunks && start < m.M; ++ch, start += kSkChunkRows) {
+    const bool full = start + kSkChunkRows <= m.M;
+    if (m.act == OPT_ACT_NONE) { if (full) chunk(start + wofs, T{}, T{}); else chunk(start + wofs, F{}, T{}); }
+    else { if (full) chunk(start + wofs, T{}, F{}); else chunk(start + wofs, F{}, F{}); }
   }
 }
 
