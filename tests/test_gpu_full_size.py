@@ -138,3 +138,38 @@ def test_c4_full_three_groups(step):
     assert esc < 1e-3 * tot
     assert worst_b <= TOL_BF16 and worst_c <= TOL_BF16, (worst_b, worst_c)
     assert worst_e2e <= 3 * TOL_BF16, worst_e2e
+
+
+def test_c4_full_one_launch_towers(step):
+    """SURVEY 8(f) rank 1 at configs[4]'s full size, on the step's own tensors: the 512 towers as ONE chained-Linear
+    launch (from the step's bf16 LN output: bitwise equal to the two-group path) and as ONE LayerNorm-folded launch
+    (from the raw inputs: sampled rows against graphs.ln_linear2, reading Q25)."""
+    import paper_2607_02945_b200 as ob
+    ga, gb, gc = step["C4a_batched_layernorm"], step["C4b_grouped_linear_relu"], step["C4c_grouped_linear_concat"]
+    towers = ga.cfg["towers"]
+    T, A = ga.ain.tensor, ga.amid.tensor
+    ref_out = gc.aout.tensor(gc.iy)
+    out2, out3 = torch.empty_like(ref_out), torch.empty_like(ref_out)
+    p2 = ob.opt_linear2_plan_create([ob.linear2_member(A(i["xn"]), T(i["w1"]), T(i["b1"]), T(i["w2"]), T(i["b2"]),
+                                                       out2[:, k * t["out"]:(k + 1) * t["out"]], 1, 0)
+                                     for k, (i, t) in enumerate(zip(ga.idx, towers))], BF16)
+    p3 = ob.opt_ln_linear2_plan_create([ob.ln_linear2_member(T(i["x"]), T(i["gamma"]), T(i["beta"]), t["eps"], T(i["w1"]), T(i["b1"]),
+                                                             T(i["w2"]), T(i["b2"]), out3[:, k * t["out"]:(k + 1) * t["out"]], 1, 0)
+                                        for k, (i, t) in enumerate(zip(ga.idx, towers))], BF16)
+    n0 = ob.opt_launch_count()
+    p2.launch(); p3.launch()
+    torch.cuda.synchronize()
+    assert ob.opt_launch_count() - n0 == 2
+    assert torch.equal(out2.view(torch.int16), ref_out.view(torch.int16))
+    worst = 0.0
+    for k in range(0, len(towers), 4):                 # every 4th tower: all (D, H) classes, 128 towers
+        t = towers[k]
+        rows = sample_rows(t["B"], 6, 5000 + k)
+        rsel = torch.from_numpy(rows).cuda()
+        o = to_host(out3[rsel, k * t["out"]:(k + 1) * t["out"]])
+        r = graphs.ln_linear2(dict(t, x=np.ascontiguousarray(t["x"][rows]), act1=1, act2=0), BF16)
+        worst = max(worst, row_l2_rel_err(o, r["y64"], BF16))
+    assert worst <= TOL_BF16, worst
+    # and the two one-launch results differ only by the LN output's rounding (Q25)
+    d = (out3.float() - out2.float()).norm(dim=1) / out2.float().norm(dim=1).clamp_min(1e-30)
+    assert float(d.max()) <= TOL_BF16
