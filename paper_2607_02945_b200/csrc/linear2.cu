@@ -33,8 +33,9 @@
 //   * prologue: every CTA folds a share of the members (W1g and the augmented slice into the plan's workspace) and
 //     publishes a per-member epoch flag; the scheduler warp waits for a member's flag before it queues one of its
 //     tiles (no grid-wide barrier: a CTA only ever waits for a prologue, and prologues wait for nothing);
-//   * the raw X tile feeds MMA1 with W1g; four extra warps compute mu_r, sigma_r of the 128 rows from the same
-//     shared-memory tile WHILE the MMAs run (shifted single pass, fp32) and write the augmented A slice;
+//   * the raw X tile feeds MMA1 with W1g; the epilogue warps compute mu_r, sigma_r of the 128 rows from the same
+//     shared-memory tile WHILE the MMAs run (two threads per row, shifted single pass, fp32) and write the augmented
+//     A slice (extra statistics warps would put > 12 warps on the SM: <= 128 registers, measured 30 us slower);
 //   * epilogue 1 is h = act1(rstd_r * acc): no per-column operand at all.
 #include <algorithm>
 #include <cstdlib>
@@ -53,8 +54,6 @@ constexpr int kT_W1Stages = 4;
 constexpr int kT_EpiWarps = 8;
 constexpr int kT_FirstEpiWarp = 3;
 constexpr int kT_Mma2Warp = kT_FirstEpiWarp + kT_EpiWarps;     // warp 11: layer-2 MMA issuer
-constexpr int kT_StatWarp0 = kT_Mma2Warp + 1;                  // LN: warps 12..15 row statistics
-constexpr int kT_StatWarps = 4;
 constexpr int kT_KBlockBytes = kT_BM * kT_BK * 2;          // 16 KB: a 128 x 64 bf16 k-block
 constexpr int kT_W2KBlockBytes = kT_MaxN * kT_BK * 2;      // 8 KB: a 64 x 64 k-block of W2
 constexpr int kT_QDepth = 4;
@@ -70,7 +69,7 @@ constexpr int kT_OffOut = kT_OffW2 + 2 * 2 * kT_W2KBlockBytes;                  
 constexpr int kT_OffQ = kT_OffOut + 4 * 4096;                                     // +16 KB output staging (4 warps x 32 rows x 128 B)
 template <bool LN>
 struct L2Cfg {
-  static constexpr int kThreads = 32 * (LN ? kT_StatWarp0 + kT_StatWarps : kT_Mma2Warp + 1);
+  static constexpr int kThreads = 32 * (kT_Mma2Warp + 1);
   // LN: the augmented A k-slice (a 128 x 64 k-block in the swizzled layout, 16 columns used) sits before the queue
   static constexpr int kOffAug = kT_OffQ;
   static constexpr int kOffQ = kT_OffQ + (LN ? kT_KBlockBytes : 0);
@@ -78,8 +77,8 @@ struct L2Cfg {
   static constexpr int kOffB2 = LN ? 0 : kT_MaxH * 2;
   static constexpr int kQEntryOff = kOffB2 + kT_MaxN * 2;
   static constexpr int kQSlotBytes = kQEntryOff + 32;
-  static constexpr int kOffStats = kOffQ + kT_QDepth * kQSlotBytes;               // LN: 2 x 128 rows x rstd
-  static constexpr int kOffBar = kOffStats + (LN ? 2 * kT_BM * 4 : 0);
+  static constexpr int kOffStats = kOffQ + kT_QDepth * kQSlotBytes;               // LN: partial row sums, 2 halves x 128 rows x {sum, sumsq}
+  static constexpr int kOffBar = kOffStats + (LN ? 2 * kT_BM * 8 : 0);
   static constexpr int kSmemBytes = kOffBar + 384;
   static_assert(kSmemBytes <= 227 * 1024, "chained-GEMM shared memory map exceeds 227 KB");
 };
@@ -126,48 +125,22 @@ __device__ __forceinline__ void epi_act(const uint32_t (&v)[64], uint32_t bias_a
   }
 }
 
-// LN kernel: 14 warps put four warps on every SM sub-partition, i.e. at most 128 registers per thread, so its
-// epilogue works on 32 accumulator columns at a time.
-// Layer 1: h = act(rstd_r * acc) (this thread's row; the per-column terms were added by the tensor core).
+// LN, layer 1: h = act(rstd_r * acc) (this thread's row; the per-column terms were added by the tensor core).
 template <int ACT>
-__device__ __forceinline__ void epi_math_ln32(const uint32_t (&v)[32], float A, uint32_t (&p)[16]) {
+__device__ __forceinline__ void epi_math_ln(const uint32_t (&v)[64], float A, uint32_t (&p)[32]) {
 #pragma unroll
-  for (int j = 0; j < 16; ++j) {
+  for (int j = 0; j < 32; ++j) {
     const float f0 = A * __uint_as_float(v[2 * j]), f1 = A * __uint_as_float(v[2 * j + 1]);
     if (ACT == OPT_ACT_RELU) p[j] = pack_relu_bf16x2(f0, f1);
     else p[j] = pack_bf16x2(act_f32<true>(f0, ACT), act_f32<true>(f1, ACT));
   }
 }
-__device__ __forceinline__ void epi_act_ln32(const uint32_t (&v)[32], float A, int act, uint32_t (&p)[16]) {
+__device__ __forceinline__ void epi_act_ln(const uint32_t (&v)[64], float A, int act, uint32_t (&p)[32]) {
   switch (act) {
-    case OPT_ACT_RELU: epi_math_ln32<OPT_ACT_RELU>(v, A, p); break;
-    case OPT_ACT_NONE: epi_math_ln32<OPT_ACT_NONE>(v, A, p); break;
-    case OPT_ACT_TANH: epi_math_ln32<OPT_ACT_TANH>(v, A, p); break;
-    default:           epi_math_ln32<OPT_ACT_SIGMOID>(v, A, p); break;
-  }
-}
-// Layer 2, 32 columns: + bias (bf16 in the queue slot), activation, RNE.
-template <int ACT>
-__device__ __forceinline__ void epi_math32(const uint32_t (&v)[32], uint32_t bias_addr, uint32_t (&p)[16]) {
-#pragma unroll
-  for (int j = 0; j < 4; ++j) {          // 8 columns per step
-    const uint4 b = lds128(bias_addr + 16 * j);
-    const uint32_t bw[4] = {b.x, b.y, b.z, b.w};
-#pragma unroll
-    for (int t = 0; t < 4; ++t) {
-      const float lo = __uint_as_float(v[8 * j + 2 * t]) + bf16_lo(bw[t]);
-      const float hi = __uint_as_float(v[8 * j + 2 * t + 1]) + bf16_hi(bw[t]);
-      if (ACT == OPT_ACT_RELU) p[4 * j + t] = pack_relu_bf16x2(lo, hi);
-      else p[4 * j + t] = pack_bf16x2(act_f32<true>(lo, ACT), act_f32<true>(hi, ACT));
-    }
-  }
-}
-__device__ __forceinline__ void epi_act32(const uint32_t (&v)[32], uint32_t bias_addr, int act, uint32_t (&p)[16]) {
-  switch (act) {
-    case OPT_ACT_RELU: epi_math32<OPT_ACT_RELU>(v, bias_addr, p); break;
-    case OPT_ACT_NONE: epi_math32<OPT_ACT_NONE>(v, bias_addr, p); break;
-    case OPT_ACT_TANH: epi_math32<OPT_ACT_TANH>(v, bias_addr, p); break;
-    default:           epi_math32<OPT_ACT_SIGMOID>(v, bias_addr, p); break;
+    case OPT_ACT_RELU: epi_math_ln<OPT_ACT_RELU>(v, A, p); break;
+    case OPT_ACT_NONE: epi_math_ln<OPT_ACT_NONE>(v, A, p); break;
+    case OPT_ACT_TANH: epi_math_ln<OPT_ACT_TANH>(v, A, p); break;
+    default:           epi_math_ln<OPT_ACT_SIGMOID>(v, A, p); break;
   }
 }
 
@@ -252,8 +225,7 @@ grouped_linear2_sm100_kernel(const L2Member* __restrict__ members, const uint4* 
   auto q_full = [&](int s) { return bar_base + kB2 + 128u + 8u * s; };
   auto q_empty = [&](int s) { return bar_base + kB2 + 128u + 8u * (kT_QDepth + s); };
   const uint32_t tmem_ptr_addr = bar_base + kB2 + 128u + 16u * kT_QDepth;
-  auto st_full = [&](int s) { return tmem_ptr_addr + 8u + 8u * s; };           // LN: row statistics of a tile
-  auto st_empty = [&](int s) { return tmem_ptr_addr + 24u + 8u * s; };
+  auto st_full = [&](int s) { return tmem_ptr_addr + 8u + 8u * s; };           // LN: the augmented A slice of a tile is written
   static_assert(16 + 16 * kT_W1Stages + 128 + 16 * kT_QDepth + 8 + 32 <= 384, "barrier area");
   auto q_slot = [&](int s) { return sbase + Cfg::kOffQ + (uint32_t)s * kT_QSlotBytes; };
   constexpr uint32_t kQEntryOff = Cfg::kQEntryOff, kOffB2 = Cfg::kOffB2;
@@ -262,8 +234,8 @@ grouped_linear2_sm100_kernel(const L2Member* __restrict__ members, const uint4* 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
 
   if (warp == 0 && lane == 0) {
-    mbar_init(xa_full, 1); mbar_init(xa_empty, LN ? 1 + kT_StatWarps : 1);      // LN: the statistics warps read the X tile too
-    if (LN) for (int s = 0; s < 2; ++s) { mbar_init(st_full(s), kT_StatWarps); mbar_init(st_empty(s), kT_EpiWarps); }
+    mbar_init(xa_full, 1); mbar_init(xa_empty, LN ? 1 + kT_EpiWarps : 1);       // LN: the epilogue warps read the X tile too (row statistics)
+    if (LN) for (int s = 0; s < 2; ++s) mbar_init(st_full(s), kT_EpiWarps / 2);
     for (int s = 0; s < kT_W1Stages; ++s) { mbar_init(w1_full(s), 1); mbar_init(w1_empty(s), 1); }
     for (int s = 0; s < 2; ++s) {
       mbar_init(w2_full(s), 1); mbar_init(w2_empty(s), 1);
@@ -271,7 +243,7 @@ grouped_linear2_sm100_kernel(const L2Member* __restrict__ members, const uint4* 
       mbar_init(h_full(s), kT_EpiWarps); mbar_init(h_empty(s), 1);
       mbar_init(a2_full(s), 1); mbar_init(a2_empty(s), kT_EpiWarps);
     }
-    for (int s = 0; s < kT_QDepth; ++s) { mbar_init(q_full(s), 1); mbar_init(q_empty(s), 3 + kT_EpiWarps + (LN ? kT_StatWarps : 0)); }
+    for (int s = 0; s < kT_QDepth; ++s) { mbar_init(q_full(s), 1); mbar_init(q_empty(s), 3 + kT_EpiWarps); }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     fence_proxy_async_smem();
   }
@@ -486,7 +458,7 @@ grouped_linear2_sm100_kernel(const L2Member* __restrict__ members, const uint4* 
             if (++w1s == kT_W1Stages) { w1s = 0; w1ph ^= 1; }
           }
           if (LN) {                                          // + (-mu_r s_n + sigma_r c_n): one K=16 step
-            if (c == 0) mbar_wait(st_full(gt & 1u), (gt >> 1) & 1u);   // the statistics warps have written the A slice
+            if (c == 0) mbar_wait(st_full(gt & 1u), (gt >> 1) & 1u);   // the epilogue warps have written the A slice
             mbar_wait(w1_full(w1s), w1ph);
             tc_fence_after();
             tc_mma_bf16(acc1, umma_desc_sw128(aug_base), wd0 + (uint64_t)w1s * kKB, idesc1, 1);
@@ -536,57 +508,6 @@ grouped_linear2_sm100_kernel(const L2Member* __restrict__ members, const uint4* 
         ++gt;
       }
     }
-  } else if (LN && warp >= kT_StatWarp0) {
-    // -------------------------------------------- LN: row statistics of the X tile ----
-    // Each lane owns one of the tile's 128 rows and reads it from the swizzled tile while MMA1 runs on it.
-    // Shifted single pass (shift = the row's first element): sum(x - x0), sum((x - x0)^2) in fp32.
-    const int sw = warp - kT_StatWarp0;
-    int qs = 0; uint32_t qph = 0;
-    uint32_t gt = 0;
-    for (;;) {
-      mbar_wait(q_full(qs), qph);
-      const uint4 e0 = lds128(q_slot(qs) + kQEntryOff);
-      __syncwarp();
-      if (lane == 0) mbar_arrive(q_empty(qs));
-      if (++qs == kT_QDepth) { qs = 0; qph ^= 1; }
-      if ((int)e0.x < 0) break;
-      const int K = __ldg(&folds[(int)e0.x].K);
-      const float eps = __ldg(&folds[(int)e0.x].eps);
-      const uint32_t ss = gt & 1u;
-      mbar_wait(st_empty(ss), ((gt >> 1) & 1u) ^ 1u);
-      mbar_wait(xa_full, gt & 1u);
-      const int r0 = sw * 32 + lane;
-      const uint32_t a0 = sbase + kT_OffX + (uint32_t)r0 * 128u;
-      const uint32_t x7 = (uint32_t)(lane & 7);                   // r0 & 7
-      const float s0 = bf16_lo(lds128(a0 + (x7 << 4)).x);         // logical chunk 0, element 0: the shift
-      const f32x2 ns = pk2(-s0, -s0);
-      f32x2 sumA = pk2(0.f, 0.f), sumB = sumA, sqA = sumA, sqB = sumA;
-      const int nv = K >> 3;
-#pragma unroll 4
-      for (int c = 0; c < nv; ++c) {
-        const uint4 u = lds128(a0 + (uint32_t)(c >> 3) * kT_KBlockBytes + ((((uint32_t)c & 7u) ^ x7) << 4));
-        const f32x2 d0 = add2(bf2_to_f2(u.x), ns), d1 = add2(bf2_to_f2(u.y), ns);
-        const f32x2 d2 = add2(bf2_to_f2(u.z), ns), d3 = add2(bf2_to_f2(u.w), ns);
-        sumA = add2(sumA, d0); sqA = fma2(d0, d0, sqA);
-        sumB = add2(sumB, d1); sqB = fma2(d1, d1, sqB);
-        sumA = add2(sumA, d2); sqA = fma2(d2, d2, sqA);
-        sumB = add2(sumB, d3); sqB = fma2(d3, d3, sqB);
-      }
-      const float inv = 1.f / (float)K;
-      const float m0 = sum2(add2(sumA, sumB)) * inv;
-      const float sig = sqrtf(fmaxf(fmaf(-m0, m0, sum2(add2(sqA, sqB)) * inv), 0.f) + eps), nmu = -(s0 + m0);
-      // augmented A slice of this row: -mu_h, -mu_h, -mu_l, sigma_h, sigma_h, sigma_l, 0, 0 | 0 x 8
-      const uint32_t mh = pack_bf16x2(nmu, 0.f) & 0xFFFFu, gh2 = pack_bf16x2(sig, 0.f) & 0xFFFFu;
-      const uint32_t ml = pack_bf16x2(nmu - bf16_lo(mh), 0.f) & 0xFFFFu, gl = pack_bf16x2(sig - bf16_lo(gh2), 0.f) & 0xFFFFu;
-      const uint32_t arow = aug_base + (uint32_t)r0 * 128u;
-      sts128(arow + (x7 << 4), make_uint4(mh | (mh << 16), ml | (gh2 << 16), gh2 | (gl << 16), 0u));
-      sts128(arow + ((1u ^ x7) << 4), make_uint4(0u, 0u, 0u, 0u));
-      asm volatile("st.shared.f32 [%0], %1;" ::"r"(stats_base + ss * (kT_BM * 4) + (uint32_t)r0 * 4u), "f"(1.f / sig) : "memory");
-      fence_proxy_async_smem();                      // the A slice is read by the tensor core
-      __syncwarp();
-      if (lane == 0) { mbar_arrive(st_full(ss)); mbar_arrive(xa_empty); }
-      ++gt;
-    }
   } else {
     // ----------------------------------------------------------- epilogue ----
     // Per hidden chunk: acc1 -> registers -> + b1, act1, RNE -> the hidden tile in shared memory (layer-2 A operand).
@@ -609,32 +530,17 @@ grouped_linear2_sm100_kernel(const L2Member* __restrict__ members, const uint4* 
       const uint32_t s2 = p_gt & 1u;
       mbar_wait(a2_full(s2), (p_gt >> 1) & 1u);
       tc_fence_after();
-      uint32_t p[32];
-      if constexpr (LN) {                      // 32 columns at a time; only the storing warps read the accumulator
-        uint32_t(&pa)[16] = *reinterpret_cast<uint32_t(*)[16]>(&p[0]);
-        uint32_t(&pb)[16] = *reinterpret_cast<uint32_t(*)[16]>(&p[16]);
-        if (half == 0) {
-          const uint32_t t = tmem_base + lane_off + 256u + s2 * 64u;
-          uint32_t v[32];
-          tc_ld_32x32(t, v); tc_wait_ld();
-          epi_act32(v, p_slot + kOffB2, p_act2, pa);
-          tc_ld_32x32(t + 32, v); tc_wait_ld();
-          epi_act32(v, p_slot + kOffB2 + 64, p_act2, pb);
-        }
-        tc_fence_before();
-        __syncwarp();
-        if (lane == 0) mbar_arrive(a2_empty(s2));
-      } else {
-        uint32_t v[64];
+      uint32_t v[64], p[32];
+      {
         const uint32_t t = tmem_base + lane_off + 256u + s2 * 64u;
         tc_ld_32x32(t, *reinterpret_cast<uint32_t(*)[32]>(&v[0]));
         tc_ld_32x32(t + 32, *reinterpret_cast<uint32_t(*)[32]>(&v[32]));
         tc_wait_ld();
-        tc_fence_before();
-        __syncwarp();
-        if (lane == 0) mbar_arrive(a2_empty(s2));
-        if (half == 0) epi_act(v, p_slot + kOffB2, p_act2, p);
       }
+      tc_fence_before();
+      __syncwarp();
+      if (lane == 0) mbar_arrive(a2_empty(s2));
+      if (half == 0) epi_act(v, p_slot + kOffB2, p_act2, p);
       if (half == 0) {
         if (lane == 0) tma_store_wait_read<0>();       // this warp's previous store has read the staging tile
         __syncwarp();
@@ -662,12 +568,60 @@ grouped_linear2_sm100_kernel(const L2Member* __restrict__ members, const uint4* 
       const int act1 = (int)(e0.w & 0xFFu), act2 = (int)((e0.w >> 8) & 0xFFu);
       const int nch = (H + kT_HC - 1) / kT_HC;
       float lnA = 0.f;                                // LN: rstd of this thread's row
-      if (LN) {
+      if constexpr (LN) {
+        // Row statistics from the resident X tile while MMA1 runs on it: the two threads of a row (the warps of one
+        // TMEM quadrant) take alternate 16-byte pieces, shifted single pass (shift = the row's first element),
+        // partial sums exchanged through shared memory; the half-0 thread writes the row's augmented A slice
+        // (-mu_h, -mu_h, -mu_l, sigma_h, sigma_h, sigma_l, 0...).
+        const int K = __ldg(&folds[(int)e0.x].K);
+        const float eps = __ldg(&folds[(int)e0.x].eps);
         const uint32_t ss = gt & 1u;
-        mbar_wait(st_full(ss), (gt >> 1) & 1u);
-        asm volatile("ld.shared.f32 %0, [%1];" : "=f"(lnA) : "r"(stats_base + ss * (kT_BM * 4) + (uint32_t)(quad * 32 + lane) * 4u) : "memory");
+        mbar_wait(xa_full, gt & 1u);
+        const int r0 = quad * 32 + lane;
+        const uint32_t a0 = sbase + kT_OffX + (uint32_t)r0 * 128u;
+        const uint32_t x7 = (uint32_t)(lane & 7);                   // r0 & 7
+        const float s0 = bf16_lo(lds128(a0 + (x7 << 4)).x);
+        const f32x2 ns = pk2(-s0, -s0);
+        f32x2 sumA = pk2(0.f, 0.f), sumB = sumA, sqA = sumA, sqB = sumA;
+        const int nv = K >> 3;
+#pragma unroll 4
+        for (int c = half; c < nv; c += 2) {
+          const uint4 u = lds128(a0 + (uint32_t)(c >> 3) * kT_KBlockBytes + ((((uint32_t)c & 7u) ^ x7) << 4));
+          const f32x2 d0 = add2(bf2_to_f2(u.x), ns), d1 = add2(bf2_to_f2(u.y), ns);
+          const f32x2 d2 = add2(bf2_to_f2(u.z), ns), d3 = add2(bf2_to_f2(u.w), ns);
+          sumA = add2(sumA, d0); sqA = fma2(d0, d0, sqA);
+          sumB = add2(sumB, d1); sqB = fma2(d1, d1, sqB);
+          sumA = add2(sumA, d2); sqA = fma2(d2, d2, sqA);
+          sumB = add2(sumB, d3); sqB = fma2(d3, d3, sqB);
+        }
+        float psum = sum2(add2(sumA, sumB)), psq = sum2(add2(sqA, sqB));
+        const uint32_t mine_addr = stats_base + ((uint32_t)half * kT_BM + (uint32_t)r0) * 8u;
+        const uint32_t peer_addr = stats_base + ((uint32_t)(half ^ 1) * kT_BM + (uint32_t)r0) * 8u;
+        asm volatile("st.shared.v2.f32 [%0], {%1, %2};" ::"r"(mine_addr), "f"(psum), "f"(psq) : "memory");
+        asm volatile("bar.sync %0, 64;" ::"r"(1 + quad) : "memory");
+        float osum, osq;
+        asm volatile("ld.shared.v2.f32 {%0, %1}, [%2];" : "=f"(osum), "=f"(osq) : "r"(peer_addr) : "memory");
+        asm volatile("bar.sync %0, 64;" ::"r"(1 + quad) : "memory");    // both have read before either writes the next tile's
+        // same order in both threads: (half 0) + (half 1)
+        const float tsum = half ? osum + psum : psum + osum, tsq = half ? osq + psq : psq + osq;
+        const float inv = 1.f / (float)K;
+        const float m0 = tsum * inv;
+        const float sig = sqrtf(fmaxf(fmaf(-m0, m0, tsq * inv), 0.f) + eps), nmu = -(s0 + m0);
+        lnA = 1.f / sig;
+        if (half == 0) {
+          const uint32_t mh = pack_bf16x2(nmu, 0.f) & 0xFFFFu, gh2 = pack_bf16x2(sig, 0.f) & 0xFFFFu;
+          const uint32_t ml = pack_bf16x2(nmu - bf16_lo(mh), 0.f) & 0xFFFFu, gl = pack_bf16x2(sig - bf16_lo(gh2), 0.f) & 0xFFFFu;
+          const uint32_t arow = aug_base + (uint32_t)r0 * 128u;
+          // (single-buffered: X(t+1) only lands after every MMA1 of tile t, the slice's last reader, has retired)
+          sts128(arow + (x7 << 4), make_uint4(mh | (mh << 16), ml | (gh2 << 16), gh2 | (gl << 16), 0u));
+          sts128(arow + ((1u ^ x7) << 4), make_uint4(0u, 0u, 0u, 0u));
+          fence_proxy_async_smem();                    // the A slice is read by the tensor core
+        }
         __syncwarp();
-        if (lane == 0) mbar_arrive(st_empty(ss));
+        if (lane == 0) {
+          mbar_arrive(xa_empty);
+          if (half == 0) mbar_arrive(st_full(ss));
+        }
       }
       for (int c = 0; c < nch; ++c) {
         const uint32_t g = gh + (uint32_t)c;
@@ -678,29 +632,7 @@ grouped_linear2_sm100_kernel(const L2Member* __restrict__ members, const uint4* 
         mbar_wait(a1_full(s), ph);
         tc_fence_after();
         const uint32_t t = tmem_base + lane_off + (uint32_t)s * 128u + (uint32_t)half * 64u;
-        if constexpr (LN) {                            // (columns past the chunk's width hold stale data: never used)
-          uint32_t va[32], vb[32], q[16];
-          tc_ld_32x32(t, va);
-          tc_ld_32x32(t + 32, vb);
-          tc_wait_ld();
-          tc_fence_before();
-          __syncwarp();
-          if (lane == 0) mbar_arrive(a1_empty(s));
-          mbar_wait(h_empty(0), (g & 1u) ^ 1u);
-          const uint32_t hrow = sbase + kT_OffH + (uint32_t)half * kT_KBlockBytes + row_off;
-          epi_act_ln32(va, lnA, act1, q);
-          if (mine) {
-#pragma unroll
-            for (int j = 0; j < 4; ++j)
-              sts128(hrow + ((j ^ (lane & 7)) << 4), make_uint4(q[4 * j], q[4 * j + 1], q[4 * j + 2], q[4 * j + 3]));
-          }
-          epi_act_ln32(vb, lnA, act1, q);
-          if (mine) {
-#pragma unroll
-            for (int j = 0; j < 4; ++j)
-              sts128(hrow + (((j + 4) ^ (lane & 7)) << 4), make_uint4(q[4 * j], q[4 * j + 1], q[4 * j + 2], q[4 * j + 3]));
-          }
-        } else {
+        {                                              // (columns past the chunk's width hold stale data: never used)
           uint32_t v[64], p[32];
           tc_ld_32x32(t, *reinterpret_cast<uint32_t(*)[32]>(&v[0]));
           tc_ld_32x32(t + 32, *reinterpret_cast<uint32_t(*)[32]>(&v[32]));
@@ -708,7 +640,8 @@ grouped_linear2_sm100_kernel(const L2Member* __restrict__ members, const uint4* 
           tc_fence_before();
           __syncwarp();
           if (lane == 0) mbar_arrive(a1_empty(s));     // acc1 stage is in registers: MMA1 of chunk c+2 may overwrite it
-          epi_act(v, slot + (uint32_t)(c * kT_HC + half * 64) * 2u, act1, p);
+          if constexpr (LN) epi_act_ln(v, lnA, act1, p);
+          else epi_act(v, slot + (uint32_t)(c * kT_HC + half * 64) * 2u, act1, p);
           // the hidden tile is single-buffered: MMA2 of chunk c-1 has normally retired by the time this chunk's
           // accumulator has been read and converted
           mbar_wait(h_empty(0), (g & 1u) ^ 1u);
