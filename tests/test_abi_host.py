@@ -103,6 +103,59 @@ def test_host_validation_runs_before_any_cuda_call(ob):
     assert ob.opt_launch_count() == 0
 
 
+def test_host_validation_of_the_next_row_entry_points(ob):
+    """the section-8(f) entry points validate on the host too: chained Linear (+ LayerNorm), LayerNorm backward,
+    skinny groups (relaxed stride rule), extended / FP8 pointwise ops -- no GPU needed, nothing launched."""
+    import torch
+    A, B, Cc, D, E = 0x10000000, 0x20000000, 0x30000000, 0x40000000, 0x50000000
+    l2 = lambda **kw: ob.opt_linear2_member(**{**dict(x=A, ldx=64, w1=B, ldw1=64, b1=None, w2=Cc, ldw2=128, b2=None, y=D, ldy=64,
+                                                      M=256, K=64, H=128, N=64, act1=1, act2=0), **kw})
+    for member, status in [(l2(K=512, ldx=512, ldw1=512), ob.OPT_ERR_UNSUPPORTED), (l2(H=1024, ldw2=1024), ob.OPT_ERR_UNSUPPORTED),
+                           (l2(N=128, ldy=128), ob.OPT_ERR_UNSUPPORTED), (l2(H=120, ldw2=120), ob.OPT_ERR_ALIGNMENT),
+                           (l2(y=A), ob.OPT_ERR_ALIAS), (l2(act1=7), ob.OPT_ERR_INVALID_ARG), (l2(ldw2=64), ob.OPT_ERR_INVALID_ARG)]:
+        with pytest.raises(ob.OptError) as e:
+            ob.opt_linear2_plan_create([member], ob.OPT_BF16)
+        assert e.value.status == status, (e.value, status)
+    with pytest.raises(ob.OptError) as e:
+        ob.opt_linear2_plan_create([l2()], ob.OPT_F32)
+    assert e.value.status == ob.OPT_ERR_UNSUPPORTED
+    lnl = lambda chain, **kw: ob.opt_ln_linear2_member(**{**dict(chain=chain, gamma=E, beta=None, eps=1e-5, reserved=0), **kw})
+    for member, status in [(lnl(l2(), eps=-1.0), ob.OPT_ERR_INVALID_ARG), (lnl(l2(), gamma=E + 2), ob.OPT_ERR_ALIGNMENT),
+                           (lnl(l2(y=E)), ob.OPT_ERR_ALIAS), (lnl(l2(K=512, ldx=512, ldw1=512)), ob.OPT_ERR_UNSUPPORTED)]:
+        with pytest.raises(ob.OptError) as e:
+            ob.opt_ln_linear2_plan_create([member], ob.OPT_BF16)
+        assert e.value.status == status, (e.value, status)
+    # skinny groups: even row strides are enough, odd ones are not; a non-skinny member in the group restores ld % 8
+    sk = lambda **kw: ob.opt_linear_member(**{**dict(x=A, ldx=4, w=B, ldw=4, bias=None, y=Cc, ldy=2, M=1000, N=2, K=4, act=0, layout=0), **kw})
+    with pytest.raises(ob.OptError) as e:
+        ob.opt_linear_plan_create([sk(ldx=5)], ob.OPT_BF16)
+    assert e.value.status == ob.OPT_ERR_ALIGNMENT
+    big = ob.opt_linear_member(x=D, ldx=64, w=E, ldw=64, bias=None, y=0x60000000, ldy=64, M=128, N=64, K=64, act=0, layout=0)
+    with pytest.raises(ob.OptError) as e:
+        ob.opt_linear_plan_create([sk(), big], ob.OPT_BF16)
+    assert e.value.status == ob.OPT_ERR_ALIGNMENT
+    if not torch.cuda.is_available():
+        with pytest.raises(ob.OptError) as e:      # valid skinny group: only the device is missing
+            ob.opt_linear_plan_create([sk()], ob.OPT_BF16)
+        assert e.value.status == ob.OPT_ERR_NO_DEVICE
+    # LayerNorm backward: D <= 512, multiples of 8
+    lb = lambda **kw: ob.opt_layernorm_bwd_member(**{**dict(x=A, ldx=64, dy=B, lddy=64, gamma=None, dx=Cc, lddx=64, dgamma=None, dbeta=None,
+                                                            rows=16, D=64, eps=1e-5), **kw})
+    for member, status in [(lb(D=1024, ldx=1024, lddy=1024, lddx=1024), ob.OPT_ERR_UNSUPPORTED), (lb(D=60), ob.OPT_ERR_ALIGNMENT),
+                           (lb(dx=A), ob.OPT_ERR_ALIAS)]:
+        with pytest.raises(ob.OptError) as e:
+            ob.opt_layernorm_bwd_plan_create([member], ob.OPT_BF16)
+        assert e.value.status == status, (e.value, status)
+    # pointwise: binary op without a second operand, FP8 on fp32 activations, unknown op
+    ch = lambda **kw: ob.opt_chunk(**{**dict(src=A, lds=64, dst=B, ldd=64, rows=4, width=64, op=0, src2=None, lds2=0, p0=0.0, p1=0.0, p2=0.0), **kw})
+    for chunk, io, status in [(ch(op=ob.OPT_PW_MUL), ob.OPT_BF16, ob.OPT_ERR_INVALID_ARG), (ch(op=ob.OPT_PW_QUANT_E4M3, p0=1.0), ob.OPT_F32, ob.OPT_ERR_UNSUPPORTED),
+                              (ch(op=11), ob.OPT_BF16, ob.OPT_ERR_INVALID_ARG), (ch(op=ob.OPT_PW_SUB, src2=B + 64, lds2=64), ob.OPT_BF16, ob.OPT_ERR_ALIAS)]:
+        with pytest.raises(ob.OptError) as e:
+            ob.opt_pointwise_plan_create([chunk], io)
+        assert e.value.status == status, (e.value, status)
+    assert ob.opt_launch_count() == 0
+
+
 def test_product_never_imports_the_oracle():
     pkg = os.path.join(ROOT, "paper_2607_02945_b200")
     for dirpath, _, files in os.walk(pkg):
