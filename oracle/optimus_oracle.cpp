@@ -183,6 +183,9 @@ void oracle_pointwise(const void* src, int64_t lds, int32_t rows, int32_t width,
 //   op 4 clamp:      y = min(max(x, lo), hi), NaN propagates            (torch.clamp)
 //   op 5 nan_to_num: NaN -> p0, +inf -> p1, -inf -> p2, else x          (torch.nan_to_num)
 //   op 6 / 7 / 8:    a - b, a / b, a * b                                (aten.sub / div / mul)
+//   op 11 relu_bwd:  y = (b <= 0) ? 0 : a   -- a = incoming gradient, b = the ReLU's forward output (or its input:
+//                    same mask); the backward of the ReLU epilogue of a grouped Linear in a post-grad graph
+//                    (batch_linear_post_grad; training QPS is the headline)
 // b may be NULL for the unary ops.
 void oracle_pointwise_ext(const void* a, int64_t lda, const void* b, int64_t ldb, int32_t rows, int32_t width,
                           int op, double p0, double p1, double p2, int dt, double* out) {
@@ -203,6 +206,7 @@ void oracle_pointwise_ext(const void* a, int64_t lda, const void* b, int64_t ldb
         case 6: y = x - widen(b, (int64_t)r * ldb + c, dt); break;
         case 7: y = x / widen(b, (int64_t)r * ldb + c, dt); break;
         case 8: y = x * widen(b, (int64_t)r * ldb + c, dt); break;
+        case 11: y = widen(b, (int64_t)r * ldb + c, dt) <= 0.0 ? 0.0 : x; break;
         default: y = x; break;
       }
       out[(int64_t)r * width + c] = y;

@@ -502,6 +502,30 @@ def test_pointwise_ext_identities_on_random_data():
     assert np.array_equal(oracle.pointwise_ext(a, None, oracle.PW_NAN_TO_NUM, [0.0, 1.0, -1.0], BF16), a64)   # finite: untouched
 
 
+def test_relu_backward_hand_values_and_finite_differences():
+    """ReLU backward (op 11: the ReLU epilogue of a grouped Linear in a post-grad graph, PAPER.md:292
+    batch_linear_post_grad): hand values incl. both zeros, then the derivative of a numpy ReLU by central
+    differences, and the two mask sources (forward output / forward input) agreeing."""
+    g = np.array([[1.5, -2.0, 3.0, 4.0, -5.0, 6.0]], dtype=np.float32)
+    y = np.array([[2.0, 0.0, -0.0, -1.0, 1e-30, 0.5]], dtype=np.float32)
+    got = oracle.pointwise_ext(g, y, oracle.PW_RELU_BWD, [], F32)
+    assert np.array_equal(got, np.array([[1.5, 0.0, 0.0, 0.0, -5.0, 6.0]]))
+    # numpy forward, perturbed: d/dx sum(relu(x) * g) = g * [x > 0] away from the kink
+    x = wl.tensor_normal(17, 1, (5, 24), 0.0, 1.0, F32)
+    x = np.where(np.abs(x) < 1e-2, np.float32(0.5), x)
+    gg = wl.tensor_normal(17, 2, (5, 24), 0.0, 1.0, F32)
+    x64, g64, h = x.astype(np.float64), gg.astype(np.float64), 1e-4
+    fd = ((np.maximum(x64 + h, 0.0) - np.maximum(x64 - h, 0.0)) / (2 * h)) * g64
+    assert np.allclose(oracle.pointwise_ext(gg, x, oracle.PW_RELU_BWD, [], F32), fd, rtol=0, atol=1e-9)
+    out = np.maximum(x, np.float32(0.0))                  # mask from the forward OUTPUT: same gradient
+    assert np.array_equal(oracle.pointwise_ext(gg, out, oracle.PW_RELU_BWD, [], F32),
+                          oracle.pointwise_ext(gg, x, oracle.PW_RELU_BWD, [], F32))
+    # bf16 storage: the gradient passes through bit-exactly where the mask is on
+    gb = wl.tensor_normal(17, 3, (4, 16), 0.0, 3.0, BF16); mb = wl.tensor_normal(17, 4, (4, 16), 0.0, 1.0, BF16)
+    r = oracle.pointwise_ext(gb, mb, oracle.PW_RELU_BWD, [], BF16)
+    assert np.array_equal(r, np.where(oracle.widen(mb, BF16) > 0, oracle.widen(gb, BF16), 0.0))
+
+
 # ------------------------------------------ backward of the grouped Linear (SURVEY 8(f) rank 3) --
 def test_linear_backward_integers_and_adjointness():
     """dgrad / wgrad against numpy integer arithmetic (exact), and the adjoint identities that DEFINE them:
