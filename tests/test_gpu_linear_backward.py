@@ -67,3 +67,74 @@ def test_random_towers(ob, seed):
     for (dx, dw), m in zip(outs, members):
         assert row_l2_rel_err(dx, graphs.linear_dgrad(m["dy"], m["w"]), BF16) <= 1e-2
         assert row_l2_rel_err(dw, graphs.linear_wgrad(m["dy"], m["x"]), BF16) <= 1e-2
+
+
+def test_relu_backward_group_bit_exact(ob):
+    """OPT_PW_RELU_BWD: the gradient masks of N ReLU epilogues in ONE launch -- dense members, column slices of a
+    concat buffer, fp32, both zeros in the mask: bit-exact against the oracle (no arithmetic, only a select)."""
+    import oracle
+    from util import F32
+    rng = np.random.default_rng(91)
+    shapes = [(300, 512), (77, 200), (1000, 64), (129, 1032), (64, 8), (5, 4096)]
+    W = sum(w for _, w in shapes)
+    chunks, host, keep = [], [], []
+    for i, (r, w) in enumerate(shapes):
+        g = wl.tensor_normal(91, 2 * i + 1, (r, w), 0.0, 2.0, BF16)
+        y = wl.tensor_normal(91, 2 * i + 2, (r, w), 0.0, 1.0, BF16).copy()
+        y[(y & 0x8000) != 0] = 0x8000 if i % 2 else 0x0000        # what a ReLU leaves: 0 (or -0) where x <= 0
+        y.reshape(-1)[::53] = 0x8000
+        pad = 24 if i % 2 else 0                                  # odd members: slices of wider buffers
+        dg = to_dev(np.pad(g, ((0, 0), (0, pad))), BF16)[:, :w]
+        dy = to_dev(np.pad(y, ((0, 0), (8, pad))), BF16)[:, 8:8 + w]
+        dd = empty_dev((r, w + pad), BF16, fill=float("nan"))[:, :w]
+        chunks.append(ob.chunk(dg, dd, ob.OPT_PW_RELU_BWD, dy))
+        host.append((g, y)); keep.append((dg, dy, dd))
+    plan = ob.opt_pointwise_plan_create(chunks, BF16)
+    n0 = ob.opt_launch_count()
+    plan.launch()
+    torch.cuda.synchronize()
+    assert ob.opt_launch_count() - n0 == 1
+    for (g, y), (_, _, dd) in zip(host, keep):
+        ref = oracle.round_to_storage(oracle.pointwise_ext(g, y, oracle.PW_RELU_BWD, [], BF16), BF16)
+        assert to_host(dd).tobytes() == ref.tobytes()
+    # fp32, in place on the gradient
+    g = wl.tensor_normal(92, 1, (100, 36), 0, 2, F32); y = np.maximum(wl.tensor_normal(92, 2, (100, 36), 0, 1, F32), np.float32(0))
+    dg, dy = to_dev(g, F32), to_dev(y, F32)
+    ob.opt_pointwise_plan_create([ob.chunk(dg, dg, ob.OPT_PW_RELU_BWD, dy)], F32).launch()
+    torch.cuda.synchronize()
+    assert np.array_equal(to_host(dg), oracle.round_to_storage(oracle.pointwise_ext(g, y, oracle.PW_RELU_BWD, [], F32), F32))
+
+
+def test_full_backward_of_a_linear_relu_group(ob):
+    """Forward Y_i = relu(X_i W_i^T + b_i) (one launch), then the whole backward in three launches: the ReLU masks
+    of all members, all dgrads, all wgrads -- against the oracle run one op at a time on the same forward output."""
+    import oracle
+    members = []
+    for i, (M, N, K) in enumerate([(300, 128, 64), (512, 64, 256), (1000, 256, 128), (257, 136, 72)]):
+        members.append(dict(x=wl.tensor_normal(7, 4 * i + 1, (M, K), 0, 1, BF16), w=wl.tensor_normal(7, 4 * i + 2, (N, K), 0, K ** -0.5, BF16),
+                            b=wl.tensor_normal(7, 4 * i + 3, (N,), 0, 0.1, BF16), g=wl.tensor_normal(7, 4 * i + 4, (M, N), 0, 1, BF16)))
+    dev, fwd, msk, dg, wg = [], [], [], [], []
+    for m in members:
+        (M, K), N = m["x"].shape, m["w"].shape[0]
+        x, w, b, g = (to_dev(m[k], BF16) for k in ("x", "w", "b", "g"))
+        y, dz = empty_dev((M, N), BF16), empty_dev((M, N), BF16, fill=float("nan"))
+        dx, dw = empty_dev((M, K), BF16, fill=float("nan")), empty_dev((N, K), BF16, fill=float("nan"))
+        dev.append((x, w, b, g, y, dz, dx, dw))
+        fwd.append(ob.linear_member(x, w, b, y, ob.OPT_ACT_RELU))
+        msk.append(ob.chunk(g, dz, ob.OPT_PW_RELU_BWD, y))
+        dg.append(ob.linear_member(dz, w, None, dx, 0, ob.OPT_LAYOUT_W_TRANSPOSED))
+        wg.append(ob.linear_member(dz, x, None, dw, 0, ob.OPT_LAYOUT_X_TRANSPOSED | ob.OPT_LAYOUT_W_TRANSPOSED))
+    n0 = ob.opt_launch_count()
+    ob.opt_linear_plan_create(fwd, BF16).launch()
+    ob.opt_pointwise_plan_create(msk, BF16).launch()
+    ob.opt_linear_plan_create(dg, BF16).launch()
+    ob.opt_linear_plan_create(wg, BF16).launch()
+    torch.cuda.synchronize()
+    assert ob.opt_launch_count() - n0 == 4
+    for m, d in zip(members, dev):
+        y = to_host(d[4])                                          # the mask source both sides use: the stored forward output
+        dz = oracle.round_to_storage(oracle.pointwise_ext(m["g"], y, oracle.PW_RELU_BWD, [], BF16), BF16)
+        assert to_host(d[5]).tobytes() == dz.tobytes()
+        assert 0.2 < np.mean(dz == 0) < 0.8                        # the mask really cuts about half
+        assert row_l2_rel_err(to_host(d[6]), graphs.linear_dgrad(dz, m["w"]), BF16) <= 1e-2
+        assert row_l2_rel_err(to_host(d[7]), graphs.linear_wgrad(dz, m["x"]), BF16) <= 1e-2
