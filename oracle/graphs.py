@@ -113,3 +113,23 @@ def linear_dgrad(dy, w, dt=BF16):
 def linear_wgrad(dy, x, dt=BF16):
     """Backward w.r.t. the weight: dW[N,K] = dY[M,N]^T X[M,K] (sum over m in index order), fp64."""
     return linear(_transposed(dy), _transposed(x), None, dt)
+
+
+def linear_bias_grad(dz, dt=BF16):
+    """Backward of y = x W^T + b w.r.t. the bias: db[n] = sum_m dZ[m, n], rows added in index order, fp64
+    (PAPER.md:292 batch_linear_post_grad; PAPER.md:437 training)."""
+    z = widen(dz, dt)
+    db = np.zeros(z.shape[1], dtype=np.float64)
+    for r in range(z.shape[0]):
+        db += z[r]
+    return db
+
+
+def linear_relu_backward(m, dy, dt=BF16):
+    """The whole backward of one member y = relu(x W^T + b), one op at a time, the mask taken from the STORED forward
+    output y (reading Q26): dz = dy where y > 0 else 0 (storage dtype: a select, exact); db = column sums of dz;
+    dX = dz W; dW = dz^T x.  -> dict(dz (storage), db64, dx64, dw64)."""
+    from . import PW_RELU_BWD, pointwise_ext
+    y = round_to_storage(linear_member(dict(m, act=1), dt), dt)
+    dz = round_to_storage(pointwise_ext(dy, y, PW_RELU_BWD, [], dt), dt)
+    return dict(y=y, dz=dz, db64=linear_bias_grad(dz, dt), dx64=linear_dgrad(dz, m["w"], dt), dw64=linear_wgrad(dz, m["x"], dt))

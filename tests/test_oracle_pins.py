@@ -544,6 +544,34 @@ def test_linear_backward_integers_and_adjointness():
 
 
 # --------------------------------------------- LayerNorm backward --
+def test_bias_grad_and_full_linear_relu_backward_by_finite_differences():
+    """linear_bias_grad: hand values; equals dY^T . 1 through the pinned `linear`; and the whole backward of
+    relu(x W^T + b) (mask, db, dX, dW) against central differences of a NUMPY forward in fp64."""
+    dz = np.array([[1.0, -2.0, 0.5], [3.0, 4.0, -0.5], [-1.0, 0.25, 8.0]], dtype=np.float32)
+    assert np.array_equal(graphs.linear_bias_grad(dz, F32), [3.0, 2.25, 8.0])
+    g = wl.tensor_normal(23, 1, (37, 12), 0.0, 1.0, F32)
+    ones = np.ones((37, 1), dtype=np.float32)
+    assert np.allclose(graphs.linear_bias_grad(g, F32), graphs.linear_wgrad(g, ones, F32)[:, 0], rtol=0, atol=1e-12)
+    x = wl.tensor_normal(23, 2, (9, 6), 0.0, 1.0, F32); w = wl.tensor_normal(23, 3, (5, 6), 0.0, 0.5, F32)
+    b = wl.tensor_normal(23, 4, (5,), 0.0, 0.5, F32); dy = wl.tensor_normal(23, 5, (9, 5), 0.0, 1.0, F32)
+    r = graphs.linear_relu_backward(dict(x=x, w=w, b=b), dy, F32)
+    x64, w64, b64, dy64 = (a.astype(np.float64) for a in (x, w, b, dy))
+    loss = lambda xx, ww, bb: float((np.maximum(xx @ ww.T + bb, 0.0) * dy64).sum())
+    assert np.abs(x64 @ w64.T + b64).min() > 1e-3                       # no pre-activation sits on the kink
+    h = 1e-6
+    def fd(a, which):
+        out = np.zeros_like(a)
+        for idx in np.ndindex(a.shape):
+            ap, am = a.copy(), a.copy(); ap[idx] += h; am[idx] -= h
+            args_p = [x64, w64, b64]; args_m = [x64, w64, b64]
+            args_p[which], args_m[which] = ap, am
+            out[idx] = (loss(*args_p) - loss(*args_m)) / (2 * h)
+        return out
+    assert np.allclose(r["db64"], fd(b64, 2), rtol=0, atol=1e-6)
+    assert np.allclose(r["dx64"], fd(x64, 0), rtol=0, atol=1e-6)
+    assert np.allclose(r["dw64"], fd(w64, 1), rtol=0, atol=1e-6)
+
+
 def test_layernorm_backward_finite_differences_and_identities():
     """dx, dgamma, dbeta against central finite differences of the oracle's OWN forward are not a pin (same code
     base), so the forward used here is numpy's: L(x, gamma, beta) = sum(dy * LN(x)) in fp64.  Plus the closed forms:
