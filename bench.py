@@ -847,6 +847,16 @@ def run_product(args):
                             wgrad_us=round(tw_, 1), wgrad_tflops=round(iwg["flops"] / tw_ / 1e6, 1),
                             frac_tensor_dgrad=round(idg["flops"] / td / 1e6 / peaks["bf16_tflops"], 4),
                             frac_tensor_wgrad=round(iwg["flops"] / tw_ / 1e6 / peaks["bf16_tflops"], 4))
+            # bias gradients db = column sums of dY of the 128 members (slices of the concat gradient), one launch
+            dbs = [torch.empty(m["N"], dtype=torch.float32, device=device) for m in g2.cfg["members"]]
+            pb = ob.opt_bias_grad_plan_create([ob.bias_grad_member(dy_cat[:, m["col_off"]:m["col_off"] + m["N"]], d)
+                                               for m, d in zip(g2.cfg["members"], dbs)], BF16, ob.OPT_F32, step.dev_index)
+            pb.launch()
+            torch.cuda.synchronize()
+            tb_ = cold2(pb.launch)
+            backward.update(bias_grad_us=round(tb_, 1), bias_grad_gbs=round(pb.info()["bytes"] / tb_ / 1e3, 1),
+                            bias_grad_frac_hbm=round(pb.info()["bytes"] / tb_ / 1e3 / peaks["hbm_gbs"], 4))
+            del dbs
             # LayerNorm backward of C4a's 512 members (dx, dgamma, dbeta), one launch
             c4a = [g for g in step.groups if g.name.startswith("C4a")]
             if c4a:

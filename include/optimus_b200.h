@@ -209,6 +209,20 @@ typedef struct {
   float eps;
 } opt_layernorm_bwd_member;
 
+/* One member of a batched bias gradient (the third output of the backward of
+ * y = x W^T + b, PAPER.md:292 batch_linear_post_grad on post-grad graphs, PAPER.md:437 training):
+ *     db[n] = sum over m of dZ[m, n]
+ * dz:[M,N] (ldz, elements; a column slice of a concat buffer is fine), db:[N] in the param dtype (device
+ * pointers, caller-owned).  bf16 activations, N % 8 == 0, 16-byte aligned pointers, ldz % 8 == 0 (else
+ * OPT_ERR_ALIGNMENT).  fp32 accumulation; rows are added in a fixed order (row groups, then row parts, through a
+ * plan-owned workspace): bitwise reproducible, no atomics on data.  opt_plan_info: flops = M N adds, bytes = dZ + db. */
+typedef struct {
+  const void* dz;
+  int64_t ldz;
+  void* db;
+  int32_t M, N;
+} opt_bias_grad_member;
+
 /* One chunk of a multi-tensor pointwise / split-cat pass -- batch_relu,
  * batch_sigmoid, batch_aten_tanh, batch_detach and the data
  * movement left over by the split/cat rewrites (Listing 2):
@@ -256,6 +270,8 @@ opt_status opt_layernorm_plan_create(const opt_layernorm_member* members, int32_
                                      opt_dtype param, int device, opt_plan** plan);
 opt_status opt_layernorm_bwd_plan_create(const opt_layernorm_bwd_member* members, int32_t n, opt_dtype io,
                                          opt_dtype param, int device, opt_plan** plan);
+opt_status opt_bias_grad_plan_create(const opt_bias_grad_member* members, int32_t n, opt_dtype io,
+                                     opt_dtype param, int device, opt_plan** plan);
 opt_status opt_pointwise_plan_create(const opt_chunk* chunks, int32_t n, opt_dtype io, int device,
                                      opt_plan** plan);
 

@@ -47,6 +47,10 @@ class opt_layernorm_bwd_member(C.Structure):
                 ("rows", C.c_int32), ("D", C.c_int32), ("eps", C.c_float)]
 
 
+class opt_bias_grad_member(C.Structure):
+    _fields_ = [("dz", C.c_void_p), ("ldz", C.c_int64), ("db", C.c_void_p), ("M", C.c_int32), ("N", C.c_int32)]
+
+
 class opt_chunk(C.Structure):
     _fields_ = [("src", C.c_void_p), ("lds", C.c_int64), ("dst", C.c_void_p), ("ldd", C.c_int64),
                 ("rows", C.c_int32), ("width", C.c_int32), ("op", C.c_int32),
@@ -90,6 +94,7 @@ def lib():
                                                 C.c_int, pp]
         L.opt_layernorm_bwd_plan_create.argtypes = [C.POINTER(opt_layernorm_bwd_member), C.c_int32, C.c_int, C.c_int,
                                                     C.c_int, pp]
+        L.opt_bias_grad_plan_create.argtypes = [C.POINTER(opt_bias_grad_member), C.c_int32, C.c_int, C.c_int, C.c_int, pp]
         L.opt_pointwise_plan_create.argtypes = [C.POINTER(opt_chunk), C.c_int32, C.c_int, C.c_int, pp]
         L.opt_plan_launch.argtypes = [C.c_void_p, C.c_void_p]
         L.opt_plan_launch_host.argtypes = [C.c_void_p, C.POINTER(opt_host_copy), C.c_int32, C.c_void_p]
@@ -99,7 +104,7 @@ def lib():
         L.opt_last_error.restype = C.c_char_p
         L.opt_launch_count.restype = C.c_uint64
         L.opt_version.restype = C.c_char_p
-        for f in (L.opt_linear_plan_create, L.opt_linear2_plan_create, L.opt_ln_linear2_plan_create, L.opt_layernorm_plan_create, L.opt_layernorm_bwd_plan_create, L.opt_pointwise_plan_create,
+        for f in (L.opt_linear_plan_create, L.opt_linear2_plan_create, L.opt_ln_linear2_plan_create, L.opt_layernorm_plan_create, L.opt_layernorm_bwd_plan_create, L.opt_bias_grad_plan_create, L.opt_pointwise_plan_create,
                   L.opt_plan_launch, L.opt_plan_launch_host, L.opt_plan_info, L.opt_plan_destroy):
             f.restype = C.c_int
         _lib = L
@@ -182,6 +187,11 @@ def opt_layernorm_bwd_plan_create(members, io, param=None, device=0):
                    io if param is None else param, device)
 
 
+def opt_bias_grad_plan_create(members, io, param=None, device=0):
+    return _create(lib().opt_bias_grad_plan_create, opt_bias_grad_member, members, io,
+                   io if param is None else param, device)
+
+
 def opt_pointwise_plan_create(chunks, io, device=0):
     return _create(lib().opt_pointwise_plan_create, opt_chunk, chunks, io, device)
 
@@ -260,6 +270,12 @@ def layernorm_bwd_member(x, dy, gamma, dx, dgamma, dbeta, eps):
     ptr = lambda t: None if t is None else t.data_ptr()
     return opt_layernorm_bwd_member(x.data_ptr(), _ld(x), dy.data_ptr(), _ld(dy), ptr(gamma), dx.data_ptr(), _ld(dx),
                                     ptr(dgamma), ptr(dbeta), rows, D, float(eps))
+
+
+def bias_grad_member(dz, db):
+    M, N = dz.shape
+    assert tuple(db.shape) == (N,)
+    return opt_bias_grad_member(dz.data_ptr(), _ld(dz), db.data_ptr(), M, N)
 
 
 def chunk(src, dst, op=OPT_PW_COPY, src2=None, params=()):

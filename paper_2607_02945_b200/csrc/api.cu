@@ -113,6 +113,7 @@ static cudaError_t launch_kind(const opt_plan* p, cudaStream_t s) {
     case kPlanLinear2: case kPlanLnLinear2: return launch_linear2(p, s);
     case kPlanLinearSkinny: return launch_linear_skinny(p, s);
     case kPlanLayerNormBwd: return launch_layernorm_bwd(p, s);
+    case kPlanBiasGrad: return launch_bias_grad(p, s);
     default: return cudaErrorInvalidValue;
   }
 }

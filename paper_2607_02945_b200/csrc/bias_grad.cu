@@ -1,0 +1,213 @@
+// batched_bias_grad: the bias gradients of N independent Linear layers in ONE launch (
+// batch_linear_post_grad operates on post-grad graphs, and the headline metric is TRAINING
+// throughput):
+//
+//   db[n] = sum over m of dZ[m, n]            dZ:[M,N] bf16, db:[N] fp32 or bf16
+//
+// Design (HBM-bound: dZ read once, nothing else of size moves):
+//   * a work item is (member, row part, 256-column tile); a 16-byte vector column of the tile is owned by one lane,
+//     the L = 2^k lanes that cover the tile walk a row together (coalesced 16 L-byte segments), the 256/L row
+//     groups of the block stride over the part's rows, four rows of loads in flight per thread;
+//   * fp32 accumulators in registers (packed f32x2 adds); at the end of the part the row groups are summed through
+//     shared memory in group order and the part's partial goes to a plan-owned workspace; the LAST block of a
+//     member (atomic ticket, re-armed by that block) adds the parts in part order and writes db: one launch,
+//     no atomics on data, bitwise reproducible from run to run.
+#include <algorithm>
+#include <cstring>
+
+#include "common.h"
+
+namespace optb {
+
+struct BgMember {
+  const char* dz; char* db;
+  int64_t ldz16;                   // row stride in 16-byte vectors
+  float* ws;                       // [nparts][N] fp32 partial sums (plan workspace)
+  int32_t* ticket;                 // blocks of this member that have finished
+  int32_t rows, nvec, nparts, nblocks;
+  int32_t l_log2;                  // lanes per row of a column tile
+};
+struct BgBlock { int32_t member, row0, nrows, part, vec0; };
+
+constexpr int kBgThreads = 256;
+constexpr int kBgTileVec = 32;       // 32 vectors = 256 bf16 columns per tile
+constexpr int kBgInflight = 4;       // rows of loads in flight per thread
+
+template <bool P_BF16, int LL>
+__device__ __forceinline__ void bg_block(const BgMember& m, const BgBlock& b, float* red) {
+  constexpr int L = 1 << LL;
+  constexpr int rpp = kBgThreads >> LL;
+  const int lane_in_row = threadIdx.x & (L - 1);
+  const int row_in_pass = threadIdx.x >> LL;
+  const int N = m.nvec * 8;
+  const int vec = b.vec0 + lane_in_row;
+  const bool act = vec < m.nvec;
+  const int4* zb = reinterpret_cast<const int4*>(m.dz) + (int64_t)b.row0 * m.ldz16 + vec;
+  f32x2 acc[4] = {0ull, 0ull, 0ull, 0ull};
+  if (act) {
+    int r = row_in_pass;
+    for (; r + (kBgInflight - 1) * rpp < b.nrows; r += kBgInflight * rpp) {
+      int4 v[kBgInflight];
+#pragma unroll
+      for (int j = 0; j < kBgInflight; ++j) v[j] = __ldcs(zb + (int64_t)(r + j * rpp) * m.ldz16);
+#pragma unroll
+      for (int j = 0; j < kBgInflight; ++j) {
+        const uint32_t* u = reinterpret_cast<const uint32_t*>(&v[j]);
+#pragma unroll
+        for (int k = 0; k < 4; ++k) acc[k] = add2(acc[k], bf2_to_f2(u[k]));
+      }
+    }
+    for (; r < b.nrows; r += rpp) {
+      const int4 v = __ldcs(zb + (int64_t)r * m.ldz16);
+      const uint32_t* u = reinterpret_cast<const uint32_t*>(&v);
+#pragma unroll
+      for (int k = 0; k < 4; ++k) acc[k] = add2(acc[k], bf2_to_f2(u[k]));
+    }
+  }
+  // ---- row groups -> shared memory -> group-order sum -> workspace part
+#pragma unroll
+  for (int k = 0; k < 4; ++k) reinterpret_cast<f32x2*>(red + row_in_pass * (L * 8) + lane_in_row * 8)[k] = acc[k];
+  __syncthreads();
+  float* part = m.ws + (size_t)b.part * N;
+  for (int c = threadIdx.x; c < L * 8; c += kBgThreads) {
+    const int col = b.vec0 * 8 + c;
+    if (col < N) {
+      float a = 0.f;
+#pragma unroll 8
+      for (int g = 0; g < rpp; ++g) a += red[g * (L * 8) + c];
+      part[col] = a;
+    }
+  }
+  // ---- last block of the member: add the parts in part order, write db, re-arm the ticket
+  __shared__ int is_last;
+  __threadfence();
+  __syncthreads();
+  if (threadIdx.x == 0) is_last = atomicAdd(m.ticket, 1) == m.nblocks - 1;
+  __syncthreads();
+  if (!is_last) return;
+  __threadfence();
+  for (int c = threadIdx.x; c < N; c += kBgThreads) {
+    float a = 0.f;
+    for (int p = 0; p < m.nparts; ++p) a += __ldcg(m.ws + (size_t)p * N + c);
+    if (P_BF16) reinterpret_cast<__nv_bfloat16*>(m.db)[c] = __float2bfloat16_rn(a);
+    else reinterpret_cast<float*>(m.db)[c] = a;
+  }
+  if (threadIdx.x == 0) *m.ticket = 0;
+}
+
+template <bool P_BF16>
+__global__ void __launch_bounds__(kBgThreads, 6)
+batched_bias_grad_kernel(const BgMember* __restrict__ members, const BgBlock* __restrict__ blocks) {
+  __shared__ __align__(16) float bg_red[kBgThreads * 8];      // [256/L][L*8] floats = 8 KB
+  const BgBlock b = blocks[blockIdx.x];
+  const BgMember m = members[b.member];
+  switch (m.l_log2) {      // block-uniform
+    case 0: bg_block<P_BF16, 0>(m, b, bg_red); break;
+    case 1: bg_block<P_BF16, 1>(m, b, bg_red); break;
+    case 2: bg_block<P_BF16, 2>(m, b, bg_red); break;
+    case 3: bg_block<P_BF16, 3>(m, b, bg_red); break;
+    case 4: bg_block<P_BF16, 4>(m, b, bg_red); break;
+    default: bg_block<P_BF16, 5>(m, b, bg_red); break;
+  }
+}
+
+cudaError_t launch_bias_grad(const opt_plan* p, cudaStream_t s) {
+  const char* base = static_cast<const char*>(p->dev_tables);
+  auto* members = reinterpret_cast<const BgMember*>(base + p->off0);
+  auto* blocks = reinterpret_cast<const BgBlock*>(base + p->off1);
+  if (p->param == OPT_BF16) batched_bias_grad_kernel<true><<<p->grid, p->block, 0, s>>>(members, blocks);
+  else batched_bias_grad_kernel<false><<<p->grid, p->block, 0, s>>>(members, blocks);
+  return cudaGetLastError();
+}
+
+}  // namespace optb
+
+using namespace optb;
+
+extern "C" opt_status opt_bias_grad_plan_create(const opt_bias_grad_member* members, int32_t n, opt_dtype io,
+                                                opt_dtype param, int device, opt_plan** plan) {
+  if (plan) *plan = nullptr;
+  if (!plan || !members) return fail(OPT_ERR_INVALID_ARG, "opt_bias_grad_plan_create: NULL argument");
+  if (n < 1 || n > 65535) return fail(OPT_ERR_INVALID_ARG, "n = %d outside [1, 65535]", n);
+  if ((io != OPT_F32 && io != OPT_BF16) || (param != OPT_F32 && param != OPT_BF16)) return fail(OPT_ERR_INVALID_ARG, "bad dtype");
+  if (io != OPT_BF16) return fail(OPT_ERR_UNSUPPORTED, "the bias gradient is implemented for bf16 activations only");
+  const int pesz = elem_size(param);
+  std::vector<Region> regions;
+  std::vector<BgMember> tab;
+  std::vector<BgBlock> blocks;
+  std::vector<int64_t> ws_off;            // float offset of each member's partials in the workspace
+  int64_t bytes = 0, ws_floats = 0, flops = 0;
+  for (int32_t i = 0; i < n; ++i) {
+    const opt_bias_grad_member& m = members[i];
+    if (!m.dz || !m.db) return fail(OPT_ERR_INVALID_ARG, "member %d: NULL pointer", i);
+    if (m.M < 1 || m.N < 1) return fail(OPT_ERR_INVALID_ARG, "member %d: M=%d N=%d must be >= 1", i, m.M, m.N);
+    if (m.M > 1 && m.ldz < m.N) return fail(OPT_ERR_INVALID_ARG, "member %d: row stride smaller than N", i);
+    if (!aligned16(m.dz) || !aligned16(m.db)) return fail(OPT_ERR_ALIGNMENT, "member %d: pointers must be 16-byte aligned", i);
+    if (m.N % 8) return fail(OPT_ERR_ALIGNMENT, "member %d: N=%d is not a multiple of 8", i, m.N);
+    if (m.M > 1 && m.ldz % 8) return fail(OPT_ERR_ALIGNMENT, "member %d: row stride must be a multiple of 8 elements", i);
+    regions.push_back({(uintptr_t)m.dz, m.ldz * 2, (int64_t)m.N * 2, m.M, false, i});
+    regions.push_back({(uintptr_t)m.db, 0, (int64_t)m.N * pesz, 1, true, i});
+    bytes += (int64_t)m.M * m.N * 2 + (int64_t)m.N * pesz;
+    flops += (int64_t)m.M * m.N;
+    const int nvec = m.N / 8;
+    int ll = 0;
+    while (ll < 5 && (1 << ll) < nvec) ++ll;
+    const int L = 1 << ll, rpp = kBgThreads >> ll;
+    const int nctile = (nvec + kBgTileVec - 1) / kBgTileVec;
+    // rows per block: whole groups of in-flight passes, ~128 KB of dZ per block
+    const int64_t chunk_rows = (int64_t)rpp * kBgInflight;
+    const int64_t rpb = chunk_rows * std::max<int64_t>(1, 131072 / (chunk_rows * L * 16));
+    const int32_t nparts = (int32_t)((m.M + rpb - 1) / rpb);
+    BgMember t;
+    memset(&t, 0, sizeof t);
+    t.dz = (const char*)m.dz; t.db = (char*)m.db; t.ldz16 = m.ldz / 8;
+    t.rows = m.M; t.nvec = nvec; t.nparts = nparts; t.nblocks = nparts * nctile; t.l_log2 = ll;
+    tab.push_back(t);
+    ws_off.push_back(ws_floats);
+    ws_floats += (int64_t)nparts * m.N;
+    for (int32_t part = 0; part < nparts; ++part)
+      for (int32_t ct = 0; ct < nctile; ++ct)
+        blocks.push_back({i, (int32_t)(part * rpb), (int32_t)std::min<int64_t>(rpb, m.M - part * rpb), part, ct * kBgTileVec});
+  }
+  if (opt_status st = check_independent(regions, /*allow_inplace_self=*/false)) return st;
+  if (blocks.size() > (size_t)INT32_MAX) return fail(OPT_ERR_UNSUPPORTED, "too many work items");
+
+  int num_sms = 0;
+  if (opt_status st = open_device(device, &num_sms)) return st;
+  auto align_up = [](size_t x) { return (x + 255) & ~size_t(255); };
+  opt_plan* p = new opt_plan();
+  p->kind = kPlanBiasGrad; p->device = device; p->io = io; p->param = param; p->n_members = n;
+  p->bytes = bytes; p->flops = flops;
+  // workspace: per-part partial column sums (fully written before they are read: no initialisation needed)
+  if (cudaMalloc(&p->workspace, std::max<int64_t>(ws_floats, 1) * sizeof(float)) != cudaSuccess) {
+    cudaGetLastError(); delete p;
+    return fail(OPT_ERR_CUDA, "cudaMalloc of the %lld-byte partial-sum workspace failed", (long long)ws_floats * 4);
+  }
+  p->off0 = 0;
+  p->off1 = align_up(tab.size() * sizeof(BgMember));
+  p->off2 = p->off1 + align_up(blocks.size() * sizeof(BgBlock));
+  const size_t total = p->off2 + align_up((size_t)n * sizeof(int32_t));      // per-member tickets, zero-initialised
+  std::vector<char> blob(total, 0);
+  memcpy(blob.data() + p->off1, blocks.data(), blocks.size() * sizeof(BgBlock));
+  if (cudaMalloc(&p->dev_tables, total) != cudaSuccess) {
+    cudaGetLastError(); cudaFree(p->workspace); delete p;
+    return fail(OPT_ERR_CUDA, "cudaMalloc of the plan tables failed");
+  }
+  p->table_bytes = total;
+  for (int32_t i = 0; i < n; ++i) {
+    tab[i].ws = static_cast<float*>(p->workspace) + ws_off[i];
+    tab[i].ticket = reinterpret_cast<int32_t*>(static_cast<char*>(p->dev_tables) + p->off2) + i;
+  }
+  memcpy(blob.data(), tab.data(), tab.size() * sizeof(BgMember));
+  cudaError_t e = cudaMemcpy(p->dev_tables, blob.data(), total, cudaMemcpyHostToDevice);
+  if (e != cudaSuccess) {
+    cudaFree(p->dev_tables); cudaFree(p->workspace); delete p;
+    return fail(OPT_ERR_CUDA, "plan upload failed: %s", cudaGetErrorString(e));
+  }
+  p->grid = dim3((unsigned)blocks.size());
+  p->block = dim3(kBgThreads);
+  p->smem = 0;
+  p->total_tiles = (int32_t)blocks.size();
+  *plan = p;
+  return OPT_OK;
+}

@@ -51,7 +51,7 @@ struct Region {
 opt_status check_independent(std::vector<Region>& regions, bool allow_inplace_self);
 
 // ---------------------------------------------------------------- the plan --
-enum PlanKind { kPlanPointwise = 1, kPlanLayerNorm = 2, kPlanLinearBf16 = 3, kPlanLinearF32 = 4, kPlanLinear2 = 5, kPlanLayerNormBwd = 6, kPlanLnLinear2 = 7, kPlanLinearSkinny = 8 };
+enum PlanKind { kPlanPointwise = 1, kPlanLayerNorm = 2, kPlanLinearBf16 = 3, kPlanLinearF32 = 4, kPlanLinear2 = 5, kPlanLayerNormBwd = 6, kPlanLnLinear2 = 7, kPlanLinearSkinny = 8, kPlanBiasGrad = 9 };
 
 }  // namespace optb
 
@@ -59,7 +59,7 @@ struct opt_plan {
   int kind = 0;
   int device = 0;
   void* dev_tables = nullptr;   // one device allocation holding every table of the plan
-  void* workspace = nullptr;    // optional scratch owned by the plan (LayerNorm backward: per-block partial sums)
+  void* workspace = nullptr;    // optional scratch owned by the plan (LayerNorm backward / bias gradient: per-block partial sums)
   size_t table_bytes = 0;
   // offsets of sub-tables inside dev_tables (meaning depends on kind)
   size_t off0 = 0, off1 = 0, off2 = 0, off3 = 0;
@@ -84,6 +84,7 @@ cudaError_t launch_linear_skinny(const opt_plan* p, cudaStream_t s);
 bool skinny_linear_member(const opt_linear_member& m);
 opt_status plan_skinny_linear(const opt_linear_member* members, int32_t n, opt_plan* p);
 cudaError_t launch_layernorm_bwd(const opt_plan* p, cudaStream_t s);
+cudaError_t launch_bias_grad(const opt_plan* p, cudaStream_t s);
 
 // host->device upload of a table blob; allocates p->dev_tables
 opt_status upload_tables(opt_plan* p, const void* host_blob, size_t bytes);

@@ -42,6 +42,7 @@ def test_struct_layouts_match_header(ob):
     assert ctypes.sizeof(ob.opt_chunk) == 80
     assert ctypes.sizeof(ob.opt_linear2_member) == 104 and ctypes.sizeof(ob.opt_ln_linear2_member) == 128
     assert ctypes.sizeof(ob.opt_host_copy) == 32
+    assert ctypes.sizeof(ob.opt_bias_grad_member) == 32 and ctypes.sizeof(ob.opt_layernorm_bwd_member) == 88
 
 
 def test_sass_is_blackwell_native():
@@ -146,6 +147,18 @@ def test_host_validation_of_the_next_row_entry_points(ob):
         with pytest.raises(ob.OptError) as e:
             ob.opt_layernorm_bwd_plan_create([member], ob.OPT_BF16)
         assert e.value.status == status, (e.value, status)
+    # bias gradient: N % 8, aligned pointers and strides, db must not lie inside dz, fp32 activations unsupported
+    bgm = lambda **kw: ob.opt_bias_grad_member(**{**dict(dz=A, ldz=64, db=B, M=16, N=64), **kw})
+    for member, io, status in [(bgm(N=60), ob.OPT_BF16, ob.OPT_ERR_ALIGNMENT), (bgm(ldz=68), ob.OPT_BF16, ob.OPT_ERR_ALIGNMENT), (bgm(db=B + 8), ob.OPT_BF16, ob.OPT_ERR_ALIGNMENT),
+                               (bgm(db=A + 128), ob.OPT_BF16, ob.OPT_ERR_ALIAS), (bgm(ldz=32), ob.OPT_BF16, ob.OPT_ERR_INVALID_ARG), (bgm(M=0), ob.OPT_BF16, ob.OPT_ERR_INVALID_ARG),
+                               (bgm(dz=None), ob.OPT_BF16, ob.OPT_ERR_INVALID_ARG), (bgm(), ob.OPT_F32, ob.OPT_ERR_UNSUPPORTED)]:
+        with pytest.raises(ob.OptError) as e:
+            ob.opt_bias_grad_plan_create([member], io)
+        assert e.value.status == status, (e.value, status)
+    if not torch.cuda.is_available():
+        with pytest.raises(ob.OptError) as e:      # valid group: only the device is missing
+            ob.opt_bias_grad_plan_create([bgm()], ob.OPT_BF16, ob.OPT_F32)
+        assert e.value.status == ob.OPT_ERR_NO_DEVICE
     # pointwise: binary op without a second operand, FP8 on fp32 activations, unknown op
     ch = lambda **kw: ob.opt_chunk(**{**dict(src=A, lds=64, dst=B, ldd=64, rows=4, width=64, op=0, src2=None, lds2=0, p0=0.0, p1=0.0, p2=0.0), **kw})
     for chunk, io, status in [(ch(op=ob.OPT_PW_MUL), ob.OPT_BF16, ob.OPT_ERR_INVALID_ARG), (ch(op=ob.OPT_PW_QUANT_E4M3, p0=1.0), ob.OPT_F32, ob.OPT_ERR_UNSUPPORTED),

@@ -1,0 +1,149 @@
+"""GPU parity: batched bias gradient db[n] = sum_m dZ[m, n] of N Linear layers in ONE launch vs the CPU oracle
+(through the C ABI).  SURVEY.md 8(f) rank 3; PAPER.md:292 batch_linear_post_grad, PAPER.md:437 training.
+
+Tolerance (reading Q27): the kernel adds in fp32 along a fixed tree of depth
+d <= rows per thread + row groups + row parts <= 200 for every shape below, so per column
+|db - ref| <= d 2^-24 sum_m |dZ[m, n]| <= 2e-5 sum_m |dZ[m, n]|; a bf16 result adds its own rounding 2^-8 |ref|.
+Sums of small integers are exact: bit for bit."""
+import numpy as np
+import pytest
+import torch
+
+import oracle
+from oracle import graphs
+import workloads as wl
+from util import BF16, F32, empty_dev, row_l2_rel_err, to_dev, to_host, values64
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def ob():
+    import paper_2607_02945_b200 as ob
+    return ob
+
+
+def run(ob, dzs, param_dt, pad=0, launches=1):
+    """dzs: host bf16-bit arrays [M,N]; pad > 0: each is a column slice of a wider device buffer."""
+    dev = []
+    for z in dzs:
+        M, N = z.shape
+        buf = empty_dev((M, N + 2 * pad), BF16, fill=float("nan"))
+        buf[:, pad:pad + N] = to_dev(z, BF16)
+        db = empty_dev((N,), param_dt, fill=float("nan"))
+        dev.append((buf, db))
+    plan = ob.opt_bias_grad_plan_create([ob.bias_grad_member(buf[:, pad:pad + z.shape[1]], db) for (buf, db), z in zip(dev, dzs)],
+                                        BF16, param_dt)
+    outs = []
+    for _ in range(launches):
+        for _, db in dev:
+            db.fill_(float("nan"))
+        n0 = ob.opt_launch_count()
+        plan.launch()
+        torch.cuda.synchronize()
+        assert ob.opt_launch_count() - n0 == 1
+        outs.append([to_host(db) for _, db in dev])
+    return outs, plan
+
+
+def check(got, z, param_dt):
+    ref = graphs.linear_bias_grad(z, BF16)
+    l1 = np.abs(values64(z, BF16)).sum(axis=0)
+    g64 = values64(got, param_dt)
+    bound = 2e-5 * l1 + (2.0 ** -8 * np.abs(ref) if param_dt == BF16 else 0.0)
+    assert np.all(np.abs(g64 - ref) <= bound), float(np.max(np.abs(g64 - ref) - bound))
+
+
+SHAPES = [(300, 512), (77, 200), (1000, 64), (129, 1032), (64, 8), (5, 4096), (1, 24), (100000, 16), (8192, 264), (4097, 40)]
+
+
+@pytest.mark.parametrize("param_dt", [F32, BF16])
+def test_integers_bit_exact(ob, param_dt):
+    rng = np.random.default_rng(61)
+    dzs = [wl.bf16_bits_from_f32(rng.integers(-2, 3, s).astype(np.float32)) for s in SHAPES]
+    (outs,), _ = run(ob, dzs, param_dt)
+    for got, z in zip(outs, dzs):
+        ref = graphs.linear_bias_grad(z, BF16)                 # |sums| <= 2e5 < 2^24: every fp32 partial is exact
+        assert got.tobytes() == oracle.round_to_storage(ref, param_dt).tobytes(), z.shape
+
+
+@pytest.mark.parametrize("param_dt,pad", [(F32, 0), (BF16, 0), (F32, 24)])
+def test_random_group(ob, param_dt, pad):
+    dzs = [wl.tensor_normal(62, i + 1, s, 0.1 * (i % 3), 1.0 + i, BF16) for i, s in enumerate(SHAPES)]
+    outs, _ = run(ob, dzs, param_dt, pad=pad, launches=3)
+    for got, z in zip(outs[0], dzs):
+        check(got, z, param_dt)
+    # fixed summation order + re-armed tickets: every relaunch gives the same bits
+    for again in outs[1:]:
+        for a, b in zip(outs[0], again):
+            assert a.tobytes() == b.tobytes()
+
+
+def test_many_small_members(ob):
+    """300 members of random shape in one launch (ragged tails, 1-row members, several column tiles)."""
+    rng = np.random.default_rng(63)
+    shapes = [(int(rng.integers(1, 700)), 8 * int(rng.integers(1, 80))) for _ in range(300)]
+    dzs = [wl.tensor_normal(63, i + 1, s, 0.0, 1.0, BF16) for i, s in enumerate(shapes)]
+    (outs,), plan = run(ob, dzs, F32)
+    for got, z in zip(outs, dzs):
+        check(got, z, F32)
+    assert plan.info()["bytes"] == sum(z.size * 2 + z.shape[1] * 4 for z in dzs)
+
+
+def test_whole_backward_of_a_linear_relu_group(ob):
+    """Forward Y_i = relu(X_i W_i^T + b_i) (one launch) and the whole backward in four launches -- ReLU masks, bias
+    gradients, dgrads, wgrads -- against graphs.linear_relu_backward, which runs its OWN forward in fp64 (no oracle
+    input comes from the CUDA path).  The two forwards may disagree in the sign of a pre-activation that is zero to
+    rounding, so the masks are compared as sets: <= 1e-4 of the elements may differ."""
+    members = []
+    for i, (M, N, K) in enumerate([(300, 128, 64), (512, 64, 256), (1000, 256, 128), (257, 136, 72)]):
+        members.append(dict(x=wl.tensor_normal(8, 4 * i + 1, (M, K), 0, 1, BF16), w=wl.tensor_normal(8, 4 * i + 2, (N, K), 0, K ** -0.5, BF16),
+                            b=wl.tensor_normal(8, 4 * i + 3, (N,), 0, 0.1, BF16), g=wl.tensor_normal(8, 4 * i + 4, (M, N), 0, 1, BF16)))
+    dev, fwd, msk, bg, dg, wg = [], [], [], [], [], []
+    for m in members:
+        (M, K), N = m["x"].shape, m["w"].shape[0]
+        x, w, b, g = (to_dev(m[k], BF16) for k in ("x", "w", "b", "g"))
+        y, dz = empty_dev((M, N), BF16), empty_dev((M, N), BF16, fill=float("nan"))
+        dx, dw, db = empty_dev((M, K), BF16, fill=float("nan")), empty_dev((N, K), BF16, fill=float("nan")), empty_dev((N,), F32, fill=float("nan"))
+        dev.append((x, w, b, g, y, dz, dx, dw, db))
+        fwd.append(ob.linear_member(x, w, b, y, ob.OPT_ACT_RELU))
+        msk.append(ob.chunk(g, dz, ob.OPT_PW_RELU_BWD, y))
+        bg.append(ob.bias_grad_member(dz, db))
+        dg.append(ob.linear_member(dz, w, None, dx, 0, ob.OPT_LAYOUT_W_TRANSPOSED))
+        wg.append(ob.linear_member(dz, x, None, dw, 0, ob.OPT_LAYOUT_X_TRANSPOSED | ob.OPT_LAYOUT_W_TRANSPOSED))
+    n0 = ob.opt_launch_count()
+    ob.opt_linear_plan_create(fwd, BF16).launch()
+    ob.opt_pointwise_plan_create(msk, BF16).launch()
+    ob.opt_bias_grad_plan_create(bg, BF16, F32).launch()
+    ob.opt_linear_plan_create(dg, BF16).launch()
+    ob.opt_linear_plan_create(wg, BF16).launch()
+    torch.cuda.synchronize()
+    assert ob.opt_launch_count() - n0 == 5
+    for m, d in zip(members, dev):
+        r = graphs.linear_relu_backward(m, m["g"], BF16)
+        dz = to_host(d[5])
+        assert np.mean(dz != r["dz"]) <= 1e-4
+        assert 0.2 < np.mean(dz == 0) < 0.8
+        l1 = np.abs(values64(r["dz"], BF16)).sum(axis=0)
+        gmax = np.abs(values64(m["g"], BF16)).max()
+        nflip = int((dz != r["dz"]).sum())
+        assert np.all(np.abs(to_host(d[8]).astype(np.float64) - r["db64"]) <= 2e-5 * l1 + nflip * gmax)
+        if nflip == 0:
+            assert row_l2_rel_err(to_host(d[6]), r["dx64"], BF16) <= 1e-2
+            assert row_l2_rel_err(to_host(d[7]), r["dw64"], BF16) <= 1e-2
+
+
+def test_full_size_c2_bias_grads(ob):
+    """configs[2] at full size, the launch bench.py times: the 128 members' gradients are column slices of ONE
+    [4096, sum N] concat buffer.  Oracle on every column of 16 sampled members."""
+    M, Ns = 4096, [int(n) for n in np.random.default_rng(64).choice([128, 256, 512, 1024], size=128)]      # configs[2]'s recipe
+    off = np.concatenate([[0], np.cumsum(Ns)])
+    gen = torch.Generator(device="cuda").manual_seed(64)
+    dy_cat = torch.empty((M, int(off[-1])), dtype=torch.bfloat16, device="cuda").normal_(0.0, 1.0, generator=gen)
+    dbs = [torch.full((n,), float("nan"), dtype=torch.float32, device="cuda") for n in Ns]
+    plan = ob.opt_bias_grad_plan_create([ob.bias_grad_member(dy_cat[:, off[i]:off[i + 1]], dbs[i]) for i in range(len(Ns))], BF16, F32)
+    plan.launch()
+    torch.cuda.synchronize()
+    for i in list(range(0, len(Ns), 9)) + [len(Ns) - 1]:
+        z = to_host(dy_cat[:, off[i]:off[i + 1]])
+        check(to_host(dbs[i]), z, F32)
