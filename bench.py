@@ -499,6 +499,7 @@ def run_side(args):
       --side ln_linear2  the whole C4 block (LayerNorm folded into the chain, opt_ln_linear2) as one launch
       --side skinny    the paper's four skinny aten.mm as one group (streaming row kernel)
       --side fp8       configs[4]'s saved LayerNorm outputs -> FP8 E4M3 and back (one launch each)
+      --side bias_grad the 512 bias gradients of configs[4]'s Linear+ReLU group (column sums of [8192, H]), one launch
       --side lhs       batch_linear_lhs: 8 members (N=64) on ONE input X [262144, 512]; OPT_GEMM_NO_LHS=1 = plain order
     Prints one JSON line; not the bench metric."""
     import torch
@@ -549,6 +550,28 @@ def run_side(args):
         plan.launch()
         torch.cuda.synchronize()
         print(json.dumps(dict(side="skinny", us=round(timed(plan.launch, 3), 1), **plan.info())))
+    elif args.side == "bias_grad":
+        rng = np.random.default_rng(4)
+        hs = [int(h) for h in rng.choice([128, 256, 512], size=512)]                          # configs[4]'s hidden widths
+        dz = [torch.randn(8192, h, device="cuda", dtype=torch.bfloat16) for h in hs]
+        db = [torch.empty(h, device="cuda", dtype=torch.float32) for h in hs]
+        plan = ob.opt_bias_grad_plan_create([ob.bias_grad_member(z, d) for z, d in zip(dz, db)], BF16, ob.OPT_F32, 0)
+        plan.launch()
+        torch.cuda.synchronize()
+        res = dict(side="bias_grad", us=round(timed(plan.launch, 5), 1), **plan.info())
+        # the ReLU mask fused in front: dZ = dY where y > 0, written once and summed in the same pass (3 M N elements of
+        # traffic) against the two-launch path OPT_PW_RELU_BWD + bias gradient (4 M N)
+        ys = [torch.randn(8192, h, device="cuda", dtype=torch.bfloat16).clamp_(min=0) for h in hs]
+        outs = [torch.empty_like(z) for z in dz]
+        pf = ob.opt_bias_grad_plan_create([ob.bias_grad_member(z, d, y, o) for z, d, y, o in zip(dz, db, ys, outs)], BF16, ob.OPT_F32, 0)
+        pm = ob.opt_pointwise_plan_create([ob.chunk(z, o, ob.OPT_PW_RELU_BWD, y) for z, y, o in zip(dz, ys, outs)], BF16, 0)
+        pb2 = ob.opt_bias_grad_plan_create([ob.bias_grad_member(o, d) for o, d in zip(outs, db)], BF16, ob.OPT_F32, 0)
+        pf.launch(); pm.launch(); pb2.launch()
+        torch.cuda.synchronize()
+        res.update(fused_mask_us=round(timed(pf.launch, 5), 1), fused_mask_bytes=pf.info()["bytes"],
+                   two_launch_us=round(timed(lambda: (pm.launch(), pb2.launch()), 5), 1),
+                   two_launch_bytes=pm.info()["bytes"] + pb2.info()["bytes"])
+        print(json.dumps(res))
     elif args.side == "fp8":
         step = Step("cuda:0", FULL, pinned_host=False, configs=("c4",))
         ga = step.groups[0]
@@ -854,7 +877,8 @@ def run_product(args):
             pb.launch()
             torch.cuda.synchronize()
             tb_ = cold2(pb.launch)
-            backward.update(bias_grad_us=round(tb_, 1), bias_grad_gbs=round(pb.info()["bytes"] / tb_ / 1e3, 1),
+            backward.update(bias_grad_workload="configs[2]: 128 bias gradients db = column sums of the members' slices of the [4096, sum N] concat gradient, one launch",
+                            bias_grad_us=round(tb_, 1), bias_grad_gbs=round(pb.info()["bytes"] / tb_ / 1e3, 1),
                             bias_grad_frac_hbm=round(pb.info()["bytes"] / tb_ / 1e3 / peaks["hbm_gbs"], 4))
             del dbs
             # LayerNorm backward of C4a's 512 members (dx, dgamma, dbeta), one launch
@@ -877,6 +901,32 @@ def run_product(args):
                                 layernorm_bwd_us=round(tl, 1), layernorm_bwd_gbs=round(il["bytes"] / tl / 1e3, 1),
                                 layernorm_bwd_frac_hbm=round(il["bytes"] / tl / 1e3 / peaks["hbm_gbs"], 4))
                 del keep2
+                # bias gradients of C4b's 512 Linear+ReLU members: column sums of a [B, H] gradient per member (the hidden
+                # tensors stand in for dH: same shapes and layout), one launch
+                db4 = [torch.empty(ga.amid.tensor(i["h"]).shape[1], dtype=torch.float32, device=device) for i in ga.idx]
+                pb4 = ob.opt_bias_grad_plan_create([ob.bias_grad_member(ga.amid.tensor(i["h"]), d) for i, d in zip(ga.idx, db4)],
+                                                   BF16, ob.OPT_F32, step.dev_index)
+                pb4.launch()
+                torch.cuda.synchronize()
+                tb4 = cold2(pb4.launch)
+                backward.update(bias_grad_c4_workload="configs[4] Linear+ReLU group: 512 bias gradients db = column sums of [8192, H], one launch",
+                                bias_grad_c4_us=round(tb4, 1), bias_grad_c4_gbs=round(pb4.info()["bytes"] / tb4 / 1e3, 1),
+                                bias_grad_c4_frac_hbm=round(pb4.info()["bytes"] / tb4 / 1e3 / peaks["hbm_gbs"], 4))
+                # the same with the ReLU mask fused in front (dZ = dH-gradient where h > 0, written once, summed in the same pass)
+                # against OPT_PW_RELU_BWD followed by the plain bias gradient
+                gh = [torch.empty_like(ga.amid.tensor(i["h"])).normal_(0.0, 1.0) for i in ga.idx]
+                dzs = [torch.empty_like(g_) for g_ in gh]
+                pf4 = ob.opt_bias_grad_plan_create([ob.bias_grad_member(g_, d, ga.amid.tensor(i["h"]), z) for g_, d, i, z in zip(gh, db4, ga.idx, dzs)],
+                                                   BF16, ob.OPT_F32, step.dev_index)
+                pm4 = ob.opt_pointwise_plan_create([ob.chunk(g_, z, ob.OPT_PW_RELU_BWD, ga.amid.tensor(i["h"])) for g_, i, z in zip(gh, ga.idx, dzs)], BF16, step.dev_index)
+                pz4 = ob.opt_bias_grad_plan_create([ob.bias_grad_member(z, d) for z, d in zip(dzs, db4)], BF16, ob.OPT_F32, step.dev_index)
+                pf4.launch(); pm4.launch(); pz4.launch()
+                torch.cuda.synchronize()
+                tf4, tm4 = cold2(pf4.launch), cold2(lambda: (pm4.launch(), pz4.launch()))
+                backward.update(relu_mask_bias_grad_fused_us=round(tf4, 1), relu_mask_bias_grad_fused_gbs=round(pf4.info()["bytes"] / tf4 / 1e3, 1),
+                                relu_mask_bias_grad_fused_frac_hbm=round(pf4.info()["bytes"] / tf4 / 1e3 / peaks["hbm_gbs"], 4),
+                                relu_mask_then_bias_grad_two_launches_us=round(tm4, 1))
+                del db4, pb4, gh, dzs, pf4, pm4, pz4
                 # activation_quantization_aten_pass: the 512 saved LayerNorm outputs -> FP8 E4M3 and back, one launch each
                 A = ga.amid.tensor
                 q8 = [torch.empty(A(i["xn"]).shape, dtype=torch.uint8, device=device) for i in ga.idx]
@@ -1032,7 +1082,7 @@ def main():
     ap.add_argument("--profile", action="store_true",
                     help="only the step's own launches (no cpu_baseline, no unfused baseline, no copy reference): for ncu")
     ap.add_argument("--ref-frac", type=float, default=0.0, help="reference arm: override the row-sample fraction")
-    ap.add_argument("--side", default=None, choices=["linear2", "ln_linear2", "lhs", "skinny", "fp8"], help="stand-alone side workload for ncu (not the metric)")
+    ap.add_argument("--side", default=None, choices=["linear2", "ln_linear2", "lhs", "skinny", "fp8", "bias_grad"], help="stand-alone side workload for ncu (not the metric)")
     args = ap.parse_args()
     if args.side:
         return run_side(args)

@@ -215,12 +215,23 @@ typedef struct {
  * dz:[M,N] (ldz, elements; a column slice of a concat buffer is fine), db:[N] in the param dtype (device
  * pointers, caller-owned).  bf16 activations, N % 8 == 0, 16-byte aligned pointers, ldz % 8 == 0 (else
  * OPT_ERR_ALIGNMENT).  fp32 accumulation; rows are added in a fixed order (row groups, then row parts, through a
- * plan-owned workspace): bitwise reproducible, no atomics on data.  opt_plan_info: flops = M N adds, bytes = dZ + db. */
+ * plan-owned workspace): bitwise reproducible, no atomics on data.  opt_plan_info: flops = M N adds, bytes = dZ + db.
+ *
+ * Fused ReLU mask (y != NULL; zero-initialise the struct otherwise): dz then holds the gradient dY that arrives at the
+ * ReLU epilogue, y:[M,N] (ldy) the STORED forward output, and the member computes, in the same pass,
+ *     dZ[m, n] = (y[m, n] <= 0) ? +0 : dY[m, n]      (torch threshold_backward == OPT_PW_RELU_BWD, bit-exact)
+ *     db[n]    = sum over m of dZ[m, n]
+ * dZ is written to dz_out:[M,N] (lddz_out) unless dz_out is NULL; dz_out == dz with lddz_out == ldz (in place) is
+ * allowed.  y and dz_out follow the alignment rules of dz.                                                          */
 typedef struct {
   const void* dz;
   int64_t ldz;
   void* db;
   int32_t M, N;
+  const void* y;
+  int64_t ldy;
+  void* dz_out;
+  int64_t lddz_out;
 } opt_bias_grad_member;
 
 /* One chunk of a multi-tensor pointwise / split-cat pass -- batch_relu,

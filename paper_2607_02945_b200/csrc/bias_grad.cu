@@ -4,6 +4,10 @@
 //
 //   db[n] = sum over m of dZ[m, n]            dZ:[M,N] bf16, db:[N] fp32 or bf16
 //
+// and, when a member names the stored forward output y of a ReLU epilogue, the mask of that ReLU fused in front
+// (vertical fusion inside the backward): dZ = dY where y > 0 else 0 is formed in registers from dY and
+// y, written once (dz_out, optional) and summed in the same pass -- 3 M N instead of 4 M N elements of HBM traffic.
+//
 // Design (HBM-bound: dZ read once, nothing else of size moves):
 //   * a work item is (member, row part, 256-column tile); a 16-byte vector column of the tile is owned by one lane,
 //     the L = 2^k lanes that cover the tile walk a row together (coalesced 16 L-byte segments), the 256/L row
@@ -21,7 +25,8 @@ namespace optb {
 
 struct BgMember {
   const char* dz; char* db;
-  int64_t ldz16;                   // row stride in 16-byte vectors
+  const char* y; char* dzo;        // fused ReLU mask: stored forward output, masked gradient out (either may be NULL)
+  int64_t ldz16, ldy16, lddzo16;   // row strides in 16-byte vectors
   float* ws;                       // [nparts][N] fp32 partial sums (plan workspace)
   int32_t* ticket;                 // blocks of this member that have finished
   int32_t rows, nvec, nparts, nblocks;
@@ -31,9 +36,29 @@ struct BgBlock { int32_t member, row0, nrows, part, vec0; };
 
 constexpr int kBgThreads = 256;
 constexpr int kBgTileVec = 32;       // 32 vectors = 256 bf16 columns per tile
-constexpr int kBgInflight = 4;       // rows of loads in flight per thread
+#ifndef BG_INFLIGHT
+#define BG_INFLIGHT 4
+#endif
+#ifndef BG_BLOCK_BYTES
+#define BG_BLOCK_BYTES 131072
+#endif
+#ifndef BG_MINBLOCKS
+#define BG_MINBLOCKS 6
+#endif
+constexpr int kBgInflight = BG_INFLIGHT;       // rows of loads in flight per thread
 
-template <bool P_BF16, int LL>
+// torch threshold_backward on a bf16 pair: keep the gradient unless y <= 0 (a NaN y keeps it); the zero written is +0
+__device__ __forceinline__ uint32_t bg_mask2(uint32_t g, uint32_t y) {
+  const uint32_t m = (bf16_lo(y) <= 0.f ? 0u : 0x0000FFFFu) | (bf16_hi(y) <= 0.f ? 0u : 0xFFFF0000u);
+  return g & m;
+}
+__device__ __forceinline__ int4 bg_mask(int4 g, const int4& y) {
+  g.x = (int)bg_mask2((uint32_t)g.x, (uint32_t)y.x); g.y = (int)bg_mask2((uint32_t)g.y, (uint32_t)y.y);
+  g.z = (int)bg_mask2((uint32_t)g.z, (uint32_t)y.z); g.w = (int)bg_mask2((uint32_t)g.w, (uint32_t)y.w);
+  return g;
+}
+
+template <bool P_BF16, int LL, bool MASK>
 __device__ __forceinline__ void bg_block(const BgMember& m, const BgBlock& b, float* red) {
   constexpr int L = 1 << LL;
   constexpr int rpp = kBgThreads >> LL;
@@ -45,20 +70,33 @@ __device__ __forceinline__ void bg_block(const BgMember& m, const BgBlock& b, fl
   const int4* zb = reinterpret_cast<const int4*>(m.dz) + (int64_t)b.row0 * m.ldz16 + vec;
   f32x2 acc[4] = {0ull, 0ull, 0ull, 0ull};
   if (act) {
+    const int4* yb = MASK ? reinterpret_cast<const int4*>(m.y) + (int64_t)b.row0 * m.ldy16 + vec : nullptr;
+    int4* ob = MASK && m.dzo ? reinterpret_cast<int4*>(m.dzo) + (int64_t)b.row0 * m.lddzo16 + vec : nullptr;
     int r = row_in_pass;
     for (; r + (kBgInflight - 1) * rpp < b.nrows; r += kBgInflight * rpp) {
-      int4 v[kBgInflight];
-#pragma unroll
-      for (int j = 0; j < kBgInflight; ++j) v[j] = __ldcs(zb + (int64_t)(r + j * rpp) * m.ldz16);
+      int4 v[kBgInflight], y[MASK ? kBgInflight : 1];
 #pragma unroll
       for (int j = 0; j < kBgInflight; ++j) {
+        v[j] = __ldcs(zb + (int64_t)(r + j * rpp) * m.ldz16);
+        if (MASK) y[j] = __ldcs(yb + (int64_t)(r + j * rpp) * m.ldy16);
+      }
+#pragma unroll
+      for (int j = 0; j < kBgInflight; ++j) {
+        if (MASK) {
+          v[j] = bg_mask(v[j], y[j]);
+          if (ob) __stcs(ob + (int64_t)(r + j * rpp) * m.lddzo16, v[j]);
+        }
         const uint32_t* u = reinterpret_cast<const uint32_t*>(&v[j]);
 #pragma unroll
         for (int k = 0; k < 4; ++k) acc[k] = add2(acc[k], bf2_to_f2(u[k]));
       }
     }
     for (; r < b.nrows; r += rpp) {
-      const int4 v = __ldcs(zb + (int64_t)r * m.ldz16);
+      int4 v = __ldcs(zb + (int64_t)r * m.ldz16);
+      if (MASK) {
+        v = bg_mask(v, __ldcs(yb + (int64_t)r * m.ldy16));
+        if (ob) __stcs(ob + (int64_t)r * m.lddzo16, v);
+      }
       const uint32_t* u = reinterpret_cast<const uint32_t*>(&v);
 #pragma unroll
       for (int k = 0; k < 4; ++k) acc[k] = add2(acc[k], bf2_to_f2(u[k]));
@@ -95,19 +133,32 @@ __device__ __forceinline__ void bg_block(const BgMember& m, const BgBlock& b, fl
   if (threadIdx.x == 0) *m.ticket = 0;
 }
 
-template <bool P_BF16>
-__global__ void __launch_bounds__(kBgThreads, 6)
+// Two instantiations chosen per plan: groups without a fused mask run 6 blocks per SM in 40 registers; a masked member
+// keeps twice the vectors in flight (dY and y) and needs 64 registers (4 blocks per SM) to stay out of local memory.
+template <bool P_BF16, bool ANY_MASK>
+__global__ void __launch_bounds__(kBgThreads, ANY_MASK ? 4 : BG_MINBLOCKS)
 batched_bias_grad_kernel(const BgMember* __restrict__ members, const BgBlock* __restrict__ blocks) {
   __shared__ __align__(16) float bg_red[kBgThreads * 8];      // [256/L][L*8] floats = 8 KB
   const BgBlock b = blocks[blockIdx.x];
   const BgMember m = members[b.member];
-  switch (m.l_log2) {      // block-uniform
-    case 0: bg_block<P_BF16, 0>(m, b, bg_red); break;
-    case 1: bg_block<P_BF16, 1>(m, b, bg_red); break;
-    case 2: bg_block<P_BF16, 2>(m, b, bg_red); break;
-    case 3: bg_block<P_BF16, 3>(m, b, bg_red); break;
-    case 4: bg_block<P_BF16, 4>(m, b, bg_red); break;
-    default: bg_block<P_BF16, 5>(m, b, bg_red); break;
+  if (!ANY_MASK || m.y == nullptr) {     // block-uniform
+    switch (m.l_log2) {
+      case 0: bg_block<P_BF16, 0, false>(m, b, bg_red); break;
+      case 1: bg_block<P_BF16, 1, false>(m, b, bg_red); break;
+      case 2: bg_block<P_BF16, 2, false>(m, b, bg_red); break;
+      case 3: bg_block<P_BF16, 3, false>(m, b, bg_red); break;
+      case 4: bg_block<P_BF16, 4, false>(m, b, bg_red); break;
+      default: bg_block<P_BF16, 5, false>(m, b, bg_red); break;
+    }
+  } else {
+    switch (m.l_log2) {
+      case 0: bg_block<P_BF16, 0, true>(m, b, bg_red); break;
+      case 1: bg_block<P_BF16, 1, true>(m, b, bg_red); break;
+      case 2: bg_block<P_BF16, 2, true>(m, b, bg_red); break;
+      case 3: bg_block<P_BF16, 3, true>(m, b, bg_red); break;
+      case 4: bg_block<P_BF16, 4, true>(m, b, bg_red); break;
+      default: bg_block<P_BF16, 5, true>(m, b, bg_red); break;
+    }
   }
 }
 
@@ -115,8 +166,14 @@ cudaError_t launch_bias_grad(const opt_plan* p, cudaStream_t s) {
   const char* base = static_cast<const char*>(p->dev_tables);
   auto* members = reinterpret_cast<const BgMember*>(base + p->off0);
   auto* blocks = reinterpret_cast<const BgBlock*>(base + p->off1);
-  if (p->param == OPT_BF16) batched_bias_grad_kernel<true><<<p->grid, p->block, 0, s>>>(members, blocks);
-  else batched_bias_grad_kernel<false><<<p->grid, p->block, 0, s>>>(members, blocks);
+  const bool any_mask = p->nstages != 0;      // stored in nstages
+  if (p->param == OPT_BF16) {
+    if (any_mask) batched_bias_grad_kernel<true, true><<<p->grid, p->block, 0, s>>>(members, blocks);
+    else batched_bias_grad_kernel<true, false><<<p->grid, p->block, 0, s>>>(members, blocks);
+  } else {
+    if (any_mask) batched_bias_grad_kernel<false, true><<<p->grid, p->block, 0, s>>>(members, blocks);
+    else batched_bias_grad_kernel<false, false><<<p->grid, p->block, 0, s>>>(members, blocks);
+  }
   return cudaGetLastError();
 }
 
@@ -145,9 +202,17 @@ extern "C" opt_status opt_bias_grad_plan_create(const opt_bias_grad_member* memb
     if (!aligned16(m.dz) || !aligned16(m.db)) return fail(OPT_ERR_ALIGNMENT, "member %d: pointers must be 16-byte aligned", i);
     if (m.N % 8) return fail(OPT_ERR_ALIGNMENT, "member %d: N=%d is not a multiple of 8", i, m.N);
     if (m.M > 1 && m.ldz % 8) return fail(OPT_ERR_ALIGNMENT, "member %d: row stride must be a multiple of 8 elements", i);
+    if (m.dz_out && !m.y) return fail(OPT_ERR_INVALID_ARG, "member %d: dz_out without y (the mask source)", i);
+    if (m.y) {
+      if (!aligned16(m.y) || !aligned16(m.dz_out)) return fail(OPT_ERR_ALIGNMENT, "member %d: pointers must be 16-byte aligned", i);
+      if (m.M > 1 && (m.ldy < m.N || (m.dz_out && m.lddz_out < m.N))) return fail(OPT_ERR_INVALID_ARG, "member %d: row stride smaller than N", i);
+      if (m.M > 1 && (m.ldy % 8 || (m.dz_out && m.lddz_out % 8))) return fail(OPT_ERR_ALIGNMENT, "member %d: row stride must be a multiple of 8 elements", i);
+      regions.push_back({(uintptr_t)m.y, m.ldy * 2, (int64_t)m.N * 2, m.M, false, i});
+      if (m.dz_out) regions.push_back({(uintptr_t)m.dz_out, m.lddz_out * 2, (int64_t)m.N * 2, m.M, true, i});
+    }
     regions.push_back({(uintptr_t)m.dz, m.ldz * 2, (int64_t)m.N * 2, m.M, false, i});
     regions.push_back({(uintptr_t)m.db, 0, (int64_t)m.N * pesz, 1, true, i});
-    bytes += (int64_t)m.M * m.N * 2 + (int64_t)m.N * pesz;
+    bytes += (int64_t)m.M * m.N * 2 * (1 + (m.y ? 1 : 0) + (m.dz_out ? 1 : 0)) + (int64_t)m.N * pesz;
     flops += (int64_t)m.M * m.N;
     const int nvec = m.N / 8;
     int ll = 0;
@@ -156,11 +221,12 @@ extern "C" opt_status opt_bias_grad_plan_create(const opt_bias_grad_member* memb
     const int nctile = (nvec + kBgTileVec - 1) / kBgTileVec;
     // rows per block: whole groups of in-flight passes, ~128 KB of dZ per block
     const int64_t chunk_rows = (int64_t)rpp * kBgInflight;
-    const int64_t rpb = chunk_rows * std::max<int64_t>(1, 131072 / (chunk_rows * L * 16));
+    const int64_t rpb = chunk_rows * std::max<int64_t>(1, BG_BLOCK_BYTES / (chunk_rows * L * 16));
     const int32_t nparts = (int32_t)((m.M + rpb - 1) / rpb);
     BgMember t;
     memset(&t, 0, sizeof t);
     t.dz = (const char*)m.dz; t.db = (char*)m.db; t.ldz16 = m.ldz / 8;
+    t.y = (const char*)m.y; t.dzo = (char*)m.dz_out; t.ldy16 = m.ldy / 8; t.lddzo16 = m.lddz_out / 8;
     t.rows = m.M; t.nvec = nvec; t.nparts = nparts; t.nblocks = nparts * nctile; t.l_log2 = ll;
     tab.push_back(t);
     ws_off.push_back(ws_floats);
@@ -169,7 +235,7 @@ extern "C" opt_status opt_bias_grad_plan_create(const opt_bias_grad_member* memb
       for (int32_t ct = 0; ct < nctile; ++ct)
         blocks.push_back({i, (int32_t)(part * rpb), (int32_t)std::min<int64_t>(rpb, m.M - part * rpb), part, ct * kBgTileVec});
   }
-  if (opt_status st = check_independent(regions, /*allow_inplace_self=*/false)) return st;
+  if (opt_status st = check_independent(regions, /*allow_inplace_self=*/true)) return st;
   if (blocks.size() > (size_t)INT32_MAX) return fail(OPT_ERR_UNSUPPORTED, "too many work items");
 
   int num_sms = 0;
@@ -207,6 +273,8 @@ extern "C" opt_status opt_bias_grad_plan_create(const opt_bias_grad_member* memb
   p->grid = dim3((unsigned)blocks.size());
   p->block = dim3(kBgThreads);
   p->smem = 0;
+  p->nstages = 0;
+  for (const BgMember& t : tab) if (t.y) p->nstages = 1;
   p->total_tiles = (int32_t)blocks.size();
   *plan = p;
   return OPT_OK;

@@ -90,9 +90,45 @@ def test_many_small_members(ob):
     assert plan.info()["bytes"] == sum(z.size * 2 + z.shape[1] * 4 for z in dzs)
 
 
-def test_whole_backward_of_a_linear_relu_group(ob):
+def test_fused_relu_mask(ob):
+    """y given: dZ = dY where y > 0 (torch threshold_backward: a NaN y keeps the gradient, -0 and +0 cut it) formed,
+    written and summed in one pass.  dz_out bit-exact against the oracle's pointwise op 11; db within the summation
+    bound of the oracle's column sums of that dZ.  Members: separate dz_out, slices of wider buffers, in place,
+    and no dz_out at all."""
+    devs, descs, host = [], [], []
+    for i, (M, N) in enumerate(SHAPES):
+        g = wl.tensor_normal(65, 2 * i + 1, (M, N), 0.0, 2.0, BF16)
+        y = wl.tensor_normal(65, 2 * i + 2, (M, N), 0.0, 1.0, BF16).copy()
+        y[(y & 0x8000) != 0] = 0x8000 if i % 2 else 0x0000        # what a ReLU leaves: 0 (or -0) where x <= 0
+        y.reshape(-1)[::53] = 0x8000
+        y.reshape(-1)[7::211] = 0x7FC0                            # NaN forward value
+        pad = 24 if i % 2 else 0
+        dg = to_dev(np.pad(g, ((0, 0), (0, pad))), BF16)[:, :N]
+        dy = to_dev(np.pad(y, ((0, 0), (8, pad))), BF16)[:, 8:8 + N]
+        mode = i % 3                                              # 0: separate output, 1: in place, 2: no output
+        out = empty_dev((M, N + pad), BF16, fill=float("nan"))[:, :N] if mode == 0 else (dg if mode == 1 else None)
+        db = empty_dev((N,), F32, fill=float("nan"))
+        descs.append(ob.bias_grad_member(dg, db, dy, out))
+        devs.append((dg, dy, out, db)); host.append((g, y, mode))
+    plan = ob.opt_bias_grad_plan_create(descs, BF16, F32)
+    n0 = ob.opt_launch_count()
+    plan.launch()
+    torch.cuda.synchronize()
+    assert ob.opt_launch_count() - n0 == 1
+    for (dg, dy, out, db), (g, y, mode) in zip(devs, host):
+        ref = oracle.round_to_storage(oracle.pointwise_ext(g, y, oracle.PW_RELU_BWD, [], BF16), BF16)
+        if out is not None:
+            assert to_host(out).tobytes() == ref.tobytes(), (g.shape, mode)
+        else:
+            assert to_host(dg).tobytes() == g.tobytes()            # inputs untouched
+        check(to_host(db), ref, F32)
+    assert plan.info()["bytes"] == sum(g.size * 2 * (3 if mode < 2 else 2) + g.shape[1] * 4 for g, _, mode in host)
+
+
+@pytest.mark.parametrize("fused", [False, True])
+def test_whole_backward_of_a_linear_relu_group(ob, fused):
     """Forward Y_i = relu(X_i W_i^T + b_i) (one launch) and the whole backward in four launches -- ReLU masks, bias
-    gradients, dgrads, wgrads -- against graphs.linear_relu_backward, which runs its OWN forward in fp64 (no oracle
+    gradients, dgrads, wgrads (three with the mask fused into the bias-gradient launch) -- against graphs.linear_relu_backward, which runs its OWN forward in fp64 (no oracle
     input comes from the CUDA path).  The two forwards may disagree in the sign of a pre-activation that is zero to
     rounding, so the masks are compared as sets: <= 1e-4 of the elements may differ."""
     members = []
@@ -108,17 +144,18 @@ def test_whole_backward_of_a_linear_relu_group(ob):
         dev.append((x, w, b, g, y, dz, dx, dw, db))
         fwd.append(ob.linear_member(x, w, b, y, ob.OPT_ACT_RELU))
         msk.append(ob.chunk(g, dz, ob.OPT_PW_RELU_BWD, y))
-        bg.append(ob.bias_grad_member(dz, db))
+        bg.append(ob.bias_grad_member(g, db, y, dz) if fused else ob.bias_grad_member(dz, db))
         dg.append(ob.linear_member(dz, w, None, dx, 0, ob.OPT_LAYOUT_W_TRANSPOSED))
         wg.append(ob.linear_member(dz, x, None, dw, 0, ob.OPT_LAYOUT_X_TRANSPOSED | ob.OPT_LAYOUT_W_TRANSPOSED))
     n0 = ob.opt_launch_count()
     ob.opt_linear_plan_create(fwd, BF16).launch()
-    ob.opt_pointwise_plan_create(msk, BF16).launch()
-    ob.opt_bias_grad_plan_create(bg, BF16, F32).launch()
+    if not fused:
+        ob.opt_pointwise_plan_create(msk, BF16).launch()
+    ob.opt_bias_grad_plan_create(bg, BF16, F32).launch()       # fused: the mask is formed, written and summed here
     ob.opt_linear_plan_create(dg, BF16).launch()
     ob.opt_linear_plan_create(wg, BF16).launch()
     torch.cuda.synchronize()
-    assert ob.opt_launch_count() - n0 == 5
+    assert ob.opt_launch_count() - n0 == (4 if fused else 5)
     for m, d in zip(members, dev):
         r = graphs.linear_relu_backward(m, m["g"], BF16)
         dz = to_host(d[5])
