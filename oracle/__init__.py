@@ -135,13 +135,16 @@ def pointwise(src, op, dt):
 
 PW_CLAMP, PW_NAN_TO_NUM, PW_SUB, PW_DIV, PW_MUL = 4, 5, 6, 7, 8
 PW_RELU_BWD = 11
+PW_TANH_BWD = 12
+PW_SIGMOID_BWD = 13
 
 
 def pointwise_ext(a, b, op, params, dt):
     """Table-1 pointwise patterns beyond relu/tanh/sigmoid, fp64, torch semantics:
     op 4 clamp(a, lo=params[0], hi=params[1]); op 5 nan_to_num(a, nan=params[0], posinf=params[1],
     neginf=params[2]); op 6/7/8 a - b, a / b, a * b; op 11 ReLU backward: a where b > 0 (or b is NaN), else 0
-    (a = incoming gradient, b = the ReLU's output or input).  Parameters are the fp32 values the descriptor carries."""
+    (a = incoming gradient, b = the ReLU's output or input); op 12 tanh backward a (1 - b^2), op 13 sigmoid backward
+    a (1 - b) b (b = the stored forward OUTPUT; torch tanh_backward / sigmoid_backward).  Parameters are the fp32 values the descriptor carries."""
     _chk(a, dt, 2)
     rows, width = a.shape
     if b is not None:

@@ -186,6 +186,9 @@ void oracle_pointwise(const void* src, int64_t lds, int32_t rows, int32_t width,
 //   op 11 relu_bwd:  y = (b <= 0) ? 0 : a   -- a = incoming gradient, b = the ReLU's forward output (or its input:
 //                    same mask); the backward of the ReLU epilogue of a grouped Linear in a post-grad graph
 //                    (batch_linear_post_grad; training QPS is the headline)
+//   op 12 tanh_bwd:    y = a (1 - b^2)    -- b = the STORED forward output tanh(z)    (torch tanh_backward)
+//   op 13 sigmoid_bwd: y = a (1 - b) b    -- b = the STORED forward output sigmoid(z) (torch sigmoid_backward)
+//                    the backward of the other two epilogues of the grouped Linear (same passages as op 11)
 // b may be NULL for the unary ops.
 void oracle_pointwise_ext(const void* a, int64_t lda, const void* b, int64_t ldb, int32_t rows, int32_t width,
                           int op, double p0, double p1, double p2, int dt, double* out) {
@@ -207,6 +210,8 @@ void oracle_pointwise_ext(const void* a, int64_t lda, const void* b, int64_t ldb
         case 7: y = x / widen(b, (int64_t)r * ldb + c, dt); break;
         case 8: y = x * widen(b, (int64_t)r * ldb + c, dt); break;
         case 11: y = widen(b, (int64_t)r * ldb + c, dt) <= 0.0 ? 0.0 : x; break;
+        case 12: { const double t = widen(b, (int64_t)r * ldb + c, dt); y = x * (1.0 - t * t); break; }
+        case 13: { const double t = widen(b, (int64_t)r * ldb + c, dt); y = x * ((1.0 - t) * t); break; }
         default: y = x; break;
       }
       out[(int64_t)r * width + c] = y;

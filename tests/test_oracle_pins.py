@@ -526,6 +526,34 @@ def test_relu_backward_hand_values_and_finite_differences():
     assert np.array_equal(r, np.where(oracle.widen(mb, BF16) > 0, oracle.widen(gb, BF16), 0.0))
 
 
+def test_tanh_and_sigmoid_backward_hand_values_and_finite_differences():
+    """Ops 12 / 13 (backward of the tanh / sigmoid epilogues, PAPER.md:292 batch_linear_post_grad on post-grad graphs):
+    hand values at outputs where the closed form is a short decimal, then central differences of numpy's own
+    tanh / logistic through the forward output, and the limits y -> +-1 (tanh) and y -> 0, 1 (sigmoid): gradient 0."""
+    g = np.array([[2.0, -4.0, 1.0, 8.0]], dtype=np.float32)
+    y = np.array([[0.5, -0.5, 0.0, 1.0]], dtype=np.float32)
+    assert np.array_equal(oracle.pointwise_ext(g, y, oracle.PW_TANH_BWD, [], F32), [[1.5, -3.0, 1.0, 0.0]])
+    ys = np.array([[0.5, 0.25, 0.0, 1.0]], dtype=np.float32)
+    assert np.array_equal(oracle.pointwise_ext(g, ys, oracle.PW_SIGMOID_BWD, [], F32), [[0.5, -0.75, 0.0, 0.0]])
+    z = wl.tensor_normal(18, 1, (6, 20), 0.0, 1.5, F32).astype(np.float64)
+    gg = wl.tensor_normal(18, 2, (6, 20), 0.0, 1.0, F32)
+    h = 1e-5
+    for op, f in ((oracle.PW_TANH_BWD, np.tanh), (oracle.PW_SIGMOID_BWD, lambda t: 1.0 / (1.0 + np.exp(-t)))):
+        fd = (f(z + h) - f(z - h)) / (2 * h) * gg.astype(np.float64)
+        out32 = f(z).astype(np.float32)                                  # the stored forward output (fp32 storage)
+        got = oracle.pointwise_ext(gg, out32, op, [], F32)
+        assert np.allclose(got, fd, rtol=0, atol=2e-6), np.abs(got - fd).max()      # fp32 rounding of y: 6e-8 * |dy/dy| terms
+    # the two ops differ (a swapped op code fails): at y = 0.5, tanh' = 0.75, sigmoid' = 0.25
+    half = np.full((1, 1), 0.5, dtype=np.float32); one = np.ones((1, 1), dtype=np.float32)
+    assert oracle.pointwise_ext(one, half, oracle.PW_TANH_BWD, [], F32)[0, 0] == 0.75
+    assert oracle.pointwise_ext(one, half, oracle.PW_SIGMOID_BWD, [], F32)[0, 0] == 0.25
+    # bf16 storage: widened exactly, product in fp64
+    gb = wl.tensor_normal(18, 3, (4, 16), 0.0, 3.0, BF16); yb = wl.tensor_uniform(18, 4, (4, 16), -1.0, 1.0, BF16)
+    a, b = oracle.widen(gb, BF16), oracle.widen(yb, BF16)
+    assert np.array_equal(oracle.pointwise_ext(gb, yb, oracle.PW_TANH_BWD, [], BF16), a * (1.0 - b * b))
+    assert np.array_equal(oracle.pointwise_ext(gb, yb, oracle.PW_SIGMOID_BWD, [], BF16), a * ((1.0 - b) * b))
+
+
 # ------------------------------------------ backward of the grouped Linear (SURVEY 8(f) rank 3) --
 def test_linear_backward_integers_and_adjointness():
     """dgrad / wgrad against numpy integer arithmetic (exact), and the adjoint identities that DEFINE them:
