@@ -133,3 +133,14 @@ def linear_relu_backward(m, dy, dt=BF16):
     y = round_to_storage(linear_member(dict(m, act=1), dt), dt)
     dz = round_to_storage(pointwise_ext(dy, y, PW_RELU_BWD, [], dt), dt)
     return dict(y=y, dz=dz, db64=linear_bias_grad(dz, dt), dx64=linear_dgrad(dz, m["w"], dt), dw64=linear_wgrad(dz, m["x"], dt))
+
+
+def linear_act_backward(m, dy, act, dt=BF16):
+    """The whole backward of one member y = act(x W^T + b) for act in {1 relu, 2 tanh, 3 sigmoid}, one op at a time,
+    the activation's derivative taken from the STORED forward output y (pointwise_ext ops 11 / 12 / 13):
+    dz (storage), db = column sums of dz, dX = dz W, dW = dz^T x.  -> dict(y, dz, db64, dx64, dw64)."""
+    from . import PW_RELU_BWD, PW_SIGMOID_BWD, PW_TANH_BWD, pointwise_ext
+    op = {1: PW_RELU_BWD, 2: PW_TANH_BWD, 3: PW_SIGMOID_BWD}[act]
+    y = round_to_storage(linear_member(dict(m, act=act), dt), dt)
+    dz = round_to_storage(pointwise_ext(dy, y, op, [], dt), dt)
+    return dict(y=y, dz=dz, db64=linear_bias_grad(dz, dt), dx64=linear_dgrad(dz, m["w"], dt), dw64=linear_wgrad(dz, m["x"], dt))

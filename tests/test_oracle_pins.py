@@ -600,6 +600,32 @@ def test_bias_grad_and_full_linear_relu_backward_by_finite_differences():
     assert np.allclose(r["dw64"], fd(w64, 1), rtol=0, atol=1e-6)
 
 
+@pytest.mark.parametrize("act", [2, 3])
+def test_full_linear_tanh_sigmoid_backward_by_finite_differences(act):
+    """graphs.linear_act_backward for the tanh / sigmoid epilogues against central differences of a NUMPY fp64 forward
+    (fp32 storage: the stored output carries a 6e-8 rounding, the gate is 1e-5); act = 1 equals linear_relu_backward."""
+    x = wl.tensor_normal(24, 2, (9, 6), 0.0, 1.0, F32); w = wl.tensor_normal(24, 3, (5, 6), 0.0, 0.5, F32)
+    b = wl.tensor_normal(24, 4, (5,), 0.0, 0.5, F32); dy = wl.tensor_normal(24, 5, (9, 5), 0.0, 1.0, F32)
+    r = graphs.linear_act_backward(dict(x=x, w=w, b=b), dy, act, F32)
+    x64, w64, b64, dy64 = (a.astype(np.float64) for a in (x, w, b, dy))
+    f = np.tanh if act == 2 else (lambda t: 1.0 / (1.0 + np.exp(-t)))
+    loss = lambda xx, ww, bb: float((f(xx @ ww.T + bb) * dy64).sum())
+    h = 1e-6
+    def fd(a, which):
+        out = np.zeros_like(a)
+        for idx in np.ndindex(a.shape):
+            ap, am = a.copy(), a.copy(); ap[idx] += h; am[idx] -= h
+            args_p = [x64, w64, b64]; args_m = [x64, w64, b64]
+            args_p[which], args_m[which] = ap, am
+            out[idx] = (loss(*args_p) - loss(*args_m)) / (2 * h)
+        return out
+    assert np.allclose(r["db64"], fd(b64, 2), rtol=0, atol=1e-5)
+    assert np.allclose(r["dx64"], fd(x64, 0), rtol=0, atol=1e-5)
+    assert np.allclose(r["dw64"], fd(w64, 1), rtol=0, atol=1e-5)
+    r1, r0 = graphs.linear_act_backward(dict(x=x, w=w, b=b), dy, 1, F32), graphs.linear_relu_backward(dict(x=x, w=w, b=b), dy, F32)
+    assert all(np.array_equal(r1[k], r0[k]) for k in r0)
+
+
 def test_layernorm_backward_finite_differences_and_identities():
     """dx, dgamma, dbeta against central finite differences of the oracle's OWN forward are not a pin (same code
     base), so the forward used here is numpy's: L(x, gamma, beta) = sum(dy * LN(x)) in fp64.  Plus the closed forms:
