@@ -85,7 +85,11 @@ typedef enum {
   OPT_PW_DEQUANT_E4M3 = 10, /* dst (bf16) = value(src fp8 code, lds in fp8 elements) * p0                          */
   /* backward of the ReLU epilogue of a grouped Linear in a post-grad graph (batch_linear_post_grad):
    * src = incoming gradient, src2 = the ReLU's forward output (or input: same mask); feeds the dgrad / wgrad groups */
-  OPT_PW_RELU_BWD = 11      /* dst = (src2 <= 0) ? 0 : src   (exact; a NaN in src2 lets the gradient through)      */
+  OPT_PW_RELU_BWD = 11,     /* dst = (src2 <= 0) ? 0 : src   (exact; a NaN in src2 lets the gradient through)      */
+  /* backward of the tanh / sigmoid epilogues (torch tanh_backward / sigmoid_backward): src = incoming gradient,
+   * src2 = the STORED forward output; fp32 arithmetic, one rounding to the storage dtype                           */
+  OPT_PW_TANH_BWD = 12,     /* dst = src * (1 - src2^2)                                                             */
+  OPT_PW_SIGMOID_BWD = 13   /* dst = src * (1 - src2) * src2                                                        */
 } opt_pw_op;
 
 /* Storage of the two operands of a grouped Linear member.  Default 0: x is [M,K], w is [N,K] (torch nn.Linear).
@@ -250,7 +254,7 @@ typedef struct {
   int64_t ldd;
   int32_t rows, width;
   int32_t op; /* opt_pw_op */
-  const void* src2; /* second operand of OPT_PW_SUB / DIV / MUL / RELU_BWD, else NULL */
+  const void* src2; /* second operand of OPT_PW_SUB / DIV / MUL / *_BWD, else NULL */
   int64_t lds2;
   float p0, p1, p2; /* CLAMP: lo, hi;  NAN_TO_NUM: nan, posinf, neginf */
 } opt_chunk;

@@ -10,7 +10,7 @@ from .binding import (  # noqa: F401
     OPT_F32, OPT_BF16,
     OPT_ACT_NONE, OPT_ACT_RELU, OPT_ACT_TANH, OPT_ACT_SIGMOID,
     OPT_PW_COPY, OPT_PW_RELU, OPT_PW_TANH, OPT_PW_SIGMOID,
-    OPT_PW_CLAMP, OPT_PW_NAN_TO_NUM, OPT_PW_SUB, OPT_PW_DIV, OPT_PW_MUL, OPT_PW_QUANT_E4M3, OPT_PW_DEQUANT_E4M3, OPT_PW_RELU_BWD,
+    OPT_PW_CLAMP, OPT_PW_NAN_TO_NUM, OPT_PW_SUB, OPT_PW_DIV, OPT_PW_MUL, OPT_PW_QUANT_E4M3, OPT_PW_DEQUANT_E4M3, OPT_PW_RELU_BWD, OPT_PW_TANH_BWD, OPT_PW_SIGMOID_BWD,
     OPT_LAYOUT_X_TRANSPOSED, OPT_LAYOUT_W_TRANSPOSED,
     OPT_OK, OPT_ERR_INVALID_ARG, OPT_ERR_UNSUPPORTED, OPT_ERR_ALIGNMENT, OPT_ERR_ALIAS, OPT_ERR_CUDA,
     OPT_ERR_NO_DEVICE,

@@ -10,6 +10,7 @@ OPT_PW_COPY, OPT_PW_RELU, OPT_PW_TANH, OPT_PW_SIGMOID = 0, 1, 2, 3
 OPT_PW_CLAMP, OPT_PW_NAN_TO_NUM, OPT_PW_SUB, OPT_PW_DIV, OPT_PW_MUL = 4, 5, 6, 7, 8
 OPT_PW_QUANT_E4M3, OPT_PW_DEQUANT_E4M3 = 9, 10
 OPT_PW_RELU_BWD = 11
+OPT_PW_TANH_BWD, OPT_PW_SIGMOID_BWD = 12, 13
 OPT_LAYOUT_X_TRANSPOSED, OPT_LAYOUT_W_TRANSPOSED = 1, 2
 (OPT_OK, OPT_ERR_INVALID_ARG, OPT_ERR_UNSUPPORTED, OPT_ERR_ALIGNMENT, OPT_ERR_ALIAS, OPT_ERR_CUDA,
  OPT_ERR_NO_DEVICE) = range(7)

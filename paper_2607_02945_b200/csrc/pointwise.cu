@@ -46,7 +46,7 @@ struct PwGroup {
   int32_t src_span;       // STAGED mode: vectors of one source row staged in smem (0 = direct mode)
   int32_t dst_span;       // STAGED mode: vectors of one destination row staged for a bulk store (0 = direct stores)
   int32_t tile_rows;      // STAGED mode: rows per block
-  int32_t ext_op;         // EXT mode (0 = off): OPT_PW_CLAMP .. OPT_PW_RELU_BWD, one chunk per group, no map
+  int32_t ext_op;         // EXT mode (0 = off): OPT_PW_CLAMP .. OPT_PW_SIGMOID_BWD, one chunk per group, no map
   const char* src2;       // EXT mode: second operand of the binary ops
   int64_t lds2_16;
   float p0, p1, p2;       // EXT mode: scalar parameters
@@ -107,6 +107,8 @@ __device__ __forceinline__ float pw_ext_scalar(float x, float y, int op, float p
     case OPT_PW_SUB: return x - y;
     case OPT_PW_DIV: return x / y;                                             // IEEE division (no fast-math)
     case OPT_PW_RELU_BWD: return y <= 0.f ? 0.f : x;                           // gradient where the forward value is > 0
+    case OPT_PW_TANH_BWD: return x * fmaf(-y, y, 1.f);                         // y = tanh(z) stored: dz = dy (1 - y^2)
+    case OPT_PW_SIGMOID_BWD: return x * ((1.f - y) * y);                       // y = sigmoid(z) stored: dz = dy (1 - y) y
     default: return x * y;                                                     // OPT_PW_MUL
   }
 }
@@ -371,8 +373,8 @@ extern "C" opt_status opt_pointwise_plan_create(const opt_chunk* chunks, int32_t
     const opt_chunk& c = chunks[i];
     if (!c.src || !c.dst) return fail(OPT_ERR_INVALID_ARG, "chunk %d: NULL pointer", i);
     if (c.rows < 1 || c.width < 1) return fail(OPT_ERR_INVALID_ARG, "chunk %d: rows=%d width=%d must be >= 1", i, c.rows, c.width);
-    if (c.op < OPT_PW_COPY || c.op > OPT_PW_RELU_BWD) return fail(OPT_ERR_INVALID_ARG, "chunk %d: bad op %d", i, c.op);
-    const bool ext = c.op >= OPT_PW_CLAMP, binary = (c.op >= OPT_PW_SUB && c.op <= OPT_PW_MUL) || c.op == OPT_PW_RELU_BWD;
+    if (c.op < OPT_PW_COPY || c.op > OPT_PW_SIGMOID_BWD) return fail(OPT_ERR_INVALID_ARG, "chunk %d: bad op %d", i, c.op);
+    const bool ext = c.op >= OPT_PW_CLAMP, binary = (c.op >= OPT_PW_SUB && c.op <= OPT_PW_MUL) || c.op >= OPT_PW_RELU_BWD;
     const bool fp8 = c.op == OPT_PW_QUANT_E4M3 || c.op == OPT_PW_DEQUANT_E4M3;
     if (fp8 && io != OPT_BF16) return fail(OPT_ERR_UNSUPPORTED, "chunk %d: FP8 quantisation is implemented for bf16 activations only", i);
     // element sizes of the two sides: quantise writes fp8, dequantise reads fp8

@@ -164,7 +164,7 @@ def test_host_validation_of_the_next_row_entry_points(ob):
     # pointwise: binary op without a second operand, FP8 on fp32 activations, unknown op
     ch = lambda **kw: ob.opt_chunk(**{**dict(src=A, lds=64, dst=B, ldd=64, rows=4, width=64, op=0, src2=None, lds2=0, p0=0.0, p1=0.0, p2=0.0), **kw})
     for chunk, io, status in [(ch(op=ob.OPT_PW_MUL), ob.OPT_BF16, ob.OPT_ERR_INVALID_ARG), (ch(op=ob.OPT_PW_QUANT_E4M3, p0=1.0), ob.OPT_F32, ob.OPT_ERR_UNSUPPORTED),
-                              (ch(op=12), ob.OPT_BF16, ob.OPT_ERR_INVALID_ARG), (ch(op=ob.OPT_PW_RELU_BWD), ob.OPT_BF16, ob.OPT_ERR_INVALID_ARG), (ch(op=ob.OPT_PW_SUB, src2=B + 64, lds2=64), ob.OPT_BF16, ob.OPT_ERR_ALIAS)]:
+                              (ch(op=14), ob.OPT_BF16, ob.OPT_ERR_INVALID_ARG), (ch(op=ob.OPT_PW_RELU_BWD), ob.OPT_BF16, ob.OPT_ERR_INVALID_ARG), (ch(op=ob.OPT_PW_TANH_BWD), ob.OPT_BF16, ob.OPT_ERR_INVALID_ARG), (ch(op=ob.OPT_PW_SIGMOID_BWD), ob.OPT_BF16, ob.OPT_ERR_INVALID_ARG), (ch(op=ob.OPT_PW_SUB, src2=B + 64, lds2=64), ob.OPT_BF16, ob.OPT_ERR_ALIAS)]:
         with pytest.raises(ob.OptError) as e:
             ob.opt_pointwise_plan_create([chunk], io)
         assert e.value.status == status, (e.value, status)
