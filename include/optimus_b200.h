@@ -226,7 +226,10 @@ typedef struct {
  *     dZ[m, n] = (y[m, n] <= 0) ? +0 : dY[m, n]      (torch threshold_backward == OPT_PW_RELU_BWD, bit-exact)
  *     db[n]    = sum over m of dZ[m, n]
  * dZ is written to dz_out:[M,N] (lddz_out) unless dz_out is NULL; dz_out == dz with lddz_out == ldz (in place) is
- * allowed.  y and dz_out follow the alignment rules of dz.                                                          */
+ * allowed.  y and dz_out follow the alignment rules of dz.  act (opt_act; needs y) selects the epilogue whose
+ * derivative is fused: OPT_ACT_NONE / OPT_ACT_RELU the mask above, OPT_ACT_TANH dZ = dY (1 - y^2), OPT_ACT_SIGMOID
+ * dZ = dY (1 - y) y -- dZ rounded to bf16 exactly as OPT_PW_TANH_BWD / OPT_PW_SIGMOID_BWD do, and db sums the
+ * ROUNDED dZ (what a separate bias-gradient launch would read).                                                     */
 typedef struct {
   const void* dz;
   int64_t ldz;
@@ -236,6 +239,7 @@ typedef struct {
   int64_t ldy;
   void* dz_out;
   int64_t lddz_out;
+  int32_t act; /* opt_act */
 } opt_bias_grad_member;
 
 /* One chunk of a multi-tensor pointwise / split-cat pass -- batch_relu,

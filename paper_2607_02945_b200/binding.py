@@ -50,7 +50,7 @@ class opt_layernorm_bwd_member(C.Structure):
 
 class opt_bias_grad_member(C.Structure):
     _fields_ = [("dz", C.c_void_p), ("ldz", C.c_int64), ("db", C.c_void_p), ("M", C.c_int32), ("N", C.c_int32),
-                ("y", C.c_void_p), ("ldy", C.c_int64), ("dz_out", C.c_void_p), ("lddz_out", C.c_int64)]
+                ("y", C.c_void_p), ("ldy", C.c_int64), ("dz_out", C.c_void_p), ("lddz_out", C.c_int64), ("act", C.c_int32)]
 
 
 class opt_chunk(C.Structure):
@@ -274,15 +274,15 @@ def layernorm_bwd_member(x, dy, gamma, dx, dgamma, dbeta, eps):
                                     ptr(dgamma), ptr(dbeta), rows, D, float(eps))
 
 
-def bias_grad_member(dz, db, y=None, dz_out=None):
-    """db = column sums of dz; with y (stored ReLU output): of the masked gradient, which goes to dz_out if given."""
+def bias_grad_member(dz, db, y=None, dz_out=None, act=0):
+    """db = column sums of dz; with y (stored ReLU output): of the masked gradient (act 2 / 3: of dz times the tanh / sigmoid derivative), which goes to dz_out if given."""
     M, N = dz.shape
     assert tuple(db.shape) == (N,)
     assert y is None or tuple(y.shape) == (M, N)
     assert dz_out is None or (y is not None and tuple(dz_out.shape) == (M, N))
     return opt_bias_grad_member(dz.data_ptr(), _ld(dz), db.data_ptr(), M, N,
                                 None if y is None else y.data_ptr(), 0 if y is None else _ld(y),
-                                None if dz_out is None else dz_out.data_ptr(), 0 if dz_out is None else _ld(dz_out))
+                                None if dz_out is None else dz_out.data_ptr(), 0 if dz_out is None else _ld(dz_out), int(act))
 
 
 def chunk(src, dst, op=OPT_PW_COPY, src2=None, params=()):

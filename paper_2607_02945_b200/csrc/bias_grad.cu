@@ -31,6 +31,7 @@ struct BgMember {
   int32_t* ticket;                 // blocks of this member that have finished
   int32_t rows, nvec, nparts, nblocks;
   int32_t l_log2;                  // lanes per row of a column tile
+  int32_t act;                     // fused derivative: 0 / 1 ReLU mask, 2 tanh, 3 sigmoid
 };
 struct BgBlock { int32_t member, row0, nrows, part, vec0; };
 
@@ -55,6 +56,20 @@ __device__ __forceinline__ uint32_t bg_mask2(uint32_t g, uint32_t y) {
 __device__ __forceinline__ int4 bg_mask(int4 g, const int4& y) {
   g.x = (int)bg_mask2((uint32_t)g.x, (uint32_t)y.x); g.y = (int)bg_mask2((uint32_t)g.y, (uint32_t)y.y);
   g.z = (int)bg_mask2((uint32_t)g.z, (uint32_t)y.z); g.w = (int)bg_mask2((uint32_t)g.w, (uint32_t)y.w);
+  return g;
+}
+
+// derivative of the epilogue from its stored output, applied to a 16-byte vector of gradients: act 0 / 1 the ReLU mask
+// (bit-exact select), 2 tanh dy (1 - y^2), 3 sigmoid dy (1 - y) y -- fp32, one rounding to bf16, the same arithmetic as
+// OPT_PW_TANH_BWD / OPT_PW_SIGMOID_BWD of the pointwise kernel (bitwise equal results)
+__device__ __forceinline__ float bg_dact(float g, float y, int act) { return act == 2 ? g * fmaf(-y, y, 1.f) : g * ((1.f - y) * y); }
+__device__ __forceinline__ int4 bg_deriv(int4 g, const int4& y, int act) {
+  if (act <= 1) return bg_mask(g, y);
+  uint32_t* ug = reinterpret_cast<uint32_t*>(&g);
+  const uint32_t* uy = reinterpret_cast<const uint32_t*>(&y);
+#pragma unroll
+  for (int i = 0; i < 4; ++i)
+    ug[i] = pack_bf16x2(bg_dact(bf16_lo(ug[i]), bf16_lo(uy[i]), act), bg_dact(bf16_hi(ug[i]), bf16_hi(uy[i]), act));
   return g;
 }
 
@@ -83,7 +98,7 @@ __device__ __forceinline__ void bg_block(const BgMember& m, const BgBlock& b, fl
 #pragma unroll
       for (int j = 0; j < kBgInflight; ++j) {
         if (MASK) {
-          v[j] = bg_mask(v[j], y[j]);
+          v[j] = bg_deriv(v[j], y[j], m.act);
           if (ob) __stcs(ob + (int64_t)(r + j * rpp) * m.lddzo16, v[j]);
         }
         const uint32_t* u = reinterpret_cast<const uint32_t*>(&v[j]);
@@ -94,7 +109,7 @@ __device__ __forceinline__ void bg_block(const BgMember& m, const BgBlock& b, fl
     for (; r < b.nrows; r += rpp) {
       int4 v = __ldcs(zb + (int64_t)r * m.ldz16);
       if (MASK) {
-        v = bg_mask(v, __ldcs(yb + (int64_t)r * m.ldy16));
+        v = bg_deriv(v, __ldcs(yb + (int64_t)r * m.ldy16), m.act);
         if (ob) __stcs(ob + (int64_t)r * m.lddzo16, v);
       }
       const uint32_t* u = reinterpret_cast<const uint32_t*>(&v);
@@ -202,6 +217,8 @@ extern "C" opt_status opt_bias_grad_plan_create(const opt_bias_grad_member* memb
     if (!aligned16(m.dz) || !aligned16(m.db)) return fail(OPT_ERR_ALIGNMENT, "member %d: pointers must be 16-byte aligned", i);
     if (m.N % 8) return fail(OPT_ERR_ALIGNMENT, "member %d: N=%d is not a multiple of 8", i, m.N);
     if (m.M > 1 && m.ldz % 8) return fail(OPT_ERR_ALIGNMENT, "member %d: row stride must be a multiple of 8 elements", i);
+    if (m.act < OPT_ACT_NONE || m.act > OPT_ACT_SIGMOID) return fail(OPT_ERR_INVALID_ARG, "member %d: bad act %d", i, m.act);
+    if (m.act > OPT_ACT_RELU && !m.y) return fail(OPT_ERR_INVALID_ARG, "member %d: act %d needs y (the stored forward output)", i, m.act);
     if (m.dz_out && !m.y) return fail(OPT_ERR_INVALID_ARG, "member %d: dz_out without y (the mask source)", i);
     if (m.y) {
       if (!aligned16(m.y) || !aligned16(m.dz_out)) return fail(OPT_ERR_ALIGNMENT, "member %d: pointers must be 16-byte aligned", i);
@@ -226,7 +243,7 @@ extern "C" opt_status opt_bias_grad_plan_create(const opt_bias_grad_member* memb
     BgMember t;
     memset(&t, 0, sizeof t);
     t.dz = (const char*)m.dz; t.db = (char*)m.db; t.ldz16 = m.ldz / 8;
-    t.y = (const char*)m.y; t.dzo = (char*)m.dz_out; t.ldy16 = m.ldy / 8; t.lddzo16 = m.lddz_out / 8;
+    t.y = (const char*)m.y; t.dzo = (char*)m.dz_out; t.ldy16 = m.ldy / 8; t.lddzo16 = m.lddz_out / 8; t.act = m.act;
     t.rows = m.M; t.nvec = nvec; t.nparts = nparts; t.nblocks = nparts * nctile; t.l_log2 = ll;
     tab.push_back(t);
     ws_off.push_back(ws_floats);

@@ -42,7 +42,7 @@ def test_struct_layouts_match_header(ob):
     assert ctypes.sizeof(ob.opt_chunk) == 80
     assert ctypes.sizeof(ob.opt_linear2_member) == 104 and ctypes.sizeof(ob.opt_ln_linear2_member) == 128
     assert ctypes.sizeof(ob.opt_host_copy) == 32
-    assert ctypes.sizeof(ob.opt_bias_grad_member) == 64 and ctypes.sizeof(ob.opt_layernorm_bwd_member) == 88
+    assert ctypes.sizeof(ob.opt_bias_grad_member) == 72 and ctypes.sizeof(ob.opt_layernorm_bwd_member) == 88
 
 
 def test_sass_is_blackwell_native():
@@ -148,11 +148,11 @@ def test_host_validation_of_the_next_row_entry_points(ob):
             ob.opt_layernorm_bwd_plan_create([member], ob.OPT_BF16)
         assert e.value.status == status, (e.value, status)
     # bias gradient: N % 8, aligned pointers and strides, db must not lie inside dz, fp32 activations unsupported
-    bgm = lambda **kw: ob.opt_bias_grad_member(**{**dict(dz=A, ldz=64, db=B, M=16, N=64, y=None, ldy=0, dz_out=None, lddz_out=0), **kw})
+    bgm = lambda **kw: ob.opt_bias_grad_member(**{**dict(dz=A, ldz=64, db=B, M=16, N=64, y=None, ldy=0, dz_out=None, lddz_out=0, act=0), **kw})
     for member, io, status in [(bgm(N=60), ob.OPT_BF16, ob.OPT_ERR_ALIGNMENT), (bgm(ldz=68), ob.OPT_BF16, ob.OPT_ERR_ALIGNMENT), (bgm(db=B + 8), ob.OPT_BF16, ob.OPT_ERR_ALIGNMENT),
                                (bgm(db=A + 128), ob.OPT_BF16, ob.OPT_ERR_ALIAS), (bgm(ldz=32), ob.OPT_BF16, ob.OPT_ERR_INVALID_ARG), (bgm(M=0), ob.OPT_BF16, ob.OPT_ERR_INVALID_ARG),
                                (bgm(dz=None), ob.OPT_BF16, ob.OPT_ERR_INVALID_ARG), (bgm(), ob.OPT_F32, ob.OPT_ERR_UNSUPPORTED),
-                               (bgm(dz_out=Cc, lddz_out=64), ob.OPT_BF16, ob.OPT_ERR_INVALID_ARG), (bgm(y=Cc, ldy=60), ob.OPT_BF16, ob.OPT_ERR_INVALID_ARG),
+                               (bgm(dz_out=Cc, lddz_out=64), ob.OPT_BF16, ob.OPT_ERR_INVALID_ARG), (bgm(y=Cc, ldy=60), ob.OPT_BF16, ob.OPT_ERR_INVALID_ARG), (bgm(act=2), ob.OPT_BF16, ob.OPT_ERR_INVALID_ARG), (bgm(y=Cc, ldy=64, act=4), ob.OPT_BF16, ob.OPT_ERR_INVALID_ARG),
                                (bgm(y=Cc, ldy=64, dz_out=A + 16, lddz_out=64), ob.OPT_BF16, ob.OPT_ERR_ALIAS)]:
         with pytest.raises(ob.OptError) as e:
             ob.opt_bias_grad_plan_create([member], io)

@@ -125,6 +125,57 @@ def test_fused_relu_mask(ob):
     assert plan.info()["bytes"] == sum(g.size * 2 * (3 if mode < 2 else 2) + g.shape[1] * 4 for g, _, mode in host)
 
 
+@pytest.mark.parametrize("act", [2, 3])
+def test_fused_tanh_sigmoid_derivative(ob, act):
+    """act = tanh / sigmoid with y given: dZ = dY (1 - y^2) / dY (1 - y) y formed, rounded to bf16, written and summed in
+    one pass.  (1) Exact case -- y from {0.5, -0.5 | 0.25, 0, 1}, gradients multiples of 16: every product is exact, so
+    dz_out AND db are bit for bit the oracle's.  (2) Random case: dz_out <= 2 bf16 ulp of the oracle's op 12 / 13 and
+    bitwise equal to what the pointwise kernel writes for the same op; db within the summation bound plus the two
+    ulp (2^-7 relative) each summed element may differ by."""
+    from util import bf16_ulp_distance
+    oop = oracle.PW_TANH_BWD if act == 2 else oracle.PW_SIGMOID_BWD
+    pop = ob.OPT_PW_TANH_BWD if act == 2 else ob.OPT_PW_SIGMOID_BWD
+    rng = np.random.default_rng(66 + act)
+    yset = np.array([0.5, -0.5 if act == 2 else 0.25, 0.0, 1.0], dtype=np.float32)
+    exact, rand = [], []
+    for i, (M, N) in enumerate(SHAPES):
+        exact.append((wl.bf16_bits_from_f32((16 * rng.integers(-3, 4, (M, N))).astype(np.float32)), wl.bf16_bits_from_f32(yset[rng.integers(0, 4, (M, N))])))
+        z = wl.tensor_normal(67, 2 * i + 2, (M, N), 0.0, 2.0, BF16)
+        rand.append((wl.tensor_normal(67, 2 * i + 1, (M, N), 0.0, 2.0, BF16), oracle.round_to_storage(oracle.pointwise(z, act, BF16), BF16)))
+    for case, members in (("exact", exact), ("random", rand)):
+        devs, descs, chunks = [], [], []
+        for i, (g, y) in enumerate(members):
+            M, N = g.shape
+            pad = 24 if i % 2 else 0
+            dg = to_dev(np.pad(g, ((0, 0), (0, pad))), BF16)[:, :N]
+            dy = to_dev(np.pad(y, ((0, 0), (8, pad))), BF16)[:, 8:8 + N]
+            out = empty_dev((M, N + pad), BF16, fill=float("nan"))[:, :N]
+            out2 = empty_dev((M, N), BF16, fill=float("nan"))
+            db = empty_dev((N,), F32, fill=float("nan"))
+            descs.append(ob.bias_grad_member(dg, db, dy, out, act))
+            chunks.append(ob.chunk(dg, out2, pop, dy))
+            devs.append((out, out2, db, dg, dy))              # keep the inputs alive until the launches are done
+        n0 = ob.opt_launch_count()
+        ob.opt_bias_grad_plan_create(descs, BF16, F32).launch()
+        torch.cuda.synchronize()
+        assert ob.opt_launch_count() - n0 == 1
+        ob.opt_pointwise_plan_create(chunks, BF16).launch()
+        torch.cuda.synchronize()
+        for (g, y), (out, out2, db, _, _) in zip(members, devs):
+            ref64 = oracle.pointwise_ext(g, y, oop, [], BF16)
+            ref = oracle.round_to_storage(ref64, BF16)
+            got = to_host(out)
+            assert got.tobytes() == to_host(out2).tobytes(), (case, g.shape)
+            rdb = graphs.linear_bias_grad(ref, BF16)
+            if case == "exact":
+                assert np.array_equal(values64(got, BF16), ref64), g.shape
+                assert to_host(db).tobytes() == oracle.round_to_storage(rdb, F32).tobytes(), g.shape
+            else:
+                assert bf16_ulp_distance(got, ref).max() <= 2
+                l1 = np.abs(values64(ref, BF16)).sum(axis=0)
+                assert np.all(np.abs(to_host(db).astype(np.float64) - rdb) <= (2e-5 + 2.0 ** -7) * l1)
+
+
 @pytest.mark.parametrize("fused", [False, True])
 def test_whole_backward_of_a_linear_relu_group(ob, fused):
     """Forward Y_i = relu(X_i W_i^T + b_i) (one launch) and the whole backward in four launches -- ReLU masks, bias
