@@ -880,6 +880,20 @@ def run_product(args):
             backward.update(bias_grad_workload="configs[2]: 128 bias gradients db = column sums of the members' slices of the [4096, sum N] concat gradient, one launch",
                             bias_grad_us=round(tb_, 1), bias_grad_gbs=round(pb.info()["bytes"] / tb_ / 1e3, 1),
                             bias_grad_frac_hbm=round(pb.info()["bytes"] / tb_ / 1e3 / peaks["hbm_gbs"], 4))
+            # the whole backward of the group, three launches back to back in one timed region: ReLU mask fused into the
+            # bias-gradient launch (dY and the stored output Y read, dZ written in place of dY, db summed), dgrads and
+            # wgrads (which read dY's buffer, now holding dZ)
+            pfb = ob.opt_bias_grad_plan_create([ob.bias_grad_member(dy_cat[:, m["col_off"]:m["col_off"] + m["N"]], d,
+                                                                    ycat[:, m["col_off"]:m["col_off"] + m["N"]],
+                                                                    dy_cat[:, m["col_off"]:m["col_off"] + m["N"]], ob.OPT_ACT_RELU)
+                                                for m, d in zip(g2.cfg["members"], dbs)], BF16, ob.OPT_F32, step.dev_index)
+            pfb.launch()
+            torch.cuda.synchronize()
+            tfb = cold2(pfb.launch)
+            tall = cold2(lambda: (pfb.launch(), pd.launch(), pw.launch()))
+            backward.update(whole_backward_workload="configs[2]: backward of the 128 Linear+bias+ReLU members in 3 launches (fused mask + bias gradient in place, dgrad, wgrad)",
+                            relu_mask_bias_grad_fused_c2_us=round(tfb, 1), relu_mask_bias_grad_fused_c2_gbs=round(pfb.info()["bytes"] / tfb / 1e3, 1),
+                            whole_backward_us=round(tall, 1), whole_backward_launches=3)
             del dbs
             # LayerNorm backward of C4a's 512 members (dx, dgamma, dbeta), one launch
             c4a = [g for g in step.groups if g.name.startswith("C4a")]
