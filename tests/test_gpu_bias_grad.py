@@ -235,3 +235,50 @@ def test_full_size_c2_bias_grads(ob):
     for i in list(range(0, len(Ns), 9)) + [len(Ns) - 1]:
         z = to_host(dy_cat[:, off[i]:off[i + 1]])
         check(to_host(dbs[i]), z, F32)
+
+
+def test_stress_many_members_mixed_modes_relaunched(ob):
+    """4000 members in one plan -- tiny (1..3 rows, one block, one part), ragged, multi-part, plain / ReLU mask /
+    tanh / sigmoid derivative mixed, with and without dz_out -- launched 10 times back to back without a sync:
+    the self re-arming tickets must leave every relaunch bitwise identical, and every member within its bound."""
+    rng = np.random.default_rng(68)
+    host, descs, keep = [], [], []
+    big = torch.empty(64 << 20, dtype=torch.bfloat16, device="cuda")         # one arena: members are slices of it
+    big_y = torch.empty_like(big)
+    big.normal_(0.0, 1.0, generator=torch.Generator(device="cuda").manual_seed(68))
+    big_y.uniform_(-1.0, 1.0, generator=torch.Generator(device="cuda").manual_seed(69))
+    off = 0
+    for i in range(4000):
+        kind = i % 5
+        M = int(rng.integers(1, 4)) if kind == 0 else int(rng.integers(1, 3000)) if kind < 4 else int(rng.integers(9000, 20000))
+        N = 8 * int(rng.integers(1, 9 if kind == 4 else 40))
+        if off + M * N > big.numel():
+            break
+        z = big[off:off + M * N].view(M, N); y = big_y[off:off + M * N].view(M, N)
+        off += (M * N + 7) // 8 * 8
+        mode = int(rng.integers(0, 4))                                       # 0 plain, 1 relu, 2 tanh, 3 sigmoid
+        db = torch.full((N,), float("nan"), dtype=torch.float32, device="cuda")
+        out = torch.empty((M, N), dtype=torch.bfloat16, device="cuda") if mode and i % 2 else None
+        descs.append(ob.bias_grad_member(z, db) if mode == 0 else ob.bias_grad_member(z, db, y, out, mode))
+        keep.append((z, y, db, out, mode))
+    plan = ob.opt_bias_grad_plan_create(descs, BF16, F32)
+    plan.launch()
+    torch.cuda.synchronize()
+    first = torch.cat([k[2] for k in keep]).clone()
+    for k in keep:
+        k[2].fill_(float("nan"))
+    for _ in range(10):
+        plan.launch()
+    torch.cuda.synchronize()
+    assert torch.equal(torch.cat([k[2] for k in keep]).view(torch.int32), first.view(torch.int32))
+    ops = {1: oracle.PW_RELU_BWD, 2: oracle.PW_TANH_BWD, 3: oracle.PW_SIGMOID_BWD}
+    for j in list(range(0, len(keep), 37)) + [len(keep) - 1]:              # oracle on a sample of the members
+        z, y, db, out, mode = keep[j]
+        zh = to_host(z)
+        if mode:
+            zh = oracle.round_to_storage(oracle.pointwise_ext(zh, to_host(y), ops[mode], [], BF16), BF16)
+        l1 = np.abs(values64(zh, BF16)).sum(axis=0)
+        slack = (2e-5 if mode < 2 else 2e-5 + 2.0 ** -7) * l1
+        assert np.all(np.abs(to_host(db).astype(np.float64) - graphs.linear_bias_grad(zh, BF16)) <= slack), (j, mode, z.shape)
+        if out is not None and mode == 1:
+            assert to_host(out).tobytes() == zh.tobytes()
