@@ -252,6 +252,13 @@ extern "C" opt_status opt_bias_grad_plan_create(const opt_bias_grad_member* memb
       for (int32_t ct = 0; ct < nctile; ++ct)
         blocks.push_back({i, (int32_t)(part * rpb), (int32_t)std::min<int64_t>(rpb, m.M - part * rpb), part, ct * kBgTileVec});
   }
+  // launch order.  Dense members (ldz == N) stay member-major: a block's rows are one contiguous range.  Members that
+  // are column slices of a wider buffer go part-major -- blocks that run together then read the SAME rows of
+  // neighbouring members, i.e. neighbouring bytes of the same DRAM rows (configs[2]'s concat gradient: 102 -> 97 us)
+  {
+    auto key = [&](const BgBlock& b) { return members[b.member].M > 1 && members[b.member].ldz != members[b.member].N ? b.part + 1 : 0; };
+    std::stable_sort(blocks.begin(), blocks.end(), [&](const BgBlock& a, const BgBlock& b) { return key(a) < key(b); });
+  }
   if (opt_status st = check_independent(regions, /*allow_inplace_self=*/true)) return st;
   if (blocks.size() > (size_t)INT32_MAX) return fail(OPT_ERR_UNSUPPORTED, "too many work items");
 
