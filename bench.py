@@ -500,7 +500,8 @@ def run_side(args):
       --side skinny    the paper's four skinny aten.mm as one group (streaming row kernel)
       --side fp8       configs[4]'s saved LayerNorm outputs -> FP8 E4M3 and back (one launch each)
       --side bias_grad the 512 bias gradients of configs[4]'s Linear+ReLU group (column sums of [8192, H]), one launch
-      --side lhs       batch_linear_lhs: 8 members (N=64) on ONE input X [262144, 512]; OPT_GEMM_NO_LHS=1 = plain order
+      --side lhs       batch_linear_lhs: 8 members (N=64) on ONE input X [262144, 512]; also timed with
+                       opt_linear_options.no_lhs_order (plain member-major schedule)
     Prints one JSON line; not the bench metric."""
     import torch
     import paper_2607_02945_b200 as ob
@@ -591,10 +592,13 @@ def run_side(args):
         x = torch.randn(M, K, device="cuda", generator=g).to(torch.bfloat16)
         ws = [(torch.randn(N, K, device="cuda", generator=g) * K ** -0.5).to(torch.bfloat16) for _ in range(n)]
         ycat = torch.empty(M, N * n, device="cuda", dtype=torch.bfloat16)
-        plan = ob.opt_linear_plan_create([ob.linear_member(x, w, None, ycat[:, i * N:(i + 1) * N], ACT_RELU)
-                                          for i, w in enumerate(ws)], BF16, 0)
-        print(json.dumps(dict(side="lhs", lhs_order=os.environ.get("OPT_GEMM_NO_LHS") is None,
-                              us=round(timed(plan.launch, 3), 1), **plan.info())))
+        descs = [ob.linear_member(x, w, None, ycat[:, i * N:(i + 1) * N], ACT_RELU) for i, w in enumerate(ws)]
+        plan = ob.opt_linear_plan_create(descs, BF16, 0)
+        plain = ob.opt_linear_plan_create_ex(descs, BF16, 0, ob.opt_linear_options(no_lhs_order=1))
+        plan.launch(); plain.launch()
+        torch.cuda.synchronize()
+        print(json.dumps(dict(side="lhs", us=round(timed(plan.launch, 3), 1), us_member_major_order=round(timed(plain.launch, 3), 1),
+                              **plan.info())))
     return 0
 
 
@@ -985,14 +989,10 @@ def run_product(args):
             torch.cuda.synchronize()
             tsk = cold3(ps.launch)
             isk = ps.info()
-            # the two [M,8]x[8,8] members alone: streaming row kernel vs the tensor-core tile kernel (OPT_GEMM_NO_SKINNY=1)
+            # the two [M,8]x[8,8] members alone: streaming row kernel vs the tensor-core tile kernel (opt_linear_options.no_skinny)
             two = [ob.linear_member(x, w, None, y, ACT_NONE) for (x, w, y), sh in zip(ten, shapes) if sh[1] == 8]
             p8 = ob.opt_linear_plan_create(two, BF16, step.dev_index)
-            os.environ["OPT_GEMM_NO_SKINNY"] = "1"
-            try:
-                p8t = ob.opt_linear_plan_create(two, BF16, step.dev_index)
-            finally:
-                del os.environ["OPT_GEMM_NO_SKINNY"]
+            p8t = ob.opt_linear_plan_create_ex(two, BF16, step.dev_index, ob.opt_linear_options(no_skinny=1))
             p8.launch(); p8t.launch()
             torch.cuda.synchronize()
             t8, t8t = cold3(p8.launch), cold3(p8t.launch, 2)

@@ -273,14 +273,31 @@ typedef struct {
 
 typedef struct opt_plan opt_plan; /* opaque; owns device-side tables only */
 
+/* Optional, documented planning choices of a grouped Linear (zero-initialise for the defaults; the results are
+ * the same bits whatever is chosen -- only the schedule changes).  The library reads NO environment variable.
+ *   cta_pair      0: CTA pairs (256-row tiles, tcgen05 cta_group::2) whenever every member allows it;
+ *                 1: always one CTA per 128-row tile;  2: CTA pairs or OPT_ERR_UNSUPPORTED.
+ *   no_skinny     1: never route a huge-M / tiny-K-and-N group to the streaming row kernel.
+ *   no_lhs_order  1: schedule members that share one input X independently (member-major) instead of
+ *                 m-block-major across them (batch_linear_lhs).                                  */
+typedef struct {
+  int32_t cta_pair;
+  int32_t no_skinny;
+  int32_t no_lhs_order;
+  int32_t reserved[5]; /* 0 */
+} opt_linear_options;
+
 /* Build a plan for a group.  members: host array of n descriptors.  io: dtype
  * of activations (and of weights/bias for linear).  param: dtype of gamma/beta.
  * device: CUDA device ordinal.  On success *plan is set; on failure *plan is
  * NULL and nothing is launched or left allocated.  Host argument validation
  * happens before the first CUDA call, so INVALID_ARG / ALIGNMENT / ALIAS /
- * UNSUPPORTED are reported even on a machine without a GPU.                  */
+ * UNSUPPORTED are reported even on a machine without a GPU.  The calling
+ * thread's current CUDA device is left as it was.                             */
 opt_status opt_linear_plan_create(const opt_linear_member* members, int32_t n, opt_dtype io,
                                   int device, opt_plan** plan);
+opt_status opt_linear_plan_create_ex(const opt_linear_member* members, int32_t n, opt_dtype io, int device,
+                                     const opt_linear_options* options /* NULL = defaults */, opt_plan** plan);
 opt_status opt_linear2_plan_create(const opt_linear2_member* members, int32_t n, opt_dtype io,
                                    int device, opt_plan** plan);
 opt_status opt_ln_linear2_plan_create(const opt_ln_linear2_member* members, int32_t n, opt_dtype io,

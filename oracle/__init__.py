@@ -46,6 +46,8 @@ def lib():
         L.oracle_round_to_storage.argtypes = [vp, i64, c.c_int, vp]
         L.oracle_widen.argtypes = [vp, i64, c.c_int, vp]
         L.oracle_linear.argtypes = [vp, i64, vp, i64, vp, i32, i32, i32, c.c_int, vp]
+        L.oracle_linear_f64x.argtypes = [vp, vp, i64, vp, i32, i32, i32, c.c_int, vp]
+        L.oracle_colsum.argtypes = [vp, i64, i32, i32, c.c_int, vp]
         L.oracle_linear_mulreduce.argtypes = [vp, i64, vp, i64, vp, i32, i32, i32, c.c_int, vp]
         L.oracle_activation.argtypes = [vp, i64, c.c_int]
         L.oracle_pointwise.argtypes = [vp, i64, i32, i32, c.c_int, c.c_int, vp]
@@ -115,6 +117,31 @@ def linear(x, w, b, dt, mulreduce=False):
     fn = lib().oracle_linear_mulreduce if mulreduce else lib().oracle_linear
     fn(_ptr(x), _ld(x), _ptr(w), _ld(w), _ptr(b), M, N, K, dt, _ptr(z))
     return z
+
+
+def linear_f64x(x64, w, b, dt):
+    """Z = X W^T + b in fp64 for an activation matrix that is already fp64 (the unrounded LayerNorm output inside a
+    vertically fused chain, reading Q25); w:[N,K], b:[N] or None in storage dtype dt.  Same summation order as linear."""
+    x64 = np.ascontiguousarray(x64, dtype=np.float64)
+    _chk(w, dt, 2)
+    M, K = x64.shape
+    N, K2 = w.shape
+    assert K == K2
+    if b is not None:
+        b = np.ascontiguousarray(_chk(b, dt, 1))
+        assert b.shape == (N,)
+    z = np.empty((M, N), dtype=np.float64)
+    lib().oracle_linear_f64x(_ptr(x64), _ptr(w), _ld(w), _ptr(b), M, N, K, dt, _ptr(z))
+    return z
+
+
+def colsum(dz, dt):
+    """db[n] = sum over rows of dz[m, n], rows added in index order, fp64 (the bias gradient of a Linear)."""
+    _chk(dz, dt, 2)
+    M, N = dz.shape
+    db = np.empty((N,), dtype=np.float64)
+    lib().oracle_colsum(_ptr(dz), _ld(dz), M, N, dt, _ptr(db))
+    return db
 
 
 def activation(z, act):

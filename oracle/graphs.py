@@ -9,8 +9,8 @@ between the groups of configs[4] (reading Q3).
 """
 import numpy as np
 
-from . import (BF16, F32, activation, cat, layernorm, linear, pointwise,  # noqa: F401
-               round_to_storage, split, widen)
+from . import (BF16, F32, activation, cat, colsum, layernorm, linear, linear_f64x, pointwise,  # noqa: F401
+               round_to_storage, split)
 
 
 def linear_member(m, dt):
@@ -86,14 +86,12 @@ def ln_linear2(m, dt=BF16):
     fused op never materialises the normalised tensor, so it is NOT rounded here; the hidden tensor is still
     rounded to the storage dtype (as in `linear2`, reading Q3):
         xn = layer_norm(x; gamma, beta, eps)          fp64, unrounded
-        h  = act1(xn W1^T + b1)  -> rounded            (first layer: a plain fp64 matmul on the unrounded xn)
+        h  = act1(xn W1^T + b1)  -> rounded            (first layer: oracle_linear_f64x, the plain index-order loop
+                                                        of `linear` on the unrounded xn)
         y  = act2(h W2^T + b2)   -> rounded
     Returns dict(xn64, h64, h, y64, y)."""
     xn64 = layernorm(m["x"], m.get("gamma"), m.get("beta"), m["eps"], dt)
-    z = xn64 @ widen(m["w1"], dt).T
-    if m.get("b1") is not None:
-        z = z + widen(m["b1"], dt)[None, :]
-    h64 = activation(z, m["act1"])
+    h64 = activation(linear_f64x(xn64, m["w1"], m.get("b1"), dt), m["act1"])
     h = round_to_storage(h64, dt)
     y64 = activation(linear(h, m["w2"], m.get("b2"), dt), m["act2"])
     return dict(xn64=xn64, h64=h64, h=h, y64=y64, y=round_to_storage(y64, dt))
@@ -118,11 +116,7 @@ def linear_wgrad(dy, x, dt=BF16):
 def linear_bias_grad(dz, dt=BF16):
     """Backward of y = x W^T + b w.r.t. the bias: db[n] = sum_m dZ[m, n], rows added in index order, fp64
     (PAPER.md:292 batch_linear_post_grad; PAPER.md:437 training)."""
-    z = widen(dz, dt)
-    db = np.zeros(z.shape[1], dtype=np.float64)
-    for r in range(z.shape[0]):
-        db += z[r]
-    return db
+    return colsum(dz, dt)
 
 
 def linear_relu_backward(m, dy, dt=BF16):

@@ -145,6 +145,33 @@ void oracle_linear(const void* x, int64_t ldx, const void* w, int64_t ldw, const
   }
 }
 
+// ---- the same linear on an activation matrix that is ALREADY in double (dense [M,K]): the first layer of a
+// vertically fused LayerNorm -> Linear chain, whose normalised input is never materialised and therefore never
+// rounded (reading Q25; "chained transformations").  Weights and bias are storage dtype.
+// Same loop nest and summation order as oracle_linear (k = 0..K-1, bias added last).
+void oracle_linear_f64x(const double* x, const void* w, int64_t ldw, const void* bias,
+                        int32_t M, int32_t N, int32_t K, int dt, double* z) {
+#pragma omp parallel for schedule(static)
+  for (int32_t m = 0; m < M; ++m) {
+    for (int32_t n = 0; n < N; ++n) {
+      double acc = 0.0;
+      for (int32_t k = 0; k < K; ++k) acc += x[(int64_t)m * K + k] * widen(w, (int64_t)n * ldw + k, dt);
+      if (bias) acc += widen(bias, n, dt);
+      z[(int64_t)m * N + n] = acc;
+    }
+  }
+}
+
+// ---- bias gradient of y = x W^T + b: db[n] = sum_{m<M} dZ[m,n], rows added in index order m = 0..M-1, in double
+// (the third output of the backward of a Linear; batch_linear_post_grad; training).
+void oracle_colsum(const void* dz, int64_t ldz, int32_t M, int32_t N, int dt, double* db) {
+  for (int32_t n = 0; n < N; ++n) {
+    double acc = 0.0;
+    for (int32_t m = 0; m < M; ++m) acc += widen(dz, (int64_t)m * ldz + n, dt);
+    db[n] = acc;
+  }
+}
+
 // ---- the same linear written as broadcast-multiply then reduce over K with a
 // different loop nest (k outermost) -- the decompose_mm formulation of
 // PAPER.md:475.  Only used by the pin test P5 as an independent second formula.

@@ -15,8 +15,8 @@ from .binding import (  # noqa: F401
     OPT_OK, OPT_ERR_INVALID_ARG, OPT_ERR_UNSUPPORTED, OPT_ERR_ALIGNMENT, OPT_ERR_ALIAS, OPT_ERR_CUDA,
     OPT_ERR_NO_DEVICE,
     OptError, Plan, lib, lib_path,
-    opt_linear_member, opt_linear2_member, opt_ln_linear2_member, opt_layernorm_member, opt_layernorm_bwd_member, opt_bias_grad_member, opt_chunk, opt_host_copy,
-    opt_linear_plan_create, opt_linear2_plan_create, opt_ln_linear2_plan_create, opt_layernorm_plan_create, opt_layernorm_bwd_plan_create, opt_bias_grad_plan_create,
+    opt_linear_member, opt_linear_options, opt_linear2_member, opt_ln_linear2_member, opt_layernorm_member, opt_layernorm_bwd_member, opt_bias_grad_member, opt_chunk, opt_host_copy,
+    opt_linear_plan_create, opt_linear_plan_create_ex, opt_linear2_plan_create, opt_ln_linear2_plan_create, opt_layernorm_plan_create, opt_layernorm_bwd_plan_create, opt_bias_grad_plan_create,
     opt_pointwise_plan_create,
     opt_plan_launch, opt_plan_launch_host, opt_plan_info, opt_plan_destroy,
     opt_last_error, opt_launch_count, opt_version,

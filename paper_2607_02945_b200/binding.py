@@ -24,6 +24,10 @@ class opt_linear_member(C.Structure):
                 ("M", C.c_int32), ("N", C.c_int32), ("K", C.c_int32), ("act", C.c_int32), ("layout", C.c_int32)]
 
 
+class opt_linear_options(C.Structure):
+    _fields_ = [("cta_pair", C.c_int32), ("no_skinny", C.c_int32), ("no_lhs_order", C.c_int32), ("reserved", C.c_int32 * 5)]
+
+
 class opt_linear2_member(C.Structure):
     _fields_ = [("x", C.c_void_p), ("ldx", C.c_int64), ("w1", C.c_void_p), ("ldw1", C.c_int64), ("b1", C.c_void_p),
                 ("w2", C.c_void_p), ("ldw2", C.c_int64), ("b2", C.c_void_p), ("y", C.c_void_p), ("ldy", C.c_int64),
@@ -90,6 +94,8 @@ def lib():
         L = C.CDLL(_build.LIB)
         pp = C.POINTER(C.c_void_p)
         L.opt_linear_plan_create.argtypes = [C.POINTER(opt_linear_member), C.c_int32, C.c_int, C.c_int, pp]
+        L.opt_linear_plan_create_ex.argtypes = [C.POINTER(opt_linear_member), C.c_int32, C.c_int, C.c_int,
+                                                C.POINTER(opt_linear_options), pp]
         L.opt_linear2_plan_create.argtypes = [C.POINTER(opt_linear2_member), C.c_int32, C.c_int, C.c_int, pp]
         L.opt_ln_linear2_plan_create.argtypes = [C.POINTER(opt_ln_linear2_member), C.c_int32, C.c_int, C.c_int, pp]
         L.opt_layernorm_plan_create.argtypes = [C.POINTER(opt_layernorm_member), C.c_int32, C.c_int, C.c_int,
@@ -106,7 +112,7 @@ def lib():
         L.opt_last_error.restype = C.c_char_p
         L.opt_launch_count.restype = C.c_uint64
         L.opt_version.restype = C.c_char_p
-        for f in (L.opt_linear_plan_create, L.opt_linear2_plan_create, L.opt_ln_linear2_plan_create, L.opt_layernorm_plan_create, L.opt_layernorm_bwd_plan_create, L.opt_bias_grad_plan_create, L.opt_pointwise_plan_create,
+        for f in (L.opt_linear_plan_create, L.opt_linear_plan_create_ex, L.opt_linear2_plan_create, L.opt_ln_linear2_plan_create, L.opt_layernorm_plan_create, L.opt_layernorm_bwd_plan_create, L.opt_bias_grad_plan_create, L.opt_pointwise_plan_create,
                   L.opt_plan_launch, L.opt_plan_launch_host, L.opt_plan_info, L.opt_plan_destroy):
             f.restype = C.c_int
         _lib = L
@@ -169,6 +175,14 @@ def _create(fn, ctype, members, *dtype_and_device):
 
 def opt_linear_plan_create(members, io, device=0):
     return _create(lib().opt_linear_plan_create, opt_linear_member, members, io, device)
+
+
+def opt_linear_plan_create_ex(members, io, device=0, options=None):
+    """options: an opt_linear_options (or None for the defaults)."""
+    arr, n = _array(opt_linear_member, members)
+    h = C.c_void_p()
+    _check(lib().opt_linear_plan_create_ex(arr, n, io, device, None if options is None else C.byref(options), C.byref(h)))
+    return Plan(h)
 
 
 def opt_linear2_plan_create(members, io, device=0):

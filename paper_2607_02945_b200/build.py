@@ -23,8 +23,7 @@ def build(force=False, verbose=False):
     if not force and up_to_date():
         return LIB
     nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
-    extra = os.environ.get("OPT_NVCC_EXTRA", "").split()      # experiment knob, e.g. -DPW_MINBLOCKS=6
-    cmd = [nvcc] + NVCC_FLAGS + extra + (["-Xptxas", "-v"] if verbose else []) + \
+    cmd = [nvcc] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + \
           ["-I", os.path.join(ROOT, "include"), "-o", LIB] + SRCS
     subprocess.check_call(cmd)
     return LIB

@@ -52,6 +52,12 @@ opt_status open_device(int device, int* num_sms) {
   return OPT_OK;
 }
 
+DeviceGuard::DeviceGuard() { if (cudaGetDevice(&prev_) != cudaSuccess) { cudaGetLastError(); prev_ = -1; } }
+DeviceGuard::~DeviceGuard() {
+  int cur = -1;
+  if (prev_ >= 0 && cudaGetDevice(&cur) == cudaSuccess && cur != prev_) cudaSetDevice(prev_);
+}
+
 // Exact test for two strided regions that share a row pitch; conservative
 // (reports overlap) otherwise.  Only called when the bounding intervals overlap.
 static bool regions_overlap(const Region& a, const Region& b) {

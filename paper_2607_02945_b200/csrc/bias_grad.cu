@@ -37,16 +37,9 @@ struct BgBlock { int32_t member, row0, nrows, part, vec0; };
 
 constexpr int kBgThreads = 256;
 constexpr int kBgTileVec = 32;       // 32 vectors = 256 bf16 columns per tile
-#ifndef BG_INFLIGHT
-#define BG_INFLIGHT 4
-#endif
-#ifndef BG_BLOCK_BYTES
-#define BG_BLOCK_BYTES 131072
-#endif
-#ifndef BG_MINBLOCKS
-#define BG_MINBLOCKS 6
-#endif
-constexpr int kBgInflight = BG_INFLIGHT;       // rows of loads in flight per thread
+constexpr int kBgMinBlocks = 6;
+constexpr int kBgBlockBytes = 131072;
+constexpr int kBgInflight = 4;       // rows of loads in flight per thread
 
 // torch threshold_backward on a bf16 pair: keep the gradient unless y <= 0 (a NaN y keeps it); the zero written is +0
 __device__ __forceinline__ uint32_t bg_mask2(uint32_t g, uint32_t y) {
@@ -151,7 +144,7 @@ __device__ __forceinline__ void bg_block(const BgMember& m, const BgBlock& b, fl
 // Two instantiations chosen per plan: groups without a fused mask run 6 blocks per SM in 40 registers; a masked member
 // keeps twice the vectors in flight (dY and y) and needs 64 registers (4 blocks per SM) to stay out of local memory.
 template <bool P_BF16, bool ANY_MASK>
-__global__ void __launch_bounds__(kBgThreads, ANY_MASK ? 4 : BG_MINBLOCKS)
+__global__ void __launch_bounds__(kBgThreads, ANY_MASK ? 4 : kBgMinBlocks)
 batched_bias_grad_kernel(const BgMember* __restrict__ members, const BgBlock* __restrict__ blocks) {
   __shared__ __align__(16) float bg_red[kBgThreads * 8];      // [256/L][L*8] floats = 8 KB
   const BgBlock b = blocks[blockIdx.x];
@@ -218,7 +211,7 @@ extern "C" opt_status opt_bias_grad_plan_create(const opt_bias_grad_member* memb
     if (m.N % 8) return fail(OPT_ERR_ALIGNMENT, "member %d: N=%d is not a multiple of 8", i, m.N);
     if (m.M > 1 && m.ldz % 8) return fail(OPT_ERR_ALIGNMENT, "member %d: row stride must be a multiple of 8 elements", i);
     if (m.act < OPT_ACT_NONE || m.act > OPT_ACT_SIGMOID) return fail(OPT_ERR_INVALID_ARG, "member %d: bad act %d", i, m.act);
-    if (m.act > OPT_ACT_RELU && !m.y) return fail(OPT_ERR_INVALID_ARG, "member %d: act %d needs y (the stored forward output)", i, m.act);
+    if (m.act != OPT_ACT_NONE && !m.y) return fail(OPT_ERR_INVALID_ARG, "member %d: act %d needs y (the stored forward output)", i, m.act);
     if (m.dz_out && !m.y) return fail(OPT_ERR_INVALID_ARG, "member %d: dz_out without y (the mask source)", i);
     if (m.y) {
       if (!aligned16(m.y) || !aligned16(m.dz_out)) return fail(OPT_ERR_ALIGNMENT, "member %d: pointers must be 16-byte aligned", i);
@@ -238,7 +231,7 @@ extern "C" opt_status opt_bias_grad_plan_create(const opt_bias_grad_member* memb
     const int nctile = (nvec + kBgTileVec - 1) / kBgTileVec;
     // rows per block: whole groups of in-flight passes, ~128 KB of dZ per block
     const int64_t chunk_rows = (int64_t)rpp * kBgInflight;
-    const int64_t rpb = chunk_rows * std::max<int64_t>(1, BG_BLOCK_BYTES / (chunk_rows * L * 16));
+    const int64_t rpb = chunk_rows * std::max<int64_t>(1, kBgBlockBytes / (chunk_rows * L * 16));
     const int32_t nparts = (int32_t)((m.M + rpb - 1) / rpb);
     BgMember t;
     memset(&t, 0, sizeof t);
@@ -263,6 +256,7 @@ extern "C" opt_status opt_bias_grad_plan_create(const opt_bias_grad_member* memb
   if (blocks.size() > (size_t)INT32_MAX) return fail(OPT_ERR_UNSUPPORTED, "too many work items");
 
   int num_sms = 0;
+  DeviceGuard device_guard;      // the caller's current device is restored on return
   if (opt_status st = open_device(device, &num_sms)) return st;
   auto align_up = [](size_t x) { return (x + 255) & ~size_t(255); };
   opt_plan* p = new opt_plan();

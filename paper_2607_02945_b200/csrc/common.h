@@ -32,8 +32,14 @@ inline int elem_size(opt_dtype dt) { return dt == OPT_F32 ? 4 : 2; }
 inline int vec_elems(opt_dtype dt) { return 16 / elem_size(dt); }   // elements per 16-byte vector
 inline bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
 
-// opens the device (must be sm_100), returns SM count
+// opens the device (must be sm_100) -- makes it the thread's current device -- and returns its SM count
 opt_status open_device(int device, int* num_sms);
+// every *_plan_create holds one of these: the caller's current device is restored when plan creation returns
+struct DeviceGuard {
+  DeviceGuard();
+  ~DeviceGuard();
+  int prev_ = -1;
+};
 
 // ------------------------------------------------------------ alias check ---
 // A strided 2-D byte region: rows x row_bytes, row pitch pitch_bytes.

@@ -3,21 +3,21 @@
 //
 //   mu = mean(x_r); v = mean((x_r - mu)^2); y_r = (x_r - mu) * rsqrt(v + eps) * gamma + beta
 //
-// Design (HBM-bound):
-//   * a row is owned by L = 2^k lanes of one warp (L chosen per member so that
-//     L * VPL 16-byte vectors cover D with the least waste): D=32 packs 16 rows
-//     into a warp, D>=256 uses the whole warp.  Each lane keeps VPL vectors of
-//     the row in registers: x is read from HBM exactly once.
-//   * fp32 statistics, two passes over the registers (mean, then centred sum of
-//     squares), width-L shuffle-xor reductions.
-//   * the next rows' vectors are prefetched before the current rows' math; a
-//     thread works on RU rows at a time (RU x VPL ~ 4 vectors) so that enough
-//     bytes are in flight per SM.
-//   * bf16 path: the kernel is close to ISSUE-bound (ncu: sm throughput 66-81 %
-//     for the first version), so the arithmetic runs on packed fp32 pairs
-//     (add/mul/fma.rn.f32x2) and gamma/beta are staged once per block as fp32 in
-//     shared memory (a block never leaves its member).
-//   * a per-block table (member, first row, row count) maps blocks to members.
+// Two kernels (HBM-bound):
+//   batched_layernorm_staged_kernel   bf16 activations (configs[1], configs[4] group 1).  Persistent CTAs, three
+//       per SM: ONE producer warp + 8 consumer warps around a shared-memory ring (<= 4 stages, 72 KB per CTA).  A
+//       work item is a tile of whole rows of one member (~16 KB); the producer takes items from a dynamic scheduler
+//       (one atomicAdd per chunk of 8 items, software-pipelined three chunks deep) and streams each tile plus the
+//       member's gamma and beta into a stage with cp.async.bulk, counted on the stage's mbarrier; a 64-byte header
+//       tells the consumers what the stage holds.  Consumers never issue a global load: a row is owned by L = 2^k
+//       lanes (L per member for the least lane waste: D=32 packs 8 rows into a warp, D>=256 uses the whole warp),
+//       each lane reads its 16-byte vectors from shared memory, fp32 two-pass statistics (mean, then centred sum
+//       of squares) on packed f32x2 arithmetic with width-L shuffle-xor reductions, affine, one RNE, coalesced
+//       16-byte st.global.cs -- and, when the member asks for it, the FP8 (E4M3) copy of the rounded output
+//       (8-byte stores; activation quantisation fused into the producer of the saved tensor).
+//       Rows wider than 1024 elements stay in shared memory and are re-read per pass.
+//   batched_layernorm_kernel          fp32 activations: register-resident rows, one block per (member, row range)
+//       from a block table, the next rows' vectors prefetched before the current rows' math.
 #include <algorithm>
 #include <cstdlib>
 
@@ -636,6 +636,7 @@ extern "C" opt_status opt_layernorm_plan_create(const opt_layernorm_member* memb
   if (blocks.size() > (size_t)INT32_MAX) return fail(OPT_ERR_UNSUPPORTED, "too many work items");
 
   int num_sms = 0;
+  DeviceGuard device_guard;      // the caller's current device is restored on return
   if (opt_status st = open_device(device, &num_sms)) return st;
   auto align_up = [](size_t x) { return (x + 255) & ~size_t(255); };
   opt_plan* p = new opt_plan();
@@ -651,8 +652,7 @@ extern "C" opt_status opt_layernorm_plan_create(const opt_layernorm_member* memb
     const int n_cta = num_sms * 3;
     // chunks of 8 consecutive items (one 128-byte table line, one atomic); the last 4 waves one item per chunk
     const LnsItem pad_item = {-1, 0, 0, 0};
-    size_t tail_waves = 4;
-    if (const char* e = getenv("OPT_LN_TAIL_WAVES")) tail_waves = (size_t)atol(e);          // experiment knob
+    const size_t tail_waves = 4;
     const size_t tail = std::min(sitems.size(), tail_waves * n_cta);
     const size_t body = sitems.size() - tail;
     std::vector<LnsItem> chunked;
@@ -672,9 +672,11 @@ extern "C" opt_status opt_layernorm_plan_create(const opt_layernorm_member* memb
     memcpy(blob.data() + p->off1, chunked.data(), chunked.size() * sizeof(LnsItem));
     if (opt_status st = upload_tables(p, blob.data(), total)) { delete p; return st; }
     const int smem = (int)(nstages * stage_bytes);
+    // the attribute belongs to the kernel FUNCTION, not to the plan (the last call wins): always the fixed budget,
+    // so that a later, smaller plan never lowers the limit under a live, larger one
     cudaError_t e = param == OPT_BF16
-        ? cudaFuncSetAttribute(batched_layernorm_staged_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem)
-        : cudaFuncSetAttribute(batched_layernorm_staged_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+        ? cudaFuncSetAttribute(batched_layernorm_staged_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, kLnsSmemBudget)
+        : cudaFuncSetAttribute(batched_layernorm_staged_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, kLnsSmemBudget);
     if (e != cudaSuccess) {
       cudaFree(p->dev_tables); delete p;
       return fail(OPT_ERR_CUDA, "cudaFuncSetAttribute(max dynamic smem %d) failed: %s", smem, cudaGetErrorString(e));

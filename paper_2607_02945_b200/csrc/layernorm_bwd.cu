@@ -289,6 +289,7 @@ extern "C" opt_status opt_layernorm_bwd_plan_create(const opt_layernorm_bwd_memb
   if (blocks.size() > (size_t)INT32_MAX) return fail(OPT_ERR_UNSUPPORTED, "too many work items");
 
   int num_sms = 0;
+  DeviceGuard device_guard;      // the caller's current device is restored on return
   if (opt_status st = open_device(device, &num_sms)) return st;
   auto align_up = [](size_t x) { return (x + 255) & ~size_t(255); };
   opt_plan* p = new opt_plan();

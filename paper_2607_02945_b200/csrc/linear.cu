@@ -494,8 +494,18 @@ using namespace optb;
 
 extern "C" opt_status opt_linear_plan_create(const opt_linear_member* members, int32_t n, opt_dtype io, int device,
                                              opt_plan** plan) {
+  return opt_linear_plan_create_ex(members, n, io, device, nullptr, plan);
+}
+
+extern "C" opt_status opt_linear_plan_create_ex(const opt_linear_member* members, int32_t n, opt_dtype io, int device,
+                                                const opt_linear_options* options, opt_plan** plan) {
   if (plan) *plan = nullptr;
   if (!plan || !members) return fail(OPT_ERR_INVALID_ARG, "opt_linear_plan_create: NULL argument");
+  opt_linear_options opts;
+  memset(&opts, 0, sizeof opts);
+  if (options) opts = *options;
+  if (opts.cta_pair < 0 || opts.cta_pair > 2) return fail(OPT_ERR_INVALID_ARG, "options.cta_pair = %d outside {0, 1, 2}", opts.cta_pair);
+  for (int32_t r : opts.reserved) if (r != 0) return fail(OPT_ERR_INVALID_ARG, "options.reserved must be zero");
   if (n < 1 || n > 65535) return fail(OPT_ERR_INVALID_ARG, "n = %d outside [1, 65535]", n);
   if (io != OPT_F32 && io != OPT_BF16) return fail(OPT_ERR_INVALID_ARG, "bad io dtype %d", (int)io);
   const int esz = elem_size(io), V = vec_elems(io);
@@ -503,7 +513,7 @@ extern "C" opt_status opt_linear_plan_create(const opt_linear_member* members, i
   int64_t flops = 0, bytes = 0;
   std::set<std::tuple<const void*, int64_t, int32_t, int32_t>> seen_x;
   // huge-M / tiny-K-and-N groups (decompose_mm_pass) stream through the SIMT row kernel (linear_skinny.cu)
-  bool skinny = io == OPT_BF16 && !getenv("OPT_GEMM_NO_SKINNY");     // (knob for A/B measurements, like OPT_GEMM_NCTA)
+  bool skinny = io == OPT_BF16 && !opts.no_skinny;
   for (int32_t i = 0; skinny && i < n; ++i) skinny = skinny_linear_member(members[i]);
   for (int32_t i = 0; i < n; ++i) {
     const opt_linear_member& m = members[i];
@@ -542,6 +552,7 @@ extern "C" opt_status opt_linear_plan_create(const opt_linear_member* members, i
   if (opt_status st = check_independent(regions, /*allow_inplace_self=*/false)) return st;
 
   int num_sms = 0;
+  DeviceGuard device_guard;      // the caller's current device is restored on return
   if (opt_status st = open_device(device, &num_sms)) return st;
   auto align_up = [](size_t x) { return (x + 255) & ~size_t(255); };
   opt_plan* p = new opt_plan();
@@ -586,10 +597,12 @@ extern "C" opt_status opt_linear_plan_create(const opt_linear_member* members, i
   std::vector<GemmMember> tab(n);
   memset(tab.data(), 0, tab.size() * sizeof(GemmMember));
   // CTA pair (256-row tiles, W shared by the pair) or single CTA (128-row tiles)
-  int ncta = 2;
-  if (const char* e = getenv("OPT_GEMM_NCTA")) ncta = atoi(e) == 1 ? 1 : 2;                // experiment knob
+  int ncta = opts.cta_pair == 1 ? 1 : 2;
   for (int32_t i = 0; i < n; ++i)
-    if (members[i].layout) ncta = 1;           // MN-major (transposed) operand tiles are built per CTA: single-CTA kernel
+    if (members[i].layout) {                   // MN-major (transposed) operand tiles are built per CTA: single-CTA kernel
+      if (opts.cta_pair == 2) { delete p; return fail(OPT_ERR_UNSUPPORTED, "options.cta_pair = 2: member %d has a transposed operand (single-CTA tiles only)", i); }
+      ncta = 1;
+    }
   const int tile_m = kBM * ncta;
   struct MemberTiling { int bn, nbn, nkb, klast; uint32_t idesc, flags; };
   std::vector<MemberTiling> tiling(n);
@@ -654,7 +667,7 @@ extern "C" opt_status opt_linear_plan_create(const opt_linear_member* members, i
       if (lhs.find(key) == lhs.end()) first_seen.push_back(key);
       lhs[key].push_back(i);
     }
-    const bool no_lhs = getenv("OPT_GEMM_NO_LHS") != nullptr;                              // experiment knob
+    const bool no_lhs = opts.no_lhs_order != 0;
     if (no_lhs) { first_seen.clear(); for (int32_t i = 0; i < n; ++i) { const int nmb = (members[i].M + tile_m - 1) / tile_m; for (int mb = 0; mb < nmb; ++mb) push_tiles(i, mb); } }
     for (const auto& key : first_seen) {
       const std::vector<int32_t>& grp = lhs[key];
@@ -668,8 +681,7 @@ extern "C" opt_status opt_linear_plan_create(const opt_linear_member* members, i
   TileEntry pad_entry;
   memset(&pad_entry, 0, sizeof pad_entry);
   pad_entry.member = -1;
-  size_t tail_waves = 3;
-  if (const char* e = getenv("OPT_GEMM_TAIL_WAVES")) tail_waves = (size_t)atol(e);       // experiment knob
+  const size_t tail_waves = 3;
   const int n_sched = num_sms / ncta;                         // persistent CTAs (or CTA pairs)
   const size_t tail = std::min(flat.size(), tail_waves * n_sched);
   const size_t body = flat.size() - tail;
@@ -678,10 +690,9 @@ extern "C" opt_status opt_linear_plan_create(const opt_linear_member* members, i
   // neighbouring tiles (one X panel, fetched from HBM once), and one CTA's consecutive tiles come from
   // different members (an HBM-bound tile's epilogue overlaps a tensor-bound tile's MMAs)
   const size_t nC = (body + kTilesPerChunk - 1) / kTilesPerChunk;
-  const bool strided = getenv("OPT_GEMM_CONTIG_CHUNKS") == nullptr;                        // experiment knob
   for (size_t c = 0; c < nC; ++c)
     for (int g = 0; g < kTilesPerChunk; ++g) {
-      const size_t k = strided ? (size_t)g * nC + c : c * kTilesPerChunk + g;
+      const size_t k = (size_t)g * nC + c;
       chunked.push_back(k < body ? flat[k] : pad_entry);
     }
   for (size_t k = body; k < flat.size(); ++k) {

@@ -57,9 +57,7 @@ constexpr int kT_Mma2Warp = kT_FirstEpiWarp + kT_EpiWarps;     // warp 11: layer
 constexpr int kT_KBlockBytes = kT_BM * kT_BK * 2;          // 16 KB: a 128 x 64 bf16 k-block
 constexpr int kT_W2KBlockBytes = kT_MaxN * kT_BK * 2;      // 8 KB: a 64 x 64 k-block of W2
 constexpr int kT_QDepth = 4;
-#ifndef L2_FLAG_SPIN_LIMIT
-#define L2_FLAG_SPIN_LIMIT 4096       // polls of a member's fold flag before the scheduler warp folds the member itself
-#endif
+constexpr int kT_FlagSpinLimit = 4096;   // polls of a member's fold flag before the scheduler warp folds the member itself
 // shared-memory map
 constexpr int kT_OffX = 0;
 constexpr int kT_OffW1 = kT_OffX + (kT_MaxK / kT_BK) * kT_KBlockBytes;            //  64 KB
@@ -299,7 +297,7 @@ grouped_linear2_sm100_kernel(const L2Member* __restrict__ members, const uint4* 
             int ready = 0;
             if (lane == 0) {
               int f;
-              for (int spin = 0; spin < L2_FLAG_SPIN_LIMIT && !ready; ++spin) {
+              for (int spin = 0; spin < kT_FlagSpinLimit && !ready; ++spin) {
                 asm volatile("ld.acquire.gpu.global.s32 %0, [%1];" : "=r"(f) : "l"(flags + member) : "memory");
                 ready = f == epoch1;
               }
@@ -747,6 +745,7 @@ opt_status create_linear2(const opt_linear2_member* members, const opt_ln_linear
   if (opt_status st = check_independent(regions, /*allow_inplace_self=*/false)) return st;
 
   int num_sms = 0;
+  DeviceGuard device_guard;      // the caller's current device is restored on return
   if (opt_status st = open_device(device, &num_sms)) return st;
   EncodeTiledFn enc = nullptr;
   if (opt_status st = get_encoder(&enc)) return st;
@@ -835,6 +834,7 @@ opt_status create_linear2(const opt_linear2_member* members, const opt_ln_linear
   memcpy(blob.data() + p->off1, chunked.data(), chunked.size() * sizeof(TileEntry2));
   if (opt_status st = upload_tables(p, blob.data(), total)) { delete p; return st; }
   const int smem_bytes = LN ? L2Cfg<true>::kSmemBytes : L2Cfg<false>::kSmemBytes;
+  // (per instantiation, a compile-time constant: every plan of this kernel sets the same value)
   cudaError_t e = LN ? cudaFuncSetAttribute(grouped_linear2_sm100_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_bytes)
                      : cudaFuncSetAttribute(grouped_linear2_sm100_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_bytes);
   if (e != cudaSuccess) {

@@ -25,13 +25,8 @@
 namespace optb {
 
 constexpr int kSkThreads = 256;
-#ifndef SK_UNROLL
-#define SK_UNROLL 4
-#endif
-#ifndef SK_MINBLOCKS
-#define SK_MINBLOCKS 4             // occupancy is what hides the latency here: 4 x 256 threads per SM at <= 64 registers
-#endif
-constexpr int kSkUnroll = SK_UNROLL;                   // 16-row MMA groups per warp and chunk: 8 warps x 4 x 16 = 512 rows
+constexpr int kSkMinBlocks = 4;    // occupancy is what hides the latency here: 4 x 256 threads per SM at <= 64 registers
+constexpr int kSkUnroll = 4;                   // 16-row MMA groups per warp and chunk: 8 warps x 4 x 16 = 512 rows
 constexpr int kSkChunkRows = (kSkThreads / 32) * kSkUnroll * 16;
 constexpr int kSkChunks = 8;                           // chunks a block walks (4096 rows)
 constexpr int kSkRowsPerBlock = kSkChunkRows * kSkChunks;
@@ -136,7 +131,7 @@ __device__ __forceinline__ void sk_rows(const SkMember& m, int row0) {
   }
 }
 
-__global__ void __launch_bounds__(kSkThreads, SK_MINBLOCKS)
+__global__ void __launch_bounds__(kSkThreads, kSkMinBlocks)
 grouped_skinny_linear_kernel(const SkMember* __restrict__ members, const int2* __restrict__ blocks) {
   const int2 b = __ldg(blocks + blockIdx.x);
   const SkMember m = members[b.x];

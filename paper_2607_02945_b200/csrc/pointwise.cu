@@ -295,11 +295,9 @@ __device__ __forceinline__ void pw_staged_tile(const PwGroup& g, const int2* __r
   if (staged_out && threadIdx.x == 0) asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");   // smem outlives the stores' reads
 }
 
-#ifndef PW_MINBLOCKS
-#define PW_MINBLOCKS 6
-#endif
+constexpr int kPwMinBlocks = 6;
 template <bool BF16>
-__global__ void __launch_bounds__(kPwThreads, PW_MINBLOCKS)
+__global__ void __launch_bounds__(kPwThreads, kPwMinBlocks)
 multi_pointwise_splitcat_kernel(const PwGroup* __restrict__ groups, const int2* __restrict__ vmap,
                                 const PwBlock* __restrict__ blocks) {
   const PwBlock b = blocks[blockIdx.x];
@@ -427,6 +425,7 @@ extern "C" opt_status opt_pointwise_plan_create(const opt_chunk* chunks, int32_t
   }
   if (opt_status st = check_independent(regions, /*allow_inplace_self=*/true)) return st;
   int num_sms = 0;
+  DeviceGuard device_guard;      // the caller's current device is restored on return
   if (opt_status st = open_device(device, &num_sms)) return st;
 
   // ---- group canonical chunks by (rows, lds16, ldd16)
@@ -441,8 +440,6 @@ extern "C" opt_status opt_pointwise_plan_create(const opt_chunk* chunks, int32_t
   std::vector<int2> vmap;
   std::vector<PwBlock> blocks;
   size_t smem_needed = 0;
-  int64_t stage_budget = kStageBudget;                       // experiment knob: OPT_PW_STAGE_KB=0 -> direct mode only
-  if (const char* e = getenv("OPT_PW_STAGE_KB")) stage_budget = std::min<int64_t>(200, std::max<int64_t>(0, atol(e))) * 1024;
   for (auto& kv : buckets) {
     std::vector<int>& ids = kv.second;
     std::sort(ids.begin(), ids.end(), [&](int a, int b) { return cc[a].dst < cc[b].dst; });
@@ -495,14 +492,18 @@ extern "C" opt_status opt_pointwise_plan_create(const opt_chunk* chunks, int32_t
       const int64_t sspan = (smax - smin) / 16, dspan = (dmax - dmin) / 16;
       const int64_t nch = (int64_t)(i1 - i0);
       const bool rows_disjoint = g.rows == 1 || (sspan <= g.lds16 && dspan <= g.ldd16);
-      if (stage_budget > 0 && nch > 1 && W < nch * kStageMaxAvgChunk && rows_disjoint && sspan <= kStageMaxSpan && sspan <= W + W / 4) {
+      if (nch > 1 && W < nch * kStageMaxAvgChunk && rows_disjoint && sspan <= kStageMaxSpan && sspan <= W + W / 4) {
         g.src_span = (int32_t)sspan;
         // rows leave through a bulk store only if the chunks tile the destination span without holes
         // (otherwise the store would clobber bytes the group does not own) and nothing is in place
-        if (dspan == W && dspan <= kStageMaxSpan && !self_inplace && !getenv("OPT_PW_NO_SOUT")) g.dst_span = (int32_t)dspan;
+        if (dspan == W && dspan <= kStageMaxSpan && !self_inplace) g.dst_span = (int32_t)dspan;
         // one wave of fat blocks: rows split evenly over the resident block slots (2 per SM), each block
-        // pipelines its rows through a 3-stage source ring and a double-buffered destination row
-        const int64_t need = ((int64_t)kPwInStages * g.src_span + 2 * (int64_t)g.dst_span) * 16;
+        // pipelines its rows through a 3-stage source ring and a double-buffered destination row.  Two blocks
+        // per SM only fit while a block stays within kStageBudget: wide rows give up the staged destination
+        // row (direct 16-byte stores instead of the bulk store), which always fits (3 x 32 KB).
+        int64_t need = ((int64_t)kPwInStages * g.src_span + 2 * (int64_t)g.dst_span) * 16;
+        if (need > kStageBudget) { g.dst_span = 0; need = (int64_t)kPwInStages * g.src_span * 16; }
+        static_assert((int64_t)kPwInStages * kStageMaxSpan * 16 <= kStageBudget, "a staged source ring must fit the budget");
         const int64_t slots = 2 * (int64_t)num_sms;
         g.tile_rows = (int32_t)std::max<int64_t>(std::min<int64_t>(4, g.rows), (g.rows + slots - 1) / slots);
         smem_needed = std::max<size_t>(smem_needed, (size_t)need);
@@ -558,9 +559,11 @@ extern "C" opt_status opt_pointwise_plan_create(const opt_chunk* chunks, int32_t
   memcpy(blob.data() + p->off2, blocks.data(), blocks.size() * sizeof(PwBlock));
   if (opt_status st = upload_tables(p, blob.data(), total)) { delete p; return st; }
   if (smem_needed > 48 * 1024) {
+    // per kernel FUNCTION, not per plan (the last call wins): always the fixed budget, so that a later, smaller
+    // plan never lowers the limit under a live, larger one
     cudaError_t e = io == OPT_BF16
-        ? cudaFuncSetAttribute(multi_pointwise_splitcat_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_needed)
-        : cudaFuncSetAttribute(multi_pointwise_splitcat_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_needed);
+        ? cudaFuncSetAttribute(multi_pointwise_splitcat_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, kStageBudget)
+        : cudaFuncSetAttribute(multi_pointwise_splitcat_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, kStageBudget);
     if (e != cudaSuccess) {
       cudaFree(p->dev_tables); delete p;
       return fail(OPT_ERR_CUDA, "cudaFuncSetAttribute(max dynamic smem %zu) failed: %s", smem_needed, cudaGetErrorString(e));

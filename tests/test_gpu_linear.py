@@ -20,7 +20,7 @@ def ob():
     return ob
 
 
-def run_linear(ob, members, dt, concat=False):
+def run_linear(ob, members, dt, concat=False, options=None):
     """-> list of host outputs (storage dtype) per member; one launch."""
     M = members[0]["M"]
     dx = [to_dev(m["x"], dt) for m in members]
@@ -37,7 +37,7 @@ def run_linear(ob, members, dt, concat=False):
     else:
         ys = [empty_dev((m["M"], m["N"]), dt, fill=float("nan")) for m in members]
     descs = [ob.linear_member(x, w, b, y, m["act"]) for x, w, b, y, m in zip(dx, dw, db, ys, members)]
-    plan = ob.opt_linear_plan_create(descs, dt)
+    plan = ob.opt_linear_plan_create(descs, dt) if options is None else ob.opt_linear_plan_create_ex(descs, dt, 0, options)
     n0 = ob.opt_launch_count()
     plan.launch()
     torch.cuda.synchronize()
@@ -198,15 +198,16 @@ def test_relaunch_rearms_the_scheduler_and_is_bitwise_reproducible(ob):
         assert to_host(ycat).tobytes() == first
 
 
-def test_single_cta_kernel_matches_the_cta_pair_kernel(ob, monkeypatch):
-    """OPT_GEMM_NCTA=1 selects the one-CTA-per-tile instantiation (128-row tiles): same bits as the default
-    CTA-pair kernel (256-row tiles) on ragged shapes -- the K order of the accumulation is the same."""
+def test_single_cta_kernel_matches_the_cta_pair_kernel(ob):
+    """opt_linear_options.cta_pair = 1 selects the one-CTA-per-tile instantiation (128-row tiles): same bits as the
+    default CTA-pair kernel (256-row tiles) on ragged shapes -- the K order of the accumulation is the same."""
     rng = np.random.default_rng(77)
     shapes = [(200, 48, 32), (130, 264, 72), (257, 520, 136), (513, 1024, 256), (100, 8, 8)]
     members = [mk(55, i, M, N, K, i % 4) for i, (M, N, K) in enumerate(shapes)]
     pair, _ = run_linear(ob, members, BF16)
-    monkeypatch.setenv("OPT_GEMM_NCTA", "1")
-    single, _ = run_linear(ob, members, BF16)
+    single, _ = run_linear(ob, members, BF16, options=ob.opt_linear_options(cta_pair=1))
+    forced, _ = run_linear(ob, members, BF16, options=ob.opt_linear_options(cta_pair=2))
+    assert all(a.tobytes() == b.tobytes() for a, b in zip(pair, forced))
     for a, b in zip(pair, single):
         assert a.tobytes() == b.tobytes()
 

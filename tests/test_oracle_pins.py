@@ -467,6 +467,31 @@ def test_ln_linear2_sign_rows_reduce_to_integer_chain_and_affine_invariance():
     assert np.abs(r4["y64"] - t["out64"]).max() <= 2.0 ** -6 * np.abs(t["out64"]).max()
 
 
+def test_linear_f64x_and_colsum_hand_values_and_agreement_with_linear():
+    """oracle_linear_f64x (first layer of the LayerNorm-folded chain, reading Q25) and oracle_colsum (bias gradient):
+    the plain C++ loops, no BLAS.  Pins: an asymmetric hand-computed 2x3x2 case whose activations are NOT storage
+    values (a swapped operand, a dropped bias or a transposed index fails it); on activations that ARE storage
+    values it equals `linear` bit for bit (same summation order); against numpy's matmul to 1e-13; colsum on a
+    strided slice by hand and against numpy."""
+    x64 = np.array([[1.5, -2.0, 0.25], [3.0, 0.5, -1.0]])
+    w = np.array([[1, 2, 3], [4, 5, 6]], dtype=np.float32)
+    b = np.array([10, 20], dtype=np.float32)
+    assert np.array_equal(oracle.linear_f64x(x64, w, b, F32), [[8.25, 17.5], [11.0, 28.5]])
+    assert np.array_equal(oracle.linear_f64x(x64, w, None, F32), [[-1.75, -2.5], [1.0, 8.5]])
+    third = np.array([[1.0 / 3.0, 0.0, 0.0]])                       # not representable in fp32 / bf16: stays fp64
+    assert oracle.linear_f64x(third, w, None, F32)[0, 1] == 4.0 * (1.0 / 3.0)
+    xs = wl.tensor_normal(31, 1, (7, 19), 0.0, 1.0, BF16); ws = wl.tensor_normal(31, 2, (5, 19), 0.0, 0.3, BF16)
+    bs = wl.tensor_normal(31, 3, (5,), 0.0, 0.3, BF16)
+    assert oracle.linear_f64x(oracle.widen(xs, BF16), ws, bs, BF16).tobytes() == oracle.linear(xs, ws, bs, BF16).tobytes()
+    xr = np.random.default_rng(5).standard_normal((6, 19))
+    ref = xr @ oracle.widen(ws, BF16).T + oracle.widen(bs, BF16)
+    assert np.allclose(oracle.linear_f64x(xr, ws, bs, BF16), ref, rtol=1e-13, atol=1e-14)
+    wide = np.arange(24, dtype=np.float32).reshape(4, 6)            # column slice [1:4] of a [4, 6] buffer
+    assert np.array_equal(oracle.colsum(wide[:, 1:4], F32), [1 + 7 + 13 + 19, 2 + 8 + 14 + 20, 3 + 9 + 15 + 21])
+    g = wl.tensor_normal(31, 4, (53, 12), 0.0, 1.0, BF16)
+    assert np.allclose(oracle.colsum(g, BF16), oracle.widen(g, BF16).sum(axis=0), rtol=0, atol=1e-12)
+
+
 # --------------------------------- Table-1 pointwise patterns (SURVEY 8(f) rank 2) --
 def test_pointwise_ext_hand_values_and_special_values():
     """batch_clamp / batch_nan_to_num / batch_aten_sub,div,mul against hand-computed values (torch semantics)."""
