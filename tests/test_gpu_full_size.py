@@ -31,6 +31,18 @@ def sample_rows(n_rows, k, seed):
     return np.array(sorted(rows))
 
 
+def tile_boundary_rows(n_rows, k, seed):
+    """>= k rows: both sides of EVERY 128-row boundary (each CTA's half of every 256-row pair tile, hence every
+    pair-tile boundary too), the first and last rows, and seeded random rows up to k."""
+    rows = {0, 1, n_rows - 2, n_rows - 1}
+    for b in range(128, n_rows, 128):
+        rows.update((b - 1, b))
+    rng = np.random.default_rng(seed)
+    while len(rows) < k:
+        rows.update(int(r) for r in rng.integers(0, n_rows, size=k - len(rows)))
+    return np.array(sorted(r for r in rows if 0 <= r < n_rows))
+
+
 @pytest.fixture(scope="module")
 def step():
     import bench
@@ -74,7 +86,8 @@ def test_c2_full_grouped_linear(step):
     ycat = g.aout.tensor(g.iy)
     worst = 0.0
     for i, m in enumerate(g.cfg["members"]):
-        rows = sample_rows(m["M"], 12, 2000 + i)
+        rows = tile_boundary_rows(m["M"], 256, 2000 + i)
+        assert len(rows) >= 256
         got = to_host(ycat[torch.from_numpy(rows).cuda(), m["col_off"]:m["col_off"] + m["N"]])
         sub = dict(m, x=np.ascontiguousarray(m["x"][rows]))
         z64 = graphs.linear_member(sub, BF16)
@@ -111,6 +124,90 @@ def test_c3_full_split_pointwise_cat(step):
         dpos += w
 
 
+def test_c3_full_all_rows_against_the_oracle(step):
+    """Every one of the 8192 x 8192 outputs against the oracle (reading Q16 (iii)), in row blocks: <= 2 bf16 ulp of
+    f(source element at the mapped index); the oracle's pointwise is row-parallel, 67 M elements take seconds."""
+    g = step["C3_split_pointwise_cat"]
+    cfg = g.cfg
+    out = to_host(g.aout.tensor(g.iy))
+    x, widths, ops, perm = cfg["x"], cfg["widths"], cfg["ops"], cfg["perm"]
+    worst = 0
+    for r0 in range(0, cfg["rows"], 1024):
+        _, ref = graphs.split_pointwise_cat(np.ascontiguousarray(x[r0:r0 + 1024]), widths, ops, perm, BF16)
+        worst = max(worst, int(bf16_ulp_distance(out[r0:r0 + 1024], ref).max()))
+    assert worst <= 2, "max ulp %d" % worst
+
+
+def test_c3_full_movement_bit_exact_on_the_whole_tensor(step):
+    """`north_star`: "movement checked bit-exact" (reading Q16 (i) and (ii)) at configs[3]'s
+    FULL size, same widths / permutation / launch shape as the timed plan, every op = COPY:
+    (i) the whole output equals the oracle's split -> cat in permuted order, byte for byte;
+    (ii) with the identity permutation the output IS the input (split followed by cat of the same chunks)."""
+    import paper_2607_02945_b200 as ob
+    g = step["C3_split_pointwise_cat"]
+    cfg = g.cfg
+    x_dev = g.ain.tensor(g.ix)
+    widths, perm = cfg["widths"], cfg["perm"]
+    n = len(widths)
+    out = torch.empty_like(x_dev)
+    out.fill_(float("nan"))
+    plan = ob.opt_pointwise_plan_create(ob.split_cat_chunks(x_dev, out, widths, [wl.gen.PW_COPY] * n, perm), BF16)
+    assert plan.info()["tiles"] == g.plan.info()["tiles"], "same launch shape as the timed plan"
+    n0 = ob.opt_launch_count()
+    plan.launch()
+    torch.cuda.synchronize()
+    assert ob.opt_launch_count() - n0 == 1
+    assert to_host(out).tobytes() == graphs.split_copy_cat(cfg["x"], widths, perm).tobytes()
+    out.fill_(float("nan"))
+    ident = ob.opt_pointwise_plan_create(ob.split_cat_chunks(x_dev, out, widths, [wl.gen.PW_COPY] * n, list(range(n))), BF16)
+    ident.launch()
+    torch.cuda.synchronize()
+    assert to_host(out).tobytes() == np.ascontiguousarray(cfg["x"]).tobytes()
+    assert graphs.split_copy_cat(cfg["x"], widths, list(range(n))).tobytes() == np.ascontiguousarray(cfg["x"]).tobytes()
+
+
+def _single_member_outputs(ob, descs_of, out_like):
+    """Run every member as its OWN one-member plan into a fresh buffer shaped like the group's output."""
+    alt = torch.empty_like(out_like)
+    alt.fill_(float("nan"))
+    plans = [ob.opt_linear_plan_create([d], BF16) for d in descs_of(alt)]
+    for p in plans:
+        p.launch()
+    torch.cuda.synchronize()
+    return alt
+
+
+def test_c2_full_fused_equals_single_member_plans_bitwise(step):
+    """All 4096 rows of all 128 members: the ONE fused launch against 128 single-member launches of the same library
+    (same tile shapes and K order => the same bits).  Catches any scheduler / queue / concat-slot fault in rows the
+    oracle sample does not visit; the single-member plans are themselves gated against the oracle on small shapes."""
+    import paper_2607_02945_b200 as ob
+    g = step["C2_grouped_linear_tower"]
+    ycat = g.aout.tensor(g.iy)
+    T = g.ain.tensor
+    alt = _single_member_outputs(ob, lambda buf: [ob.linear_member(T(ix), T(iw), T(ib), buf[:, m["col_off"]:m["col_off"] + m["N"]], m["act"])
+                                                  for (ix, iw, ib), m in zip(g.idx, g.cfg["members"])], ycat)
+    assert torch.equal(alt.view(torch.int16), ycat.view(torch.int16))
+
+
+def test_c4_full_fused_equals_single_member_plans_bitwise(step):
+    """Same cross-check for configs[4]'s two GEMM groups (all 8192 rows of all 512 towers)."""
+    import paper_2607_02945_b200 as ob
+    ga, gc = step["C4a_batched_layernorm"], step["C4c_grouped_linear_concat"]
+    T, A = ga.ain.tensor, ga.amid.tensor
+    towers = ga.cfg["towers"]
+    for k, (i, t) in enumerate(zip(ga.idx, towers)):          # group 2: per-tower hidden tensors
+        h = A(i["h"])
+        alt = torch.empty_like(h)
+        ob.opt_linear_plan_create([ob.linear_member(A(i["xn"]), T(i["w1"]), T(i["b1"]), alt, 1)], BF16).launch()
+        torch.cuda.synchronize()
+        assert torch.equal(alt.view(torch.int16), h.view(torch.int16)), k
+    out = gc.aout.tensor(gc.iy)
+    alt = _single_member_outputs(ob, lambda buf: [ob.linear_member(A(i["h"]), T(i["w2"]), T(i["b2"]), buf[:, k * t["out"]:(k + 1) * t["out"]], 0)
+                                                  for k, (i, t) in enumerate(zip(ga.idx, towers))], out)
+    assert torch.equal(alt.view(torch.int16), out.view(torch.int16))
+
+
 def test_c4_full_three_groups(step):
     ga, gb, gc = step["C4a_batched_layernorm"], step["C4b_grouped_linear_relu"], step["C4c_grouped_linear_concat"]
     towers = ga.cfg["towers"]
@@ -118,9 +215,9 @@ def test_c4_full_three_groups(step):
     amid = ga.amid
     esc = tot = 0
     worst_b = worst_c = worst_e2e = 0.0
-    for k in range(0, len(towers), 4):                 # every 4th tower: all (D, H) classes, 128 towers
+    for k in range(0, len(towers), 2):                 # every 2nd tower: all (D, H) classes, 256 towers
         t, i = towers[k], ga.idx[k]
-        rows = sample_rows(t["B"], 6, 4000 + k)
+        rows = tile_boundary_rows(t["B"], 256, 4000 + k)   # both sides of every 128-row boundary + random rows
         rsel = torch.from_numpy(rows).cuda()
         xn = to_host(amid.tensor(i["xn"])[rsel])
         h = to_host(amid.tensor(i["h"])[rsel])
