@@ -504,6 +504,7 @@ def run_side(args):
                        opt_linear_options.no_lhs_order (plain member-major schedule)
     Prints one JSON line; not the bench metric."""
     import torch
+    from ctypes import c_void_p as C_void_p
     import paper_2607_02945_b200 as ob
     torch.cuda.set_device(0)
     stream = torch.cuda.current_stream()
@@ -573,6 +574,66 @@ def run_side(args):
                    two_launch_us=round(timed(lambda: (pm.launch(), pb2.launch()), 5), 1),
                    two_launch_bytes=pm.info()["bytes"] + pb2.info()["bytes"])
         print(json.dumps(res))
+    elif args.side == "gemm_trace":
+        # where the grouped GEMM's warp roles wait: the pipeline-trace build of the library (-DOPTB_GEMM_TRACE; a
+        # separate .so) adds up clock64() cycles spent blocked per barrier, one record per CTA.  Workloads: configs[2]
+        # (with the ring-depth sensitivity) and the batch_linear_lhs side group (8 x N=64 on one X).
+        from paper_2607_02945_b200 import binding
+        binding.use_trace_library()
+        grid = 148
+        buf = torch.zeros(grid * 16, dtype=torch.int64, device="cuda")
+        assert binding.lib().opt_trace_set_gemm_buffer(C_void_p(buf.data_ptr())) == 0
+        flush = torch.empty(256 * 1024 * 1024, dtype=torch.uint8, device="cuda")
+
+        def trace(plan):
+            for _ in range(3):
+                plan.launch()
+            torch.cuda.synchronize()
+            us = timed(plan.launch, 5)
+            buf.zero_()
+            flush.fill_(1)
+            plan.launch()
+            torch.cuda.synchronize()
+            r = buf.cpu().numpy().reshape(grid, 16).astype(np.float64)
+            lead, peer = r[0::2], r[1::2]
+            pct = lambda a, tot: [round(float(v), 1) for v in np.percentile(100.0 * a / np.maximum(tot, 1), [0, 50, 100])]
+            return dict(us=round(us, 1), pairs=int(lead.shape[0]),
+                        mma_total_cycles_min_med_max=[int(v) for v in np.percentile(lead[:, 3], [0, 50, 100])],
+                        mma_wait_full_pct=pct(lead[:, 5], lead[:, 3]), mma_wait_tempty_pct=pct(lead[:, 6], lead[:, 3]),
+                        mma_wait_queue_pct=pct(lead[:, 4], lead[:, 3]),
+                        mma_issue_pct=pct(lead[:, 3] - lead[:, 4] - lead[:, 5] - lead[:, 6], lead[:, 3]),
+                        tiles_per_pair_min_med_max=[int(v) for v in np.percentile(lead[:, 7], [0, 50, 100])],
+                        tensor_cycles_per_pair_min_med_max=[int(v) for v in np.percentile(lead[:, 8] * 2, [0, 50, 100])],
+                        tensor_busy_pct=pct(lead[:, 8] * 2, lead[:, 3]),
+                        producer_wait_empty_pct=pct(lead[:, 2], lead[:, 0]), producer_wait_queue_pct=pct(lead[:, 1], lead[:, 0]),
+                        peer_producer_wait_empty_pct=pct(peer[:, 2], peer[:, 0]),
+                        epilogue_wait_tfull_pct=pct(lead[:, 11], lead[:, 9]), epilogue_wait_store_pct=pct(lead[:, 12], lead[:, 9]),
+                        epilogue_wait_queue_pct=pct(lead[:, 10], lead[:, 9]))
+
+        step = Step("cuda:0", FULL, pinned_host=False, configs=("c2",))
+        g = step.groups[0]
+        c2 = trace(g.plan)
+        depth = {}
+        for ns in (2, 3, 4, 5):        # ring-depth sensitivity (trace build only): latency-bound or bandwidth-bound?
+            o = ob.opt_linear_options(); o.reserved[0] = ns
+            ycat = g.aout.tensor(g.iy)
+            pd = ob.opt_linear_plan_create_ex([ob.linear_member(g.ain.tensor(ix), g.ain.tensor(iw), g.ain.tensor(ib),
+                                                                 ycat[:, m["col_off"]:m["col_off"] + m["N"]], m["act"])
+                                               for (ix, iw, ib), m in zip(g.idx, g.cfg["members"])], BF16, 0, o)
+            pd.launch(); torch.cuda.synchronize()
+            depth[str(ns)] = round(timed(pd.launch, 5), 1)
+        c2["us_by_ring_stages"] = depth
+        del step, g
+        M, K, N, n = 262144, 512, 64, 8
+        gen = torch.Generator(device="cuda").manual_seed(0)
+        x = torch.randn(M, K, device="cuda", generator=gen).to(torch.bfloat16)
+        ws = [(torch.randn(N, K, device="cuda", generator=gen) * K ** -0.5).to(torch.bfloat16) for _ in range(n)]
+        ycat = torch.empty(M, N * n, device="cuda", dtype=torch.bfloat16)
+        lhs = trace(ob.opt_linear_plan_create([ob.linear_member(x, w, None, ycat[:, i * N:(i + 1) * N], ACT_RELU) for i, w in enumerate(ws)], BF16, 0))
+        print(json.dumps(dict(side="gemm_trace", configs2=c2, batch_linear_lhs_8xN64=lhs,
+                              note="percentages of the role's own loop time, [min, median, max] over the CTA pairs; tensor cycles = "
+                                   "sum over tiles of k-blocks x (BN / 256) x 512 (a 256 x 256 x 64 k-block keeps the pair's tensor "
+                                   "pipes busy for 512 cycles)")))
     elif args.side == "fp8":
         step = Step("cuda:0", FULL, pinned_host=False, configs=("c4",))
         ga = step.groups[0]
@@ -1096,7 +1157,7 @@ def main():
     ap.add_argument("--profile", action="store_true",
                     help="only the step's own launches (no cpu_baseline, no unfused baseline, no copy reference): for ncu")
     ap.add_argument("--ref-frac", type=float, default=0.0, help="reference arm: override the row-sample fraction")
-    ap.add_argument("--side", default=None, choices=["linear2", "ln_linear2", "lhs", "skinny", "fp8", "bias_grad"], help="stand-alone side workload for ncu (not the metric)")
+    ap.add_argument("--side", default=None, choices=["linear2", "ln_linear2", "lhs", "skinny", "fp8", "bias_grad", "gemm_trace"], help="stand-alone side workload for ncu (not the metric)")
     args = ap.parse_args()
     if args.side:
         return run_side(args)

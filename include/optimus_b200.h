@@ -126,6 +126,16 @@ typedef struct {
   int32_t M, N, K;
   int32_t act;    /* opt_act */
   int32_t layout; /* 0, or OPT_LAYOUT_* flags: an operand stored transposed (bf16 groups only) */
+  /* Optional FP8 copy of the output, written by the same epilogue (activation quantisation fused into the op that
+   * produces the saved activation: activation_quantization_aten_pass, `use_scaling`):
+   *     y8[m, n] = e4m3_rne_satfinite( bf16(Y[m, n]) * scale8 )          (OCP E4M3, 1 byte per element)
+   * i.e. exactly what OPT_PW_QUANT_E4M3 with p0 = scale8 produces from the stored bf16 Y -- bit for bit -- without
+   * the extra read of Y.  y8:[M,N] bytes, row stride ldy8 BYTES (ldy8 % 16 == 0, 16-byte aligned base, N % 16 == 0).
+   * y8 == NULL: no FP8 output.  With y8 given, y may be NULL (only the FP8 copy is written).  bf16 groups, layout 0.
+   * Zero-initialise the three fields otherwise.                                                                    */
+  void* y8;
+  int64_t ldy8;
+  float scale8;
 } opt_linear_member;
 
 /* One member of a grouped CHAINED Linear -- two Linear layers of a tower fused
@@ -180,7 +190,7 @@ typedef struct {
  *     mu = mean(x_r), v = mean((x_r - mu)^2)  (biased), over the last dim D
  *     y_r = (x_r - mu) / sqrt(v + eps) * gamma + beta
  * x:[rows,D] (ldx), y:[rows,D] (ldy), gamma/beta:[D] or NULL (NULL = 1 / 0).
- * Statistics and affine in fp32 (two-pass over registers), one rounding.     */
+ * Statistics and affine in fp32 (two-pass), one rounding.                     */
 typedef struct {
   const void* x;
   int64_t ldx;
@@ -190,6 +200,12 @@ typedef struct {
   const void* beta;
   int32_t rows, D;
   float eps;
+  /* Optional FP8 (E4M3) copy of the output, same contract as opt_linear_member.y8:
+   *     y8[r, j] = e4m3_rne_satfinite( bf16(y[r, j]) * scale8 ),   y8:[rows,D] bytes, row stride ldy8 BYTES (% 8 == 0),
+   * 8-byte aligned base; bf16 activations only.  With y8 given, y may be NULL.  Zero-initialise otherwise.        */
+  void* y8;
+  int64_t ldy8;
+  float scale8;
 } opt_layernorm_member;
 
 /* One member of a batched LayerNorm BACKWARD (torch

@@ -10,7 +10,7 @@ between the groups of configs[4] (reading Q3).
 import numpy as np
 
 from . import (BF16, F32, activation, cat, colsum, layernorm, linear, linear_f64x, pointwise,  # noqa: F401
-               round_to_storage, split)
+               quant_e4m3, round_to_storage, split)
 
 
 def linear_member(m, dt):
@@ -28,6 +28,28 @@ def linear_group(members, dt):
 def linear_group_concat(members, dt):
     z64, ys = linear_group(members, dt)
     return z64, cat(ys)
+
+
+def saved_activation_fp8(y_storage, scale, dt=BF16):
+    """activation_quantization_aten_pass as the unfused graph runs it: the op's output
+    is first materialised in the storage dtype, THEN quantised -- code = e4m3_rne_satfinite(y_storage * scale).
+    A fused epilogue that also emits the FP8 copy must produce exactly these codes (reading Q29).  No new arithmetic:
+    `quant_e4m3` applied to the rounded output."""
+    return quant_e4m3(y_storage, scale, dt)
+
+
+def linear_member_fp8(m, scale, dt=BF16):
+    """Linear + bias + activation, rounded to storage, and the FP8 copy of that rounded tensor.  -> (y64, y, codes)."""
+    y64 = linear_member(m, dt)
+    y = round_to_storage(y64, dt)
+    return y64, y, saved_activation_fp8(y, scale, dt)
+
+
+def layernorm_fp8(m, scale, dt=BF16):
+    """LayerNorm, rounded to storage, and the FP8 copy of that rounded tensor.  -> (y64, y, codes)."""
+    y64 = layernorm(m["x"], m.get("gamma"), m.get("beta"), m["eps"], dt)
+    y = round_to_storage(y64, dt)
+    return y64, y, saved_activation_fp8(y, scale, dt)
 
 
 def layernorm_group(members, dt):

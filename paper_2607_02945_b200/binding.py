@@ -21,7 +21,8 @@ _STATUS_NAMES = ["OPT_OK", "OPT_ERR_INVALID_ARG", "OPT_ERR_UNSUPPORTED", "OPT_ER
 class opt_linear_member(C.Structure):
     _fields_ = [("x", C.c_void_p), ("ldx", C.c_int64), ("w", C.c_void_p), ("ldw", C.c_int64),
                 ("bias", C.c_void_p), ("y", C.c_void_p), ("ldy", C.c_int64),
-                ("M", C.c_int32), ("N", C.c_int32), ("K", C.c_int32), ("act", C.c_int32), ("layout", C.c_int32)]
+                ("M", C.c_int32), ("N", C.c_int32), ("K", C.c_int32), ("act", C.c_int32), ("layout", C.c_int32),
+                ("y8", C.c_void_p), ("ldy8", C.c_int64), ("scale8", C.c_float)]
 
 
 class opt_linear_options(C.Structure):
@@ -43,7 +44,8 @@ class opt_ln_linear2_member(C.Structure):
 class opt_layernorm_member(C.Structure):
     _fields_ = [("x", C.c_void_p), ("ldx", C.c_int64), ("y", C.c_void_p), ("ldy", C.c_int64),
                 ("gamma", C.c_void_p), ("beta", C.c_void_p),
-                ("rows", C.c_int32), ("D", C.c_int32), ("eps", C.c_float)]
+                ("rows", C.c_int32), ("D", C.c_int32), ("eps", C.c_float),
+                ("y8", C.c_void_p), ("ldy8", C.c_int64), ("scale8", C.c_float)]
 
 
 class opt_layernorm_bwd_member(C.Structure):
@@ -78,20 +80,31 @@ _lib = None
 
 
 def lib_path():
-    return _build.LIB
+    return _lib_path or _build.LIB
+
+
+_lib_path = None
+
+
+def use_trace_library():
+    """Measurement aid (bench.py --side gemm_trace): make this process load the pipeline-trace build of the library
+    (liboptimus_b200_trace.so: same kernels + wait-cycle counters in the grouped GEMM).  Call before the first use."""
+    global _lib_path
+    assert _lib is None, "the library is already loaded"
+    _lib_path = _build.build(trace=True)
 
 
 def lib():
     """Load (building if needed) liboptimus_b200.so.  Raises if it cannot be had: no fallback."""
     global _lib
     if _lib is None:
-        if not os.path.exists(_build.LIB) or not _build.up_to_date():
+        if _lib_path is None and (not os.path.exists(_build.LIB) or not _build.up_to_date()):
             try:
                 _build.build()
             except Exception as e:  # noqa: BLE001
                 if not os.path.exists(_build.LIB):
                     raise ImportError("liboptimus_b200.so is missing and could not be built with nvcc: %r" % (e,))
-        L = C.CDLL(_build.LIB)
+        L = C.CDLL(_lib_path or _build.LIB)
         pp = C.POINTER(C.c_void_p)
         L.opt_linear_plan_create.argtypes = [C.POINTER(opt_linear_member), C.c_int32, C.c_int, C.c_int, pp]
         L.opt_linear_plan_create_ex.argtypes = [C.POINTER(opt_linear_member), C.c_int32, C.c_int, C.c_int,
@@ -246,14 +259,18 @@ def _ld(t):
     return t.stride(0)
 
 
-def linear_member(x, w, bias, y, act=OPT_ACT_NONE, layout=0):
-    """layout: OPT_LAYOUT_* flags; a transposed operand is passed as it is stored ([K,M] / [K,N])."""
-    M, N = y.shape
+def linear_member(x, w, bias, y, act=OPT_ACT_NONE, layout=0, y8=None, scale8=0.0):
+    """layout: OPT_LAYOUT_* flags; a transposed operand is passed as it is stored ([K,M] / [K,N]).
+    y8: optional uint8 [M,N] tensor for the FP8 (E4M3) copy of the output (y may then be None)."""
+    M, N = (y if y is not None else y8).shape
     K = x.shape[0] if layout & OPT_LAYOUT_X_TRANSPOSED else x.shape[1]
     assert tuple(x.shape) == ((K, M) if layout & OPT_LAYOUT_X_TRANSPOSED else (M, K))
     assert tuple(w.shape) == ((K, N) if layout & OPT_LAYOUT_W_TRANSPOSED else (N, K))
+    assert y8 is None or (tuple(y8.shape) == (M, N) and y8.element_size() == 1)
     return opt_linear_member(x.data_ptr(), _ld(x), w.data_ptr(), _ld(w),
-                             None if bias is None else bias.data_ptr(), y.data_ptr(), _ld(y), M, N, K, int(act), int(layout))
+                             None if bias is None else bias.data_ptr(), None if y is None else y.data_ptr(),
+                             0 if y is None else _ld(y), M, N, K, int(act), int(layout),
+                             None if y8 is None else y8.data_ptr(), 0 if y8 is None else _ld(y8), float(scale8))
 
 
 def linear2_member(x, w1, b1, w2, b2, y, act1=OPT_ACT_RELU, act2=OPT_ACT_NONE):
@@ -272,12 +289,15 @@ def ln_linear2_member(x, gamma, beta, eps, w1, b1, w2, b2, y, act1=OPT_ACT_RELU,
                                  None if beta is None else beta.data_ptr(), float(eps), 0)
 
 
-def layernorm_member(x, y, gamma, beta, eps):
+def layernorm_member(x, y, gamma, beta, eps, y8=None, scale8=0.0):
+    """y8: optional uint8 [rows,D] tensor for the FP8 (E4M3) copy of the output (y may then be None)."""
     rows, D = x.shape
-    assert tuple(y.shape) == (rows, D)
-    return opt_layernorm_member(x.data_ptr(), _ld(x), y.data_ptr(), _ld(y),
+    assert y is None or tuple(y.shape) == (rows, D)
+    assert y8 is None or (tuple(y8.shape) == (rows, D) and y8.element_size() == 1)
+    return opt_layernorm_member(x.data_ptr(), _ld(x), None if y is None else y.data_ptr(), 0 if y is None else _ld(y),
                                 None if gamma is None else gamma.data_ptr(),
-                                None if beta is None else beta.data_ptr(), rows, D, float(eps))
+                                None if beta is None else beta.data_ptr(), rows, D, float(eps),
+                                None if y8 is None else y8.data_ptr(), 0 if y8 is None else _ld(y8), float(scale8))
 
 
 def layernorm_bwd_member(x, dy, gamma, dx, dgamma, dbeta, eps):

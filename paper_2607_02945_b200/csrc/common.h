@@ -4,6 +4,7 @@
 #pragma once
 #include <cuda_runtime.h>
 #include <cuda_bf16.h>
+#include <cuda_fp8.h>
 
 #include <cstdarg>
 #include <cstdint>
@@ -134,6 +135,15 @@ __device__ __forceinline__ uint32_t pack_bf16x2(float lo, float hi) {
 }
 __device__ __forceinline__ float bf16_lo(uint32_t u) { return __uint_as_float(u << 16); }
 __device__ __forceinline__ float bf16_hi(uint32_t u) { return __uint_as_float(u & 0xFFFF0000u); }
+
+// FP8 (OCP E4M3) quantisation of four bf16 values held as two packed pairs (reading Q24: the product value x scale
+// is formed in fp32, then one saturating round-to-nearest-even; NaN -> NaN).  Lowest column in the low byte.  ONE
+// definition for the stand-alone op (OPT_PW_QUANT_E4M3) and the fused epilogues (grouped Linear, batched LayerNorm).
+__device__ __forceinline__ uint32_t quant4_e4m3(uint32_t a, uint32_t b, float scale) {
+  const uint32_t lo = __nv_cvt_float2_to_fp8x2(make_float2(bf16_lo(a) * scale, bf16_hi(a) * scale), __NV_SATFINITE, __NV_E4M3);
+  const uint32_t hi = __nv_cvt_float2_to_fp8x2(make_float2(bf16_lo(b) * scale, bf16_hi(b) * scale), __NV_SATFINITE, __NV_E4M3);
+  return lo | (hi << 16);
+}
 
 // ---- packed fp32 pairs (sm_100 add/mul/fma.rn.f32x2) -------------------------
 typedef unsigned long long f32x2;

@@ -239,13 +239,14 @@ struct LnsHdr {               // what the consumers need of a staged item (writt
   int32_t member, row0, nrows, nvec;
   char* y; int64_t ldy16;
   float eps, inv_D; uint32_t shape;       // l_log2 | vpl << 8 | has_gamma << 16 | has_beta << 17
-  uint32_t pad[5];
+  uint32_t pad;
+  char* y8; int32_t ldy8_8; float scale8;  // FP8 copy of the output (Q8 kernel): base, row stride in 8-byte vectors, scale
 };
 static_assert(sizeof(LnsHdr) == kLnsHdrBytes, "LnsHdr is the 64-byte stage header");
 
 // FAST: every lane's vectors exist (D = 8 L VPL), the tile is whole passes, gamma and beta are present --
 // the common case, compiled without any predicate or branch in the loop body.
-template <bool P_BF16, int VPL, int RU, bool FAST>
+template <bool P_BF16, int VPL, int RU, bool FAST, bool Q8>
 __device__ __forceinline__ void lns_tile(const LnsHdr& h, uint32_t tile, uint32_t sgamma, uint32_t sbeta) {
   const int l_log2 = h.shape & 0xFF;
   const bool has_g = FAST || ((h.shape >> 16) & 1), has_b = FAST || ((h.shape >> 17) & 1);
@@ -265,8 +266,12 @@ __device__ __forceinline__ void lns_tile(const LnsHdr& h, uint32_t tile, uint32_
   const uint32_t row_step = (uint32_t)rpp * row_bytes;
   int4* yrow = yb + (int64_t)(h.row0 + row_in_pass) * h.ldy16 + lane_in_row;
   const int64_t y_step = (int64_t)rpp * h.ldy16;
+  // FP8 copy of the rounded output (activation quantisation fused into the LayerNorm)
+  int2* y8row = Q8 ? reinterpret_cast<int2*>(h.y8) + (int64_t)(h.row0 + row_in_pass) * h.ldy8_8 + lane_in_row : nullptr;
+  const int64_t y8_step = Q8 ? (int64_t)rpp * h.ldy8_8 : 0;
+  const bool wr_y = !Q8 || h.y != nullptr, wr_y8 = Q8 && h.y8 != nullptr;
   int rbase = row_in_pass;
-  for (int it = 0; it < niter; ++it, xaddr += RU * row_step, yrow += RU * y_step, rbase += RU * rpp) {
+  for (int it = 0; it < niter; ++it, xaddr += RU * row_step, yrow += RU * y_step, y8row += RU * y8_step, rbase += RU * rpp) {
     f32x2 x[RU][VPL][4];
     float s[RU], q[RU];
 #pragma unroll
@@ -322,14 +327,16 @@ __device__ __forceinline__ void lns_tile(const LnsHdr& h, uint32_t tile, uint32_
         o.y = (int)f2_to_bf2(fma2(mul2(x[u][i][1], rstd2), g[1], b[1]));
         o.z = (int)f2_to_bf2(fma2(mul2(x[u][i][2], rstd2), g[2], b[2]));
         o.w = (int)f2_to_bf2(fma2(mul2(x[u][i][3], rstd2), g[3], b[3]));
-        __stcs(yrow + u * y_step + i * L, o);
+        if (wr_y) __stcs(yrow + u * y_step + i * L, o);
+        if (wr_y8) __stcs(y8row + u * y8_step + i * L, make_int2((int)quant4_e4m3((uint32_t)o.x, (uint32_t)o.y, h.scale8),
+                                                                 (int)quant4_e4m3((uint32_t)o.z, (uint32_t)o.w, h.scale8)));
       }
     }
   }
 }
 
 // rows wider than 4 vectors per lane (D > 1024): the row stays in shared memory and is re-read per pass
-template <bool P_BF16>
+template <bool P_BF16, bool Q8>
 __device__ __forceinline__ void lns_tile_wide(const LnsHdr& h, uint32_t tile, uint32_t sgamma, uint32_t sbeta) {
   const bool has_g = (h.shape >> 16) & 1, has_b = (h.shape >> 17) & 1;
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -366,16 +373,21 @@ __device__ __forceinline__ void lns_tile_wide(const LnsHdr& h, uint32_t tile, ui
       uint32_t o[4];
 #pragma unroll
       for (int k = 0; k < 4; ++k) o[k] = f2_to_bf2(fma2(mul2(add2(bf2_to_f2(ww[k]), nmu2), rstd2), g[k], b[k]));
-      __stcs(yb + (int64_t)(h.row0 + r) * h.ldy16 + v, make_int4((int)o[0], (int)o[1], (int)o[2], (int)o[3]));
+      if (!Q8 || h.y != nullptr) __stcs(yb + (int64_t)(h.row0 + r) * h.ldy16 + v, make_int4((int)o[0], (int)o[1], (int)o[2], (int)o[3]));
+      if (Q8 && h.y8 != nullptr)
+        __stcs(reinterpret_cast<int2*>(h.y8) + (int64_t)(h.row0 + r) * h.ldy8_8 + v,
+               make_int2((int)quant4_e4m3(o[0], o[1], h.scale8), (int)quant4_e4m3(o[2], o[3], h.scale8)));
     }
   }
 }
 
 // stage layout: [tile_max bytes of rows][gamma: pmax][beta: pmax][64-byte header]
-template <bool P_BF16>
+// Q8: some member wants the FP8 (E4M3) copy of its output; `ext` then holds one 16-byte record per member
+// {y8 pointer, row stride in 8-byte vectors, scale8} (y8 == NULL: none for that member).
+template <bool P_BF16, bool Q8>
 __global__ void __launch_bounds__(kLnsThreads, 3)
 batched_layernorm_staged_kernel(const LnsMember* __restrict__ members, const LnsItem* __restrict__ items, int n_chunks,
-                                int* __restrict__ counters, int nstages, int tile_max, int pmax) {
+                                int* __restrict__ counters, int nstages, int tile_max, int pmax, const uint4* __restrict__ ext) {
   extern __shared__ __align__(128) uint8_t lns_smem[];
   __shared__ __align__(8) uint64_t bars[2 * kLnsMaxStages];
   const uint32_t sbase = lns_smem_u32(lns_smem);
@@ -410,15 +422,22 @@ batched_layernorm_staged_kernel(const LnsMember* __restrict__ members, const Lns
       if (mem >= 0) v = __ldg(reinterpret_cast<const uint4*>(members + mem) + (lane & 3));
       return v;
     };
+    auto load_ext = [&](const int4& line) {        // lane g < 8: the FP8 record of item g's member
+      uint4 v = make_uint4(0, 0, 0, 0);
+      if (Q8 && lane < kLnsItemsPerChunk && line.x >= 0) v = __ldg(ext + line.x);
+      return v;
+    };
     int c0 = blockIdx.x;
     int4 line0 = load_line(c0);
     int c1 = __shfl_sync(0xffffffffu, fetch_id(), 0);
     int4 line1 = load_line(c1);
     int c2 = fetch_id();
     uint4 mv0 = load_members(line0);
+    uint4 xv0 = load_ext(line0);
     while (c0 < n_chunks) {
       c2 = __shfl_sync(0xffffffffu, c2, 0);
       const uint4 mv1 = load_members(line1);
+      const uint4 xv1 = load_ext(line1);
       const int4 line2 = load_line(c2);
       const int c3 = fetch_id();
 #pragma unroll 1
@@ -440,6 +459,9 @@ batched_layernorm_staged_kernel(const LnsMember* __restrict__ members, const Lns
         m.l_log2 = (uint8_t)(shp & 0xFF); m.vpl = (uint8_t)((shp >> 8) & 0xFF); m.contiguous = (uint8_t)((shp >> 16) & 0xFF);
         const uint32_t row_bytes = (uint32_t)m.nvec * 16u;
         const uint32_t pbytes = (uint32_t)m.nvec * (P_BF16 ? 16u : 32u);
+        uint4 xe = make_uint4(0, 0, 0, 0);
+        if (Q8) { xe.x = __shfl_sync(0xffffffffu, xv0.x, g); xe.y = __shfl_sync(0xffffffffu, xv0.y, g);
+                  xe.z = __shfl_sync(0xffffffffu, xv0.z, g); xe.w = __shfl_sync(0xffffffffu, xv0.w, g); }
         lns_mbar_wait(empty_bar(s), ph ^ 1);
         const uint32_t stage = sbase + (uint32_t)s * stage_bytes;
         const uint32_t fb = full_bar(s);
@@ -452,6 +474,7 @@ batched_layernorm_staged_kernel(const LnsMember* __restrict__ members, const Lns
                        "r"((uint32_t)m.ldy16), "r"((uint32_t)((uint64_t)m.ldy16 >> 32)) : "memory");
           asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(ha + 32), "r"(__float_as_uint(m.eps)), "r"(__float_as_uint(m.inv_D)),
                        "r"(shape), "r"(0) : "memory");
+          if (Q8) asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(ha + 48), "r"(xe.x), "r"(xe.y), "r"(xe.z), "r"(xe.w) : "memory");
           const uint32_t tx = (uint32_t)nrows * row_bytes + (m.gamma ? pbytes : 0u) + (m.beta ? pbytes : 0u);
           asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(fb), "r"(tx) : "memory");
           if (m.gamma) lns_bulk_load(stage + tile_max, m.gamma, pbytes, fb);
@@ -463,7 +486,7 @@ batched_layernorm_staged_kernel(const LnsMember* __restrict__ members, const Lns
             lns_bulk_load(stage + (uint32_t)r * row_bytes, m.x + (int64_t)(row0 + r) * m.ldx16 * 16, row_bytes, fb);
         if (++s == nstages) { s = 0; ph ^= 1; }
       }
-      c0 = c1; line0 = line1; mv0 = mv1;
+      c0 = c1; line0 = line1; mv0 = mv1; xv0 = xv1;
       c1 = c2; line1 = line2;
       c2 = c3;
     }
@@ -488,22 +511,27 @@ batched_layernorm_staged_kernel(const LnsMember* __restrict__ members, const Lns
       h.y = reinterpret_cast<char*>(((uint64_t)h1.y << 32) | h1.x);
       h.ldy16 = (int64_t)(((uint64_t)h1.w << 32) | h1.z);
       h.eps = __uint_as_float(h2.x); h.inv_D = __uint_as_float(h2.y); h.shape = h2.z;
+      h.y8 = nullptr; h.ldy8_8 = 0; h.scale8 = 0.f;
       if (h.member < 0) break;
+      if (Q8) {
+        const uint4 h3 = lns_lds128(ha + 48);
+        h.y8 = reinterpret_cast<char*>(((uint64_t)h3.y << 32) | h3.x); h.ldy8_8 = (int32_t)h3.z; h.scale8 = __uint_as_float(h3.w);
+      }
       const uint32_t tile = sbase + (uint32_t)s * stage_bytes;
       const uint32_t sg = tile + tile_max, sb = sg + pmax;
       const int vpl = (h.shape >> 8) & 0xFF, ll = h.shape & 0xFF;
       const int ru = vpl == 1 ? 4 : vpl == 2 ? 2 : 1;
       const bool fast = (h.shape >> 16) == 3u && h.nvec == (vpl << ll) && h.nrows % ((kLnsConsumers >> ll) * ru) == 0;
       switch (fast ? vpl : vpl + 8) {   // CTA-uniform
-        case 1: lns_tile<P_BF16, 1, 4, true>(h, tile, sg, sb); break;
-        case 2: lns_tile<P_BF16, 2, 2, true>(h, tile, sg, sb); break;
-        case 3: lns_tile<P_BF16, 3, 1, true>(h, tile, sg, sb); break;
-        case 4: lns_tile<P_BF16, 4, 1, true>(h, tile, sg, sb); break;
-        case 9: lns_tile<P_BF16, 1, 4, false>(h, tile, sg, sb); break;
-        case 10: lns_tile<P_BF16, 2, 2, false>(h, tile, sg, sb); break;
-        case 11: lns_tile<P_BF16, 3, 1, false>(h, tile, sg, sb); break;
-        case 12: lns_tile<P_BF16, 4, 1, false>(h, tile, sg, sb); break;
-        default: lns_tile_wide<P_BF16>(h, tile, sg, sb); break;
+        case 1: lns_tile<P_BF16, 1, 4, true, Q8>(h, tile, sg, sb); break;
+        case 2: lns_tile<P_BF16, 2, 2, true, Q8>(h, tile, sg, sb); break;
+        case 3: lns_tile<P_BF16, 3, 1, true, Q8>(h, tile, sg, sb); break;
+        case 4: lns_tile<P_BF16, 4, 1, true, Q8>(h, tile, sg, sb); break;
+        case 9: lns_tile<P_BF16, 1, 4, false, Q8>(h, tile, sg, sb); break;
+        case 10: lns_tile<P_BF16, 2, 2, false, Q8>(h, tile, sg, sb); break;
+        case 11: lns_tile<P_BF16, 3, 1, false, Q8>(h, tile, sg, sb); break;
+        case 12: lns_tile<P_BF16, 4, 1, false, Q8>(h, tile, sg, sb); break;
+        default: lns_tile_wide<P_BF16, Q8>(h, tile, sg, sb); break;
       }
       __syncwarp();
       if (lane == 0) asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(empty_bar(s)) : "memory");
@@ -536,12 +564,13 @@ cudaError_t launch_layernorm(const opt_plan* p, cudaStream_t s) {
     auto* members = reinterpret_cast<const LnsMember*>(base + p->off0);
     auto* items = reinterpret_cast<const LnsItem*>(base + p->off1);
     int* counters = reinterpret_cast<int*>(base + p->off2);
-    if (p_bf16)
-      batched_layernorm_staged_kernel<true><<<p->grid, p->block, p->smem, s>>>(members, items, p->n_chunks, counters, p->nstages,
-                                                                              p->ln_tile_max, p->ln_pmax);
-    else
-      batched_layernorm_staged_kernel<false><<<p->grid, p->block, p->smem, s>>>(members, items, p->n_chunks, counters, p->nstages,
-                                                                               p->ln_tile_max, p->ln_pmax);
+    const uint4* ext = p->off3 ? reinterpret_cast<const uint4*>(base + p->off3) : nullptr;
+#define LNS_LAUNCH(PB, Q)                                                                                               \
+    batched_layernorm_staged_kernel<PB, Q><<<p->grid, p->block, p->smem, s>>>(members, items, p->n_chunks, counters,   \
+                                                                              p->nstages, p->ln_tile_max, p->ln_pmax, ext)
+    if (ext) { if (p_bf16) LNS_LAUNCH(true, true); else LNS_LAUNCH(false, true); }
+    else { if (p_bf16) LNS_LAUNCH(true, false); else LNS_LAUNCH(false, false); }
+#undef LNS_LAUNCH
     return cudaGetLastError();
   }
   auto* members = reinterpret_cast<const LnMember*>(base + p->off0);
@@ -570,25 +599,36 @@ extern "C" opt_status opt_layernorm_plan_create(const opt_layernorm_member* memb
   std::vector<LnsItem> sitems;
   int64_t tile_max = 0, pmax = 0;
   int64_t bytes = 0;
+  bool any_y8 = false;
+  std::vector<uint4> sext;          // bf16 staged path: FP8 record per member {y8 lo, y8 hi, ldy8 / 8, scale8}
   for (int32_t i = 0; i < n; ++i) {
     const opt_layernorm_member& m = members[i];
-    if (!m.x || !m.y) return fail(OPT_ERR_INVALID_ARG, "member %d: NULL pointer", i);
+    if (!m.x || (!m.y && !m.y8)) return fail(OPT_ERR_INVALID_ARG, "member %d: NULL pointer", i);
     if (m.rows < 1 || m.D < 1) return fail(OPT_ERR_INVALID_ARG, "member %d: rows=%d D=%d must be >= 1", i, m.rows, m.D);
     if (!(m.eps >= 0.f)) return fail(OPT_ERR_INVALID_ARG, "member %d: eps must be >= 0", i);
-    if (m.rows > 1 && (m.ldx < m.D || m.ldy < m.D)) return fail(OPT_ERR_INVALID_ARG, "member %d: row stride smaller than D", i);
+    if (m.rows > 1 && (m.ldx < m.D || (m.y && m.ldy < m.D))) return fail(OPT_ERR_INVALID_ARG, "member %d: row stride smaller than D", i);
     if (!aligned16(m.x) || !aligned16(m.y) || !aligned16(m.gamma) || !aligned16(m.beta))
       return fail(OPT_ERR_ALIGNMENT, "member %d: pointers must be 16-byte aligned", i);
     if (m.D % V) return fail(OPT_ERR_ALIGNMENT, "member %d: D=%d is not a multiple of %d", i, m.D, V);
-    if (m.rows > 1 && (m.ldx % V || m.ldy % V))
+    if (m.rows > 1 && (m.ldx % V || (m.y && m.ldy % V)))
       return fail(OPT_ERR_ALIGNMENT, "member %d: row strides must be multiples of %d elements", i, V);
+    if (m.y8) {      // FP8 copy of the output (activation quantisation fused into the LayerNorm)
+      if (io != OPT_BF16) return fail(OPT_ERR_UNSUPPORTED, "member %d: the FP8 output is implemented for bf16 activations", i);
+      if (!(m.scale8 > 0.f) || !(m.scale8 < INFINITY)) return fail(OPT_ERR_INVALID_ARG, "member %d: scale8 must be a positive finite number", i);
+      if (m.rows > 1 && m.ldy8 < m.D) return fail(OPT_ERR_INVALID_ARG, "member %d: ldy8 smaller than D", i);
+      if ((reinterpret_cast<uintptr_t>(m.y8) & 7u) || m.ldy8 % 8)
+        return fail(OPT_ERR_ALIGNMENT, "member %d: y8 needs an 8-byte aligned base and ldy8 %% 8 == 0", i);
+      any_y8 = true;
+    }
     const int nvec = m.D / V;
     if (nvec > 32 * kLnMaxVpl)
       return fail(OPT_ERR_UNSUPPORTED, "member %d: D=%d exceeds the register-resident limit %d", i, m.D, 32 * kLnMaxVpl * V);
     regions.push_back({(uintptr_t)m.x, m.ldx * esz, (int64_t)m.D * esz, m.rows, false, i});
-    regions.push_back({(uintptr_t)m.y, m.ldy * esz, (int64_t)m.D * esz, m.rows, true, i});
+    if (m.y) regions.push_back({(uintptr_t)m.y, m.ldy * esz, (int64_t)m.D * esz, m.rows, true, i});
+    if (m.y8) regions.push_back({(uintptr_t)m.y8, m.ldy8, (int64_t)m.D, m.rows, true, i});
     if (m.gamma) regions.push_back({(uintptr_t)m.gamma, 0, (int64_t)m.D * pesz, 1, false, i});
     if (m.beta) regions.push_back({(uintptr_t)m.beta, 0, (int64_t)m.D * pesz, 1, false, i});
-    bytes += 2ll * m.rows * m.D * esz + (m.gamma ? (int64_t)m.D * pesz : 0) + (m.beta ? (int64_t)m.D * pesz : 0);
+    bytes += (int64_t)m.rows * m.D * esz * (m.y ? 2 : 1) + (m.y8 ? (int64_t)m.rows * m.D : 0) + (m.gamma ? (int64_t)m.D * pesz : 0) + (m.beta ? (int64_t)m.D * pesz : 0);
 
     // lanes per row: least waste, then 2..4 vectors per lane, then wider
     int best_l = -1, best_vpl = 0;
@@ -607,6 +647,10 @@ extern "C" opt_status opt_layernorm_plan_create(const opt_layernorm_member* memb
       t.ldx16 = m.ldx / V; t.ldy16 = m.ldy / V; t.nvec = nvec; t.eps = m.eps; t.inv_D = 1.0f / (float)m.D;
       t.l_log2 = (uint8_t)best_l; t.vpl = (uint8_t)best_vpl; t.contiguous = (m.rows == 1 || m.ldx == m.D); t.pad = 0;
       stab.push_back(t);
+      const uint64_t y8p = reinterpret_cast<uint64_t>(m.y8);
+      float sc = m.y8 ? m.scale8 : 0.f;
+      uint32_t scbits; memcpy(&scbits, &sc, 4);
+      sext.push_back(make_uint4((uint32_t)y8p, (uint32_t)(y8p >> 32), (uint32_t)(m.ldy8 / 8), scbits));
       // work items: whole rows, ~16 KB, a multiple of what one pass of the CTA covers
       const int64_t row_bytes = (int64_t)nvec * 16;
       const int rpp = kLnsConsumers >> best_l;
@@ -666,17 +710,23 @@ extern "C" opt_status opt_layernorm_plan_create(const opt_layernorm_member* memb
     p->off0 = 0;
     p->off1 = align_up(stab.size() * sizeof(LnsMember));
     p->off2 = p->off1 + align_up(chunked.size() * sizeof(LnsItem));
-    const size_t total = p->off2 + 256;                        // scheduler counters, zero-initialised
+    p->off3 = any_y8 ? p->off2 + 256 : 0;                      // FP8 records (selects the Q8 kernel)
+    const size_t total = p->off2 + 256 + (any_y8 ? align_up(sext.size() * sizeof(uint4)) : 0);   // + scheduler counters, zero-initialised
     std::vector<char> blob(total, 0);
     memcpy(blob.data(), stab.data(), stab.size() * sizeof(LnsMember));
     memcpy(blob.data() + p->off1, chunked.data(), chunked.size() * sizeof(LnsItem));
+    if (any_y8) memcpy(blob.data() + p->off3, sext.data(), sext.size() * sizeof(uint4));
     if (opt_status st = upload_tables(p, blob.data(), total)) { delete p; return st; }
     const int smem = (int)(nstages * stage_bytes);
     // the attribute belongs to the kernel FUNCTION, not to the plan (the last call wins): always the fixed budget,
     // so that a later, smaller plan never lowers the limit under a live, larger one
-    cudaError_t e = param == OPT_BF16
-        ? cudaFuncSetAttribute(batched_layernorm_staged_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, kLnsSmemBudget)
-        : cudaFuncSetAttribute(batched_layernorm_staged_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, kLnsSmemBudget);
+    cudaError_t e = cudaSuccess;
+    if (any_y8) e = param == OPT_BF16
+        ? cudaFuncSetAttribute(batched_layernorm_staged_kernel<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, kLnsSmemBudget)
+        : cudaFuncSetAttribute(batched_layernorm_staged_kernel<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, kLnsSmemBudget);
+    else e = param == OPT_BF16
+        ? cudaFuncSetAttribute(batched_layernorm_staged_kernel<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, kLnsSmemBudget)
+        : cudaFuncSetAttribute(batched_layernorm_staged_kernel<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, kLnsSmemBudget);
     if (e != cudaSuccess) {
       cudaFree(p->dev_tables); delete p;
       return fail(OPT_ERR_CUDA, "cudaFuncSetAttribute(max dynamic smem %d) failed: %s", smem, cudaGetErrorString(e));

@@ -132,15 +132,7 @@ __device__ __forceinline__ int4 pw_ext_apply(int4 a, int4 b, int op, float p0, f
 // FP8 E4M3 quantise / dequantise of saved activations (activation_quantization_aten_pass): the
 // bf16 side moves 16-byte vectors, the fp8 side the matching 8-byte vectors; p0 is the scale.  Saturating RNE, NaN -> NaN.
 __device__ __forceinline__ int2 pw_quant_e4m3(int4 v, float scale) {
-  const uint32_t* u = reinterpret_cast<const uint32_t*>(&v);
-  uint32_t o[2];
-#pragma unroll
-  for (int i = 0; i < 2; ++i) {
-    const uint32_t lo = __nv_cvt_float2_to_fp8x2(make_float2(bf16_lo(u[2 * i]) * scale, bf16_hi(u[2 * i]) * scale), __NV_SATFINITE, __NV_E4M3);
-    const uint32_t hi = __nv_cvt_float2_to_fp8x2(make_float2(bf16_lo(u[2 * i + 1]) * scale, bf16_hi(u[2 * i + 1]) * scale), __NV_SATFINITE, __NV_E4M3);
-    o[i] = lo | (hi << 16);
-  }
-  return make_int2((int)o[0], (int)o[1]);
+  return make_int2((int)quant4_e4m3((uint32_t)v.x, (uint32_t)v.y, scale), (int)quant4_e4m3((uint32_t)v.z, (uint32_t)v.w, scale));
 }
 __device__ __forceinline__ int4 pw_dequant_e4m3(int2 v, float scale) {
   const uint32_t w[2] = {(uint32_t)v.x, (uint32_t)v.y};

@@ -38,6 +38,10 @@ __device__ __forceinline__ void tma_load_2d(uint32_t dst, const void* tmap, uint
       "cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4}], [%2];"
       ::"r"(dst), "l"(tmap), "r"(bar), "r"(c0), "r"(c1) : "memory");
 }
+// warm L2 with one box of a tensor (no shared-memory destination, nothing to wait for)
+__device__ __forceinline__ void tma_prefetch_l2_2d(const void* tmap, int c0, int c1) {
+  asm volatile("cp.async.bulk.prefetch.tensor.2d.L2.global.tile [%0, {%1, %2}];" ::"l"(tmap), "r"(c0), "r"(c1) : "memory");
+}
 __device__ __forceinline__ void tma_store_2d(const void* tmap, uint32_t src, int c0, int c1) {
   asm volatile("cp.async.bulk.tensor.2d.global.shared::cta.bulk_group [%0, {%2, %3}], [%1];"
                ::"l"(tmap), "r"(src), "r"(c0), "r"(c1) : "memory");
@@ -201,6 +205,22 @@ inline opt_status encode_2d(EncodeTiledFn enc, CUtensorMap* tm, const void* base
   cuuint32_t estr[2] = {1, 1};
   CUresult r = enc(tm, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, const_cast<void*>(base), dims, strides, box, estr,
                    CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, promo, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  if (r != CUDA_SUCCESS)
+    return fail(OPT_ERR_CUDA, "cuTensorMapEncodeTiled(%s of member %d: rows=%lld cols=%lld ld=%lld box=%dx%d) -> CUresult %d",
+                what, member, (long long)rows, (long long)cols, (long long)ld, box_cols, box_rows, (int)r);
+  return OPT_OK;
+}
+
+// 2-D uint8 tensor [rows, cols] (FP8 codes), row stride ld BYTES, box {box_cols, box_rows}, 64-byte swizzle
+inline opt_status encode_2d_u8(EncodeTiledFn enc, CUtensorMap* tm, const void* base, int64_t rows, int64_t cols, int64_t ld,
+                               int box_cols, int box_rows, const char* what, int member) {
+  cuuint64_t dims[2] = {(cuuint64_t)cols, (cuuint64_t)rows};
+  cuuint64_t strides[1] = {(cuuint64_t)ld};
+  cuuint32_t box[2] = {(cuuint32_t)box_cols, (cuuint32_t)box_rows};
+  cuuint32_t estr[2] = {1, 1};
+  CUresult r = enc(tm, CU_TENSOR_MAP_DATA_TYPE_UINT8, 2, const_cast<void*>(base), dims, strides, box, estr,
+                   CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_64B, CU_TENSOR_MAP_L2_PROMOTION_NONE,
+                   CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
   if (r != CUDA_SUCCESS)
     return fail(OPT_ERR_CUDA, "cuTensorMapEncodeTiled(%s of member %d: rows=%lld cols=%lld ld=%lld box=%dx%d) -> CUresult %d",
                 what, member, (long long)rows, (long long)cols, (long long)ld, box_cols, box_rows, (int)r);

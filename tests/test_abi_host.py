@@ -37,8 +37,8 @@ def test_every_declared_symbol_is_exported(ob):
 
 
 def test_struct_layouts_match_header(ob):
-    assert ctypes.sizeof(ob.opt_linear_member) == 80
-    assert ctypes.sizeof(ob.opt_layernorm_member) == 64
+    assert ctypes.sizeof(ob.opt_linear_member) == 104      # + y8, ldy8, scale8 (tests/test_header_is_c.py checks every offset against gcc)
+    assert ctypes.sizeof(ob.opt_layernorm_member) == 88
     assert ctypes.sizeof(ob.opt_chunk) == 80
     assert ctypes.sizeof(ob.opt_linear2_member) == 104 and ctypes.sizeof(ob.opt_ln_linear2_member) == 128
     assert ctypes.sizeof(ob.opt_host_copy) == 32

@@ -492,6 +492,28 @@ def test_linear_f64x_and_colsum_hand_values_and_agreement_with_linear():
     assert np.allclose(oracle.colsum(g, BF16), oracle.widen(g, BF16).sum(axis=0), rtol=0, atol=1e-12)
 
 
+def test_saved_activation_fp8_is_quantisation_of_the_rounded_output():
+    """Reading Q29: the FP8 copy a fused epilogue emits is the quantisation of the ROUNDED storage-dtype output (what
+    the unfused graph's separate quantise op reads), not of the fp64 / fp32 pre-rounding value.  Hand case where the
+    two differ: z = 1.0625 + 2^-9 (bf16 keeps 8 significand bits: rounds DOWN to 1.0625 = 17/16, a tie between the
+    E4M3 neighbours 1.0 and 1.125 -> ties-to-even gives 1.0 = code 0x38; quantising z itself rounds UP to 1.125 =
+    0x39).  Also: the composition equals the two ops applied by hand, codes of integer outputs are exact."""
+    zval = 1.0625 + 2.0 ** -9          # built as a K = 2 dot product (zval itself is not a bf16 value)
+    m = dict(x=bf16(np.array([[1.0, 1.0]])), w=bf16(np.array([[1.0625, 2.0 ** -9]])), b=None, act=0)
+    y64, y, codes = graphs.linear_member_fp8(m, 1.0, BF16)
+    assert y64[0, 0] == zval and wl.f32_from_bf16_bits(y)[0, 0] == 1.0625
+    assert codes[0, 0] == 0x38 and oracle.quant_e4m3(np.array([[zval]], dtype=np.float32), 1.0, F32)[0, 0] == 0x39
+    rng = np.random.default_rng(3)
+    mi = dict(x=bf16(rng.integers(-1, 2, (5, 8))), w=bf16(rng.integers(-1, 2, (6, 8))), b=bf16(rng.integers(-2, 3, (6,))), act=1)
+    y64, y, codes = graphs.linear_member_fp8(mi, 0.5, BF16)
+    assert y64.max() <= 10 and np.array_equal(oracle.dequant_e4m3(codes, 2.0), y64)       # n / 2, n <= 15: 4 significant bits, exact codes
+    ln = dict(x=wl.tensor_normal(41, 1, (7, 24), 0.5, 2.0, BF16), gamma=wl.tensor_normal(41, 2, (24,), 1.0, 0.3, BF16),
+              beta=wl.tensor_normal(41, 3, (24,), 0.0, 0.3, BF16), eps=1e-5)
+    y64, y, codes = graphs.layernorm_fp8(ln, 16.0, BF16)
+    assert y.tobytes() == oracle.round_to_storage(oracle.layernorm(ln["x"], ln["gamma"], ln["beta"], 1e-5, BF16), BF16).tobytes()
+    assert codes.tobytes() == oracle.quant_e4m3(y, 16.0, BF16).tobytes()
+
+
 # --------------------------------- Table-1 pointwise patterns (SURVEY 8(f) rank 2) --
 def test_pointwise_ext_hand_values_and_special_values():
     """batch_clamp / batch_nan_to_num / batch_aten_sub,div,mul against hand-computed values (torch semantics)."""
