@@ -43,9 +43,64 @@ SMALL = dict(c1_rows=256, c1_n=16, c2_M=512, c2_n=16, c3_rows=512, c3_width=2048
              c4_B=512, c4_n=24)
 
 
-# dram__bytes_read.sum + dram__bytes_write.sum of the three grouped-GEMM launches of one step (C2, C4b, C4c), from
-# the committed `ncu --set full` capture profiles/r01_profiles.md section 2 (algorithmic: 7 912 453 120 bytes)
-GEMM_DRAM_TRAFFIC_PER_STEP = 7_843_725_000
+NCU_SUMMARY = os.path.join(ROOT, "profiles", "r02_ncu_full_metrics.csv")
+GEMM_SOURCES = ["paper_2607_02945_b200/csrc/grouped_gemm_sm100.cuh", "paper_2607_02945_b200/csrc/linear.cu",
+                "paper_2607_02945_b200/csrc/sm100_ptx.h"]
+
+
+def gemm_source_sha():
+    import hashlib
+    h = hashlib.sha256()
+    for f in GEMM_SOURCES:
+        with open(os.path.join(ROOT, f), "rb") as fh:
+            h.update(fh.read())
+    return h.hexdigest()[:16]
+
+
+def ncu_traffic_of_gemm_launches():
+    """roofline.traffic: dram__bytes_read.sum + dram__bytes_write.sum of the step's three grouped-GEMM launches (C2,
+    C4b, C4c), read at run time from the committed ncu summary (profiles/r02_ncu_full_metrics.csv, written by
+    `bench.py --ncu-summary` from one `ncu --set full` capture of `bench.py --profile`).  The summary records the
+    sha of the kernel's sources at capture time: if the sources have changed since, the figure is stale -> None."""
+    import csv
+    if not os.path.exists(NCU_SUMMARY):
+        return None, "no ncu summary committed"
+    rows = {r[0]: r[1:] for r in csv.reader(open(NCU_SUMMARY)) if r}
+    if rows.get("gemm_source_sha16", ["", ""])[1] != gemm_source_sha():
+        return None, "stale: %s was captured from other kernel sources" % os.path.basename(NCU_SUMMARY)
+    names = rows["metric"][1:]
+    total = 0.0
+    for key in ("dram__bytes_read.sum", "dram__bytes_write.sum"):
+        unit, vals = rows[key][0], rows[key][1:]
+        scale = {"byte": 1.0, "Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9}[unit]
+        total += sum(float(v) * scale for n_, v in zip(names, vals) if "GEMM" in n_)
+    return int(total), "profiles/%s (ncu --set full, one step)" % os.path.basename(NCU_SUMMARY)
+
+
+def write_ncu_summary(rep):
+    """`python bench.py --ncu-summary gpurun_out/prof_r02_full.ncu-rep > profiles/r02_ncu_full_metrics.csv` (on the
+    CPU box): one column per launch of the captured step, the metrics the roofline discussion uses, and the sha of the
+    grouped GEMM's sources."""
+    import csv
+    import subprocess
+    raw = subprocess.run(["ncu", "-i", rep, "--page", "raw", "--csv"], capture_output=True, text=True, check=True).stdout
+    rows = list(csv.reader(raw.splitlines()))
+    hdr, units, data = rows[0], rows[1], rows[2:]
+    labels = ["C1 LN", "C2 GEMM", "C3 pointwise", "C4a LN", "C4b GEMM", "C4c GEMM"]
+    keep = ["Kernel Name", "Grid Size", "Block Size", "gpu__time_duration.sum", "dram__bytes_read.sum", "dram__bytes_write.sum",
+            "gpu__dram_throughput.avg.pct_of_peak_sustained_elapsed", "sm__pipe_tensor_cycles_active.avg.pct_of_peak_sustained_active",
+            "sm__throughput.avg.pct_of_peak_sustained_elapsed", "smsp__issue_active.avg.pct_of_peak_sustained_active",
+            "lts__throughput.avg.pct_of_peak_sustained_elapsed", "lts__t_bytes.sum", "lts__t_sectors_srcunit_tex.sum",
+            "l1tex__m_xbar2l1tex_read_bytes.sum", "sm__warps_active.avg.pct_of_peak_sustained_active", "launch__registers_per_thread",
+            "sm__cycles_active.avg", "sm__cycles_elapsed.max", "smsp__cycles_active.avg", "launch__shared_mem_per_block_dynamic"]
+    w = csv.writer(sys.stdout)
+    w.writerow(["metric", "unit"] + labels[:len(data)])
+    for k in keep:
+        if k in hdr:
+            i = hdr.index(k)
+            w.writerow([k, units[i]] + [d[i] for d in data])
+    w.writerow(["gemm_source_sha16", "", gemm_source_sha()] + [""] * (len(data) - 1))
+    return 0
 
 
 def load_peaks():
@@ -414,34 +469,77 @@ class ClockWatch(threading.Thread):
 
 
 # ------------------------------------------------------------- CPU oracle ----
-def oracle_sample_step(frac=1.0):
-    """The oracle, as it stands, on a bounded ROW sample of the step's workload; returns
-    (extrapolated microseconds per full step, seconds actually spent, description, cores)."""
+def oracle_step(rows, cfgs=None):
+    """The oracle, as it stands, over `rows` rows per group of the step's workload (all members, all columns):
+    rows = dict(c1_rows, c2_M, c3_rows, c4_B).  cfgs: already generated full-size configs to slice rows from
+    (else generated here).  Returns the seconds spent per group [C1, C2, C3, C4]."""
     import oracle
     from oracle import graphs
+
+    def head(a, r):
+        return np.ascontiguousarray(a[:r])
+    if cfgs is None:
+        c1, c2 = wl.config1(rows=rows["c1_rows"]), wl.config2(M=rows["c2_M"])
+        c3, c4 = wl.config3(rows=rows["c3_rows"]), wl.config4(B=rows["c4_B"])
+    else:   # the first `rows` rows of the full-size tensors (the generators draw row-major: the same values)
+        c1 = dict(members=[dict(m, x=head(m["x"], rows["c1_rows"])) for m in cfgs["c1"]["members"]])
+        c2 = dict(members=[dict(m, x=head(m["x"], rows["c2_M"])) for m in cfgs["c2"]["members"]])
+        c3 = dict(cfgs["c3"], x=head(cfgs["c3"]["x"], rows["c3_rows"]))
+        c4 = dict(towers=[dict(t, x=head(t["x"], rows["c4_B"])) for t in cfgs["c4"]["towers"]])
+    parts = []
+    t = time.perf_counter(); graphs.layernorm_group(c1["members"], BF16); parts.append(time.perf_counter() - t)
+    t = time.perf_counter(); graphs.linear_group_concat(c2["members"], BF16); parts.append(time.perf_counter() - t)
+    t = time.perf_counter(); graphs.split_pointwise_cat(c3["x"], c3["widths"], c3["ops"], c3["perm"], BF16); parts.append(time.perf_counter() - t)
+    t = time.perf_counter()
+    outs = [graphs.recsys_tower(tw)["out"] for tw in c4["towers"]]
+    oracle.cat(outs)
+    parts.append(time.perf_counter() - t)
+    return parts
+
+
+FULL_ROWS = dict(c1_rows=FULL["c1_rows"], c2_M=FULL["c2_M"], c3_rows=FULL["c3_rows"], c4_B=FULL["c4_B"])
+
+
+def oracle_sample_step(frac=1.0):
+    """--impl reference: the oracle on a bounded ROW sample; returns (extrapolated microseconds per full step,
+    seconds actually spent, description, cores)."""
+    import oracle
     base = dict(c1_rows=2048, c2_M=256, c3_rows=2048, c4_B=128)
     rows = {k: max(8, int(v * frac) // 8 * 8) for k, v in base.items()}
     rows["c1_rows"] = min(rows["c1_rows"], FULL["c1_rows"])
     cores = oracle.max_threads()
-    c1 = wl.config1(rows=rows["c1_rows"])
-    c2 = wl.config2(M=rows["c2_M"])
-    c3 = wl.config3(rows=rows["c3_rows"])
-    c4 = wl.config4(B=rows["c4_B"])
-    parts = []
-    t = time.perf_counter(); graphs.layernorm_group(c1["members"], BF16); parts.append((time.perf_counter() - t, FULL["c1_rows"] / rows["c1_rows"]))
-    t = time.perf_counter(); graphs.linear_group_concat(c2["members"], BF16); parts.append((time.perf_counter() - t, FULL["c2_M"] / rows["c2_M"]))
-    t = time.perf_counter(); graphs.split_pointwise_cat(c3["x"], c3["widths"], c3["ops"], c3["perm"], BF16); parts.append((time.perf_counter() - t, FULL["c3_rows"] / rows["c3_rows"]))
-    t = time.perf_counter()
-    outs = [graphs.recsys_tower(tw)["out"] for tw in c4["towers"]]
-    oracle.cat(outs)
-    parts.append((time.perf_counter() - t, FULL["c4_B"] / rows["c4_B"]))
-    spent = sum(p[0] for p in parts)
-    full_us = sum(p[0] * p[1] for p in parts) * 1e6
+    parts = oracle_step(rows)
+    scale = [FULL_ROWS[k] / rows[k] for k in ("c1_rows", "c2_M", "c3_rows", "c4_B")]
+    spent = sum(parts)
+    full_us = sum(p * f for p, f in zip(parts, scale)) * 1e6
     desc = ("rows sampled per group: C1 %d/%d, C2 %d/%d, C3 %d/%d, C4 %d/%d (all members, all columns); "
             "time scaled by rows_full/rows_sampled per group" %
             (rows["c1_rows"], FULL["c1_rows"], rows["c2_M"], FULL["c2_M"], rows["c3_rows"], FULL["c3_rows"],
              rows["c4_B"], FULL["c4_B"]))
     return full_us, spent, desc, cores
+
+
+def oracle_full_step(cfgs, small=False):
+    """cpu_baseline of the product arm (SURVEY 8(d) "CPU oracle timing"): the oracle ONCE over ALL rows of every
+    group on all host cores -- measured, not extrapolated -- plus a 1-thread figure on a stated sub-sample."""
+    import oracle
+    cores = oracle.max_threads()
+    rows = dict(FULL_ROWS) if not small else dict(c1_rows=SMALL["c1_rows"], c2_M=SMALL["c2_M"], c3_rows=SMALL["c3_rows"], c4_B=SMALL["c4_B"])
+    parts = oracle_step(rows, cfgs)
+    sub = {k: max(8, v // 64) for k, v in rows.items()}            # 1 thread: 1/64 of the rows of every group
+    oracle.set_threads(1)
+    try:
+        p1 = oracle_step(sub, cfgs)
+    finally:
+        oracle.set_threads(cores)
+    t1_full_us = sum(p * rows[k] / sub[k] for p, k in zip(p1, ("c1_rows", "c2_M", "c3_rows", "c4_B"))) * 1e6
+    return dict(value=round(sum(parts) * 1e6, 1), unit="us", cores=cores, kind="oracle", extrapolated=False,
+                sample="ALL rows of every group, once: C1 %d, C2 %d, C3 %d, C4 %d rows (all members, all columns)" %
+                       (rows["c1_rows"], rows["c2_M"], rows["c3_rows"], rows["c4_B"]),
+                cpu_seconds=round(sum(parts), 2), seconds_per_group=dict(zip(("C1", "C2", "C3", "C4"), [round(p, 2) for p in parts])),
+                threads_1=dict(value=round(t1_full_us, 1), unit="us", extrapolated=True, cpu_seconds=round(sum(p1), 2),
+                               sample="1 thread on 1/64 of the rows of every group (C1 %d, C2 %d, C3 %d, C4 %d), scaled by 64" %
+                                      (sub["c1_rows"], sub["c2_M"], sub["c3_rows"], sub["c4_B"])))
 
 
 def run_reference(args):
@@ -463,8 +561,11 @@ def run_reference(args):
                 ms_per_step=v / 1e3, higher_is_better=False, scaling="weak", vs_baseline=None, dtype="f64",
                 data="synthetic", impl="reference",
                 config=dict(workload=WORKLOAD_NAME, l2="n/a (CPU)"),
-                cpu_baseline=dict(value=v, unit="us", cores=cores, kind="oracle", sample=desc,
-                                  cpu_seconds_per_sampled_step=spent_all / max(1, K)),
+                cpu_baseline=dict(value=v, unit="us", cores=cores, kind="oracle", sample=desc, extrapolated=True,
+                                  measured_seconds_per_step=spent_all / max(1, K), measured_seconds_total=spent_all,
+                                  note="each step times the oracle on the row sample; value = that time scaled by "
+                                       "rows_full / rows_sampled per group (the full-size oracle pass, ~40 s, is timed once "
+                                       "in the product arm's cpu_baseline)"),
                 e2e=dict(value=v, unit="us", h2d_bytes_per_step=0, d2h_bytes_per_step=0), gpu_launches=0)
     print(json.dumps(line))
     return 0
@@ -754,29 +855,34 @@ def run_product(args):
     # ---- (4) size-matched plain-copy reference for the HBM-bound groups: a device-to-device copy of the same
     # number of bytes (half read, half written), cold L2, same event protocol.  Small groups cannot reach the
     # large-copy peak whatever the kernel: launch ramp and tail are a fixed ~8 us.
-    copy_ref = {}
+    copy_ref, isolated = {}, {}
     flush = torch.empty(256 * 1024 * 1024, dtype=torch.uint8, device=device)
     for g in step.groups:
-        if g.kind == "linear" or args.profile:
+        if args.profile:
             continue
-        n = g.info["bytes"] // 2
-        a = torch.empty(n, dtype=torch.uint8, device=device)
-        b = torch.empty(n, dtype=torch.uint8, device=device)
-        b.copy_(a)
+        with_copy = g.kind != "linear"
+        if with_copy:
+            n = g.info["bytes"] // 2
+            a = torch.empty(n, dtype=torch.uint8, device=device)
+            b = torch.empty(n, dtype=torch.uint8, device=device)
+            b.copy_(a)
         ts, tk = [], []
         for _ in range(10):
-            flush.fill_(1)
-            c0, c1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-            c0.record(stream); b.copy_(a); c1.record(stream)
-            torch.cuda.synchronize()
-            ts.append(c0.elapsed_time(c1) * 1e3)
+            if with_copy:
+                flush.fill_(1)
+                c0, c1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                c0.record(stream); b.copy_(a); c1.record(stream)
+                torch.cuda.synchronize()
+                ts.append(c0.elapsed_time(c1) * 1e3)
             flush.fill_(1)
             c0, c1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
             c0.record(stream); g.plan.launch(); c1.record(stream)
             torch.cuda.synchronize()
             tk.append(c0.elapsed_time(c1) * 1e3)
-        copy_ref[g.name] = (float(np.mean(ts)), float(np.mean(tk)))
-        del a, b
+        isolated[g.name] = float(np.mean(tk))
+        if with_copy:
+            copy_ref[g.name] = (float(np.mean(ts)), float(np.mean(tk)))
+            del a, b
     del flush
 
     # ---- (5) one-launch-per-op baseline (same library, single-member plans), outside the timed step
@@ -1094,18 +1200,46 @@ def run_product(args):
                                   frac_of_same_size_copy=round(cus / kus, 4),
                                   isolated_frac_hbm=round(by / (kus * 1e-6) / 1e9 / peaks["hbm_gbs"], 4))
 
+    # what north_star grades, per group, MEASURED in this run (CUDA events): in the step (power-capped, sustained
+    # clocks) and isolated (cold L2, burst clocks).  HBM-bound groups against the measured copy bandwidth; configs[2]
+    # (the "large-tower config", reading Q23) against the measured bf16 tensor peak -- burst for the isolated launch,
+    # sustained for the in-step one -- with the roofline time as the per-member sum of max(tensor, HBM) next to it.
+    per_group = {}
+    for g, us in zip(step.groups, per_group_us):
+        fl, by = g.info["flops"], g.info["bytes"]
+        iso = isolated.get(g.name)
+        d = dict(bound=g.bound, in_step_us=round(us, 2), isolated_us=None if iso is None else round(iso, 2))
+        if g.bound == "hbm":
+            d.update(frac_hbm_in_step=round(by / (us * 1e-6) / 1e9 / peaks["hbm_gbs"], 4),
+                     frac_hbm_isolated=None if iso is None else round(by / (iso * 1e-6) / 1e9 / peaks["hbm_gbs"], 4))
+            if g.name in copy_ref:
+                d.update(same_size_copy_us=round(copy_ref[g.name][0], 2))
+        else:
+            d.update(frac_tensor_in_step_vs_sustained_peak=round(fl / (us * 1e-6) / 1e12 / peaks["bf16_tflops_sustained"], 4),
+                     frac_tensor_in_step_vs_burst_peak=round(fl / (us * 1e-6) / 1e12 / peaks["bf16_tflops"], 4),
+                     frac_tensor_isolated_vs_burst_peak=None if iso is None else round(fl / (iso * 1e-6) / 1e12 / peaks["bf16_tflops"], 4))
+            ms_ = g.cfg["members"]
+            t_sum = sum(max(2.0 * m["M"] * m["N"] * m["K"] / (peaks["bf16_tflops"] * 1e12),
+                            2.0 * (m["M"] * m["K"] + m["N"] * m["K"] + m["N"] + m["M"] * m["N"]) / (peaks["hbm_gbs"] * 1e9)) for m in ms_) * 1e6
+            t_roof = max(fl / (peaks["bf16_tflops"] * 1e12), by / (peaks["hbm_gbs"] * 1e9)) * 1e6
+            d.update(roofline_us=round(t_roof, 2), roofline_per_member_sum_of_max_us=round(t_sum, 2),
+                     frac_roofline_isolated=None if iso is None else round(t_roof / iso, 4),
+                     frac_roofline_per_member_isolated=None if iso is None else round(t_sum / iso, 4))
+        per_group[g.name] = d
+
     # dominant kernel of the step = the grouped GEMM (3 of the 6 launches); over a step it is HBM-bound
-    # (C4b/C4c at 85 and 52 flop/B; C2 sits on the ridge and is reported against tensor peak in "groups")
+    # (C4b/C4c at 85 and 52 flop/B; C2 sits on the ridge and is reported against tensor peak in per_group)
     gemm = [(g, us) for g, us in zip(step.groups, per_group_us) if g.kind == "linear"]
     gemm_bytes = sum(g.info["bytes"] for g, _ in gemm)
     gemm_us = sum(us for _, us in gemm)
     achieved = gemm_bytes / (gemm_us * 1e-6) / 1e9
+    traffic, traffic_note = (None, "debug sizes") if args.small else ncu_traffic_of_gemm_launches()
     roofline = dict(bound="hbm", kernel="grouped_gemm_sm100_kernel", achieved=round(achieved, 1), peak=peaks["hbm_gbs"],
                     unit="GB/s", frac=round(achieved / peaks["hbm_gbs"], 4),
-                    traffic=GEMM_DRAM_TRAFFIC_PER_STEP if not args.small else None,
+                    traffic=traffic, traffic_source=traffic_note,
                     peak_source=peaks["source"] + ", burst copy figure",
                     launches_per_step=len(gemm), bytes_per_step=gemm_bytes, us_per_step=round(gemm_us, 2),
-                    share_of_step=round(gemm_us / sum(per_group_us), 4))
+                    share_of_step=round(gemm_us / sum(per_group_us), 4), per_group=per_group)
     c2 = groups.get("C2_grouped_linear_tower")
     roofline_tensor = None
     if c2:
@@ -1133,9 +1267,8 @@ def run_product(args):
                 build_seconds=round(build_s, 1), lib=ob.opt_version())
 
     if rank == 0 and not args.no_cpu and not args.profile and world >= 1:
-        us, spent, desc, cores = oracle_sample_step(1.0 if not args.small else 0.25)
-        line["cpu_baseline"] = dict(value=round(us, 1), unit="us", cores=cores, kind="oracle", sample=desc,
-                                    cpu_seconds=round(spent, 2))
+        cfgs = {g.name[:2].lower(): g.cfg for g in step.groups}
+        line["cpu_baseline"] = oracle_full_step(cfgs, small=args.small)
     if rank == 0:
         print(json.dumps(line))
     if world > 1:
@@ -1158,7 +1291,10 @@ def main():
                     help="only the step's own launches (no cpu_baseline, no unfused baseline, no copy reference): for ncu")
     ap.add_argument("--ref-frac", type=float, default=0.0, help="reference arm: override the row-sample fraction")
     ap.add_argument("--side", default=None, choices=["linear2", "ln_linear2", "lhs", "skinny", "fp8", "bias_grad", "gemm_trace"], help="stand-alone side workload for ncu (not the metric)")
+    ap.add_argument("--ncu-summary", default=None, metavar="REP", help="CPU box: print the csv summary of an ncu --set full capture of `bench.py --profile`")
     args = ap.parse_args()
+    if args.ncu_summary:
+        return write_ncu_summary(args.ncu_summary)
     if args.side:
         return run_side(args)
     if args.impl == "reference":
