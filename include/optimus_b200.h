@@ -213,7 +213,7 @@ typedef struct {
  *     dx     = rstd * (g - mean(g) - xhat * mean(g * xhat))      rows x D
  *     dgamma = sum over rows of dy * xhat ;  dbeta = sum over rows of dy      [D]
  * x, dy:[rows,D] (ldx, lddy), gamma:[D] or NULL (= 1), dx:[rows,D] (lddx); dgamma / dbeta: [D] in the param
- * dtype, or NULL when not wanted.  bf16 activations, D % 8 == 0, D <= 512 (else OPT_ERR_UNSUPPORTED).  fp32
+ * dtype, or NULL when not wanted.  bf16 activations, D % 8 == 0, D <= 2048 (the forward's limit; else OPT_ERR_UNSUPPORTED).  fp32
  * arithmetic; the column sums are added in a fixed order (bitwise reproducible, no atomics on data).            */
 typedef struct {
   const void* x;
@@ -233,8 +233,8 @@ typedef struct {
  * y = x W^T + b, PAPER.md:292 batch_linear_post_grad on post-grad graphs, PAPER.md:437 training):
  *     db[n] = sum over m of dZ[m, n]
  * dz:[M,N] (ldz, elements; a column slice of a concat buffer is fine), db:[N] in the param dtype (device
- * pointers, caller-owned).  bf16 activations, N % 8 == 0, 16-byte aligned pointers, ldz % 8 == 0 (else
- * OPT_ERR_ALIGNMENT).  fp32 accumulation; rows are added in a fixed order (row groups, then row parts, through a
+ * pointers, caller-owned).  bf16 activations: N % 8 == 0, 16-byte aligned pointers, ldz % 8 == 0 (fp32 activations --
+ * configs[0]-like groups -- multiples of 4; else OPT_ERR_ALIGNMENT).  fp32 accumulation; rows are added in a fixed order (row groups, then row parts, through a
  * plan-owned workspace): bitwise reproducible, no atomics on data.  opt_plan_info: flops = M N adds, bytes = dZ + db.
  *
  * Fused ReLU mask (y != NULL; zero-initialise the struct otherwise): dz then holds the gradient dY that arrives at the

@@ -170,10 +170,59 @@ batched_bias_grad_kernel(const BgMember* __restrict__ members, const BgBlock* __
   }
 }
 
+// ---- fp32 groups (configs[0]-like: tiny, latency-bound).  One block per (member, 32-column tile): thread (tx, ty)
+// adds rows ty, ty + 8, ... of column col0 + tx in row order, the 8 row groups are added in group order through shared
+// memory: deterministic, no workspace, no tickets.  The fused derivative is plain fp32 arithmetic on the stored output
+// (mask: a select; tanh dy (1 - y^2); sigmoid dy (1 - y) y), dZ written as fp32, db sums the dZ it wrote.
+struct BgF32Member {
+  const float* dz; const float* y; float* dzo; char* db;
+  int64_t ldz, ldy, lddzo;
+  int32_t rows, N, act, pad;
+};
+struct BgF32Block { int32_t member, col0; };
+
+template <bool P_BF16>
+__global__ void __launch_bounds__(256)
+batched_bias_grad_f32_kernel(const BgF32Member* __restrict__ members, const BgF32Block* __restrict__ blocks) {
+  __shared__ float red[8][33];
+  const BgF32Block b = blocks[blockIdx.x];
+  const BgF32Member m = members[b.member];
+  const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;
+  const int col = b.col0 + tx;
+  float acc = 0.f;
+  if (col < m.N) {
+    for (int r = ty; r < m.rows; r += 8) {
+      float v = __ldg(m.dz + (int64_t)r * m.ldz + col);
+      if (m.y != nullptr) {
+        const float y = __ldg(m.y + (int64_t)r * m.ldy + col);
+        v = m.act <= 1 ? (y <= 0.f ? 0.f : v) : bg_dact(v, y, m.act);
+        if (m.dzo != nullptr) m.dzo[(int64_t)r * m.lddzo + col] = v;
+      }
+      acc += v;
+    }
+  }
+  red[ty][tx] = acc;
+  __syncthreads();
+  if (ty == 0 && col < m.N) {
+    float a = 0.f;
+#pragma unroll
+    for (int g = 0; g < 8; ++g) a += red[g][tx];
+    if (P_BF16) reinterpret_cast<__nv_bfloat16*>(m.db)[col] = __float2bfloat16_rn(a);
+    else reinterpret_cast<float*>(m.db)[col] = a;
+  }
+}
+
 cudaError_t launch_bias_grad(const opt_plan* p, cudaStream_t s) {
   const char* base = static_cast<const char*>(p->dev_tables);
   auto* members = reinterpret_cast<const BgMember*>(base + p->off0);
   auto* blocks = reinterpret_cast<const BgBlock*>(base + p->off1);
+  if (p->io == OPT_F32) {
+    auto* m32 = reinterpret_cast<const BgF32Member*>(base + p->off0);
+    auto* b32 = reinterpret_cast<const BgF32Block*>(base + p->off1);
+    if (p->param == OPT_BF16) batched_bias_grad_f32_kernel<true><<<p->grid, p->block, 0, s>>>(m32, b32);
+    else batched_bias_grad_f32_kernel<false><<<p->grid, p->block, 0, s>>>(m32, b32);
+    return cudaGetLastError();
+  }
   const bool any_mask = p->nstages != 0;      // stored in nstages
   if (p->param == OPT_BF16) {
     if (any_mask) batched_bias_grad_kernel<true, true><<<p->grid, p->block, 0, s>>>(members, blocks);
@@ -195,8 +244,56 @@ extern "C" opt_status opt_bias_grad_plan_create(const opt_bias_grad_member* memb
   if (!plan || !members) return fail(OPT_ERR_INVALID_ARG, "opt_bias_grad_plan_create: NULL argument");
   if (n < 1 || n > 65535) return fail(OPT_ERR_INVALID_ARG, "n = %d outside [1, 65535]", n);
   if ((io != OPT_F32 && io != OPT_BF16) || (param != OPT_F32 && param != OPT_BF16)) return fail(OPT_ERR_INVALID_ARG, "bad dtype");
-  if (io != OPT_BF16) return fail(OPT_ERR_UNSUPPORTED, "the bias gradient is implemented for bf16 activations only");
   const int pesz = elem_size(param);
+  if (io == OPT_F32) {      // fp32 groups: the simple deterministic column-tile kernel
+    std::vector<Region> regions;
+    std::vector<BgF32Member> tab;
+    std::vector<BgF32Block> blocks;
+    int64_t bytes = 0, flops = 0;
+    for (int32_t i = 0; i < n; ++i) {
+      const opt_bias_grad_member& m = members[i];
+      if (!m.dz || !m.db) return fail(OPT_ERR_INVALID_ARG, "member %d: NULL pointer", i);
+      if (m.M < 1 || m.N < 1) return fail(OPT_ERR_INVALID_ARG, "member %d: M=%d N=%d must be >= 1", i, m.M, m.N);
+      if (m.M > 1 && (m.ldz < m.N || (m.y && m.ldy < m.N) || (m.dz_out && m.lddz_out < m.N))) return fail(OPT_ERR_INVALID_ARG, "member %d: row stride smaller than N", i);
+      if (!aligned16(m.dz) || !aligned16(m.db) || !aligned16(m.y) || !aligned16(m.dz_out)) return fail(OPT_ERR_ALIGNMENT, "member %d: pointers must be 16-byte aligned", i);
+      if (m.N % 4 || (m.M > 1 && (m.ldz % 4 || (m.y && m.ldy % 4) || (m.dz_out && m.lddz_out % 4))))
+        return fail(OPT_ERR_ALIGNMENT, "member %d: N and the row strides must be multiples of 4 elements", i);
+      if (m.act < OPT_ACT_NONE || m.act > OPT_ACT_SIGMOID) return fail(OPT_ERR_INVALID_ARG, "member %d: bad act %d", i, m.act);
+      if (m.act != OPT_ACT_NONE && !m.y) return fail(OPT_ERR_INVALID_ARG, "member %d: act %d needs y (the stored forward output)", i, m.act);
+      if (m.dz_out && !m.y) return fail(OPT_ERR_INVALID_ARG, "member %d: dz_out without y (the mask source)", i);
+      if (m.y) regions.push_back({(uintptr_t)m.y, m.ldy * 4, (int64_t)m.N * 4, m.M, false, i});
+      if (m.dz_out) regions.push_back({(uintptr_t)m.dz_out, m.lddz_out * 4, (int64_t)m.N * 4, m.M, true, i});
+      regions.push_back({(uintptr_t)m.dz, m.ldz * 4, (int64_t)m.N * 4, m.M, false, i});
+      regions.push_back({(uintptr_t)m.db, 0, (int64_t)m.N * pesz, 1, true, i});
+      bytes += (int64_t)m.M * m.N * 4 * (1 + (m.y ? 1 : 0) + (m.dz_out ? 1 : 0)) + (int64_t)m.N * pesz;
+      flops += (int64_t)m.M * m.N;
+      BgF32Member t;
+      memset(&t, 0, sizeof t);
+      t.dz = (const float*)m.dz; t.y = (const float*)m.y; t.dzo = (float*)m.dz_out; t.db = (char*)m.db;
+      t.ldz = m.ldz; t.ldy = m.ldy; t.lddzo = m.lddz_out; t.rows = m.M; t.N = m.N; t.act = m.act;
+      tab.push_back(t);
+      for (int32_t c0 = 0; c0 < m.N; c0 += 32) blocks.push_back({i, c0});
+    }
+    if (opt_status st = check_independent(regions, /*allow_inplace_self=*/true)) return st;
+    int num_sms = 0;
+    DeviceGuard device_guard;      // the caller's current device is restored on return
+    if (opt_status st = open_device(device, &num_sms)) return st;
+    auto align_up = [](size_t x) { return (x + 255) & ~size_t(255); };
+    opt_plan* p = new opt_plan();
+    p->kind = kPlanBiasGrad; p->device = device; p->io = io; p->param = param; p->n_members = n;
+    p->bytes = bytes; p->flops = flops;
+    p->off0 = 0;
+    p->off1 = align_up(tab.size() * sizeof(BgF32Member));
+    const size_t total = p->off1 + align_up(blocks.size() * sizeof(BgF32Block));
+    std::vector<char> blob(total, 0);
+    memcpy(blob.data(), tab.data(), tab.size() * sizeof(BgF32Member));
+    memcpy(blob.data() + p->off1, blocks.data(), blocks.size() * sizeof(BgF32Block));
+    if (opt_status st = upload_tables(p, blob.data(), total)) { delete p; return st; }
+    p->grid = dim3((unsigned)blocks.size()); p->block = dim3(256); p->smem = 0;
+    p->total_tiles = (int32_t)blocks.size();
+    *plan = p;
+    return OPT_OK;
+  }
   std::vector<Region> regions;
   std::vector<BgMember> tab;
   std::vector<BgBlock> blocks;

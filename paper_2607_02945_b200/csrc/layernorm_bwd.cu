@@ -191,15 +191,132 @@ __device__ __forceinline__ void lnb_block(const LnbMember& m, const LnbBlock& b,
   if (threadIdx.x == 0) *m.ticket = 0;
 }
 
-// Two instantiations: groups whose rows all fit one vector per lane (D <= 256) run 4 blocks per SM in 64
-// registers; groups with wider rows keep two vectors per lane and run 2 blocks per SM without spilling.
+// Rows wider than 512 elements (up to 2048, the forward kernel's limit): a WARP owns a row, lane l holds vectors
+// l, l + 32, ... (<= 8) of x and dy packed in registers, statistics by full-warp butterflies as above; the column sums
+// cannot stay in registers (128 per lane), so every warp accumulates into its own [2][D] fp32 strip of shared memory
+// (a lane only ever touches its own columns: no conflicts, no synchronisation inside the row loop); gamma is staged
+// once per block as fp32.  The block's 8 strips are then added in warp order -> workspace part -> same last-block
+// reduction as the narrow path: bitwise reproducible.
+constexpr int kLnbWideVpl = 8;
+template <bool P_BF16>
+__device__ __forceinline__ void lnb_block_wide(const LnbMember& m, const LnbBlock& b, float* smem) {
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  constexpr int kWarps = kLnbThreads / 32;
+  const int D = m.nvec * 8;
+  float* sgam = smem;                               // [D]
+  float* acc = smem + D + (size_t)warp * 2 * D;     // this warp's [2][D]: dy * xhat, dy
+  for (int c = threadIdx.x; c < D; c += kLnbThreads) {
+    float g = 1.f;
+    if (m.gamma != nullptr) g = P_BF16 ? __bfloat162float(reinterpret_cast<const __nv_bfloat16*>(m.gamma)[c]) : reinterpret_cast<const float*>(m.gamma)[c];
+    sgam[c] = g;
+  }
+  for (int c = lane; c < 2 * D; c += 32) acc[c] = 0.f;
+  __syncthreads();
+  const int4* xb = reinterpret_cast<const int4*>(m.x);
+  const int4* dyb = reinterpret_cast<const int4*>(m.dy);
+  int4* dxb = reinterpret_cast<int4*>(m.dx);
+  for (int r = warp; r < b.nrows; r += kWarps) {
+    int4 xs[kLnbWideVpl], ds[kLnbWideVpl];
+#pragma unroll
+    for (int i = 0; i < kLnbWideVpl; ++i) {
+      xs[i] = ds[i] = make_int4(0, 0, 0, 0);
+      if (lane + 32 * i < m.nvec) {
+        xs[i] = __ldcs(xb + (int64_t)(b.row0 + r) * m.ldx16 + lane + 32 * i);
+        ds[i] = __ldcs(dyb + (int64_t)(b.row0 + r) * m.lddy16 + lane + 32 * i);
+      }
+    }
+    f32x2 s2 = 0ull, sg2 = 0ull, sgx2 = 0ull;
+#pragma unroll
+    for (int i = 0; i < kLnbWideVpl; ++i) {
+      if (lane + 32 * i >= m.nvec) continue;
+      const uint32_t* ux = reinterpret_cast<const uint32_t*>(&xs[i]);
+      const uint32_t* ud = reinterpret_cast<const uint32_t*>(&ds[i]);
+      const float4 g0 = *reinterpret_cast<const float4*>(sgam + (lane + 32 * i) * 8), g1 = *reinterpret_cast<const float4*>(sgam + (lane + 32 * i) * 8 + 4);
+      const f32x2 gv[4] = {pk2(g0.x, g0.y), pk2(g0.z, g0.w), pk2(g1.x, g1.y), pk2(g1.z, g1.w)};
+#pragma unroll
+      for (int k = 0; k < 4; ++k) {
+        const f32x2 xv = bf2_to_f2(ux[k]), g = mul2(bf2_to_f2(ud[k]), gv[k]);
+        s2 = add2(s2, xv); sg2 = add2(sg2, g); sgx2 = fma2(g, xv, sgx2);
+      }
+    }
+    const float s = lnb_rowsum<5>(sum2(s2)), sg = lnb_rowsum<5>(sum2(sg2));
+    float sgx = lnb_rowsum<5>(sum2(sgx2));
+    const float mu = s * m.inv_D;
+    const f32x2 nmu2 = pk2(-mu, -mu);
+    f32x2 q2 = 0ull;
+#pragma unroll
+    for (int i = 0; i < kLnbWideVpl; ++i) {
+      if (lane + 32 * i >= m.nvec) continue;
+      const uint32_t* ux = reinterpret_cast<const uint32_t*>(&xs[i]);
+#pragma unroll
+      for (int k = 0; k < 4; ++k) { const f32x2 d = add2(bf2_to_f2(ux[k]), nmu2); q2 = fma2(d, d, q2); }
+    }
+    const float q = lnb_rowsum<5>(sum2(q2));
+    const float rstd = rsqrtf(q * m.inv_D + m.eps);
+    sgx = rstd * (sgx - mu * sg);
+    const float mg = sg * m.inv_D, mgx = sgx * m.inv_D;
+    const f32x2 rstd2 = pk2(rstd, rstd), nmg2 = pk2(-mg, -mg), nmgx2 = pk2(-mgx, -mgx);
+#pragma unroll
+    for (int i = 0; i < kLnbWideVpl; ++i) {
+      if (lane + 32 * i >= m.nvec) continue;
+      const int col = (lane + 32 * i) * 8;
+      const uint32_t* ux = reinterpret_cast<const uint32_t*>(&xs[i]);
+      const uint32_t* ud = reinterpret_cast<const uint32_t*>(&ds[i]);
+      const float4 g0 = *reinterpret_cast<const float4*>(sgam + col), g1 = *reinterpret_cast<const float4*>(sgam + col + 4);
+      const f32x2 gv[4] = {pk2(g0.x, g0.y), pk2(g0.z, g0.w), pk2(g1.x, g1.y), pk2(g1.z, g1.w)};
+      f32x2* ag = reinterpret_cast<f32x2*>(acc + col);
+      f32x2* ab = reinterpret_cast<f32x2*>(acc + D + col);
+      uint32_t o[4];
+#pragma unroll
+      for (int k = 0; k < 4; ++k) {
+        const f32x2 dyv = bf2_to_f2(ud[k]);
+        const f32x2 xh = mul2(add2(bf2_to_f2(ux[k]), nmu2), rstd2);
+        ag[k] = fma2(dyv, xh, ag[k]);
+        ab[k] = add2(ab[k], dyv);
+        o[k] = f2_to_bf2(mul2(fma2(xh, nmgx2, fma2(dyv, gv[k], nmg2)), rstd2));
+      }
+      __stcs(dxb + (int64_t)(b.row0 + r) * m.lddx16 + lane + 32 * i, make_int4((int)o[0], (int)o[1], (int)o[2], (int)o[3]));
+    }
+  }
+  if (m.dgamma == nullptr && m.dbeta == nullptr) return;
+  __syncthreads();
+  float* part = m.ws + (size_t)b.part * 2 * D;
+  for (int c = threadIdx.x; c < 2 * D; c += kLnbThreads) {
+    float a = 0.f;
+    for (int w = 0; w < kWarps; ++w) a += smem[D + (size_t)w * 2 * D + c];
+    part[c] = a;
+  }
+  __shared__ int is_last_w;
+  __threadfence();
+  __syncthreads();
+  if (threadIdx.x == 0) is_last_w = atomicAdd(m.ticket, 1) == m.nparts - 1;
+  __syncthreads();
+  if (!is_last_w) return;
+  __threadfence();
+  for (int c = threadIdx.x; c < D; c += kLnbThreads) {
+    float a = 0.f, bb = 0.f;
+    for (int p = 0; p < m.nparts; ++p) {
+      a += __ldcg(m.ws + (size_t)p * 2 * D + c);
+      bb += __ldcg(m.ws + (size_t)p * 2 * D + D + c);
+    }
+    if (m.dgamma) lnb_store_param<P_BF16>(m.dgamma, c, a);
+    if (m.dbeta) lnb_store_param<P_BF16>(m.dbeta, c, bb);
+  }
+  if (threadIdx.x == 0) *m.ticket = 0;
+}
+
+// Three instantiations: groups whose rows all fit one vector per lane (D <= 256) run 4 blocks per SM in 64
+// registers; groups with rows up to 512 keep two vectors per lane and run 2 blocks per SM without spilling; groups
+// with a member wider than that run one block per SM (the wide path's shared-memory strips, up to 136 KB).
 template <bool P_BF16, int MAXVPL>
-__global__ void __launch_bounds__(kLnbThreads, MAXVPL == 1 ? 4 : 2)
+__global__ void __launch_bounds__(kLnbThreads, MAXVPL == 1 ? 4 : MAXVPL == 2 ? 2 : 1)
 batched_layernorm_bwd_kernel(const LnbMember* __restrict__ members, const LnbBlock* __restrict__ blocks) {
-  extern __shared__ __align__(16) float lnb_red[];      // 2 x rpp x D floats <= 32 KB
+  extern __shared__ __align__(16) float lnb_red[];      // narrow: 2 x rpp x D floats <= 32 KB; wide: (1 + 16) x D floats
   const LnbBlock b = blocks[blockIdx.x];
   const LnbMember m = members[b.member];
-  if (MAXVPL == 1 || m.vpl == 1) {
+  if (MAXVPL > 2 && m.vpl > 2) {
+    lnb_block_wide<P_BF16>(m, b, lnb_red);
+  } else if (MAXVPL == 1 || m.vpl == 1) {
     switch (m.l_log2) {      // block-uniform
       case 0: lnb_block<P_BF16, 1, 0>(m, b, lnb_red); break;
       case 1: lnb_block<P_BF16, 1, 1>(m, b, lnb_red); break;
@@ -217,13 +334,15 @@ cudaError_t launch_layernorm_bwd(const opt_plan* p, cudaStream_t s) {
   const char* base = static_cast<const char*>(p->dev_tables);
   auto* members = reinterpret_cast<const LnbMember*>(base + p->off0);
   auto* blocks = reinterpret_cast<const LnbBlock*>(base + p->off1);
-  const bool narrow = p->nstages == 1;      // max vectors per lane over the group (stored in nstages)
+  const int mv = p->nstages;      // max vectors per lane over the group (stored in nstages)
   if (p->param == OPT_BF16) {
-    if (narrow) batched_layernorm_bwd_kernel<true, 1><<<p->grid, p->block, p->smem, s>>>(members, blocks);
-    else batched_layernorm_bwd_kernel<true, 2><<<p->grid, p->block, p->smem, s>>>(members, blocks);
+    if (mv == 1) batched_layernorm_bwd_kernel<true, 1><<<p->grid, p->block, p->smem, s>>>(members, blocks);
+    else if (mv == 2) batched_layernorm_bwd_kernel<true, 2><<<p->grid, p->block, p->smem, s>>>(members, blocks);
+    else batched_layernorm_bwd_kernel<true, 8><<<p->grid, p->block, p->smem, s>>>(members, blocks);
   } else {
-    if (narrow) batched_layernorm_bwd_kernel<false, 1><<<p->grid, p->block, p->smem, s>>>(members, blocks);
-    else batched_layernorm_bwd_kernel<false, 2><<<p->grid, p->block, p->smem, s>>>(members, blocks);
+    if (mv == 1) batched_layernorm_bwd_kernel<false, 1><<<p->grid, p->block, p->smem, s>>>(members, blocks);
+    else if (mv == 2) batched_layernorm_bwd_kernel<false, 2><<<p->grid, p->block, p->smem, s>>>(members, blocks);
+    else batched_layernorm_bwd_kernel<false, 8><<<p->grid, p->block, p->smem, s>>>(members, blocks);
   }
   return cudaGetLastError();
 }
@@ -245,6 +364,7 @@ extern "C" opt_status opt_layernorm_bwd_plan_create(const opt_layernorm_bwd_memb
   std::vector<LnbBlock> blocks;
   std::vector<int64_t> ws_off;            // float offset of each member's partials in the workspace
   int64_t bytes = 0, ws_floats = 0;
+  int max_wide_D = 0;
   for (int32_t i = 0; i < n; ++i) {
     const opt_layernorm_bwd_member& m = members[i];
     if (!m.x || !m.dy || !m.dx) return fail(OPT_ERR_INVALID_ARG, "member %d: NULL pointer", i);
@@ -256,7 +376,8 @@ extern "C" opt_status opt_layernorm_bwd_plan_create(const opt_layernorm_bwd_memb
     if (m.D % 8) return fail(OPT_ERR_ALIGNMENT, "member %d: D=%d is not a multiple of 8", i, m.D);
     if (m.rows > 1 && (m.ldx % 8 || m.lddy % 8 || m.lddx % 8)) return fail(OPT_ERR_ALIGNMENT, "member %d: row strides must be multiples of 8 elements", i);
     const int nvec = m.D / 8;
-    if (nvec > 32 * kLnbMaxVpl) return fail(OPT_ERR_UNSUPPORTED, "member %d: D=%d exceeds the register-resident limit %d", i, m.D, 32 * kLnbMaxVpl * 8);
+    if (nvec > 32 * kLnbWideVpl) return fail(OPT_ERR_UNSUPPORTED, "member %d: D=%d exceeds the limit %d", i, m.D, 32 * kLnbWideVpl * 8);
+    const bool wide = nvec > 32 * kLnbMaxVpl;           // a warp per row, column sums in shared memory
     regions.push_back({(uintptr_t)m.x, m.ldx * 2, (int64_t)m.D * 2, m.rows, false, i});
     regions.push_back({(uintptr_t)m.dy, m.lddy * 2, (int64_t)m.D * 2, m.rows, false, i});
     regions.push_back({(uintptr_t)m.dx, m.lddx * 2, (int64_t)m.D * 2, m.rows, true, i});
@@ -267,10 +388,12 @@ extern "C" opt_status opt_layernorm_bwd_plan_create(const opt_layernorm_bwd_memb
     // lanes per row
     int ll = 0;
     while (ll < 5 && (1 << ll) < nvec) ++ll;                  // one vector per lane when the row fits a warp
-    while ((nvec + (1 << ll) - 1) / (1 << ll) > kLnbMaxVpl) ++ll;
+    while (ll < 5 && (nvec + (1 << ll) - 1) / (1 << ll) > kLnbMaxVpl) ++ll;
     const int L = 1 << ll, vpl = (nvec + L - 1) / L, rpp = kLnbThreads >> ll;
-    // rows per block: whole passes, ~64 KB of x per block
-    const int64_t passes = std::max<int64_t>(1, 65536 / ((int64_t)rpp * m.D * 2));
+    if (wide) max_wide_D = std::max(max_wide_D, m.D);
+    // rows per block: whole passes, ~64 KB of x per block (wide rows: ~512 KB, the block's shared-memory strips are
+    // zeroed and reduced once per block)
+    const int64_t passes = std::max<int64_t>(1, (wide ? 524288 : 65536) / ((int64_t)rpp * m.D * 2));
     const int64_t rpb = rpp * passes;
     const int32_t nparts = (int32_t)((m.rows + rpb - 1) / rpb);
     LnbMember t;
@@ -319,17 +442,20 @@ extern "C" opt_status opt_layernorm_bwd_plan_create(const opt_layernorm_bwd_memb
   cudaError_t e = cudaMemcpy(p->dev_tables, blob.data(), total, cudaMemcpyHostToDevice);
   int max_vpl = 1;
   for (const LnbMember& t : tab) max_vpl = std::max(max_vpl, t.vpl);
+  max_vpl = max_vpl > 2 ? 8 : max_vpl;
   p->nstages = max_vpl;
-  const void* fn = param == OPT_BF16 ? (max_vpl == 1 ? (const void*)batched_layernorm_bwd_kernel<true, 1> : (const void*)batched_layernorm_bwd_kernel<true, 2>)
-                                     : (max_vpl == 1 ? (const void*)batched_layernorm_bwd_kernel<false, 1> : (const void*)batched_layernorm_bwd_kernel<false, 2>);
-  if (e == cudaSuccess) e = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, 32768);
+  const void* fn = param == OPT_BF16 ? (max_vpl == 1 ? (const void*)batched_layernorm_bwd_kernel<true, 1> : max_vpl == 2 ? (const void*)batched_layernorm_bwd_kernel<true, 2> : (const void*)batched_layernorm_bwd_kernel<true, 8>)
+                                     : (max_vpl == 1 ? (const void*)batched_layernorm_bwd_kernel<false, 1> : max_vpl == 2 ? (const void*)batched_layernorm_bwd_kernel<false, 2> : (const void*)batched_layernorm_bwd_kernel<false, 8>);
+  // (a fixed maximum per instantiation, never a per-plan value: the attribute belongs to the kernel function)
+  const int kWideSmemMax = (1 + 2 * (kLnbThreads / 32)) * 32 * kLnbWideVpl * 8 * (int)sizeof(float);      // 139264
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, max_vpl > 2 ? kWideSmemMax : 32768);
   if (e != cudaSuccess) {
     cudaFree(p->dev_tables); cudaFree(p->workspace); delete p;
     return fail(OPT_ERR_CUDA, "plan upload failed: %s", cudaGetErrorString(e));
   }
   p->grid = dim3((unsigned)blocks.size());
   p->block = dim3(kLnbThreads);
-  p->smem = 32768;
+  p->smem = std::max<size_t>(32768, (size_t)(1 + 2 * (kLnbThreads / 32)) * max_wide_D * sizeof(float));
   p->total_tiles = (int32_t)blocks.size();
   *plan = p;
   return OPT_OK;

@@ -142,16 +142,16 @@ def test_host_validation_of_the_next_row_entry_points(ob):
     # LayerNorm backward: D <= 512, multiples of 8
     lb = lambda **kw: ob.opt_layernorm_bwd_member(**{**dict(x=A, ldx=64, dy=B, lddy=64, gamma=None, dx=Cc, lddx=64, dgamma=None, dbeta=None,
                                                             rows=16, D=64, eps=1e-5), **kw})
-    for member, status in [(lb(D=1024, ldx=1024, lddy=1024, lddx=1024), ob.OPT_ERR_UNSUPPORTED), (lb(D=60), ob.OPT_ERR_ALIGNMENT),
+    for member, status in [(lb(D=4096, ldx=4096, lddy=4096, lddx=4096), ob.OPT_ERR_UNSUPPORTED), (lb(D=60), ob.OPT_ERR_ALIGNMENT),
                            (lb(dx=A), ob.OPT_ERR_ALIAS)]:
         with pytest.raises(ob.OptError) as e:
             ob.opt_layernorm_bwd_plan_create([member], ob.OPT_BF16)
         assert e.value.status == status, (e.value, status)
-    # bias gradient: N % 8, aligned pointers and strides, db must not lie inside dz, fp32 activations unsupported
+    # bias gradient: N % 8 (fp32 activations: % 4), aligned pointers and strides, db must not lie inside dz
     bgm = lambda **kw: ob.opt_bias_grad_member(**{**dict(dz=A, ldz=64, db=B, M=16, N=64, y=None, ldy=0, dz_out=None, lddz_out=0, act=0), **kw})
     for member, io, status in [(bgm(N=60), ob.OPT_BF16, ob.OPT_ERR_ALIGNMENT), (bgm(ldz=68), ob.OPT_BF16, ob.OPT_ERR_ALIGNMENT), (bgm(db=B + 8), ob.OPT_BF16, ob.OPT_ERR_ALIGNMENT),
                                (bgm(db=A + 128), ob.OPT_BF16, ob.OPT_ERR_ALIAS), (bgm(ldz=32), ob.OPT_BF16, ob.OPT_ERR_INVALID_ARG), (bgm(M=0), ob.OPT_BF16, ob.OPT_ERR_INVALID_ARG),
-                               (bgm(dz=None), ob.OPT_BF16, ob.OPT_ERR_INVALID_ARG), (bgm(), ob.OPT_F32, ob.OPT_ERR_UNSUPPORTED),
+                               (bgm(dz=None), ob.OPT_BF16, ob.OPT_ERR_INVALID_ARG), (bgm(N=62), ob.OPT_F32, ob.OPT_ERR_ALIGNMENT), (bgm(act=1), ob.OPT_F32, ob.OPT_ERR_INVALID_ARG),
                                (bgm(dz_out=Cc, lddz_out=64), ob.OPT_BF16, ob.OPT_ERR_INVALID_ARG), (bgm(y=Cc, ldy=60), ob.OPT_BF16, ob.OPT_ERR_INVALID_ARG), (bgm(act=2), ob.OPT_BF16, ob.OPT_ERR_INVALID_ARG), (bgm(y=Cc, ldy=64, act=4), ob.OPT_BF16, ob.OPT_ERR_INVALID_ARG),
                                (bgm(y=Cc, ldy=64, dz_out=A + 16, lddz_out=64), ob.OPT_BF16, ob.OPT_ERR_ALIAS)]:
         with pytest.raises(ob.OptError) as e:

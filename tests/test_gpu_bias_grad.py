@@ -282,3 +282,48 @@ def test_stress_many_members_mixed_modes_relaunched(ob):
         assert np.all(np.abs(to_host(db).astype(np.float64) - graphs.linear_bias_grad(zh, BF16)) <= slack), (j, mode, z.shape)
         if out is not None and mode == 1:
             assert to_host(out).tobytes() == zh.tobytes()
+
+
+def test_fp32_groups_configs0_backward(ob):
+    """fp32 activations (configs[0]-like groups, "bias gradient for fp32 groups"): plain column sums,
+    the fused ReLU mask (bit-exact select) and the fused tanh / sigmoid derivative, fp32 and bf16 parameter dtype.
+    Sums of small integers bit for bit; random data within the fp32 summation bound (depth M/8 + 8, reading Q28)."""
+    rng = np.random.default_rng(3)
+    # integers: exact
+    zi = [rng.integers(-3, 4, (M, N)).astype(np.float32) for M, N in [(64, 32), (64, 16), (1000, 64), (7, 48), (333, 100)]]
+    dz = [torch.from_numpy(z).cuda() for z in zi]
+    for pdt, tdt in ((F32, torch.float32), (BF16, torch.bfloat16)):
+        db = [torch.full((z.shape[1],), float("nan"), dtype=tdt, device="cuda") for z in zi]
+        n0 = ob.opt_launch_count()
+        ob.opt_bias_grad_plan_create([ob.bias_grad_member(z, d) for z, d in zip(dz, db)], F32, pdt).launch()
+        torch.cuda.synchronize()
+        assert ob.opt_launch_count() - n0 == 1
+        for z, d in zip(zi, db):
+            assert np.array_equal(d.float().cpu().numpy().astype(np.float64), graphs.linear_bias_grad(z, F32))
+    # configs[0]: the whole backward of the tanh group's epilogue (dZ = dY (1 - y^2), db) in one launch, and a ReLU variant
+    c0 = wl.config0()
+    for act, op in ((2, oracle.PW_TANH_BWD), (3, oracle.PW_SIGMOID_BWD), (1, oracle.PW_RELU_BWD)):
+        keep, descs = [], []
+        for i, m in enumerate(c0["members"]):
+            y64 = graphs.linear_member(dict(m, act=act), F32)
+            y = oracle.round_to_storage(y64, F32)
+            dy = wl.tensor_normal(77, i + 1, y.shape, 0.0, 1.0, F32)
+            ty, tdy = torch.from_numpy(y).cuda(), torch.from_numpy(dy).cuda()
+            tdz = torch.full_like(tdy, float("nan")); tdb = torch.full((y.shape[1],), float("nan"), device="cuda")
+            keep.append((y, dy, tdz, tdb, ty, tdy))
+            descs.append(ob.bias_grad_member(tdy, tdb, ty, tdz, act))
+        ob.opt_bias_grad_plan_create(descs, F32, F32).launch()
+        torch.cuda.synchronize()
+        for y, dy, tdz, tdb, _, _ in keep:
+            ref = oracle.pointwise_ext(dy, y, op, [], F32)
+            got = tdz.cpu().numpy()
+            if act == 1:
+                assert got.tobytes() == oracle.round_to_storage(ref, F32).tobytes()
+            else:
+                assert np.allclose(got, ref, rtol=3e-7, atol=1e-30)          # one or two fp32 roundings
+            l1 = np.abs(got.astype(np.float64)).sum(axis=0)
+            assert np.all(np.abs(tdb.cpu().numpy().astype(np.float64) - graphs.linear_bias_grad(got, F32)) <= 2e-5 * l1 + 1e-30)
+    # errors: N % 4, act without y
+    with pytest.raises(ob.OptError) as e:
+        ob.opt_bias_grad_plan_create([ob.bias_grad_member(torch.zeros(8, 8, device="cuda")[:, :6], torch.zeros(6, device="cuda"))], F32, F32)
+    assert e.value.status == ob.OPT_ERR_ALIGNMENT

@@ -98,11 +98,34 @@ def test_relaunch_is_bitwise_reproducible_many_parts(ob):
         assert snap() == first
 
 
+def test_wide_rows_up_to_the_forward_limit(ob):
+    """512 < D <= 2048 (a warp per row, column sums in shared memory): every D the forward takes has a backward;
+    wide and narrow members mixed in one launch, ragged row counts, several partial-sum parts, NULL gamma, fp32
+    parameters, dx-only; relaunches give the same bits."""
+    dims = [520, 768, 1024, 1032, 1536, 2040, 2048, 256, 64]
+    rows = [300, 17, 1000, 5, 129, 64, 700, 333, 2000]
+    members = [mk(13, i, r, D, gamma=(i % 4 != 1)) for i, (r, D) in enumerate(zip(rows, dims))]
+    dev, plan = run_bwd(ob, members, pad=8)
+    check(dev, members, pad=8)
+    snap = lambda: b"".join(to_host(t).tobytes() for d in dev for t in (d[2], d[4], d[5]))
+    first = snap()
+    for d in dev:
+        d[4].fill_(float("nan")); d[5].fill_(float("nan"))
+    plan.launch()
+    torch.cuda.synchronize()
+    assert snap() == first
+    mf = [dict(m, gamma=None if m["gamma"] is None else wl.f32_from_bf16_bits(m["gamma"])) for m in members]
+    dev, _ = run_bwd(ob, mf, param_dt=F32)
+    check(dev, mf, param_dt=F32)
+    dev, _ = run_bwd(ob, members, want_params=False)
+    check(dev, members, want_params=False)
+
+
 def test_errors(ob):
-    x = empty_dev((4, 1024), BF16, fill=0.0)
-    y = empty_dev((4, 1024), BF16, fill=0.0)
-    z = empty_dev((4, 1024), BF16, fill=0.0)
-    with pytest.raises(ob.OptError) as e:              # D = 1024 exceeds the register-resident limit
+    x = empty_dev((4, 4096), BF16, fill=0.0)
+    y = empty_dev((4, 4096), BF16, fill=0.0)
+    z = empty_dev((4, 4096), BF16, fill=0.0)
+    with pytest.raises(ob.OptError) as e:              # D = 4096 exceeds the limit (2048, as in the forward)
         ob.opt_layernorm_bwd_plan_create([ob.layernorm_bwd_member(x, y, None, z, None, None, 1e-5)], BF16)
     assert e.value.status == ob.OPT_ERR_UNSUPPORTED
     with pytest.raises(ob.OptError) as e:              # dx overlaps x
