@@ -291,8 +291,8 @@ typedef struct opt_plan opt_plan; /* opaque; owns device-side tables only */
 
 /* Optional, documented planning choices of a grouped Linear (zero-initialise for the defaults; the results are
  * the same bits whatever is chosen -- only the schedule changes).  The library reads NO environment variable.
- *   cta_pair      0: CTA pairs (256-row tiles, tcgen05 cta_group::2) whenever every member allows it;
- *                 1: always one CTA per 128-row tile;  2: CTA pairs or OPT_ERR_UNSUPPORTED.
+ *   cta_pair      0 (default) or 2: CTA pairs (256-row tiles, tcgen05 cta_group::2, the W tile shared by the pair);
+ *                 1: one CTA per 128-row tile.
  *   no_skinny     1: never route a huge-M / tiny-K-and-N group to the streaming row kernel.
  *   no_lhs_order  1: schedule members that share one input X independently (member-major) instead of
  *                 m-block-major across them (batch_linear_lhs).                                  */

@@ -301,8 +301,15 @@ grouped_gemm_sm100_kernel(const GemmMember* __restrict__ members, const uint4* _
             // the leader's barrier counts the bytes of both CTAs
             if (rank == 0) mbar_expect_tx(full_bar(stage), 2 * (kABytes + b_bytes));
             const uint32_t lb = mapa(full_bar(stage), 0);
-            tma_load_2d_pair(sa, &m->tmA, lb, kb * kBK, m0);
-            if (composite) {
+            if (e1.y & kTransX) {                    // stored [K, M]: two 64x64 boxes (contraction rows, M contiguous)
+              tma_load_2d_pair(sa, &m->tmA, lb, m0, kb * kBK);
+              tma_load_2d_pair(sa + 8192, &m->tmA, lb, m0 + 64, kb * kBK);
+            } else {
+              tma_load_2d_pair(sa, &m->tmA, lb, kb * kBK, m0);
+            }
+            if (e1.y & kTransW) {                    // stored [K, N]: this CTA's BN/2 columns = BN/128 boxes of 64
+              for (int j = 0; j < bn / 128; ++j) tma_load_2d_pair(sa + kABytes + j * 8192, &m->tmB, lb, n0 + 64 * j, kb * kBK);
+            } else if (composite) {
 #pragma unroll
               for (int j = 0; j < 4; ++j)
                 if (j < nbox) tma_load_2d_pair(sa + kABytes + j * box_bytes, box_tm[j], lb, kb * kBK, box_row[j]);
@@ -357,14 +364,14 @@ grouped_gemm_sm100_kernel(const GemmMember* __restrict__ members, const uint4* _
           TR_WAIT(tr_full, mbar_wait(full_bar(stage), phase));
           tc_fence_after();
           const uint32_t sa = sbase + stage * stage_bytes;
-          const bool tx = NCTA == 1 && (e1.y & kTransX), tw = NCTA == 1 && (e1.y & kTransW);
+          const bool tx = (e1.y & kTransX) != 0, tw = (e1.y & kTransW) != 0;
           const uint64_t adesc = tx ? umma_desc_sw128_mn(sa) : umma_desc_sw128(sa);
           const uint64_t bdesc = tw ? umma_desc_sw128_mn(sa + kABytes) : umma_desc_sw128(sa + kABytes);
           // per K=16 step: K-major +32 bytes inside the swizzle row (+2 encoded); MN-major +2 groups of 8 rows (+128)
           const uint64_t astep = tx ? 128 : 2, bstep = tw ? 128 : 2;
           const int ksteps = kb + 1 < nkb ? kBK / 16 : klast;
           for (int k = 0; k < ksteps; ++k) {
-            if (NCTA == 2) tc_mma_bf16_pair(d_tmem, adesc + 2 * k, bdesc + 2 * k, idesc, (kb | k) != 0);
+            if (NCTA == 2) tc_mma_bf16_pair(d_tmem, adesc + astep * k, bdesc + bstep * k, idesc, (kb | k) != 0);
             else tc_mma_bf16(d_tmem, adesc + astep * k, bdesc + bstep * k, idesc, (kb | k) != 0);
           }
           // frees the smem stage (in both CTAs) when these MMAs retire

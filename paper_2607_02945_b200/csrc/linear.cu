@@ -256,12 +256,9 @@ extern "C" opt_status opt_linear_plan_create_ex(const opt_linear_member* members
   std::vector<GemmMember> tab(n);
   memset(tab.data(), 0, tab.size() * sizeof(GemmMember));
   // CTA pair (256-row tiles, W shared by the pair) or single CTA (128-row tiles)
-  int ncta = opts.cta_pair == 1 ? 1 : 2;
-  for (int32_t i = 0; i < n; ++i)
-    if (members[i].layout) {                   // MN-major (transposed) operand tiles are built per CTA: single-CTA kernel
-      if (opts.cta_pair == 2) { delete p; return fail(OPT_ERR_UNSUPPORTED, "options.cta_pair = 2: member %d has a transposed operand (single-CTA tiles only)", i); }
-      ncta = 1;
-    }
+  // (transposed operands run through both: a CTA of a pair stages its own 128 rows of X^T and its own half of the
+  // W^T tile as rows of 64 x 64 boxes, so a transposed-W tile of a pair is a multiple of 128 columns wide)
+  const int ncta = opts.cta_pair == 1 ? 1 : 2;
   const int tile_m = kBM * ncta;
   struct MemberTiling { int bn, nbn, nkb, klast; uint32_t flags, cflags; };
   std::vector<MemberTiling> tiling(n);
@@ -277,7 +274,7 @@ extern "C" opt_status opt_linear_plan_create_ex(const opt_linear_member* members
     GemmMember& t = tab[i];
     const bool tx = m.layout & OPT_LAYOUT_X_TRANSPOSED, tw = m.layout & OPT_LAYOUT_W_TRANSPOSED;
     int bn = choose_bn(m.N);
-    if (tw) bn = (bn + 63) / 64 * 64;          // MN-major W tiles are rows of 64x64 boxes
+    if (tw) bn = std::min(kMaxBN, (bn + 64 * ncta - 1) / (64 * ncta) * (64 * ncta));   // MN-major W tiles are rows of 64x64 boxes per CTA
     opt_status st;
     // K-major operand: box {64 k, rows};  transposed operand (stored [K, out]): box {64 out, 64 k}
     st = tx ? encode_2d(enc, &t.tmA, m.x, m.K, m.M, m.ldx, 64, kBK, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, "X^T", i)
