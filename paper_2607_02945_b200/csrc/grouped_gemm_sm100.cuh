@@ -360,23 +360,42 @@ grouped_gemm_sm100_kernel(const GemmMember* __restrict__ members, const uint4* _
         TR_WAIT(tr_tempty, mbar_wait(tempty_bar(as), aphase ^ 1));   // the epilogues (of both CTAs) have drained this accumulator stage
         tc_fence_after();
         const uint32_t d_tmem = tmem_base + as * kMaxBN;
-        for (int kb = 0; kb < nkb; ++kb) {
-          TR_WAIT(tr_full, mbar_wait(full_bar(stage), phase));
-          tc_fence_after();
-          const uint32_t sa = sbase + stage * stage_bytes;
-          const bool tx = (e1.y & kTransX) != 0, tw = (e1.y & kTransW) != 0;
-          const uint64_t adesc = tx ? umma_desc_sw128_mn(sa) : umma_desc_sw128(sa);
-          const uint64_t bdesc = tw ? umma_desc_sw128_mn(sa + kABytes) : umma_desc_sw128(sa + kABytes);
-          // per K=16 step: K-major +32 bytes inside the swizzle row (+2 encoded); MN-major +2 groups of 8 rows (+128)
-          const uint64_t astep = tx ? 128 : 2, bstep = tw ? 128 : 2;
-          const int ksteps = kb + 1 < nkb ? kBK / 16 : klast;
-          for (int k = 0; k < ksteps; ++k) {
-            if (NCTA == 2) tc_mma_bf16_pair(d_tmem, adesc + astep * k, bdesc + bstep * k, idesc, (kb | k) != 0);
-            else tc_mma_bf16(d_tmem, adesc + astep * k, bdesc + bstep * k, idesc, (kb | k) != 0);
+        // the issue loop sits on the critical path between "stage landed" and "tensor pipe busy": everything that does
+        // not change inside a tile is hoisted, and the common K-major case keeps compile-time descriptor steps
+        const bool tx = (e1.y & kTransX) != 0, tw = (e1.y & kTransW) != 0;
+        if (!tx && !tw) {
+          for (int kb = 0; kb < nkb; ++kb) {
+            TR_WAIT(tr_full, mbar_wait(full_bar(stage), phase));
+            tc_fence_after();
+            const uint32_t sa = sbase + stage * stage_bytes;
+            const uint64_t adesc = umma_desc_sw128(sa), bdesc = umma_desc_sw128(sa + kABytes);
+            const int ksteps = kb + 1 < nkb ? kBK / 16 : klast;
+            // per K=16 step: +32 bytes inside the 128-byte swizzle row (+2 encoded)
+            for (int k = 0; k < ksteps; ++k) {
+              if (NCTA == 2) tc_mma_bf16_pair(d_tmem, adesc + 2 * k, bdesc + 2 * k, idesc, (kb | k) != 0);
+              else tc_mma_bf16(d_tmem, adesc + 2 * k, bdesc + 2 * k, idesc, (kb | k) != 0);
+            }
+            // frees the smem stage (in both CTAs) when these MMAs retire
+            if (NCTA == 2) tc_commit_pair(empty_bar(stage)); else tc_commit(empty_bar(stage));
+            if (++stage == nstages) { stage = 0; phase ^= 1; }
           }
-          // frees the smem stage (in both CTAs) when these MMAs retire
-          if (NCTA == 2) tc_commit_pair(empty_bar(stage)); else tc_commit(empty_bar(stage));
-          if (++stage == nstages) { stage = 0; phase ^= 1; }
+        } else {
+          // an operand stored transposed: MN-major descriptors, a K=16 step is two groups of 8 contraction rows (+128)
+          const uint64_t astep = tx ? 128 : 2, bstep = tw ? 128 : 2;
+          for (int kb = 0; kb < nkb; ++kb) {
+            TR_WAIT(tr_full, mbar_wait(full_bar(stage), phase));
+            tc_fence_after();
+            const uint32_t sa = sbase + stage * stage_bytes;
+            const uint64_t adesc = tx ? umma_desc_sw128_mn(sa) : umma_desc_sw128(sa);
+            const uint64_t bdesc = tw ? umma_desc_sw128_mn(sa + kABytes) : umma_desc_sw128(sa + kABytes);
+            const int ksteps = kb + 1 < nkb ? kBK / 16 : klast;
+            for (int k = 0; k < ksteps; ++k) {
+              if (NCTA == 2) tc_mma_bf16_pair(d_tmem, adesc + astep * k, bdesc + bstep * k, idesc, (kb | k) != 0);
+              else tc_mma_bf16(d_tmem, adesc + astep * k, bdesc + bstep * k, idesc, (kb | k) != 0);
+            }
+            if (NCTA == 2) tc_commit_pair(empty_bar(stage)); else tc_commit(empty_bar(stage));
+            if (++stage == nstages) { stage = 0; phase ^= 1; }
+          }
         }
         if (NCTA == 2) tc_commit_pair(tfull_bar(as)); else tc_commit(tfull_bar(as));   // accumulator complete
         if (++as == kAccStages) { as = 0; aphase ^= 1; }
