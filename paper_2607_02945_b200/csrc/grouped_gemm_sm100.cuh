@@ -345,44 +345,67 @@ grouped_gemm_sm100_kernel(const GemmMember* __restrict__ members, const uint4* _
       int stage = 0; uint32_t phase = 0;
       int as = 0; uint32_t aphase = 0;
       int qs = 0; uint32_t qph = 0;
+      // K-major shared-memory descriptors of the current ring stage, advanced with the stage (no rebuild per k-block)
+      const uint64_t adesc_ring0 = umma_desc_sw128(sbase), desc_stage_step = (uint64_t)(stage_bytes >> 4);
+      uint64_t adesc_ring = adesc_ring0, bdesc_ring = adesc_ring0 + (kABytes >> 4);
       TR_DECL(tr_q); TR_DECL(tr_full); TR_DECL(tr_tempty); TR_DECL(tr_t0); TR_DECL(tr_tiles); TR_DECL(tr_kb);
       TR_NOW(tr_t0);
-      for (;;) {
+      // the next tile's header is taken from the queue BEFORE the last k-block of the current tile is issued, while
+      // the tensor pipe still has work: the queue wait + two shared-memory loads are off the tile-to-tile path
+      uint4 e0, e1;
+      auto next_header = [&]() {
         TR_WAIT(tr_q, mbar_wait(qfull_bar(qs), qph));
-        const uint4 e0 = lds128(q_slot(qs) + kQHeadOff);
-        const uint4 e1 = lds128(q_slot(qs) + kQHeadOff + 16);
+        e0 = lds128(q_slot(qs) + kQHeadOff);
+        e1 = lds128(q_slot(qs) + kQHeadOff + 16);
         arrive_leader(qempty_bar(qs));
         if (++qs == kQDepth) { qs = 0; qph ^= 1; }
+      };
+      next_header();
+      for (;;) {
         if ((int)e0.x < 0) break;
         const uint32_t idesc = e0.w;
         const int nkb = (int)(e1.x >> 16), klast = (int)(e1.y & 0xFFu);
+        const bool tx = (e1.y & kTransX) != 0, tw = (e1.y & kTransW) != 0;
         TR_ADD(tr_tiles, 1); TR_ADD(tr_kb, nkb * (int)(e1.x & 0xFFFFu));     // k-blocks weighted by tile width = tensor work
         TR_WAIT(tr_tempty, mbar_wait(tempty_bar(as), aphase ^ 1));   // the epilogues (of both CTAs) have drained this accumulator stage
         tc_fence_after();
         const uint32_t d_tmem = tmem_base + as * kMaxBN;
         // the issue loop sits on the critical path between "stage landed" and "tensor pipe busy": everything that does
         // not change inside a tile is hoisted, and the common K-major case keeps compile-time descriptor steps
-        const bool tx = (e1.y & kTransX) != 0, tw = (e1.y & kTransW) != 0;
         if (!tx && !tw) {
           for (int kb = 0; kb < nkb; ++kb) {
+            if (kb + 1 == nkb) next_header();    // (e0 / e1 of THIS tile are not used below this point)
             TR_WAIT(tr_full, mbar_wait(full_bar(stage), phase));
             tc_fence_after();
-            const uint32_t sa = sbase + stage * stage_bytes;
-            const uint64_t adesc = umma_desc_sw128(sa), bdesc = umma_desc_sw128(sa + kABytes);
-            const int ksteps = kb + 1 < nkb ? kBK / 16 : klast;
             // per K=16 step: +32 bytes inside the 128-byte swizzle row (+2 encoded)
-            for (int k = 0; k < ksteps; ++k) {
-              if (NCTA == 2) tc_mma_bf16_pair(d_tmem, adesc + 2 * k, bdesc + 2 * k, idesc, (kb | k) != 0);
-              else tc_mma_bf16(d_tmem, adesc + 2 * k, bdesc + 2 * k, idesc, (kb | k) != 0);
+            if (kb + 1 < nkb) {                  // a whole k-block: four steps, straight-line
+              if (NCTA == 2) {
+                tc_mma_bf16_pair(d_tmem, adesc_ring, bdesc_ring, idesc, (uint32_t)kb);
+                tc_mma_bf16_pair(d_tmem, adesc_ring + 2, bdesc_ring + 2, idesc, 1u);
+                tc_mma_bf16_pair(d_tmem, adesc_ring + 4, bdesc_ring + 4, idesc, 1u);
+                tc_mma_bf16_pair(d_tmem, adesc_ring + 6, bdesc_ring + 6, idesc, 1u);
+              } else {
+                tc_mma_bf16(d_tmem, adesc_ring, bdesc_ring, idesc, (uint32_t)kb);
+                tc_mma_bf16(d_tmem, adesc_ring + 2, bdesc_ring + 2, idesc, 1u);
+                tc_mma_bf16(d_tmem, adesc_ring + 4, bdesc_ring + 4, idesc, 1u);
+                tc_mma_bf16(d_tmem, adesc_ring + 6, bdesc_ring + 6, idesc, 1u);
+              }
+            } else {
+              for (int k = 0; k < klast; ++k) {
+                if (NCTA == 2) tc_mma_bf16_pair(d_tmem, adesc_ring + 2 * k, bdesc_ring + 2 * k, idesc, (kb | k) != 0);
+                else tc_mma_bf16(d_tmem, adesc_ring + 2 * k, bdesc_ring + 2 * k, idesc, (kb | k) != 0);
+              }
             }
             // frees the smem stage (in both CTAs) when these MMAs retire
             if (NCTA == 2) tc_commit_pair(empty_bar(stage)); else tc_commit(empty_bar(stage));
-            if (++stage == nstages) { stage = 0; phase ^= 1; }
+            adesc_ring += desc_stage_step; bdesc_ring += desc_stage_step;
+            if (++stage == nstages) { stage = 0; phase ^= 1; adesc_ring = adesc_ring0; bdesc_ring = adesc_ring0 + (kABytes >> 4); }
           }
         } else {
           // an operand stored transposed: MN-major descriptors, a K=16 step is two groups of 8 contraction rows (+128)
           const uint64_t astep = tx ? 128 : 2, bstep = tw ? 128 : 2;
           for (int kb = 0; kb < nkb; ++kb) {
+            if (kb + 1 == nkb) next_header();
             TR_WAIT(tr_full, mbar_wait(full_bar(stage), phase));
             tc_fence_after();
             const uint32_t sa = sbase + stage * stage_bytes;
@@ -394,7 +417,8 @@ grouped_gemm_sm100_kernel(const GemmMember* __restrict__ members, const uint4* _
               else tc_mma_bf16(d_tmem, adesc + astep * k, bdesc + bstep * k, idesc, (kb | k) != 0);
             }
             if (NCTA == 2) tc_commit_pair(empty_bar(stage)); else tc_commit(empty_bar(stage));
-            if (++stage == nstages) { stage = 0; phase ^= 1; }
+            adesc_ring += desc_stage_step; bdesc_ring += desc_stage_step;
+            if (++stage == nstages) { stage = 0; phase ^= 1; adesc_ring = adesc_ring0; bdesc_ring = adesc_ring0 + (kABytes >> 4); }
           }
         }
         if (NCTA == 2) tc_commit_pair(tfull_bar(as)); else tc_commit(tfull_bar(as));   // accumulator complete
