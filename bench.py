@@ -601,6 +601,9 @@ def run_side(args):
       --side skinny    the paper's four skinny aten.mm as one group (streaming row kernel)
       --side fp8       configs[4]'s saved LayerNorm outputs -> FP8 E4M3 and back (one launch each)
       --side bias_grad the 512 bias gradients of configs[4]'s Linear+ReLU group (column sums of [8192, H]), one launch
+      --side fp8_fused configs[4]'s LayerNorm and Linear+ReLU groups writing bf16 AND the FP8 copy in one launch vs two launches
+      --side backward  configs[2] dgrad / wgrad / fused mask + bias gradient, configs[4] LayerNorm backward, one launch each
+      --side gemm_trace  wait-cycle counters of the grouped GEMM's warp roles (trace build of the library)
       --side lhs       batch_linear_lhs: 8 members (N=64) on ONE input X [262144, 512]; also timed with
                        opt_linear_options.no_lhs_order (plain member-major schedule)
     Prints one JSON line; not the bench metric."""
@@ -645,6 +648,66 @@ def run_side(args):
         plan.launch()
         torch.cuda.synchronize()
         print(json.dumps(dict(side="ln_linear2", us=round(timed(plan.launch, 3), 1), **plan.info())))
+    elif args.side == "backward":
+        # backward groups at full size, one launch each (for ncu): configs[2] dgrad, wgrad, fused ReLU-mask + bias gradient;
+        # configs[4] LayerNorm-group backward
+        step = Step("cuda:0", FULL, pinned_host=False, configs=("c2",))
+        g2 = step.groups[0]
+        g2.plan.launch()
+        ycat = g2.aout.tensor(g2.iy)
+        dy_cat = torch.empty_like(ycat).normal_(0.0, 1.0)
+        dg, wg, bg, keep = [], [], [], []
+        for (ix, iw, ib), m in zip(g2.idx, g2.cfg["members"]):
+            x, w = g2.ain.tensor(ix), g2.ain.tensor(iw)
+            sl = slice(m["col_off"], m["col_off"] + m["N"])
+            dx, dw, db = torch.empty_like(x), torch.empty_like(w), torch.empty(m["N"], dtype=torch.float32, device="cuda")
+            keep.append((dx, dw, db))
+            dg.append(ob.linear_member(dy_cat[:, sl], w, None, dx, ACT_NONE, ob.OPT_LAYOUT_W_TRANSPOSED))
+            wg.append(ob.linear_member(dy_cat[:, sl], x, None, dw, ACT_NONE, ob.OPT_LAYOUT_X_TRANSPOSED | ob.OPT_LAYOUT_W_TRANSPOSED))
+            bg.append(ob.bias_grad_member(dy_cat[:, sl], db, ycat[:, sl], dy_cat[:, sl], ob.OPT_ACT_RELU))
+        pb = ob.opt_bias_grad_plan_create(bg, BF16, ob.OPT_F32, 0)
+        pd, pw = ob.opt_linear_plan_create(dg, BF16, 0), ob.opt_linear_plan_create(wg, BF16, 0)
+        for p_ in (pb, pd, pw):
+            p_.launch()
+        torch.cuda.synchronize()
+        res = dict(side="backward", c2_mask_bias_grad_us=round(timed(pb.launch, 3), 1), c2_dgrad_us=round(timed(pd.launch, 3), 1),
+                   c2_wgrad_us=round(timed(pw.launch, 3), 1), c2_dgrad_flops=pd.info()["flops"], c2_mask_bias_grad_bytes=pb.info()["bytes"])
+        del step, g2, keep, dy_cat, pb, pd, pw
+        cfg4 = wl.config4()
+        lb, keep = [], []
+        for t in cfg4["towers"]:
+            x = torch.from_numpy(t["x"].view(np.int16)).cuda().view(torch.bfloat16)
+            gam = torch.from_numpy(t["gamma"].view(np.int16)).cuda().view(torch.bfloat16)
+            dyl = torch.empty_like(x).normal_(0.0, 1.0)
+            dxl, dgl, dbl = torch.empty_like(x), torch.empty_like(gam), torch.empty_like(gam)
+            keep.append((x, gam, dyl, dxl, dgl, dbl))
+            lb.append(ob.layernorm_bwd_member(x, dyl, gam, dxl, dgl, dbl, 1e-5))
+        pl = ob.opt_layernorm_bwd_plan_create(lb, BF16, BF16, 0)
+        pl.launch()
+        torch.cuda.synchronize()
+        res.update(c4_layernorm_bwd_us=round(timed(pl.launch, 3), 1), c4_layernorm_bwd_bytes=pl.info()["bytes"])
+        print(json.dumps(res))
+    elif args.side == "fp8_fused":
+        # activation quantisation fused into the producer: configs[4]'s LayerNorm group writing its bf16
+        # output AND the FP8 copy in one launch, next to LayerNorm + OPT_PW_QUANT_E4M3 (two launches); same for C4b's GEMM
+        step = Step("cuda:0", FULL, pinned_host=False, configs=("c4",))
+        ga, gb, gc = step.groups
+        T, A = ga.ain.tensor, ga.amid.tensor
+        q8 = [torch.empty(A(i["xn"]).shape, dtype=torch.uint8, device="cuda") for i in ga.idx]
+        pf = ob.opt_layernorm_plan_create([ob.layernorm_member(T(i["x"]), A(i["xn"]), T(i["gamma"]), T(i["beta"]), t["eps"], q, 16.0)
+                                           for i, t, q in zip(ga.idx, ga.cfg["towers"], q8)], BF16, BF16, 0)
+        pq = ob.opt_pointwise_plan_create([ob.chunk(A(i["xn"]), q, ob.OPT_PW_QUANT_E4M3, None, [16.0]) for i, q in zip(ga.idx, q8)], BF16, 0)
+        h8 = [torch.empty(A(i["h"]).shape, dtype=torch.uint8, device="cuda") for i in ga.idx]
+        pg = ob.opt_linear_plan_create([ob.linear_member(A(i["xn"]), T(i["w1"]), T(i["b1"]), A(i["h"]), ACT_RELU, 0, q, 8.0)
+                                        for i, q in zip(ga.idx, h8)], BF16, 0)
+        ph = ob.opt_pointwise_plan_create([ob.chunk(A(i["h"]), q, ob.OPT_PW_QUANT_E4M3, None, [8.0]) for i, q in zip(ga.idx, h8)], BF16, 0)
+        for p_ in (ga.plan, pf, pq, gb.plan, pg, ph):
+            p_.launch()
+        torch.cuda.synchronize()
+        print(json.dumps(dict(side="fp8_fused", ln_us=round(timed(ga.plan.launch, 3), 1), ln_with_fp8_copy_us=round(timed(pf.launch, 3), 1),
+                              quant_launch_us=round(timed(pq.launch, 3), 1), ln_bytes=ga.plan.info()["bytes"], ln_with_fp8_bytes=pf.info()["bytes"],
+                              gemm_us=round(timed(gb.plan.launch, 3), 1), gemm_with_fp8_copy_us=round(timed(pg.launch, 3), 1),
+                              gemm_quant_launch_us=round(timed(ph.launch, 3), 1), gemm_bytes=gb.plan.info()["bytes"], gemm_with_fp8_bytes=pg.info()["bytes"])))
     elif args.side == "skinny":
         shapes = [(18583840, 8, 8), (25247936, 4, 2), (22502112, 8, 8), (17980096, 4, 2)]       # PAPER.md:477, (M, K, N)
         ten = [(torch.randn(M, K, device="cuda", dtype=torch.bfloat16), torch.randn(N, K, device="cuda", dtype=torch.bfloat16),
@@ -1290,7 +1353,7 @@ def main():
     ap.add_argument("--profile", action="store_true",
                     help="only the step's own launches (no cpu_baseline, no unfused baseline, no copy reference): for ncu")
     ap.add_argument("--ref-frac", type=float, default=0.0, help="reference arm: override the row-sample fraction")
-    ap.add_argument("--side", default=None, choices=["linear2", "ln_linear2", "lhs", "skinny", "fp8", "bias_grad", "gemm_trace"], help="stand-alone side workload for ncu (not the metric)")
+    ap.add_argument("--side", default=None, choices=["linear2", "ln_linear2", "lhs", "skinny", "fp8", "fp8_fused", "bias_grad", "backward", "gemm_trace"], help="stand-alone side workload for ncu (not the metric)")
     ap.add_argument("--ncu-summary", default=None, metavar="REP", help="CPU box: print the csv summary of an ncu --set full capture of `bench.py --profile`")
     args = ap.parse_args()
     if args.ncu_summary:

@@ -384,8 +384,12 @@ __device__ __forceinline__ void lns_tile_wide(const LnsHdr& h, uint32_t tile, ui
 // stage layout: [tile_max bytes of rows][gamma: pmax][beta: pmax][64-byte header]
 // Q8: some member wants the FP8 (E4M3) copy of its output; `ext` then holds one 16-byte record per member
 // {y8 pointer, row stride in 8-byte vectors, scale8} (y8 == NULL: none for that member).
-template <bool P_BF16, bool Q8>
-__global__ void __launch_bounds__(kLnsThreads, 3)
+// OCC: CTAs per SM the instantiation is compiled for.  3 (72 registers) for small groups -- a few items per CTA, where
+// the launch ramp dominates and more resident CTAs start more loads at once (configs[1]: 33 vs 38 us); 2 (no spills)
+// for large groups (configs[4]'s LayerNorm group: 303 vs 314 us) and for the Q8 instantiation, whose extra pointers /
+// flags of the FP8 store would spill at 72 registers.  The bytes in flight are set by the ring either way.
+template <bool P_BF16, bool Q8, int OCC>
+__global__ void __launch_bounds__(kLnsThreads, OCC)
 batched_layernorm_staged_kernel(const LnsMember* __restrict__ members, const LnsItem* __restrict__ items, int n_chunks,
                                 int* __restrict__ counters, int nstages, int tile_max, int pmax, const uint4* __restrict__ ext) {
   extern __shared__ __align__(128) uint8_t lns_smem[];
@@ -565,11 +569,12 @@ cudaError_t launch_layernorm(const opt_plan* p, cudaStream_t s) {
     auto* items = reinterpret_cast<const LnsItem*>(base + p->off1);
     int* counters = reinterpret_cast<int*>(base + p->off2);
     const uint4* ext = p->off3 ? reinterpret_cast<const uint4*>(base + p->off3) : nullptr;
-#define LNS_LAUNCH(PB, Q)                                                                                               \
-    batched_layernorm_staged_kernel<PB, Q><<<p->grid, p->block, p->smem, s>>>(members, items, p->n_chunks, counters,   \
-                                                                              p->nstages, p->ln_tile_max, p->ln_pmax, ext)
-    if (ext) { if (p_bf16) LNS_LAUNCH(true, true); else LNS_LAUNCH(false, true); }
-    else { if (p_bf16) LNS_LAUNCH(true, false); else LNS_LAUNCH(false, false); }
+#define LNS_LAUNCH(PB, Q, OCC)                                                                                              \
+    batched_layernorm_staged_kernel<PB, Q, OCC><<<p->grid, p->block, p->smem, s>>>(members, items, p->n_chunks, counters,  \
+                                                                                   p->nstages, p->ln_tile_max, p->ln_pmax, ext)
+    if (ext) { if (p_bf16) LNS_LAUNCH(true, true, 2); else LNS_LAUNCH(false, true, 2); }
+    else if (p->ncta == 2) { if (p_bf16) LNS_LAUNCH(true, false, 2); else LNS_LAUNCH(false, false, 2); }
+    else { if (p_bf16) LNS_LAUNCH(true, false, 3); else LNS_LAUNCH(false, false, 3); }
 #undef LNS_LAUNCH
     return cudaGetLastError();
   }
@@ -693,7 +698,9 @@ extern "C" opt_status opt_layernorm_plan_create(const opt_layernorm_member* memb
     const int64_t stage_bytes = tile_max + 2 * pmax + kLnsHdrBytes;
     const int nstages = (int)std::min<int64_t>(kLnsMaxStages, kLnsSmemBudget / stage_bytes);
     if (nstages < 2) { delete p; return fail(OPT_ERR_UNSUPPORTED, "LayerNorm rows too wide for the shared-memory ring"); }
-    const int n_cta = num_sms * 3;
+    // CTAs per SM (see the kernel): 2 for large groups (>= 64 items per CTA) and whenever an FP8 copy is written, else 3
+    const int occ = (any_y8 || sitems.size() >= (size_t)64 * 2 * num_sms) ? 2 : 3;
+    const int n_cta = num_sms * occ;
     // chunks of 8 consecutive items (one 128-byte table line, one atomic); the last 4 waves one item per chunk
     const LnsItem pad_item = {-1, 0, 0, 0};
     const size_t tail_waves = 4;
@@ -720,13 +727,11 @@ extern "C" opt_status opt_layernorm_plan_create(const opt_layernorm_member* memb
     const int smem = (int)(nstages * stage_bytes);
     // the attribute belongs to the kernel FUNCTION, not to the plan (the last call wins): always the fixed budget,
     // so that a later, smaller plan never lowers the limit under a live, larger one
-    cudaError_t e = cudaSuccess;
-    if (any_y8) e = param == OPT_BF16
-        ? cudaFuncSetAttribute(batched_layernorm_staged_kernel<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, kLnsSmemBudget)
-        : cudaFuncSetAttribute(batched_layernorm_staged_kernel<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, kLnsSmemBudget);
-    else e = param == OPT_BF16
-        ? cudaFuncSetAttribute(batched_layernorm_staged_kernel<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, kLnsSmemBudget)
-        : cudaFuncSetAttribute(batched_layernorm_staged_kernel<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, kLnsSmemBudget);
+    const bool pb = param == OPT_BF16;
+    const void* fn = any_y8 ? (pb ? (const void*)batched_layernorm_staged_kernel<true, true, 2> : (const void*)batched_layernorm_staged_kernel<false, true, 2>)
+                   : occ == 2 ? (pb ? (const void*)batched_layernorm_staged_kernel<true, false, 2> : (const void*)batched_layernorm_staged_kernel<false, false, 2>)
+                              : (pb ? (const void*)batched_layernorm_staged_kernel<true, false, 3> : (const void*)batched_layernorm_staged_kernel<false, false, 3>);
+    cudaError_t e = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, kLnsSmemBudget);
     if (e != cudaSuccess) {
       cudaFree(p->dev_tables); delete p;
       return fail(OPT_ERR_CUDA, "cudaFuncSetAttribute(max dynamic smem %d) failed: %s", smem, cudaGetErrorString(e));
@@ -736,6 +741,7 @@ extern "C" opt_status opt_layernorm_plan_create(const opt_layernorm_member* memb
     p->smem = (size_t)smem;
     p->total_tiles = (int32_t)sitems.size();
     p->n_chunks = (int32_t)n_chunks; p->nstages = nstages; p->ln_tile_max = (int32_t)tile_max; p->ln_pmax = (int32_t)pmax;
+    p->ncta = occ;                                             // which instantiation launch_layernorm picks
     *plan = p;
     return OPT_OK;
   }
