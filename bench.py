@@ -87,6 +87,8 @@ def write_ncu_summary(rep):
     rows = list(csv.reader(raw.splitlines()))
     hdr, units, data = rows[0], rows[1], rows[2:]
     labels = ["C1 LN", "C2 GEMM", "C3 pointwise", "C4a LN", "C4b GEMM", "C4c GEMM"]
+    if len(data) != 6:          # a side-workload capture: one column per captured launch, in capture order
+        labels = ["launch %d" % i for i in range(len(data))]
     keep = ["Kernel Name", "Grid Size", "Block Size", "gpu__time_duration.sum", "dram__bytes_read.sum", "dram__bytes_write.sum",
             "gpu__dram_throughput.avg.pct_of_peak_sustained_elapsed", "sm__pipe_tensor_cycles_active.avg.pct_of_peak_sustained_active",
             "sm__throughput.avg.pct_of_peak_sustained_elapsed", "smsp__issue_active.avg.pct_of_peak_sustained_active",
