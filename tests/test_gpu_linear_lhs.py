@@ -111,3 +111,73 @@ def test_two_lhs_groups_and_loose_members_in_one_launch(ob):
     _, ref = graphs.linear_group(ms, BF16)
     for y, r in zip(ys, ref):
         assert to_host(y).tobytes() == r.tobytes()
+
+
+def test_relaunch_and_cuda_graph_replay_of_a_composite_fp8_plan(ob):
+    """the plan re-arms its scheduler counters at the end of every launch: relaunches and CUDA-graph replays of a plan
+    with composite tiles and FP8 copies give the same bits."""
+    x, ms = lhs_group(93, 700, 200, [64, 128, 64, 256, 64], [0, 1, 2, 3, 1], [True] * 5)
+    xd = to_dev(x, BF16)
+    outs, q8, plan = run(ob, xd, ms, ob.opt_linear_options(), True, fp8_scale=2.0)
+    first = b"".join(o.tobytes() for o in outs) + b"".join(q.tobytes() for q in q8 if q is not None)
+    # `run` keeps no handle on its device buffers, so rebuild a plan whose buffers we own
+    dw = [to_dev(m["w"], BF16) for m in ms]
+    db = [to_dev(m["b"], BF16) for m in ms]
+    ycat = empty_dev((700, sum(m["N"] for m in ms)), BF16, fill=float("nan"))
+    off = np.concatenate(([0], np.cumsum([m["N"] for m in ms])))
+    y8 = [torch.full((700, m["N"]), 0xAA, dtype=torch.uint8, device="cuda") if i % 2 == 0 else None for i, m in enumerate(ms)]
+    plan = ob.opt_linear_plan_create([ob.linear_member(xd, w, b, ycat[:, off[i]:off[i + 1]], m["act"], 0, y8[i], 2.0)
+                                      for i, (w, b, m) in enumerate(zip(dw, db, ms))], BF16)
+    snap = lambda: b"".join(to_host(ycat[:, off[i]:off[i + 1]]).tobytes() for i in range(len(ms))) + \
+        b"".join(q.cpu().numpy().tobytes() for q in y8 if q is not None)
+    for _ in range(3):
+        ycat.fill_(float("nan"))
+        plan.launch()
+        torch.cuda.synchronize()
+        assert snap() == first
+    g, s = torch.cuda.CUDAGraph(), torch.cuda.Stream()
+    s.wait_stream(torch.cuda.current_stream())
+    with torch.cuda.graph(g, stream=s):
+        plan.launch(s.cuda_stream)
+    for _ in range(2):
+        ycat.fill_(float("nan"))
+        g.replay()
+        torch.cuda.synchronize()
+        assert snap() == first
+
+
+def test_stress_many_lhs_groups_random_shapes_against_single_member_plans(ob):
+    """60 members over 6 shared inputs (+ loose ones), random N (aligned and unaligned to 64), activations, bias on / off,
+    FP8 copies on / off, ragged M and K: ONE launch must equal, bit for bit, the same members run as single-member plans."""
+    rng = np.random.default_rng(23)
+    conv = lambda a: wl.bf16_bits_from_f32(a.astype(np.float32))
+    members, xs = [], []
+    for gidx in range(6):
+        M, K = int(rng.integers(1, 700)), int(rng.choice([8, 24, 64, 72, 128, 200, 320]))
+        aligned = gidx % 2 == 0
+        xs.append(to_dev(wl.tensor_normal(300 + gidx, 1, (M, K), 0, 1, BF16), BF16))
+        for j in range(int(rng.integers(2, 12))):
+            N = int(rng.choice([64, 128, 192, 256, 320])) if aligned else int(rng.choice([16, 40, 64, 104, 128, 264]))
+            members.append(dict(xi=gidx, M=M, K=K, N=N, act=int(rng.integers(0, 4)), bias=bool(rng.integers(0, 2)),
+                                fp8=bool(rng.integers(0, 2)) and N % 16 == 0))
+    rng.shuffle(members)                                       # members of a group need not be adjacent in the descriptor array
+    dev, fused, singles = [], [], []
+    for i, m in enumerate(members):
+        w = to_dev(wl.tensor_normal(400, 2 * i, (m["N"], m["K"]), 0, m["K"] ** -0.5, BF16), BF16)
+        b = to_dev(wl.tensor_normal(400, 2 * i + 1, (m["N"],), 0, 0.2, BF16), BF16) if m["bias"] else None
+        ya, yb = (empty_dev((m["M"], m["N"]), BF16, fill=float("nan")) for _ in range(2))
+        qa, qb = ((torch.full((m["M"], m["N"]), 0xAA, dtype=torch.uint8, device="cuda") if m["fp8"] else None) for _ in range(2))
+        dev.append((w, b, ya, yb, qa, qb))
+        fused.append(ob.linear_member(xs[m["xi"]], w, b, ya, m["act"], 0, qa, 3.0))
+        singles.append(ob.linear_member(xs[m["xi"]], w, b, yb, m["act"], 0, qb, 3.0))
+    n0 = ob.opt_launch_count()
+    ob.opt_linear_plan_create(fused, BF16).launch()
+    torch.cuda.synchronize()
+    assert ob.opt_launch_count() - n0 == 1
+    for d in singles:
+        ob.opt_linear_plan_create([d], BF16).launch()
+    torch.cuda.synchronize()
+    for (w, b, ya, yb, qa, qb), m in zip(dev, members):
+        assert torch.equal(ya.view(torch.int16), yb.view(torch.int16)), m
+        assert qa is None or torch.equal(qa, qb), m
+        assert not torch.isnan(ya.float()).any()
