@@ -30,6 +30,7 @@ struct LnbMember {
 struct LnbBlock { int32_t member, row0, nrows, part; };
 
 constexpr int kLnbThreads = 256;
+constexpr int kLnbSlotKB = 32;       // thread-private cp.async prefetch slots per block (alias the reduction buffer)
 constexpr int kLnbMaxVpl = 2;        // D <= 512: x, dy and the two column accumulators stay in registers
 
 __device__ __forceinline__ void lnb_unpack(const int4& v, float (&f)[8]) {
@@ -83,19 +84,34 @@ __device__ __forceinline__ void lnb_block(const LnbMember& m, const LnbBlock& b,
     }
   }
   const int npass = (b.nrows + rpp - 1) / rpp;
-  int4 nx[VPL], nd[VPL];                    // the next pass's vectors, in flight during this pass's arithmetic
+  // The kernel is bound by loads in flight, not by issue slots, and registers are what it cannot spare (64 x 4 blocks
+  // per SM): the vectors of the next kPD passes travel through THREAD-PRIVATE slots of shared memory filled with
+  // cp.async (no register is held while a load is in flight).  The slots alias the reduction buffer `red`, which is only
+  // used after the row loop (a __syncthreads separates the two uses).
+  constexpr int kPD = kLnbSlotKB / (8 * VPL);                           // kLnbSlotKB of slots per block: 4 passes (VPL 1), 2 (VPL 2); 48 KB measured no faster
+  const uint32_t slot0 = (uint32_t)__cvta_generic_to_shared(red) + threadIdx.x * 16u;
+  auto slot = [&](int pass, int i, int which) {                         // [pass % kPD][i][x | dy][thread]
+    return slot0 + (uint32_t)((((pass % kPD) * VPL + i) * 2 + which) * kLnbThreads) * 16u;
+  };
   auto fetch = [&](int pass) {
     const int r = pass * rpp + row_in_pass;
 #pragma unroll
     for (int i = 0; i < VPL; ++i) {
-      nx[i] = nd[i] = make_int4(0, 0, 0, 0);
       if (pass < npass && r < b.nrows && act[i]) {
-        nx[i] = __ldcs(xb + (int64_t)(b.row0 + r) * m.ldx16 + lane_in_row + i * L);
-        nd[i] = __ldcs(dyb + (int64_t)(b.row0 + r) * m.lddy16 + lane_in_row + i * L);
+        const int4* gx = xb + (int64_t)(b.row0 + r) * m.ldx16 + lane_in_row + i * L;
+        const int4* gd = dyb + (int64_t)(b.row0 + r) * m.lddy16 + lane_in_row + i * L;
+        asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(slot(pass, i, 0)), "l"(gx) : "memory");
+        asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(slot(pass, i, 1)), "l"(gd) : "memory");
+      } else if (pass < npass) {                                        // rows / vectors that do not exist read as zeros
+        asm volatile("st.shared.v4.b32 [%0], {%1, %1, %1, %1};" ::"r"(slot(pass, i, 0)), "r"(0) : "memory");
+        asm volatile("st.shared.v4.b32 [%0], {%1, %1, %1, %1};" ::"r"(slot(pass, i, 1)), "r"(0) : "memory");
       }
     }
+    asm volatile("cp.async.commit_group;" ::: "memory");               // one group per pass, empty ones included
   };
-  fetch(0);
+#pragma unroll
+  for (int pp = 0; pp < kPD; ++pp) fetch(pp);
+  int4 nx[VPL], nd[VPL];
   for (int pass = 0; pass < npass; ++pass) {
     const int r = pass * rpp + row_in_pass;
     const bool ok = r < b.nrows;
@@ -103,6 +119,12 @@ __device__ __forceinline__ void lnb_block(const LnbMember& m, const LnbBlock& b,
     // three row sums that do not depend on the mean go through ONE butterfly: sum x, sum g, sum g x  (g = dy gamma);
     // sum g xhat = rstd (sum g x - mu sum g)
     f32x2 s2 = 0ull, sg2 = 0ull, sgx2 = 0ull;
+    asm volatile("cp.async.wait_group %0;" ::"n"(kPD - 1) : "memory");   // this pass's group has landed
+#pragma unroll
+    for (int i = 0; i < VPL; ++i) {
+      asm volatile("ld.shared.v4.b32 {%0, %1, %2, %3}, [%4];" : "=r"(nx[i].x), "=r"(nx[i].y), "=r"(nx[i].z), "=r"(nx[i].w) : "r"(slot(pass, i, 0)) : "memory");
+      asm volatile("ld.shared.v4.b32 {%0, %1, %2, %3}, [%4];" : "=r"(nd[i].x), "=r"(nd[i].y), "=r"(nd[i].z), "=r"(nd[i].w) : "r"(slot(pass, i, 1)) : "memory");
+    }
 #pragma unroll
     for (int i = 0; i < VPL; ++i) {
       const uint32_t* ux = reinterpret_cast<const uint32_t*>(&nx[i]);
@@ -115,7 +137,7 @@ __device__ __forceinline__ void lnb_block(const LnbMember& m, const LnbBlock& b,
         s2 = add2(s2, x[i][k]); sg2 = add2(sg2, g); sgx2 = fma2(g, x[i][k], sgx2);
       }
     }
-    fetch(pass + 1);
+    fetch(pass + kPD);                       // refill the slot this pass has just read
     const float s = lnb_rowsum<LL>(sum2(s2)), sg = lnb_rowsum<LL>(sum2(sg2));
     float sgx = lnb_rowsum<LL>(sum2(sgx2));
     const float mu = s * m.inv_D;
@@ -152,6 +174,8 @@ __device__ __forceinline__ void lnb_block(const LnbMember& m, const LnbBlock& b,
   // ---- column sums of the block: row groups -> shared memory -> fixed-order sum -> workspace part
   const bool want = m.dgamma != nullptr || m.dbeta != nullptr;
   if (!want) return;
+  asm volatile("cp.async.wait_group 0;" ::: "memory");
+  __syncthreads();                          // every thread is done with its prefetch slots: `red` becomes the reduction buffer
   float* red_g = red;                       // [rpp][D]
   float* red_b = red + rpp * D;
 #pragma unroll
@@ -448,14 +472,14 @@ extern "C" opt_status opt_layernorm_bwd_plan_create(const opt_layernorm_bwd_memb
                                      : (max_vpl == 1 ? (const void*)batched_layernorm_bwd_kernel<false, 1> : max_vpl == 2 ? (const void*)batched_layernorm_bwd_kernel<false, 2> : (const void*)batched_layernorm_bwd_kernel<false, 8>);
   // (a fixed maximum per instantiation, never a per-plan value: the attribute belongs to the kernel function)
   const int kWideSmemMax = (1 + 2 * (kLnbThreads / 32)) * 32 * kLnbWideVpl * 8 * (int)sizeof(float);      // 139264
-  if (e == cudaSuccess) e = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, max_vpl > 2 ? kWideSmemMax : 32768);
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, max_vpl > 2 ? kWideSmemMax : kLnbSlotKB * 1024);
   if (e != cudaSuccess) {
     cudaFree(p->dev_tables); cudaFree(p->workspace); delete p;
     return fail(OPT_ERR_CUDA, "plan upload failed: %s", cudaGetErrorString(e));
   }
   p->grid = dim3((unsigned)blocks.size());
   p->block = dim3(kLnbThreads);
-  p->smem = std::max<size_t>(32768, (size_t)(1 + 2 * (kLnbThreads / 32)) * max_wide_D * sizeof(float));
+  p->smem = std::max<size_t>((size_t)kLnbSlotKB * 1024, (size_t)(1 + 2 * (kLnbThreads / 32)) * max_wide_D * sizeof(float));
   p->total_tiles = (int32_t)blocks.size();
   *plan = p;
   return OPT_OK;
