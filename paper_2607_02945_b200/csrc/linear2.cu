@@ -44,13 +44,30 @@
 
 namespace optb {
 
+// Pipeline trace build (-DOPTB_GEMM_TRACE: liboptimus_b200_trace.so only, see grouped_gemm_sm100.cuh): cycles each
+// warp role spends blocked on each barrier, one record of 32 counters per CTA.
+#ifdef OPTB_GEMM_TRACE
+__device__ unsigned long long* g_l2_trace = nullptr;       // [gridDim.x][32] or NULL
+#define T2_DECL(name) long long name = 0
+#define T2_NOW(name) name = clock64()
+#define T2_WAIT(acc, stmt) do { const long long t0__ = clock64(); stmt; acc += clock64() - t0__; } while (0)
+#define T2_ADD(acc, val) acc += (val)
+#define T2_STORE(slot, val) do { if (g_l2_trace) g_l2_trace[(size_t)blockIdx.x * 32 + (slot)] = (unsigned long long)(val); } while (0)
+#else
+#define T2_DECL(name)
+#define T2_NOW(name) do { } while (0)
+#define T2_WAIT(acc, stmt) do { stmt; } while (0)
+#define T2_ADD(acc, val) do { } while (0)
+#define T2_STORE(slot, val) do { } while (0)
+#endif
+
 constexpr int kT_BM = 128;            // tile rows
 constexpr int kT_BK = 64;             // k-block: one 128-byte swizzle row of bf16
 constexpr int kT_HC = 128;            // hidden chunk: UMMA N of layer 1, K of layer 2 per chunk
 constexpr int kT_MaxK = 256;          // layer-1 K (input features): the X tile is at most 4 k-blocks
 constexpr int kT_MaxH = 512;          // hidden width: b1 travels in the queue slot
 constexpr int kT_MaxN = 64;           // layer-2 N
-constexpr int kT_W1Stages = 4;
+constexpr int kT_W1Stages = 6;
 constexpr int kT_EpiWarps = 8;
 constexpr int kT_FirstEpiWarp = 3;
 constexpr int kT_Mma2Warp = kT_FirstEpiWarp + kT_EpiWarps;     // warp 11: layer-2 MMA issuer
@@ -61,8 +78,7 @@ constexpr int kT_FlagSpinLimit = 4096;   // polls of a member's fold flag before
 // shared-memory map
 constexpr int kT_OffX = 0;
 constexpr int kT_OffW1 = kT_OffX + (kT_MaxK / kT_BK) * kT_KBlockBytes;            //  64 KB
-constexpr int kT_OffH = kT_OffW1 + kT_W1Stages * kT_KBlockBytes;                  // +96 KB
-constexpr int kT_OffW2 = kT_OffH + 2 * kT_KBlockBytes;                            // +32 KB (one hidden tile: 2 k-blocks)
+constexpr int kT_OffW2 = kT_OffW1 + kT_W1Stages * kT_KBlockBytes;                 // +96 KB
 constexpr int kT_OffOut = kT_OffW2 + 2 * 2 * kT_W2KBlockBytes;                    // +32 KB
 constexpr int kT_OffQ = kT_OffOut + 4 * 4096;                                     // +16 KB output staging (4 warps x 32 rows x 128 B)
 template <bool LN>
@@ -71,16 +87,17 @@ struct L2Cfg {
   // LN: the augmented A k-slice (a 128 x 64 k-block in the swizzled layout, 16 columns used) sits before the queue
   static constexpr int kOffAug = kT_OffQ;
   static constexpr int kOffQ = kT_OffQ + (LN ? kT_KBlockBytes : 0);
-  // queue slot:  b1 (bf16) | b2 | TileEntry2     or, LN:  b2 | TileEntry2
-  static constexpr int kOffB2 = LN ? 0 : kT_MaxH * 2;
-  static constexpr int kQEntryOff = kOffB2 + kT_MaxN * 2;
+  // queue slot:  b1 (widened to fp32) | b2 (fp32) | TileEntry2     or, LN (no room for more):  b2 (bf16) | TileEntry2
+  static constexpr int kOffB2 = LN ? 0 : kT_MaxH * 4;
+  static constexpr int kQEntryOff = kOffB2 + kT_MaxN * (LN ? 2 : 4);
   static constexpr int kQSlotBytes = kQEntryOff + 32;
   static constexpr int kOffStats = kOffQ + kT_QDepth * kQSlotBytes;               // LN: partial row sums, 2 halves x 128 rows x {sum, sumsq}
   static constexpr int kOffBar = kOffStats + (LN ? 2 * kT_BM * 8 : 0);
   static constexpr int kSmemBytes = kOffBar + 384;
   static_assert(kSmemBytes <= 227 * 1024, "chained-GEMM shared memory map exceeds 227 KB");
 };
-constexpr int kT_TmemCols = 512;      // acc1: columns [0,256), acc2: [256,384)
+constexpr int kT_TmemCols = 512;      // acc1: columns [0,256), acc2: [256,384), hidden tile (bf16 pairs): [384,512)
+constexpr uint32_t kT_TmemAcc2 = 256, kT_TmemH = 384;
 
 struct alignas(128) L2Member {
   CUtensorMap tmX;       // X  [M,K]   box {64, 128}  load
@@ -114,12 +131,45 @@ __device__ __forceinline__ uint32_t l2_idesc(int n) {   // kind::f16, bf16 x bf1
   return (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(n >> 3) << 17) | ((uint32_t)(kT_BM >> 4) << 24);
 }
 
-__device__ __forceinline__ void epi_act(const uint32_t (&v)[64], uint32_t bias_addr, int act, uint32_t (&p)[32]) {
+// Epilogue math of one 32-row x 64-column piece held in v[64] (this thread: one row): + bias (fp32 in the tile's queue
+// slot: the scheduler warp widened it once per tile), activation, RNE to bf16 -> 32 packed pairs.  Packed f32x2 adds:
+// the same fp32 sums as the grouped GEMM's epilogue (bitwise), in a third of the instructions.
+template <int ACT>
+__device__ __forceinline__ void epi2_math(const uint32_t (&v)[64], uint32_t bias_addr, uint32_t (&p)[32]) {
+#pragma unroll
+  for (int j = 0; j < 16; ++j) {         // 4 columns per step
+    const uint4 b = lds128(bias_addr + 16 * j);
+    f32x2 s0, s1;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(s0) : "r"(v[4 * j]), "r"(v[4 * j + 1]));
+    asm("mov.b64 %0, {%1, %2};" : "=l"(s1) : "r"(v[4 * j + 2]), "r"(v[4 * j + 3]));
+    f32x2 b0, b1;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(b0) : "r"(b.x), "r"(b.y));
+    asm("mov.b64 %0, {%1, %2};" : "=l"(b1) : "r"(b.z), "r"(b.w));
+    s0 = add2(s0, b0); s1 = add2(s1, b1);
+    float f0, f1, f2, f3;
+    asm("mov.b64 {%0, %1}, %2;" : "=f"(f0), "=f"(f1) : "l"(s0));
+    asm("mov.b64 {%0, %1}, %2;" : "=f"(f2), "=f"(f3) : "l"(s1));
+    if (ACT == OPT_ACT_RELU) { p[2 * j] = pack_relu_bf16x2(f0, f1); p[2 * j + 1] = pack_relu_bf16x2(f2, f3); }
+    else {
+      p[2 * j] = pack_bf16x2(act_f32<true>(f0, ACT), act_f32<true>(f1, ACT));
+      p[2 * j + 1] = pack_bf16x2(act_f32<true>(f2, ACT), act_f32<true>(f3, ACT));
+    }
+  }
+}
+__device__ __forceinline__ void epi_act_b16(const uint32_t (&v)[64], uint32_t bias_addr, int act, uint32_t (&p)[32]) {   // bf16 bias
   switch (act) {
     case OPT_ACT_RELU: epi_math<OPT_ACT_RELU>(v, bias_addr, p); break;
     case OPT_ACT_NONE: epi_math<OPT_ACT_NONE>(v, bias_addr, p); break;
     case OPT_ACT_TANH: epi_math<OPT_ACT_TANH>(v, bias_addr, p); break;
     default:           epi_math<OPT_ACT_SIGMOID>(v, bias_addr, p); break;
+  }
+}
+__device__ __forceinline__ void epi_act(const uint32_t (&v)[64], uint32_t bias_addr, int act, uint32_t (&p)[32]) {
+  switch (act) {
+    case OPT_ACT_RELU: epi2_math<OPT_ACT_RELU>(v, bias_addr, p); break;
+    case OPT_ACT_NONE: epi2_math<OPT_ACT_NONE>(v, bias_addr, p); break;
+    case OPT_ACT_TANH: epi2_math<OPT_ACT_TANH>(v, bias_addr, p); break;
+    default:           epi2_math<OPT_ACT_SIGMOID>(v, bias_addr, p); break;
   }
 }
 
@@ -339,11 +389,19 @@ grouped_linear2_sm100_kernel(const L2Member* __restrict__ members, const uint4* 
         if (cur < 0) continue;             // warp-uniform
         mbar_wait(q_empty(qs), qph ^ 1);
         const uint32_t slot = q_slot(qs);
-        if (!LN) {
-          sts128(slot + 16 * lane, c1a);
-          sts128(slot + 512 + 16 * lane, c1b);
+        auto widen = [](uint32_t a, uint32_t b) { return make_uint4(a << 16, a & 0xFFFF0000u, b << 16, b & 0xFFFF0000u); };
+        if (!LN) {                           // 8 bf16 per lane -> 8 fp32: units [8 lane, 8 lane + 8) and 256 + the same
+          sts128(slot + 32 * lane, widen(c1a.x, c1a.y));
+          sts128(slot + 32 * lane + 16, widen(c1a.z, c1a.w));
+          sts128(slot + 1024 + 32 * lane, widen(c1b.x, c1b.y));
+          sts128(slot + 1024 + 32 * lane + 16, widen(c1b.z, c1b.w));
         }
-        if (lane < kT_MaxN / 8) sts128(slot + kOffB2 + 16 * lane, c2);
+        if (LN) {
+          if (lane < kT_MaxN / 8) sts128(slot + kOffB2 + 16 * lane, c2);
+        } else if (lane < kT_MaxN / 8) {
+          sts128(slot + kOffB2 + 32 * lane, widen(c2.x, c2.y));
+          sts128(slot + kOffB2 + 32 * lane + 16, widen(c2.z, c2.w));
+        }
         if ((lane >> 1) == g) sts128(slot + kQEntryOff + 16 * (lane & 1), e);
         __syncwarp();
         if (lane == 0) mbar_arrive(q_full(qs));
@@ -370,8 +428,10 @@ grouped_linear2_sm100_kernel(const L2Member* __restrict__ members, const uint4* 
       int qs = 0; uint32_t qph = 0;
       int w1s = 0; uint32_t w1ph = 0;
       uint32_t gt = 0, gh = 0;                       // tiles / hidden chunks issued so far
+      T2_DECL(tr_t0); T2_DECL(tr_q); T2_DECL(tr_xe); T2_DECL(tr_w1e); T2_DECL(tr_w2e);
+      T2_NOW(tr_t0);
       for (;;) {
-        mbar_wait(q_full(qs), qph);
+        T2_WAIT(tr_q, mbar_wait(q_full(qs), qph));
         const uint4 e0 = lds128(q_slot(qs) + kQEntryOff);
         mbar_arrive(q_empty(qs));
         if (++qs == kT_QDepth) { qs = 0; qph ^= 1; }
@@ -383,14 +443,14 @@ grouped_linear2_sm100_kernel(const L2Member* __restrict__ members, const uint4* 
         const int nch = (H + kT_HC - 1) / kT_HC;
         if (LN) asm volatile("fence.proxy.async;" ::: "memory");   // W1g: generic-proxy writes of this launch -> TMA reads
         // X tile: resident for the whole tile, reloaded when the last MMA1 of the previous tile has retired
-        mbar_wait(xa_empty, (gt & 1u) ^ 1u);
+        T2_WAIT(tr_xe, mbar_wait(xa_empty, (gt & 1u) ^ 1u));
         mbar_expect_tx(xa_full, (uint32_t)nkb1 * kT_KBlockBytes);
         for (int kb = 0; kb < nkb1; ++kb) tma_load_2d(sbase + kT_OffX + kb * kT_KBlockBytes, &m->tmX, xa_full, kb * kT_BK, m0);
         ++gt;
         auto load_w2 = [&](int c, uint32_t g) {       // chunk c's slice of W2: [N, 128] = up to two 64-wide k-blocks
           const int s = (int)(g & 1u);
           const int bn = min(kT_HC, H - c * kT_HC), nkb2 = (bn + kT_BK - 1) / kT_BK;
-          mbar_wait(w2_empty(s), ((g >> 1) & 1u) ^ 1u);
+          T2_WAIT(tr_w2e, mbar_wait(w2_empty(s), ((g >> 1) & 1u) ^ 1u));
           mbar_expect_tx(w2_full(s), (uint32_t)(nkb2 * N * kT_BK * 2));
           for (int j = 0; j < nkb2; ++j)
             tma_load_2d(sbase + kT_OffW2 + s * 2 * kT_W2KBlockBytes + j * kT_W2KBlockBytes, &m->tmW2, w2_full(s),
@@ -398,7 +458,7 @@ grouped_linear2_sm100_kernel(const L2Member* __restrict__ members, const uint4* 
         };
         for (int c = 0; c < nch; ++c) {
           for (int kb = 0; kb < nkb1; ++kb) {
-            mbar_wait(w1_empty(w1s), w1ph ^ 1);
+            T2_WAIT(tr_w1e, mbar_wait(w1_empty(w1s), w1ph ^ 1));
             mbar_expect_tx(w1_full(w1s), kT_KBlockBytes);
             tma_load_2d(sbase + kT_OffW1 + w1s * kT_KBlockBytes, &m->tmW1, w1_full(w1s), kb * kT_BK, c * kT_HC);
             if (++w1s == kT_W1Stages) { w1s = 0; w1ph ^= 1; }
@@ -414,6 +474,7 @@ grouped_linear2_sm100_kernel(const L2Member* __restrict__ members, const uint4* 
         load_w2(nch - 1, gh + nch - 1);
         gh += (uint32_t)nch;
       }
+      T2_STORE(0, clock64() - tr_t0); T2_STORE(1, tr_q); T2_STORE(2, tr_xe); T2_STORE(3, tr_w1e); T2_STORE(4, tr_w2e);
     }
   } else if (warp == 1) {
     // ------------------------------------------ MMA issuer, layer 1 ----
@@ -425,8 +486,10 @@ grouped_linear2_sm100_kernel(const L2Member* __restrict__ members, const uint4* 
       uint32_t gt = 0, g = 0;
       const uint64_t xd0 = umma_desc_sw128(sbase + kT_OffX), wd0 = umma_desc_sw128(sbase + kT_OffW1);
       constexpr uint64_t kKB = kT_KBlockBytes >> 4;            // descriptor address units (16 bytes) per k-block
+      T2_DECL(tr_t0); T2_DECL(tr_q); T2_DECL(tr_a1e); T2_DECL(tr_xf); T2_DECL(tr_w1f); T2_DECL(tr_tiles); T2_DECL(tr_tc);
+      T2_NOW(tr_t0);
       for (;;) {
-        mbar_wait(q_full(qs), qph);
+        T2_WAIT(tr_q, mbar_wait(q_full(qs), qph));
         const uint4 e0 = lds128(q_slot(qs) + kQEntryOff);
         mbar_arrive(q_empty(qs));
         if (++qs == kT_QDepth) { qs = 0; qph ^= 1; }
@@ -436,12 +499,13 @@ grouped_linear2_sm100_kernel(const L2Member* __restrict__ members, const uint4* 
         for (int c = 0; c < nch; ++c, ++g) {
           const uint32_t s = g & 1u;
           const uint32_t idesc1 = l2_idesc(min(kT_HC, H - c * kT_HC));
-          mbar_wait(a1_empty(s), ((g >> 1) & 1u) ^ 1u);      // epilogue has drained this acc1 stage
-          if (c == 0) mbar_wait(xa_full, gt & 1u);
+          T2_WAIT(tr_a1e, mbar_wait(a1_empty(s), ((g >> 1) & 1u) ^ 1u));      // epilogue has drained this acc1 stage
+          if (c == 0) T2_WAIT(tr_xf, mbar_wait(xa_full, gt & 1u));
+          T2_ADD(tr_tc, (min(kT_HC, H - c * kT_HC) / 2) * ((nkb1 - 1) * 4 + klast1) + (min(kT_HC, H - c * kT_HC) / 16) * ((int)(e0.w >> 16) / 2));
           tc_fence_after();
           const uint32_t acc1 = tmem_base + s * 128u;
           for (int kb = 0; kb < nkb1; ++kb) {
-            mbar_wait(w1_full(w1s), w1ph);
+            T2_WAIT(tr_w1f, mbar_wait(w1_full(w1s), w1ph));
             tc_fence_after();
             const uint64_t adesc = xd0 + (uint64_t)kb * kKB, bdesc = wd0 + (uint64_t)w1s * kKB;
             if (kb + 1 < nkb1) {                             // +32 bytes (= +2 encoded) per K=16 step
@@ -467,7 +531,10 @@ grouped_linear2_sm100_kernel(const L2Member* __restrict__ members, const uint4* 
           if (c == nch - 1) tc_commit(xa_empty);             // the X tile may be replaced
         }
         ++gt;
+        T2_ADD(tr_tiles, 1);
       }
+      T2_STORE(5, clock64() - tr_t0); T2_STORE(6, tr_q); T2_STORE(7, tr_a1e); T2_STORE(8, tr_xf); T2_STORE(9, tr_w1f);
+      T2_STORE(10, tr_tiles); T2_STORE(11, tr_tc);
     }
   } else if (warp == kT_Mma2Warp) {
     // ------------------------------------------ MMA issuer, layer 2 ----
@@ -475,36 +542,40 @@ grouped_linear2_sm100_kernel(const L2Member* __restrict__ members, const uint4* 
     if (lane == 0) {
       int qs = 0; uint32_t qph = 0;
       uint32_t gt = 0, g = 0;
-      const uint64_t hd0 = umma_desc_sw128(sbase + kT_OffH), w2d0 = umma_desc_sw128(sbase + kT_OffW2);
-      constexpr uint64_t kKB = kT_KBlockBytes >> 4, kW2KB = kT_W2KBlockBytes >> 4;
+      const uint64_t w2d0 = umma_desc_sw128(sbase + kT_OffW2);
+      constexpr uint64_t kW2KB = kT_W2KBlockBytes >> 4;
+      T2_DECL(tr_t0); T2_DECL(tr_q); T2_DECL(tr_a2e); T2_DECL(tr_w2f); T2_DECL(tr_hf);
+      T2_NOW(tr_t0);
       for (;;) {
-        mbar_wait(q_full(qs), qph);
+        T2_WAIT(tr_q, mbar_wait(q_full(qs), qph));
         const uint4 e0 = lds128(q_slot(qs) + kQEntryOff);
         mbar_arrive(q_empty(qs));
         if (++qs == kT_QDepth) { qs = 0; qph ^= 1; }
         if ((int)e0.x < 0) break;
         const int H = (int)(e0.z & 0xFFFFu), N = (int)(e0.w >> 16);
         const int nch = (H + kT_HC - 1) / kT_HC;
-        const uint32_t acc2 = tmem_base + 256u + (gt & 1u) * 64u;
+        const uint32_t acc2 = tmem_base + kT_TmemAcc2 + (gt & 1u) * 64u;
         const uint32_t idesc2 = l2_idesc(N);
-        mbar_wait(a2_empty(gt & 1u), ((gt >> 1) & 1u) ^ 1u);   // the epilogue has drained this acc2 stage
+        T2_WAIT(tr_a2e, mbar_wait(a2_empty(gt & 1u), ((gt >> 1) & 1u) ^ 1u));   // the epilogue has drained this acc2 stage
         for (int c = 0; c < nch; ++c, ++g) {
           const uint32_t s = g & 1u;
           const int ksteps = min(kT_HC, H - c * kT_HC) / 16;
-          mbar_wait(w2_full(s), (g >> 1) & 1u);
-          mbar_wait(h_full(0), g & 1u);
+          T2_WAIT(tr_w2f, mbar_wait(w2_full(s), (g >> 1) & 1u));
+          T2_WAIT(tr_hf, mbar_wait(h_full(s), (g >> 1) & 1u));
           tc_fence_after();
           const uint64_t wd = w2d0 + (uint64_t)s * 2 * kW2KB;
+          const uint32_t ht = tmem_base + kT_TmemH + s * 64u;                // A operand: 8 TMEM columns per K=16 step
           for (int k = 0; k < ksteps; ++k) {
-            const uint64_t j = (uint64_t)(k >> 2), kk = (uint64_t)(k & 3);   // k-block, K=16 step inside it
-            tc_mma_bf16(acc2, hd0 + j * kKB + 2 * kk, wd + j * kW2KB + 2 * kk, idesc2, (c | k) != 0);
+            const uint64_t j = (uint64_t)(k >> 2), kk = (uint64_t)(k & 3);   // k-block of W2, K=16 step inside it
+            tc_mma_bf16_ts(acc2, ht + 8u * (uint32_t)k, wd + j * kW2KB + 2 * kk, idesc2, (c | k) != 0);
           }
-          tc_commit(h_empty(0));
+          tc_commit(h_empty(s));
           tc_commit(w2_empty(s));
         }
         tc_commit(a2_full(gt & 1u));
         ++gt;
       }
+      T2_STORE(12, clock64() - tr_t0); T2_STORE(13, tr_q); T2_STORE(14, tr_a2e); T2_STORE(15, tr_w2f); T2_STORE(16, tr_hf);
     }
   } else {
     // ----------------------------------------------------------- epilogue ----
@@ -515,7 +586,6 @@ grouped_linear2_sm100_kernel(const L2Member* __restrict__ members, const uint4* 
     const int quad = warp & 3;               // TMEM lane quadrant this warp may read
     const int half = ew >> 2;                // which 64-column half of a 128-wide hidden chunk
     const uint32_t lane_off = (uint32_t)(quad * 32) << 16;
-    const uint32_t row_off = (uint32_t)(quad * 32 + lane) * 128u;      // this thread's row inside a k-block
     int qs = 0; uint32_t qph = 0;
     uint32_t gt = 0, gh = 0;
     // the tile whose layer-2 accumulator is still to be drained
@@ -524,13 +594,17 @@ grouped_linear2_sm100_kernel(const L2Member* __restrict__ members, const uint4* 
     int p_qs = 0, p_act2 = 0, p_m0 = 0;
     const L2Member* p_m = nullptr;
     const uint32_t sbuf = sbase + kT_OffOut + (uint32_t)quad * 4096u;  // output staging (warps with half == 0)
+    T2_DECL(tr_t0); T2_DECL(tr_q); T2_DECL(tr_a1f); T2_DECL(tr_he); T2_DECL(tr_a2f); T2_DECL(tr_st); T2_DECL(tr_drain); T2_DECL(tr_xf);
+    T2_DECL(tr_s_ld); T2_DECL(tr_s_math); T2_DECL(tr_s_sts); T2_DECL(tr_s_fence); T2_DECL(tr_chunks);
+    T2_NOW(tr_t0);
     auto drain = [&]() {
+      T2_DECL(tr_d0); T2_NOW(tr_d0);
       const uint32_t s2 = p_gt & 1u;
-      mbar_wait(a2_full(s2), (p_gt >> 1) & 1u);
+      T2_WAIT(tr_a2f, mbar_wait(a2_full(s2), (p_gt >> 1) & 1u));
       tc_fence_after();
       uint32_t v[64], p[32];
       {
-        const uint32_t t = tmem_base + lane_off + 256u + s2 * 64u;
+        const uint32_t t = tmem_base + lane_off + kT_TmemAcc2 + s2 * 64u;
         tc_ld_32x32(t, *reinterpret_cast<uint32_t(*)[32]>(&v[0]));
         tc_ld_32x32(t + 32, *reinterpret_cast<uint32_t(*)[32]>(&v[32]));
         tc_wait_ld();
@@ -538,9 +612,12 @@ grouped_linear2_sm100_kernel(const L2Member* __restrict__ members, const uint4* 
       tc_fence_before();
       __syncwarp();
       if (lane == 0) mbar_arrive(a2_empty(s2));
-      if (half == 0) epi_act(v, p_slot + kOffB2, p_act2, p);
       if (half == 0) {
-        if (lane == 0) tma_store_wait_read<0>();       // this warp's previous store has read the staging tile
+        if constexpr (LN) epi_act_b16(v, p_slot + kOffB2, p_act2, p);
+        else epi_act(v, p_slot + kOffB2, p_act2, p);
+      }
+      if (half == 0) {
+        T2_WAIT(tr_st, if (lane == 0) tma_store_wait_read<0>());       // this warp's previous store has read the staging tile
         __syncwarp();
 #pragma unroll
         for (int j = 0; j < 8; ++j)
@@ -554,9 +631,10 @@ grouped_linear2_sm100_kernel(const L2Member* __restrict__ members, const uint4* 
       }
       __syncwarp();                          // every lane has read the slot's b2
       if (lane == 0) mbar_arrive(q_empty(p_qs));
+      T2_ADD(tr_drain, clock64() - tr_d0);
     };
     for (;;) {
-      mbar_wait(q_full(qs), qph);
+      T2_WAIT(tr_q, mbar_wait(q_full(qs), qph));
       const uint32_t slot = q_slot(qs);
       const uint4 e0 = lds128(slot + kQEntryOff);
       if ((int)e0.x < 0) break;
@@ -574,7 +652,7 @@ grouped_linear2_sm100_kernel(const L2Member* __restrict__ members, const uint4* 
         const int K = __ldg(&folds[(int)e0.x].K);
         const float eps = __ldg(&folds[(int)e0.x].eps);
         const uint32_t ss = gt & 1u;
-        mbar_wait(xa_full, gt & 1u);
+        T2_WAIT(tr_xf, mbar_wait(xa_full, gt & 1u));
         const int r0 = quad * 32 + lane;
         const uint32_t a0 = sbase + kT_OffX + (uint32_t)r0 * 128u;
         const uint32_t x7 = (uint32_t)(lane & 7);                   // r0 & 7
@@ -627,32 +705,38 @@ grouped_linear2_sm100_kernel(const L2Member* __restrict__ members, const uint4* 
         const uint32_t ph = (g >> 1) & 1u;
         const int bn = min(kT_HC, H - c * kT_HC);
         const bool mine = half * 64 < bn;            // this warp's 64 columns exist in the chunk
-        mbar_wait(a1_full(s), ph);
+        T2_WAIT(tr_a1f, mbar_wait(a1_full(s), ph));
         tc_fence_after();
         const uint32_t t = tmem_base + lane_off + (uint32_t)s * 128u + (uint32_t)half * 64u;
         {                                              // (columns past the chunk's width hold stale data: never used)
           uint32_t v[64], p[32];
+          T2_DECL(tq0); T2_DECL(tq1); T2_DECL(tq2); T2_DECL(tq3); T2_DECL(tq4);
+          T2_NOW(tq0);
           tc_ld_32x32(t, *reinterpret_cast<uint32_t(*)[32]>(&v[0]));
           tc_ld_32x32(t + 32, *reinterpret_cast<uint32_t(*)[32]>(&v[32]));
           tc_wait_ld();
+          T2_NOW(tq1);
           tc_fence_before();
           __syncwarp();
           if (lane == 0) mbar_arrive(a1_empty(s));     // acc1 stage is in registers: MMA1 of chunk c+2 may overwrite it
           if constexpr (LN) epi_act_ln(v, lnA, act1, p);
-          else epi_act(v, slot + (uint32_t)(c * kT_HC + half * 64) * 2u, act1, p);
-          // the hidden tile is single-buffered: MMA2 of chunk c-1 has normally retired by the time this chunk's
-          // accumulator has been read and converted
-          mbar_wait(h_empty(0), (g & 1u) ^ 1u);
-          if (mine) {
-            const uint32_t hrow = sbase + kT_OffH + (uint32_t)half * kT_KBlockBytes + row_off;
-#pragma unroll
-            for (int j = 0; j < 8; ++j)                // K-major, 128-byte swizzle: 16-byte piece j of row r sits at j ^ (r & 7)
-              sts128(hrow + ((j ^ (lane & 7)) << 4), make_uint4(p[4 * j], p[4 * j + 1], p[4 * j + 2], p[4 * j + 3]));
-          }
+          else epi_act(v, slot + (uint32_t)(c * kT_HC + half * 64) * 4u, act1, p);
+          T2_NOW(tq2);
+          // the hidden tile lives in TENSOR MEMORY (two buffers of 64 columns: a column holds two consecutive hidden
+          // units of this thread's row): MMA2 of chunk c-2 has long retired
+          T2_WAIT(tr_he, mbar_wait(h_empty(s), ph ^ 1u));
+          T2_NOW(tq3);
+          tc_fence_after();
+          if (mine) tc_st_32x32(tmem_base + lane_off + kT_TmemH + (uint32_t)s * 64u + (uint32_t)half * 32u, p);
+          tc_wait_st();
+          T2_NOW(tq4);
+          T2_ADD(tr_s_ld, tq1 - tq0); T2_ADD(tr_s_math, tq2 - tq1); T2_ADD(tr_s_sts, tq4 - tq3);
         }
-        fence_proxy_async_smem();                      // generic-proxy writes -> visible to the tensor core's reads
+        T2_DECL(tq5); T2_NOW(tq5);
+        tc_fence_before();
         __syncwarp();
-        if (lane == 0) mbar_arrive(h_full(0));
+        if (lane == 0) mbar_arrive(h_full(s));
+        T2_ADD(tr_s_fence, clock64() - tq5); T2_ADD(tr_chunks, 1);
         if (c == 0 && pend) { drain(); pend = false; }
       }
       gh += (uint32_t)nch;
@@ -663,6 +747,11 @@ grouped_linear2_sm100_kernel(const L2Member* __restrict__ members, const uint4* 
     }
     if (pend) drain();
     if (lane == 0) tma_store_wait_all();
+    if (ew == 0 && lane == 0) {
+      T2_STORE(17, clock64() - tr_t0); T2_STORE(18, tr_q); T2_STORE(19, tr_a1f); T2_STORE(20, tr_he); T2_STORE(21, tr_a2f);
+      T2_STORE(22, tr_st); T2_STORE(23, tr_drain); T2_STORE(24, tr_xf);
+      T2_STORE(25, tr_s_ld); T2_STORE(26, tr_s_math); T2_STORE(27, tr_s_sts); T2_STORE(28, tr_s_fence); T2_STORE(29, tr_chunks);
+    }
   }
 
   tc_fence_before();
@@ -672,6 +761,14 @@ grouped_linear2_sm100_kernel(const L2Member* __restrict__ members, const uint4* 
     asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "n"(kT_TmemCols) : "memory");
   }
 }
+
+#ifdef OPTB_GEMM_TRACE
+// trace build only: where the chained kernel writes its per-CTA wait-cycle records ([grid][32] uint64), or NULL
+extern "C" int opt_trace_set_linear2_buffer(void* device_buffer) {
+  unsigned long long* p = static_cast<unsigned long long*>(device_buffer);
+  return (int)cudaMemcpyToSymbol(optb::g_l2_trace, &p, sizeof p);
+}
+#endif
 
 cudaError_t launch_linear2(const opt_plan* p, cudaStream_t s) {
   char* base = static_cast<char*>(p->dev_tables);
