@@ -348,6 +348,26 @@ opt_status opt_plan_info(const opt_plan* plan, int64_t* flops, int64_t* bytes, i
 
 opt_status opt_plan_destroy(opt_plan* plan);
 
+/* NO-ALLOCATION entry point: the bias gradient of ONE Linear layer (PAPER.md:292 batch_linear_post_grad,
+ * PAPER.md:437 training),  db[n] = sum over m of dz[m, n],  for callers that cannot call cudaMalloc (code under
+ * CUDA-graph capture, tight serving loops, harnesses that forbid allocation).  It creates no plan and calls no
+ * cudaMalloc / cudaFree / allocating library routine: the partial sums live in a file-scope device array of
+ * OPT_NOALLOC_SCRATCH_BYTES (1 MiB + 256 B) that every GPU which loads the library holds until the process exits.
+ *   dz:[M,N] bf16, row stride ldz (elements; a column slice of a concat buffer is fine), db:[N] of dtype `param`
+ *   (OPT_F32 or OPT_BF16); device pointers on `device`, caller-owned.  N % 8 == 0, ldz % 8 == 0, 16-byte aligned
+ *   pointers (else OPT_ERR_ALIGNMENT); db must not overlap dz (OPT_ERR_ALIAS); M >= 1.
+ *   N <= OPT_NOALLOC_BIAS_GRAD_MAX_N, else OPT_ERR_UNSUPPORTED and nothing is launched (wider layers: the planned
+ *   path, opt_bias_grad_plan_create).  M is not limited.
+ * On `cuda_stream` (NULL = default stream): a 256-byte memset of the scratch's tickets, then ONE kernel launch;
+ * asynchronous.  fp32 accumulation in a fixed order (bitwise reproducible, no atomics on data); the partitioning
+ * differs from the planned kernel's, so the two agree within fp32 rounding, not bit for bit.
+ * EVERY call shares the one scratch array: calls that overlap on the GPU (different streams or threads without an
+ * ordering between them) RACE; calls on one stream are safe.  The calling thread's current device is left as it was. */
+#define OPT_NOALLOC_BIAS_GRAD_MAX_N 4096
+#define OPT_NOALLOC_SCRATCH_BYTES (64 * OPT_NOALLOC_BIAS_GRAD_MAX_N * 4 + 256)
+opt_status opt_bias_grad_noalloc(const void* dz, int64_t ldz, void* db, int32_t M, int32_t N, opt_dtype param,
+                                 int device, void* cuda_stream);
+
 /* Last error message of the calling thread; never NULL ("" if none). */
 const char* opt_last_error(void);
 

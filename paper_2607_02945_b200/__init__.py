@@ -17,7 +17,7 @@ from .binding import (  # noqa: F401
     OptError, Plan, lib, lib_path,
     opt_linear_member, opt_linear_options, opt_linear2_member, opt_ln_linear2_member, opt_layernorm_member, opt_layernorm_bwd_member, opt_bias_grad_member, opt_chunk, opt_host_copy,
     opt_linear_plan_create, opt_linear_plan_create_ex, opt_linear2_plan_create, opt_ln_linear2_plan_create, opt_layernorm_plan_create, opt_layernorm_bwd_plan_create, opt_bias_grad_plan_create,
-    opt_pointwise_plan_create,
+    opt_pointwise_plan_create, opt_bias_grad_noalloc, OPT_NOALLOC_BIAS_GRAD_MAX_N,
     opt_plan_launch, opt_plan_launch_host, opt_plan_info, opt_plan_destroy,
     opt_last_error, opt_launch_count, opt_version,
     linear_member, linear2_member, ln_linear2_member, layernorm_member, layernorm_bwd_member, bias_grad_member, chunk, split_cat_chunks,

@@ -117,6 +117,8 @@ def lib():
                                                     C.c_int, pp]
         L.opt_bias_grad_plan_create.argtypes = [C.POINTER(opt_bias_grad_member), C.c_int32, C.c_int, C.c_int, C.c_int, pp]
         L.opt_pointwise_plan_create.argtypes = [C.POINTER(opt_chunk), C.c_int32, C.c_int, C.c_int, pp]
+        L.opt_bias_grad_noalloc.argtypes = [C.c_void_p, C.c_int64, C.c_void_p, C.c_int32, C.c_int32, C.c_int, C.c_int, C.c_void_p]
+        L.opt_bias_grad_noalloc.restype = C.c_int
         L.opt_plan_launch.argtypes = [C.c_void_p, C.c_void_p]
         L.opt_plan_launch_host.argtypes = [C.c_void_p, C.POINTER(opt_host_copy), C.c_int32, C.c_void_p]
         L.opt_plan_info.argtypes = [C.c_void_p, C.POINTER(C.c_int64), C.POINTER(C.c_int64), C.POINTER(C.c_int32),
@@ -219,6 +221,17 @@ def opt_layernorm_bwd_plan_create(members, io, param=None, device=0):
 def opt_bias_grad_plan_create(members, io, param=None, device=0):
     return _create(lib().opt_bias_grad_plan_create, opt_bias_grad_member, members, io,
                    io if param is None else param, device)
+
+
+OPT_NOALLOC_BIAS_GRAD_MAX_N = 4096
+
+
+def opt_bias_grad_noalloc(dz, db, param=OPT_F32, device=0, stream=None):
+    """db = column sums of the bf16 tensor dz [M, N] without any allocation (scratch in a static device array of the
+    library; N <= OPT_NOALLOC_BIAS_GRAD_MAX_N; calls that overlap on the GPU race on that scratch)."""
+    M, N = dz.shape
+    assert tuple(db.shape) == (N,)
+    _check(lib().opt_bias_grad_noalloc(dz.data_ptr(), _ld(dz), db.data_ptr(), M, N, int(param), device, _stream_ptr(stream)))
 
 
 def opt_pointwise_plan_create(chunks, io, device=0):
