@@ -606,6 +606,7 @@ def run_side(args):
       --side fp8_fused configs[4]'s LayerNorm and Linear+ReLU groups writing bf16 AND the FP8 copy in one launch vs two launches
       --side backward  configs[2] dgrad / wgrad / fused mask + bias gradient, configs[4] LayerNorm backward, one launch each
       --side gemm_trace  wait-cycle counters of the grouped GEMM's warp roles (trace build of the library)
+      --side linear2_trace  the same for the chained kernel (opt_linear2 / opt_ln_linear2 on configs[4]'s towers)
       --side lhs       batch_linear_lhs: 8 members (N=64) on ONE input X [262144, 512]; also timed with
                        opt_linear_options.no_lhs_order (plain member-major schedule)
     Prints one JSON line; not the bench metric."""
@@ -800,6 +801,61 @@ def run_side(args):
                               note="percentages of the role's own loop time, [min, median, max] over the CTA pairs; tensor cycles = "
                                    "sum over tiles of k-blocks x (BN / 256) x 512 (a 256 x 256 x 64 k-block keeps the pair's tensor "
                                    "pipes busy for 512 cycles)")))
+    elif args.side == "linear2_trace":
+        # where the chained kernel's warp roles wait (trace build of the library, like gemm_trace): one record of 32
+        # counters per CTA, for opt_linear2 and opt_ln_linear2 on configs[4]'s towers
+        from paper_2607_02945_b200 import binding
+        binding.use_trace_library()
+        step = Step("cuda:0", FULL, pinned_host=False, configs=("c4",))
+        ga, gb, gc = step.groups
+        T, A = ga.ain.tensor, ga.amid.tensor
+        out2 = torch.empty_like(gc.aout.tensor(ga.iy))
+        ga.plan.launch()
+        torch.cuda.synchronize()
+        grid = 148
+        buf = torch.zeros(grid * 32, dtype=torch.int64, device="cuda")
+        assert binding.lib().opt_trace_set_linear2_buffer(C_void_p(buf.data_ptr())) == 0
+        flush = torch.empty(256 * 1024 * 1024, dtype=torch.uint8, device="cuda")
+        roles = {"producer": (0, dict(queue=1, x_empty=2, w1_empty=3, w2_empty=4)),
+                 "mma1": (5, dict(queue=6, acc1_empty=7, x_full=8, w1_full=9)),
+                 "mma2": (12, dict(queue=13, acc2_empty=14, w2_full=15, h_full=16)),
+                 "epilogue": (17, dict(queue=18, acc1_full=19, h_empty=20, acc2_full=21, store=22, drain_total=23, x_full=24,
+                                       seg_tmem_load=25, seg_math=26, seg_hidden_store=27, seg_publish=28))}
+
+        def trace(plan):
+            for _ in range(3):
+                plan.launch()
+            torch.cuda.synchronize()
+            us = timed(plan.launch, 5)
+            buf.zero_()
+            flush.fill_(1)
+            plan.launch()
+            torch.cuda.synchronize()
+            r = buf.cpu().numpy().reshape(grid, 32).astype(np.float64)
+            pct = lambda a, tot: [round(float(v), 1) for v in np.percentile(100.0 * a / np.maximum(tot, 1), [0, 50, 100])]
+            out = dict(us=round(us, 1))
+            for role, (tot, d) in roles.items():
+                out[role] = dict(total_cycles_min_med_max=[int(v) for v in np.percentile(r[:, tot], [0, 50, 100])],
+                                 **{k + "_pct": pct(r[:, i], r[:, tot]) for k, i in d.items()})
+            out["tiles_per_cta_min_med_max"] = [int(v) for v in np.percentile(r[:, 10], [0, 50, 100])]
+            out["hidden_chunks_per_cta_min_med_max"] = [int(v) for v in np.percentile(r[:, 29], [0, 50, 100])]
+            out["epilogue_cycles_per_chunk"] = {k: round(float(np.median(r[:, i] / np.maximum(r[:, 29], 1))), 1)
+                                                for k, i in dict(tmem_load=25, math=26, hidden_store=27, publish=28).items()}
+            out["tensor_busy_pct"] = pct(r[:, 11], r[:, 5])
+            return out
+
+        towers = list(enumerate(zip(ga.idx, ga.cfg["towers"])))
+        p2 = ob.opt_linear2_plan_create([ob.linear2_member(A(i["xn"]), T(i["w1"]), T(i["b1"]), T(i["w2"]), T(i["b2"]),
+                                                           out2[:, k * t["out"]:(k + 1) * t["out"]], ACT_RELU, ACT_NONE) for k, (i, t) in towers], BF16, 0)
+        res = dict(side="linear2_trace", linear2=trace(p2))
+        del p2
+        pl = ob.opt_ln_linear2_plan_create([ob.ln_linear2_member(T(i["x"]), T(i["gamma"]), T(i["beta"]), t["eps"], T(i["w1"]), T(i["b1"]), T(i["w2"]),
+                                                                 T(i["b2"]), out2[:, k * t["out"]:(k + 1) * t["out"]], ACT_RELU, ACT_NONE)
+                                            for k, (i, t) in towers], BF16, 0)
+        res["ln_linear2"] = trace(pl)
+        res["note"] = ("percentages of the role's own loop time, [min, median, max] over the 148 CTAs; tensor cycles = per hidden chunk "
+                       "(chunk width / 2) x K=16 steps of layer 1 + (chunk width / 16) x (N / 2) of layer 2")
+        print(json.dumps(res))
     elif args.side == "fp8":
         step = Step("cuda:0", FULL, pinned_host=False, configs=("c4",))
         ga = step.groups[0]
@@ -1355,7 +1411,7 @@ def main():
     ap.add_argument("--profile", action="store_true",
                     help="only the step's own launches (no cpu_baseline, no unfused baseline, no copy reference): for ncu")
     ap.add_argument("--ref-frac", type=float, default=0.0, help="reference arm: override the row-sample fraction")
-    ap.add_argument("--side", default=None, choices=["linear2", "ln_linear2", "lhs", "skinny", "fp8", "fp8_fused", "bias_grad", "backward", "gemm_trace"], help="stand-alone side workload for ncu (not the metric)")
+    ap.add_argument("--side", default=None, choices=["linear2", "ln_linear2", "lhs", "skinny", "fp8", "fp8_fused", "bias_grad", "backward", "gemm_trace", "linear2_trace"], help="stand-alone side workload for ncu (not the metric)")
     ap.add_argument("--ncu-summary", default=None, metavar="REP", help="CPU box: print the csv summary of an ncu --set full capture of `bench.py --profile`")
     args = ap.parse_args()
     if args.ncu_summary:
