@@ -457,6 +457,7 @@ grouped_linear2_sm100_kernel(const L2Member* __restrict__ members, const uint4* 
                         c * kT_HC + j * kT_BK, 0);
         };
         for (int c = 0; c < nch; ++c) {
+          if (c >= 1) load_w2(c - 1, gh + c - 1);        // before W1 of chunk c: this thread may block on the W1 ring, and MMA2 of chunk c - 1 must not wait for its (small) W2 slice behind that
           for (int kb = 0; kb < nkb1; ++kb) {
             T2_WAIT(tr_w1e, mbar_wait(w1_empty(w1s), w1ph ^ 1));
             mbar_expect_tx(w1_full(w1s), kT_KBlockBytes);
@@ -469,7 +470,6 @@ grouped_linear2_sm100_kernel(const L2Member* __restrict__ members, const uint4* 
             tma_load_2d(sbase + kT_OffW1 + w1s * kT_KBlockBytes, &m->tmAug, w1_full(w1s), 0, c * kT_HC);
             if (++w1s == kT_W1Stages) { w1s = 0; w1ph ^= 1; }
           }
-          if (c >= 1) load_w2(c - 1, gh + c - 1);
         }
         load_w2(nch - 1, gh + nch - 1);
         gh += (uint32_t)nch;
@@ -560,8 +560,8 @@ grouped_linear2_sm100_kernel(const L2Member* __restrict__ members, const uint4* 
         for (int c = 0; c < nch; ++c, ++g) {
           const uint32_t s = g & 1u;
           const int ksteps = min(kT_HC, H - c * kT_HC) / 16;
-          T2_WAIT(tr_w2f, mbar_wait(w2_full(s), (g >> 1) & 1u));
           T2_WAIT(tr_hf, mbar_wait(h_full(s), (g >> 1) & 1u));
+          T2_WAIT(tr_w2f, mbar_wait(w2_full(s), (g >> 1) & 1u));
           tc_fence_after();
           const uint64_t wd = w2d0 + (uint64_t)s * 2 * kW2KB;
           const uint32_t ht = tmem_base + kT_TmemH + s * 64u;                // A operand: 8 TMEM columns per K=16 step
@@ -649,8 +649,9 @@ grouped_linear2_sm100_kernel(const L2Member* __restrict__ members, const uint4* 
         // TMEM quadrant) take alternate 16-byte pieces, shifted single pass (shift = the row's first element),
         // partial sums exchanged through shared memory; the half-0 thread writes the row's augmented A slice
         // (-mu_h, -mu_h, -mu_l, sigma_h, sigma_h, sigma_l, 0...).
-        const int K = __ldg(&folds[(int)e0.x].K);
-        const float eps = __ldg(&folds[(int)e0.x].eps);
+        const uint4 e1 = lds128(slot + kQEntryOff + 16);           // LN: the b1 field holds K | eps << 32 (no global load on the per-tile chain)
+        const int K = (int)e1.x;
+        const float eps = __uint_as_float(e1.y);
         const uint32_t ss = gt & 1u;
         T2_WAIT(tr_xf, mbar_wait(xa_full, gt & 1u));
         const int r0 = quad * 32 + lane;
@@ -893,7 +894,14 @@ opt_status create_linear2(const opt_linear2_member* members, const opt_ln_linear
       e.member = i; e.m0 = mb * kT_BM;
       e.shape = (uint32_t)m.H | ((uint32_t)nkb1 << 16) | ((uint32_t)klast1 << 24);
       e.misc = (uint32_t)m.act1 | ((uint32_t)m.act2 << 8) | ((uint32_t)m.N << 16);
-      e.b1 = LN ? nullptr : m.b1; e.b2 = m.b2;
+      e.b2 = m.b2;
+      if (LN) {      // no b1 operand (folded into c): the slot carries K and eps for the row statistics
+        uint32_t eps_bits;
+        memcpy(&eps_bits, &folds[i].eps, 4);
+        e.b1 = reinterpret_cast<const void*>((uintptr_t)((uint64_t)(uint32_t)m.K | ((uint64_t)eps_bits << 32)));
+      } else {
+        e.b1 = m.b1;
+      }
       flat.push_back(e);
     }
   }
