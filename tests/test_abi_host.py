@@ -183,3 +183,22 @@ def test_product_never_imports_the_oracle():
             txt = open(os.path.join(ROOT, "oracle", f)).read()
             assert "import paper_2607_02945_b200" not in txt and "from paper_2607_02945_b200" not in txt, f
             assert "csrc" not in txt and "optimus_b200.h" not in txt, f
+
+
+def test_no_alloc_entry_point_validates_on_the_host(ob):
+    """opt_bias_grad_noalloc: the limit of its static scratch and the argument rules are reported before any CUDA call."""
+    L = ob.lib()
+    dz, db = ctypes.c_void_p(0x10000000), ctypes.c_void_p(0x20000000)          # never dereferenced: validation only
+    call = lambda dz_, ldz, db_, M, N, param=ob.OPT_F32: L.opt_bias_grad_noalloc(dz_, ldz, db_, M, N, param, 0, None)
+    n0 = ob.opt_launch_count()
+    assert call(dz, 8192, db, 64, ob.OPT_NOALLOC_BIAS_GRAD_MAX_N + 8) == ob.OPT_ERR_UNSUPPORTED
+    assert "OPT_NOALLOC_BIAS_GRAD_MAX_N" in ob.opt_last_error()
+    assert call(None, 64, db, 64, 64) == ob.OPT_ERR_INVALID_ARG
+    assert call(dz, 64, db, 0, 64) == ob.OPT_ERR_INVALID_ARG
+    assert call(dz, 32, db, 64, 64) == ob.OPT_ERR_INVALID_ARG                   # ldz < N
+    assert call(dz, 64, db, 64, 64, 7) == ob.OPT_ERR_INVALID_ARG                # bad dtype
+    assert call(dz, 64, db, 64, 60) == ob.OPT_ERR_ALIGNMENT                     # N % 8
+    assert call(dz, 68, db, 64, 64) == ob.OPT_ERR_ALIGNMENT                     # ldz % 8
+    assert call(ctypes.c_void_p(0x10000008), 64, db, 64, 64) == ob.OPT_ERR_ALIGNMENT
+    assert call(dz, 64, ctypes.c_void_p(0x10000000 + 64 * 8), 64, 64) == ob.OPT_ERR_ALIAS   # db inside dz
+    assert ob.opt_launch_count() == n0
