@@ -31,6 +31,7 @@ struct LnbBlock { int32_t member, row0, nrows, part; };
 
 constexpr int kLnbThreads = 256;
 constexpr int kLnbSlotKB = 32;       // thread-private cp.async prefetch slots per block (alias the reduction buffer)
+constexpr int kLnbTargetBlocks = 16 * 148;   // blocks a large group should still have (see the planner)
 constexpr int kLnbMaxVpl = 2;        // D <= 512: x, dy and the two column accumulators stay in registers
 
 __device__ __forceinline__ void lnb_unpack(const int4& v, float (&f)[8]) {
@@ -389,6 +390,15 @@ extern "C" opt_status opt_layernorm_bwd_plan_create(const opt_layernorm_bwd_memb
   std::vector<int64_t> ws_off;            // float offset of each member's partials in the workspace
   int64_t bytes = 0, ws_floats = 0;
   int max_wide_D = 0;
+  // Rows per block of the register path: a block pays a prologue (kPD passes to fill its prefetch slots) and an
+  // epilogue (column sums through shared memory, a workspace part, the ticket), so long blocks are cheaper per row --
+  // configs[4]'s LayerNorm shapes: 64 KB of x per block 504 us, 128 KB 476 us, 256 KB 473 us -- as long as the group
+  // still fills the machine: aim at >= kLnbTargetBlocks blocks (16 per SM of the 148-SM part: four waves of four
+  // blocks per SM), between 64 KB and 256 KB of x per block.
+  int64_t group_x_bytes = 0;
+  for (int32_t i = 0; i < n; ++i)
+    if (members[i].rows > 0 && members[i].D > 0) group_x_bytes += (int64_t)members[i].rows * members[i].D * 2;
+  const int64_t block_x_bytes = std::min<int64_t>(262144, std::max<int64_t>(65536, group_x_bytes / kLnbTargetBlocks));
   for (int32_t i = 0; i < n; ++i) {
     const opt_layernorm_bwd_member& m = members[i];
     if (!m.x || !m.dy || !m.dx) return fail(OPT_ERR_INVALID_ARG, "member %d: NULL pointer", i);
@@ -415,9 +425,9 @@ extern "C" opt_status opt_layernorm_bwd_plan_create(const opt_layernorm_bwd_memb
     while (ll < 5 && (nvec + (1 << ll) - 1) / (1 << ll) > kLnbMaxVpl) ++ll;
     const int L = 1 << ll, vpl = (nvec + L - 1) / L, rpp = kLnbThreads >> ll;
     if (wide) max_wide_D = std::max(max_wide_D, m.D);
-    // rows per block: whole passes, ~64 KB of x per block (wide rows: ~512 KB, the block's shared-memory strips are
-    // zeroed and reduced once per block)
-    const int64_t passes = std::max<int64_t>(1, (wide ? 524288 : 65536) / ((int64_t)rpp * m.D * 2));
+    // rows per block: whole passes, block_x_bytes of x per block (wide rows: ~512 KB, the block's shared-memory strips
+    // are zeroed and reduced once per block)
+    const int64_t passes = std::max<int64_t>(1, (wide ? 524288 : block_x_bytes) / ((int64_t)rpp * m.D * 2));
     const int64_t rpb = rpp * passes;
     const int32_t nparts = (int32_t)((m.rows + rpb - 1) / rpb);
     LnbMember t;
