@@ -385,12 +385,19 @@ extern "C" opt_status opt_linear_plan_create_ex(const opt_linear_member* members
   }
   tiles = (int64_t)flat.size();
   if (tiles > INT32_MAX / 2) { delete p; return fail(OPT_ERR_UNSUPPORTED, "too many tiles"); }
-  // Chunks of 4 tiles (four 128-byte lines, one atomic); the last ~3 waves go one tile per chunk so that the
-  // tail of the persistent loop is balanced at tile granularity.
+  // Chunks of 4 tiles (four 128-byte lines, one atomic); the last waves go one tile per chunk so that the tail of the
+  // persistent loop is balanced at tile granularity.  How many: a 4-tile chunk of long tiles taken just before the tail
+  // keeps its CTA busy for several tile times, and the tail has to hold that much work per CTA to level it -- with
+  // configs[2]'s tiles (8.8 k-blocks on average, up to 16) 3 waves left the CTA pairs finishing 10 % apart (trace:
+  // 365 k .. 406 k cycles) and 16 waves are 4 % faster (263 -> 252 us; 24: the same, 40: slower again); short tiles
+  // (configs[4]'s groups: 2 - 5 k-blocks, HBM-bound) do not need it and would outrun a scheduler that serves one tile
+  // per atomic (C4b: 594 us with 3 - 6 waves, 601 with 16).  Hence twice the average k-block count, in [3, 16].
   TileEntry pad_entry;
   memset(&pad_entry, 0, sizeof pad_entry);
   pad_entry.member = -1;
-  const size_t tail_waves = 3;
+  uint64_t sum_nkb = 0;
+  for (const TileEntry& e : flat) sum_nkb += e.bn_nkb >> 16;
+  const size_t tail_waves = std::min<size_t>(16, std::max<size_t>(3, (size_t)((2 * sum_nkb + flat.size() / 2) / std::max<size_t>(1, flat.size()))));
   const int n_sched = num_sms / ncta;                         // persistent CTAs (or CTA pairs)
   const size_t tail = std::min(flat.size(), tail_waves * n_sched);
   const size_t body = flat.size() - tail;
