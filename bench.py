@@ -791,13 +791,19 @@ def run_side(args):
             depth[str(ns)] = round(timed(pd.launch, 5), 1)
         c2["us_by_ring_stages"] = depth
         del step, g
+        step4 = Step("cuda:0", FULL, pinned_host=False, configs=("c4",))       # the two HBM-bound GEMM groups of configs[4]
+        for g4 in step4.groups:
+            g4.plan.launch()
+        torch.cuda.synchronize()
+        c4 = {g4.name: trace(g4.plan) for g4 in step4.groups if g4.kind == "linear"}
+        del step4
         M, K, N, n = 262144, 512, 64, 8
         gen = torch.Generator(device="cuda").manual_seed(0)
         x = torch.randn(M, K, device="cuda", generator=gen).to(torch.bfloat16)
         ws = [(torch.randn(N, K, device="cuda", generator=gen) * K ** -0.5).to(torch.bfloat16) for _ in range(n)]
         ycat = torch.empty(M, N * n, device="cuda", dtype=torch.bfloat16)
         lhs = trace(ob.opt_linear_plan_create([ob.linear_member(x, w, None, ycat[:, i * N:(i + 1) * N], ACT_RELU) for i, w in enumerate(ws)], BF16, 0))
-        print(json.dumps(dict(side="gemm_trace", configs2=c2, batch_linear_lhs_8xN64=lhs,
+        print(json.dumps(dict(side="gemm_trace", configs2=c2, configs4=c4, batch_linear_lhs_8xN64=lhs,
                               note="percentages of the role's own loop time, [min, median, max] over the CTA pairs; tensor cycles = "
                                    "sum over tiles of k-blocks x (BN / 256) x 512 (a 256 x 256 x 64 k-block keeps the pair's tensor "
                                    "pipes busy for 512 cycles)")))
