@@ -448,7 +448,11 @@ class ClockWatch(threading.Thread):
                 mhz = nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM)
                 reasons = nv.nvmlDeviceGetCurrentClocksEventReasons(self.h)
                 util = nv.nvmlDeviceGetUtilizationRates(self.h).gpu
-                self.samples.append((mhz, reasons, util))
+                try:
+                    mw = nv.nvmlDeviceGetPowerUsage(self.h)
+                except Exception:  # noqa: BLE001
+                    mw = None
+                self.samples.append((mhz, reasons, util, mw))
             except Exception:  # noqa: BLE001
                 pass
             time.sleep(0.01)
@@ -466,8 +470,12 @@ class ClockWatch(threading.Thread):
                  ("sw_thermal_slowdown", nv.nvmlClocksEventReasonSwThermalSlowdown),
                  ("sw_power_cap", nv.nvmlClocksEventReasonSwPowerCap),
                  ("hw_power_brake", nv.nvmlClocksEventReasonHwPowerBrakeSlowdown)]
-        return dict(sm_mhz=mhz[len(mhz) // 2], sm_max_mhz=self.max_mhz, samples=len(mhz),
-                    reasons=[n for n, b in names if bits & b])
+        out = dict(sm_mhz=mhz[len(mhz) // 2], sm_max_mhz=self.max_mhz, samples=len(mhz),
+                   reasons=[n for n, b in names if bits & b])
+        watts = sorted(s[3] / 1000.0 for s in self.samples if s[3] is not None)
+        if watts:
+            out["power_w"] = round(watts[len(watts) // 2], 0)
+        return out
 
 
 # ------------------------------------------------------------- CPU oracle ----
@@ -607,6 +615,7 @@ def run_side(args):
       --side backward  configs[2] dgrad / wgrad / fused mask + bias gradient, configs[4] LayerNorm backward, one launch each
       --side gemm_trace  wait-cycle counters of the grouped GEMM's warp roles (trace build of the library)
       --side linear2_trace  the same for the chained kernel (opt_linear2 / opt_ln_linear2 on configs[4]'s towers)
+      --side power       every group launched back to back for 1.5 s: time, board power, SM clock (what the power cap does)
       --side lhs       batch_linear_lhs: 8 members (N=64) on ONE input X [262144, 512]; also timed with
                        opt_linear_options.no_lhs_order (plain member-major schedule)
     Prints one JSON line; not the bench metric."""
@@ -861,6 +870,51 @@ def run_side(args):
         res["ln_linear2"] = trace(pl)
         res["note"] = ("percentages of the role's own loop time, [min, median, max] over the 148 CTAs; tensor cycles = per hidden chunk "
                        "(chunk width / 2) x K=16 steps of layer 1 + (chunk width / 16) x (N / 2) of layer 2")
+        print(json.dumps(res))
+    elif args.side == "power":
+        # What the power cap does to each group: a group launched back to back for 1.5 s (no L2 flush, no gaps), with SM
+        # clock and board power sampled through NVML; next to a device copy and a cuBLAS GEMM as references.  The step's
+        # 50-step timed region (about 90 ms) sits between the burst figures (isolated, cold L2) and these sustained ones.
+        step = Step("cuda:0", FULL, pinned_host=False)
+
+        def sustained(fn, seconds=1.5, batch=50):
+            for _ in range(20):
+                fn()
+            torch.cuda.synchronize()
+            w = ClockWatch(0)
+            w.start()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            t0, n = time.time(), 0
+            e0.record()
+            while time.time() - t0 < seconds:
+                for _ in range(batch):
+                    fn()
+                n += batch
+                torch.cuda.synchronize()
+            e1.record()
+            torch.cuda.synchronize()
+            w.stop_flag.set()
+            w.join(timeout=2)
+            c = w.summary()
+            us = e0.elapsed_time(e1) * 1e3 / n
+            return dict(us=round(us, 1), power_w=c.get("power_w"), sm_mhz=c.get("sm_mhz"), sm_max_mhz=c.get("sm_max_mhz"),
+                        joule_per_launch=None if c.get("power_w") is None else round(c["power_w"] * us * 1e-6, 3))
+
+        res = dict(side="power")
+        for g in step.groups:
+            res[g.name] = dict(sustained(g.plan.launch), algorithmic_bytes=g.info["bytes"])
+
+        def whole():
+            for g in step.groups:
+                g.plan.launch()
+        res["step"] = sustained(whole, 3.0, 10)
+        del step
+        a = torch.empty(1500 * 1024 * 1024, dtype=torch.uint8, device="cuda")
+        b = torch.empty_like(a)
+        res["device_copy_3.1GB"] = dict(sustained(lambda: b.copy_(a)), algorithmic_bytes=2 * a.numel())
+        del a, b
+        x = torch.randn(8192, 8192, device="cuda", dtype=torch.bfloat16)
+        res["cublas_bf16_8192^3"] = dict(sustained(lambda: torch.matmul(x, x)), flops=2 * 8192 ** 3)
         print(json.dumps(res))
     elif args.side == "fp8":
         step = Step("cuda:0", FULL, pinned_host=False, configs=("c4",))
@@ -1417,7 +1471,7 @@ def main():
     ap.add_argument("--profile", action="store_true",
                     help="only the step's own launches (no cpu_baseline, no unfused baseline, no copy reference): for ncu")
     ap.add_argument("--ref-frac", type=float, default=0.0, help="reference arm: override the row-sample fraction")
-    ap.add_argument("--side", default=None, choices=["linear2", "ln_linear2", "lhs", "skinny", "fp8", "fp8_fused", "bias_grad", "backward", "gemm_trace", "linear2_trace"], help="stand-alone side workload for ncu (not the metric)")
+    ap.add_argument("--side", default=None, choices=["linear2", "ln_linear2", "lhs", "skinny", "fp8", "fp8_fused", "bias_grad", "backward", "gemm_trace", "linear2_trace", "power"], help="stand-alone side workload for ncu (not the metric)")
     ap.add_argument("--ncu-summary", default=None, metavar="REP", help="CPU box: print the csv summary of an ncu --set full capture of `bench.py --profile`")
     args = ap.parse_args()
     if args.ncu_summary:
